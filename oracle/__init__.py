@@ -1,0 +1,235 @@
+"""ctypes front end of the CPU fp64 oracle (oracle/fitrig_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this package.  It does not
+import, link or read anything of the CUDA path (paper_2509_21754_b200).
+
+All arithmetic lives in the C file; this module only marshals numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "fitrig_oracle.c")
+_LIB = os.path.join(_HERE, "libfitrig_oracle.so")
+
+REF_ABS, REF_LITERAL, REF_FLOOR = 0, 1, 2
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 (no fast-math) -fopenmp; rebuilt when the source is newer than the library."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.run(["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"],
+                       check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        c_f32pp = ctypes.POINTER(ctypes.c_void_p)
+        dp, ip64, ip32 = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p
+        L.fitrig_oracle_num_threads.restype = ctypes.c_int
+        L.fitrig_oracle_set_threads.argtypes = [ctypes.c_int]
+        L.fitrig_oracle_global_max.restype = ctypes.c_double
+        L.fitrig_oracle_global_max.argtypes = [c_f32pp, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, ctypes.c_double]
+        L.fitrig_oracle_tlisi.restype = ctypes.c_int
+        L.fitrig_oracle_tlisi.argtypes = [c_f32pp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                          ctypes.c_double, ctypes.c_int, ctypes.c_double,
+                                          dp, dp, dp, ip64, dp, dp]
+        L.fitrig_oracle_zscore.restype = None
+        L.fitrig_oracle_zscore.argtypes = [dp, ctypes.c_int, ctypes.c_int64, dp, dp, dp]
+        L.fitrig_oracle_select.restype = ctypes.c_int64
+        L.fitrig_oracle_select.argtypes = [dp, ip64, ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_double,
+                                           ip32, ip32, ip32, ip64, dp, ctypes.c_int64]
+        L.fitrig_oracle_spectrum.restype = None
+        L.fitrig_oracle_spectrum.argtypes = [dp, ctypes.c_int, ctypes.c_int64, dp, ip32]
+        L.fitrig_oracle_select_spectrum.restype = ctypes.c_int64
+        L.fitrig_oracle_select_spectrum.argtypes = [dp, ip32, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                    ctypes.c_int, ctypes.c_double, ip32, ip32, ip32, ip64, dp,
+                                                    ctypes.c_int64]
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().fitrig_oracle_num_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().fitrig_oracle_set_threads(int(n))
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _snap_ptrs(snaps: Sequence[np.ndarray], H: int, W: int):
+    keep = []
+    arr = (ctypes.c_void_p * len(snaps))()
+    for i, s in enumerate(snaps):
+        s = np.ascontiguousarray(s, dtype=np.float32)
+        assert s.shape == (H, W), (s.shape, H, W)
+        keep.append(s)
+        arr[i] = s.ctypes.data
+    return arr, keep
+
+
+def as_snapshots(stack) -> List[np.ndarray]:
+    """[L,H,W] array (numpy or CPU torch) or a list of [H,W] arrays -> list of fp32 numpy views."""
+    if hasattr(stack, "detach"):
+        stack = stack.detach().cpu().numpy()
+    if isinstance(stack, np.ndarray):
+        assert stack.ndim == 3
+        return [stack[i] for i in range(stack.shape[0])]
+    return [s.detach().cpu().numpy() if hasattr(s, "detach") else np.asarray(s) for s in stack]
+
+
+def global_max(stack, C: float = 1e-6) -> float:
+    snaps = as_snapshots(stack)
+    H, W = snaps[0].shape
+    arr, keep = _snap_ptrs(snaps, H, W)
+    return float(lib().fitrig_oracle_global_max(arr, len(snaps), H, W, float(C)))
+
+
+@dataclass
+class TlisiResult:
+    M: float
+    U: int
+    Ty: int
+    Tx: int
+    sumD: np.ndarray  # [U,Ty,Tx] float64
+    maxD: np.ndarray
+    sumR: np.ndarray
+    argmax: np.ndarray  # [U,Ty,Tx] int64, y*W + x
+    q: np.ndarray
+    tlisi: np.ndarray
+
+
+def tlisi(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None) -> TlisiResult:
+    """Eq. 2-6 for every unit and tile.  M=None -> O1 global max of the given stack (floored at C)."""
+    snaps = as_snapshots(stack)
+    L = len(snaps)
+    H, W = snaps[0].shape
+    arr, keep = _snap_ptrs(snaps, H, W)
+    if M is None:
+        M = float(lib().fitrig_oracle_global_max(arr, L, H, W, float(C)))
+    U = L - 2
+    if U < 1:
+        raise ValueError("need L >= 3 snapshots (PAPER.md:155)")
+    Ty, Tx = -(-H // tile), -(-W // tile)
+    shp = (U, Ty, Tx)
+    out = [np.zeros(shp, dtype=np.float64) for _ in range(5)]
+    arg = np.zeros(shp, dtype=np.int64)
+    rc = lib().fitrig_oracle_tlisi(arr, L, H, W, int(tile), float(C), int(ref_mode), float(M),
+                                   _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), _ptr(arg), _ptr(out[3]), _ptr(out[4]))
+    if rc != 0:
+        raise ValueError("fitrig_oracle_tlisi: bad arguments")
+    return TlisiResult(M, U, Ty, Tx, out[0], out[1], out[2], arg, out[3], out[4])
+
+
+def zscore(v: np.ndarray):
+    """Eq. 8 / Eq. 11 over the last axes of v[U, ...] -> (mu[U], sigma[U], z like v)."""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    U = v.shape[0]
+    n = int(np.prod(v.shape[1:]))
+    mu = np.zeros(U)
+    sd = np.zeros(U)
+    z = np.zeros_like(v)
+    lib().fitrig_oracle_zscore(_ptr(v), U, n, _ptr(mu), _ptr(sd), _ptr(z))
+    return mu, sd, z
+
+
+@dataclass
+class Candidates:
+    x: np.ndarray
+    y: np.ndarray
+    snapshot: np.ndarray  # unit index u (branch 0) or peak bin k* (branch 1)
+    tile: np.ndarray  # ty*Tx + tx
+    score: np.ndarray
+    n_found: int
+
+
+def select(z: np.ndarray, argmax: np.ndarray, W: int, tau: float, capacity: int = 1 << 22) -> Candidates:
+    """Eq. 9: { t | z > tau } in (u, ty, tx) order."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    argmax = np.ascontiguousarray(argmax, dtype=np.int64)
+    U = z.shape[0]
+    n = int(np.prod(z.shape[1:]))
+    x = np.zeros(capacity, np.int32)
+    y = np.zeros(capacity, np.int32)
+    u = np.zeros(capacity, np.int32)
+    t = np.zeros(capacity, np.int64)
+    sc = np.zeros(capacity, np.float64)
+    k = int(lib().fitrig_oracle_select(_ptr(z), _ptr(argmax), U, n, int(W), float(tau),
+                                       _ptr(x), _ptr(y), _ptr(u), _ptr(t), _ptr(sc), capacity))
+    m = min(k, capacity)
+    return Candidates(x[:m], y[:m], u[:m], t[:m], sc[:m], k)
+
+
+def spectrum(q: np.ndarray):
+    """Eq. 10 with h = max magnitude: (eta[Ty,Tx], kstar[Ty,Tx]) from q[U,Ty,Tx]."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    U = q.shape[0]
+    n = int(np.prod(q.shape[1:]))
+    eta = np.zeros(q.shape[1:], np.float64)
+    ks = np.zeros(q.shape[1:], np.int32)
+    lib().fitrig_oracle_spectrum(_ptr(q), U, n, _ptr(eta), _ptr(ks))
+    return eta, ks
+
+
+def select_spectrum(z: np.ndarray, kstar: np.ndarray, H: int, W: int, tile: int, tau: float,
+                    capacity: int = 1 << 22) -> Candidates:
+    """Eq. 12 on the eta z-scores; record = (tile centre, k*, z), R18."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    kstar = np.ascontiguousarray(kstar, dtype=np.int32)
+    Ty, Tx = z.shape[-2], z.shape[-1]
+    x = np.zeros(capacity, np.int32)
+    y = np.zeros(capacity, np.int32)
+    kk = np.zeros(capacity, np.int32)
+    t = np.zeros(capacity, np.int64)
+    sc = np.zeros(capacity, np.float64)
+    k = int(lib().fitrig_oracle_select_spectrum(_ptr(z), _ptr(kstar), Ty, Tx, int(H), int(W), int(tile), float(tau),
+                                                _ptr(x), _ptr(y), _ptr(kk), _ptr(t), _ptr(sc), capacity))
+    m = min(k, capacity)
+    return Candidates(x[:m], y[:m], kk[:m], t[:m], sc[:m], k)
+
+
+@dataclass
+class DetectResult:
+    res: TlisiResult
+    mu: np.ndarray
+    sigma: np.ndarray
+    z: np.ndarray
+    cands: Candidates
+    eta: Optional[np.ndarray] = None
+    kstar: Optional[np.ndarray] = None
+
+
+def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
+        tau: float = 5.0, branch: int = 0) -> DetectResult:
+    """Whole path on one stack: O1..O7 (branch 0) or O1..O5 + O8 (branch 1)."""
+    snaps = as_snapshots(stack)
+    H, W = snaps[0].shape
+    res = tlisi(snaps, tile, C, ref_mode, M)
+    if branch == 0:
+        mu, sd, z = zscore(res.q)
+        c = select(z, res.argmax, W, tau)
+        return DetectResult(res, mu, sd, z, c)
+    eta, ks = spectrum(res.q)
+    mu, sd, z = zscore(eta[None])
+    c = select_spectrum(z[0], ks, H, W, tile, tau)
+    return DetectResult(res, mu, sd, z[0], c, eta, ks)

@@ -1,0 +1,246 @@
+/* fitrig_oracle.c -- CPU fp64 ORACLE for the FITrig hot path (tLISI map + detection).
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call this file.
+ * It shares no code, header, table or constant with the CUDA path
+ * (paper_2509_21754_b200/csrc) and neither includes the other.
+ *
+ * What it is: the plain definition of tLISI and of the detection rules, written
+ * out in the paper's order and notation, evaluated in double precision on the same
+ * fp32 input bits the GPU sees.  No blocking, fusion or reordering; the only
+ * concession to run time is an OpenMP "parallel for" over independent (unit, tile-row)
+ * pairs, which the paper itself states are independent.
+ *
+ * Citations are /root/reference/PAPER.md line numbers (+ equation).  Readings R1..R23
+ * of silent / ambiguous passages are SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Notation (0-based): snapshots x_0..x_{L-1}, each H x W row-major fp32.
+ * Unit u = 0..L-3 uses x_u, x_{u+1}, x_{u+2}  (the paper's s = u+1).
+ * Tiles: Ty = ceil(H/N_T), Tx = ceil(W/N_T); tile (ty,tx) covers rows
+ * [ty*N_T, min(H,(ty+1)*N_T)), cols likewise (R5: partial edge tiles keep their own
+ * pixel count n_t).
+ *
+ * Pins (tests/test_oracle_pins.py, tests/golden/): P1..P13 of SURVEY.md section 8(c).
+ * Every function below is pinned; none is "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_REF_ABS 0     /* R1 (default): x_hat = |x|, |x| == 0 -> C                      */
+#define ORACLE_REF_LITERAL 1 /* Eq. 5 exactly as printed: x_hat = x, x == 0 -> C (signed)      */
+#define ORACLE_REF_FLOOR 2   /* x_hat = max(x, C)                                             */
+
+int fitrig_oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void fitrig_oracle_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+/* O1.  M = max( max_{s=1..L} x^(s), C )  -- the signed maximum pixel value over ALL
+ * pixels of ALL L snapshots, floored at C.  PAPER.md:153 (Eq. 2 denominator), 189
+ * ("maximum pixel value across all snapshots"), 223 (M definition).  R2, R14. */
+double fitrig_oracle_global_max(const float* const* snaps, int L, int64_t H, int64_t W, double C) {
+  double m = C;
+  for (int s = 0; s < L; ++s) {
+    const float* x = snaps[s];
+    double ms = C;
+#pragma omp parallel for reduction(max : ms)
+    for (int64_t i = 0; i < H * W; ++i) {
+      double v = (double)x[i];
+      if (v > ms) ms = v;
+    }
+    if (ms > m) m = ms;
+  }
+  return m;
+}
+
+/* Reference intensity x_hat^(s+1), Eq. 5 under reading R1. */
+static double ref_intensity(double x, double C, int ref_mode) {
+  if (ref_mode == ORACLE_REF_LITERAL) return (x == 0.0) ? C : x;
+  if (ref_mode == ORACLE_REF_FLOOR) return (x > C) ? x : C;
+  double a = fabs(x);
+  return (a == 0.0) ? C : a;
+}
+
+/* O2..O5.  For every unit u and tile t:
+ *   D^(s)   = |x^(s+1) - x^(s)|                                   Eq. 3
+ *   Delta   = |D^(s) - D^(s+1)|
+ *   r_i     = Delta_i / x_hat_i  if that is < 1, else 1           Eq. 4-5
+ *   q       = mean(Delta) * max(Delta) * mean(r) / (M * M)        Eq. 2, PAPER.md:153 (R13: M^2)
+ *   tLISI   = 1 - q
+ * Outputs are [U][Ty][Tx]; any output pointer may be NULL.
+ * argmax = y*W + x of the first (lowest row-major) pixel attaining max(Delta) in the tile (R20).
+ * Returns 0, or -1 on bad arguments (R10: L < 3). */
+int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile, double C, int ref_mode,
+                        double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
+                        double* tlisi) {
+  if (L < 3 || H < 1 || W < 1 || tile < 1 || !snaps) return -1;
+  const int U = L - 2;
+  const int Ty = (H + tile - 1) / tile, Tx = (W + tile - 1) / tile;
+#pragma omp parallel for collapse(2) schedule(dynamic, 1)
+  for (int u = 0; u < U; ++u) {
+    for (int ty = 0; ty < Ty; ++ty) {
+      const float* x0 = snaps[u];     /* x^(s)   */
+      const float* x1 = snaps[u + 1]; /* x^(s+1), the reference image */
+      const float* x2 = snaps[u + 2]; /* x^(s+2) */
+      for (int tx = 0; tx < Tx; ++tx) {
+        const int r0 = ty * tile, r1 = (r0 + tile < H) ? r0 + tile : H;
+        const int c0 = tx * tile, c1 = (c0 + tile < W) ? c0 + tile : W;
+        double s_delta = 0.0, m_delta = 0.0, s_r = 0.0;
+        int64_t arg = (int64_t)r0 * W + c0;
+        int first = 1;
+        for (int i = r0; i < r1; ++i) {
+          for (int j = c0; j < c1; ++j) {
+            const int64_t p = (int64_t)i * W + j;
+            const double a = (double)x0[p], b = (double)x1[p], c = (double)x2[p];
+            const double D1 = fabs(b - a);
+            const double D2 = fabs(c - b);
+            const double delta = fabs(D1 - D2);
+            const double xh = ref_intensity(b, C, ref_mode);
+            const double ratio = delta / xh;
+            const double r = (ratio < 1.0) ? ratio : 1.0;
+            s_delta += delta;
+            s_r += r;
+            if (first || delta > m_delta) {
+              m_delta = delta;
+              arg = p;
+              first = 0;
+            }
+          }
+        }
+        const double n_t = (double)(r1 - r0) * (double)(c1 - c0);
+        const double mean_delta = s_delta / n_t;
+        const double mean_r = s_r / n_t;
+        const double qv = mean_delta * m_delta * mean_r / (M * M);
+        const int64_t o = ((int64_t)u * Ty + ty) * Tx + tx;
+        if (sumD) sumD[o] = s_delta;
+        if (maxD) maxD[o] = m_delta;
+        if (sumR) sumR[o] = s_r;
+        if (argmax) argmax[o] = arg;
+        if (q) q[o] = qv;
+        if (tlisi) tlisi[o] = 1.0 - qv;
+      }
+    }
+  }
+  return 0;
+}
+
+/* O6.  z-score of the tile matrix of each unit, Eq. 8:
+ *   z_t = ((1 - tLISI_t) - (1 - mu)) / sigma = (q_t - mean(q)) / std(q)
+ * with the population standard deviation (R3); sigma == 0 -> z = 0 everywhere (R4).
+ * v is [U][n]; mu, sigma are [U]; z is [U][n]. */
+void fitrig_oracle_zscore(const double* v, int U, int64_t n, double* mu, double* sigma, double* z) {
+  for (int u = 0; u < U; ++u) {
+    const double* a = v + (int64_t)u * n;
+    double s = 0.0;
+    for (int64_t i = 0; i < n; ++i) s += a[i];
+    const double m = s / (double)n;
+    double ss = 0.0;
+    for (int64_t i = 0; i < n; ++i) ss += (a[i] - m) * (a[i] - m);
+    const double sd = sqrt(ss / (double)n);
+    if (mu) mu[u] = m;
+    if (sigma) sigma[u] = sd;
+    if (z)
+      for (int64_t i = 0; i < n; ++i) z[(int64_t)u * n + i] = (sd == 0.0) ? 0.0 : (a[i] - m) / sd;
+  }
+}
+
+/* O7.  Candidate set { t | z_t^(s) > tau }, Eq. 9, strict '>' (R6),
+ * listed in (u, ty, tx) order; (x, y) = column, row of the tile's first max-Delta pixel (R16, R20).
+ * Returns the total number found; at most `capacity` are written. */
+int64_t fitrig_oracle_select(const double* z, const int64_t* argmax, int U, int64_t n, int W, double tau,
+                             int32_t* out_x, int32_t* out_y, int32_t* out_u, int64_t* out_tile, double* out_z,
+                             int64_t capacity) {
+  int64_t k = 0;
+  for (int u = 0; u < U; ++u)
+    for (int64_t t = 0; t < n; ++t) {
+      const double zv = z[(int64_t)u * n + t];
+      if (zv > tau) {
+        if (k < capacity) {
+          const int64_t p = argmax ? argmax[(int64_t)u * n + t] : 0;
+          if (out_x) out_x[k] = (int32_t)(p % W);
+          if (out_y) out_y[k] = (int32_t)(p / W);
+          if (out_u) out_u[k] = u;
+          if (out_tile) out_tile[k] = t;
+          if (out_z) out_z[k] = zv;
+        }
+        ++k;
+      }
+    }
+  return k;
+}
+
+/* O8.  Image-frequency branch, Eq. 10 with h = maximum spectral magnitude
+ * (PAPER.md:503):  per tile t,
+ *   a_u   = q_t(u) - mean_u q_t(u)                 (DC removed; |F[tLISI-mean]| == |F[q-mean]|)
+ *   F_k   = sum_u a_u exp(-2 pi i k u / U)         unnormalised DFT of length U (any U, R17)
+ *   eta_t = max_{1 <= k <= floor(U/2)} |F_k| ,  kstar = first k attaining it
+ * q is [U][n]; eta, kstar are [n]. */
+void fitrig_oracle_spectrum(const double* q, int U, int64_t n, double* eta, int32_t* kstar) {
+  const double two_pi = 6.283185307179586476925286766559;
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < n; ++t) {
+    double mean = 0.0;
+    for (int u = 0; u < U; ++u) mean += q[(int64_t)u * n + t];
+    mean /= (double)U;
+    double best = 0.0;
+    int32_t kb = (U / 2 >= 1) ? 1 : 0;
+    for (int k = 1; k <= U / 2; ++k) {
+      double re = 0.0, im = 0.0;
+      for (int u = 0; u < U; ++u) {
+        const double a = q[(int64_t)u * n + t] - mean;
+        const double ang = -two_pi * (double)k * (double)u / (double)U;
+        re += a * cos(ang);
+        im += a * sin(ang);
+      }
+      const double mag = sqrt(re * re + im * im);
+      if (k == 1 || mag > best) {
+        best = mag;
+        kb = k;
+      }
+    }
+    eta[t] = best;
+    if (kstar) kstar[t] = kb;
+  }
+}
+
+/* Eq. 11-12 are fitrig_oracle_zscore(eta, 1, n, ...) followed by the same
+ * strict threshold; the candidate record for this branch is (tile centre, kstar, z), R18:
+ *   x = tx*N_T + w_t/2, y = ty*N_T + h_t/2 (integer division; w_t, h_t the tile's extent). */
+int64_t fitrig_oracle_select_spectrum(const double* z, const int32_t* kstar, int Ty, int Tx, int H, int W,
+                                      int tile, double tau, int32_t* out_x, int32_t* out_y, int32_t* out_k,
+                                      int64_t* out_tile, double* out_z, int64_t capacity) {
+  int64_t k = 0;
+  for (int ty = 0; ty < Ty; ++ty)
+    for (int tx = 0; tx < Tx; ++tx) {
+      const int64_t t = (int64_t)ty * Tx + tx;
+      if (z[t] > tau) {
+        if (k < capacity) {
+          const int r0 = ty * tile, r1 = (r0 + tile < H) ? r0 + tile : H;
+          const int c0 = tx * tile, c1 = (c0 + tile < W) ? c0 + tile : W;
+          if (out_x) out_x[k] = c0 + (c1 - c0) / 2;
+          if (out_y) out_y[k] = r0 + (r1 - r0) / 2;
+          if (out_k) out_k[k] = kstar[t];
+          if (out_tile) out_tile[k] = t;
+          if (out_z) out_z[k] = z[t];
+        }
+        ++k;
+      }
+    }
+  return k;
+}

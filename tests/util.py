@@ -1,0 +1,155 @@
+"""Test-only helpers: slow, independent restatements used to pin the oracle, and comparison rules.
+
+Nothing here is imported by the oracle or by the CUDA path.
+"""
+from __future__ import annotations
+
+import json
+import math
+import os
+from typing import List
+
+import numpy as np
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def golden(name: str) -> dict:
+    with open(os.path.join(GOLDEN, name)) as f:
+        return json.load(f)
+
+
+def brute_force_tlisi(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0, M=None):
+    """Pure-Python per-tile triple loop in Eq. 2's MEAN form, python floats (fp64)."""
+    L, H, W = stack.shape
+    U = L - 2
+    Ty, Tx = -(-H // tile), -(-W // tile)
+    if M is None:
+        M = max(float(stack.max()), C)
+    q = np.zeros((U, Ty, Tx))
+    arg = np.zeros((U, Ty, Tx), dtype=np.int64)
+    parts = np.zeros((3, U, Ty, Tx))
+    for u in range(U):
+        for ty in range(Ty):
+            for tx in range(Tx):
+                deltas: List[float] = []
+                rs: List[float] = []
+                pos: List[int] = []
+                for i in range(ty * tile, min(H, (ty + 1) * tile)):
+                    for j in range(tx * tile, min(W, (tx + 1) * tile)):
+                        a, b, c = float(stack[u, i, j]), float(stack[u + 1, i, j]), float(stack[u + 2, i, j])
+                        d = abs(abs(b - a) - abs(c - b))
+                        if ref_mode == 0:
+                            xh = abs(b) if b != 0.0 else C
+                        elif ref_mode == 1:
+                            xh = b if b != 0.0 else C
+                        else:
+                            xh = max(b, C)
+                        deltas.append(d)
+                        rs.append(min(d / xh, 1.0))
+                        pos.append(i * W + j)
+                n = len(deltas)
+                mean_d = math.fsum(deltas) / n
+                mean_r = math.fsum(rs) / n
+                mx = max(deltas)
+                q[u, ty, tx] = mean_d * mx * mean_r / (M * M)
+                arg[u, ty, tx] = pos[deltas.index(mx)]
+                parts[:, u, ty, tx] = (math.fsum(deltas), mx, math.fsum(rs))
+    return q, arg, parts, M
+
+
+def alg1_route_tlisi(stack: np.ndarray, tile: int, block_dim: int, C: float = 1e-6):
+    """Eq. 6 SUM form walked with Alg. 1's thread/pixel index formula, Eq. 7.
+
+    Square images with N divisible by N_T only (the algorithm's own assumption);
+    |x| reference (R1).  Emulates `block_dim` threads with per-thread partials B1,B2,B3 and a final
+    reduction, i.e. a third, differently ordered route to the same number.
+    """
+    L, N, N2 = stack.shape
+    assert N == N2 and N % tile == 0
+    U = L - 2
+    nt = N // tile
+    M = max(float(stack.max()), C)
+    out = np.zeros((U, nt, nt))
+    K = -(-tile * tile // block_dim)
+    for u in range(U):
+        delta = np.abs(np.abs(stack[u + 1].astype(np.float64) - stack[u]) - np.abs(stack[u + 2].astype(np.float64) - stack[u + 1]))
+        ref = stack[u + 1].astype(np.float64)
+        for block in range(nt * nt):
+            t_x, t_y = block // nt, block % nt
+            B1 = [0.0] * block_dim
+            B2 = [0.0] * block_dim
+            B3 = [0.0] * block_dim
+            for thread in range(block_dim):
+                for k in range(1, K + 1):
+                    lin = thread + (k - 1) * block_dim
+                    if lin < tile * tile:
+                        p_x = t_x * tile + lin // tile
+                        p_y = t_y * tile + lin % tile
+                        d = delta.flat[p_x * N + p_y]
+                        xr = abs(ref.flat[p_x * N + p_y])
+                        xr = xr if xr != 0.0 else C
+                        B1[thread] += d
+                        B2[thread] = max(B2[thread], d)
+                        B3[thread] += (d / xr) if (d / xr) < 1.0 else 1.0
+            out[u, t_x, t_y] = 1.0 - (sum(B1) * max(B2) * sum(B3)) / ((tile * tile) ** 2 * M * M)
+    return out
+
+
+def expected_active_units(active, L: int):
+    """Units whose two difference images differ in whether they contain the transient (R11).
+
+    Snapshot-index bookkeeping only: unit u uses snapshots u, u+1, u+2; D_u holds the transient iff
+    exactly one of snapshots u, u+1 has it on.
+    """
+    act = set(active)
+    out = []
+    for u in range(L - 2):
+        a, b, c = (u in act), (u + 1 in act), (u + 2 in act)
+        if (a != b) != (b != c):
+            out.append(u)
+    return out
+
+
+# ----- comparison rules of SURVEY.md R21/R22 (used by the GPU parity tests) -----
+Q_RTOL = 1e-4
+
+
+def assert_map_close(q_gpu, q_ref, tl_gpu=None, tl_ref=None, rtol=Q_RTOL):
+    q_gpu = np.asarray(q_gpu, dtype=np.float64)
+    q_ref = np.asarray(q_ref, dtype=np.float64)
+    assert q_gpu.shape == q_ref.shape, (q_gpu.shape, q_ref.shape)
+    err = np.abs(q_gpu - q_ref)
+    bound = rtol * np.abs(q_ref) + 1e-30
+    bad = err > bound
+    assert not bad.any(), (f"{int(bad.sum())} of {bad.size} q values outside rtol={rtol}; worst rel "
+                           f"{float((err / (np.abs(q_ref) + 1e-300)).max()):.3e}")
+    if tl_gpu is not None:
+        tl_gpu = np.asarray(tl_gpu, dtype=np.float64)
+        assert np.all(np.abs(tl_gpu - tl_ref) <= rtol * np.abs(tl_ref) + 1e-30)
+
+
+def compare_candidates(gpu, ref_z, ref_mu, ref_sigma, tau, Tx, n_tiles, rtol=Q_RTOL, branch=0):
+    """Candidate-set equality up to the borderline band of R22.
+
+    gpu: list of (x, y, snapshot, score, tile_index, unit_index); ref_z: [U, n_tiles] oracle z.
+    Returns the number of borderline tiles that were tolerated.
+    """
+    ref_z = np.asarray(ref_z, dtype=np.float64).reshape(ref_z.shape[0], -1)
+    U = ref_z.shape[0]
+    band = np.zeros_like(ref_z)
+    for u in range(U):
+        cv = abs(ref_mu[u]) / ref_sigma[u] if ref_sigma[u] > 0 else 0.0
+        band[u] = rtol * (cv + np.abs(ref_z[u]))
+    must = ref_z > tau + band
+    must_not = ref_z < tau - band
+    got = np.zeros_like(must)
+    last = (-1, -1)
+    for (x, y, snap, score, t, u) in gpu:
+        assert (u, t) > last, "candidates must be strictly ascending in (unit, tile row, tile col)"
+        last = (u, t)
+        got[u, t] = True
+        assert abs(score - ref_z[u, t]) <= band[u, t] + 1e-6 * abs(ref_z[u, t]) + 1e-30, (score, ref_z[u, t], band[u, t])
+    assert not (must & ~got).any(), f"missing {int((must & ~got).sum())} non-borderline candidates"
+    assert not (must_not & got).any(), f"{int((must_not & got).sum())} spurious non-borderline candidates"
+    return int((~must & ~must_not).sum())
