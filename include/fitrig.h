@@ -1,0 +1,180 @@
+/* fitrig.h -- C ABI of the B200-native FITrig hot path (arxiv 2509.21754).
+ *
+ * The library computes, on one NVIDIA B200 (sm_100a):
+ *   1. the tLISI transient-index map of a time series of radio snapshot images
+ *      (Eq. 2-6), one value per N_T x N_T tile and per three-snapshot
+ *      unit, and
+ *   2. the significance-thresholded, compacted candidate list
+ *      (image domain: Eq. 8-9; image-frequency domain: Eq. 10-12,
+ *      PAPER.md:343-359 with h = maximum spectral magnitude).
+ *
+ * Citations are /root/reference/PAPER.md line numbers.  "R<n>" are the readings of silent or
+ * ambiguous passages listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Snapshots x_0 .. x_{L-1}: H x W fp32, row-major, finite values (R9).  Pixel magnitudes
+ *     below the fp32 normal range (|x| < 1.2e-38, other than exact zero) are unsupported.
+ *   - Unit u = 0 .. L-3 uses x_u, x_{u+1}, x_{u+2}; x_{u+1} is the reference image
+ *     (the paper's s = u + 1).  U = L - 2 units.
+ *   - Tiles: Ty = ceil(H / N_T), Tx = ceil(W / N_T); partial edge tiles keep their own pixel
+ *     count (R5).  Maps are [U][Ty][Tx], row-major.
+ *   - Image axes: x = column (fastest), y = row (R16).
+ *   - Every call returns FITRIG_OK (0) or a negative FITRIG_ERR_* code; fitrig_last_error()
+ *     then describes it.  No exceptions, no abort, nothing printed.
+ *   - There is NO CPU fallback: without a CUDA device every compute call fails with
+ *     FITRIG_ERR_CUDA.
+ *   - Pointers are marked (device) or (host).  Nothing here is a torch type; a CUDA stream is
+ *     passed as void* (cudaStream_t; NULL = the legacy default stream).
+ */
+#ifndef FITRIG_H_
+#define FITRIG_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FITRIG_OK 0
+#define FITRIG_ERR_INVALID_ARG (-1) /* H,W < 1; L < 3 (R10); tile < 1; NULL pointer; bad strip_rows / mode   */
+#define FITRIG_ERR_CUDA (-2)        /* a CUDA call failed; message carries cudaGetErrorString                 */
+#define FITRIG_ERR_NOMEM (-3)       /* device or pinned-host allocation failed                                */
+#define FITRIG_ERR_STATE (-4)       /* fitrig_detect / getters before any fitrig_tlisi / fitrig_stream        */
+#define FITRIG_ERR_CAPACITY (-5)    /* more candidates than `capacity`: first `capacity` written, n_found=all */
+
+#define FITRIG_REF_ABS 0     /* x_hat = |x|, |x| == 0 -> C   (default, R1)                       */
+#define FITRIG_REF_LITERAL 1 /* x_hat = x,   x == 0   -> C   (Eq. 5 exactly as printed)          */
+#define FITRIG_REF_FLOOR 2   /* x_hat = max(x, C)                                                */
+
+#define FITRIG_BRANCH_IMAGE 0     /* Eq. 8-9   z-score of each unit's tile matrix                  */
+#define FITRIG_BRANCH_FREQUENCY 1 /* Eq. 10-12 temporal DFT of each tile's series, h = max |F_k|   */
+
+typedef struct fitrig_ctx fitrig_ctx; /* opaque; owns every workspace and the current map */
+
+/* Zero-initialised == the paper's defaults. */
+typedef struct {
+  int32_t tile;       /* N_T >= 1; 0 -> 32                                         */
+  float C;            /* Eq. 5 constant; <= 0 -> 1e-6; otherwise must be >= 1e-30   */
+  int32_t ref_mode;   /* FITRIG_REF_*                                                             */
+  float M_override;   /* > 0: use as M instead of the global maximum; 0 -> compute */
+  int32_t branch;     /* FITRIG_BRANCH_*                                                          */
+  int32_t strip_rows; /* fitrig_stream strip height, multiple of tile; 0 -> auto                  */
+  int32_t device;     /* CUDA device ordinal                                                      */
+  int32_t reserved[9];
+} fitrig_params;
+
+/* One candidate, 16 bytes.
+ * Image branch:     (x, y) = pixel of max |D^(s) - D^(s+1)| inside the selected tile, first in
+ *                   row-major order on ties (R20); the paper's tile index is (y / N_T, x / N_T);
+ *                   snapshot = unit index u; score = z_t^(s) of Eq. 8.
+ * Frequency branch: (x, y) = tile centre; snapshot = k*, the DFT bin of the spectral maximum
+ *                   (frequency k* / (U * T_s)); score = z_t of Eq. 11 (R18). */
+typedef struct {
+  int32_t x, y, snapshot;
+  float score;
+} fitrig_candidate;
+
+/* How the library will run a problem; pure host arithmetic (no CUDA call), see fitrig_plan_query. */
+typedef struct {
+  int32_t units, Ty, Tx;     /* map dimensions                                                   */
+  int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, W % 4 == 0)         */
+                             /* 1: generic kernel (any N_T, any W)                               */
+  int32_t time_chunks;       /* K: each tile's L snapshots are split into K chunks (+2 halo)     */
+  int32_t units_per_chunk;   /*                                                                  */
+  int32_t warps_per_cta;     /* fused path: one persistent CTA per SM, this many warps           */
+  int32_t stages;            /* fused path: depth of each warp's TMA ring                        */
+  int32_t grid;              /* CTAs launched                                                    */
+  int32_t smem_bytes;        /* dynamic shared memory per CTA                                    */
+  int32_t strip_rows;        /* fitrig_stream: rows per strip (multiple of N_T)                  */
+  int32_t n_strips;          /* fitrig_stream: strips per image                                  */
+  int32_t n_strip_buffers;   /* fitrig_stream: device strip buffers in rotation                  */
+  int32_t reserved;
+  int64_t strip_buffer_bytes;
+  int64_t workspace_bytes;   /* device bytes fitrig_create allocates (without strip buffers)     */
+} fitrig_plan;
+
+/* fitrig_plan_query -- derive tile grid and launch plan for L snapshots of H x W on a device with
+ * `num_sms` SMs (0 -> 148, one B200).  Host only; usable without a GPU.  Tile grid per R5.
+ * Errors: FITRIG_ERR_INVALID_ARG as for fitrig_create. */
+int fitrig_plan_query(int32_t H, int32_t W, int32_t n_snapshots, const fitrig_params* params /*host, may be NULL*/,
+                      int32_t num_sms, fitrig_plan* out /*host*/);
+
+/* fitrig_create -- allocate a context for L = n_snapshots images of H x W.
+ * params (host) may be NULL (all defaults).  *out receives the context; caller frees it with
+ * fitrig_destroy.  Allocates device workspaces proportional to the MAP (U*Ty*Tx), never to the
+ * images.  Errors: INVALID_ARG (H, W < 1; L < 3; tile < 1; unknown ref_mode / branch; strip_rows not
+ * a multiple of tile), CUDA, NOMEM. */
+int fitrig_create(int32_t H, int32_t W, int32_t n_snapshots, const fitrig_params* params, fitrig_ctx** out);
+
+/* fitrig_destroy -- free everything the context owns (synchronises the device).  NULL is OK. */
+int fitrig_destroy(fitrig_ctx* ctx);
+
+/* fitrig_map_dims -- U = L - 2 units and the Ty x Tx tile grid.  Any out may be NULL. */
+int fitrig_map_dims(const fitrig_ctx* ctx, int32_t* units, int32_t* Ty, int32_t* Tx);
+
+/* fitrig_tlisi -- the tLISI map of a device-resident stack (Eq. 2-6; steps a1-a7 of DESIGN.md).
+ *   d_stack (device)  [L][H][W] fp32, contiguous; owned by the caller, read once, never written.
+ *   d_tlisi (device)  [U][Ty][Tx] fp32 tLISI = 1 - q; may be NULL.  Owned by the caller.
+ * The context keeps q = 1 - tLISI in fp32 (its complement carries the signal, R21), the per-tile
+ * raw sums, the global M and per-unit mean / population std of q (Eq. 8, R3); this
+ * "current map" is what fitrig_detect consumes.  Asynchronous on `cuda_stream`.
+ * Errors: INVALID_ARG (NULL stack), CUDA. */
+int fitrig_tlisi(fitrig_ctx* ctx, const float* d_stack, float* d_tlisi, void* cuda_stream);
+
+/* fitrig_detect -- threshold the current map at z > sigma_threshold (strict, R6) and return the
+ * compacted candidate list (Eq. 9, or Eq. 10-12 when params.branch = FREQUENCY).
+ *   h_out (host)      room for `capacity` candidates, sorted ascending by (snapshot-or-unit,
+ *                     tile row, tile col); frequency branch: by (tile row, tile col).
+ *   n_found (host)    total number of candidates (may exceed capacity -> FITRIG_ERR_CAPACITY).
+ * May be called repeatedly with different thresholds without recomputing the map.  sigma == 0 for
+ * a unit (identical snapshots, one tile) gives z = 0 and no candidate (R4).  Synchronises
+ * `cuda_stream` once.  Errors: STATE (no current map), INVALID_ARG, CAPACITY, CUDA. */
+int fitrig_detect(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate* h_out, int64_t capacity,
+                  int64_t* n_found, void* cuda_stream);
+
+/* fitrig_stream -- same result as fitrig_tlisi for snapshots that live in HOST memory
+ * (Fig. 14: transfers overlapped with the trigger kernels; here at row-strip
+ * granularity so images need not be resident).
+ *   h_snapshots (host) array of L host pointers, each [H][W] fp32.  Pinned (page-locked) memory
+ *                      is needed for the copies to overlap compute; pageable memory works, slowly.
+ *   h_tlisi (host)     [U][Ty][Tx] fp32, may be NULL; valid after `cuda_stream` is synchronised.
+ * Strips of params.strip_rows rows (all L snapshots of those rows) rotate through device
+ * buffers: strip i+1 is copied while strip i is reduced.  Errors: INVALID_ARG, NOMEM, CUDA. */
+int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream);
+
+/* fitrig_get_stats -- M and the per-unit mean / population std of q = 1 - tLISI
+ * (Eq. 8; mu_tLISI = 1 - mu_q).  Frequency branch after fitrig_detect: mu[0], sigma[0] describe
+ * eta (Eq. 11) instead.  Host outputs, each may be NULL; mu, sigma need U doubles.  Synchronises. */
+int fitrig_get_stats(const fitrig_ctx* ctx, float* M, double* mu, double* sigma);
+
+/* fitrig_get_map -- copy one of the context's maps to host memory (synchronises).
+ *   which = 0: q = 1 - tLISI   [U][Ty][Tx] fp32      which = 1: tLISI        [U][Ty][Tx] fp32
+ *   which = 2: eta (Eq. 10)    [Ty][Tx] fp32         which = 3: k* as fp32   [Ty][Tx]
+ * 2 and 3 need the frequency branch and a previous fitrig_detect. */
+int fitrig_get_map(const fitrig_ctx* ctx, int32_t which, float* h_out);
+
+/* fitrig_get_raw -- per-tile partial results of Eq. 6, each [U][Ty][Tx], host, may be
+ * NULL: sum of Delta, max of Delta, sum of r, and the first max-Delta pixel as x and y (R20). */
+int fitrig_get_raw(const fitrig_ctx* ctx, float* sumD, float* maxD, float* sumR, int32_t* arg_x, int32_t* arg_y);
+
+/* fitrig_profile -- enable (1) / disable (0) CUDA-event timing of the library's own kernels on the
+ * launching stream.  fitrig_last_timing then reports, for the last fitrig_tlisi / fitrig_stream,
+ * the summed duration of the fused (or generic) tLISI kernel launches, the number of such launches,
+ * and the duration of the finalise+statistics kernel, in milliseconds (synchronises). */
+int fitrig_profile(fitrig_ctx* ctx, int32_t enable);
+int fitrig_last_timing(const fitrig_ctx* ctx, float* main_kernel_ms, int32_t* main_kernel_launches,
+                       float* finalize_ms);
+
+/* fitrig_launch_count -- kernels launched by this context since creation (for bench.py's gpu_launches). */
+int fitrig_launch_count(const fitrig_ctx* ctx, int64_t* n);
+
+/* fitrig_last_error -- thread-local message of the last failing call on this thread; never NULL. */
+const char* fitrig_last_error(void);
+
+/* fitrig_version -- "fitrig-b200 <major>.<minor>". */
+const char* fitrig_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FITRIG_H_ */

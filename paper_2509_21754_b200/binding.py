@@ -1,0 +1,271 @@
+"""ctypes binding of include/fitrig.h.  Same names as the C ABI, minus the fitrig_ prefix, as methods
+of `Context`.  No arithmetic of the method happens here; there is no CPU fallback: if libfitrig.so is
+missing or no CUDA device is present every compute call raises."""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+
+OK, ERR_INVALID_ARG, ERR_CUDA, ERR_NOMEM, ERR_STATE, ERR_CAPACITY = 0, -1, -2, -3, -4, -5
+REF_ABS, REF_LITERAL, REF_FLOOR = 0, 1, 2
+BRANCH_IMAGE, BRANCH_FREQUENCY = 0, 1
+
+
+class FitrigError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"fitrig error {code}: {msg}")
+        self.code = code
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("tile", ctypes.c_int32), ("C", ctypes.c_float), ("ref_mode", ctypes.c_int32),
+                ("M_override", ctypes.c_float), ("branch", ctypes.c_int32), ("strip_rows", ctypes.c_int32),
+                ("device", ctypes.c_int32), ("reserved", ctypes.c_int32 * 9)]
+
+
+class _Candidate(ctypes.Structure):
+    _fields_ = [("x", ctypes.c_int32), ("y", ctypes.c_int32), ("snapshot", ctypes.c_int32),
+                ("score", ctypes.c_float)]
+
+
+class _Plan(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in
+                ("units", "Ty", "Tx", "path", "time_chunks", "units_per_chunk", "warps_per_cta", "stages", "grid",
+                 "smem_bytes", "strip_rows", "n_strips", "n_strip_buffers", "reserved")] + \
+               [("strip_buffer_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64)]
+
+
+CANDIDATE_DTYPE = np.dtype([("x", np.int32), ("y", np.int32), ("snapshot", np.int32), ("score", np.float32)])
+
+
+@dataclass
+class Candidate:
+    x: int
+    y: int
+    snapshot: int
+    score: float
+
+
+@dataclass
+class Plan:
+    units: int
+    Ty: int
+    Tx: int
+    path: int
+    time_chunks: int
+    units_per_chunk: int
+    warps_per_cta: int
+    stages: int
+    grid: int
+    smem_bytes: int
+    strip_rows: int
+    n_strips: int
+    n_strip_buffers: int
+    strip_buffer_bytes: int
+    workspace_bytes: int
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return os.path.join(_PKG, "libfitrig.so")
+
+
+def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
+    """dlopen the in-tree libfitrig.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if build_if_missing:
+        from . import build as _b
+        if _b.stale():
+            _b.build()
+    if not os.path.exists(path):
+        raise FitrigError(ERR_CUDA, f"{path} not found: run `python -m paper_2509_21754_b200.build`")
+    L = ctypes.CDLL(path)
+    vp, i32, i64, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+    P = ctypes.POINTER
+    L.fitrig_plan_query.argtypes = [i32, i32, i32, P(_Params), i32, P(_Plan)]
+    L.fitrig_create.argtypes = [i32, i32, i32, P(_Params), P(vp)]
+    L.fitrig_destroy.argtypes = [vp]
+    L.fitrig_map_dims.argtypes = [vp, P(i32), P(i32), P(i32)]
+    L.fitrig_tlisi.argtypes = [vp, vp, vp, vp]
+    L.fitrig_detect.argtypes = [vp, f32, vp, i64, P(i64), vp]
+    L.fitrig_stream.argtypes = [vp, P(vp), vp, vp]
+    L.fitrig_get_stats.argtypes = [vp, P(f32), vp, vp]
+    L.fitrig_get_map.argtypes = [vp, i32, vp]
+    L.fitrig_get_raw.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.fitrig_profile.argtypes = [vp, i32]
+    L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32)]
+    L.fitrig_launch_count.argtypes = [vp, P(i64)]
+    for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
+              "fitrig_detect", "fitrig_stream", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count"):
+        getattr(L, n).restype = ctypes.c_int
+    L.fitrig_last_error.restype = ctypes.c_char_p
+    L.fitrig_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def exported_symbols() -> List[str]:
+    """Names include/fitrig.h declares (parsed from the header)."""
+    import re
+    hdr = os.path.join(os.path.dirname(_PKG), "include", "fitrig.h")
+    with open(hdr) as f:
+        txt = f.read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(fitrig_[a-z_]+)\s*\(", txt)))
+
+
+def last_error() -> str:
+    return load_library().fitrig_last_error().decode()
+
+
+def version() -> str:
+    return load_library().fitrig_version().decode()
+
+
+def _check(rc: int, allow: Tuple[int, ...] = ()) -> int:
+    if rc != OK and rc not in allow:
+        raise FitrigError(rc, last_error())
+    return rc
+
+
+def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_IMAGE, strip_rows=0, device=0):
+    p = _Params()
+    p.tile, p.C, p.ref_mode, p.M_override = int(tile), float(C), int(ref_mode), float(M_override)
+    p.branch, p.strip_rows, p.device = int(branch), int(strip_rows), int(device)
+    return p
+
+
+def plan_query(H: int, W: int, n_snapshots: int, num_sms: int = 0, **params) -> Plan:
+    """fitrig_plan_query: host-only, works without a GPU."""
+    L = load_library()
+    p = _make_params(**params)
+    out = _Plan()
+    _check(L.fitrig_plan_query(H, W, n_snapshots, ctypes.byref(p), num_sms, ctypes.byref(out)))
+    return Plan(**{f: getattr(out, f) for f in Plan.__dataclass_fields__})
+
+
+def _dev_ptr(t) -> int:
+    """Device pointer of a torch CUDA tensor (or a raw integer address)."""
+    if t is None:
+        return 0
+    if isinstance(t, int):
+        return t
+    assert t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float32", "need a contiguous CUDA fp32 tensor"
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+class Context:
+    """fitrig_ctx.  Methods mirror the C ABI: tlisi, detect, stream, get_stats, get_map, get_raw, ..."""
+
+    def __init__(self, H: int, W: int, n_snapshots: int, **params):
+        self._L = load_library()
+        self._h = ctypes.c_void_p()
+        p = _make_params(**params)
+        _check(self._L.fitrig_create(H, W, n_snapshots, ctypes.byref(p), ctypes.byref(self._h)))
+        self.H, self.W, self.L = H, W, n_snapshots
+        u, ty, tx = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+        _check(self._L.fitrig_map_dims(self._h, ctypes.byref(u), ctypes.byref(ty), ctypes.byref(tx)))
+        self.units, self.Ty, self.Tx = u.value, ty.value, tx.value
+        self.branch = int(params.get("branch", BRANCH_IMAGE))
+        self.tile = int(params.get("tile", 0)) or 32
+
+    def map_dims(self) -> Tuple[int, int, int]:
+        return self.units, self.Ty, self.Tx
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._L.fitrig_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # ---- compute calls ----
+    def tlisi(self, d_stack, d_tlisi=None, stream=None) -> None:
+        _check(self._L.fitrig_tlisi(self._h, _dev_ptr(d_stack), _dev_ptr(d_tlisi), _stream_ptr(stream)))
+
+    def detect(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None, out: Optional[np.ndarray] = None):
+        """Returns (structured array of candidates actually written, n_found).  Raises on errors other than
+        FITRIG_ERR_CAPACITY (then n_found > len(result))."""
+        if out is None:
+            out = np.zeros(max(capacity, 1), dtype=CANDIDATE_DTYPE)
+        n = ctypes.c_int64(0)
+        _check(self._L.fitrig_detect(self._h, float(sigma_threshold), out.ctypes.data, int(capacity), ctypes.byref(n),
+                                     _stream_ptr(stream)), allow=(ERR_CAPACITY,))
+        return out[: min(n.value, capacity)], n.value
+
+    def stream(self, h_snapshots: Sequence, h_tlisi=None, stream=None) -> None:
+        """h_snapshots: L host tensors/arrays of [H, W] fp32 (pinned for overlap)."""
+        arr = (ctypes.c_void_p * self.L)()
+        assert len(h_snapshots) == self.L
+        for i, s in enumerate(h_snapshots):
+            arr[i] = s.data_ptr() if hasattr(s, "data_ptr") else s.ctypes.data
+        out = 0
+        if h_tlisi is not None:
+            out = h_tlisi.data_ptr() if hasattr(h_tlisi, "data_ptr") else h_tlisi.ctypes.data
+        _check(self._L.fitrig_stream(self._h, arr, out, _stream_ptr(stream)))
+
+    # ---- getters ----
+    def get_stats(self):
+        M = ctypes.c_float()
+        mu = np.zeros(self.units)
+        sd = np.zeros(self.units)
+        _check(self._L.fitrig_get_stats(self._h, ctypes.byref(M), mu.ctypes.data, sd.ctypes.data))
+        return M.value, mu, sd
+
+    def get_map(self, which: int = 0) -> np.ndarray:
+        shape = (self.units, self.Ty, self.Tx) if which in (0, 1) else (self.Ty, self.Tx)
+        out = np.zeros(shape, dtype=np.float32)
+        _check(self._L.fitrig_get_map(self._h, int(which), out.ctypes.data))
+        return out
+
+    def get_raw(self):
+        shape = (self.units, self.Ty, self.Tx)
+        sd, md, sr = (np.zeros(shape, np.float32) for _ in range(3))
+        ax, ay = (np.zeros(shape, np.int32) for _ in range(2))
+        _check(self._L.fitrig_get_raw(self._h, sd.ctypes.data, md.ctypes.data, sr.ctypes.data, ax.ctypes.data,
+                                      ay.ctypes.data))
+        return sd, md, sr, ax, ay
+
+    def profile(self, enable: bool = True) -> None:
+        _check(self._L.fitrig_profile(self._h, int(bool(enable))))
+
+    def last_timing(self):
+        a, n, b = ctypes.c_float(), ctypes.c_int32(), ctypes.c_float()
+        _check(self._L.fitrig_last_timing(self._h, ctypes.byref(a), ctypes.byref(n), ctypes.byref(b)))
+        return a.value, n.value, b.value
+
+    def launch_count(self) -> int:
+        n = ctypes.c_int64()
+        _check(self._L.fitrig_launch_count(self._h, ctypes.byref(n)))
+        return n.value

@@ -1,0 +1,597 @@
+// fitrig.cu -- C ABI (include/fitrig.h) of the B200-native FITrig hot path: context, launch
+// logic, strip streaming.  All arithmetic of the method runs in the kernels of kernels.cuh; this
+// file only allocates, encodes TMA descriptors, launches and copies.  There is no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "fitrig.h"
+#include "kernels.cuh"
+#include "plan.h"
+
+using namespace fitrig;
+
+// ---------------------------------------------------------------------------------------------
+// errors
+// ---------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                               \
+  do {                                                                                               \
+    cudaError_t e__ = (expr);                                                                        \
+    if (e__ != cudaSuccess) {                                                                        \
+      const int code__ = (e__ == cudaErrorMemoryAllocation) ? FITRIG_ERR_NOMEM : FITRIG_ERR_CUDA;    \
+      (void)cudaGetLastError();                                                                      \
+      return fail(code__, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    }                                                                                                \
+  } while (0)
+
+extern "C" const char* fitrig_last_error(void) { return g_err; }
+extern "C" const char* fitrig_version(void) { return "fitrig-b200 0.1"; }
+
+// ---------------------------------------------------------------------------------------------
+// context
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static const int kMaxStripBuffers = 3;
+static const long long kHostStageCands = 4096;  // candidates fetched together with the count
+
+struct CandHeader {
+  unsigned long long total;
+  unsigned long long pad;
+};
+
+struct fitrig_ctx {
+  NormParams prm;
+  int H, W, L, U, Ty, Tx;
+  long long nt, nmap;
+  int num_sms;
+  fitrig_plan plan;
+  EncodeTiledFn encode;
+  // map
+  RawTile* raw;
+  float *q, *tlisi, *M_dev;
+  unsigned* gmax_key;
+  StatPartial* parts;
+  unsigned* counters;
+  double *mu, *sigma;
+  int fin_nblk;
+  // frequency branch
+  float* eta;
+  int* kstar;
+  float2* tw;
+  StatPartial* sparts;
+  unsigned* scounter;
+  double *smu, *ssigma;
+  int spec_nblk;
+  bool eta_valid;
+  // compaction
+  unsigned char* cand_dev;  // CandHeader + candidates
+  long long cand_cap;
+  unsigned* blk_counts;
+  int compact_grid_max;
+  unsigned char* cand_host;  // pinned: CandHeader + kHostStageCands candidates
+  // streaming
+  float* strip_buf[kMaxStripBuffers];
+  int n_strip_buf;
+  long long strip_buf_elems;
+  cudaStream_t copy_stream;
+  cudaEvent_t ev_copied[kMaxStripBuffers], ev_free[kMaxStripBuffers], ev_entry;
+  bool ev_free_pending[kMaxStripBuffers];
+  // profiling
+  bool profile;
+  std::vector<cudaEvent_t> ev_pool;  // pairs: start, stop of each main-kernel launch of the last call
+  int ev_used;
+  cudaEvent_t ev_fin0, ev_fin1;
+  bool fin_timed;
+  bool have_map;
+  long long launches;
+};
+
+static void free_ctx(fitrig_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->prm.device);
+  cudaDeviceSynchronize();
+  cudaFree(c->raw); cudaFree(c->q); cudaFree(c->tlisi); cudaFree(c->M_dev); cudaFree(c->gmax_key);
+  cudaFree(c->parts); cudaFree(c->counters); cudaFree(c->mu); cudaFree(c->sigma);
+  cudaFree(c->eta); cudaFree(c->kstar); cudaFree(c->tw); cudaFree(c->sparts); cudaFree(c->scounter);
+  cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cand_dev); cudaFree(c->blk_counts);
+  if (c->cand_host) cudaFreeHost(c->cand_host);
+  for (int i = 0; i < kMaxStripBuffers; ++i) {
+    cudaFree(c->strip_buf[i]);
+    if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
+    if (c->ev_free[i]) cudaEventDestroy(c->ev_free[i]);
+  }
+  if (c->ev_entry) cudaEventDestroy(c->ev_entry);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+  if (c->ev_fin0) cudaEventDestroy(c->ev_fin0);
+  if (c->ev_fin1) cudaEventDestroy(c->ev_fin1);
+  (void)cudaGetLastError();
+  delete c;
+}
+
+template <int REF, int NS>
+static cudaError_t set_fused_attr() {
+  return cudaFuncSetAttribute(tlisi_fused_kernel<REF, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              kMaxSmemPerCta);
+}
+
+extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_params* params, fitrig_ctx** out) {
+  if (!out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: out is NULL");
+  *out = nullptr;
+  NormParams np;
+  const char* why = "";
+  int rc = normalize_params(H, W, L, params, &np, &why);
+  if (rc != FITRIG_OK) return fail(rc, "fitrig_create: %s", why);
+
+  int ndev = 0;
+  CUDA_TRY(cudaGetDeviceCount(&ndev));
+  if (np.device >= ndev) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: device %d of %d", np.device, ndev);
+  CUDA_TRY(cudaSetDevice(np.device));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, np.device));
+  if (prop.major < 10)
+    return fail(FITRIG_ERR_CUDA, "fitrig_create: device %d is sm_%d%d; this library is built for sm_100a (B200) only",
+                np.device, prop.major, prop.minor);
+
+  fitrig_ctx* c = new (std::nothrow) fitrig_ctx();
+  if (!c) return fail(FITRIG_ERR_NOMEM, "fitrig_create: host allocation failed");
+  c->prm = np;
+  c->H = H; c->W = W; c->L = L; c->U = L - 2;
+  c->num_sms = prop.multiProcessorCount;
+  rc = fitrig_plan_query(H, W, L, params, c->num_sms, &c->plan);
+  if (rc != FITRIG_OK) { delete c; return fail(rc, "fitrig_create: plan failed"); }
+  c->Ty = c->plan.Ty; c->Tx = c->plan.Tx;
+  c->nt = (long long)c->Ty * c->Tx;
+  c->nmap = c->nt * c->U;
+  if (c->nmap * (long long)std::max(1, c->plan.time_chunks) > 0x7fffffffll) {
+    delete c;
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: map of %lld entries is too large", c->nmap);
+  }
+
+#define CTX_TRY(expr)                                                                                 \
+  do {                                                                                                \
+    cudaError_t e__ = (expr);                                                                         \
+    if (e__ != cudaSuccess) {                                                                         \
+      const int code__ = (e__ == cudaErrorMemoryAllocation) ? FITRIG_ERR_NOMEM : FITRIG_ERR_CUDA;     \
+      (void)cudaGetLastError();                                                                       \
+      free_ctx(c);                                                                                    \
+      return fail(code__, "fitrig_create: %s failed: %s", #expr, cudaGetErrorString(e__));            \
+    }                                                                                                 \
+  } while (0)
+
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  CTX_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+  if (!fn || qres != cudaDriverEntryPointSuccess) {
+    free_ctx(c);
+    return fail(FITRIG_ERR_CUDA, "fitrig_create: cuTensorMapEncodeTiled not available in this driver");
+  }
+  c->encode = (EncodeTiledFn)fn;
+
+  CTX_TRY(cudaMalloc(&c->raw, sizeof(RawTile) * c->nmap));
+  CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
+  CTX_TRY(cudaMalloc(&c->tlisi, sizeof(float) * c->nmap));
+  CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float)));
+  CTX_TRY(cudaMalloc(&c->gmax_key, sizeof(unsigned)));
+  c->fin_nblk = (int)std::max<long long>(1, std::min<long long>(64, (c->nt + 2047) / 2048));
+  CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * c->U * c->fin_nblk));
+  CTX_TRY(cudaMalloc(&c->counters, sizeof(unsigned) * c->U));
+  CTX_TRY(cudaMemset(c->counters, 0, sizeof(unsigned) * c->U));
+  CTX_TRY(cudaMalloc(&c->mu, sizeof(double) * c->U));
+  CTX_TRY(cudaMalloc(&c->sigma, sizeof(double) * c->U));
+  if (np.branch == FITRIG_BRANCH_FREQUENCY) {
+    CTX_TRY(cudaMalloc(&c->eta, sizeof(float) * c->nt));
+    CTX_TRY(cudaMalloc(&c->kstar, sizeof(int) * c->nt));
+    CTX_TRY(cudaMalloc(&c->tw, sizeof(float2) * c->U));
+    std::vector<float2> tw(c->U);
+    for (int j = 0; j < c->U; ++j) {  // exp(-2 pi i j / U), Eq. 10's Fourier kernel (R17)
+      const double a = -2.0 * M_PI * (double)j / (double)c->U;
+      tw[j].x = (float)cos(a);
+      tw[j].y = (float)sin(a);
+    }
+    CTX_TRY(cudaMemcpy(c->tw, tw.data(), sizeof(float2) * c->U, cudaMemcpyHostToDevice));
+    c->spec_nblk = (int)std::max<long long>(1, std::min<long long>(4 * c->num_sms, (c->nt + 127) / 128));
+    CTX_TRY(cudaMalloc(&c->sparts, sizeof(StatPartial) * c->spec_nblk));
+    CTX_TRY(cudaMalloc(&c->scounter, sizeof(unsigned)));
+    CTX_TRY(cudaMemset(c->scounter, 0, sizeof(unsigned)));
+    CTX_TRY(cudaMalloc(&c->smu, sizeof(double)));
+    CTX_TRY(cudaMalloc(&c->ssigma, sizeof(double)));
+  }
+  int occ = 0;
+  CTX_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, compact_kernel, 512, 0));
+  c->compact_grid_max = std::max(1, occ) * c->num_sms;
+  CTX_TRY(cudaMalloc(&c->blk_counts, sizeof(unsigned) * c->compact_grid_max));
+  c->cand_cap = kHostStageCands;
+  CTX_TRY(cudaMalloc(&c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * c->cand_cap));
+  CTX_TRY(cudaHostAlloc(&c->cand_host, sizeof(CandHeader) + sizeof(fitrig_candidate) * kHostStageCands,
+                        cudaHostAllocDefault));
+  CTX_TRY(cudaEventCreate(&c->ev_fin0));
+  CTX_TRY(cudaEventCreate(&c->ev_fin1));
+  if (c->plan.path == 0) {
+    CTX_TRY((set_fused_attr<0, 2>())); CTX_TRY((set_fused_attr<0, 3>())); CTX_TRY((set_fused_attr<0, 4>()));
+    CTX_TRY((set_fused_attr<1, 2>())); CTX_TRY((set_fused_attr<1, 3>())); CTX_TRY((set_fused_attr<1, 4>()));
+    CTX_TRY((set_fused_attr<2, 2>())); CTX_TRY((set_fused_attr<2, 3>())); CTX_TRY((set_fused_attr<2, 4>()));
+  }
+#undef CTX_TRY
+  *out = c;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_destroy(fitrig_ctx* ctx) {
+  free_ctx(ctx);
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_map_dims(const fitrig_ctx* ctx, int32_t* units, int32_t* Ty, int32_t* Tx) {
+  if (!ctx) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_map_dims: ctx is NULL");
+  if (units) *units = ctx->U;
+  if (Ty) *Ty = ctx->Ty;
+  if (Tx) *Tx = ctx->Tx;
+  return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// launches
+// ---------------------------------------------------------------------------------------------
+static int prof_begin(fitrig_ctx* c, cudaStream_t st) {
+  if (!c->profile) return FITRIG_OK;
+  while ((int)c->ev_pool.size() < 2 * (c->ev_used + 1)) {
+    cudaEvent_t e;
+    CUDA_TRY(cudaEventCreate(&e));
+    c->ev_pool.push_back(e);
+  }
+  CUDA_TRY(cudaEventRecord(c->ev_pool[2 * c->ev_used], st));
+  return FITRIG_OK;
+}
+static int prof_end(fitrig_ctx* c, cudaStream_t st) {
+  if (!c->profile) return FITRIG_OK;
+  CUDA_TRY(cudaEventRecord(c->ev_pool[2 * c->ev_used + 1], st));
+  c->ev_used++;
+  return FITRIG_OK;
+}
+
+template <int REF>
+static cudaError_t launch_fused_stage(int stages, dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                      const CUtensorMap& tm, const FusedParams& fp) {
+  switch (stages) {
+    case 2: tlisi_fused_kernel<REF, 2><<<grid, block, smem, st>>>(tm, fp); break;
+    case 3: tlisi_fused_kernel<REF, 3><<<grid, block, smem, st>>>(tm, fp); break;
+    default: tlisi_fused_kernel<REF, 4><<<grid, block, smem, st>>>(tm, fp); break;
+  }
+  return cudaGetLastError();
+}
+
+// tLISI partial sums of `rows` image rows (all L snapshots) that start at tile row ty_base.
+// base: device pointer to snapshot 0 of those rows; snap_stride: elements between snapshots.
+static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int ty_base,
+                             bool with_max, cudaStream_t st) {
+  const int tile = c->prm.tile;
+  const int rows_tiles = (rows + tile - 1) / tile;
+  fitrig_plan pl = c->plan;
+  const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
+  if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
+  if (pl.path == 0 && (rows_tiles != c->Ty)) plan_launch(tile, c->W, rows_tiles, c->Tx, c->U, c->num_sms, &pl);
+
+  int rc = prof_begin(c, st);
+  if (rc) return rc;
+  if (pl.path == 0) {
+    CUtensorMap tm;
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)c->L};
+    const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
+    const cuuint32_t box[3] = {kFastTile, kFastTile, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = c->encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    FusedParams fp;
+    fp.raw = c->raw; fp.gmax_key = c->gmax_key;
+    fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
+    fp.U = c->U; fp.K = pl.time_chunks; fp.cu = pl.units_per_chunk;
+    fp.nitems = rows_tiles * c->Tx * pl.time_chunks;
+    fp.C = c->prm.C;
+    const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
+    cudaError_t e;
+    switch (c->prm.ref_mode) {
+      case FITRIG_REF_ABS: e = launch_fused_stage<FITRIG_REF_ABS>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_LITERAL: e = launch_fused_stage<FITRIG_REF_LITERAL>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
+      default: e = launch_fused_stage<FITRIG_REF_FLOOR>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
+    }
+    CUDA_TRY(e);
+    c->launches++;
+  } else {
+    if (with_max) {
+      // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
+      for (int s = 0; s < c->L; ++s) {
+        stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)s * snap_stride,
+                                                                       (long long)rows * c->W, c->gmax_key);
+        CUDA_TRY(cudaGetLastError());
+        c->launches++;
+      }
+    }
+    GenericParams gp;
+    gp.base = base; gp.snap_stride = snap_stride; gp.rows = rows; gp.W = c->W; gp.tile = tile;
+    gp.raw = c->raw; gp.Tx = c->Tx; gp.Ty = c->Ty; gp.ty_base = ty_base; gp.rows_tiles = rows_tiles; gp.U = c->U;
+    int G = 1;
+    const long long n_t = (long long)tile * tile;
+    while (G < 32 && G < n_t) G <<= 1;
+    gp.G = G;
+    gp.C = c->prm.C;
+    const long long groups = (long long)rows_tiles * c->Tx * c->U;
+    const long long threads = groups * G;
+    const long long blocks = (threads + 255) / 256;
+    if (blocks > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "generic path: too many tiles for one launch");
+    switch (c->prm.ref_mode) {
+      case FITRIG_REF_ABS: tlisi_generic_kernel<FITRIG_REF_ABS><<<(unsigned)blocks, 256, 0, st>>>(gp); break;
+      case FITRIG_REF_LITERAL: tlisi_generic_kernel<FITRIG_REF_LITERAL><<<(unsigned)blocks, 256, 0, st>>>(gp); break;
+      default: tlisi_generic_kernel<FITRIG_REF_FLOOR><<<(unsigned)blocks, 256, 0, st>>>(gp); break;
+    }
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+  }
+  return prof_end(c, st);
+}
+
+static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st) {
+  FinalizeParams fp;
+  fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
+  fp.gmax_key = c->gmax_key; fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
+  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
+  fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
+  if (c->profile) CUDA_TRY(cudaEventRecord(c->ev_fin0, st));
+  finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
+  CUDA_TRY(cudaGetLastError());
+  if (c->profile) { CUDA_TRY(cudaEventRecord(c->ev_fin1, st)); c->fin_timed = true; }
+  c->launches++;
+  c->have_map = true;
+  c->eta_valid = false;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_tlisi(fitrig_ctx* c, const float* d_stack, float* d_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: ctx is NULL");
+  if (!d_stack) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: d_stack is NULL");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  c->ev_used = 0;
+  c->fin_timed = false;
+  CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, sizeof(unsigned), st));
+  int rc = launch_tlisi_rows(c, d_stack, (long long)c->H * c->W, c->H, 0, true, st);
+  if (rc) return rc;
+  return launch_finalize(c, d_tlisi, st);
+}
+
+extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: ctx is NULL");
+  if (!h_snapshots) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots is NULL");
+  for (int s = 0; s < c->L; ++s)
+    if (!h_snapshots[s]) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots[%d] is NULL", s);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  const int rows_per = c->plan.strip_rows, nstrips = c->plan.n_strips, nbuf = c->plan.n_strip_buffers;
+  if (!c->copy_stream) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
+    c->strip_buf_elems = (long long)c->L * rows_per * c->W;
+    for (int b = 0; b < nbuf; ++b) {
+      CUDA_TRY(cudaMalloc(&c->strip_buf[b], sizeof(float) * c->strip_buf_elems));
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copied[b], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_free[b], cudaEventDisableTiming));
+    }
+    c->n_strip_buf = nbuf;
+  }
+  c->ev_used = 0;
+  c->fin_timed = false;
+  CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, sizeof(unsigned), st));
+  // the copy stream may not run ahead of work already queued on the caller's stream
+  CUDA_TRY(cudaEventRecord(c->ev_entry, st));
+  CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
+  for (int b = 0; b < nbuf; ++b) c->ev_free_pending[b] = false;
+  const long long snap_stride = (long long)rows_per * c->W;
+  for (int i = 0; i < nstrips; ++i) {
+    const int b = i % nbuf;
+    const int r0 = i * rows_per;
+    const int rows = std::min(rows_per, c->H - r0);
+    if (c->ev_free_pending[b]) CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_free[b], 0));
+    for (int s = 0; s < c->L; ++s) {  // snapshot s, rows r0..r0+rows: contiguous on both sides
+      CUDA_TRY(cudaMemcpyAsync(c->strip_buf[b] + (long long)s * snap_stride, h_snapshots[s] + (long long)r0 * c->W,
+                               sizeof(float) * (long long)rows * c->W, cudaMemcpyHostToDevice, c->copy_stream));
+    }
+    CUDA_TRY(cudaEventRecord(c->ev_copied[b], c->copy_stream));
+    CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copied[b], 0));
+    int rc = launch_tlisi_rows(c, c->strip_buf[b], snap_stride, rows, r0 / c->prm.tile, true, st);
+    if (rc) return rc;
+    CUDA_TRY(cudaEventRecord(c->ev_free[b], st));
+    c->ev_free_pending[b] = true;
+  }
+  int rc = launch_finalize(c, nullptr, st);
+  if (rc) return rc;
+  if (h_tlisi) CUDA_TRY(cudaMemcpyAsync(h_tlisi, c->tlisi, sizeof(float) * c->nmap, cudaMemcpyDeviceToHost, st));
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
+                             void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: ctx is NULL");
+  if (!n_found) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: n_found is NULL");
+  if (capacity < 0 || (capacity > 0 && !h_out)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: bad h_out/capacity");
+  if (!(tau == tau)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: sigma_threshold is NaN");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_detect: no current map (call fitrig_tlisi or fitrig_stream first)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  const bool freq = c->prm.branch == FITRIG_BRANCH_FREQUENCY;
+  if (freq && !c->eta_valid) {
+    SpectrumParams sp;
+    sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = c->nt; sp.U = c->U;
+    sp.nblk = c->spec_nblk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
+    spectrum_kernel<<<c->spec_nblk, 128, sizeof(float2) * c->U, st>>>(sp);
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+    c->eta_valid = true;
+  }
+  const long long rows = freq ? 1 : c->U;
+  const long long N = rows * c->nt;
+  const long long want = std::min<long long>(capacity, N);
+  if (want > c->cand_cap) {  // grow the device list (rare: only for very low thresholds)
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaFree(c->cand_dev));
+    c->cand_dev = nullptr;
+    c->cand_cap = 0;
+    CUDA_TRY(cudaMalloc(&c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * want));
+    c->cand_cap = want;
+  }
+  CompactParams cp;
+  cp.v = freq ? c->eta : c->q;
+  cp.raw = c->raw; cp.kstar = c->kstar;
+  cp.mu = freq ? c->smu : c->mu; cp.sigma = freq ? c->ssigma : c->sigma;
+  cp.tau = tau; cp.rows = (int)rows; cp.nt = c->nt;
+  cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.branch = c->prm.branch;
+  cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
+  cp.cap = std::min<long long>(c->cand_cap, std::max<long long>(capacity, 0));
+  cp.total = reinterpret_cast<unsigned long long*>(c->cand_dev);
+  cp.blk_counts = c->blk_counts;
+  const int threads = 512;
+  int grid = (int)std::min<long long>(c->compact_grid_max, (N + threads - 1) / threads);
+  grid = std::max(grid, 1);
+  cp.seg = ((N + grid - 1) / grid + threads - 1) / threads * threads;
+  void* args[] = {&cp};
+  CUDA_TRY(cudaLaunchCooperativeKernel((void*)compact_kernel, dim3(grid), dim3(threads), args, 0, st));
+  c->launches++;
+  // count + the first kHostStageCands candidates in one copy; a second copy only for longer lists
+  const long long first = std::min<long long>(cp.cap, kHostStageCands);
+  CUDA_TRY(cudaMemcpyAsync(c->cand_host, c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * first,
+                           cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  const long long total = (long long)reinterpret_cast<CandHeader*>(c->cand_host)->total;
+  const long long nwrite = std::min<long long>(total, cp.cap);
+  const long long n1 = std::min(nwrite, first);
+  if (n1 > 0) memcpy(h_out, c->cand_host + sizeof(CandHeader), sizeof(fitrig_candidate) * n1);
+  if (nwrite > n1) {
+    CUDA_TRY(cudaMemcpyAsync(h_out + n1, cp.out + n1, sizeof(fitrig_candidate) * (nwrite - n1),
+                             cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+  }
+  *n_found = total;
+  if (total > capacity)
+    return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)capacity);
+  return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// getters
+// ---------------------------------------------------------------------------------------------
+extern "C" int fitrig_get_stats(const fitrig_ctx* c, float* M, double* mu, double* sigma) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_get_stats: ctx is NULL");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_get_stats: no current map");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  if (M) CUDA_TRY(cudaMemcpy(M, c->M_dev, sizeof(float), cudaMemcpyDeviceToHost));
+  const bool freq_stats = c->prm.branch == FITRIG_BRANCH_FREQUENCY && c->eta_valid;
+  if (mu) {
+    CUDA_TRY(cudaMemcpy(mu, c->mu, sizeof(double) * c->U, cudaMemcpyDeviceToHost));
+    if (freq_stats) CUDA_TRY(cudaMemcpy(mu, c->smu, sizeof(double), cudaMemcpyDeviceToHost));
+  }
+  if (sigma) {
+    CUDA_TRY(cudaMemcpy(sigma, c->sigma, sizeof(double) * c->U, cudaMemcpyDeviceToHost));
+    if (freq_stats) CUDA_TRY(cudaMemcpy(sigma, c->ssigma, sizeof(double), cudaMemcpyDeviceToHost));
+  }
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_get_map(const fitrig_ctx* c, int32_t which, float* h_out) {
+  if (!c || !h_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_get_map: NULL argument");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_get_map: no current map");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  switch (which) {
+    case 0: CUDA_TRY(cudaMemcpy(h_out, c->q, sizeof(float) * c->nmap, cudaMemcpyDeviceToHost)); break;
+    case 1: CUDA_TRY(cudaMemcpy(h_out, c->tlisi, sizeof(float) * c->nmap, cudaMemcpyDeviceToHost)); break;
+    case 2:
+    case 3: {
+      if (c->prm.branch != FITRIG_BRANCH_FREQUENCY || !c->eta_valid)
+        return fail(FITRIG_ERR_STATE, "fitrig_get_map: eta needs the frequency branch and a previous fitrig_detect");
+      if (which == 2) {
+        CUDA_TRY(cudaMemcpy(h_out, c->eta, sizeof(float) * c->nt, cudaMemcpyDeviceToHost));
+      } else {
+        std::vector<int> k(c->nt);
+        CUDA_TRY(cudaMemcpy(k.data(), c->kstar, sizeof(int) * c->nt, cudaMemcpyDeviceToHost));
+        for (long long i = 0; i < c->nt; ++i) h_out[i] = (float)k[i];
+      }
+      break;
+    }
+    default: return fail(FITRIG_ERR_INVALID_ARG, "fitrig_get_map: which = %d", which);
+  }
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_get_raw(const fitrig_ctx* c, float* sumD, float* maxD, float* sumR, int32_t* ax, int32_t* ay) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_get_raw: ctx is NULL");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_get_raw: no current map");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  std::vector<RawTile> r(c->nmap);
+  CUDA_TRY(cudaMemcpy(r.data(), c->raw, sizeof(RawTile) * c->nmap, cudaMemcpyDeviceToHost));
+  const int tile = c->prm.tile;
+  for (long long i = 0; i < c->nmap; ++i) {
+    const long long t = i % c->nt;
+    const int ty = (int)(t / c->Tx), tx = (int)(t % c->Tx);
+    if (sumD) sumD[i] = r[i].sumD;
+    if (maxD) maxD[i] = r[i].maxD;
+    if (sumR) sumR[i] = r[i].sumR;
+    if (ax) ax[i] = tx * tile + r[i].pos % tile;
+    if (ay) ay[i] = ty * tile + r[i].pos / tile;
+  }
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_profile(fitrig_ctx* c, int32_t enable) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_profile: ctx is NULL");
+  c->profile = enable != 0;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_last_timing(const fitrig_ctx* c, float* main_ms, int32_t* main_launches, float* fin_ms) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_last_timing: ctx is NULL");
+  if (!c->profile || !c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_last_timing: profiling was not enabled");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  float tot = 0.f;
+  for (int i = 0; i < c->ev_used; ++i) {
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
+    tot += ms;
+  }
+  if (main_ms) *main_ms = tot;
+  if (main_launches) *main_launches = c->ev_used;
+  if (fin_ms) {
+    *fin_ms = 0.f;
+    if (c->fin_timed) CUDA_TRY(cudaEventElapsedTime(fin_ms, c->ev_fin0, c->ev_fin1));
+  }
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_launch_count(const fitrig_ctx* c, int64_t* n) {
+  if (!c || !n) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_launch_count: NULL argument");
+  *n = c->launches;
+  return FITRIG_OK;
+}

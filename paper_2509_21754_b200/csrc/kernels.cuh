@@ -1,0 +1,613 @@
+// kernels.cuh -- sm_100a CUDA kernels of the FITrig hot path (arxiv 2509.21754).
+//
+//   tlisi_fused_kernel    steps a1-a5: |x_{s+1}-x_s|, second difference, clamped ratio, per-tile
+//                         sum/max/argmax/sum and the global maximum, in ONE pass that reads every
+//                         snapshot byte once.  A warp owns one 32x32 tile and marches it through
+//                         time; tiles arrive through a per-warp ring of TMA boxes (cp.async.bulk.tensor).
+//   tlisi_generic_kernel  the same per-tile quantities for any tile size / alignment (3 reads per pixel-unit).
+//   stack_max_kernel      global maximum for the generic path.
+//   finalize_kernel       step a6-a7: q = mean(D)*max(D)*mean(r)/M^2, tLISI = 1-q, per-unit mean/std.
+//   spectrum_kernel       step a10: per-tile temporal DFT, eta = max |F_k|, k*.
+//   compact_kernel        step a8: z-score, strict threshold, ordered compaction (ballot + prefix sums).
+//
+// Citations: PAPER.md line numbers; R<n> = readings in DESIGN.md.
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "fitrig.h"
+#include "plan.h"
+
+namespace fitrig {
+namespace cg = cooperative_groups;
+
+// Per-tile, per-unit partial results of Eq. 6: sum Delta, max Delta, sum r, and the
+// tile-relative position (row * N_T + col) of the first max-Delta pixel (R20).  16 bytes.
+struct __align__(16) RawTile {
+  float sumD;
+  float maxD;
+  float sumR;
+  int32_t pos;
+};
+
+// ---------------------------------------------------------------------------------------------
+// small device helpers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+// One 32x32 fp32 box of snapshot z at pixel (x, y) -> shared memory; completes on `bar`.
+__device__ __forceinline__ void tma_load_tile(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z,
+                                              uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ float rcp_approx(float a) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
+// order-preserving float -> uint key (so atomicMax / redux.max on uints orders signed floats)
+__device__ __forceinline__ unsigned float_to_key(float f) {
+  unsigned b = __float_as_uint(f);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__host__ __device__ __forceinline__ float key_to_float(unsigned k) {
+  unsigned b = (k & 0x80000000u) ? (k & 0x7fffffffu) : ~k;
+#ifdef __CUDA_ARCH__
+  return __uint_as_float(b);
+#else
+  float f;
+  memcpy(&f, &b, 4);
+  return f;
+#endif
+}
+
+// Clamped ratio r of Eq. 4-5 for one pixel: delta >= 0, ref = x^(s+1).
+//   ABS     x_hat = |ref|, |ref| == 0 -> C     r = min(delta / x_hat, 1)
+//   LITERAL x_hat = ref,   ref == 0   -> C     (r may be negative)
+//   FLOOR   x_hat = max(ref, C)
+// delta * rcp saturates to [0,1]; the saturating multiply also maps 0 * inf (= NaN) to 0, which is
+// the value Eq. 5 gives (R8).
+template <int REF_MODE>
+__device__ __forceinline__ float clamped_ratio(float delta, float ref, float C) {
+  if (REF_MODE == FITRIG_REF_ABS) {
+    float a = fabsf(ref);
+    a = (a == 0.f) ? C : a;
+    return __saturatef(delta * rcp_approx(a));
+  } else if (REF_MODE == FITRIG_REF_LITERAL) {
+    float a = (ref == 0.f) ? C : ref;
+    float qv = delta * rcp_approx(a);
+    qv = (qv != qv) ? 0.f : qv;  // 0 * inf
+    return fminf(qv, 1.f);
+  } else {
+    float a = fmaxf(ref, C);
+    return __saturatef(delta * rcp_approx(a));
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused time-marching tLISI kernel (N_T = 32)
+// ---------------------------------------------------------------------------------------------
+struct FusedParams {
+  RawTile* raw;        // [U][Ty][Tx] whole map
+  unsigned* gmax_key;  // ordered key of the running global maximum (atomicMax)
+  int Tx, Ty;          // whole-map tile grid
+  int rows_tiles;      // tile rows covered by this launch (whole image, or one strip)
+  int ty_base;         // first tile row of this launch inside the whole map
+  int U;               // units = L - 2
+  int K;               // time chunks
+  int cu;              // units per chunk
+  int nitems;          // rows_tiles * Tx * K
+  float C;
+};
+
+struct ItemCoord {
+  int tx, ty_local, u0, nsteps;
+};
+
+__device__ __forceinline__ ItemCoord decode_item(const FusedParams& p, int item) {
+  ItemCoord c;
+  const int per_chunk = p.rows_tiles * p.Tx;
+  const int k = item / per_chunk;
+  const int t = item - k * per_chunk;
+  c.ty_local = t / p.Tx;
+  c.tx = t - c.ty_local * p.Tx;
+  c.u0 = k * p.cu;
+  const int u1 = min(p.U, c.u0 + p.cu);
+  c.nsteps = u1 - c.u0 + 2;  // snapshots u0 .. u1+1
+  return c;
+}
+
+// Lane l of the warp owns, in each 32x32 tile, columns 4*(l%8)..+3 of rows (l/8) + 4*j, j = 0..7:
+// a quarter warp reads one 128-byte tile row from shared memory (conflict free), and the 32 pixels
+// of a lane are visited in increasing row-major order (so a strict '>' keeps the first maximum).
+template <int REF_MODE, int NSTAGE>
+__global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
+    tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
+  extern __shared__ __align__(1024) unsigned char smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nwarps = blockDim.x >> 5;
+  unsigned char* ring = smem + (size_t)warp * NSTAGE * kTileBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * NSTAGE * kTileBytes) + warp * NSTAGE;
+
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < NSTAGE; ++i) mbar_init(smem_u32(&bars[i]), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int total_warps = gridDim.x * nwarps;
+  const int warp_global = blockIdx.x * nwarps + warp;
+  const uint64_t policy = l2_evict_first_policy();
+  const uint32_t ring_addr = smem_u32(ring);
+  const uint32_t bar_addr = smem_u32(bars);
+
+  // ---- producer cursor (lane 0 issues; all lanes track it, it is warp uniform) ----
+  int p_item = warp_global, p_step = 0;
+  ItemCoord pc = decode_item(p, p_item < p.nitems ? p_item : 0);
+  auto issue_next = [&](int slot) {
+    if (p_item < p.nitems) {
+      if (lane == 0) {
+        const uint32_t bar = bar_addr + slot * 8;
+        mbar_arrive_expect_tx(bar, kTileBytes);
+        tma_load_tile(ring_addr + slot * kTileBytes, &tmap, bar, pc.tx * kFastTile, pc.ty_local * kFastTile,
+                      pc.u0 + p_step, policy);
+      }
+      if (++p_step == pc.nsteps) {
+        p_step = 0;
+        p_item += total_warps;
+        if (p_item < p.nitems) pc = decode_item(p, p_item);
+      }
+    }
+  };
+#pragma unroll
+  for (int i = 0; i < NSTAGE; ++i) issue_next(i);
+
+  float xp[32], dp[32];  // x_{s-1} and the signed difference x_{s-1} - x_{s-2} of this lane's pixels
+  float gmax = -3.402823466e38f;
+  int slot = 0;
+  uint32_t phase = 0;
+  const int lrow = lane >> 3, lcol = (lane & 7) * 4;
+
+  for (int item = warp_global; item < p.nitems; item += total_warps) {
+    const ItemCoord c = decode_item(p, item);
+    const int ty = p.ty_base + c.ty_local;
+    for (int step = 0; step < c.nsteps; ++step) {
+      mbar_wait(bar_addr + slot * 8, phase);
+      float4 cur[8];
+      const float4* src = reinterpret_cast<const float4*>(ring + (size_t)slot * kTileBytes) + lane;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) cur[j] = src[j * 32];  // row (lane/8)+4j, 16-byte column group lane%8
+      __syncwarp();        // every lane has its copy: the slot may be refilled
+      issue_next(slot);    // prefetch NSTAGE steps ahead
+      if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        gmax = fmaxf(gmax, fmaxf(fmaxf(cur[j].x, cur[j].y), fmaxf(cur[j].z, cur[j].w)));
+      }
+
+      if (step == 0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { xp[4 * j] = cur[j].x; xp[4 * j + 1] = cur[j].y; xp[4 * j + 2] = cur[j].z; xp[4 * j + 3] = cur[j].w; }
+      } else if (step == 1) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float v[4] = {cur[j].x, cur[j].y, cur[j].z, cur[j].w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e) { dp[4 * j + e] = v[e] - xp[4 * j + e]; xp[4 * j + e] = v[e]; }
+        }
+      } else {
+        float S = 0.f, R = 0.f, Mx = 0.f;
+        int kmax = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float v[4] = {cur[j].x, cur[j].y, cur[j].z, cur[j].w};
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int k = 4 * j + e;
+            const float d = v[e] - xp[k];                       // D^(s+1) (signed), Eq. 3
+            const float delta = fabsf(fabsf(d) - fabsf(dp[k]));  // |D^(s) - D^(s+1)|
+            S += delta;
+            if (delta > Mx) { Mx = delta; kmax = k; }
+            R += clamped_ratio<REF_MODE>(delta, xp[k], p.C);     // reference image x^(s+1)
+            dp[k] = d;
+            xp[k] = v[e];
+          }
+        }
+        // ---- warp reduction: exact max + first position by redux, the two sums by one butterfly ----
+        const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
+        const unsigned tmax = __reduce_max_sync(0xffffffffu, mbits);
+        const int mypos = (lrow + 4 * (kmax >> 2)) * kFastTile + lcol + (kmax & 3);
+        const unsigned tpos = __reduce_min_sync(0xffffffffu, mbits == tmax ? (unsigned)mypos : 0x7fffffffu);
+        const bool hi = lane & 16;
+        float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, 16);
+        vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
+        vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
+        vsum += __shfl_xor_sync(0xffffffffu, vsum, 2);
+        vsum += __shfl_xor_sync(0xffffffffu, vsum, 1);
+        const float rsum = __shfl_sync(0xffffffffu, vsum, 16);  // lanes 0-15 hold sum S, 16-31 sum R
+        if (lane == 0) {
+          const int u = c.u0 + step - 2;
+          RawTile o;
+          o.sumD = vsum;
+          o.maxD = __uint_as_float(tmax);
+          o.sumR = rsum;
+          o.pos = (int32_t)tpos;
+          *reinterpret_cast<float4*>(&p.raw[((size_t)u * p.Ty + ty) * p.Tx + c.tx]) = *reinterpret_cast<float4*>(&o);
+        }
+      }
+    }
+  }
+  // ---- global maximum (a5): zero-filled out-of-bounds pixels are harmless because M >= C > 0 ----
+  const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
+  if (lane == 0 && warp_global < p.nitems) atomicMax(p.gmax_key, key);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Generic path: any tile size, any width / alignment.  G (power of two <= 32) lanes share one tile.
+// ---------------------------------------------------------------------------------------------
+struct GenericParams {
+  const float* base;        // first snapshot of this launch's rows
+  long long snap_stride;    // elements between consecutive snapshots
+  int rows;                 // image rows covered by this launch (strip height, or H)
+  int W;
+  int tile;
+  RawTile* raw;
+  int Tx, Ty, ty_base, rows_tiles, U;
+  int G;                    // lanes per tile
+  float C;
+};
+
+template <int REF_MODE>
+__global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams p) {
+  const int lane = threadIdx.x & 31;
+  const int gl = lane & (p.G - 1);
+  const long long group = ((long long)blockIdx.x * blockDim.x + threadIdx.x) / p.G;
+  const long long per_unit = (long long)p.rows_tiles * p.Tx;
+  const long long nitems = per_unit * p.U;
+  const bool live = group < nitems;
+  float S = 0.f, R = 0.f, Mx = 0.f;
+  int pos = 0x7fffffff;
+  int u = 0, ty_local = 0, tx = 0;
+  if (live) {
+    u = (int)(group / per_unit);
+    const long long t = group - (long long)u * per_unit;
+    ty_local = (int)(t / p.Tx);
+    tx = (int)(t - (long long)ty_local * p.Tx);
+    const int r0 = ty_local * p.tile, c0 = tx * p.tile;
+    const int h = min(p.tile, p.rows - r0), w = min(p.tile, p.W - c0);
+    const float* x0 = p.base + (long long)u * p.snap_stride;
+    const float* x1 = x0 + p.snap_stride;
+    const float* x2 = x1 + p.snap_stride;
+    bool first = true;
+    for (int i = gl; i < h * w; i += p.G) {
+      const int r = i / w, c = i - r * w;
+      const long long o = (long long)(r0 + r) * p.W + (c0 + c);
+      const float a = x0[o], b = x1[o], cc = x2[o];
+      const float delta = fabsf(fabsf(b - a) - fabsf(cc - b));
+      S += delta;
+      if (first || delta > Mx) { Mx = delta; pos = r * p.tile + c; first = false; }
+      R += clamped_ratio<REF_MODE>(delta, b, p.C);
+    }
+  }
+  for (int off = p.G >> 1; off > 0; off >>= 1) {
+    S += __shfl_xor_sync(0xffffffffu, S, off);
+    R += __shfl_xor_sync(0xffffffffu, R, off);
+    const float om = __shfl_xor_sync(0xffffffffu, Mx, off);
+    const int op = __shfl_xor_sync(0xffffffffu, pos, off);
+    if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
+  }
+  if (live && gl == 0) {
+    RawTile o;
+    o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
+    p.raw[((size_t)u * p.Ty + (p.ty_base + ty_local)) * p.Tx + tx] = o;
+  }
+}
+
+// Global maximum over n floats (generic path; the fused path folds this into its single pass).
+__global__ void __launch_bounds__(256) stack_max_kernel(const float* __restrict__ x, long long n, unsigned* gmax_key) {
+  float m = -3.402823466e38f;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) m = fmaxf(m, x[i]);
+  const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(m));
+  if ((threadIdx.x & 31) == 0) atomicMax(gmax_key, key);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Block-level helpers for the statistics (fp64, deterministic order)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum(double v, double* sh /*[32]*/) {
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if (lane == 0) sh[warp] = v;
+  __syncthreads();
+  double t = 0.0;
+  for (int i = 0; i < nw; ++i) t += sh[i];  // same order in every thread
+  return t;
+}
+
+struct StatPartial {
+  double n, mean, m2;
+};
+
+// Mean and population standard deviation of v[row][0..n) from per-block (n, mean, M2) partials that
+// are merged in block order with Chan's update -- a two-pass variance per block, deterministic.
+// The last block of each row to finish does the merge (threadfence + counter).
+__device__ __forceinline__ void row_stats_block(const float* v, long long begin, long long end, int row, int nblk,
+                                                StatPartial* parts, unsigned* counters, double* mu, double* sigma,
+                                                double* sh) {
+  double s = 0.0;
+  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) s += (double)v[i];
+  const double cnt = (double)(end - begin);
+  const double mean_b = block_sum(s, sh) / (cnt > 0 ? cnt : 1.0);
+  double s2 = 0.0;
+  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) {
+    const double d = (double)v[i] - mean_b;
+    s2 += d * d;
+  }
+  const double m2_b = block_sum(s2, sh);
+  __shared__ bool is_last;
+  if (threadIdx.x == 0) {
+    StatPartial sp;
+    sp.n = cnt; sp.mean = mean_b; sp.m2 = m2_b;
+    parts[(size_t)row * nblk + blockIdx.x] = sp;
+    __threadfence();
+    const unsigned done = atomicAdd(&counters[row], 1u);
+    is_last = (done == (unsigned)nblk - 1);
+  }
+  __syncthreads();
+  if (is_last && threadIdx.x == 0) {
+    __threadfence();
+    double n = 0.0, mean = 0.0, m2 = 0.0;
+    for (int b = 0; b < nblk; ++b) {
+      const volatile StatPartial* sp = &parts[(size_t)row * nblk + b];
+      const double nb = sp->n, mb = sp->mean, m2b = sp->m2;
+      if (nb <= 0) continue;
+      const double tot = n + nb, dlt = mb - mean;
+      mean += dlt * (nb / tot);
+      m2 += m2b + dlt * dlt * (n * nb / tot);
+      n = tot;
+    }
+    mu[row] = mean;
+    sigma[row] = (n > 0) ? sqrt(m2 / n) : 0.0;
+    counters[row] = 0;  // ready for the next call
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// finalize: q, tLISI, per-unit statistics (a6, a7)
+// ---------------------------------------------------------------------------------------------
+struct FinalizeParams {
+  const RawTile* raw;
+  float* q;            // [U][Ty][Tx]
+  float* tlisi;        // context copy, [U][Ty][Tx]
+  float* tlisi_user;   // caller's device buffer or NULL
+  const unsigned* gmax_key;
+  float* M_out;        // device scalar: the M that was used
+  float M_override;
+  float C;
+  int H, W, tile, Ty, Tx, U;
+  int nblk;            // blocks per unit
+  StatPartial* parts;  // [U][nblk]
+  unsigned* counters;  // [U]
+  double* mu;          // [U]
+  double* sigma;       // [U]
+};
+
+__global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
+  __shared__ double sh[32];
+  const int u = blockIdx.y;
+  const long long nt = (long long)p.Ty * p.Tx;
+  const long long per = (nt + p.nblk - 1) / p.nblk;
+  const long long begin = min(nt, (long long)blockIdx.x * per), end = min(nt, begin + per);
+  // M = max(max_s x^(s), C), PAPER.md:223 (R2: signed max), or the caller's override
+  float M = fmaxf(key_to_float(*p.gmax_key), p.C);
+  if (p.M_override > 0.f) M = p.M_override;
+  if (blockIdx.x == 0 && u == 0 && threadIdx.x == 0) *p.M_out = M;
+  const double inv_m2 = 1.0 / ((double)M * (double)M);
+  const size_t base = (size_t)u * nt;
+  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
+    const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
+    const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
+    const double n_t = (double)h * (double)w;  // R5: partial tiles use their own pixel count
+    const RawTile r = p.raw[base + t];
+    // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2
+    const double qd = ((double)r.sumD / n_t) * (double)r.maxD * ((double)r.sumR / n_t) * inv_m2;
+    const float qf = (float)qd;
+    p.q[base + t] = qf;
+    const float tl = (float)(1.0 - qd);
+    p.tlisi[base + t] = tl;
+    if (p.tlisi_user) p.tlisi_user[base + t] = tl;
+  }
+  __syncthreads();  // this block's q values are re-read below (by the same threads, but keep it simple)
+  row_stats_block(p.q + base, begin, end, u, p.nblk, p.parts, p.counters, p.mu, p.sigma, sh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// spectrum: per-tile temporal DFT (a10), Eq. 10 with h = max magnitude
+// ---------------------------------------------------------------------------------------------
+struct SpectrumParams {
+  const float* q;       // [U][nt]
+  const float2* tw;     // [U] twiddles (cos, -sin)(2 pi j / U)
+  float* eta;           // [nt]
+  int* kstar;           // [nt]
+  long long nt;
+  int U;
+  int nblk;
+  StatPartial* parts;   // [nblk]
+  unsigned* counters;   // [1]
+  double* mu;           // [1]
+  double* sigma;        // [1]
+};
+
+__global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
+  __shared__ double sh[32];
+  extern __shared__ float2 tws[];  // U twiddles
+  for (int i = threadIdx.x; i < p.U; i += blockDim.x) tws[i] = p.tw[i];
+  __syncthreads();
+  const long long per = (p.nt + p.nblk - 1) / p.nblk;
+  const long long begin = min(p.nt, (long long)blockIdx.x * per), end = min(p.nt, begin + per);
+  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
+    float mean = 0.f;
+    for (int u = 0; u < p.U; ++u) mean += p.q[(size_t)u * p.nt + t];
+    mean /= (float)p.U;  // DC removed
+    float best = 0.f;
+    int kb = (p.U / 2 >= 1) ? 1 : 0;
+    for (int k = 1; k <= p.U / 2; ++k) {
+      float re = 0.f, im = 0.f;
+      int j = 0;  // (k * u) mod U
+      for (int u = 0; u < p.U; ++u) {
+        const float a = p.q[(size_t)u * p.nt + t] - mean;
+        const float2 w = tws[j];
+        re = fmaf(a, w.x, re);
+        im = fmaf(a, w.y, im);
+        j += k;
+        if (j >= p.U) j -= p.U;
+      }
+      const float mag = sqrtf(re * re + im * im);
+      if (k == 1 || mag > best) { best = mag; kb = k; }
+    }
+    p.eta[t] = best;
+    p.kstar[t] = kb;
+  }
+  __syncthreads();
+  row_stats_block(p.eta, begin, end, 0, p.nblk, p.parts, p.counters, p.mu, p.sigma, sh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// compact: z-score, strict threshold, ordered compaction (a8).  Cooperative launch: every block
+// counts the candidates of its contiguous segment, grid sync, then writes them at the exclusive
+// prefix of the lower blocks' counts, in (row, tile) order: warp ballot + popc inside a warp,
+// a 32-entry scan across the warps of a block.
+// ---------------------------------------------------------------------------------------------
+struct CompactParams {
+  const float* v;       // q [U][nt] (image branch) or eta [1][nt] (frequency branch)
+  const RawTile* raw;   // image branch: argmax positions
+  const int* kstar;     // frequency branch
+  const double* mu;     // [rows]
+  const double* sigma;  // [rows]
+  float tau;
+  int rows;             // U or 1
+  long long nt;         // tiles per row
+  int Tx, Ty, H, W, tile, branch;
+  fitrig_candidate* out;
+  long long cap;        // device capacity of `out`
+  unsigned long long* total;
+  unsigned* blk_counts; // [gridDim.x]
+  long long seg;        // entries per block (multiple of blockDim.x)
+};
+
+__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float* z_out) {
+  const int row = (int)(i / p.nt);
+  const double sd = p.sigma[row];
+  const double z = (sd > 0.0) ? ((double)p.v[i] - p.mu[row]) / sd : 0.0;  // Eq. 8 on q (R21); R4
+  *z_out = (float)z;
+  return (float)z > p.tau;  // strict, R6
+}
+
+__global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
+  cg::grid_group grid = cg::this_grid();
+  __shared__ unsigned warp_cnt[32];
+  __shared__ unsigned long long block_base;
+  const long long N = (long long)p.rows * p.nt;
+  const long long begin = min(N, (long long)blockIdx.x * p.seg), end = min(N, begin + p.seg);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  // ---- pass 1: count ----
+  unsigned cnt = 0;
+  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) {
+    float z;
+    cnt += compact_flag(p, i, &z) ? 1u : 0u;
+  }
+  cnt = __reduce_add_sync(0xffffffffu, cnt);
+  if (lane == 0) warp_cnt[warp] = cnt;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned t = 0;
+    for (int w = 0; w < nw; ++w) t += warp_cnt[w];
+    p.blk_counts[blockIdx.x] = t;
+  }
+  grid.sync();
+  // ---- exclusive prefix over lower blocks (integer adds: order free) ----
+  if (threadIdx.x == 0) block_base = 0;
+  __syncthreads();
+  unsigned long long below = 0;
+  for (int b = threadIdx.x; b < (int)blockIdx.x; b += blockDim.x) below += p.blk_counts[b];
+  for (int off = 16; off > 0; off >>= 1) below += __shfl_xor_sync(0xffffffffu, below, off);
+  if (lane == 0 && below) atomicAdd(&block_base, below);
+  __syncthreads();
+  if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) *p.total = block_base + p.blk_counts[blockIdx.x];
+  unsigned long long running = block_base;
+  // ---- pass 2: write in order, one blockDim.x-wide chunk at a time ----
+  for (long long c0 = begin; c0 < end; c0 += blockDim.x) {
+    const long long i = c0 + threadIdx.x;
+    float z = 0.f;
+    const bool f = (i < end) && compact_flag(p, i, &z);
+    const unsigned bal = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) warp_cnt[warp] = __popc(bal);
+    __syncthreads();
+    unsigned before = 0, chunk_total = 0;
+    for (int w = 0; w < nw; ++w) {
+      const unsigned cw = warp_cnt[w];
+      if (w < warp) before += cw;
+      chunk_total += cw;
+    }
+    if (f) {
+      const unsigned long long dst = running + before + __popc(bal & ((1u << lane) - 1u));
+      if ((long long)dst < p.cap) {
+        const int row = (int)(i / p.nt);
+        const long long t = i - (long long)row * p.nt;
+        const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
+        fitrig_candidate cd;
+        if (p.branch == FITRIG_BRANCH_IMAGE) {
+          const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
+          cd.x = tx * p.tile + pos % p.tile;
+          cd.y = ty * p.tile + pos / p.tile;
+          cd.snapshot = row;
+        } else {
+          const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
+          cd.x = tx * p.tile + w / 2;  // tile centre (R18)
+          cd.y = ty * p.tile + h / 2;
+          cd.snapshot = p.kstar[t];
+        }
+        cd.score = z;
+        p.out[dst] = cd;
+      }
+    }
+    running += chunk_total;
+    __syncthreads();
+  }
+}
+
+}  // namespace fitrig

@@ -1,0 +1,70 @@
+"""CPU tier: the C-ABI library loads without a GPU and exports every symbol include/fitrig.h declares;
+host-only entry points (plan query, argument validation) behave as the header says."""
+import ctypes
+
+import pytest
+
+import paper_2509_21754_b200 as fitrig
+from paper_2509_21754_b200 import binding
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    L = fitrig.load_library()
+    names = fitrig.exported_symbols()
+    assert {"fitrig_create", "fitrig_tlisi", "fitrig_detect", "fitrig_stream"} <= set(names)
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/fitrig.h but not exported"
+    assert fitrig.version().startswith("fitrig-b200")
+    assert isinstance(fitrig.last_error(), str)
+
+
+def test_struct_layouts_match_header():
+    assert ctypes.sizeof(binding._Candidate) == 16  # "16 bytes" in fitrig.h
+    assert ctypes.sizeof(binding._Params) == 64
+    assert binding.CANDIDATE_DTYPE.itemsize == 16
+
+
+def test_plan_query_tile_grid_and_partial_tiles():
+    p = fitrig.plan_query(50000, 50000, 4)
+    assert (p.units, p.Ty, p.Tx) == (2, 1563, 1563)  # ceil(50000/32), R5
+    assert p.path == 0 and p.strip_rows % 32 == 0 and p.n_strips * p.strip_rows >= 50000
+    p = fitrig.plan_query(250, 250, 8, tile=8)
+    assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 1)  # generic kernel for N_T != 32
+    p = fitrig.plan_query(256, 250, 8)
+    assert p.path == 1  # W % 4 != 0: rows are not 16-byte aligned, no TMA
+    p = fitrig.plan_query(256, 252, 8)
+    assert p.path == 0 and p.Tx == 8
+
+
+def test_plan_query_fits_slots_to_the_tile_count():
+    # 4096 tiles on 148 SMs: 14 warps/CTA gives 2 x 2072 slots (two full rounds) instead of 1.73 rounds at 16
+    p = fitrig.plan_query(2048, 2048, 64, num_sms=148)
+    assert p.time_chunks == 1 and p.warps_per_cta == 14 and p.grid == 148
+    assert p.smem_bytes <= 227 * 1024 and p.stages >= 3
+    # tiny problem: split time so that the GPU is not left to 64 warps
+    p = fitrig.plan_query(256, 256, 8, num_sms=148)
+    assert p.time_chunks > 1 and p.time_chunks * p.units_per_chunk >= 6
+
+
+@pytest.mark.parametrize("H,W,L,kw", [
+    (0, 16, 3, {}), (16, 0, 3, {}), (16, 16, 2, {}),  # R10: L < 3
+    (16, 16, 3, {"tile": -1}), (16, 16, 3, {"ref_mode": 7}), (16, 16, 3, {"branch": 2}),
+    (64, 64, 3, {"tile": 32, "strip_rows": 48}),  # not a multiple of tile
+    (16, 16, 3, {"C": 1e-35}),
+])
+def test_invalid_arguments_are_rejected_before_any_cuda_call(H, W, L, kw):
+    with pytest.raises(fitrig.FitrigError) as e:
+        fitrig.plan_query(H, W, L, **kw)
+    assert e.value.code == binding.ERR_INVALID_ARG
+    with pytest.raises(fitrig.FitrigError) as e:
+        fitrig.Context(H, W, L, **kw)
+    assert e.value.code == binding.ERR_INVALID_ARG
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(fitrig.FitrigError) as e:
+        fitrig.Context(64, 64, 4)
+    assert e.value.code == binding.ERR_CUDA  # fails loudly; nothing routes to the oracle

@@ -111,16 +111,59 @@ def expected_active_units(active, L: int):
     return out
 
 
+def _tile_reduce(a: np.ndarray, tile: int, op):
+    """[H, W] -> [Ty, Tx] with zero padding (only used for non-negative quantities)."""
+    H, W = a.shape
+    Ty, Tx = -(-H // tile), -(-W // tile)
+    p = np.zeros((Ty * tile, Tx * tile), dtype=np.float64)
+    p[:H, :W] = a
+    return op(op(p.reshape(Ty, tile, Tx, tile), axis=3), axis=1)
+
+
+def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0):
+    """First-order bound on what fp32 evaluation of Eq. 3-5 can differ from exact arithmetic, per tile.
+
+    fl(b-a) = (b-a)(1+d), |d| <= 2^-24, three times: |Delta_fp32 - Delta| <= 2^-24 (D1 + D2 + Delta); a factor 2
+    is added for the neglected second-order terms.  For r = min(Delta / x_hat, 1): the same error divided by
+    |x_hat| (capped at 1) plus 2^-21 r for the approximate reciprocal and the multiply.
+    Returns (eS, eM, eR), each [U, Ty, Tx]: slack of sum Delta, max Delta, sum r.
+    """
+    L = stack.shape[0]
+    eS, eM, eR = [], [], []
+    x = stack.astype(np.float64)
+    for u in range(L - 2):
+        D1, D2 = np.abs(x[u + 1] - x[u]), np.abs(x[u + 2] - x[u + 1])
+        dl = np.abs(D1 - D2)
+        e = 2.0 ** -23 * (D1 + D2 + dl)
+        b = x[u + 1]
+        if ref_mode == 0:
+            xh = np.where(b == 0, C, np.abs(b))
+        elif ref_mode == 1:
+            xh = np.abs(np.where(b == 0, C, b))
+        else:
+            xh = np.maximum(b, C)
+        r = np.minimum(dl / xh, 1.0)
+        er = np.minimum(e / xh, 1.0) + 2.0 ** -21 * np.abs(r)
+        eS.append(_tile_reduce(e, tile, np.sum))
+        eM.append(_tile_reduce(e, tile, np.max))
+        eR.append(_tile_reduce(er, tile, np.sum))
+    return np.stack(eS), np.stack(eM), np.stack(eR)
+
+
 # ----- comparison rules of SURVEY.md R21/R22 (used by the GPU parity tests) -----
 Q_RTOL = 1e-4
 
 
-def assert_map_close(q_gpu, q_ref, tl_gpu=None, tl_ref=None, rtol=Q_RTOL):
+def assert_map_close(q_gpu, q_ref, tl_gpu=None, tl_ref=None, rtol=Q_RTOL, slack=None):
+    """|q_gpu - q_ref| <= rtol |q_ref| (+ `slack`, the derived fp32 input-rounding bound, for tiles so small
+    that |D^(s) - D^(s+1)| is dominated by cancellation, e.g. N_T = 1)."""
     q_gpu = np.asarray(q_gpu, dtype=np.float64)
     q_ref = np.asarray(q_ref, dtype=np.float64)
     assert q_gpu.shape == q_ref.shape, (q_gpu.shape, q_ref.shape)
     err = np.abs(q_gpu - q_ref)
     bound = rtol * np.abs(q_ref) + 1e-30
+    if slack is not None:
+        bound = bound + slack
     bad = err > bound
     assert not bad.any(), (f"{int(bad.sum())} of {bad.size} q values outside rtol={rtol}; worst rel "
                            f"{float((err / (np.abs(q_ref) + 1e-300)).max()):.3e}")
