@@ -79,8 +79,8 @@ typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
   int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, W % 4 == 0)         */
                              /* 1: generic kernel (any N_T, any W)                               */
-  int32_t time_chunks;       /* K: each tile's L snapshots are split into K chunks (+2 halo)     */
-  int32_t units_per_chunk;   /*                                                                  */
+  int32_t units_per_warp;    /* fused path: (tile, unit) pairs per warp, ceil(tiles * U / warps) */
+  int32_t reserved0;
   int32_t warps_per_cta;     /* fused path: one persistent CTA per SM, this many warps           */
   int32_t stages;            /* fused path: depth of each warp's TMA ring                        */
   int32_t grid;              /* CTAs launched                                                    */

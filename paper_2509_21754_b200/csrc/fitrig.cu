@@ -163,7 +163,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   c->Ty = c->plan.Ty; c->Tx = c->plan.Tx;
   c->nt = (long long)c->Ty * c->Tx;
   c->nmap = c->nt * c->U;
-  if (c->nmap * (long long)std::max(1, c->plan.time_chunks) > 0x7fffffffll) {
+  if (c->nmap > 0x7fffffffll) {
     delete c;
     return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: map of %lld entries is too large", c->nmap);
   }
@@ -306,9 +306,9 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
     fp.raw = c->raw; fp.gmax_key = c->gmax_key;
+    fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
-    fp.U = c->U; fp.K = pl.time_chunks; fp.cu = pl.units_per_chunk;
-    fp.nitems = rows_tiles * c->Tx * pl.time_chunks;
+    fp.U = c->U; fp.G = rows_tiles * c->Tx * c->U;
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     cudaError_t e;

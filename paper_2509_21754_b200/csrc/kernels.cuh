@@ -117,46 +117,130 @@ __device__ __forceinline__ float clamped_ratio(float delta, float ref, float C) 
 // Fused time-marching tLISI kernel (N_T = 32)
 // ---------------------------------------------------------------------------------------------
 struct FusedParams {
-  RawTile* raw;        // [U][Ty][Tx] whole map
-  unsigned* gmax_key;  // ordered key of the running global maximum (atomicMax)
-  int Tx, Ty;          // whole-map tile grid
-  int rows_tiles;      // tile rows covered by this launch (whole image, or one strip)
-  int ty_base;         // first tile row of this launch inside the whole map
-  int U;               // units = L - 2
-  int K;               // time chunks
-  int cu;              // units per chunk
-  int nitems;          // rows_tiles * Tx * K
+  RawTile* raw;          // [U][Ty][Tx] whole map
+  unsigned* gmax_key;    // ordered key of the running global maximum (atomicMax)
+  const float* base;     // snapshot 0 of this launch's rows (the memory the TMA descriptor covers)
+  long long snap_stride; // elements between consecutive snapshots
+  int W;                 // image width (row pitch in elements)
+  int Tx, Ty;            // whole-map tile grid
+  int rows_tiles;        // tile rows covered by this launch (whole image, or one strip)
+  int ty_base;           // first tile row of this launch inside the whole map
+  int U;                 // units = L - 2
+  int G;                 // rows_tiles * Tx * U: (tile, unit) pairs of this launch, tile-major
   float C;
 };
 
-struct ItemCoord {
-  int tx, ty_local, u0, nsteps;
+// Work distribution: the G (tile, unit) pairs of a launch, ordered tile-major / time-minor, are cut
+// into one contiguous range per warp (range w = [w*G/n, (w+1)*G/n)), so every warp carries the same
+// load whatever the tile count.  A range is walked as "segments": a run of consecutive units of one
+// tile, which costs its units + 2 snapshots to march through (the 2-snapshot halo is re-read only
+// where a cut falls inside a tile's time series: at most once per warp).
+struct Segment {
+  int tx, ty_local, u0, nsteps;  // tile, first unit, snapshots to load (= units + 2)
 };
 
-__device__ __forceinline__ ItemCoord decode_item(const FusedParams& p, int item) {
-  ItemCoord c;
-  const int per_chunk = p.rows_tiles * p.Tx;
-  const int k = item / per_chunk;
-  const int t = item - k * per_chunk;
-  c.ty_local = t / p.Tx;
-  c.tx = t - c.ty_local * p.Tx;
-  c.u0 = k * p.cu;
-  const int u1 = min(p.U, c.u0 + p.cu);
-  c.nsteps = u1 - c.u0 + 2;  // snapshots u0 .. u1+1
+__device__ __forceinline__ Segment decode_segment(const FusedParams& p, int g, int g_end) {
+  Segment c;
+  const int tile = g / p.U;
+  c.u0 = g - tile * p.U;
+  c.ty_local = tile / p.Tx;
+  c.tx = tile - c.ty_local * p.Tx;
+  c.nsteps = min(p.U - c.u0, g_end - g) + 2;
   return c;
 }
 
-// Lane l of the warp owns, in each 32x32 tile, columns 4*(l%8)..+3 of rows (l/8) + 4*j, j = 0..7:
-// a quarter warp reads one 128-byte tile row from shared memory (conflict free), and the 32 pixels
-// of a lane are visited in increasing row-major order (so a strict '>' keeps the first maximum).
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// One 32x32 tile from a ring slot into registers.  Lane l owns columns 4*(l%8)..+3 of rows
+// (l/8) + 4*j, j = 0..7: a quarter warp reads one 128-byte tile row (conflict free), and the 32
+// pixels of a lane are held in increasing row-major order.
+__device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* slot_ptr, int lane) {
+  const float4* src = reinterpret_cast<const float4*>(slot_ptr) + lane;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float4 t = src[j * 32];
+    N[4 * j] = t.x; N[4 * j + 1] = t.y; N[4 * j + 2] = t.z; N[4 * j + 3] = t.w;
+  }
+}
+
+// Running signed maximum (a5) and the smallest magnitude of a freshly loaded tile.  zmin == 0 tells
+// the NEXT step, whose reference image this tile is, that Eq. 5's "x == 0 -> C" case occurs.
+__device__ __forceinline__ void scan_tile(const float (&N)[32], float& gmax, float& zmin) {
+  float z = 3.402823466e38f;
+#pragma unroll
+  for (int k = 0; k < 32; ++k) {
+    gmax = fmaxf(gmax, N[k]);
+    z = fminf(z, fabsf(N[k]));
+  }
+  zmin = z;
+}
+
+// Steps a1-a4 for the 32 pixels of one lane: N = x^(s+2) (new), X = x^(s+1) (reference image,
+// PAPER.md:203), dp = signed x^(s+1) - x^(s).  Returns the lane's sum Delta, sum r, max Delta and the
+// index j (0..7) of the first 4-pixel group that attains it; dp becomes x^(s+2) - x^(s+1).
+//
+// REF_ABS: r = sat(Delta * rcp(|x|)).  rcp(0) = +inf, so a zero reference pixel yields 1 (Delta > 0)
+// or sat(NaN) = 0 (Delta == 0) instead of Eq. 5's min(Delta / C, 1); `zero_ref` (warp uniform, known
+// from scan_tile one step earlier) adds the difference first, so the per-pixel x == 0 test leaves
+// the hot loop.
+template <int REF_MODE>
+__device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)[32], float (&dp)[32], float C,
+                                          bool zero_ref, float& S, float& R, float& Mx, int& jmax) {
+  float S0 = 0.f, S1 = 0.f, R0 = 0.f, R1 = 0.f;
+  Mx = 0.f;
+  jmax = 0;
+  if (REF_MODE == FITRIG_REF_ABS && zero_ref) {
+    const float invC = rcp_approx(C);
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      if (X[k] == 0.f) {
+        const float delta = fabsf(fabsf(N[k] - X[k]) - fabsf(dp[k]));
+        R0 += __saturatef(delta * invC) - (delta > 0.f ? 1.f : 0.f);
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    float dl[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int k = 4 * j + e;
+      const float d = N[k] - X[k];                          // signed D^(s+1), Eq. 3
+      const float delta = fabsf(fabsf(d) - fabsf(dp[k]));   // |D^(s) - D^(s+1)|
+      dp[k] = d;
+      dl[e] = delta;
+      const float r = (REF_MODE == FITRIG_REF_ABS) ? __saturatef(delta * rcp_approx(fabsf(X[k])))
+                                                    : clamped_ratio<REF_MODE>(delta, X[k], C);
+      if (j & 1) { S1 += delta; R1 += r; } else { S0 += delta; R0 += r; }
+    }
+    const float g = fmaxf(fmaxf(dl[0], dl[1]), fmaxf(dl[2], dl[3]));
+    if (g > Mx) { Mx = g; jmax = j; }  // strict: keeps the first group in row-major order
+  }
+  S = S0 + S1;
+  R = R0 + R1;
+}
+
+// A warp owns one 32x32 tile and marches it through time; tiles arrive through a per-warp ring of
+// TMA boxes.  The two most recent snapshots live in registers (A/B ping-pong, no copies), so every
+// snapshot byte is read from HBM once.  The arg-max of Delta (R20) is tracked per 16-byte group in
+// the loop; which of its 4 pixels it was is found one step later from a 48-byte re-read (3 x
+// cp.async of data that was in flight moments ago) by lane 0, off the critical path.
 template <int REF_MODE, int NSTAGE>
 __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // the shuffle tells the compiler the warp index is warp uniform, so cursors and addresses derived
+  // from it live in uniform registers and the vector registers are left to the three tile arrays
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   const int nwarps = blockDim.x >> 5;
   unsigned char* ring = smem + (size_t)warp * NSTAGE * kTileBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)nwarps * NSTAGE * kTileBytes) + warp * NSTAGE;
+  unsigned char* after_ring = smem + (size_t)nwarps * NSTAGE * kTileBytes;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(after_ring) + warp * NSTAGE;
+  float4* scratch = reinterpret_cast<float4*>(after_ring + (((size_t)nwarps * NSTAGE * 8 + 15) & ~(size_t)15)) + warp * kScratchVec;
 
   if (lane == 0) {
 #pragma unroll
@@ -171,12 +255,17 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
   const uint64_t policy = l2_evict_first_policy();
   const uint32_t ring_addr = smem_u32(ring);
   const uint32_t bar_addr = smem_u32(bars);
+  const uint32_t scratch_addr = smem_u32(scratch);
+
+  // this warp's range of (tile, unit) pairs
+  const int g_begin = (int)((long long)warp_global * p.G / total_warps);
+  const int g_end = (int)((long long)(warp_global + 1) * p.G / total_warps);
 
   // ---- producer cursor (lane 0 issues; all lanes track it, it is warp uniform) ----
-  int p_item = warp_global, p_step = 0;
-  ItemCoord pc = decode_item(p, p_item < p.nitems ? p_item : 0);
+  int p_g = g_begin, p_step = 0;
+  Segment pc = decode_segment(p, p_g < g_end ? p_g : 0, g_end);
   auto issue_next = [&](int slot) {
-    if (p_item < p.nitems) {
+    if (p_g < g_end) {
       if (lane == 0) {
         const uint32_t bar = bar_addr + slot * 8;
         mbar_arrive_expect_tx(bar, kTileBytes);
@@ -185,93 +274,107 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
       }
       if (++p_step == pc.nsteps) {
         p_step = 0;
-        p_item += total_warps;
-        if (p_item < p.nitems) pc = decode_item(p, p_item);
+        p_g += pc.nsteps - 2;
+        if (p_g < g_end) pc = decode_segment(p, p_g, g_end);
       }
     }
   };
 #pragma unroll
   for (int i = 0; i < NSTAGE; ++i) issue_next(i);
 
-  float xp[32], dp[32];  // x_{s-1} and the signed difference x_{s-1} - x_{s-2} of this lane's pixels
-  float gmax = -3.402823466e38f;
+  float A[32], B[32], dp[32];
+  float gmax = -3.402823466e38f, zA = 1.f, zB = 1.f;
   int slot = 0;
   uint32_t phase = 0;
   const int lrow = lane >> 3, lcol = (lane & 7) * 4;
 
-  for (int item = warp_global; item < p.nitems; item += total_warps) {
-    const ItemCoord c = decode_item(p, item);
-    const int ty = p.ty_base + c.ty_local;
-    for (int step = 0; step < c.nsteps; ++step) {
-      mbar_wait(bar_addr + slot * 8, phase);
-      float4 cur[8];
-      const float4* src = reinterpret_cast<const float4*>(ring + (size_t)slot * kTileBytes) + lane;
-#pragma unroll
-      for (int j = 0; j < 8; ++j) cur[j] = src[j * 32];  // row (lane/8)+4j, 16-byte column group lane%8
-      __syncwarp();        // every lane has its copy: the slot may be refilled
-      issue_next(slot);    // prefetch NSTAGE steps ahead
-      if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+  // next snapshot of the current item: ring slot -> registers, then refill the slot NSTAGE steps ahead
+  auto acquire = [&](float (&N)[32], float& zmin) {
+    mbar_wait(bar_addr + slot * 8, phase);
+    load_tile(N, ring + (size_t)slot * kTileBytes, lane);
+    __syncwarp();  // every lane has its copy: the slot may be refilled
+    issue_next(slot);
+    if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+    scan_tile(N, gmax, zmin);
+  };
 
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        gmax = fmaxf(gmax, fmaxf(fmaxf(cur[j].x, cur[j].y), fmaxf(cur[j].z, cur[j].w)));
-      }
+  // ---- one record is always "pending": its arg-max group is known, the pixel inside it is not.
+  // Lane 0 parks it in the warp's scratch (registers are for the tile arrays): scratch[0..2] the
+  // re-read pixels, scratch[3] = {sum Delta, sum r, max bits, group position}, scratch[4] = map index.
+  bool pend = false;
+  auto resolve_pending = [&]() {  // lane 0 only
+    cp_async_wait_all();
+    const float4 a = scratch[0], b = scratch[1], c = scratch[2], rec = scratch[3];
+    const unsigned long long idx = *reinterpret_cast<const unsigned long long*>(&scratch[4]);
+    const float mx = rec.z;
+    // the same three fp32 operations as tile_step -> bit-identical Delta
+    const float e0 = fabsf(fabsf(c.x - b.x) - fabsf(b.x - a.x));
+    const float e1 = fabsf(fabsf(c.y - b.y) - fabsf(b.y - a.y));
+    const float e2 = fabsf(fabsf(c.z - b.z) - fabsf(b.z - a.z));
+    const int e = (e0 == mx) ? 0 : (e1 == mx) ? 1 : (e2 == mx) ? 2 : 3;
+    RawTile o;
+    o.sumD = rec.x;
+    o.maxD = mx;
+    o.sumR = rec.y;
+    o.pos = __float_as_int(rec.w) + e;
+    *reinterpret_cast<float4*>(&p.raw[idx]) = *reinterpret_cast<float4*>(&o);
+  };
 
-      if (step == 0) {
+  // warp reduction of one (tile, unit): exact max + first group by redux, the two sums by one butterfly
+  auto finish = [&](const Segment& c, int step, float S, float R, float Mx, int jmax) {
+    const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
+    const unsigned tmax = __reduce_max_sync(0xffffffffu, mbits);
+    const int gpos = (lrow + 4 * jmax) * kFastTile + lcol;
+    const unsigned tg = __reduce_min_sync(0xffffffffu, mbits == tmax ? (unsigned)gpos : 0x7fffffffu);
+    const bool hi = lane & 16;
+    float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, 16);
+    vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
+    vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
+    vsum += __shfl_xor_sync(0xffffffffu, vsum, 2);
+    vsum += __shfl_xor_sync(0xffffffffu, vsum, 1);
+    const float rsum = __shfl_sync(0xffffffffu, vsum, 16);  // lanes 0-15 hold sum S, 16-31 sum R
+    if (lane == 0) {
+      if (pend) resolve_pending();
+      const int u = c.u0 + step - 2;
+      scratch[3] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
+      *reinterpret_cast<unsigned long long*>(&scratch[4]) =
+          ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + c.tx;
+      // the winning group's 4 pixels in x_u, x_{u+1}, x_{u+2}: in bounds (a zero-filled pixel has Delta 0)
+      const float* src = p.base + (long long)u * p.snap_stride +
+                         (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (c.tx * kFastTile + (int)(tg & 31));
+      cp_async16(scratch_addr, src);
+      cp_async16(scratch_addr + 16, src + p.snap_stride);
+      cp_async16(scratch_addr + 32, src + 2 * p.snap_stride);
+      cp_async_commit();
+    }
+    pend = true;
+  };
+
+  for (int g = g_begin; g < g_end;) {
+    const Segment c = decode_segment(p, g, g_end);
+    g += c.nsteps - 2;
+    acquire(A, zA);  // x_{u0}
+    acquire(B, zB);  // x_{u0+1}
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { xp[4 * j] = cur[j].x; xp[4 * j + 1] = cur[j].y; xp[4 * j + 2] = cur[j].z; xp[4 * j + 3] = cur[j].w; }
-      } else if (step == 1) {
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const float v[4] = {cur[j].x, cur[j].y, cur[j].z, cur[j].w};
-#pragma unroll
-          for (int e = 0; e < 4; ++e) { dp[4 * j + e] = v[e] - xp[4 * j + e]; xp[4 * j + e] = v[e]; }
-        }
-      } else {
-        float S = 0.f, R = 0.f, Mx = 0.f;
-        int kmax = 0;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const float v[4] = {cur[j].x, cur[j].y, cur[j].z, cur[j].w};
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int k = 4 * j + e;
-            const float d = v[e] - xp[k];                       // D^(s+1) (signed), Eq. 3
-            const float delta = fabsf(fabsf(d) - fabsf(dp[k]));  // |D^(s) - D^(s+1)|
-            S += delta;
-            if (delta > Mx) { Mx = delta; kmax = k; }
-            R += clamped_ratio<REF_MODE>(delta, xp[k], p.C);     // reference image x^(s+1)
-            dp[k] = d;
-            xp[k] = v[e];
-          }
-        }
-        // ---- warp reduction: exact max + first position by redux, the two sums by one butterfly ----
-        const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
-        const unsigned tmax = __reduce_max_sync(0xffffffffu, mbits);
-        const int mypos = (lrow + 4 * (kmax >> 2)) * kFastTile + lcol + (kmax & 3);
-        const unsigned tpos = __reduce_min_sync(0xffffffffu, mbits == tmax ? (unsigned)mypos : 0x7fffffffu);
-        const bool hi = lane & 16;
-        float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, 16);
-        vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
-        vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
-        vsum += __shfl_xor_sync(0xffffffffu, vsum, 2);
-        vsum += __shfl_xor_sync(0xffffffffu, vsum, 1);
-        const float rsum = __shfl_sync(0xffffffffu, vsum, 16);  // lanes 0-15 hold sum S, 16-31 sum R
-        if (lane == 0) {
-          const int u = c.u0 + step - 2;
-          RawTile o;
-          o.sumD = vsum;
-          o.maxD = __uint_as_float(tmax);
-          o.sumR = rsum;
-          o.pos = (int32_t)tpos;
-          *reinterpret_cast<float4*>(&p.raw[((size_t)u * p.Ty + ty) * p.Tx + c.tx]) = *reinterpret_cast<float4*>(&o);
-        }
-      }
+    for (int k = 0; k < 32; ++k) dp[k] = B[k] - A[k];
+    int step = 2;
+    while (true) {
+      float S, R, Mx;
+      int jmax;
+      acquire(A, zA);
+      tile_step<REF_MODE>(A, B, dp, p.C, __any_sync(0xffffffffu, zB == 0.f), S, R, Mx, jmax);
+      finish(c, step, S, R, Mx, jmax);
+      if (++step >= c.nsteps) break;
+      acquire(B, zB);
+      tile_step<REF_MODE>(B, A, dp, p.C, __any_sync(0xffffffffu, zA == 0.f), S, R, Mx, jmax);
+      finish(c, step, S, R, Mx, jmax);
+      if (++step >= c.nsteps) break;
     }
   }
+  if (lane == 0 && pend) resolve_pending();
   // ---- global maximum (a5): zero-filled out-of-bounds pixels are harmless because M >= C > 0 ----
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
-  if (lane == 0 && warp_global < p.nitems) atomicMax(p.gmax_key, key);
+  if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
 }
 
 // ---------------------------------------------------------------------------------------------

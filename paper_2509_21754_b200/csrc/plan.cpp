@@ -41,18 +41,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
   return FITRIG_OK;
 }
 
-// Fused path cost model.  Work items are (tile, time chunk); a warp marches one item through its
-// ceil(U/K)+2 snapshots.  One persistent CTA per SM with w warps gives num_sms*w slots, and the
-// kernel is bandwidth bound, so a round of items costs ~ w * steps (bytes the slots could have
-// moved, busy or idle).  Minimising rounds*steps*w favours (K, w) whose slot count divides the item
-// count: e.g. 4096 tiles on 148 SMs -> w = 14 (2 x 2072 slots) instead of 16 (1.73 rounds).
+// Fused path: one persistent CTA per SM; each warp owns a contiguous range of the G = tiles * U
+// (tile, unit) pairs (see kernels.cuh), so the load is balanced for every tile count and only the
+// warp count, ring depth and grid are chosen here.  12 warps x 168 registers keep three 32-pixel
+// tile arrays per lane in registers without spills; 12 x 4 x 4 KB = 192 KB of TMA boxes in flight
+// per SM is several times the HBM latency-bandwidth product (~50 KB per SM).
 void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
   const bool force_generic = env_int("FITRIG_FORCE_GENERIC", 0) != 0;
   if (tile != kFastTile || (W % 4) != 0 || force_generic) {
     plan->path = 1;
-    plan->time_chunks = 1;
-    plan->units_per_chunk = U;
+    plan->units_per_warp = 0;
     plan->warps_per_cta = 8;
     plan->stages = 0;
     plan->smem_bytes = 0;
@@ -60,45 +59,26 @@ void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fit
     return;
   }
   plan->path = 0;
-  const long long tiles = (long long)tile_rows * Tx;
-  double best = 1e300;
-  int bK = 1, bw = kMaxWarpsPerCta, bs = 3;
-  const int maxK = std::min(U, 16);
-  for (int K = 1; K <= maxK; ++K) {
-    const int cu = (U + K - 1) / K;
-    const int Keff = (U + cu - 1) / cu;
-    if (Keff != K) continue;
-    const int steps = cu + 2;
-    for (int w = kMinWarpsPerCta; w <= kMaxWarpsPerCta; ++w) {
-      const long long slots = (long long)num_sms * w;
-      const long long items = tiles * K;
-      const long long rounds = (items + slots - 1) / slots;
-      // an SM needs ~6 warps of loads in flight to pull its share of HBM bandwidth; below that a
-      // round is latency bound and costs the same as with 6 (so under-filled GPUs prefer more chunks)
-      const double per_sm = (double)items / num_sms;
-      const double w_eff = std::max(6.0, std::min((double)w, per_sm));
-      // small penalties: each extra chunk re-reads 2 halo snapshots; prefer more warps on ties
-      double cost = (double)rounds * steps * w_eff * (1.0 + 1e-4 * K) + 1e-3 * (kMaxWarpsPerCta - w);
-      if (cost < best) { best = cost; bK = K; bw = w; }
-    }
-  }
-  const int fw = env_int("FITRIG_WARPS", 0), fk = env_int("FITRIG_CHUNKS", 0), fs = env_int("FITRIG_STAGES", 0);
-  if (fk > 0) bK = std::min(fk, U);
-  if (fw > 0) bw = std::max(1, std::min(fw, kMaxWarpsPerCta));
-  const int cu = (U + bK - 1) / bK;
-  bK = (U + cu - 1) / cu;
-  // deepest ring that fits: stages * warps * 4 KB (+ barriers) <= 227 KB, capped at 4
-  bs = std::min(4, (kMaxSmemPerCta - 1024) / (bw * kTileBytes));
-  if (fs > 0) bs = std::min(fs, (kMaxSmemPerCta - 1024) / (bw * kTileBytes));
+  const long long G = (long long)tile_rows * Tx * U;
+  int w = kMaxWarpsPerCta;
+  const int fw = env_int("FITRIG_WARPS", 0), fs = env_int("FITRIG_STAGES", 0), fg = env_int("FITRIG_GRID", 0);
+  if (fw > 0) w = std::max(1, std::min(fw, kMaxWarpsPerCta));
+  // small problems are latency bound: give every warp at least kMinUnitsPerWarp units, and spread the
+  // warps over as many SMs as possible
+  long long total = std::min<long long>((long long)num_sms * w, (G + kMinUnitsPerWarp - 1) / kMinUnitsPerWarp);
+  total = std::max<long long>(total, 1);
+  if (fw <= 0) w = (int)std::max<long long>(1, std::min<long long>(w, (total + num_sms - 1) / num_sms));
+  int grid = (int)std::min<long long>(num_sms, (total + w - 1) / w);
+  if (fg > 0) grid = fg;
+  // deepest ring that fits next to the mbarriers and the arg-max scratch, capped at 4
+  int bs = std::min(4, (kMaxSmemPerCta - 2048) / (w * kTileBytes));
+  if (fs > 0) bs = std::min(fs, (kMaxSmemPerCta - 2048) / (w * kTileBytes));
   bs = std::max(2, bs);
-  plan->time_chunks = bK;
-  plan->units_per_chunk = cu;
-  plan->warps_per_cta = bw;
+  plan->warps_per_cta = w;
   plan->stages = bs;
-  plan->smem_bytes = bw * bs * kTileBytes + bw * bs * 8;
-  const long long items = tiles * bK;
-  plan->grid = (int)std::min<long long>(num_sms, (items + bw - 1) / bw);
-  if (plan->grid < 1) plan->grid = 1;
+  plan->grid = std::max(1, grid);
+  plan->units_per_warp = (int32_t)((G + (long long)plan->grid * w - 1) / ((long long)plan->grid * w));
+  plan->smem_bytes = w * bs * kTileBytes + ((w * bs * 8 + 15) & ~15) + w * kScratchVec * 16;  // ring, mbarriers, scratch
 }
 
 }  // namespace fitrig

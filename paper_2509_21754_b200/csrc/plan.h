@@ -9,8 +9,9 @@ namespace fitrig {
 constexpr int kFastTile = 32;          // tile edge of the fused path (the paper's default)
 constexpr int kTileBytes = 32 * 32 * 4;  // one 32x32 fp32 tile = one TMA box
 constexpr int kMaxSmemPerCta = 227 * 1024;
-constexpr int kMaxWarpsPerCta = 16;    // 512 threads x 128 registers = the whole register file
-constexpr int kMinWarpsPerCta = 8;
+constexpr int kMaxWarpsPerCta = 12;    // 384 threads x 168 registers: A/B/dp tile arrays (96) + pipeline state, no spills
+constexpr int kMinUnitsPerWarp = 2;    // fused path: fewest (tile, unit) pairs worth a warp of its own
+constexpr int kScratchVec = 6;         // float4 per warp of arg-max scratch (fused kernel)
 
 struct NormParams {  // fitrig_params with defaults applied
   int tile;
@@ -25,10 +26,10 @@ struct NormParams {  // fitrig_params with defaults applied
 // Validates and applies defaults.  Returns FITRIG_OK or FITRIG_ERR_INVALID_ARG (+ message in *why).
 int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, NormParams* out, const char** why);
 
-// Chooses path, time chunking, warps per CTA and ring depth for `tile_rows` x Tx tiles of U units.
+// Chooses path, warps per CTA, ring depth and grid for `tile_rows` x Tx tiles of U units.
 void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan);
 
-// Debug/tuning overrides: FITRIG_WARPS, FITRIG_STAGES, FITRIG_CHUNKS, FITRIG_FORCE_GENERIC (integers).
+// Debug/tuning overrides: FITRIG_WARPS, FITRIG_STAGES, FITRIG_GRID, FITRIG_FORCE_GENERIC (integers).
 int env_int(const char* name, int dflt);
 
 }  // namespace fitrig

@@ -36,14 +36,17 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert p.path == 0 and p.Tx == 8
 
 
-def test_plan_query_fits_slots_to_the_tile_count():
-    # 4096 tiles on 148 SMs: 14 warps/CTA gives 2 x 2072 slots (two full rounds) instead of 1.73 rounds at 16
+def test_plan_query_balances_units_over_warps():
+    # 4096 tiles x 62 units on 148 SMs x 12 warps: every warp gets ceil(253952 / 1776) = 143 (tile, unit) pairs
     p = fitrig.plan_query(2048, 2048, 64, num_sms=148)
-    assert p.time_chunks == 1 and p.warps_per_cta == 14 and p.grid == 148
+    assert p.warps_per_cta == 12 and p.grid == 148 and p.units_per_warp == 143
     assert p.smem_bytes <= 227 * 1024 and p.stages >= 3
-    # tiny problem: split time so that the GPU is not left to 64 warps
+    # tiny problem (384 pairs): spread thin so that the GPU is not left to a few SMs
     p = fitrig.plan_query(256, 256, 8, num_sms=148)
-    assert p.time_chunks > 1 and p.time_chunks * p.units_per_chunk >= 6
+    assert p.grid * p.warps_per_cta >= 148 and p.units_per_warp >= 2
+    # one tile, one unit
+    p = fitrig.plan_query(32, 32, 3, num_sms=148)
+    assert p.grid == 1 and p.warps_per_cta == 1 and p.units_per_warp == 1
 
 
 @pytest.mark.parametrize("H,W,L,kw", [

@@ -173,17 +173,21 @@ def test_m_override_scales_q_but_not_candidates(tiny):
     assert [tuple(r)[:3] for r in g1["cands"][4.0][0]] == [tuple(r)[:3] for r in g2["cands"][4.0][0]]  # P7
 
 
-def test_time_chunking_gives_identical_maps(tiny, monkeypatch):
+def test_work_partition_does_not_change_the_map(tiny, monkeypatch):
+    """The per-warp ranges of (tile, unit) pairs cut tiles' time series at different places for different
+    warp counts / grids; the per-tile results must not depend on where the cuts fall."""
     st, _ = tiny
-    monkeypatch.setenv("FITRIG_CHUNKS", "1")
-    a = gpu_run(st)
-    monkeypatch.setenv("FITRIG_CHUNKS", "3")
-    monkeypatch.setenv("FITRIG_WARPS", "9")
-    monkeypatch.setenv("FITRIG_STAGES", "2")
-    b = gpu_run(st)
-    assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
-    for x, y in zip(a["raw"], b["raw"]):
-        assert np.array_equal(x, y)
+    monkeypatch.setenv("FITRIG_WARPS", "1")
+    monkeypatch.setenv("FITRIG_GRID", "1")
+    a = gpu_run(st)  # one warp walks all 384 pairs: no cut inside any tile
+    for warps, grid, stages in ((9, 7, 2), (12, 148, 4), (5, 13, 3)):
+        monkeypatch.setenv("FITRIG_WARPS", str(warps))
+        monkeypatch.setenv("FITRIG_GRID", str(grid))
+        monkeypatch.setenv("FITRIG_STAGES", str(stages))
+        b = gpu_run(st)
+        assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
+        for x, y in zip(a["raw"], b["raw"]):
+            assert np.array_equal(x, y)
 
 
 def test_fused_and_generic_kernels_agree(tiny, monkeypatch):
