@@ -344,7 +344,7 @@ def run_fitrig(args, cfg, tau, branch):
                        "candidates_per_step": int(n_found),
                        "l2": f"input {4 * pix / 1e6:.0f} MB per step vs 126 MB L2: "
                              + ("larger than L2, no flush" if 4 * pix > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
-                       "plan": {"path": "fused-tma" if plan.path == 0 else "generic", "units_per_warp": plan.units_per_warp,
+                       "plan": {"path": "fused-tma" if plan.path == 0 else "generic", "units_per_cta": plan.units_per_cta, "box_tiles": plan.box_tiles,
                                 "warps_per_cta": plan.warps_per_cta, "stages": plan.stages, "grid": plan.grid}},
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches) * world,
             "roofline": roofline, "cpu_baseline": cpu,

@@ -79,10 +79,10 @@ typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
   int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, W % 4 == 0)         */
                              /* 1: generic kernel (any N_T, any W)                               */
-  int32_t units_per_warp;    /* fused path: (tile, unit) pairs per warp, ceil(tiles * U / warps) */
-  int32_t reserved0;
-  int32_t warps_per_cta;     /* fused path: one persistent CTA per SM, this many warps           */
-  int32_t stages;            /* fused path: depth of each warp's TMA ring                        */
+  int32_t units_per_cta;     /* fused path: (box column, unit) pairs per CTA, ceil(boxes * U / grid) */
+  int32_t box_tiles;         /* fused path: adjacent tiles fetched as one TMA box (1..8)         */
+  int32_t warps_per_cta;     /* fused path: box_tiles consumer warps + 1 producer warp           */
+  int32_t stages;            /* fused path: depth of the CTA's ring of TMA boxes                 */
   int32_t grid;              /* CTAs launched                                                    */
   int32_t smem_bytes;        /* dynamic shared memory per CTA                                    */
   int32_t strip_rows;        /* fitrig_stream: rows per strip (multiple of N_T)                  */

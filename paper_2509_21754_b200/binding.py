@@ -36,7 +36,7 @@ class _Candidate(ctypes.Structure):
 
 class _Plan(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
-                ("units", "Ty", "Tx", "path", "units_per_warp", "reserved0", "warps_per_cta", "stages", "grid",
+                ("units", "Ty", "Tx", "path", "units_per_cta", "box_tiles", "warps_per_cta", "stages", "grid",
                  "smem_bytes", "strip_rows", "n_strips", "n_strip_buffers", "reserved")] + \
                [("strip_buffer_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64)]
 
@@ -58,7 +58,8 @@ class Plan:
     Ty: int
     Tx: int
     path: int
-    units_per_warp: int
+    units_per_cta: int
+    box_tiles: int
     warps_per_cta: int
     stages: int
     grid: int

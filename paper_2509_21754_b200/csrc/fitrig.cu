@@ -129,10 +129,9 @@ static void free_ctx(fitrig_ctx* c) {
   delete c;
 }
 
-template <int REF, int NS>
+template <int REF>
 static cudaError_t set_fused_attr() {
-  return cudaFuncSetAttribute(tlisi_fused_kernel<REF, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              kMaxSmemPerCta);
+  return cudaFuncSetAttribute(tlisi_fused_kernel<REF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta);
 }
 
 extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_params* params, fitrig_ctx** out) {
@@ -228,9 +227,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   CTX_TRY(cudaEventCreate(&c->ev_fin0));
   CTX_TRY(cudaEventCreate(&c->ev_fin1));
   if (c->plan.path == 0) {
-    CTX_TRY((set_fused_attr<0, 2>())); CTX_TRY((set_fused_attr<0, 3>())); CTX_TRY((set_fused_attr<0, 4>()));
-    CTX_TRY((set_fused_attr<1, 2>())); CTX_TRY((set_fused_attr<1, 3>())); CTX_TRY((set_fused_attr<1, 4>()));
-    CTX_TRY((set_fused_attr<2, 2>())); CTX_TRY((set_fused_attr<2, 3>())); CTX_TRY((set_fused_attr<2, 4>()));
+    CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
 #undef CTX_TRY
   *out = c;
@@ -270,17 +267,6 @@ static int prof_end(fitrig_ctx* c, cudaStream_t st) {
   return FITRIG_OK;
 }
 
-template <int REF>
-static cudaError_t launch_fused_stage(int stages, dim3 grid, dim3 block, size_t smem, cudaStream_t st,
-                                      const CUtensorMap& tm, const FusedParams& fp) {
-  switch (stages) {
-    case 2: tlisi_fused_kernel<REF, 2><<<grid, block, smem, st>>>(tm, fp); break;
-    case 3: tlisi_fused_kernel<REF, 3><<<grid, block, smem, st>>>(tm, fp); break;
-    default: tlisi_fused_kernel<REF, 4><<<grid, block, smem, st>>>(tm, fp); break;
-  }
-  return cudaGetLastError();
-}
-
 // tLISI partial sums of `rows` image rows (all L snapshots) that start at tile row ty_base.
 // base: device pointer to snapshot 0 of those rows; snap_stride: elements between snapshots.
 static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int ty_base,
@@ -298,7 +284,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     CUtensorMap tm;
     const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)c->L};
     const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
-    const cuuint32_t box[3] = {kFastTile, kFastTile, 1};
+    const cuuint32_t box[3] = {(cuuint32_t)(pl.box_tiles * kFastTile), kFastTile, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = c->encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, box, estr,
                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -308,16 +294,20 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.raw = c->raw; fp.gmax_key = c->gmax_key;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
-    fp.U = c->U; fp.G = rows_tiles * c->Tx * c->U;
+    fp.U = c->U;
+    fp.ntw = pl.box_tiles; fp.ngx = (c->Tx + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
+    const long long G = (long long)rows_tiles * fp.ngx * c->U;
+    if (G > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "fused path: too many (box, unit) pairs for one launch");
+    fp.G = (int)G;
+    fp.evict_first = env_int("FITRIG_EVICT_FIRST", 0);
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
-    cudaError_t e;
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: e = launch_fused_stage<FITRIG_REF_ABS>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
-      case FITRIG_REF_LITERAL: e = launch_fused_stage<FITRIG_REF_LITERAL>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
-      default: e = launch_fused_stage<FITRIG_REF_FLOOR>(pl.stages, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_ABS: tlisi_fused_kernel<FITRIG_REF_ABS><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
+      case FITRIG_REF_LITERAL: tlisi_fused_kernel<FITRIG_REF_LITERAL><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
+      default: tlisi_fused_kernel<FITRIG_REF_FLOOR><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
     }
-    CUDA_TRY(e);
+    CUDA_TRY(cudaGetLastError());
     c->launches++;
   } else {
     if (with_max) {

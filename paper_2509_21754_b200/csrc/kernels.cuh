@@ -3,7 +3,8 @@
 //   tlisi_fused_kernel    steps a1-a5: |x_{s+1}-x_s|, second difference, clamped ratio, per-tile
 //                         sum/max/argmax/sum and the global maximum, in ONE pass that reads every
 //                         snapshot byte once.  A warp owns one 32x32 tile and marches it through
-//                         time; tiles arrive through a per-warp ring of TMA boxes (cp.async.bulk.tensor).
+//                         time; a producer warp fetches rows of up to 8 adjacent tiles as single TMA
+//                         boxes (cp.async.bulk.tensor) into a CTA-wide ring guarded by full/empty mbarriers.
 //   tlisi_generic_kernel  the same per-tile quantities for any tile size / alignment (3 reads per pixel-unit).
 //   stack_max_kernel      global maximum for the generic path.
 //   finalize_kernel       step a6-a7: q = mean(D)*max(D)*mean(r)/M^2, tLISI = 1-q, per-unit mean/std.
@@ -43,6 +44,9 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t done;
   do {
@@ -60,13 +64,20 @@ __device__ __forceinline__ uint64_t l2_evict_first_policy() {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
   return pol;
 }
-// One 32x32 fp32 box of snapshot z at pixel (x, y) -> shared memory; completes on `bar`.
-__device__ __forceinline__ void tma_load_tile(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z,
-                                              uint64_t policy) {
+// One box (ntw * 32 columns x 32 rows, fp32) of snapshot z at pixel (x, y) -> shared memory; completes on `bar`.
+__device__ __forceinline__ void tma_load_box_hint(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z,
+                                                  uint64_t policy) {
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
       " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst),
       "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y, int z) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes"
+      " [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar)
       : "memory");
 }
 __device__ __forceinline__ float rcp_approx(float a) {
@@ -126,25 +137,31 @@ struct FusedParams {
   int rows_tiles;        // tile rows covered by this launch (whole image, or one strip)
   int ty_base;           // first tile row of this launch inside the whole map
   int U;                 // units = L - 2
-  int G;                 // rows_tiles * Tx * U: (tile, unit) pairs of this launch, tile-major
+  int ntw;               // tiles per TMA box = consumer warps per CTA (1..kMaxTilesPerBox)
+  int ngx;               // boxes per tile row = ceil(Tx / ntw)
+  int nstage;            // depth of the CTA's ring of boxes
+  int G;                 // rows_tiles * ngx * U: (box column, unit) pairs of this launch, box-major
+  int evict_first;       // L2 policy of the streaming loads
   float C;
 };
 
-// Work distribution: the G (tile, unit) pairs of a launch, ordered tile-major / time-minor, are cut
-// into one contiguous range per warp (range w = [w*G/n, (w+1)*G/n)), so every warp carries the same
-// load whatever the tile count.  A range is walked as "segments": a run of consecutive units of one
-// tile, which costs its units + 2 snapshots to march through (the 2-snapshot halo is re-read only
-// where a cut falls inside a tile's time series: at most once per warp).
+// Work distribution: a "group" is a row of ntw horizontally adjacent tiles, fetched as ONE TMA box of
+// 32 rows x (ntw * 128) contiguous bytes (isolated 128-byte rows cost ~15 % of the HBM bandwidth, see
+// profiles/).  The G (group, unit) pairs of a launch, ordered group-major / time-minor, are cut into
+// one contiguous range per CTA (range c = [c*G/n, (c+1)*G/n)), so every CTA carries the same load
+// whatever the tile count.  A range is walked as "segments": a run of consecutive units of one
+// group, which costs its units + 2 snapshots to march through (the 2-snapshot halo is re-read only
+// where a cut falls inside a group's time series: at most once per CTA).
 struct Segment {
-  int tx, ty_local, u0, nsteps;  // tile, first unit, snapshots to load (= units + 2)
+  int gx, ty_local, u0, nsteps;  // box column, tile row, first unit, snapshots to load (= units + 2)
 };
 
 __device__ __forceinline__ Segment decode_segment(const FusedParams& p, int g, int g_end) {
   Segment c;
-  const int tile = g / p.U;
-  c.u0 = g - tile * p.U;
-  c.ty_local = tile / p.Tx;
-  c.tx = tile - c.ty_local * p.Tx;
+  const int group = g / p.U;
+  c.u0 = g - group * p.U;
+  c.ty_local = group / p.ngx;
+  c.gx = group - c.ty_local * p.ngx;
   c.nsteps = min(p.U - c.u0, g_end - g) + 2;
   return c;
 }
@@ -155,14 +172,14 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// One 32x32 tile from a ring slot into registers.  Lane l owns columns 4*(l%8)..+3 of rows
-// (l/8) + 4*j, j = 0..7: a quarter warp reads one 128-byte tile row (conflict free), and the 32
-// pixels of a lane are held in increasing row-major order.
-__device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* slot_ptr, int lane) {
-  const float4* src = reinterpret_cast<const float4*>(slot_ptr) + lane;
+// One 32x32 tile out of a box (row pitch `pitch` bytes) into registers.  Lane l owns columns
+// 4*(l%8)..+3 of rows (l/8) + 4*j, j = 0..7: a quarter warp reads one 128-byte tile row (conflict
+// free), and the 32 pixels of a lane are held in increasing row-major order.
+__device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* tile_ptr, int pitch, int lane) {
+  const unsigned char* src = tile_ptr + (lane >> 3) * pitch + (lane & 7) * 16;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float4 t = src[j * 32];
+    const float4 t = *reinterpret_cast<const float4*>(src + 4 * j * pitch);
     N[4 * j] = t.x; N[4 * j + 1] = t.y; N[4 * j + 2] = t.z; N[4 * j + 3] = t.w;
   }
 }
@@ -224,78 +241,91 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
   R = R0 + R1;
 }
 
-// A warp owns one 32x32 tile and marches it through time; tiles arrive through a per-warp ring of
-// TMA boxes.  The two most recent snapshots live in registers (A/B ping-pong, no copies), so every
-// snapshot byte is read from HBM once.  The arg-max of Delta (R20) is tracked per 16-byte group in
-// the loop; which of its 4 pixels it was is found one step later from a 48-byte re-read (3 x
-// cp.async of data that was in flight moments ago) by lane 0, off the critical path.
-template <int REF_MODE, int NSTAGE>
-__global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
+// One persistent CTA per SM: warp `ntw` is the producer (one lane issues TMA boxes of ntw adjacent
+// tiles into the CTA's ring; full/empty mbarriers), warps 0..ntw-1 are consumers.  A consumer owns
+// one 32x32 tile of the box and marches it through time: the two most recent snapshots live in
+// registers (A/B ping-pong, no copies), so every snapshot byte is read from HBM once.  The arg-max
+// of Delta (R20) is tracked per 16-byte group in the loop; which of its 4 pixels it was is found one
+// step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
+// by lane 0, off the critical path.
+template <int REF_MODE>
+__global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   // the shuffle tells the compiler the warp index is warp uniform, so cursors and addresses derived
   // from it live in uniform registers and the vector registers are left to the three tile arrays
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-  const int nwarps = blockDim.x >> 5;
-  unsigned char* ring = smem + (size_t)warp * NSTAGE * kTileBytes;
-  unsigned char* after_ring = smem + (size_t)nwarps * NSTAGE * kTileBytes;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(after_ring) + warp * NSTAGE;
-  float4* scratch = reinterpret_cast<float4*>(after_ring + (((size_t)nwarps * NSTAGE * 8 + 15) & ~(size_t)15)) + warp * kScratchVec;
+  const int box_bytes = p.ntw * kTileBytes, pitch = p.ntw * 128;
+  unsigned char* after_ring = smem + (size_t)p.nstage * box_bytes;
+  uint64_t* full = reinterpret_cast<uint64_t*>(after_ring);
+  uint64_t* empty = full + kMaxStages;
+  float4* scratch = reinterpret_cast<float4*>(after_ring + 2 * kMaxStages * 8) + warp * kScratchVec;
 
-  if (lane == 0) {
-#pragma unroll
-    for (int i = 0; i < NSTAGE; ++i) mbar_init(smem_u32(&bars[i]), 1);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < p.nstage; ++i) {
+      mbar_init(smem_u32(&full[i]), 1);
+      mbar_init(smem_u32(&empty[i]), p.ntw);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
 
-  const int total_warps = gridDim.x * nwarps;
-  const int warp_global = blockIdx.x * nwarps + warp;
-  const uint64_t policy = l2_evict_first_policy();
-  const uint32_t ring_addr = smem_u32(ring);
-  const uint32_t bar_addr = smem_u32(bars);
-  const uint32_t scratch_addr = smem_u32(scratch);
+  // this CTA's range of (group, unit) pairs
+  const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
+  const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
+  const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty);
 
-  // this warp's range of (tile, unit) pairs
-  const int g_begin = (int)((long long)warp_global * p.G / total_warps);
-  const int g_end = (int)((long long)(warp_global + 1) * p.G / total_warps);
-
-  // ---- producer cursor (lane 0 issues; all lanes track it, it is warp uniform) ----
-  int p_g = g_begin, p_step = 0;
-  Segment pc = decode_segment(p, p_g < g_end ? p_g : 0, g_end);
-  auto issue_next = [&](int slot) {
-    if (p_g < g_end) {
-      if (lane == 0) {
-        const uint32_t bar = bar_addr + slot * 8;
-        mbar_arrive_expect_tx(bar, kTileBytes);
-        tma_load_tile(ring_addr + slot * kTileBytes, &tmap, bar, pc.tx * kFastTile, pc.ty_local * kFastTile,
-                      pc.u0 + p_step, policy);
-      }
-      if (++p_step == pc.nsteps) {
-        p_step = 0;
-        p_g += pc.nsteps - 2;
-        if (p_g < g_end) pc = decode_segment(p, p_g, g_end);
+  if (warp == p.ntw) {
+    // ---- producer ----
+    if (lane == 0) {
+      const uint64_t policy = l2_evict_first_policy();
+      const uint32_t ring_addr = smem_u32(smem);
+      int slot = 0;
+      uint32_t phase = 0;
+      for (int g = g_begin; g < g_end;) {
+        const Segment c = decode_segment(p, g, g_end);
+        g += c.nsteps - 2;
+        for (int s = 0; s < c.nsteps; ++s) {
+          mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
+          const uint32_t bar = full_addr + slot * 8;
+          mbar_arrive_expect_tx(bar, box_bytes);
+          if (p.evict_first)
+            tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
+                              c.u0 + s, policy);
+          else
+            tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
+                         c.u0 + s);
+          if (++slot == p.nstage) { slot = 0; phase ^= 1; }
+        }
       }
     }
-  };
-#pragma unroll
-  for (int i = 0; i < NSTAGE; ++i) issue_next(i);
+    return;
+  }
 
+  // ---- consumers ----
+  const unsigned char* my_col = smem + warp * 128;
+  const uint32_t scratch_addr = smem_u32(scratch);
   float A[32], B[32], dp[32];
   float gmax = -3.402823466e38f, zA = 1.f, zB = 1.f;
   int slot = 0;
   uint32_t phase = 0;
   const int lrow = lane >> 3, lcol = (lane & 7) * 4;
 
-  // next snapshot of the current item: ring slot -> registers, then refill the slot NSTAGE steps ahead
+  // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
-    mbar_wait(bar_addr + slot * 8, phase);
-    load_tile(N, ring + (size_t)slot * kTileBytes, lane);
-    __syncwarp();  // every lane has its copy: the slot may be refilled
-    issue_next(slot);
-    if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+    mbar_wait(full_addr + slot * 8, phase);
+    load_tile(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+    __syncwarp();  // every lane has its copy
+    if (lane == 0) mbar_arrive(empty_addr + slot * 8);
+    if (++slot == p.nstage) { slot = 0; phase ^= 1; }
     scan_tile(N, gmax, zmin);
+  };
+  // a warp whose tile lies beyond the image edge only keeps the ring turning
+  auto skip = [&]() {
+    mbar_wait(full_addr + slot * 8, phase);
+    if (lane == 0) mbar_arrive(empty_addr + slot * 8);
+    if (++slot == p.nstage) { slot = 0; phase ^= 1; }
   };
 
   // ---- one record is always "pending": its arg-max group is known, the pixel inside it is not.
@@ -321,7 +351,7 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
   };
 
   // warp reduction of one (tile, unit): exact max + first group by redux, the two sums by one butterfly
-  auto finish = [&](const Segment& c, int step, float S, float R, float Mx, int jmax) {
+  auto finish = [&](const Segment& c, int tx, int step, float S, float R, float Mx, int jmax) {
     const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
     const unsigned tmax = __reduce_max_sync(0xffffffffu, mbits);
     const int gpos = (lrow + 4 * jmax) * kFastTile + lcol;
@@ -338,10 +368,10 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
       const int u = c.u0 + step - 2;
       scratch[3] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
       *reinterpret_cast<unsigned long long*>(&scratch[4]) =
-          ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + c.tx;
+          ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + tx;
       // the winning group's 4 pixels in x_u, x_{u+1}, x_{u+2}: in bounds (a zero-filled pixel has Delta 0)
       const float* src = p.base + (long long)u * p.snap_stride +
-                         (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (c.tx * kFastTile + (int)(tg & 31));
+                         (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
       cp_async16(scratch_addr, src);
       cp_async16(scratch_addr + 16, src + p.snap_stride);
       cp_async16(scratch_addr + 32, src + 2 * p.snap_stride);
@@ -353,6 +383,11 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
   for (int g = g_begin; g < g_end;) {
     const Segment c = decode_segment(p, g, g_end);
     g += c.nsteps - 2;
+    const int tx = c.gx * p.ntw + warp;
+    if (tx >= p.Tx) {
+      for (int s = 0; s < c.nsteps; ++s) skip();
+      continue;
+    }
     acquire(A, zA);  // x_{u0}
     acquire(B, zB);  // x_{u0+1}
 #pragma unroll
@@ -363,11 +398,11 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
       int jmax;
       acquire(A, zA);
       tile_step<REF_MODE>(A, B, dp, p.C, __any_sync(0xffffffffu, zB == 0.f), S, R, Mx, jmax);
-      finish(c, step, S, R, Mx, jmax);
+      finish(c, tx, step, S, R, Mx, jmax);
       if (++step >= c.nsteps) break;
       acquire(B, zB);
       tile_step<REF_MODE>(B, A, dp, p.C, __any_sync(0xffffffffu, zA == 0.f), S, R, Mx, jmax);
-      finish(c, step, S, R, Mx, jmax);
+      finish(c, tx, step, S, R, Mx, jmax);
       if (++step >= c.nsteps) break;
     }
   }
@@ -376,7 +411,6 @@ __global__ void __launch_bounds__(32 * kMaxWarpsPerCta, 1)
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
 }
-
 // ---------------------------------------------------------------------------------------------
 // Generic path: any tile size, any width / alignment.  G (power of two <= 32) lanes share one tile.
 // ---------------------------------------------------------------------------------------------

@@ -41,17 +41,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
   return FITRIG_OK;
 }
 
-// Fused path: one persistent CTA per SM; each warp owns a contiguous range of the G = tiles * U
-// (tile, unit) pairs (see kernels.cuh), so the load is balanced for every tile count and only the
-// warp count, ring depth and grid are chosen here.  12 warps x 168 registers keep three 32-pixel
-// tile arrays per lane in registers without spills; 12 x 4 x 4 KB = 192 KB of TMA boxes in flight
-// per SM is several times the HBM latency-bandwidth product (~50 KB per SM).
+// Fused path: one persistent CTA per SM; the CTAs share the G = boxes * U (box column, unit) pairs
+// evenly (see kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8
+// adjacent tiles is 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes
+// of 32 KB in flight per SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
 void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
   const bool force_generic = env_int("FITRIG_FORCE_GENERIC", 0) != 0;
   if (tile != kFastTile || (W % 4) != 0 || force_generic) {
     plan->path = 1;
-    plan->units_per_warp = 0;
+    plan->units_per_cta = 0;
+    plan->box_tiles = 0;
     plan->warps_per_cta = 8;
     plan->stages = 0;
     plan->smem_bytes = 0;
@@ -59,26 +59,25 @@ void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fit
     return;
   }
   plan->path = 0;
-  const long long G = (long long)tile_rows * Tx * U;
-  int w = kMaxWarpsPerCta;
-  const int fw = env_int("FITRIG_WARPS", 0), fs = env_int("FITRIG_STAGES", 0), fg = env_int("FITRIG_GRID", 0);
-  if (fw > 0) w = std::max(1, std::min(fw, kMaxWarpsPerCta));
-  // small problems are latency bound: give every warp at least kMinUnitsPerWarp units, and spread the
-  // warps over as many SMs as possible
-  long long total = std::min<long long>((long long)num_sms * w, (G + kMinUnitsPerWarp - 1) / kMinUnitsPerWarp);
-  total = std::max<long long>(total, 1);
-  if (fw <= 0) w = (int)std::max<long long>(1, std::min<long long>(w, (total + num_sms - 1) / num_sms));
-  int grid = (int)std::min<long long>(num_sms, (total + w - 1) / w);
+  const int fb = env_int("FITRIG_BOX_TILES", 0), fs = env_int("FITRIG_STAGES", 0), fg = env_int("FITRIG_GRID", 0);
+  int ntw = std::min(kMaxTilesPerBox, Tx);
+  auto pairs = [&](int n) { return (long long)tile_rows * ((Tx + n - 1) / n) * U; };
+  // small problems are latency bound: narrower boxes give more CTAs something to do
+  while (ntw > 1 && (pairs(ntw) + kMinUnitsPerCta - 1) / kMinUnitsPerCta < num_sms) ntw = (ntw + 1) / 2;
+  if (fb > 0) ntw = std::max(1, std::min(fb, std::min(kMaxTilesPerBox, Tx)));
+  const long long G = pairs(ntw);
+  int grid = (int)std::max<long long>(1, std::min<long long>(num_sms, (G + kMinUnitsPerCta - 1) / kMinUnitsPerCta));
   if (fg > 0) grid = fg;
-  // deepest ring that fits next to the mbarriers and the arg-max scratch, capped at 4
-  int bs = std::min(4, (kMaxSmemPerCta - 2048) / (w * kTileBytes));
-  if (fs > 0) bs = std::min(fs, (kMaxSmemPerCta - 2048) / (w * kTileBytes));
-  bs = std::max(2, bs);
-  plan->warps_per_cta = w;
-  plan->stages = bs;
-  plan->grid = std::max(1, grid);
-  plan->units_per_warp = (int32_t)((G + (long long)plan->grid * w - 1) / ((long long)plan->grid * w));
-  plan->smem_bytes = w * bs * kTileBytes + ((w * bs * 8 + 15) & ~15) + w * kScratchVec * 16;  // ring, mbarriers, scratch
+  const int fit = (kMaxSmemPerCta - 2048) / (ntw * kTileBytes);
+  int stages = std::min(6, fit);
+  if (fs > 0) stages = std::min(fs, fit);
+  stages = std::max(2, std::min(stages, kMaxStages));
+  plan->box_tiles = ntw;
+  plan->warps_per_cta = ntw + 1;  // consumers + the producer
+  plan->stages = stages;
+  plan->grid = grid;
+  plan->units_per_cta = (int32_t)((G + grid - 1) / grid);
+  plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + ntw * kScratchVec * 16;  // ring, mbarriers, scratch
 }
 
 }  // namespace fitrig

@@ -9,8 +9,9 @@ namespace fitrig {
 constexpr int kFastTile = 32;          // tile edge of the fused path (the paper's default)
 constexpr int kTileBytes = 32 * 32 * 4;  // one 32x32 fp32 tile = one TMA box
 constexpr int kMaxSmemPerCta = 227 * 1024;
-constexpr int kMaxWarpsPerCta = 12;    // 384 threads x 168 registers: A/B/dp tile arrays (96) + pipeline state, no spills
-constexpr int kMinUnitsPerWarp = 2;    // fused path: fewest (tile, unit) pairs worth a warp of its own
+constexpr int kMaxTilesPerBox = 8;     // fused path: tiles per TMA box (256 columns, the TMA box limit) = consumer warps per CTA
+constexpr int kMaxStages = 8;          // fused path: deepest ring of boxes
+constexpr int kMinUnitsPerCta = 2;     // fused path: fewest (box column, unit) pairs worth a CTA of its own
 constexpr int kScratchVec = 6;         // float4 per warp of arg-max scratch (fused kernel)
 
 struct NormParams {  // fitrig_params with defaults applied
@@ -26,10 +27,10 @@ struct NormParams {  // fitrig_params with defaults applied
 // Validates and applies defaults.  Returns FITRIG_OK or FITRIG_ERR_INVALID_ARG (+ message in *why).
 int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, NormParams* out, const char** why);
 
-// Chooses path, warps per CTA, ring depth and grid for `tile_rows` x Tx tiles of U units.
+// Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
 void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan);
 
-// Debug/tuning overrides: FITRIG_WARPS, FITRIG_STAGES, FITRIG_GRID, FITRIG_FORCE_GENERIC (integers).
+// Debug/tuning overrides: FITRIG_BOX_TILES, FITRIG_STAGES, FITRIG_GRID, FITRIG_EVICT_FIRST, FITRIG_FORCE_GENERIC (integers).
 int env_int(const char* name, int dflt);
 
 }  // namespace fitrig

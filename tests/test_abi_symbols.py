@@ -36,17 +36,20 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert p.path == 0 and p.Tx == 8
 
 
-def test_plan_query_balances_units_over_warps():
-    # 4096 tiles x 62 units on 148 SMs x 12 warps: every warp gets ceil(253952 / 1776) = 143 (tile, unit) pairs
+def test_plan_query_balances_units_over_ctas():
+    # 64 x 8 boxes of 8 tiles x 62 units on 148 SMs: every CTA gets ceil(31744 / 148) = 215 (box, unit) pairs
     p = fitrig.plan_query(2048, 2048, 64, num_sms=148)
-    assert p.warps_per_cta == 12 and p.grid == 148 and p.units_per_warp == 143
-    assert p.smem_bytes <= 227 * 1024 and p.stages >= 3
-    # tiny problem (384 pairs): spread thin so that the GPU is not left to a few SMs
+    assert p.box_tiles == 8 and p.warps_per_cta == 9 and p.grid == 148 and p.units_per_cta == 215
+    assert p.smem_bytes <= 227 * 1024 and p.stages >= 4
+    # tiny problem (64 tiles x 6 units): narrow boxes, spread thin so that the GPU is not left to a few SMs
     p = fitrig.plan_query(256, 256, 8, num_sms=148)
-    assert p.grid * p.warps_per_cta >= 148 and p.units_per_warp >= 2
+    assert p.grid >= 96 and p.units_per_cta >= 2 and p.box_tiles < 8
     # one tile, one unit
     p = fitrig.plan_query(32, 32, 3, num_sms=148)
-    assert p.grid == 1 and p.warps_per_cta == 1 and p.units_per_warp == 1
+    assert p.grid == 1 and p.box_tiles == 1 and p.warps_per_cta == 2 and p.units_per_cta == 1
+    # 50000 wide: 1563 tiles = 195 boxes of 8 + one of 3 (the rest of the last box is zero-filled by TMA)
+    p = fitrig.plan_query(50000, 50000, 4, num_sms=148)
+    assert p.box_tiles == 8 and p.grid == 148
 
 
 @pytest.mark.parametrize("H,W,L,kw", [

@@ -174,20 +174,23 @@ def test_m_override_scales_q_but_not_candidates(tiny):
 
 
 def test_work_partition_does_not_change_the_map(tiny, monkeypatch):
-    """The per-warp ranges of (tile, unit) pairs cut tiles' time series at different places for different
-    warp counts / grids; the per-tile results must not depend on where the cuts fall."""
+    """The per-CTA ranges of (box, unit) pairs cut tiles' time series at different places for different box
+    widths / grids / ring depths; the per-tile results must not depend on where the cuts fall, on which warp of
+    a box owns the tile, or on boxes that hang over the image edge (box width 3 or 5 on an 8-tile row)."""
     st, _ = tiny
-    monkeypatch.setenv("FITRIG_WARPS", "1")
+    monkeypatch.setenv("FITRIG_BOX_TILES", "1")
     monkeypatch.setenv("FITRIG_GRID", "1")
-    a = gpu_run(st)  # one warp walks all 384 pairs: no cut inside any tile
-    for warps, grid, stages in ((9, 7, 2), (12, 148, 4), (5, 13, 3)):
-        monkeypatch.setenv("FITRIG_WARPS", str(warps))
+    a = gpu_run(st)  # one consumer warp walks all 384 pairs: no cut inside any tile
+    for box, grid, stages in ((3, 7, 2), (8, 148, 6), (5, 13, 3), (8, 5, 7), (2, 40, 8)):
+        monkeypatch.setenv("FITRIG_BOX_TILES", str(box))
         monkeypatch.setenv("FITRIG_GRID", str(grid))
         monkeypatch.setenv("FITRIG_STAGES", str(stages))
-        b = gpu_run(st)
-        assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
-        for x, y in zip(a["raw"], b["raw"]):
-            assert np.array_equal(x, y)
+        for evict in ("0", "1"):
+            monkeypatch.setenv("FITRIG_EVICT_FIRST", evict)
+            b = gpu_run(st)
+            assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
+            for x, y in zip(a["raw"], b["raw"]):
+                assert np.array_equal(x, y)
 
 
 def test_fused_and_generic_kernels_agree(tiny, monkeypatch):
