@@ -158,12 +158,13 @@ int fitrig_get_map(const fitrig_ctx* ctx, int32_t which, float* h_out);
 int fitrig_get_raw(const fitrig_ctx* ctx, float* sumD, float* maxD, float* sumR, int32_t* arg_x, int32_t* arg_y);
 
 /* fitrig_profile -- enable (1) / disable (0) CUDA-event timing of the library's own kernels on the
- * launching stream.  fitrig_last_timing then reports, for the last fitrig_tlisi / fitrig_stream,
- * the summed duration of the fused (or generic) tLISI kernel launches, the number of such launches,
- * and the duration of the finalise+statistics kernel, in milliseconds (synchronises). */
+ * launching stream; either call starts a new accumulation window.  fitrig_last_timing then reports, for all
+ * fitrig_tlisi / fitrig_stream calls since the window started, the summed duration of the fused (or generic)
+ * tLISI kernel launches and their number, and the summed duration and number of the finalise+statistics
+ * launches, in milliseconds (synchronises the device), and starts a new window.  Any out may be NULL. */
 int fitrig_profile(fitrig_ctx* ctx, int32_t enable);
 int fitrig_last_timing(const fitrig_ctx* ctx, float* main_kernel_ms, int32_t* main_kernel_launches,
-                       float* finalize_ms);
+                       float* finalize_ms, int32_t* finalize_launches);
 
 /* fitrig_launch_count -- kernels launched by this context since creation (for bench.py's gpu_launches). */
 int fitrig_launch_count(const fitrig_ctx* ctx, int64_t* n);

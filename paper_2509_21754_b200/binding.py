@@ -104,7 +104,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_get_map.argtypes = [vp, i32, vp]
     L.fitrig_get_raw.argtypes = [vp, vp, vp, vp, vp, vp]
     L.fitrig_profile.argtypes = [vp, i32]
-    L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32)]
+    L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
               "fitrig_detect", "fitrig_stream", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
@@ -261,9 +261,10 @@ class Context:
         _check(self._L.fitrig_profile(self._h, int(bool(enable))))
 
     def last_timing(self):
-        a, n, b = ctypes.c_float(), ctypes.c_int32(), ctypes.c_float()
-        _check(self._L.fitrig_last_timing(self._h, ctypes.byref(a), ctypes.byref(n), ctypes.byref(b)))
-        return a.value, n.value, b.value
+        """(main kernel ms, launches, finalise ms, launches), summed since profiling was enabled or last read."""
+        a, n, b, m = ctypes.c_float(), ctypes.c_int32(), ctypes.c_float(), ctypes.c_int32()
+        _check(self._L.fitrig_last_timing(self._h, ctypes.byref(a), ctypes.byref(n), ctypes.byref(b), ctypes.byref(m)))
+        return a.value, n.value, b.value, m.value
 
     def launch_count(self) -> int:
         n = ctypes.c_int64()

@@ -69,7 +69,9 @@ struct fitrig_ctx {
   // map
   RawTile* raw;
   float *q, *tlisi, *M_dev;
-  unsigned* gmax_key;
+  unsigned* gmax_key;  // two order-preserving keys of the running global maximum, used by alternate calls:
+  int key_idx;         // the finalise kernel of one call zeroes the key of the next, so no memset sits in the stream
+  bool keys_clean;
   StatPartial* parts;
   unsigned* counters;
   double *mu, *sigma;
@@ -88,7 +90,8 @@ struct fitrig_ctx {
   long long cand_cap;
   unsigned* blk_counts;
   int compact_grid_max;
-  unsigned char* cand_host;  // pinned: CandHeader + kHostStageCands candidates
+  unsigned char* cand_host;  // pinned + mapped: CandHeader + kHostStageCands candidates, written by the kernel
+  unsigned char* cand_host_dev;  // device address of cand_host
   // streaming
   float* strip_buf[kMaxStripBuffers];
   int n_strip_buf;
@@ -98,10 +101,10 @@ struct fitrig_ctx {
   bool ev_free_pending[kMaxStripBuffers];
   // profiling
   bool profile;
-  std::vector<cudaEvent_t> ev_pool;  // pairs: start, stop of each main-kernel launch of the last call
+  std::vector<cudaEvent_t> ev_pool;   // pairs: start, stop of each main-kernel launch since the last read
   int ev_used;
-  cudaEvent_t ev_fin0, ev_fin1;
-  bool fin_timed;
+  std::vector<cudaEvent_t> fin_pool;  // pairs around each finalise launch since the last read
+  int fin_used;
   bool have_map;
   long long launches;
 };
@@ -123,8 +126,7 @@ static void free_ctx(fitrig_ctx* c) {
   if (c->ev_entry) cudaEventDestroy(c->ev_entry);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
-  if (c->ev_fin0) cudaEventDestroy(c->ev_fin0);
-  if (c->ev_fin1) cudaEventDestroy(c->ev_fin1);
+  for (cudaEvent_t e : c->fin_pool) cudaEventDestroy(e);
   (void)cudaGetLastError();
   delete c;
 }
@@ -191,7 +193,9 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->tlisi, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float)));
-  CTX_TRY(cudaMalloc(&c->gmax_key, sizeof(unsigned)));
+  CTX_TRY(cudaMalloc(&c->gmax_key, 2 * sizeof(unsigned)));
+  CTX_TRY(cudaMemset(c->gmax_key, 0, 2 * sizeof(unsigned)));
+  c->keys_clean = true;
   c->fin_nblk = (int)std::max<long long>(1, std::min<long long>(64, (c->nt + 2047) / 2048));
   CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * c->U * c->fin_nblk));
   CTX_TRY(cudaMalloc(&c->counters, sizeof(unsigned) * c->U));
@@ -223,9 +227,8 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   c->cand_cap = kHostStageCands;
   CTX_TRY(cudaMalloc(&c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * c->cand_cap));
   CTX_TRY(cudaHostAlloc(&c->cand_host, sizeof(CandHeader) + sizeof(fitrig_candidate) * kHostStageCands,
-                        cudaHostAllocDefault));
-  CTX_TRY(cudaEventCreate(&c->ev_fin0));
-  CTX_TRY(cudaEventCreate(&c->ev_fin1));
+                        cudaHostAllocMapped));
+  CTX_TRY(cudaHostGetDevicePointer((void**)&c->cand_host_dev, c->cand_host, 0));
   if (c->plan.path == 0) {
     CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
@@ -291,7 +294,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
-    fp.raw = c->raw; fp.gmax_key = c->gmax_key;
+    fp.raw = c->raw; fp.gmax_key = c->gmax_key + c->key_idx;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
     fp.U = c->U;
@@ -314,7 +317,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
       for (int s = 0; s < c->L; ++s) {
         stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)s * snap_stride,
-                                                                       (long long)rows * c->W, c->gmax_key);
+                                                                       (long long)rows * c->W, c->gmax_key + c->key_idx);
         CUDA_TRY(cudaGetLastError());
         c->launches++;
       }
@@ -345,16 +348,24 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
 static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st) {
   FinalizeParams fp;
   fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
-  fp.gmax_key = c->gmax_key; fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
+  fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
   fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
   fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
-  if (c->profile) CUDA_TRY(cudaEventRecord(c->ev_fin0, st));
+  if (c->profile) {
+    while ((int)c->fin_pool.size() < 2 * (c->fin_used + 1)) {
+      cudaEvent_t e;
+      CUDA_TRY(cudaEventCreate(&e));
+      c->fin_pool.push_back(e);
+    }
+    CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used], st));
+  }
   finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
   CUDA_TRY(cudaGetLastError());
-  if (c->profile) { CUDA_TRY(cudaEventRecord(c->ev_fin1, st)); c->fin_timed = true; }
+  if (c->profile) { CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used + 1], st)); c->fin_used++; }
   c->launches++;
   c->have_map = true;
   c->eta_valid = false;
+  c->keys_clean = true;
   return FITRIG_OK;
 }
 
@@ -363,9 +374,9 @@ extern "C" int fitrig_tlisi(fitrig_ctx* c, const float* d_stack, float* d_tlisi,
   if (!d_stack) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: d_stack is NULL");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
-  c->ev_used = 0;
-  c->fin_timed = false;
-  CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, sizeof(unsigned), st));
+  if (!c->keys_clean) CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, 2 * sizeof(unsigned), st));  // a call failed half way
+  c->keys_clean = false;
+  c->key_idx ^= 1;
   int rc = launch_tlisi_rows(c, d_stack, (long long)c->H * c->W, c->H, 0, true, st);
   if (rc) return rc;
   return launch_finalize(c, d_tlisi, st);
@@ -390,9 +401,9 @@ extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, flo
     }
     c->n_strip_buf = nbuf;
   }
-  c->ev_used = 0;
-  c->fin_timed = false;
-  CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, sizeof(unsigned), st));
+  if (!c->keys_clean) CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, 2 * sizeof(unsigned), st));  // a call failed half way
+  c->keys_clean = false;
+  c->key_idx ^= 1;
   // the copy stream may not run ahead of work already queued on the caller's stream
   CUDA_TRY(cudaEventRecord(c->ev_entry, st));
   CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
@@ -459,6 +470,9 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
   cp.cap = std::min<long long>(c->cand_cap, std::max<long long>(capacity, 0));
   cp.total = reinterpret_cast<unsigned long long*>(c->cand_dev);
+  cp.host_total = reinterpret_cast<unsigned long long*>(c->cand_host_dev);
+  cp.host_out = reinterpret_cast<fitrig_candidate*>(c->cand_host_dev + sizeof(CandHeader));
+  cp.host_cap = std::min<long long>(cp.cap, kHostStageCands);
   cp.blk_counts = c->blk_counts;
   const int threads = 512;
   int grid = (int)std::min<long long>(c->compact_grid_max, (N + threads - 1) / threads);
@@ -467,10 +481,9 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   void* args[] = {&cp};
   CUDA_TRY(cudaLaunchCooperativeKernel((void*)compact_kernel, dim3(grid), dim3(threads), args, 0, st));
   c->launches++;
-  // count + the first kHostStageCands candidates in one copy; a second copy only for longer lists
-  const long long first = std::min<long long>(cp.cap, kHostStageCands);
-  CUDA_TRY(cudaMemcpyAsync(c->cand_host, c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * first,
-                           cudaMemcpyDeviceToHost, st));
+  // the kernel writes the count and the first kHostStageCands candidates straight into mapped pinned memory
+  // (no copy in the stream); a copy from the device list only for longer lists
+  const long long first = cp.host_cap;
   CUDA_TRY(cudaStreamSynchronize(st));
   const long long total = (long long)reinterpret_cast<CandHeader*>(c->cand_host)->total;
   const long long nwrite = std::min<long long>(total, cp.cap);
@@ -557,10 +570,13 @@ extern "C" int fitrig_get_raw(const fitrig_ctx* c, float* sumD, float* maxD, flo
 extern "C" int fitrig_profile(fitrig_ctx* c, int32_t enable) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_profile: ctx is NULL");
   c->profile = enable != 0;
+  c->ev_used = 0;
+  c->fin_used = 0;
   return FITRIG_OK;
 }
 
-extern "C" int fitrig_last_timing(const fitrig_ctx* c, float* main_ms, int32_t* main_launches, float* fin_ms) {
+extern "C" int fitrig_last_timing(const fitrig_ctx* c, float* main_ms, int32_t* main_launches, float* fin_ms,
+                                  int32_t* fin_launches) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_last_timing: ctx is NULL");
   if (!c->profile || !c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_last_timing: profiling was not enabled");
   CUDA_TRY(cudaSetDevice(c->prm.device));
@@ -573,10 +589,17 @@ extern "C" int fitrig_last_timing(const fitrig_ctx* c, float* main_ms, int32_t* 
   }
   if (main_ms) *main_ms = tot;
   if (main_launches) *main_launches = c->ev_used;
-  if (fin_ms) {
-    *fin_ms = 0.f;
-    if (c->fin_timed) CUDA_TRY(cudaEventElapsedTime(fin_ms, c->ev_fin0, c->ev_fin1));
+  float ftot = 0.f;
+  for (int i = 0; i < c->fin_used; ++i) {
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, c->fin_pool[2 * i], c->fin_pool[2 * i + 1]));
+    ftot += ms;
   }
+  if (fin_ms) *fin_ms = ftot;
+  if (fin_launches) *fin_launches = c->fin_used;
+  fitrig_ctx* m = const_cast<fitrig_ctx*>(c);  // reading starts a new accumulation window
+  m->ev_used = 0;
+  m->fin_used = 0;
   return FITRIG_OK;
 }
 

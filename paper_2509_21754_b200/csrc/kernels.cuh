@@ -552,6 +552,7 @@ struct FinalizeParams {
   float* tlisi;        // context copy, [U][Ty][Tx]
   float* tlisi_user;   // caller's device buffer or NULL
   const unsigned* gmax_key;
+  unsigned* gmax_key_next;  // key of the NEXT call: zeroed here so that no memset sits in the stream
   float* M_out;        // device scalar: the M that was used
   float M_override;
   float C;
@@ -572,7 +573,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
   // M = max(max_s x^(s), C), PAPER.md:223 (R2: signed max), or the caller's override
   float M = fmaxf(key_to_float(*p.gmax_key), p.C);
   if (p.M_override > 0.f) M = p.M_override;
-  if (blockIdx.x == 0 && u == 0 && threadIdx.x == 0) *p.M_out = M;
+  if (blockIdx.x == 0 && u == 0 && threadIdx.x == 0) {
+    *p.M_out = M;
+    *p.gmax_key_next = 0u;
+  }
   const double inv_m2 = 1.0 / ((double)M * (double)M);
   const size_t base = (size_t)u * nt;
   for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
@@ -662,6 +666,9 @@ struct CompactParams {
   fitrig_candidate* out;
   long long cap;        // device capacity of `out`
   unsigned long long* total;
+  unsigned long long* host_total;  // the same count, in mapped pinned host memory
+  fitrig_candidate* host_out;      // first host_cap candidates, in mapped pinned host memory
+  long long host_cap;
   unsigned* blk_counts; // [gridDim.x]
   long long seg;        // entries per block (multiple of blockDim.x)
 };
@@ -704,7 +711,10 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   for (int off = 16; off > 0; off >>= 1) below += __shfl_xor_sync(0xffffffffu, below, off);
   if (lane == 0 && below) atomicAdd(&block_base, below);
   __syncthreads();
-  if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) *p.total = block_base + p.blk_counts[blockIdx.x];
+  if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) {
+    *p.total = block_base + p.blk_counts[blockIdx.x];
+    *p.host_total = block_base + p.blk_counts[blockIdx.x];
+  }
   unsigned long long running = block_base;
   // ---- pass 2: write in order, one blockDim.x-wide chunk at a time ----
   for (long long c0 = begin; c0 < end; c0 += blockDim.x) {
@@ -740,6 +750,7 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
         }
         cd.score = z;
         p.out[dst] = cd;
+        if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
       }
     }
     running += chunk_total;
