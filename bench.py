@@ -217,6 +217,7 @@ def run_fitrig(args, cfg, tau, branch):
     import torch
     import paper_2509_21754_b200 as fitrig
     import synth
+    from paper_2509_21754_b200 import shard
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -277,10 +278,7 @@ def run_fitrig(args, cfg, tau, branch):
     # CUDA events the library recorded around its own launches, on the launching stream, during the timed region
     main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
     ctx.profile(False)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = shard.max_over_ranks(ms, dev)  # device time of the slowest rank
     value = world * pix * args.steps / (ms_max * 1e-3) / 1e6
 
     # ---- roofline of the dominant (fused) kernel ----
@@ -326,10 +324,7 @@ def run_fitrig(args, cfg, tau, branch):
         f1.record(stream)
         barrier()
         sampler.stop()
-        t2 = torch.tensor([f0.elapsed_time(f1)], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e_ms = float(t2.item()) / ksteps
+        e_ms = shard.max_over_ranks(f0.elapsed_time(f1), dev) / ksteps
         assert n2 == n_found, "streamed and resident paths disagree on the candidate count"
         e2e = {"value": world * pix / (e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * pix,
                "d2h_bytes_per_step": n_ch * (4 * U * Ty * Tx + 16) + 16 * int(min(n_found, 4096 * n_ch)), "ms_per_step": e_ms,

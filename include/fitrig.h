@@ -60,7 +60,9 @@ typedef struct {
   int32_t branch;     /* FITRIG_BRANCH_*                                                          */
   int32_t strip_rows; /* fitrig_stream strip height, multiple of tile; 0 -> auto                  */
   int32_t device;     /* CUDA device ordinal                                                      */
-  int32_t reserved[9];
+  int32_t row_offset; /* row shards (fitrig_shard_*): image row of this context's first row, a multiple of */
+                      /* tile; added to the y of every candidate.  0 for a whole image                     */
+  int32_t reserved[8];
 } fitrig_params;
 
 /* One candidate, 16 bytes.
@@ -141,6 +143,34 @@ int fitrig_detect(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate* h_ou
  * Strips of params.strip_rows rows (all L snapshots of those rows) rotate through device
  * buffers: strip i+1 is copied while strip i is reduced.  Errors: INVALID_ARG, NOMEM, CUDA. */
 int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream);
+
+/* Row shards (tiles are independent).  One image is cut into
+ * horizontal shards of whole tile rows, one context (normally one GPU) per shard, each created with the
+ * shard's own H and params.row_offset.  Only the three global scalars of the method couple the shards:
+ * M and, per unit, the mean and standard deviation of the tile matrix (Eq. 8).  Protocol,
+ * image branch only:
+ *     fitrig_tlisi(shard)                       local map, provisional (M of the shard alone)
+ *     fitrig_shard_export -> v[2 + 2U]          what the other shards need
+ *     all-gather v over the shards              the ONE exchange step (NCCL; (2 + 2U) * 8 bytes per rank)
+ *     fitrig_shard_import(all v, world)         global M, mu, sigma; this shard's q and tLISI rescaled
+ *     fitrig_detect                             this shard's candidates, y already in image rows
+ *
+ * fitrig_shard_export -- d_out (device) receives 2 + 2U doubles:
+ *   [0]            largest pixel value of this shard's L snapshots (signed, not floored at C; R2)
+ *   [1]            number of tiles per unit in this shard
+ *   [2 .. 2+U)     per unit: sum over tiles of p = (sum Delta / n_t) * max Delta * (sum r / n_t), i.e. the
+ *                  product of Eq. 2 / Eq. 6 WITHOUT the 1/M^2 factor (q = p / M^2)
+ *   [2+U .. 2+2U)  per unit: sum over tiles of p^2
+ * Asynchronous on cuda_stream.  Errors: STATE (no current map), INVALID_ARG (NULL; frequency branch), CUDA. */
+int fitrig_shard_export(fitrig_ctx* ctx, double* d_out, void* cuda_stream);
+
+/* fitrig_shard_import -- d_all (device): `world` export vectors back to back, [world][2 + 2U], in shard
+ * order (identical on every shard so that all shards derive bit-identical M, mu, sigma).  Sets
+ * M = max(max over shards, C), mu_u and sigma_u of q = p / M^2 over ALL tiles of the image (population
+ * std, R3), rewrites this shard's q and tLISI with that M, and writes tLISI to d_tlisi (device,
+ * [U][Ty_shard][Tx], may be NULL).  The shard's map is then bit-identical to the same rows of a
+ * whole-image fitrig_tlisi.  Asynchronous.  Errors: STATE, INVALID_ARG (NULL, world < 1), CUDA. */
+int fitrig_shard_import(fitrig_ctx* ctx, const double* d_all, int32_t world, float* d_tlisi, void* cuda_stream);
 
 /* fitrig_get_stats -- M and the per-unit mean / population std of q = 1 - tLISI
  * (Eq. 8; mu_tLISI = 1 - mu_q).  Frequency branch after fitrig_detect: mu[0], sigma[0] describe

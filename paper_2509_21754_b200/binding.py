@@ -26,7 +26,7 @@ class FitrigError(RuntimeError):
 class _Params(ctypes.Structure):
     _fields_ = [("tile", ctypes.c_int32), ("C", ctypes.c_float), ("ref_mode", ctypes.c_int32),
                 ("M_override", ctypes.c_float), ("branch", ctypes.c_int32), ("strip_rows", ctypes.c_int32),
-                ("device", ctypes.c_int32), ("reserved", ctypes.c_int32 * 9)]
+                ("device", ctypes.c_int32), ("row_offset", ctypes.c_int32), ("reserved", ctypes.c_int32 * 8)]
 
 
 class _Candidate(ctypes.Structure):
@@ -100,6 +100,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_tlisi.argtypes = [vp, vp, vp, vp]
     L.fitrig_detect.argtypes = [vp, f32, vp, i64, P(i64), vp]
     L.fitrig_stream.argtypes = [vp, P(vp), vp, vp]
+    L.fitrig_shard_export.argtypes = [vp, vp, vp]
+    L.fitrig_shard_import.argtypes = [vp, vp, i32, vp, vp]
     L.fitrig_get_stats.argtypes = [vp, P(f32), vp, vp]
     L.fitrig_get_map.argtypes = [vp, i32, vp]
     L.fitrig_get_raw.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -107,7 +109,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
-              "fitrig_detect", "fitrig_stream", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
+              "fitrig_detect", "fitrig_stream", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
               "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
@@ -140,10 +142,12 @@ def _check(rc: int, allow: Tuple[int, ...] = ()) -> int:
     return rc
 
 
-def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_IMAGE, strip_rows=0, device=0):
+def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_IMAGE, strip_rows=0, device=0,
+                 row_offset=0):
     p = _Params()
     p.tile, p.C, p.ref_mode, p.M_override = int(tile), float(C), int(ref_mode), float(M_override)
     p.branch, p.strip_rows, p.device = int(branch), int(strip_rows), int(device)
+    p.row_offset = int(row_offset)
     return p
 
 
@@ -234,6 +238,20 @@ class Context:
         if h_tlisi is not None:
             out = h_tlisi.data_ptr() if hasattr(h_tlisi, "data_ptr") else h_tlisi.ctypes.data
         _check(self._L.fitrig_stream(self._h, arr, out, _stream_ptr(stream)))
+
+    # ---- row shards ----
+    def shard_export(self, d_out, stream=None) -> None:
+        """d_out: CUDA float64 tensor of 2 + 2U elements."""
+        assert d_out.is_cuda and d_out.is_contiguous() and str(d_out.dtype) == "torch.float64"
+        assert d_out.numel() >= 2 + 2 * self.units
+        _check(self._L.fitrig_shard_export(self._h, d_out.data_ptr(), _stream_ptr(stream)))
+
+    def shard_import(self, d_all, world: int, d_tlisi=None, stream=None) -> None:
+        """d_all: CUDA float64 tensor [world, 2 + 2U] (the all-gathered export vectors, in shard order)."""
+        assert d_all.is_cuda and d_all.is_contiguous() and str(d_all.dtype) == "torch.float64"
+        assert d_all.numel() >= world * (2 + 2 * self.units)
+        _check(self._L.fitrig_shard_import(self._h, d_all.data_ptr(), int(world), _dev_ptr(d_tlisi),
+                                           _stream_ptr(stream)))
 
     # ---- getters ----
     def get_stats(self):

@@ -351,6 +351,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st) 
   fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
   fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
   fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
+  fp.shard_all = nullptr; fp.shard_world = 0;
   if (c->profile) {
     while ((int)c->fin_pool.size() < 2 * (c->fin_used + 1)) {
       cudaEvent_t e;
@@ -467,6 +468,7 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   cp.mu = freq ? c->smu : c->mu; cp.sigma = freq ? c->ssigma : c->sigma;
   cp.tau = tau; cp.rows = (int)rows; cp.nt = c->nt;
   cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.branch = c->prm.branch;
+  cp.row_offset = c->prm.row_offset;
   cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
   cp.cap = std::min<long long>(c->cand_cap, std::max<long long>(capacity, 0));
   cp.total = reinterpret_cast<unsigned long long*>(c->cand_dev);
@@ -497,6 +499,48 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   *n_found = total;
   if (total > capacity)
     return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)capacity);
+  return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// row shards
+// ---------------------------------------------------------------------------------------------
+extern "C" int fitrig_shard_export(fitrig_ctx* c, double* d_out, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: ctx is NULL");
+  if (!d_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: d_out is NULL");
+  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: row shards support the image branch only");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_shard_export: no current map (call fitrig_tlisi first)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  ShardExportParams ep;
+  ep.raw = c->raw; ep.gmax_key = c->gmax_key + c->key_idx; ep.out = d_out;
+  ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
+  ep.nblk = c->fin_nblk; ep.parts = c->parts; ep.counters = c->counters;
+  shard_export_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(ep);
+  CUDA_TRY(cudaGetLastError());
+  c->launches++;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_shard_import(fitrig_ctx* c, const double* d_all, int32_t world, float* d_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: ctx is NULL");
+  if (!d_all || world < 1) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: d_all is NULL or world < 1");
+  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: row shards support the image branch only");
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_shard_import: no current map (call fitrig_tlisi first)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  FinalizeParams fp;
+  fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi;
+  fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev;
+  fp.M_override = c->prm.M_override; fp.C = c->prm.C;
+  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
+  fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
+  fp.shard_all = d_all; fp.shard_world = world;
+  finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
+  CUDA_TRY(cudaGetLastError());
+  c->launches++;
   return FITRIG_OK;
 }
 

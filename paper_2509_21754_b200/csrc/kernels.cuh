@@ -562,6 +562,9 @@ struct FinalizeParams {
   unsigned* counters;  // [U]
   double* mu;          // [U]
   double* sigma;       // [U]
+  // row-shard mode (fitrig_shard_import): M, mu, sigma come from the all-gathered export vectors
+  const double* shard_all;  // [shard_world][2 + 2U] or NULL
+  int shard_world;
 };
 
 __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
@@ -571,7 +574,15 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
   const long long per = (nt + p.nblk - 1) / p.nblk;
   const long long begin = min(nt, (long long)blockIdx.x * per), end = min(nt, begin + per);
   // M = max(max_s x^(s), C), PAPER.md:223 (R2: signed max), or the caller's override
-  float M = fmaxf(key_to_float(*p.gmax_key), p.C);
+  float M;
+  const int vlen = 2 + 2 * p.U;  // length of one shard's export vector
+  if (p.shard_all) {
+    double m = p.shard_all[0];
+    for (int r = 1; r < p.shard_world; ++r) m = fmax(m, p.shard_all[(size_t)r * vlen]);
+    M = fmaxf((float)m, p.C);  // the entries are fp32 pixel values: the cast is exact
+  } else {
+    M = fmaxf(key_to_float(*p.gmax_key), p.C);
+  }
   if (p.M_override > 0.f) M = p.M_override;
   if (blockIdx.x == 0 && u == 0 && threadIdx.x == 0) {
     *p.M_out = M;
@@ -592,8 +603,84 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
     p.tlisi[base + t] = tl;
     if (p.tlisi_user) p.tlisi_user[base + t] = tl;
   }
+  if (p.shard_all) {
+    // Eq. 8 over ALL tiles of the image from the shards' sums of p = q * M^2, merged in shard order
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+      double n = 0.0, sp = 0.0, sp2 = 0.0;
+      for (int r = 0; r < p.shard_world; ++r) {
+        const double* v = p.shard_all + (size_t)r * vlen;
+        n += v[1];
+        sp += v[2 + u];
+        sp2 += v[2 + p.U + u];
+      }
+      const double mean_p = (n > 0) ? sp / n : 0.0;
+      const double var_p = (n > 0) ? fmax(sp2 / n - mean_p * mean_p, 0.0) : 0.0;
+      p.mu[u] = mean_p * inv_m2;
+      p.sigma[u] = sqrt(var_p) * inv_m2;
+    }
+    return;
+  }
   __syncthreads();  // this block's q values are re-read below (by the same threads, but keep it simple)
   row_stats_block(p.q + base, begin, end, u, p.nblk, p.parts, p.counters, p.mu, p.sigma, sh);
+}
+
+// ---------------------------------------------------------------------------------------------
+// row shards: what the other shards need (fitrig_shard_export)
+// ---------------------------------------------------------------------------------------------
+struct ShardExportParams {
+  const RawTile* raw;
+  const unsigned* gmax_key;
+  double* out;          // [2 + 2U]
+  int H, W, tile, Ty, Tx, U;
+  int nblk;             // blocks per unit
+  StatPartial* parts;   // [U][nblk]
+  unsigned* counters;   // [U]
+};
+
+__global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportParams p) {
+  __shared__ double sh[32];
+  const int u = blockIdx.y;
+  const long long nt = (long long)p.Ty * p.Tx;
+  const long long per = (nt + p.nblk - 1) / p.nblk;
+  const long long begin = min(nt, (long long)blockIdx.x * per), end = min(nt, begin + per);
+  const size_t base = (size_t)u * nt;
+  double s = 0.0, s2 = 0.0;
+  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
+    const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
+    const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
+    const double n_t = (double)h * (double)w;
+    const RawTile r = p.raw[base + t];
+    const double pv = ((double)r.sumD / n_t) * (double)r.maxD * ((double)r.sumR / n_t);  // Eq. 6 without 1/M^2
+    s += pv;
+    s2 += pv * pv;
+  }
+  s = block_sum(s, sh);
+  s2 = block_sum(s2, sh);
+  __shared__ bool is_last;
+  if (threadIdx.x == 0) {
+    StatPartial sp;
+    sp.n = (double)(end - begin); sp.mean = s; sp.m2 = s2;  // here: plain sums
+    p.parts[(size_t)u * p.nblk + blockIdx.x] = sp;
+    __threadfence();
+    is_last = (atomicAdd(&p.counters[u], 1u) == (unsigned)p.nblk - 1);
+  }
+  __syncthreads();
+  if (is_last && threadIdx.x == 0) {
+    __threadfence();
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < p.nblk; ++i) {  // block order: deterministic
+      const volatile StatPartial* sp = &p.parts[(size_t)u * p.nblk + i];
+      a += sp->mean;
+      b += sp->m2;
+    }
+    p.out[2 + u] = a;
+    p.out[2 + p.U + u] = b;
+    p.counters[u] = 0;
+    if (u == 0) {
+      p.out[0] = (double)key_to_float(*p.gmax_key);
+      p.out[1] = (double)nt;
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -663,6 +750,7 @@ struct CompactParams {
   int rows;             // U or 1
   long long nt;         // tiles per row
   int Tx, Ty, H, W, tile, branch;
+  int row_offset;       // image row of this context's first row (row shards), added to y
   fitrig_candidate* out;
   long long cap;        // device capacity of `out`
   unsigned long long* total;
@@ -740,12 +828,12 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
         if (p.branch == FITRIG_BRANCH_IMAGE) {
           const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
           cd.x = tx * p.tile + pos % p.tile;
-          cd.y = ty * p.tile + pos / p.tile;
+          cd.y = p.row_offset + ty * p.tile + pos / p.tile;
           cd.snapshot = row;
         } else {
           const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
           cd.x = tx * p.tile + w / 2;  // tile centre (R18)
-          cd.y = ty * p.tile + h / 2;
+          cd.y = p.row_offset + ty * p.tile + h / 2;
           cd.snapshot = p.kstar[t];
         }
         cd.score = z;

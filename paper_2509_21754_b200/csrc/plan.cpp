@@ -38,6 +38,11 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
     return FITRIG_ERR_INVALID_ARG;
   }
   out->strip_rows = p->strip_rows;
+  if (p->row_offset < 0 || (p->row_offset % out->tile) != 0) {
+    *why = "row_offset must be a non-negative multiple of tile";
+    return FITRIG_ERR_INVALID_ARG;
+  }
+  out->row_offset = p->row_offset;
   return FITRIG_OK;
 }
 

@@ -22,6 +22,7 @@ struct NormParams {  // fitrig_params with defaults applied
   int branch;
   int strip_rows;
   int device;
+  int row_offset;
 };
 
 // Validates and applies defaults.  Returns FITRIG_OK or FITRIG_ERR_INVALID_ARG (+ message in *why).

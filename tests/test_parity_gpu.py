@@ -358,6 +358,74 @@ def test_frequency_branch_odd_length_series():
 
 
 # ------------------------------------------------------------------------------------------
+# row shards: the shards of one image, run one after another on this GPU (no shard waits
+# on another: the exchange vector is simply stacked), must reproduce the whole-image result
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("H,W,world", [(256, 256, 2), (250, 252, 3), (512, 256, 4), (96, 64, 3)])
+def test_row_shards_reproduce_the_whole_image(H, W, world):
+    from paper_2509_21754_b200 import shard
+    cfg = synth.scaled(synth.CONFIGS["tiny"], H, W)
+    st, _ = synth.make_stack(cfg, device=DEV)
+    L, tau = cfg.L, (3.0 if H * W >= 256 * 250 else 1.0)  # 6 tiles cannot reach z = 3 (P7: max z <= sqrt(n-1))
+    whole = gpu_run(st, taus=(tau,))
+    rows = shard.row_shards(H, 32, world)
+    ctxs, vecs = [], []
+    try:
+        for (r0, r1) in rows:
+            ctx = fitrig.Context(r1 - r0, W, L, row_offset=r0)
+            ctxs.append(ctx)
+            ctx.tlisi(st[:, r0:r1].contiguous())
+            v = torch.empty(2 + 2 * (L - 2), dtype=torch.float64, device=DEV)
+            ctx.shard_export(v)
+            vecs.append(v)
+        allv = torch.stack(vecs).contiguous()  # what the all-gather delivers to every shard
+        qs, tls, lists = [], [], []
+        for ctx, (r0, r1) in zip(ctxs, rows):
+            U, Ty, Tx = ctx.map_dims()
+            d_tl = torch.empty((U, Ty, Tx), dtype=torch.float32, device=DEV)
+            ctx.shard_import(allv, world, d_tl)
+            c, n = ctx.detect(tau)
+            M, mu, sd = ctx.get_stats()
+            assert M == whole["M"]
+            np.testing.assert_allclose(mu, whole["mu"], rtol=1e-6)
+            np.testing.assert_allclose(sd, whole["sigma"], rtol=1e-5)
+            qs.append(ctx.get_map(0))
+            tls.append(d_tl.cpu().numpy())
+            lists.append(c.copy())
+            assert all(r0 <= int(y) < r1 for y in c["y"])
+    finally:
+        for ctx in ctxs:
+            ctx.close()
+    assert np.array_equal(np.concatenate(qs, axis=1), whole["q"])  # same raw sums, same M, same fp64 combine
+    assert np.array_equal(np.concatenate(tls, axis=1), whole["tlisi"])
+    merged = shard.merge_candidates(lists)
+    ref_c, ref_n = whole["cands"][tau]
+    # z differs in the last bits (mu, sigma from sums of p instead of the rounded q map): compare outside a 1e-5 band
+    keep = lambda c: {(int(r["snapshot"]), int(r["y"]), int(r["x"])) for r in c if abs(float(r["score"]) - tau) > 1e-5 * 20}
+    assert keep(merged) == keep(ref_c) and ref_n > 0
+    if len(merged) == len(ref_c):
+        assert np.array_equal(merged["x"], ref_c["x"]) and np.array_equal(merged["y"], ref_c["y"])
+        assert np.array_equal(merged["snapshot"], ref_c["snapshot"])
+        np.testing.assert_allclose(merged["score"], ref_c["score"], rtol=1e-4, atol=1e-5)
+
+
+def test_shard_calls_argument_and_state_errors():
+    with fitrig.Context(64, 64, 4) as ctx:
+        v = torch.empty(2 + 2 * 2, dtype=torch.float64, device=DEV)
+        with pytest.raises(fitrig.FitrigError) as e:
+            ctx.shard_export(v)
+        assert e.value.code == fitrig.binding.ERR_STATE
+    with pytest.raises(fitrig.FitrigError) as e:
+        fitrig.Context(64, 64, 4, row_offset=16)  # not a multiple of the tile
+    assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+    with fitrig.Context(64, 64, 4, branch=fitrig.BRANCH_FREQUENCY) as ctx:
+        ctx.tlisi(synth.gaussian_noise_stack(4, 64, 64, device=DEV))
+        with pytest.raises(fitrig.FitrigError) as e:
+            ctx.shard_export(torch.empty(6, dtype=torch.float64, device=DEV))
+        assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------
 # full-size configs, in the launch configuration bench.py times
 # ------------------------------------------------------------------------------------------
 def test_config2_meerkat_full_size_full_oracle():

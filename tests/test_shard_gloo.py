@@ -1,0 +1,131 @@
+"""N > 1 host logic on CPU: world_size-2 (and 3) `gloo` process groups.
+
+The CUDA kernels cannot run here, so every rank stands in for its GPU with the ORACLE restricted to its own
+row shard (tests may use the oracle); what is under test is the product's host side of the sharded path
+(paper_2509_21754_b200/shard.py): the row split, the ONE all-gather of 2 + 2U doubles, the candidate gather
+and the (unit, tile row, tile col) merge -- and that the exchange protocol of include/fitrig.h
+(fitrig_shard_export / fitrig_shard_import) reproduces the whole-image result.  The merge arithmetic of
+fitrig_shard_import is restated below in numpy from its header comment.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import oracle
+import synth
+from paper_2509_21754_b200 import shard
+from paper_2509_21754_b200.binding import CANDIDATE_DTYPE
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _export_vector(stack_rows, tile):
+    """What fitrig_shard_export returns for a shard, from the oracle: M = 1 makes q the M-free product p."""
+    r = oracle.tlisi(stack_rows, tile=tile, M=1.0)
+    U = r.U
+    mx = max(float(s.max()) for s in stack_rows)
+    v = np.zeros(2 + 2 * U)
+    v[0], v[1] = mx, r.Ty * r.Tx
+    v[2:2 + U] = r.q.reshape(U, -1).sum(axis=1)
+    v[2 + U:] = (r.q.reshape(U, -1) ** 2).sum(axis=1)
+    return v, r
+
+
+def _import(allv, U, C=1e-6):
+    """fitrig_shard_import's merge, restated from include/fitrig.h."""
+    M = max(float(np.float32(allv[:, 0].max())), C)
+    n = allv[:, 1].sum()
+    mean_p = allv[:, 2:2 + U].sum(axis=0) / n
+    var_p = np.maximum(allv[:, 2 + U:].sum(axis=0) / n - mean_p ** 2, 0.0)
+    return M, mean_p / M ** 2, np.sqrt(var_p) / M ** 2
+
+
+def _worker(rank, world, port, H, W, L, tile, tau, ret):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        oracle.set_threads(1)
+        cfg = synth.scaled(synth.CONFIGS["tiny"], H, W, L=L)
+        st, _ = synth.make_stack(cfg, device="cpu")  # same seed on every rank: the same image
+        full = [st[s].numpy() for s in range(L)]
+        r0, r1 = shard.row_shards(H, tile, world)[rank]
+        rows = [np.ascontiguousarray(x[r0:r1]) for x in full]
+        v, res = _export_vector(rows, tile)
+        allv = shard.all_gather_vectors(torch.from_numpy(v)).numpy()  # the ONE exchange
+        assert allv.shape == (world, 2 + 2 * (L - 2)) and np.array_equal(allv[rank], v)
+        M, mu, sd = _import(allv, L - 2)
+        q = res.q / M ** 2
+        z = (q - mu[:, None, None]) / sd[:, None, None]
+        sel = oracle.select(z, res.argmax, W, tau)
+        local = np.zeros(len(sel.x), dtype=CANDIDATE_DTYPE)
+        local["x"], local["y"], local["snapshot"], local["score"] = sel.x, sel.y + r0, sel.snapshot, sel.score
+        merged = shard.merge_candidates(shard.gather_candidates(local))
+        t_max = shard.max_over_ranks(10.0 + rank)
+        assert t_max == 10.0 + world - 1
+        # whole-image oracle, on every rank
+        ref = oracle.run(full, tile=tile, tau=tau)
+        assert abs(M - ref.res.M) <= 1e-12 * ref.res.M
+        np.testing.assert_allclose(mu, ref.mu, rtol=1e-10)
+        np.testing.assert_allclose(sd, ref.sigma, rtol=1e-8)
+        ty0 = r0 // tile
+        np.testing.assert_allclose(q, ref.res.q[:, ty0:ty0 + res.Ty], rtol=1e-12)
+        assert len(merged) == ref.cands.n_found > 0
+        assert np.array_equal(merged["x"], ref.cands.x) and np.array_equal(merged["y"], ref.cands.y)
+        assert np.array_equal(merged["snapshot"], ref.cands.snapshot)
+        np.testing.assert_allclose(merged["score"], ref.cands.score, rtol=1e-5)
+        ret[rank] = len(merged)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,H,W,tile", [(2, 256, 256, 32), (2, 250, 252, 32), (3, 200, 96, 8)])
+def test_row_sharded_image_over_gloo(world, H, W, tile):
+    mgr = mp.Manager()
+    ret = mgr.dict()
+    mp.spawn(_worker, args=(world, _free_port(), H, W, 8, tile, 3.0, ret), nprocs=world, join=True)
+    assert len(ret) == world and len(set(ret.values())) == 1
+
+
+def test_split_range_and_row_shards():
+    for n in (0, 1, 7, 16, 1563):
+        for world in (1, 2, 3, 8):
+            parts = [shard.split_range(n, world, r) for r in range(world)]
+            assert parts[0][0] == 0 and parts[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(parts, parts[1:]))
+            assert max(hi - lo for lo, hi in parts) - min(hi - lo for lo, hi in parts) <= 1
+    rows = shard.row_shards(50000, 32, 8)  # config 4 over 8 GPUs: 1563 tile rows, the last one 16 px
+    assert rows[0][0] == 0 and rows[-1][1] == 50000
+    assert all(a[1] == b[0] and a[0] % 32 == 0 for a, b in zip(rows, rows[1:]))
+    assert {(r1 - r0 + 31) // 32 for r0, r1 in rows} <= {195, 196}
+    assert shard.row_shards(40, 32, 4) == [(0, 0), (0, 32), (32, 32), (32, 40)]  # more ranks than tile rows
+    with pytest.raises(ValueError):
+        shard.split_range(4, 2, 2)
+
+
+def test_merge_candidates_orders_by_unit_then_shard():
+    a = np.array([(5, 3, 0, 7.0), (9, 40, 2, 6.5)], dtype=CANDIDATE_DTYPE)      # shard 0: rows 0..63
+    b = np.array([(1, 70, 0, 8.0), (2, 100, 1, 9.0), (3, 65, 2, 6.1)], dtype=CANDIDATE_DTYPE)  # shard 1
+    m = shard.merge_candidates([a, b])
+    assert [(int(r["snapshot"]), int(r["y"])) for r in m] == [(0, 3), (0, 70), (1, 100), (2, 40), (2, 65)]
+    assert len(shard.merge_candidates([])) == 0
+    assert len(shard.merge_candidates([a[:0], b[:0]])) == 0
+
+
+def test_single_process_fallbacks_need_no_process_group():
+    v = torch.arange(6, dtype=torch.float64)
+    assert shard.all_gather_vectors(v).shape == (1, 6)
+    assert shard.max_over_ranks(3.5) == 3.5
+    c = np.array([(1, 2, 3, 4.0)], dtype=CANDIDATE_DTYPE)
+    assert np.array_equal(shard.gather_candidates(c)[0], c)
