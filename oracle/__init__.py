@@ -233,3 +233,30 @@ def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Opti
     mu, sd, z = zscore(eta[None])
     c = select_spectrum(z[0], ks, H, W, tile, tau)
     return DetectResult(res, mu, sd, z[0], c, eta, ks)
+
+
+def run_realtime(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, tau: float = 5.0) -> List[DetectResult]:
+    """Real-time (snapshot-by-snapshot) form of the image branch, one DetectResult per unit n = 0..L-3.
+
+    PAPER.md:189 (section 2.2.3): "For real-time processing, this maximum can be estimated from at least three
+    past snapshots"; PAPER.md:457 (section 3.2, Fig. 14): unit n is computed as soon as x_n, x_{n+1}, x_{n+2} are
+    on the device.  Reading (R24): the normaliser of unit n is the running maximum of everything
+    seen when the unit is computed, M_n = max(max pixel of x_0 .. x_{n+2}, C) -- at least three snapshots, the
+    same rule as the batch M (R2, R14) restricted to the past.  Everything else is O2-O7 on the three
+    snapshots of the unit; candidate.snapshot = n.
+    """
+    snaps = as_snapshots(stack)
+    L = len(snaps)
+    if L < 3:
+        raise ValueError("need L >= 3 snapshots (PAPER.md:155)")
+    H, W = snaps[0].shape
+    out = []
+    running = max(float(np.max(snaps[0])), float(np.max(snaps[1])))
+    for n in range(L - 2):
+        running = max(running, float(np.max(snaps[n + 2])))  # x_{n+2} has just arrived
+        res = tlisi(snaps[n:n + 3], tile, C, ref_mode, M=max(running, C))
+        mu, sd, z = zscore(res.q)
+        c = select(z, res.argmax, W, tau)
+        c.snapshot[:] = n
+        out.append(DetectResult(res, mu, sd, z, c))
+    return out

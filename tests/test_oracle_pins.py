@@ -324,3 +324,47 @@ def test_candidates_are_ordered_and_capacity_is_honoured():
 def test_bad_arguments():
     with pytest.raises(ValueError):
         oracle.tlisi(_noise_stack(2, 8, 8), tile=4)  # R10: L < 3
+
+
+# ------------------------------------------------------------------------------------------
+# real-time form (R24): running maximum M_n, one unit per new snapshot
+# ------------------------------------------------------------------------------------------
+def test_realtime_running_maximum_closed_form_and_batch_equivalence():
+    L, H, W = 7, 32, 48
+    rng = np.random.default_rng(5)
+    st = rng.normal(size=(L, H, W)).astype(np.float32)
+    st = np.clip(st, -0.9, 0.9)
+    peaks = [1.0, 4.0, 2.0, 3.0, 8.0, 5.0, 6.0]  # largest pixel of snapshot s
+    for s, p in enumerate(peaks):
+        st[s, 3 + s, 5] = p
+    rt = oracle.run_realtime(st, tile=16, tau=1.0)
+    batch = oracle.run(st, tile=16, tau=1.0)
+    assert [r.res.M for r in rt] == [4.0, 4.0, 8.0, 8.0, 8.0]  # max of peaks[0 .. n+2], written out by hand
+    assert rt[-1].res.M == batch.res.M
+    for n, r in enumerate(rt):
+        # q scales with 1/M^2 only (Eq. 2): q_n M_n^2 == q_batch M^2; z, hence the selection, is M-free (P7)
+        np.testing.assert_allclose(r.res.q[0] * r.res.M ** 2, batch.res.q[n] * batch.res.M ** 2, rtol=1e-13)
+        np.testing.assert_allclose(r.z[0], batch.z[n], rtol=1e-9, atol=1e-12)
+        assert np.array_equal(r.res.argmax[0], batch.res.argmax[n])
+        assert set(r.cands.snapshot.tolist()) <= {n}
+    got = sorted((int(u), int(t)) for r in rt for u, t in zip(r.cands.snapshot, r.cands.tile))
+    exp = sorted((int(u), int(t)) for u, t in zip(batch.cands.snapshot, batch.cands.tile))
+    assert got == exp and len(exp) > 0
+
+
+def test_realtime_single_pixel_transient_closed_form():
+    # P8 with the running maximum: background b, one pixel +A in snapshot k only.  Unit k-2 (the transient is its
+    # third snapshot) already sees M = b + A; units before it see M = b and have q = 0.
+    L, H, W, tile, b, A, k = 8, 16, 16, 8, 4.0, 3.0, 4
+    st = np.full((L, H, W), b, dtype=np.float32)
+    st[k, 9, 2] += A
+    rt = oracle.run_realtime(st, tile=tile, tau=0.5)
+    n_t = tile * tile
+    q_expected = A * A * min(A / b, 1.0) / (n_t ** 2 * (b + A) ** 2)
+    for n, r in enumerate(rt):
+        assert r.res.M == (b if n < k - 2 else b + A)
+        q = r.res.q[0]
+        if n in (k - 2, k):
+            assert abs(q[1, 0] - q_expected) <= 1e-15 and np.count_nonzero(q) == 1
+        else:
+            assert not q.any()
