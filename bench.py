@@ -332,6 +332,33 @@ def run_fitrig(args, cfg, tau, branch):
                "roofline": {"bound": "pcie", "achieved": 4 * pix / (e_ms * 1e-3) / 1e9, "peak": h2d_gbs,
                             "unit": "GB/s", "frac": (4 * pix / (e_ms * 1e-3) / 1e9 / h2d_gbs) if h2d_gbs else None,
                             "peak_source": "pinned 1 GiB cudaMemcpyAsync H2D, best of 10, this run"}}
+        # ---- real-time leg: fitrig_push, one snapshot per call from pinned host memory (Fig. 14 timeline) ----
+        if branch == 0:
+            pctx = fitrig.Context(H, W, 3, device=local)
+            snaps0 = hosts[0]
+
+            def push_pass():
+                tot = 0
+                for s_ in snaps0 + [None]:
+                    u_, c_, n_ = pctx.push(s_, tau, None, cap, stream, out=out)
+                    tot += n_
+                pctx.push_reset()
+                return tot
+
+            push_pass()
+            barrier()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(stream)
+            t_wall = time.perf_counter()
+            n_rt = push_pass()
+            g1.record(stream)
+            barrier()
+            p_ms = shard.max_over_ranks((time.perf_counter() - t_wall) * 1e3, dev)
+            e2e["realtime"] = {"value": world * L * H * W / (p_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_snapshot": p_ms / L,
+                               "api": "fitrig_push (one pinned host snapshot per call, running M, candidates per unit)",
+                               "candidates": int(n_rt), "h2d_gbs": 4 * L * H * W / (p_ms * 1e-3) / 1e9,
+                               "timer": "host wall clock around the pass (every push synchronises)"}
+            pctx.close()
         del hosts
 
     # ---- the oracle beside it (rank 0, N = 1 only) ----

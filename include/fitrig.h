@@ -144,6 +144,32 @@ int fitrig_detect(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate* h_ou
  * buffers: strip i+1 is copied while strip i is reduced.  Errors: INVALID_ARG, NOMEM, CUDA. */
 int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream);
 
+/* Real-time mode ("for real-time processing, this maximum can be estimated from at least
+ * three past snapshots"; timeline of Fig. 14: while the n-th tLISI is computed the
+ * (n+3)-th snapshot is loaded).  The context must have been created with n_snapshots = 3 (one unit per
+ * push, maps are [1][Ty][Tx]), image branch.
+ *
+ * fitrig_push -- feed ONE new H x W snapshot (host, pinned for overlap, or device; NULL to flush) and get
+ * the result of the unit whose three snapshots had been pushed BEFORE this call:
+ *   - the copy of `snapshot` into a device ring of 4 snapshots is started on a private stream, and
+ *   - overlapped with it, unit n = x_n, x_{n+1}, x_{n+2} (0-based push order) is computed on
+ *     `cuda_stream`: steps a1-a8 with M_n = max(largest pixel of x_0 .. x_{n+2}, C), the running maximum
+ *     of everything seen so far (z and therefore the candidates do not depend on M).
+ *   *unit (host)    index n of the unit computed by this call, or -1 (the first three pushes; or nothing left)
+ *   d_tlisi (device) [Ty][Tx] tLISI of that unit, may be NULL
+ *   h_out, capacity, n_found  as fitrig_detect; candidate.snapshot = n
+ * So push(x_0), push(x_1), push(x_2) return unit = -1; push(x_3) returns unit 0; ...; push(NULL) returns
+ * the last unit.  After a call with unit >= 0 the context's current map is that unit's (getters work).
+ * The copy is asynchronous: a pushed buffer must stay valid and unchanged until the NEXT fitrig_push that
+ * returns a unit >= 0 has returned (or until fitrig_push_reset).  Synchronises `cuda_stream` when a unit
+ * is computed.  Errors: INVALID_ARG (context not created with 3 snapshots / frequency branch),
+ * NOMEM, CUDA, CAPACITY.
+ *
+ * fitrig_push_reset -- forget all pushed snapshots and the running maximum (synchronises the device). */
+int fitrig_push(fitrig_ctx* ctx, const float* snapshot, float sigma_threshold, float* d_tlisi,
+                fitrig_candidate* h_out, int64_t capacity, int64_t* n_found, int64_t* unit, void* cuda_stream);
+int fitrig_push_reset(fitrig_ctx* ctx);
+
 /* Row shards (tiles are independent).  One image is cut into
  * horizontal shards of whole tile rows, one context (normally one GPU) per shard, each created with the
  * shard's own H and params.row_offset.  Only the three global scalars of the method couple the shards:

@@ -100,6 +100,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_tlisi.argtypes = [vp, vp, vp, vp]
     L.fitrig_detect.argtypes = [vp, f32, vp, i64, P(i64), vp]
     L.fitrig_stream.argtypes = [vp, P(vp), vp, vp]
+    L.fitrig_push.argtypes = [vp, vp, f32, vp, vp, i64, P(i64), P(i64), vp]
+    L.fitrig_push_reset.argtypes = [vp]
     L.fitrig_shard_export.argtypes = [vp, vp, vp]
     L.fitrig_shard_import.argtypes = [vp, vp, i32, vp, vp]
     L.fitrig_get_stats.argtypes = [vp, P(f32), vp, vp]
@@ -109,7 +111,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
-              "fitrig_detect", "fitrig_stream", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
+              "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
               "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
@@ -238,6 +240,25 @@ class Context:
         if h_tlisi is not None:
             out = h_tlisi.data_ptr() if hasattr(h_tlisi, "data_ptr") else h_tlisi.ctypes.data
         _check(self._L.fitrig_stream(self._h, arr, out, _stream_ptr(stream)))
+
+    # ---- real-time mode ----
+    def push(self, snapshot, sigma_threshold: float, d_tlisi=None, capacity: int = 1 << 16, stream=None,
+             out: Optional[np.ndarray] = None):
+        """snapshot: [H, W] fp32 host (pinned) or CUDA tensor, or None to flush.  Returns (unit, candidates, n_found);
+        unit = -1 while fewer than three snapshots had been pushed before this call."""
+        ptr = 0
+        if snapshot is not None:
+            ptr = snapshot.data_ptr() if hasattr(snapshot, "data_ptr") else snapshot.ctypes.data
+        if out is None:
+            out = np.zeros(max(capacity, 1), dtype=CANDIDATE_DTYPE)
+        n, u = ctypes.c_int64(0), ctypes.c_int64(-1)
+        _check(self._L.fitrig_push(self._h, ptr, float(sigma_threshold), _dev_ptr(d_tlisi), out.ctypes.data,
+                                   int(capacity), ctypes.byref(n), ctypes.byref(u), _stream_ptr(stream)),
+               allow=(ERR_CAPACITY,))
+        return u.value, out[: min(n.value, capacity)], n.value
+
+    def push_reset(self) -> None:
+        _check(self._L.fitrig_push_reset(self._h))
 
     # ---- row shards ----
     def shard_export(self, d_out, stream=None) -> None:

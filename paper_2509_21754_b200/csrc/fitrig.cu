@@ -52,6 +52,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 static const int kMaxStripBuffers = 3;
+static const int kPushSlots = 4;  // x_n, x_{n+1}, x_{n+2} of the unit being computed + the snapshot being copied
 static const long long kHostStageCands = 4096;  // candidates fetched together with the count
 
 struct CandHeader {
@@ -99,6 +100,13 @@ struct fitrig_ctx {
   cudaStream_t copy_stream;
   cudaEvent_t ev_copied[kMaxStripBuffers], ev_free[kMaxStripBuffers], ev_entry;
   bool ev_free_pending[kMaxStripBuffers];
+  // real-time mode (fitrig_push): ring of kPushSlots whole snapshots, running-maximum key, Fig. 14 timeline
+  float* push_ring;
+  unsigned* push_key;
+  long long push_count;  // snapshots pushed so far
+  long long push_next;   // next unit to compute
+  cudaEvent_t ev_push_copied[4], ev_push_free[4];
+  bool push_free_pending[4];
   // profiling
   bool profile;
   std::vector<cudaEvent_t> ev_pool;   // pairs: start, stop of each main-kernel launch since the last read
@@ -122,6 +130,11 @@ static void free_ctx(fitrig_ctx* c) {
     cudaFree(c->strip_buf[i]);
     if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
     if (c->ev_free[i]) cudaEventDestroy(c->ev_free[i]);
+  }
+  cudaFree(c->push_ring); cudaFree(c->push_key);
+  for (int i = 0; i < kPushSlots; ++i) {
+    if (c->ev_push_copied[i]) cudaEventDestroy(c->ev_push_copied[i]);
+    if (c->ev_push_free[i]) cudaEventDestroy(c->ev_push_free[i]);
   }
   if (c->ev_entry) cudaEventDestroy(c->ev_entry);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -272,9 +285,16 @@ static int prof_end(fitrig_ctx* c, cudaStream_t st) {
 
 // tLISI partial sums of `rows` image rows (all L snapshots) that start at tile row ty_base.
 // base: device pointer to snapshot 0 of those rows; snap_stride: elements between snapshots.
+struct RowsOpt {
+  int z0 = 0, zmod = 0;     // real-time ring: snapshot s of the launch is slot (z0 + s) % zmod of `base`
+  unsigned* key = nullptr;  // global-maximum key to fold into (default: the key of the current call)
+};
+
 static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int ty_base,
-                             bool with_max, cudaStream_t st) {
+                             bool with_max, cudaStream_t st, const RowsOpt& opt = RowsOpt()) {
   const int tile = c->prm.tile;
+  unsigned* key = opt.key ? opt.key : c->gmax_key + c->key_idx;
+  const int nslots = opt.zmod ? opt.zmod : c->L;
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
@@ -285,7 +305,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   if (rc) return rc;
   if (pl.path == 0) {
     CUtensorMap tm;
-    const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)c->L};
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)nslots};
     const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
     const cuuint32_t box[3] = {(cuuint32_t)(pl.box_tiles * kFastTile), kFastTile, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
@@ -294,7 +314,8 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
-    fp.raw = c->raw; fp.gmax_key = c->gmax_key + c->key_idx;
+    fp.raw = c->raw; fp.gmax_key = key;
+    fp.z0 = opt.z0; fp.zmod = opt.zmod;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
     fp.U = c->U;
@@ -316,8 +337,9 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     if (with_max) {
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
       for (int s = 0; s < c->L; ++s) {
-        stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)s * snap_stride,
-                                                                       (long long)rows * c->W, c->gmax_key + c->key_idx);
+        const int slot = opt.zmod ? (opt.z0 + s) % opt.zmod : s;
+        stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)slot * snap_stride,
+                                                                       (long long)rows * c->W, key);
         CUDA_TRY(cudaGetLastError());
         c->launches++;
       }
@@ -329,6 +351,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     const long long n_t = (long long)tile * tile;
     while (G < 32 && G < n_t) G <<= 1;
     gp.G = G;
+    gp.z0 = opt.z0; gp.zmod = opt.zmod;
     gp.C = c->prm.C;
     const long long groups = (long long)rows_tiles * c->Tx * c->U;
     const long long threads = groups * G;
@@ -345,10 +368,11 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   return prof_end(c, st);
 }
 
-static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st) {
+static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, unsigned* key = nullptr) {
   FinalizeParams fp;
   fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
-  fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
+  fp.gmax_key = key ? key : c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1);
+  fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
   fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
   fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
   fp.shard_all = nullptr; fp.shard_world = 0;
@@ -432,8 +456,16 @@ extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, flo
   return FITRIG_OK;
 }
 
+static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
+                       void* cuda_stream, int unit_offset);
+
 extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
                              void* cuda_stream) {
+  return detect_core(c, tau, h_out, capacity, n_found, cuda_stream, 0);
+}
+
+static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
+                       void* cuda_stream, int unit_offset) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: ctx is NULL");
   if (!n_found) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: n_found is NULL");
   if (capacity < 0 || (capacity > 0 && !h_out)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: bad h_out/capacity");
@@ -469,6 +501,7 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   cp.tau = tau; cp.rows = (int)rows; cp.nt = c->nt;
   cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.branch = c->prm.branch;
   cp.row_offset = c->prm.row_offset;
+  cp.unit_offset = unit_offset;
   cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
   cp.cap = std::min<long long>(c->cand_cap, std::max<long long>(capacity, 0));
   cp.total = reinterpret_cast<unsigned long long*>(c->cand_dev);
@@ -500,6 +533,77 @@ extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, 
   if (total > capacity)
     return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)capacity);
   return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// real-time mode (timeline of Fig. 14)
+// ---------------------------------------------------------------------------------------------
+extern "C" int fitrig_push_reset(fitrig_ctx* c) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push_reset: ctx is NULL");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  if (c->push_key) CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
+  c->push_count = 0;
+  c->push_next = 0;
+  for (int i = 0; i < kPushSlots; ++i) c->push_free_pending[i] = false;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, float* d_tlisi, fitrig_candidate* h_out,
+                           int64_t capacity, int64_t* n_found, int64_t* unit, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: ctx is NULL");
+  if (!n_found || !unit) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: n_found or unit is NULL");
+  if (c->L != 3) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: create the context with n_snapshots = 3 (one unit per push)");
+  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: the real-time mode is the image branch (Eq. 8-9)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  const long long img = (long long)c->H * c->W;
+  if (!c->push_ring) {
+    CUDA_TRY(cudaMalloc(&c->push_ring, sizeof(float) * img * kPushSlots));
+    CUDA_TRY(cudaMalloc(&c->push_key, sizeof(unsigned)));
+    CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
+    for (int i = 0; i < kPushSlots; ++i) {
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_copied[i], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_free[i], cudaEventDisableTiming));
+    }
+    if (!c->copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    if (!c->ev_entry) CUDA_TRY(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
+  }
+  *unit = -1;
+  *n_found = 0;
+  // (1) the new snapshot starts its way to the device (host pinned memory, or a device pointer) ...
+  if (snapshot) {
+    const int slot = (int)(c->push_count % kPushSlots);
+    CUDA_TRY(cudaEventRecord(c->ev_entry, st));  // the copy may not overtake work already queued by the caller
+    CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
+    if (c->push_free_pending[slot]) CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_push_free[slot], 0));
+    CUDA_TRY(cudaMemcpyAsync(c->push_ring + (long long)slot * img, snapshot, sizeof(float) * img, cudaMemcpyDefault,
+                             c->copy_stream));
+    CUDA_TRY(cudaEventRecord(c->ev_push_copied[slot], c->copy_stream));
+  }
+  // (2) ... while the unit whose three snapshots were pushed BEFORE this call is computed (Fig. 14: copy of
+  // snapshot n+3 overlaps trigger kernel n)
+  const long long n = c->push_next;
+  int rc = FITRIG_OK;
+  if (n + 3 <= c->push_count) {
+    for (int k = 0; k < 3; ++k) CUDA_TRY(cudaStreamWaitEvent(st, c->ev_push_copied[(n + k) % kPushSlots], 0));
+    RowsOpt opt;
+    opt.z0 = (int)(n % kPushSlots); opt.zmod = kPushSlots; opt.key = c->push_key;
+    rc = launch_tlisi_rows(c, c->push_ring, img, c->H, 0, true, st, opt);
+    if (rc) return rc;
+    CUDA_TRY(cudaEventRecord(c->ev_push_free[n % kPushSlots], st));  // x_n is not needed again
+    c->push_free_pending[n % kPushSlots] = true;
+    rc = launch_finalize(c, d_tlisi, st, c->push_key);  // M = running maximum over x_0 .. x_{n+2}
+    if (rc) return rc;
+    if (n + 1 > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: unit index overflow");
+    rc = detect_core(c, tau, h_out, capacity, n_found, cuda_stream, (int)n);
+    if (rc != FITRIG_OK && rc != FITRIG_ERR_CAPACITY) return rc;
+    *unit = n;
+    c->push_next = n + 1;
+  }
+  if (snapshot) c->push_count++;
+  return rc;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -142,8 +142,11 @@ struct FusedParams {
   int nstage;            // depth of the CTA's ring of boxes
   int G;                 // rows_tiles * ngx * U: (box column, unit) pairs of this launch, box-major
   int evict_first;       // L2 policy of the streaming loads
+  int z0, zmod;          // real-time mode: snapshot s of the launch lives in slot (z0 + s) % zmod of a ring; zmod = 0: slot s
   float C;
 };
+
+__device__ __forceinline__ int ring_slot(int z0, int zmod, int s) { return zmod ? (z0 + s) % zmod : s; }
 
 // Work distribution: a "group" is a row of ntw horizontally adjacent tiles, fetched as ONE TMA box of
 // 32 rows x (ntw * 128) contiguous bytes (isolated 128-byte rows cost ~15 % of the HBM bandwidth, see
@@ -292,10 +295,10 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
           mbar_arrive_expect_tx(bar, box_bytes);
           if (p.evict_first)
             tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                              c.u0 + s, policy);
+                              ring_slot(p.z0, p.zmod, c.u0 + s), policy);
           else
             tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                         c.u0 + s);
+                         ring_slot(p.z0, p.zmod, c.u0 + s));
           if (++slot == p.nstage) { slot = 0; phase ^= 1; }
         }
       }
@@ -370,11 +373,10 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       *reinterpret_cast<unsigned long long*>(&scratch[4]) =
           ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + tx;
       // the winning group's 4 pixels in x_u, x_{u+1}, x_{u+2}: in bounds (a zero-filled pixel has Delta 0)
-      const float* src = p.base + (long long)u * p.snap_stride +
-                         (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
-      cp_async16(scratch_addr, src);
-      cp_async16(scratch_addr + 16, src + p.snap_stride);
-      cp_async16(scratch_addr + 32, src + 2 * p.snap_stride);
+      const float* src = p.base + (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
+      cp_async16(scratch_addr, src + (long long)ring_slot(p.z0, p.zmod, u) * p.snap_stride);
+      cp_async16(scratch_addr + 16, src + (long long)ring_slot(p.z0, p.zmod, u + 1) * p.snap_stride);
+      cp_async16(scratch_addr + 32, src + (long long)ring_slot(p.z0, p.zmod, u + 2) * p.snap_stride);
       cp_async_commit();
     }
     pend = true;
@@ -423,6 +425,7 @@ struct GenericParams {
   RawTile* raw;
   int Tx, Ty, ty_base, rows_tiles, U;
   int G;                    // lanes per tile
+  int z0, zmod;             // real-time mode ring (see FusedParams)
   float C;
 };
 
@@ -444,9 +447,9 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
     tx = (int)(t - (long long)ty_local * p.Tx);
     const int r0 = ty_local * p.tile, c0 = tx * p.tile;
     const int h = min(p.tile, p.rows - r0), w = min(p.tile, p.W - c0);
-    const float* x0 = p.base + (long long)u * p.snap_stride;
-    const float* x1 = x0 + p.snap_stride;
-    const float* x2 = x1 + p.snap_stride;
+    const float* x0 = p.base + (long long)ring_slot(p.z0, p.zmod, u) * p.snap_stride;
+    const float* x1 = p.base + (long long)ring_slot(p.z0, p.zmod, u + 1) * p.snap_stride;
+    const float* x2 = p.base + (long long)ring_slot(p.z0, p.zmod, u + 2) * p.snap_stride;
     bool first = true;
     for (int i = gl; i < h * w; i += p.G) {
       const int r = i / w, c = i - r * w;
@@ -751,6 +754,7 @@ struct CompactParams {
   long long nt;         // tiles per row
   int Tx, Ty, H, W, tile, branch;
   int row_offset;       // image row of this context's first row (row shards), added to y
+  int unit_offset;      // real-time mode: index of the unit the one-row map belongs to, added to `snapshot`
   fitrig_candidate* out;
   long long cap;        // device capacity of `out`
   unsigned long long* total;
@@ -829,7 +833,7 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
           const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
           cd.x = tx * p.tile + pos % p.tile;
           cd.y = p.row_offset + ty * p.tile + pos / p.tile;
-          cd.snapshot = row;
+          cd.snapshot = row + p.unit_offset;
         } else {
           const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
           cd.x = tx * p.tile + w / 2;  // tile centre (R18)

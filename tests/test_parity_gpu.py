@@ -358,6 +358,68 @@ def test_frequency_branch_odd_length_series():
 
 
 # ------------------------------------------------------------------------------------------
+# real-time mode: fitrig_push (PAPER.md:189 running maximum; Fig. 14 timeline), against oracle.run_realtime
+# ------------------------------------------------------------------------------------------
+def _push_all(ctx, snaps, tau, want_maps=True):
+    """Feed every snapshot, then flush; returns {unit: (cands, n, q, M, mu, sigma, tlisi)} in arrival order."""
+    U, Ty, Tx = ctx.map_dims()
+    got = {}
+    d_tl = torch.empty((Ty, Tx), dtype=torch.float32, device=DEV)
+    for s in list(snaps) + [None]:
+        unit, c, n = ctx.push(s, tau, d_tl)
+        if unit >= 0:
+            assert unit == len(got)  # units come out in order, one per push
+            M, mu, sd = ctx.get_stats()
+            got[unit] = (c.copy(), n, ctx.get_map(0)[0] if want_maps else None, M, mu[0], sd[0], d_tl.cpu().numpy())
+    unit, c, n = ctx.push(None, tau)  # nothing left
+    assert unit == -1 and n == 0
+    return got
+
+
+@pytest.mark.parametrize("H,W,tile,on_device", [(256, 256, 32, False), (250, 252, 32, False), (256, 256, 32, True),
+                                                (120, 100, 8, False)])
+def test_push_realtime_matches_oracle(tiny, H, W, tile, on_device):
+    st, _ = tiny
+    st = st[:, :H, :W].contiguous()
+    L, tau = st.shape[0], 3.0
+    snaps = [st[s] for s in range(L)] if on_device else [st[s].cpu().pin_memory() for s in range(L)]
+    ref = oracle.run_realtime(st.cpu().numpy(), tile=tile, tau=tau)
+    with fitrig.Context(H, W, 3, tile=tile) as ctx:
+        assert ctx.map_dims()[0] == 1
+        first = ctx.push(snaps[0], tau)
+        assert first[0] == -1 and first[2] == 0
+        ctx.push_reset()
+        got = _push_all(ctx, snaps, tau)
+        assert sorted(got) == list(range(L - 2))
+        stack_np = st.cpu().numpy()
+        for n, (c, cnt, q, M, mu, sd, tl) in got.items():
+            r = ref[n]
+            assert M == np.float32(r.res.M)  # running maximum of x_0 .. x_{n+2}
+            util.assert_map_close(q, r.res.q[0], tl, r.res.tlisi[0])
+            assert abs(mu - r.mu[0]) <= 1e-5 * abs(r.mu[0]) and abs(sd - r.sigma[0]) <= 2e-4 * r.sigma[0]
+            Tx = r.res.Tx
+            lst = [(int(k["x"]), int(k["y"]), int(k["snapshot"]), float(k["score"]),
+                    (int(k["y"]) // tile) * Tx + int(k["x"]) // tile, 0) for k in c]
+            assert all(k[2] == n for k in lst) and cnt == len(c)
+            util.compare_candidates(lst, r.z, r.mu, r.sigma, tau, Tx, r.res.Ty * Tx)
+            for (x, y, u, score, t, _) in lst:
+                assert oracle_delta_at(stack_np, n, x, y) >= (1 - 1e-5) * r.res.maxD[0].flat[t]
+        assert sum(v[1] for v in got.values()) > 0
+        # a second pass after a reset reproduces the first bit for bit
+        ctx.push_reset()
+        again = _push_all(ctx, snaps, tau)
+        for n in got:
+            assert np.array_equal(got[n][2], again[n][2]) and np.array_equal(got[n][0], again[n][0])
+
+
+def test_push_needs_a_three_snapshot_context():
+    with fitrig.Context(64, 64, 5) as ctx:
+        with pytest.raises(fitrig.FitrigError) as e:
+            ctx.push(torch.zeros(64, 64, device=DEV), 3.0)
+        assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------
 # row shards (DESIGN.md section 9): the shards of one image, run one after another on this GPU (no shard waits
 # on another: the exchange vector is simply stacked), must reproduce the whole-image result
 # ------------------------------------------------------------------------------------------
