@@ -50,6 +50,8 @@ def lib() -> ctypes.CDLL:
         L.fitrig_oracle_tlisi.argtypes = [c_f32pp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_double, ctypes.c_int, ctypes.c_double,
                                           dp, dp, dp, ip64, dp, dp]
+        L.fitrig_oracle_tlisi_f64.restype = ctypes.c_int
+        L.fitrig_oracle_tlisi_f64.argtypes = L.fitrig_oracle_tlisi.argtypes
         L.fitrig_oracle_zscore.restype = None
         L.fitrig_oracle_zscore.argtypes = [dp, ctypes.c_int, ctypes.c_int64, dp, dp, dp]
         L.fitrig_oracle_select.restype = ctypes.c_int64
@@ -119,8 +121,29 @@ class TlisiResult:
     tlisi: np.ndarray
 
 
-def tlisi(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None) -> TlisiResult:
-    """Eq. 2-6 for every unit and tile.  M=None -> O1 global max of the given stack (floored at C)."""
+def accumulate(stack, g: int) -> List[np.ndarray]:
+    """Snapshot accumulation, PAPER.md:497 (section 3.3.2) and Fig. 16 ("adding the two snapshots together and
+    outputting their sum", applied progressively): A_j = x_{gj} + x_{gj+1} + ... + x_{gj+g-1}, j = 0 .. L//g - 1,
+    summed in fp64 in snapshot order.  Reading R25: g is any integer >= 1 (the figure's pairwise tree
+    gives g = 2^m); the trailing L mod g snapshots do not form a complete group and are left out."""
+    snaps = as_snapshots(stack)
+    if g < 1:
+        raise ValueError("accumulate: g >= 1")
+    out = []
+    for j in range(len(snaps) // g):
+        a = np.zeros(snaps[0].shape, dtype=np.float64)
+        for i in range(g):
+            a += snaps[g * j + i].astype(np.float64)
+        out.append(a)
+    return out
+
+
+def tlisi(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
+          accumulate_g: int = 1) -> TlisiResult:
+    """Eq. 2-6 for every unit and tile.  M=None -> O1 global max of the images tLISI assesses (floored at C).
+    accumulate_g > 1: the images are the accumulated snapshots A_j, in fp64."""
+    if accumulate_g > 1:
+        return _tlisi_f64(accumulate(stack, accumulate_g), tile, C, ref_mode, M)
     snaps = as_snapshots(stack)
     L = len(snaps)
     H, W = snaps[0].shape
@@ -138,6 +161,28 @@ def tlisi(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Op
                                    _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), _ptr(arg), _ptr(out[3]), _ptr(out[4]))
     if rc != 0:
         raise ValueError("fitrig_oracle_tlisi: bad arguments")
+    return TlisiResult(M, U, Ty, Tx, out[0], out[1], out[2], arg, out[3], out[4])
+
+
+def _tlisi_f64(imgs: Sequence[np.ndarray], tile: int, C: float, ref_mode: int, M: Optional[float]) -> TlisiResult:
+    """O1-O5 on fp64 images (accumulated snapshots)."""
+    L = len(imgs)
+    if L < 3:
+        raise ValueError("need at least 3 (accumulated) snapshots (PAPER.md:155)")
+    H, W = imgs[0].shape
+    keep = [np.ascontiguousarray(a, dtype=np.float64) for a in imgs]
+    arr = (ctypes.c_void_p * L)(*[a.ctypes.data for a in keep])
+    if M is None:
+        M = max(max(float(a.max()) for a in keep), float(C))  # O1 on the accumulated images
+    U = L - 2
+    Ty, Tx = -(-H // tile), -(-W // tile)
+    shp = (U, Ty, Tx)
+    out = [np.zeros(shp, dtype=np.float64) for _ in range(5)]
+    arg = np.zeros(shp, dtype=np.int64)
+    rc = lib().fitrig_oracle_tlisi_f64(arr, L, H, W, int(tile), float(C), int(ref_mode), float(M),
+                                       _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), _ptr(arg), _ptr(out[3]), _ptr(out[4]))
+    if rc != 0:
+        raise ValueError("fitrig_oracle_tlisi_f64: bad arguments")
     return TlisiResult(M, U, Ty, Tx, out[0], out[1], out[2], arg, out[3], out[4])
 
 
@@ -220,11 +265,12 @@ class DetectResult:
 
 
 def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
-        tau: float = 5.0, branch: int = 0) -> DetectResult:
-    """Whole path on one stack: O1..O7 (branch 0) or O1..O5 + O8 (branch 1)."""
+        tau: float = 5.0, branch: int = 0, accumulate_g: int = 1) -> DetectResult:
+    """Whole path on one stack: O1..O7 (branch 0) or O1..O5 + O8 (branch 1); accumulate_g > 1 first combines
+    groups of g snapshots."""
     snaps = as_snapshots(stack)
     H, W = snaps[0].shape
-    res = tlisi(snaps, tile, C, ref_mode, M)
+    res = tlisi(snaps, tile, C, ref_mode, M, accumulate_g)
     if branch == 0:
         mu, sd, z = zscore(res.q)
         c = select(z, res.argmax, W, tau)

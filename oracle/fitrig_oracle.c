@@ -86,18 +86,22 @@ static double ref_intensity(double x, double C, int ref_mode) {
  * Outputs are [U][Ty][Tx]; any output pointer may be NULL.
  * argmax = y*W + x of the first (lowest row-major) pixel attaining max(Delta) in the tile (R20).
  * Returns 0, or -1 on bad arguments (R10: L < 3). */
-int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile, double C, int ref_mode,
-                        double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
-                        double* tlisi) {
+/* Pixel p of image k: the images are either the fp32 snapshots themselves or fp64 accumulated snapshots
+ * (fitrig_oracle_tlisi_f64, PAPER.md:497 / Fig. 16); widening fp32 -> fp64 is exact. */
+static double px(const void* const* img, int is_f64, int k, int64_t p) {
+  return is_f64 ? ((const double*)img[k])[p] : (double)((const float*)img[k])[p];
+}
+
+static int tlisi_core(const void* const* snaps, int is_f64, int L, int H, int W, int tile, double C, int ref_mode,
+                      double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
+                      double* tlisi) {
   if (L < 3 || H < 1 || W < 1 || tile < 1 || !snaps) return -1;
   const int U = L - 2;
   const int Ty = (H + tile - 1) / tile, Tx = (W + tile - 1) / tile;
 #pragma omp parallel for collapse(2) schedule(dynamic, 1)
   for (int u = 0; u < U; ++u) {
     for (int ty = 0; ty < Ty; ++ty) {
-      const float* x0 = snaps[u];     /* x^(s)   */
-      const float* x1 = snaps[u + 1]; /* x^(s+1), the reference image */
-      const float* x2 = snaps[u + 2]; /* x^(s+2) */
+      /* images u, u+1, u+2 are x^(s), x^(s+1) (the reference image) and x^(s+2) */
       for (int tx = 0; tx < Tx; ++tx) {
         const int r0 = ty * tile, r1 = (r0 + tile < H) ? r0 + tile : H;
         const int c0 = tx * tile, c1 = (c0 + tile < W) ? c0 + tile : W;
@@ -107,7 +111,7 @@ int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile
         for (int i = r0; i < r1; ++i) {
           for (int j = c0; j < c1; ++j) {
             const int64_t p = (int64_t)i * W + j;
-            const double a = (double)x0[p], b = (double)x1[p], c = (double)x2[p];
+            const double a = px(snaps, is_f64, u, p), b = px(snaps, is_f64, u + 1, p), c = px(snaps, is_f64, u + 2, p);
             const double D1 = fabs(b - a);
             const double D2 = fabs(c - b);
             const double delta = fabs(D1 - D2);
@@ -138,6 +142,20 @@ int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile
     }
   }
   return 0;
+}
+
+int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile, double C, int ref_mode,
+                        double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
+                        double* tlisi) {
+  return tlisi_core((const void* const*)snaps, 0, L, H, W, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
+}
+
+/* The same O2..O5 on fp64 images: used for ACCUMULATED snapshots (section 3.3.2, Fig. 16:
+ * "FITrig can be applied after combining multiple snapshots"), whose sums are formed in fp64 by the caller. */
+int fitrig_oracle_tlisi_f64(const double* const* imgs, int L, int H, int W, int tile, double C, int ref_mode,
+                            double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
+                            double* tlisi) {
+  return tlisi_core((const void* const*)imgs, 1, L, H, W, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
 }
 
 /* O6.  z-score of the tile matrix of each unit, Eq. 8:

@@ -368,3 +368,54 @@ def test_realtime_single_pixel_transient_closed_form():
             assert abs(q[1, 0] - q_expected) <= 1e-15 and np.count_nonzero(q) == 1
         else:
             assert not q.any()
+
+
+# ------------------------------------------------------------------------------------------
+# snapshot accumulation (section 3.3.2, Fig. 16; R25)
+# ------------------------------------------------------------------------------------------
+def test_accumulate_handworked_golden_and_incomplete_group_is_left_out():
+    g = util.golden("accumulate_handworked_2x2.json")
+    raw = np.array(g["raw"], dtype=np.float32)
+    acc = oracle.accumulate(raw, g["g"])
+    assert len(acc) == 3 and all(np.array_equal(a, np.array(e)) for a, e in zip(acc, g["accumulated"]))
+    for stack in (raw, raw[:6]):  # the seventh snapshot completes no group
+        r = oracle.tlisi(stack, tile=g["tile"], accumulate_g=g["g"])
+        assert (r.U, r.Ty, r.Tx) == (1, 1, 1) and r.M == g["M"]
+        assert r.sumD[0, 0, 0] == g["sumD"] and r.maxD[0, 0, 0] == g["maxD"] and r.sumR[0, 0, 0] == g["sumR"]
+        assert r.q[0, 0, 0] == g["q"] and r.tlisi[0, 0, 0] == g["tlisi"]
+        assert (int(r.argmax[0, 0, 0]) % 2, int(r.argmax[0, 0, 0]) // 2) == tuple(g["argmax_xy"])  # y*W + x, W = 2
+
+
+def test_accumulate_one_is_the_identity_and_small_integers_match_the_presummed_stack():
+    st = _noise_stack(9, 40, 56)
+    a, b = oracle.run(st, tile=8, tau=2.0), oracle.run(st, tile=8, tau=2.0, accumulate_g=1)
+    assert np.array_equal(a.res.q, b.res.q) and np.array_equal(a.z, b.z)
+    # integer-valued pixels: fp32 sums are exact, so the fp32 route on the pre-summed stack is the same computation
+    rng = np.random.default_rng(3)
+    ints = rng.integers(-50, 50, size=(12, 24, 24)).astype(np.float32)
+    pre = ints.reshape(4, 3, 24, 24).sum(axis=1).astype(np.float32)
+    x, y = oracle.run(ints, tile=8, tau=1.0, accumulate_g=3), oracle.run(pre, tile=8, tau=1.0)
+    assert x.res.M == y.res.M and np.array_equal(x.res.q, y.res.q) and np.array_equal(x.res.argmax, y.res.argmax)
+    assert np.array_equal(x.cands.tile, y.cands.tile)
+    with pytest.raises(ValueError):
+        oracle.run(ints[:8], tile=8, accumulate_g=3)  # only two complete groups: fewer than 3 snapshots
+
+
+@pytest.mark.parametrize("g", [2, 4])
+def test_accumulate_single_pixel_transient_closed_form(g):
+    # P8 on accumulated snapshots: background b in every raw snapshot, +A at one pixel of raw snapshot k only.
+    # A_j = g*b everywhere, + A in group j* = k // g: units j*-2 and j* see Delta = A at that pixel against a
+    # reference of g*b, and M = g*b + A.
+    L, H, W, tile, b, A = 8 * g, 16, 16, 8, 2.0, 3.0
+    k = 4 * g + 1
+    st = np.full((L, H, W), b, dtype=np.float32)
+    st[k, 3, 12] += A
+    r = oracle.tlisi(st, tile=tile, accumulate_g=g)
+    js = k // g
+    assert r.U == 8 - 2 and r.M == g * b + A
+    expected = A * A * min(A / (g * b), 1.0) / ((tile * tile) ** 2 * (g * b + A) ** 2)
+    for u in range(r.U):
+        if u in (js - 2, js):
+            assert abs(r.q[u, 0, 1] - expected) <= 1e-15 and np.count_nonzero(r.q[u]) == 1
+        else:
+            assert not r.q[u].any()
