@@ -15,7 +15,8 @@
  *   - Snapshots x_0 .. x_{L-1}: H x W fp32, row-major, finite values (R9).  Pixel magnitudes
  *     below the fp32 normal range (|x| < 1.2e-38, other than exact zero) are unsupported.
  *   - Unit u = 0 .. L-3 uses x_u, x_{u+1}, x_{u+2}; x_{u+1} is the reference image
- *     (the paper's s = u + 1).  U = L - 2 units.
+ *     (the paper's s = u + 1).  U = L - 2 units.  (With params.accumulate = g > 1 read
+ *     "accumulated snapshot A_j" for x_j and L / g for L throughout.)
  *   - Tiles: Ty = ceil(H / N_T), Tx = ceil(W / N_T); partial edge tiles keep their own pixel
  *     count (R5).  Maps are [U][Ty][Tx], row-major.
  *   - Image axes: x = column (fastest), y = row (R16).
@@ -62,7 +63,10 @@ typedef struct {
   int32_t device;     /* CUDA device ordinal                                                      */
   int32_t row_offset; /* row shards (fitrig_shard_*): image row of this context's first row, a multiple of */
                       /* tile; added to the y of every candidate.  0 for a whole image                     */
-  int32_t reserved[8];
+  int32_t accumulate; /* g >= 1; 0 -> 1.  Snapshot accumulation (Fig. 16): the images the method  */
+                      /* assesses are A_j = x_{gj} + .. + x_{gj+g-1}, j < L / g (an incomplete trailing group  */
+                      /* is left out, R25); units U = L / g - 2; M is the largest accumulated pixel          */
+  int32_t reserved[7];
 } fitrig_params;
 
 /* One candidate, 16 bytes.

@@ -146,7 +146,17 @@ static void free_ctx(fitrig_ctx* c) {
 
 template <int REF>
 static cudaError_t set_fused_attr() {
-  return cudaFuncSetAttribute(tlisi_fused_kernel<REF>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta);
+  cudaError_t e = cudaFuncSetAttribute(tlisi_fused_kernel<REF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       kMaxSmemPerCta);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(tlisi_fused_kernel<REF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta);
+}
+
+template <int REF>
+static void launch_fused(bool acc, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const CUtensorMap& tm,
+                         const FusedParams& fp) {
+  if (acc) tlisi_fused_kernel<REF, true><<<grid, block, smem, st>>>(tm, fp);
+  else tlisi_fused_kernel<REF, false><<<grid, block, smem, st>>>(tm, fp);
 }
 
 extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_params* params, fitrig_ctx** out) {
@@ -170,7 +180,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   fitrig_ctx* c = new (std::nothrow) fitrig_ctx();
   if (!c) return fail(FITRIG_ERR_NOMEM, "fitrig_create: host allocation failed");
   c->prm = np;
-  c->H = H; c->W = W; c->L = L; c->U = L - 2;
+  c->H = H; c->W = W; c->L = L; c->U = L / np.accumulate - 2;
   c->num_sms = prop.multiProcessorCount;
   rc = fitrig_plan_query(H, W, L, params, c->num_sms, &c->plan);
   if (rc != FITRIG_OK) { delete c; return fail(rc, "fitrig_create: plan failed"); }
@@ -315,7 +325,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
     fp.raw = c->raw; fp.gmax_key = key;
-    fp.z0 = opt.z0; fp.zmod = opt.zmod;
+    fp.z0 = opt.z0; fp.zmod = opt.zmod; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
     fp.U = c->U;
@@ -327,19 +337,20 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: tlisi_fused_kernel<FITRIG_REF_ABS><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
-      case FITRIG_REF_LITERAL: tlisi_fused_kernel<FITRIG_REF_LITERAL><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
-      default: tlisi_fused_kernel<FITRIG_REF_FLOOR><<<grid, block, pl.smem_bytes, st>>>(tm, fp); break;
+      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
+      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;
   } else {
     if (with_max) {
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
-      for (int s = 0; s < c->L; ++s) {
-        const int slot = opt.zmod ? (opt.z0 + s) % opt.zmod : s;
+      const int g = c->prm.accumulate;
+      for (int s = 0; s < c->U + 2; ++s) {  // (accumulated) images; the ring mode never accumulates
+        const int slot = opt.zmod ? (opt.z0 + s) % opt.zmod : s * g;
         stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)slot * snap_stride,
-                                                                       (long long)rows * c->W, key);
+                                                                       (long long)rows * c->W, g, snap_stride, key);
         CUDA_TRY(cudaGetLastError());
         c->launches++;
       }
@@ -351,7 +362,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     const long long n_t = (long long)tile * tile;
     while (G < 32 && G < n_t) G <<= 1;
     gp.G = G;
-    gp.z0 = opt.z0; gp.zmod = opt.zmod;
+    gp.z0 = opt.z0; gp.zmod = opt.zmod; gp.acc = c->prm.accumulate;
     gp.C = c->prm.C;
     const long long groups = (long long)rows_tiles * c->Tx * c->U;
     const long long threads = groups * G;
@@ -553,7 +564,8 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
                            int64_t capacity, int64_t* n_found, int64_t* unit, void* cuda_stream) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: ctx is NULL");
   if (!n_found || !unit) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: n_found or unit is NULL");
-  if (c->L != 3) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: create the context with n_snapshots = 3 (one unit per push)");
+  if (c->L != 3 || c->prm.accumulate != 1)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: create the context with n_snapshots = 3 (one unit per push) and no accumulation");
   if (c->prm.branch != FITRIG_BRANCH_IMAGE)
     return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: the real-time mode is the image branch (Eq. 8-9)");
   cudaStream_t st = (cudaStream_t)cuda_stream;

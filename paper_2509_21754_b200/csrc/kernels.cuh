@@ -143,6 +143,7 @@ struct FusedParams {
   int G;                 // rows_tiles * ngx * U: (box column, unit) pairs of this launch, box-major
   int evict_first;       // L2 policy of the streaming loads
   int z0, zmod;          // real-time mode: snapshot s of the launch lives in slot (z0 + s) % zmod of a ring; zmod = 0: slot s
+  int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
   float C;
 };
 
@@ -184,6 +185,15 @@ __device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* t
   for (int j = 0; j < 8; ++j) {
     const float4 t = *reinterpret_cast<const float4*>(src + 4 * j * pitch);
     N[4 * j] = t.x; N[4 * j + 1] = t.y; N[4 * j + 2] = t.z; N[4 * j + 3] = t.w;
+  }
+}
+
+__device__ __forceinline__ void add_tile(float (&N)[32], const unsigned char* tile_ptr, int pitch, int lane) {
+  const unsigned char* src = tile_ptr + (lane >> 3) * pitch + (lane & 7) * 16;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float4 t = *reinterpret_cast<const float4*>(src + 4 * j * pitch);
+    N[4 * j] += t.x; N[4 * j + 1] += t.y; N[4 * j + 2] += t.z; N[4 * j + 3] += t.w;
   }
 }
 
@@ -251,9 +261,10 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 // of Delta (R20) is tracked per 16-byte group in the loop; which of its 4 pixels it was is found one
 // step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
 // by lane 0, off the critical path.
-template <int REF_MODE>
+template <int REF_MODE, bool ACC>
 __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
+  const int acc = ACC ? p.acc : 1;  // ACC = false compiles the accumulation loops away
   extern __shared__ __align__(1024) unsigned char smem[];
   // the shuffle tells the compiler the warp index is warp uniform, so cursors and addresses derived
   // from it live in uniform registers and the vector registers are left to the three tile arrays
@@ -289,16 +300,16 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       for (int g = g_begin; g < g_end;) {
         const Segment c = decode_segment(p, g, g_end);
         g += c.nsteps - 2;
-        for (int s = 0; s < c.nsteps; ++s) {
+        for (int s = 0; s < c.nsteps * acc; ++s) {  // raw snapshots (u0 + step) * acc + i, in order
           mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
           const uint32_t bar = full_addr + slot * 8;
           mbar_arrive_expect_tx(bar, box_bytes);
           if (p.evict_first)
             tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                              ring_slot(p.z0, p.zmod, c.u0 + s), policy);
+                              ring_slot(p.z0, p.zmod, c.u0 * acc + s), policy);
           else
             tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                         ring_slot(p.z0, p.zmod, c.u0 + s));
+                         ring_slot(p.z0, p.zmod, c.u0 * acc + s));
           if (++slot == p.nstage) { slot = 0; phase ^= 1; }
         }
       }
@@ -322,6 +333,13 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     __syncwarp();  // every lane has its copy
     if (lane == 0) mbar_arrive(empty_addr + slot * 8);
     if (++slot == p.nstage) { slot = 0; phase ^= 1; }
+    for (int i = 1; i < acc; ++i) {  // accumulation: the image is the sum of acc raw snapshots, added in order
+      mbar_wait(full_addr + slot * 8, phase);
+      add_tile(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_addr + slot * 8);
+      if (++slot == p.nstage) { slot = 0; phase ^= 1; }
+    }
     scan_tile(N, gmax, zmin);
   };
   // a warp whose tile lies beyond the image edge only keeps the ring turning
@@ -332,13 +350,39 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   };
 
   // ---- one record is always "pending": its arg-max group is known, the pixel inside it is not.
-  // Lane 0 parks it in the warp's scratch (registers are for the tile arrays): scratch[0..2] the
-  // re-read pixels, scratch[3] = {sum Delta, sum r, max bits, group position}, scratch[4] = map index.
+  // Lane 0 parks it in the warp's scratch (registers are for the tile arrays): scratch[0 .. 3*acc) the
+  // re-read raw pixels of the three images, scratch[kScratchRec] = {sum Delta, sum r, max bits, group
+  // position}, scratch[kScratchRec + 1] = {map index, element offset of the group inside an image}.
   bool pend = false;
   auto resolve_pending = [&]() {  // lane 0 only
-    cp_async_wait_all();
-    const float4 a = scratch[0], b = scratch[1], c = scratch[2], rec = scratch[3];
-    const unsigned long long idx = *reinterpret_cast<const unsigned long long*>(&scratch[4]);
+    const float4 rec = scratch[kScratchRec];
+    const unsigned long long idx = reinterpret_cast<const unsigned long long*>(&scratch[kScratchRec + 1])[0];
+    float4 img[3];
+    if (acc <= kMaxAccAsync) {
+      cp_async_wait_all();
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        img[k] = scratch[k * acc];
+        for (int i = 1; i < acc; ++i) {  // the same order of fp32 additions as acquire()
+          const float4 t = scratch[k * acc + i];
+          img[k].x += t.x; img[k].y += t.y; img[k].z += t.z; img[k].w += t.w;
+        }
+      }
+    } else {  // long accumulations: plain (blocking) loads, L2 hits
+      const long long off = reinterpret_cast<const long long*>(&scratch[kScratchRec + 1])[1];
+      const int u = (int)(idx / ((unsigned long long)p.Ty * p.Tx));
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        img[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int i = 0; i < acc; ++i) {
+          const float4 t = *reinterpret_cast<const float4*>(
+              p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
+          if (i == 0) img[k] = t;
+          else { img[k].x += t.x; img[k].y += t.y; img[k].z += t.z; img[k].w += t.w; }
+        }
+      }
+    }
+    const float4 a = img[0], b = img[1], c = img[2];
     const float mx = rec.z;
     // the same three fp32 operations as tile_step -> bit-identical Delta
     const float e0 = fabsf(fabsf(c.x - b.x) - fabsf(b.x - a.x));
@@ -369,14 +413,18 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     if (lane == 0) {
       if (pend) resolve_pending();
       const int u = c.u0 + step - 2;
-      scratch[3] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
-      *reinterpret_cast<unsigned long long*>(&scratch[4]) =
+      scratch[kScratchRec] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
+      // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
+      const long long off = (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
+      reinterpret_cast<unsigned long long*>(&scratch[kScratchRec + 1])[0] =
           ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + tx;
-      // the winning group's 4 pixels in x_u, x_{u+1}, x_{u+2}: in bounds (a zero-filled pixel has Delta 0)
-      const float* src = p.base + (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
-      cp_async16(scratch_addr, src + (long long)ring_slot(p.z0, p.zmod, u) * p.snap_stride);
-      cp_async16(scratch_addr + 16, src + (long long)ring_slot(p.z0, p.zmod, u + 1) * p.snap_stride);
-      cp_async16(scratch_addr + 32, src + (long long)ring_slot(p.z0, p.zmod, u + 2) * p.snap_stride);
+      reinterpret_cast<long long*>(&scratch[kScratchRec + 1])[1] = off;
+      if (acc <= kMaxAccAsync) {
+        for (int k = 0; k < 3; ++k)
+          for (int i = 0; i < acc; ++i)
+            cp_async16(scratch_addr + (k * acc + i) * 16,
+                       p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
+      }
       cp_async_commit();
     }
     pend = true;
@@ -387,7 +435,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     g += c.nsteps - 2;
     const int tx = c.gx * p.ntw + warp;
     if (tx >= p.Tx) {
-      for (int s = 0; s < c.nsteps; ++s) skip();
+      for (int s = 0; s < c.nsteps * acc; ++s) skip();
       continue;
     }
     acquire(A, zA);  // x_{u0}
@@ -426,6 +474,7 @@ struct GenericParams {
   int Tx, Ty, ty_base, rows_tiles, U;
   int G;                    // lanes per tile
   int z0, zmod;             // real-time mode ring (see FusedParams)
+  int acc;                  // snapshot accumulation (see FusedParams)
   float C;
 };
 
@@ -447,14 +496,17 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
     tx = (int)(t - (long long)ty_local * p.Tx);
     const int r0 = ty_local * p.tile, c0 = tx * p.tile;
     const int h = min(p.tile, p.rows - r0), w = min(p.tile, p.W - c0);
-    const float* x0 = p.base + (long long)ring_slot(p.z0, p.zmod, u) * p.snap_stride;
-    const float* x1 = p.base + (long long)ring_slot(p.z0, p.zmod, u + 1) * p.snap_stride;
-    const float* x2 = p.base + (long long)ring_slot(p.z0, p.zmod, u + 2) * p.snap_stride;
+    // image k of the unit = sum of raw snapshots (u + k) * acc .. + acc - 1, added in order
+    auto image = [&](int k, long long o) {
+      float v = p.base[(long long)ring_slot(p.z0, p.zmod, (u + k) * p.acc) * p.snap_stride + o];
+      for (int i = 1; i < p.acc; ++i) v += p.base[(long long)ring_slot(p.z0, p.zmod, (u + k) * p.acc + i) * p.snap_stride + o];
+      return v;
+    };
     bool first = true;
     for (int i = gl; i < h * w; i += p.G) {
       const int r = i / w, c = i - r * w;
       const long long o = (long long)(r0 + r) * p.W + (c0 + c);
-      const float a = x0[o], b = x1[o], cc = x2[o];
+      const float a = image(0, o), b = image(1, o), cc = image(2, o);
       const float delta = fabsf(fabsf(b - a) - fabsf(cc - b));
       S += delta;
       if (first || delta > Mx) { Mx = delta; pos = r * p.tile + c; first = false; }
@@ -475,11 +527,17 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
   }
 }
 
-// Global maximum over n floats (generic path; the fused path folds this into its single pass).
-__global__ void __launch_bounds__(256) stack_max_kernel(const float* __restrict__ x, long long n, unsigned* gmax_key) {
+// Global maximum over the n pixels of one image (generic path; the fused path folds this into its single
+// pass): the image is the sum of `acc` raw snapshots `stride` elements apart, added in order.
+__global__ void __launch_bounds__(256) stack_max_kernel(const float* __restrict__ x, long long n, int acc, long long stride,
+                                                        unsigned* gmax_key) {
   float m = -3.402823466e38f;
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) m = fmaxf(m, x[i]);
+  const long long step = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += step) {
+    float v = x[i];
+    for (int k = 1; k < acc; ++k) v += x[i + k * stride];
+    m = fmaxf(m, v);
+  }
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(m));
   if ((threadIdx.x & 31) == 0) atomicMax(gmax_key, key);
 }

@@ -20,7 +20,12 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
   if (!p) p = &z;
   *why = "";
   if (H < 1 || W < 1) { *why = "H and W must be >= 1"; return FITRIG_ERR_INVALID_ARG; }
-  if (L < 3) { *why = "need at least 3 snapshots (s = 1..L-2, PAPER.md:155)"; return FITRIG_ERR_INVALID_ARG; }
+  if (p->accumulate < 0) { *why = "accumulate must be >= 1 (0 selects 1)"; return FITRIG_ERR_INVALID_ARG; }
+  out->accumulate = p->accumulate == 0 ? 1 : p->accumulate;
+  if (L / out->accumulate < 3) {
+    *why = "need at least 3 (accumulated) snapshots (s = 1..L-2, PAPER.md:155)";
+    return FITRIG_ERR_INVALID_ARG;
+  }
   if (p->tile < 0) { *why = "tile must be >= 1 (0 selects the default 32)"; return FITRIG_ERR_INVALID_ARG; }
   if (p->ref_mode < 0 || p->ref_mode > 2) { *why = "unknown ref_mode"; return FITRIG_ERR_INVALID_ARG; }
   if (p->branch < 0 || p->branch > 1) { *why = "unknown branch"; return FITRIG_ERR_INVALID_ARG; }
@@ -98,7 +103,7 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   if (rc != FITRIG_OK) return rc;
   memset(out, 0, sizeof(*out));
   const int tile = np.tile;
-  out->units = L - 2;
+  out->units = L / np.accumulate - 2;
   out->Ty = (H + tile - 1) / tile;
   out->Tx = (W + tile - 1) / tile;
   // strip schedule for fitrig_stream: ~256 MiB of snapshot rows per strip (all L snapshots), a multiple of tile

@@ -60,7 +60,7 @@ def oracle_delta_at(stack_np, u, x, y):
 
 
 def check_against_oracle(stack_gpu, g, ref, taus, tile, branch=0, ref_mode=0, C=1e-6, small_tiles=False,
-                         sample_argmax=4000, stack_np=None):
+                         sample_argmax=4000, stack_np=None, extra_slack=None):
     """stack_np: the same snapshots on the host ([L,H,W] array or list of [H,W] arrays) when the caller has them."""
     if stack_np is None:
         stack_np = stack_gpu.cpu().numpy()
@@ -68,10 +68,10 @@ def check_against_oracle(stack_gpu, g, ref, taus, tile, branch=0, ref_mode=0, C=
     # --- raw per-tile quantities of Eq. 6 ---
     sd, md, sr, ax, ay = g["raw"]
     q_slack = None
-    if small_tiles:
+    if small_tiles or extra_slack is not None:
         # N_T < 4: a tile's Delta is a cancellation of fp32-rounded differences, so a purely relative bound is
         # not attainable by ANY fp32 evaluation; add the derived first-order rounding bound (util.fp32_slack)
-        eS, eM, eR = util.fp32_slack(stack_np, tile, C, ref_mode)
+        eS, eM, eR = util.fp32_slack(np.asarray(stack_np), tile, C, ref_mode, extra=extra_slack)
         assert np.all(np.abs(sd - res.sumD) <= 2e-5 * res.sumD + eS)
         assert np.all(np.abs(md - res.maxD) <= 1e-6 * res.maxD + eM)
         assert np.all(np.abs(sr - res.sumR) <= 2e-5 * np.abs(res.sumR) + eR + 2e-5)
@@ -92,7 +92,10 @@ def check_against_oracle(stack_gpu, g, ref, taus, tile, branch=0, ref_mode=0, C=
         assert ty * tile <= ay[u, ty, tx] < (ty + 1) * tile and tx * tile <= ax[u, ty, tx] < (tx + 1) * tile
     assert exact.mean() > 0.99
     # --- M, q, tLISI ---
-    assert g["M"] == np.float32(res.M)
+    if extra_slack is None:
+        assert g["M"] == np.float32(res.M)
+    else:  # the largest ACCUMULATED pixel: g - 1 fp32 additions against the exact sum
+        assert abs(g["M"] - res.M) <= 1e-6 * res.M
     util.assert_map_close(g["q"], res.q, g["tlisi"], res.tlisi, slack=q_slack)
     if g["tlisi_out"] is not None:
         assert np.array_equal(g["tlisi_out"], g["tlisi"])
@@ -355,6 +358,45 @@ def test_frequency_branch_odd_length_series():
     ref = oracle_run(st, tile=32, tau=1.0, branch=1)
     np.testing.assert_allclose(g["eta"], ref.eta, rtol=2e-4)
     assert np.array_equal(g["kstar"], ref.kstar)
+
+
+# ------------------------------------------------------------------------------------------
+# snapshot accumulation (section 3.3.2, Fig. 16; R25)
+# ------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def long_tiny():
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 256, 256, L=20)
+    return synth.make_stack(cfg, device=DEV)
+
+
+@pytest.mark.parametrize("g,H,W,tile,use_stream", [(2, 256, 256, 32, False), (3, 250, 252, 32, False), (4, 256, 256, 32, True),
+                                                   (5, 256, 256, 32, False), (6, 128, 96, 32, True), (2, 120, 100, 8, False),
+                                                   (3, 64, 64, 1, False)])
+def test_accumulated_snapshots_match_oracle(long_tiny, g, H, W, tile, use_stream):
+    st, _ = long_tiny
+    st = st[:, :H, :W].contiguous()
+    taus = (3.0,) if (H // tile) * (W // tile) >= 40 else (1.0,)
+    kw = dict(strip_rows=64) if use_stream and tile == 32 else {}
+    gp = gpu_run(st, taus=taus, accumulate=g, tile=tile, use_stream=use_stream, **kw)
+    assert gp["dims"][0] == 20 // g - 2  # the incomplete trailing group (20 mod g snapshots) is left out
+    ref = oracle_run(st, tile=tile, tau=taus[0], accumulate_g=g)
+    acc_np = np.stack(oracle.accumulate(st.cpu().numpy(), g))  # fp64 images: what Delta is measured on
+    # fp32 sums of g snapshots carry a rounding of (g-1) 2^-24 sum|x| per pixel into the differences: derived slack
+    check_against_oracle(None, gp, ref, taus, tile, stack_np=acc_np,
+                         extra_slack=util.accumulation_slack(st.cpu().numpy(), g))
+
+
+def test_accumulate_one_is_bit_identical_and_frequency_branch_accumulates(long_tiny):
+    st, _ = long_tiny
+    a, b = gpu_run(st), gpu_run(st, accumulate=1)
+    assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
+    gq = gpu_run(st, taus=(1.0,), accumulate=2, branch=fitrig.BRANCH_FREQUENCY)
+    ref = oracle_run(st, tile=32, tau=1.0, branch=1, accumulate_g=2)
+    util.assert_map_close(gq["q"], ref.res.q)
+    np.testing.assert_allclose(gq["eta"], ref.eta, rtol=2e-4, atol=1e-12)
+    with pytest.raises(fitrig.FitrigError) as e:
+        fitrig.Context(64, 64, 8, accumulate=3)  # 8 // 3 = 2 accumulated snapshots: fewer than 3
+    assert e.value.code == fitrig.binding.ERR_INVALID_ARG
 
 
 # ------------------------------------------------------------------------------------------

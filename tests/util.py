@@ -120,7 +120,17 @@ def _tile_reduce(a: np.ndarray, tile: int, op):
     return op(op(p.reshape(Ty, tile, Tx, tile), axis=3), axis=1)
 
 
-def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0):
+def accumulation_slack(raw: np.ndarray, g: int):
+    """Per unit and pixel, what summing g fp32 snapshots in fp32 (instead of exactly) can move Delta by:
+    image A_j carries at most (g-1) 2^-24 sum_i |x_{gj+i}|; Delta_u = ||A_{u+2}-A_{u+1}| - |A_{u+1}-A_u|| sees
+    A_u and A_{u+2} once and A_{u+1} twice.  Returns [U, H, W]."""
+    L = raw.shape[0] // g
+    mag = np.abs(raw[:L * g].astype(np.float64)).reshape(L, g, *raw.shape[1:]).sum(axis=1)
+    e = (g - 1) * 2.0 ** -24 * mag
+    return e[:-2] + 2.0 * e[1:-1] + e[2:]
+
+
+def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0, extra=None):
     """First-order bound on what fp32 evaluation of Eq. 3-5 can differ from exact arithmetic, per tile.
 
     fl(b-a) = (b-a)(1+d), |d| <= 2^-24, three times: |Delta_fp32 - Delta| <= 2^-24 (D1 + D2 + Delta); a factor 2
@@ -135,6 +145,8 @@ def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0)
         D1, D2 = np.abs(x[u + 1] - x[u]), np.abs(x[u + 2] - x[u + 1])
         dl = np.abs(D1 - D2)
         e = 2.0 ** -23 * (D1 + D2 + dl)
+        if extra is not None:
+            e = e + extra[u]
         b = x[u + 1]
         if ref_mode == 0:
             xh = np.where(b == 0, C, np.abs(b))
