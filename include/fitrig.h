@@ -83,10 +83,10 @@ typedef struct {
 /* How the library will run a problem; pure host arithmetic (no CUDA call), see fitrig_plan_query. */
 typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
-  int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, W % 4 == 0)         */
+  int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, 16 or 8; W % 4 == 0)*/
                              /* 1: generic kernel (any N_T, any W)                               */
   int32_t units_per_cta;     /* fused path: (box column, unit) pairs per CTA, ceil(boxes * U / grid) */
-  int32_t box_tiles;         /* fused path: adjacent tiles fetched as one TMA box (1..8)         */
+  int32_t box_tiles;         /* fused path: adjacent 32x32 pixel blocks fetched as one TMA box (1..8) */
   int32_t warps_per_cta;     /* fused path: box_tiles consumer warps + 1 producer warp           */
   int32_t stages;            /* fused path: depth of the CTA's ring of TMA boxes                 */
   int32_t grid;              /* CTAs launched                                                    */

@@ -144,19 +144,35 @@ static void free_ctx(fitrig_ctx* c) {
   delete c;
 }
 
-template <int REF>
-static cudaError_t set_fused_attr() {
-  cudaError_t e = cudaFuncSetAttribute(tlisi_fused_kernel<REF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       kMaxSmemPerCta);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(tlisi_fused_kernel<REF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta);
+template <int REF, bool ACC, int T>
+static cudaError_t set_fused_attr_one() {
+  return cudaFuncSetAttribute(tlisi_fused_kernel<REF, ACC, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta);
 }
 
 template <int REF>
-static void launch_fused(bool acc, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const CUtensorMap& tm,
+static cudaError_t set_fused_attr() {
+  cudaError_t e;
+  if ((e = set_fused_attr_one<REF, false, 32>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, true, 32>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, false, 16>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, true, 16>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, false, 8>()) != cudaSuccess) return e;
+  return set_fused_attr_one<REF, true, 8>();
+}
+
+template <int REF, int T>
+static void launch_fused_t(bool acc, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const CUtensorMap& tm,
+                           const FusedParams& fp) {
+  if (acc) tlisi_fused_kernel<REF, true, T><<<grid, block, smem, st>>>(tm, fp);
+  else tlisi_fused_kernel<REF, false, T><<<grid, block, smem, st>>>(tm, fp);
+}
+
+template <int REF>
+static void launch_fused(bool acc, int tile, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const CUtensorMap& tm,
                          const FusedParams& fp) {
-  if (acc) tlisi_fused_kernel<REF, true><<<grid, block, smem, st>>>(tm, fp);
-  else tlisi_fused_kernel<REF, false><<<grid, block, smem, st>>>(tm, fp);
+  if (tile == 16) launch_fused_t<REF, 16>(acc, grid, block, smem, st, tm, fp);
+  else if (tile == 8) launch_fused_t<REF, 8>(acc, grid, block, smem, st, tm, fp);
+  else launch_fused_t<REF, 32>(acc, grid, block, smem, st, tm, fp);
 }
 
 extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_params* params, fitrig_ctx** out) {
@@ -309,7 +325,8 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
   if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
-  if (pl.path == 0 && (rows_tiles != c->Ty)) plan_launch(tile, c->W, rows_tiles, c->Tx, c->U, c->num_sms, &pl);
+  if (pl.path == 0 && ((long long)ty_base * tile) % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
+  if (pl.path == 0 && rows != c->H) plan_launch(tile, c->W, rows, c->U, c->num_sms, &pl);
 
   int rc = prof_begin(c, st);
   if (rc) return rc;
@@ -327,19 +344,20 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.raw = c->raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmod = opt.zmod; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
-    fp.Tx = c->Tx; fp.Ty = c->Ty; fp.rows_tiles = rows_tiles; fp.ty_base = ty_base;
+    fp.Tx = c->Tx; fp.Ty = c->Ty; fp.Tx32 = (c->W + kFastTile - 1) / kFastTile;
+    fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = ty_base;
     fp.U = c->U;
-    fp.ntw = pl.box_tiles; fp.ngx = (c->Tx + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
-    const long long G = (long long)rows_tiles * fp.ngx * c->U;
+    fp.ntw = pl.box_tiles; fp.ngx = (fp.Tx32 + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
+    const long long G = (long long)fp.rows_tiles * fp.ngx * c->U;
     if (G > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "fused path: too many (box, unit) pairs for one launch");
     fp.G = (int)G;
     fp.evict_first = env_int("FITRIG_EVICT_FIRST", 0);
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
-      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
-      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;

@@ -133,9 +133,10 @@ struct FusedParams {
   const float* base;     // snapshot 0 of this launch's rows (the memory the TMA descriptor covers)
   long long snap_stride; // elements between consecutive snapshots
   int W;                 // image width (row pitch in elements)
-  int Tx, Ty;            // whole-map tile grid
-  int rows_tiles;        // tile rows covered by this launch (whole image, or one strip)
-  int ty_base;           // first tile row of this launch inside the whole map
+  int Tx, Ty;            // whole-map tile grid (tiles of N_T = 32, 16 or 8 pixels)
+  int Tx32;              // 32-pixel block columns = ceil(W / 32): a consumer warp owns one 32x32 block
+  int rows_tiles;        // rows of 32x32 blocks covered by this launch (whole image, or one strip)
+  int ty_base;           // first tile row (in tiles of N_T) of this launch inside the whole map
   int U;                 // units = L - 2
   int ntw;               // tiles per TMA box = consumer warps per CTA (1..kMaxTilesPerBox)
   int ngx;               // boxes per tile row = ceil(Tx / ntw)
@@ -176,23 +177,45 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// One 32x32 tile out of a box (row pitch `pitch` bytes) into registers.  Lane l owns columns
-// 4*(l%8)..+3 of rows (l/8) + 4*j, j = 0..7: a quarter warp reads one 128-byte tile row (conflict
-// free), and the 32 pixels of a lane are held in increasing row-major order.
-__device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* tile_ptr, int pitch, int lane) {
-  const unsigned char* src = tile_ptr + (lane >> 3) * pitch + (lane & 7) * 16;
+// Which pixels of its warp's 32x32 block a lane holds, for tiles of T = 32, 16 or 8 pixels.  The block is
+// (32/T)^2 tiles; T*T/32 consecutive lanes share one tile, so that the 32 pixels of a lane belong to ONE tile
+// and every reduction is a butterfly over an aligned lane group.  A lane reads float4's: T/4 lanes cover a
+// tile row, a lane group covers T/8 rows per load, 8 loads cover the tile; pixels are held in row-major
+// order of the tile.  T = 32: lane l owns columns 4*(l%8)..+3 of rows (l/8) + 4*j -- a quarter warp reads
+// one 128-byte row (conflict free); T = 8 likewise; T = 16 reads two 64-byte half rows (2-way conflict).
+template <int T>
+struct LaneGeom {
+  static constexpr int LPT = T * T / 32;  // lanes per tile
+  static constexpr int F = T / 4;         // float4 (= lanes) per tile row
+  static constexpr int RPL = T / 8;       // tile rows per load
+  static constexpr int NSUB = 32 / T;     // tiles per block edge
+  __device__ static __forceinline__ int sub_row(int lane) { return (lane / LPT) / NSUB; }
+  __device__ static __forceinline__ int sub_col(int lane) { return (lane / LPT) % NSUB; }
+  __device__ static __forceinline__ int row_in_tile(int lane) { return (lane % LPT) / F; }   // + RPL * j
+  __device__ static __forceinline__ int col_in_tile(int lane) { return ((lane % LPT) % F) * 4; }
+  __device__ static __forceinline__ int block_row(int lane) { return sub_row(lane) * T + row_in_tile(lane); }
+  __device__ static __forceinline__ int block_col(int lane) { return sub_col(lane) * T + col_in_tile(lane); }
+};
+
+// The lane's 32 pixels out of a box (row pitch `pitch` bytes) into registers / added to registers.
+template <int T>
+__device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
+  using G = LaneGeom<T>;
+  const unsigned char* src = block_ptr + G::block_row(lane) * pitch + G::block_col(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float4 t = *reinterpret_cast<const float4*>(src + 4 * j * pitch);
+    const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
     N[4 * j] = t.x; N[4 * j + 1] = t.y; N[4 * j + 2] = t.z; N[4 * j + 3] = t.w;
   }
 }
 
-__device__ __forceinline__ void add_tile(float (&N)[32], const unsigned char* tile_ptr, int pitch, int lane) {
-  const unsigned char* src = tile_ptr + (lane >> 3) * pitch + (lane & 7) * 16;
+template <int T>
+__device__ __forceinline__ void add_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
+  using G = LaneGeom<T>;
+  const unsigned char* src = block_ptr + G::block_row(lane) * pitch + G::block_col(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float4 t = *reinterpret_cast<const float4*>(src + 4 * j * pitch);
+    const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
     N[4 * j] += t.x; N[4 * j + 1] += t.y; N[4 * j + 2] += t.z; N[4 * j + 3] += t.w;
   }
 }
@@ -261,9 +284,11 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 // of Delta (R20) is tracked per 16-byte group in the loop; which of its 4 pixels it was is found one
 // step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
 // by lane 0, off the critical path.
-template <int REF_MODE, bool ACC>
+template <int REF_MODE, bool ACC, int T>
 __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
+  using Geo = LaneGeom<T>;
+  constexpr int LPT = Geo::LPT, NGRP = 32 / LPT;  // lanes per tile, tiles (lane groups) per warp
   const int acc = ACC ? p.acc : 1;  // ACC = false compiles the accumulation loops away
   extern __shared__ __align__(1024) unsigned char smem[];
   // the shuffle tells the compiler the warp index is warp uniform, so cursors and addresses derived
@@ -273,7 +298,9 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   unsigned char* after_ring = smem + (size_t)p.nstage * box_bytes;
   uint64_t* full = reinterpret_cast<uint64_t*>(after_ring);
   uint64_t* empty = full + kMaxStages;
-  float4* scratch = reinterpret_cast<float4*>(after_ring + 2 * kMaxStages * 8) + warp * kScratchVec;
+  // arg-max scratch of this lane's tile (one per lane group)
+  float4* scratch = reinterpret_cast<float4*>(after_ring + 2 * kMaxStages * 8) +
+                    (warp * NGRP + (threadIdx.x & 31) / LPT) * kScratchVec;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < p.nstage; ++i) {
@@ -324,18 +351,19 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   float gmax = -3.402823466e38f, zA = 1.f, zB = 1.f;
   int slot = 0;
   uint32_t phase = 0;
-  const int lrow = lane >> 3, lcol = (lane & 7) * 4;
+  const bool leader = (lane % LPT) == 0;  // does the bookkeeping of its tile
+  const unsigned gmask = (LPT == 32) ? 0xffffffffu : (((1u << (LPT & 31)) - 1u) << (lane & ~(LPT - 1)));
 
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
     mbar_wait(full_addr + slot * 8, phase);
-    load_tile(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+    load_tile<T>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
     __syncwarp();  // every lane has its copy
     if (lane == 0) mbar_arrive(empty_addr + slot * 8);
     if (++slot == p.nstage) { slot = 0; phase ^= 1; }
     for (int i = 1; i < acc; ++i) {  // accumulation: the image is the sum of acc raw snapshots, added in order
       mbar_wait(full_addr + slot * 8, phase);
-      add_tile(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+      add_tile<T>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty_addr + slot * 8);
       if (++slot == p.nstage) { slot = 0; phase ^= 1; }
@@ -350,11 +378,11 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   };
 
   // ---- one record is always "pending": its arg-max group is known, the pixel inside it is not.
-  // Lane 0 parks it in the warp's scratch (registers are for the tile arrays): scratch[0 .. 3*acc) the
+  // The tile's leader lane parks it in the tile's scratch (registers are for the tile arrays): scratch[0 .. 3*acc) the
   // re-read raw pixels of the three images, scratch[kScratchRec] = {sum Delta, sum r, max bits, group
   // position}, scratch[kScratchRec + 1] = {map index, element offset of the group inside an image}.
   bool pend = false;
-  auto resolve_pending = [&]() {  // lane 0 only
+  auto resolve_pending = [&]() {  // leader lanes only
     const float4 rec = scratch[kScratchRec];
     const unsigned long long idx = reinterpret_cast<const unsigned long long*>(&scratch[kScratchRec + 1])[0];
     float4 img[3];
@@ -397,44 +425,49 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     *reinterpret_cast<float4*>(&p.raw[idx]) = *reinterpret_cast<float4*>(&o);
   };
 
-  // warp reduction of one (tile, unit): exact max + first group by redux, the two sums by one butterfly
+  // reduction of one (tile, unit) over the tile's lane group: exact max + first 16-byte group by redux, the two
+  // sums by one butterfly (lower half of the group carries sum Delta, upper half sum r)
   auto finish = [&](const Segment& c, int tx, int step, float S, float R, float Mx, int jmax) {
     const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
-    const unsigned tmax = __reduce_max_sync(0xffffffffu, mbits);
-    const int gpos = (lrow + 4 * jmax) * kFastTile + lcol;
-    const unsigned tg = __reduce_min_sync(0xffffffffu, mbits == tmax ? (unsigned)gpos : 0x7fffffffu);
-    const bool hi = lane & 16;
-    float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, 16);
-    vsum += __shfl_xor_sync(0xffffffffu, vsum, 8);
-    vsum += __shfl_xor_sync(0xffffffffu, vsum, 4);
-    vsum += __shfl_xor_sync(0xffffffffu, vsum, 2);
-    vsum += __shfl_xor_sync(0xffffffffu, vsum, 1);
-    const float rsum = __shfl_sync(0xffffffffu, vsum, 16);  // lanes 0-15 hold sum S, 16-31 sum R
-    if (lane == 0) {
+    const unsigned tmax = __reduce_max_sync(gmask, mbits);
+    const int gpos = (Geo::row_in_tile(lane) + Geo::RPL * jmax) * T + Geo::col_in_tile(lane);  // row-major in the tile
+    const unsigned tg = __reduce_min_sync(gmask, mbits == tmax ? (unsigned)gpos : 0x7fffffffu);
+    const bool hi = lane & (LPT / 2);
+    float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, LPT / 2);
+#pragma unroll
+    for (int off = LPT / 4; off >= 1; off >>= 1) vsum += __shfl_xor_sync(0xffffffffu, vsum, off);
+    const float rsum = __shfl_sync(0xffffffffu, vsum, (lane & ~(LPT - 1)) + LPT / 2);
+    if (leader) {
       if (pend) resolve_pending();
+      pend = false;
       const int u = c.u0 + step - 2;
-      scratch[kScratchRec] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
-      // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
-      const long long off = (long long)(c.ty_local * kFastTile + (int)(tg >> 5)) * p.W + (tx * kFastTile + (int)(tg & 31));
-      reinterpret_cast<unsigned long long*>(&scratch[kScratchRec + 1])[0] =
-          ((unsigned long long)u * p.Ty + (p.ty_base + c.ty_local)) * p.Tx + tx;
-      reinterpret_cast<long long*>(&scratch[kScratchRec + 1])[1] = off;
-      if (acc <= kMaxAccAsync) {
-        for (int k = 0; k < 3; ++k)
-          for (int i = 0; i < acc; ++i)
-            cp_async16(scratch_addr + (k * acc + i) * 16,
-                       p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
+      const int ty_t = p.ty_base + c.ty_local * Geo::NSUB + Geo::sub_row(lane);  // tile coordinates in the whole map
+      const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
+      if (ty_t < p.Ty && tx_t < p.Tx) {  // (tiles of a block that hang over the image edge do not exist)
+        scratch[kScratchRec] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
+        // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
+        const long long off = (long long)(c.ty_local * kFastTile + Geo::sub_row(lane) * T + (int)(tg / T)) * p.W +
+                              (tx * kFastTile + Geo::sub_col(lane) * T + (int)(tg % T));
+        reinterpret_cast<unsigned long long*>(&scratch[kScratchRec + 1])[0] =
+            ((unsigned long long)u * p.Ty + ty_t) * p.Tx + tx_t;
+        reinterpret_cast<long long*>(&scratch[kScratchRec + 1])[1] = off;
+        if (acc <= kMaxAccAsync) {
+          for (int k = 0; k < 3; ++k)
+            for (int i = 0; i < acc; ++i)
+              cp_async16(scratch_addr + (k * acc + i) * 16,
+                         p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
+        }
+        cp_async_commit();
+        pend = true;
       }
-      cp_async_commit();
     }
-    pend = true;
   };
 
   for (int g = g_begin; g < g_end;) {
     const Segment c = decode_segment(p, g, g_end);
     g += c.nsteps - 2;
-    const int tx = c.gx * p.ntw + warp;
-    if (tx >= p.Tx) {
+    const int tx = c.gx * p.ntw + warp;  // this warp's 32x32 block
+    if (tx >= p.Tx32) {
       for (int s = 0; s < c.nsteps * acc; ++s) skip();
       continue;
     }
@@ -456,7 +489,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       if (++step >= c.nsteps) break;
     }
   }
-  if (lane == 0 && pend) resolve_pending();
+  if (leader && pend) resolve_pending();
   // ---- global maximum (a5): zero-filled out-of-bounds pixels are harmless because M >= C > 0 ----
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);

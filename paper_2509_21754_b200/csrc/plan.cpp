@@ -51,14 +51,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
   return FITRIG_OK;
 }
 
-// Fused path: one persistent CTA per SM; the CTAs share the G = boxes * U (box column, unit) pairs
-// evenly (see kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8
-// adjacent tiles is 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes
-// of 32 KB in flight per SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
-void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan) {
+// Fused path: one persistent CTA per SM; a consumer warp owns a 32x32 pixel block = (32 / N_T)^2 tiles for
+// N_T = 32, 16 or 8, and the CTAs share the G = boxes * U (box column, unit) pairs evenly (see
+// kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8 adjacent blocks is
+// 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes of 32 KB in flight per
+// SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
+bool fused_tile(int tile) { return tile == 32 || tile == 16 || tile == 8; }
+
+void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
   const bool force_generic = env_int("FITRIG_FORCE_GENERIC", 0) != 0;
-  if (tile != kFastTile || (W % 4) != 0 || force_generic) {
+  if (!fused_tile(tile) || (W % 4) != 0 || force_generic) {
     plan->path = 1;
     plan->units_per_cta = 0;
     plan->box_tiles = 0;
@@ -69,16 +72,19 @@ void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fit
     return;
   }
   plan->path = 0;
+  const int rows32 = (rows + kFastTile - 1) / kFastTile, Tx32 = (W + kFastTile - 1) / kFastTile;
   const int fb = env_int("FITRIG_BOX_TILES", 0), fs = env_int("FITRIG_STAGES", 0), fg = env_int("FITRIG_GRID", 0);
-  int ntw = std::min(kMaxTilesPerBox, Tx);
-  auto pairs = [&](int n) { return (long long)tile_rows * ((Tx + n - 1) / n) * U; };
+  int ntw = std::min(kMaxTilesPerBox, Tx32);
+  auto pairs = [&](int n) { return (long long)rows32 * ((Tx32 + n - 1) / n) * U; };
   // small problems are latency bound: narrower boxes give more CTAs something to do
   while (ntw > 1 && (pairs(ntw) + kMinUnitsPerCta - 1) / kMinUnitsPerCta < num_sms) ntw = (ntw + 1) / 2;
-  if (fb > 0) ntw = std::max(1, std::min(fb, std::min(kMaxTilesPerBox, Tx)));
+  if (fb > 0) ntw = std::max(1, std::min(fb, std::min(kMaxTilesPerBox, Tx32)));
   const long long G = pairs(ntw);
   int grid = (int)std::max<long long>(1, std::min<long long>(num_sms, (G + kMinUnitsPerCta - 1) / kMinUnitsPerCta));
   if (fg > 0) grid = fg;
-  const int fit = (kMaxSmemPerCta - 2048) / (ntw * kTileBytes);
+  const int groups = (kFastTile / tile) * (kFastTile / tile);  // tiles per warp, each with its own arg-max scratch
+  const int scratch = ntw * groups * kScratchVec * 16;
+  const int fit = (kMaxSmemPerCta - 2048 - scratch) / (ntw * kTileBytes);
   int stages = std::min(6, fit);
   if (fs > 0) stages = std::min(fs, fit);
   stages = std::max(2, std::min(stages, kMaxStages));
@@ -87,7 +93,7 @@ void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fit
   plan->stages = stages;
   plan->grid = grid;
   plan->units_per_cta = (int32_t)((G + grid - 1) / grid);
-  plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + ntw * kScratchVec * 16;  // ring, mbarriers, scratch
+  plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + scratch;  // ring, mbarriers, scratch
 }
 
 }  // namespace fitrig
@@ -111,7 +117,8 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   if (rows == 0) {
     const long long target = 256ll << 20;
     rows = target / ((long long)L * W * 4);
-    rows = std::max<long long>(tile, rows / tile * tile);
+    const long long q = (kFastTile % tile == 0) ? kFastTile : tile;  // whole 32-row blocks for the fused path
+    rows = std::max<long long>(q, rows / q * q);
   }
   const long long Hpad = (long long)out->Ty * tile;
   rows = std::min(rows, Hpad);
@@ -119,7 +126,7 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   out->n_strips = (int32_t)((H + rows - 1) / rows);
   out->n_strip_buffers = out->n_strips >= 3 ? 3 : out->n_strips;
   out->strip_buffer_bytes = (int64_t)L * rows * W * 4;
-  plan_launch(tile, W, out->Ty, out->Tx, out->units, num_sms, out);
+  plan_launch(tile, W, H, out->units, num_sms, out);
   const int64_t n = (int64_t)out->units * out->Ty * out->Tx;
   out->workspace_bytes = n * (16 + 4 + 4) + (int64_t)out->Ty * out->Tx * 8 + (1 << 20);
   return FITRIG_OK;

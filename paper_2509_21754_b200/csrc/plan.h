@@ -6,8 +6,8 @@
 
 namespace fitrig {
 
-constexpr int kFastTile = 32;          // tile edge of the fused path (the paper's default)
-constexpr int kTileBytes = 32 * 32 * 4;  // one 32x32 fp32 tile = one TMA box
+constexpr int kFastTile = 32;          // pixel block edge of the fused path = the paper's default tile
+constexpr int kTileBytes = 32 * 32 * 4;  // one 32x32 fp32 block
 constexpr int kMaxSmemPerCta = 227 * 1024;
 constexpr int kMaxTilesPerBox = 8;     // fused path: tiles per TMA box (256 columns, the TMA box limit) = consumer warps per CTA
 constexpr int kMaxStages = 8;          // fused path: deepest ring of boxes
@@ -32,7 +32,9 @@ struct NormParams {  // fitrig_params with defaults applied
 int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, NormParams* out, const char** why);
 
 // Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
-void plan_launch(int tile, int W, int tile_rows, int Tx, int U, int num_sms, fitrig_plan* plan);
+// `rows`: image rows covered by the launch (the whole image, or one strip).
+void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan);
+bool fused_tile(int tile);  // N_T the fused kernel is instantiated for: 32, 16, 8
 
 // Debug/tuning overrides: FITRIG_BOX_TILES, FITRIG_STAGES, FITRIG_GRID, FITRIG_EVICT_FIRST, FITRIG_FORCE_GENERIC (integers).
 int env_int(const char* name, int dflt);

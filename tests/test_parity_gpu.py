@@ -137,7 +137,7 @@ def test_tiny_default_tile_all_reference_modes(tiny, ref_mode):
 
 
 @pytest.mark.parametrize("tile", [1, 2, 4, 8, 16, 64, 5, 100])
-def test_tiny_tile_sweep_generic_path(tiny, tile):
+def test_tiny_tile_sweep(tiny, tile):  # 8 and 16 take the fused kernel (sub-tiles of a warp's 32x32 block)
     st, truth = tiny
     taus = (3.0, 4.0, 5.0, 6.0)
     g = gpu_run(st, taus=taus, tile=tile, capacity=1 << 18)
@@ -149,13 +149,14 @@ def test_tiny_tile_sweep_generic_path(tiny, tile):
         assert any(int(r["x"]) == t.x and int(r["y"]) == t.y and int(r["snapshot"]) in (0, 2, 4) for r in c)
 
 
-@pytest.mark.parametrize("H,W", [(250, 252), (250, 250), (33, 36), (32, 32), (31, 64)])
-def test_partial_edge_tiles_and_odd_shapes(tiny, H, W):
+@pytest.mark.parametrize("tile", [32, 16, 8])
+@pytest.mark.parametrize("H,W", [(250, 252), (250, 250), (33, 36), (32, 32), (31, 64), (40, 72), (9, 12)])
+def test_partial_edge_tiles_and_odd_shapes(tiny, H, W, tile):
     st = tiny[0][:, :H, :W].contiguous()
-    taus = (2.0, 3.0)
-    g = gpu_run(st, taus=taus)
-    ref = oracle_run(st, tile=32, tau=3.0)
-    check_against_oracle(st, g, ref, taus, 32)
+    taus = (2.0, 3.0) if (H // tile) * (W // tile) > 12 else (0.5,)
+    g = gpu_run(st, taus=taus, tile=tile)
+    ref = oracle_run(st, tile=tile, tau=taus[-1])
+    check_against_oracle(st, g, ref, taus, tile)
 
 
 def test_unaligned_base_pointer_falls_back_to_generic_kernel(tiny):
@@ -178,31 +179,33 @@ def test_m_override_scales_q_but_not_candidates(tiny):
     assert [tuple(r)[:3] for r in g1["cands"][4.0][0]] == [tuple(r)[:3] for r in g2["cands"][4.0][0]]  # P7
 
 
-def test_work_partition_does_not_change_the_map(tiny, monkeypatch):
+@pytest.mark.parametrize("tile", [32, 16, 8])
+def test_work_partition_does_not_change_the_map(tiny, monkeypatch, tile):
     """The per-CTA ranges of (box, unit) pairs cut tiles' time series at different places for different box
     widths / grids / ring depths; the per-tile results must not depend on where the cuts fall, on which warp of
     a box owns the tile, or on boxes that hang over the image edge (box width 3 or 5 on an 8-tile row)."""
     st, _ = tiny
     monkeypatch.setenv("FITRIG_BOX_TILES", "1")
     monkeypatch.setenv("FITRIG_GRID", "1")
-    a = gpu_run(st)  # one consumer warp walks all 384 pairs: no cut inside any tile
+    a = gpu_run(st, tile=tile)  # one consumer warp walks all 384 pairs: no cut inside any tile
     for box, grid, stages in ((3, 7, 2), (8, 148, 6), (5, 13, 3), (8, 5, 7), (2, 40, 8)):
         monkeypatch.setenv("FITRIG_BOX_TILES", str(box))
         monkeypatch.setenv("FITRIG_GRID", str(grid))
         monkeypatch.setenv("FITRIG_STAGES", str(stages))
         for evict in ("0", "1"):
             monkeypatch.setenv("FITRIG_EVICT_FIRST", evict)
-            b = gpu_run(st)
+            b = gpu_run(st, tile=tile)
             assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
             for x, y in zip(a["raw"], b["raw"]):
                 assert np.array_equal(x, y)
 
 
-def test_fused_and_generic_kernels_agree(tiny, monkeypatch):
+@pytest.mark.parametrize("tile", [32, 16, 8])
+def test_fused_and_generic_kernels_agree(tiny, monkeypatch, tile):
     st, _ = tiny
-    a = gpu_run(st)
+    a = gpu_run(st, tile=tile)
     monkeypatch.setenv("FITRIG_FORCE_GENERIC", "1")
-    b = gpu_run(st)
+    b = gpu_run(st, tile=tile)
     assert np.array_equal(a["raw"][1], b["raw"][1])  # max Delta exact
     assert np.array_equal(a["raw"][3], b["raw"][3]) and np.array_equal(a["raw"][4], b["raw"][4])
     np.testing.assert_allclose(a["q"], b["q"], rtol=1e-5)
@@ -298,23 +301,27 @@ def test_repeated_calls_on_one_context_are_reproducible(tiny):
 # ------------------------------------------------------------------------------------------
 # streaming (a9)
 # ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("H,W,strip", [(256, 256, 64), (250, 252, 96), (300, 200, 32), (250, 250, 64)])
-def test_stream_equals_resident_and_oracle(tiny, H, W, strip):
+@pytest.mark.parametrize("H,W,strip,tile", [(256, 256, 64, 32), (250, 252, 96, 32), (300, 200, 32, 32), (250, 250, 64, 32),
+                                            (250, 252, 64, 16), (300, 200, 96, 8), (256, 256, 48, 16), (256, 256, 0, 8)])
+def test_stream_equals_resident_and_oracle(tiny, H, W, strip, tile):
+    # strips of 48 rows with 16-pixel tiles do not start on 32-row blocks: those launches take the generic kernel
     base = synth.gaussian_noise_stack(6, 320, 256, seed=7, device=DEV)
     st = base[:, :H, :W].contiguous()
     taus = (2.5,)
-    a = gpu_run(st, taus=taus)
-    b = gpu_run(st, taus=taus, use_stream=True, strip_rows=strip)
-    assert np.array_equal(a["q"], b["q"]) and a["M"] == b["M"]
-    assert np.array_equal(a["cands"][2.5][0], b["cands"][2.5][0])
-    ref = oracle_run(st, tile=32, tau=2.5)
-    check_against_oracle(st, b, ref, taus, 32)
+    a = gpu_run(st, taus=taus, tile=tile)
+    b = gpu_run(st, taus=taus, use_stream=True, strip_rows=strip, tile=tile)
+    if strip != 48:
+        assert np.array_equal(a["q"], b["q"])
+        assert np.array_equal(a["cands"][2.5][0], b["cands"][2.5][0])
+    assert a["M"] == b["M"]
+    ref = oracle_run(st, tile=tile, tau=2.5)
+    check_against_oracle(st, b, ref, taus, tile)
 
 
 def test_stream_generic_tile(tiny):
     st = tiny[0]
-    a = gpu_run(st, taus=(4.0,), tile=8)
-    b = gpu_run(st, taus=(4.0,), tile=8, use_stream=True, strip_rows=40)
+    a = gpu_run(st, taus=(4.0,), tile=4)
+    b = gpu_run(st, taus=(4.0,), tile=4, use_stream=True, strip_rows=40)
     assert np.array_equal(a["q"], b["q"]) and np.array_equal(a["cands"][4.0][0], b["cands"][4.0][0])
 
 
@@ -371,7 +378,8 @@ def long_tiny():
 
 @pytest.mark.parametrize("g,H,W,tile,use_stream", [(2, 256, 256, 32, False), (3, 250, 252, 32, False), (4, 256, 256, 32, True),
                                                    (5, 256, 256, 32, False), (6, 128, 96, 32, True), (2, 120, 100, 8, False),
-                                                   (3, 64, 64, 1, False)])
+                                                   (3, 64, 64, 1, False), (2, 250, 252, 16, False), (5, 256, 256, 8, True),
+                                                   (3, 120, 98, 16, False)])
 def test_accumulated_snapshots_match_oracle(long_tiny, g, H, W, tile, use_stream):
     st, _ = long_tiny
     st = st[:, :H, :W].contiguous()
@@ -419,7 +427,7 @@ def _push_all(ctx, snaps, tau, want_maps=True):
 
 
 @pytest.mark.parametrize("H,W,tile,on_device", [(256, 256, 32, False), (250, 252, 32, False), (256, 256, 32, True),
-                                                (120, 100, 8, False)])
+                                                (120, 100, 8, False), (250, 252, 16, False), (120, 102, 8, False)])
 def test_push_realtime_matches_oracle(tiny, H, W, tile, on_device):
     st, _ = tiny
     st = st[:, :H, :W].contiguous()
