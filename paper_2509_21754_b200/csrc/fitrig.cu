@@ -69,6 +69,9 @@ struct fitrig_ctx {
   EncodeTiledFn encode;
   // map
   RawTile* raw;
+  RawTile* raw_blocks;  // N_T = 32 * m > 32: one record per 32x32 block, merged into `raw` before the finalise
+  int Ty32, Tx32;
+  bool blocks_pending;  // the last tLISI launches wrote raw_blocks (fused path), not raw (generic path)
   float *q, *tlisi, *M_dev;
   unsigned* gmax_key;  // two order-preserving keys of the running global maximum, used by alternate calls:
   int key_idx;         // the finalise kernel of one call zeroes the key of the next, so no memset sits in the stream
@@ -121,7 +124,7 @@ static void free_ctx(fitrig_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->prm.device);
   cudaDeviceSynchronize();
-  cudaFree(c->raw); cudaFree(c->q); cudaFree(c->tlisi); cudaFree(c->M_dev); cudaFree(c->gmax_key);
+  cudaFree(c->raw); cudaFree(c->raw_blocks); cudaFree(c->q); cudaFree(c->tlisi); cudaFree(c->M_dev); cudaFree(c->gmax_key);
   cudaFree(c->parts); cudaFree(c->counters); cudaFree(c->mu); cudaFree(c->sigma);
   cudaFree(c->eta); cudaFree(c->kstar); cudaFree(c->tw); cudaFree(c->sparts); cudaFree(c->scounter);
   cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cand_dev); cudaFree(c->blk_counts);
@@ -229,6 +232,9 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   c->encode = (EncodeTiledFn)fn;
 
   CTX_TRY(cudaMalloc(&c->raw, sizeof(RawTile) * c->nmap));
+  c->Ty32 = (H + kFastTile - 1) / kFastTile; c->Tx32 = (W + kFastTile - 1) / kFastTile;
+  if (np.tile > kFastTile && np.tile % kFastTile == 0)
+    CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)c->U * c->Ty32 * c->Tx32));
   CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->tlisi, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float)));
@@ -341,11 +347,12 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
-    fp.raw = c->raw; fp.gmax_key = key;
+    const bool big = tile > kFastTile;  // blocks of a 32 * m tile: the kernel sees a grid of 32-pixel tiles
+    fp.raw = big ? c->raw_blocks : c->raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmod = opt.zmod; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
-    fp.Tx = c->Tx; fp.Ty = c->Ty; fp.Tx32 = (c->W + kFastTile - 1) / kFastTile;
-    fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = ty_base;
+    fp.Tx = big ? c->Tx32 : c->Tx; fp.Ty = big ? c->Ty32 : c->Ty; fp.Tx32 = c->Tx32;
+    fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = big ? ty_base * (tile / kFastTile) : ty_base;
     fp.U = c->U;
     fp.ntw = pl.box_tiles; fp.ngx = (fp.Tx32 + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
     const long long G = (long long)fp.rows_tiles * fp.ngx * c->U;
@@ -361,6 +368,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;
+    if (big) c->blocks_pending = true;
   } else {
     if (with_max) {
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
@@ -398,6 +406,16 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
 }
 
 static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, unsigned* key = nullptr) {
+  if (c->raw_blocks && c->blocks_pending) {  // N_T = 32 * m: block records -> tile records
+    MergeParams mp;
+    mp.blocks = c->raw_blocks; mp.raw = c->raw; mp.U = c->U; mp.Ty = c->Ty; mp.Tx = c->Tx;
+    mp.Ty32 = c->Ty32; mp.Tx32 = c->Tx32; mp.m = c->prm.tile / kFastTile; mp.tile = c->prm.tile;
+    const long long n = c->nmap;
+    merge_blocks_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4 * c->num_sms), 256, 0, st>>>(mp);
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+    c->blocks_pending = false;
+  }
   FinalizeParams fp;
   fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
   fp.gmax_key = key ? key : c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1);

@@ -495,6 +495,44 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
 }
 // ---------------------------------------------------------------------------------------------
+// Tiles of N_T = 32 * m pixels: the fused kernel (T = 32) leaves one record per 32x32 block; a tile is the
+// union of m x m blocks (fewer at the image edge).  Sum Delta and sum r add up, max Delta is the max, and the
+// first max-Delta pixel in row-major order OF THE TILE (R20) is the candidate with the smallest
+// row * N_T + col among the blocks that attain the max.
+// ---------------------------------------------------------------------------------------------
+struct MergeParams {
+  const RawTile* blocks;  // [U][Ty32][Tx32]
+  RawTile* raw;           // [U][Ty][Tx]
+  int U, Ty, Tx, Ty32, Tx32, m, tile;
+};
+
+__global__ void __launch_bounds__(256) merge_blocks_kernel(const MergeParams p) {
+  const long long n = (long long)p.U * p.Ty * p.Tx;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int u = (int)(i / ((long long)p.Ty * p.Tx));
+    const int t = (int)(i - (long long)u * p.Ty * p.Tx);
+    const int ty = t / p.Tx, tx = t - ty * p.Tx;
+    RawTile o;
+    o.sumD = 0.f; o.maxD = 0.f; o.sumR = 0.f; o.pos = 0x7fffffff;
+    bool first = true;
+    for (int by = 0; by < p.m; ++by) {
+      const int y32 = ty * p.m + by;
+      if (y32 >= p.Ty32) break;
+      for (int bx = 0; bx < p.m; ++bx) {
+        const int x32 = tx * p.m + bx;
+        if (x32 >= p.Tx32) break;
+        const RawTile b = p.blocks[((size_t)u * p.Ty32 + y32) * p.Tx32 + x32];
+        o.sumD += b.sumD;  // fixed (block row, block column) order: deterministic
+        o.sumR += b.sumR;
+        const int pos = (by * kFastTile + b.pos / kFastTile) * p.tile + bx * kFastTile + b.pos % kFastTile;
+        if (first || b.maxD > o.maxD || (b.maxD == o.maxD && pos < o.pos)) { o.maxD = b.maxD; o.pos = pos; first = false; }
+      }
+    }
+    p.raw[i] = o;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Generic path: any tile size, any width / alignment.  G (power of two <= 32) lanes share one tile.
 // ---------------------------------------------------------------------------------------------
 struct GenericParams {

@@ -32,8 +32,9 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 1)  # W % 4 != 0 -> generic kernel
     p = fitrig.plan_query(250, 252, 8, tile=8)
     assert (p.Ty, p.Tx, p.path) == (32, 32, 0) and p.strip_rows % 32 == 0  # N_T = 8, 16 ride the fused kernel
-    assert fitrig.plan_query(250, 252, 8, tile=16).path == 0 and fitrig.plan_query(250, 252, 8, tile=64).path == 1
-    assert fitrig.plan_query(250, 252, 8, tile=5).path == 1
+    assert fitrig.plan_query(250, 252, 8, tile=16).path == 0
+    assert fitrig.plan_query(250, 252, 8, tile=64).path == 0 and fitrig.plan_query(250, 252, 8, tile=96).path == 0  # 32 * m
+    assert fitrig.plan_query(250, 252, 8, tile=5).path == 1 and fitrig.plan_query(250, 252, 8, tile=48).path == 1
     p = fitrig.plan_query(256, 250, 8)
     assert p.path == 1  # W % 4 != 0: rows are not 16-byte aligned, no TMA
     p = fitrig.plan_query(256, 252, 8)

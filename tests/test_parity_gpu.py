@@ -149,7 +149,7 @@ def test_tiny_tile_sweep(tiny, tile):  # 8 and 16 take the fused kernel (sub-til
         assert any(int(r["x"]) == t.x and int(r["y"]) == t.y and int(r["snapshot"]) in (0, 2, 4) for r in c)
 
 
-@pytest.mark.parametrize("tile", [32, 16, 8])
+@pytest.mark.parametrize("tile", [32, 16, 8, 64, 96])
 @pytest.mark.parametrize("H,W", [(250, 252), (250, 250), (33, 36), (32, 32), (31, 64), (40, 72), (9, 12)])
 def test_partial_edge_tiles_and_odd_shapes(tiny, H, W, tile):
     st = tiny[0][:, :H, :W].contiguous()
@@ -200,7 +200,7 @@ def test_work_partition_does_not_change_the_map(tiny, monkeypatch, tile):
                 assert np.array_equal(x, y)
 
 
-@pytest.mark.parametrize("tile", [32, 16, 8])
+@pytest.mark.parametrize("tile", [32, 16, 8, 64, 128])
 def test_fused_and_generic_kernels_agree(tiny, monkeypatch, tile):
     st, _ = tiny
     a = gpu_run(st, tile=tile)
@@ -302,7 +302,8 @@ def test_repeated_calls_on_one_context_are_reproducible(tiny):
 # streaming (a9)
 # ------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("H,W,strip,tile", [(256, 256, 64, 32), (250, 252, 96, 32), (300, 200, 32, 32), (250, 250, 64, 32),
-                                            (250, 252, 64, 16), (300, 200, 96, 8), (256, 256, 48, 16), (256, 256, 0, 8)])
+                                            (250, 252, 64, 16), (300, 200, 96, 8), (256, 256, 48, 16), (256, 256, 0, 8),
+                                            (300, 200, 128, 64), (250, 252, 96, 96)])
 def test_stream_equals_resident_and_oracle(tiny, H, W, strip, tile):
     # strips of 48 rows with 16-pixel tiles do not start on 32-row blocks: those launches take the generic kernel
     base = synth.gaussian_noise_stack(6, 320, 256, seed=7, device=DEV)
