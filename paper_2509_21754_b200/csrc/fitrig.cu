@@ -65,6 +65,7 @@ struct fitrig_ctx {
   int H, W, L, U, Ty, Tx;
   long long nt, nmap;
   int num_sms;
+  long long max_pitch;
   fitrig_plan plan;
   EncodeTiledFn encode;
   // map
@@ -201,6 +202,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   c->prm = np;
   c->H = H; c->W = W; c->L = L; c->U = L / np.accumulate - 2;
   c->num_sms = prop.multiProcessorCount;
+  c->max_pitch = (long long)prop.memPitch;
   rc = fitrig_plan_query(H, W, L, params, c->num_sms, &c->plan);
   if (rc != FITRIG_OK) { delete c; return fail(rc, "fitrig_create: plan failed"); }
   c->Ty = c->plan.Ty; c->Tx = c->plan.Tx;
@@ -481,14 +483,33 @@ extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, flo
   CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
   for (int b = 0; b < nbuf; ++b) c->ev_free_pending[b] = false;
   const long long snap_stride = (long long)rows_per * c->W;
+  // snapshots that sit at a constant distance in host memory (one [L][H][W] allocation, the usual case) let a
+  // strip travel as one pitched copy instead of L small ones; pitches are limited to cudaDeviceProp::memPitch
+  long long host_stride = h_snapshots[1] - h_snapshots[0];
+  bool pitched = host_stride >= (long long)c->H * c->W && host_stride * 4 <= c->max_pitch && snap_stride * 4 <= c->max_pitch &&
+                 env_int("FITRIG_NO_PITCHED_COPY", 0) == 0;
+  for (int s = 2; s < c->L && pitched; ++s) pitched = (h_snapshots[s] - h_snapshots[s - 1]) == host_stride;
   for (int i = 0; i < nstrips; ++i) {
     const int b = i % nbuf;
     const int r0 = i * rows_per;
     const int rows = std::min(rows_per, c->H - r0);
     if (c->ev_free_pending[b]) CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_free[b], 0));
-    for (int s = 0; s < c->L; ++s) {  // snapshot s, rows r0..r0+rows: contiguous on both sides
-      CUDA_TRY(cudaMemcpyAsync(c->strip_buf[b] + (long long)s * snap_stride, h_snapshots[s] + (long long)r0 * c->W,
-                               sizeof(float) * (long long)rows * c->W, cudaMemcpyHostToDevice, c->copy_stream));
+    if (pitched) {  // equally spaced snapshots: the whole strip (L row blocks) is ONE pitched copy
+      cudaError_t e2 = cudaMemcpy2DAsync(c->strip_buf[b], sizeof(float) * snap_stride, h_snapshots[0] + (long long)r0 * c->W,
+                                         sizeof(float) * host_stride, sizeof(float) * (long long)rows * c->W, c->L,
+                                         cudaMemcpyHostToDevice, c->copy_stream);
+      if (e2 == cudaErrorInvalidValue) {  // equally spaced but separate allocations: the range check refuses
+        (void)cudaGetLastError();
+        pitched = false;
+      } else {
+        CUDA_TRY(e2);
+      }
+    }
+    if (!pitched) {
+      for (int s = 0; s < c->L; ++s) {  // snapshot s, rows r0..r0+rows: contiguous on both sides
+        CUDA_TRY(cudaMemcpyAsync(c->strip_buf[b] + (long long)s * snap_stride, h_snapshots[s] + (long long)r0 * c->W,
+                                 sizeof(float) * (long long)rows * c->W, cudaMemcpyHostToDevice, c->copy_stream));
+      }
     }
     CUDA_TRY(cudaEventRecord(c->ev_copied[b], c->copy_stream));
     CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copied[b], 0));
