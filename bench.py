@@ -52,13 +52,17 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--channels", type=int, default=0, help="imgfreq only: use the first N of the 16 channels")
+    ap.add_argument("--tile", type=int, default=32, help="N_T (the paper's default and BASELINE.json's is 32)")
     return ap.parse_args()
+
+
+TILE = 32  # N_T of this run (--tile)
 
 
 def workload_desc(cfg, tau, branch, n_ch=1):
     return (f"{cfg.name}: {f'{n_ch} channels x ' if n_ch > 1 else ''}{cfg.L} snapshots x {cfg.H}x{cfg.W} fp32 "
             f"(BASELINE.json configs[{cfg.cfg_index - 1}]), "
-            f"N_T=32, tau={tau:g}, branch={'image-frequency' if branch else 'image'}")
+            f"N_T={TILE}, tau={tau:g}, branch={'image-frequency' if branch else 'image'}")
 
 
 # ---------------------------------------------------------------------------------------------
@@ -134,7 +138,7 @@ def oracle_sample_rate(snaps, rows, tau, branch, repeats=1):
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        oracle.run(sub, tile=32, tau=tau, branch=branch)
+        oracle.run(sub, tile=TILE, tau=tau, branch=branch)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return best
@@ -244,7 +248,7 @@ def run_fitrig(args, cfg, tau, branch):
     stack = stacks[0]
     L, H, W = stack.shape
     pix = L * H * W * n_ch
-    ctx = fitrig.Context(H, W, L, device=local, branch=branch)
+    ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE)
     U, Ty, Tx = ctx.map_dims()
     d_tl = torch.empty((U, Ty, Tx), dtype=torch.float32, device=dev)
     cap = 1 << 16
@@ -282,14 +286,15 @@ def run_fitrig(args, cfg, tau, branch):
     value = world * pix * args.steps / (ms_max * 1e-3) / 1e6
 
     # ---- roofline of the dominant (fused) kernel ----
-    plan = fitrig.plan_query(H, W, L, num_sms=torch.cuda.get_device_properties(local).multi_processor_count)
+    plan = fitrig.plan_query(H, W, L, num_sms=torch.cuda.get_device_properties(local).multi_processor_count, tile=TILE)
     # one launch = one channel's stack: every snapshot pixel read once + one 16-byte record per tile and unit
     alg_bytes = 4 * (pix // n_ch) + 16 * U * Ty * Tx
+    traffic = NCU_TRAFFIC_BYTES.get(cfg.name) if TILE == 32 else None
     k_ms = main_tot / max(main_n, 1)
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(cfg.name), "kernel": "tlisi_fused_kernel" if plan.path == 0 else
+                "traffic": traffic, "kernel": "tlisi_fused_kernel" if plan.path == 0 else
                 "tlisi_generic_kernel", "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "finalize_ms": fin_tot / max(fin_n, 1), "kernel_launches_timed": main_n, "kernel_share_of_step": k_ms * n_ch * args.steps / ms}
 
@@ -334,7 +339,7 @@ def run_fitrig(args, cfg, tau, branch):
                             "peak_source": "pinned 1 GiB cudaMemcpyAsync H2D, best of 10, this run"}}
         # ---- real-time leg: fitrig_push, one snapshot per call from pinned host memory (Fig. 14 timeline) ----
         if branch == 0:
-            pctx = fitrig.Context(H, W, 3, device=local)
+            pctx = fitrig.Context(H, W, 3, device=local, tile=TILE)
             snaps0 = hosts[0]
 
             def push_pass():
@@ -380,7 +385,7 @@ def run_fitrig(args, cfg, tau, branch):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_desc(cfg, tau, branch, n_ch), "tile": 32, "tau": tau,
+            "config": {"workload": workload_desc(cfg, tau, branch, n_ch), "tile": TILE, "tau": tau,
                        "candidates_per_step": int(n_found),
                        "l2": f"input {4 * pix / 1e6:.0f} MB per step vs 126 MB L2: "
                              + ("larger than L2, no flush" if 4 * pix > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
@@ -396,7 +401,9 @@ def run_fitrig(args, cfg, tau, branch):
 
 
 def main():
+    global TILE
     args = parse_args()
+    TILE = args.tile
     import synth
     cfg = synth.CONFIGS[args.workload]
     tau = args.tau if args.tau is not None else cfg.tau

@@ -443,7 +443,8 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       const int u = c.u0 + step - 2;
       const int ty_t = p.ty_base + c.ty_local * Geo::NSUB + Geo::sub_row(lane);  // tile coordinates in the whole map
       const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
-      if (ty_t < p.Ty && tx_t < p.Tx) {  // (tiles of a block that hang over the image edge do not exist)
+      // (tiles of a block that hang over the image edge do not exist; a 32-pixel tile always does)
+      if (Geo::NSUB == 1 || (ty_t < p.Ty && tx_t < p.Tx)) {
         scratch[kScratchRec] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
         // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
         const long long off = (long long)(c.ty_local * kFastTile + Geo::sub_row(lane) * T + (int)(tg / T)) * p.W +
