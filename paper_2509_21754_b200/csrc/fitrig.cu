@@ -52,7 +52,8 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 static const int kMaxStripBuffers = 3;
-static const int kPushSlots = 4;  // x_n, x_{n+1}, x_{n+2} of the unit being computed + the snapshot being copied
+static const int kPushSlots = 4;  // (a power of two: the kernels map ring slots with a mask)
+// x_n, x_{n+1}, x_{n+2} of the unit being computed + the snapshot being copied
 static const long long kHostStageCands = 4096;  // candidates fetched together with the count
 
 struct CandHeader {
@@ -351,7 +352,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     FusedParams fp;
     const bool big = tile > kFastTile;  // blocks of a 32 * m tile: the kernel sees a grid of 32-pixel tiles
     fp.raw = big ? c->raw_blocks : c->raw; fp.gmax_key = key;
-    fp.z0 = opt.z0; fp.zmod = opt.zmod; fp.acc = c->prm.accumulate;
+    fp.z0 = opt.z0; fp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = big ? c->Tx32 : c->Tx; fp.Ty = big ? c->Ty32 : c->Ty; fp.Tx32 = c->Tx32;
     fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = big ? ty_base * (tile / kFastTile) : ty_base;
@@ -390,7 +391,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     const long long n_t = (long long)tile * tile;
     while (G < 32 && G < n_t) G <<= 1;
     gp.G = G;
-    gp.z0 = opt.z0; gp.zmod = opt.zmod; gp.acc = c->prm.accumulate;
+    gp.z0 = opt.z0; gp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; gp.acc = c->prm.accumulate;
     gp.C = c->prm.C;
     const long long groups = (long long)rows_tiles * c->Tx * c->U;
     const long long threads = groups * G;

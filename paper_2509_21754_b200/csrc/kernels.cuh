@@ -143,12 +143,13 @@ struct FusedParams {
   int nstage;            // depth of the CTA's ring of boxes
   int G;                 // rows_tiles * ngx * U: (box column, unit) pairs of this launch, box-major
   int evict_first;       // L2 policy of the streaming loads
-  int z0, zmod;          // real-time mode: snapshot s of the launch lives in slot (z0 + s) % zmod of a ring; zmod = 0: slot s
+  int z0, zmask;         // snapshot s of the launch lives in slot (z0 + s) & zmask: real-time ring of 4 slots: zmask = 3;
+                         // a plain stack: z0 = 0, zmask = 0x7fffffff (no modulo, no branch in the lane-0 paths)
   int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
   float C;
 };
 
-__device__ __forceinline__ int ring_slot(int z0, int zmod, int s) { return zmod ? (z0 + s) % zmod : s; }
+__device__ __forceinline__ int ring_slot(int z0, int zmask, int s) { return (z0 + s) & zmask; }
 
 // Work distribution: a "group" is a row of ntw horizontally adjacent tiles, fetched as ONE TMA box of
 // 32 rows x (ntw * 128) contiguous bytes (isolated 128-byte rows cost ~15 % of the HBM bandwidth, see
@@ -333,10 +334,10 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
           mbar_arrive_expect_tx(bar, box_bytes);
           if (p.evict_first)
             tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                              ring_slot(p.z0, p.zmod, c.u0 * acc + s), policy);
+                              ring_slot(p.z0, p.zmask, c.u0 * acc + s), policy);
           else
             tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                         ring_slot(p.z0, p.zmod, c.u0 * acc + s));
+                         ring_slot(p.z0, p.zmask, c.u0 * acc + s));
           if (++slot == p.nstage) { slot = 0; phase ^= 1; }
         }
       }
@@ -378,56 +379,55 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   };
 
   // ---- one record is always "pending": its arg-max group is known, the pixel inside it is not.
-  // The tile's leader lane parks it in the tile's scratch (registers are for the tile arrays): scratch[0 .. 3*acc) the
-  // re-read raw pixels of the three images, scratch[kScratchRec] = {sum Delta, sum r, max bits, group
-  // position}, scratch[kScratchRec + 1] = {map index, element offset of the group inside an image}.
+  // Everything the tile's leader lane does costs the whole warp an issue slot, so its path is kept short:
+  // the three image pointers of the current unit and the record pointer are carried along incrementally
+  // (ip0..ip2, rp below) instead of being rebuilt from indices.  The leader parks the record in the tile's
+  // scratch (registers are for the tile arrays): scratch[0 .. 3*acc) the re-read raw pixels of the three
+  // images, scratch[kScratchRec] = {sum Delta, max Delta, sum r, group position} (the RawTile layout),
+  // scratch[kScratchRec + 1] = {address of the map record}.
   bool pend = false;
   auto resolve_pending = [&]() {  // leader lanes only
     const float4 rec = scratch[kScratchRec];
-    const unsigned long long idx = reinterpret_cast<const unsigned long long*>(&scratch[kScratchRec + 1])[0];
+    RawTile* dst = *reinterpret_cast<RawTile* const*>(&scratch[kScratchRec + 1]);
+    cp_async_wait_all();
     float4 img[3];
-    if (acc <= kMaxAccAsync) {
-      cp_async_wait_all();
+    const int per_img = (acc <= kMaxAccAsync) ? acc : 1;  // parked quads per image
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        img[k] = scratch[k * acc];
+    for (int k = 0; k < 3; ++k) {
+      img[k] = scratch[k * per_img];
+      if (acc <= kMaxAccAsync) {
         for (int i = 1; i < acc; ++i) {  // the same order of fp32 additions as acquire()
           const float4 t = scratch[k * acc + i];
           img[k].x += t.x; img[k].y += t.y; img[k].z += t.z; img[k].w += t.w;
         }
       }
-    } else {  // long accumulations: plain (blocking) loads, L2 hits
-      const long long off = reinterpret_cast<const long long*>(&scratch[kScratchRec + 1])[1];
-      const int u = (int)(idx / ((unsigned long long)p.Ty * p.Tx));
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        img[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int i = 0; i < acc; ++i) {
-          const float4 t = *reinterpret_cast<const float4*>(
-              p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
-          if (i == 0) img[k] = t;
-          else { img[k].x += t.x; img[k].y += t.y; img[k].z += t.z; img[k].w += t.w; }
-        }
-      }
     }
     const float4 a = img[0], b = img[1], c = img[2];
-    const float mx = rec.z;
+    const float mx = rec.y;
     // the same three fp32 operations as tile_step -> bit-identical Delta
     const float e0 = fabsf(fabsf(c.x - b.x) - fabsf(b.x - a.x));
     const float e1 = fabsf(fabsf(c.y - b.y) - fabsf(b.y - a.y));
     const float e2 = fabsf(fabsf(c.z - b.z) - fabsf(b.z - a.z));
     const int e = (e0 == mx) ? 0 : (e1 == mx) ? 1 : (e2 == mx) ? 2 : 3;
-    RawTile o;
-    o.sumD = rec.x;
-    o.maxD = mx;
-    o.sumR = rec.y;
-    o.pos = __float_as_int(rec.w) + e;
-    *reinterpret_cast<float4*>(&p.raw[idx]) = *reinterpret_cast<float4*>(&o);
+    float4 o = rec;
+    o.w = __int_as_float(__float_as_int(rec.w) + e);
+    *reinterpret_cast<float4*>(dst) = o;
   };
+
+  // the unit being finished: its three images at this warp's block origin, and this lane's tile record
+  const float* ip0 = p.base;
+  const float* ip1 = p.base;
+  const float* ip2 = p.base;
+  RawTile* rp = p.raw;
+  bool tile_exists = true;
+  const long long raw_step = (long long)p.Ty * p.Tx;            // records per unit
+  const long long img_step = (long long)acc * p.snap_stride;    // elements between consecutive images (plain stack)
+  // position of this lane's tile inside the warp's block (0 for T = 32)
+  const int sub_off = Geo::sub_row(lane) * T * p.W + Geo::sub_col(lane) * T;
 
   // reduction of one (tile, unit) over the tile's lane group: exact max + first 16-byte group by redux, the two
   // sums by one butterfly (lower half of the group carries sum Delta, upper half sum r)
-  auto finish = [&](const Segment& c, int tx, int step, float S, float R, float Mx, int jmax) {
+  auto finish = [&](float S, float R, float Mx, int jmax) {
     const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
     const unsigned tmax = __reduce_max_sync(gmask, mbits);
     const int gpos = (Geo::row_in_tile(lane) + Geo::RPL * jmax) * T + Geo::col_in_tile(lane);  // row-major in the tile
@@ -440,28 +440,36 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     if (leader) {
       if (pend) resolve_pending();
       pend = false;
-      const int u = c.u0 + step - 2;
-      const int ty_t = p.ty_base + c.ty_local * Geo::NSUB + Geo::sub_row(lane);  // tile coordinates in the whole map
-      const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
-      // (tiles of a block that hang over the image edge do not exist; a 32-pixel tile always does)
-      if (Geo::NSUB == 1 || (ty_t < p.Ty && tx_t < p.Tx)) {
-        scratch[kScratchRec] = make_float4(vsum, rsum, __uint_as_float(tmax), __int_as_float((int)tg));
+      if (tile_exists) {  // (tiles of a block that hang over the image edge do not exist)
+        scratch[kScratchRec] = make_float4(vsum, __uint_as_float(tmax), rsum, __int_as_float((int)tg));
+        *reinterpret_cast<RawTile**>(&scratch[kScratchRec + 1]) = rp;
         // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
-        const long long off = (long long)(c.ty_local * kFastTile + Geo::sub_row(lane) * T + (int)(tg / T)) * p.W +
-                              (tx * kFastTile + Geo::sub_col(lane) * T + (int)(tg % T));
-        reinterpret_cast<unsigned long long*>(&scratch[kScratchRec + 1])[0] =
-            ((unsigned long long)u * p.Ty + ty_t) * p.Tx + tx_t;
-        reinterpret_cast<long long*>(&scratch[kScratchRec + 1])[1] = off;
+        const int off = sub_off + (int)(tg / T) * p.W + (int)(tg % T);
         if (acc <= kMaxAccAsync) {
-          for (int k = 0; k < 3; ++k)
-            for (int i = 0; i < acc; ++i)
-              cp_async16(scratch_addr + (k * acc + i) * 16,
-                         p.base + off + (long long)ring_slot(p.z0, p.zmod, (u + k) * acc + i) * p.snap_stride);
+          for (int i = 0; i < acc; ++i) {
+            cp_async16(scratch_addr + i * 16, ip0 + off + i * p.snap_stride);
+            cp_async16(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride);
+            cp_async16(scratch_addr + (2 * acc + i) * 16, ip2 + off + i * p.snap_stride);
+          }
+        } else {  // long accumulations: plain (blocking) loads, L2 hits; the three sums are parked as if acc were 1
+          const float* ip[3] = {ip0, ip1, ip2};
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            float4 v = *reinterpret_cast<const float4*>(ip[k] + off);
+            for (int i = 1; i < acc; ++i) {
+              const float4 t = *reinterpret_cast<const float4*>(ip[k] + off + i * p.snap_stride);
+              v.x += t.x; v.y += t.y; v.z += t.z; v.w += t.w;
+            }
+            scratch[k] = v;
+          }
         }
         cp_async_commit();
         pend = true;
       }
     }
+    // next unit of the segment (a plain stack: images are img_step apart; the ring mode has one unit per segment)
+    ip0 = ip1; ip1 = ip2; ip2 += img_step;
+    rp += raw_step;
   };
 
   for (int g = g_begin; g < g_end;) {
@@ -471,6 +479,16 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     if (tx >= p.Tx32) {
       for (int s = 0; s < c.nsteps * acc; ++s) skip();
       continue;
+    }
+    {
+      const long long blk = (long long)(c.ty_local * kFastTile) * p.W + tx * kFastTile;
+      ip0 = p.base + blk + (long long)ring_slot(p.z0, p.zmask, c.u0 * acc) * p.snap_stride;
+      ip1 = p.base + blk + (long long)ring_slot(p.z0, p.zmask, (c.u0 + 1) * acc) * p.snap_stride;
+      ip2 = p.base + blk + (long long)ring_slot(p.z0, p.zmask, (c.u0 + 2) * acc) * p.snap_stride;
+      const int ty_t = p.ty_base + c.ty_local * Geo::NSUB + Geo::sub_row(lane);  // tile coordinates in the whole map
+      const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
+      tile_exists = Geo::NSUB == 1 || (ty_t < p.Ty && tx_t < p.Tx);
+      rp = p.raw + ((long long)c.u0 * p.Ty + ty_t) * p.Tx + tx_t;
     }
     acquire(A, zA);  // x_{u0}
     acquire(B, zB);  // x_{u0+1}
@@ -482,11 +500,11 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       int jmax;
       acquire(A, zA);
       tile_step<REF_MODE>(A, B, dp, p.C, __any_sync(0xffffffffu, zB == 0.f), S, R, Mx, jmax);
-      finish(c, tx, step, S, R, Mx, jmax);
+      finish(S, R, Mx, jmax);
       if (++step >= c.nsteps) break;
       acquire(B, zB);
       tile_step<REF_MODE>(B, A, dp, p.C, __any_sync(0xffffffffu, zA == 0.f), S, R, Mx, jmax);
-      finish(c, tx, step, S, R, Mx, jmax);
+      finish(S, R, Mx, jmax);
       if (++step >= c.nsteps) break;
     }
   }
@@ -545,7 +563,7 @@ struct GenericParams {
   RawTile* raw;
   int Tx, Ty, ty_base, rows_tiles, U;
   int G;                    // lanes per tile
-  int z0, zmod;             // real-time mode ring (see FusedParams)
+  int z0, zmask;            // real-time mode ring (see FusedParams)
   int acc;                  // snapshot accumulation (see FusedParams)
   float C;
 };
@@ -570,8 +588,8 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
     const int h = min(p.tile, p.rows - r0), w = min(p.tile, p.W - c0);
     // image k of the unit = sum of raw snapshots (u + k) * acc .. + acc - 1, added in order
     auto image = [&](int k, long long o) {
-      float v = p.base[(long long)ring_slot(p.z0, p.zmod, (u + k) * p.acc) * p.snap_stride + o];
-      for (int i = 1; i < p.acc; ++i) v += p.base[(long long)ring_slot(p.z0, p.zmod, (u + k) * p.acc + i) * p.snap_stride + o];
+      float v = p.base[(long long)ring_slot(p.z0, p.zmask, (u + k) * p.acc) * p.snap_stride + o];
+      for (int i = 1; i < p.acc; ++i) v += p.base[(long long)ring_slot(p.z0, p.zmask, (u + k) * p.acc + i) * p.snap_stride + o];
       return v;
     };
     bool first = true;

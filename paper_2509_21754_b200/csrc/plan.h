@@ -12,7 +12,7 @@ constexpr int kMaxSmemPerCta = 227 * 1024;
 constexpr int kMaxTilesPerBox = 8;     // fused path: tiles per TMA box (256 columns, the TMA box limit) = consumer warps per CTA
 constexpr int kMaxStages = 8;          // fused path: deepest ring of boxes
 constexpr int kMinUnitsPerCta = 2;     // fused path: fewest (box column, unit) pairs worth a CTA of its own
-constexpr int kMaxAccAsync = 4;        // accumulations up to this length re-read their arg-max pixels with cp.async
+constexpr int kMaxAccAsync = 8;        // accumulations up to this length re-read their arg-max pixels with cp.async
 constexpr int kScratchRec = 3 * kMaxAccAsync;  // fused kernel scratch: [0, kScratchRec) re-read pixels, then 2 records
 constexpr int kScratchVec = kScratchRec + 2;   // float4 per warp of arg-max scratch (fused kernel)
 
