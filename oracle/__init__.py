@@ -59,6 +59,8 @@ def lib() -> ctypes.CDLL:
                                            ip32, ip32, ip32, ip64, dp, ctypes.c_int64]
         L.fitrig_oracle_spectrum.restype = None
         L.fitrig_oracle_spectrum.argtypes = [dp, ctypes.c_int, ctypes.c_int64, dp, ip32]
+        L.fitrig_oracle_spectrum_hsum.restype = None
+        L.fitrig_oracle_spectrum_hsum.argtypes = [dp, ctypes.c_int, ctypes.c_int64, ctypes.c_int, dp, ip32, dp]
         L.fitrig_oracle_select_spectrum.restype = ctypes.c_int64
         L.fitrig_oracle_select_spectrum.argtypes = [dp, ip32, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                                     ctypes.c_int, ctypes.c_double, ip32, ip32, ip32, ip64, dp,
@@ -236,6 +238,19 @@ def spectrum(q: np.ndarray):
     return eta, ks
 
 
+def spectrum_hsum(q: np.ndarray, harmonics: int, want_mag: bool = False):
+    """Eq. 10 with h = harmonic summing over 1, 2, 4, .., `harmonics` harmonics (reading R26):
+    (eta[Ty,Tx], kstar[Ty,Tx]) and, on request, the magnitude spectrum m[K, Ty, Tx]."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    U = q.shape[0]
+    n = int(np.prod(q.shape[1:]))
+    eta = np.zeros(q.shape[1:], np.float64)
+    ks = np.zeros(q.shape[1:], np.int32)
+    mag = np.zeros((U // 2,) + q.shape[1:], np.float64) if want_mag else None
+    lib().fitrig_oracle_spectrum_hsum(_ptr(q), U, n, int(harmonics), _ptr(eta), _ptr(ks), _ptr(mag))
+    return (eta, ks, mag) if want_mag else (eta, ks)
+
+
 def select_spectrum(z: np.ndarray, kstar: np.ndarray, H: int, W: int, tile: int, tau: float,
                     capacity: int = 1 << 22) -> Candidates:
     """Eq. 12 on the eta z-scores; record = (tile centre, k*, z), R18."""
@@ -265,7 +280,7 @@ class DetectResult:
 
 
 def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
-        tau: float = 5.0, branch: int = 0, accumulate_g: int = 1) -> DetectResult:
+        tau: float = 5.0, branch: int = 0, accumulate_g: int = 1, harmonics: int = 1) -> DetectResult:
     """Whole path on one stack: O1..O7 (branch 0) or O1..O5 + O8 (branch 1); accumulate_g > 1 first combines
     groups of g snapshots."""
     snaps = as_snapshots(stack)
@@ -275,7 +290,7 @@ def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Opti
         mu, sd, z = zscore(res.q)
         c = select(z, res.argmax, W, tau)
         return DetectResult(res, mu, sd, z, c)
-    eta, ks = spectrum(res.q)
+    eta, ks = spectrum(res.q) if harmonics <= 1 else spectrum_hsum(res.q, harmonics)
     mu, sd, z = zscore(eta[None])
     c = select_spectrum(z[0], ks, H, W, tile, tau)
     return DetectResult(res, mu, sd, z[0], c, eta, ks)

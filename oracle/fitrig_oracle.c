@@ -237,6 +237,57 @@ void fitrig_oracle_spectrum(const double* q, int U, int64_t n, double* eta, int3
   }
 }
 
+/* O8h.  Image-frequency branch, Eq. 10 with h = HARMONIC SUMMING ("a spectral refinement
+ * function, such as harmonic summing (Adamek et al., 2022)"; used for the real-data result,
+ * PAPER.md:389-393, Fig. 11).  The paper does not restate the rule; reading R26 is the standard
+ * incoherent harmonic sum of pulsar searching on the one-sided magnitude spectrum m_k = |F_k|, k = 1..K,
+ * K = floor(U/2):
+ *     s_h(k) = (1 / sqrt(h)) * sum_{i=1..h} m_{i*k}      for h = 1, 2, 4, ..., H  with  h*k <= K
+ *     eta    = max over (k, h) of s_h(k);   k* = the fundamental bin k of the first maximum
+ *              (k ascending, then h ascending; strict > keeps the first)
+ * H = 1 is exactly O8 (maximum magnitude).  mag_out (may be NULL) receives m_k as [K][n]. */
+void fitrig_oracle_spectrum_hsum(const double* q, int U, int64_t n, int H, double* eta, int32_t* kstar,
+                                 double* mag_out) {
+  const double two_pi = 6.283185307179586476925286766559;
+  const int K = U / 2;
+#pragma omp parallel for schedule(static)
+  for (int64_t t = 0; t < n; ++t) {
+    double* m = (double*)malloc(sizeof(double) * (size_t)(K + 1));
+    double mean = 0.0;
+    for (int u = 0; u < U; ++u) mean += q[(int64_t)u * n + t];
+    mean /= (double)U;
+    for (int k = 1; k <= K; ++k) {
+      double re = 0.0, im = 0.0;
+      for (int u = 0; u < U; ++u) {
+        const double a = q[(int64_t)u * n + t] - mean;
+        const double ang = -two_pi * (double)k * (double)u / (double)U;
+        re += a * cos(ang);
+        im += a * sin(ang);
+      }
+      m[k] = sqrt(re * re + im * im);
+      if (mag_out) mag_out[(int64_t)(k - 1) * n + t] = m[k];
+    }
+    double best = 0.0;
+    int32_t kb = (K >= 1) ? 1 : 0;
+    int first = 1;
+    for (int k = 1; k <= K; ++k) {
+      for (int h = 1; h <= H && h * k <= K; h *= 2) {
+        double s = 0.0;
+        for (int i = 1; i <= h; ++i) s += m[i * k];
+        s /= sqrt((double)h);
+        if (first || s > best) {
+          best = s;
+          kb = k;
+          first = 0;
+        }
+      }
+    }
+    eta[t] = best;
+    if (kstar) kstar[t] = kb;
+    free(m);
+  }
+}
+
 /* Eq. 11-12 are fitrig_oracle_zscore(eta, 1, n, ...) followed by the same
  * strict threshold; the candidate record for this branch is (tile centre, kstar, z), R18:
  *   x = tx*N_T + w_t/2, y = ty*N_T + h_t/2 (integer division; w_t, h_t the tile's extent). */

@@ -419,3 +419,51 @@ def test_accumulate_single_pixel_transient_closed_form(g):
             assert abs(r.q[u, 0, 1] - expected) <= 1e-15 and np.count_nonzero(r.q[u]) == 1
         else:
             assert not r.q[u].any()
+
+
+# ------------------------------------------------------------------------------------------
+# harmonic summing as the spectral refinement h of Eq. 10 (R26)
+# ------------------------------------------------------------------------------------------
+def test_harmonic_sum_one_harmonic_is_the_maximum_magnitude():
+    rng = np.random.default_rng(8)
+    q = rng.random((30, 5, 7))
+    e1, k1 = oracle.spectrum(q)
+    eh, kh = oracle.spectrum_hsum(q, 1)
+    assert np.array_equal(e1, eh) and np.array_equal(k1, kh)
+
+
+@pytest.mark.parametrize("U,k0,amps", [(64, 3, (2.0, 1.0, 0.0, 0.5)), (30, 2, (1.0, 1.0, 0.0, 1.0)), (48, 5, (3.0, 0.0, 0.0, 0.0))])
+def test_harmonic_sum_closed_form_comb(U, k0, amps):
+    # q_u = c + sum_j A_j cos(2 pi j k0 u / U), j = 1..4, all j*k0 below Nyquist: m_{j k0} = A_j U / 2 exactly,
+    # every other bin is 0, so s_h(k0) = (U/2) (A_1 + .. + A_h) / sqrt(h) and eta is the largest of h = 1, 2, 4
+    u = np.arange(U)
+    series = 0.7 + sum(A * np.cos(2 * np.pi * (j + 1) * k0 * u / U) for j, A in enumerate(amps))
+    q = series.reshape(U, 1, 1)
+    eta, ks, mag = oracle.spectrum_hsum(q, 4, want_mag=True)
+    for j, A in enumerate(amps):
+        assert abs(mag[(j + 1) * k0 - 1, 0, 0] - A * U / 2) <= 1e-9 * U
+    cand = [(U / 2) * sum(amps[:h]) / np.sqrt(h) for h in (1, 2, 4)]
+    assert abs(eta[0, 0] - max(cand)) <= 1e-9 * U and ks[0, 0] == k0
+    # with one harmonic only the strongest single line counts
+    e1, k1 = oracle.spectrum_hsum(q, 1)
+    jbest = int(np.argmax(amps))
+    assert abs(e1[0, 0] - amps[jbest] * U / 2) <= 1e-9 * U and k1[0, 0] == (jbest + 1) * k0
+
+
+def test_harmonic_sum_brute_force_against_numpy_rfft():
+    rng = np.random.default_rng(21)
+    U, H = 40, 8
+    q = rng.random((U, 3, 4))
+    eta, ks = oracle.spectrum_hsum(q, H)
+    m = np.abs(np.fft.rfft(q - q.mean(axis=0), axis=0))  # bins 0..U/2
+    K = U // 2
+    for idx in np.ndindex(3, 4):
+        best, kb = -1.0, 0
+        for k in range(1, K + 1):
+            h = 1
+            while h <= H and h * k <= K:
+                s = m[(slice(k, h * k + 1, k),) + idx].sum() / np.sqrt(h)
+                if s > best * (1 + 1e-12):
+                    best, kb = s, k
+                h *= 2
+        assert abs(eta[idx] - best) <= 1e-10 * best and ks[idx] == kb
