@@ -66,7 +66,10 @@ typedef struct {
   int32_t accumulate; /* g >= 1; 0 -> 1.  Snapshot accumulation (Fig. 16): the images the method  */
                       /* assesses are A_j = x_{gj} + .. + x_{gj+g-1}, j < L / g (an incomplete trailing group  */
                       /* is left out, R25); units U = L / g - 2; M is the largest accumulated pixel          */
-  int32_t reserved[7];
+  int32_t harmonics;  /* frequency branch: H = 1, 2, 4, .., 32; 0 -> 1.  The spectral refinement h of Eq. 10:          */
+                      /* H = 1 maximum magnitude; H > 1 harmonic summing (R26):      */
+                      /* eta = max over k and h in {1,2,4..H}, h*k <= U/2, of (|F_k| + |F_2k| + .. + |F_hk|)/sqrt(h) */
+  int32_t reserved[6];
 } fitrig_params;
 
 /* One candidate, 16 bytes.

@@ -842,6 +842,8 @@ struct SpectrumParams {
   const float2* tw;     // [U] twiddles (cos, -sin)(2 pi j / U)
   float* eta;           // [nt]
   int* kstar;           // [nt]
+  float* mag;           // [U/2][nt] magnitude spectrum (harmonic summing only), or NULL
+  int harmonics;        // H >= 1: h = harmonic sum over 1, 2, 4, .., H harmonics (R26); 1: maximum magnitude
   long long nt;
   int U;
   int nblk;
@@ -864,7 +866,8 @@ __global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
     mean /= (float)p.U;  // DC removed
     float best = 0.f;
     int kb = (p.U / 2 >= 1) ? 1 : 0;
-    for (int k = 1; k <= p.U / 2; ++k) {
+    const int K = p.U / 2;
+    for (int k = 1; k <= K; ++k) {
       float re = 0.f, im = 0.f;
       int j = 0;  // (k * u) mod U
       for (int u = 0; u < p.U; ++u) {
@@ -876,7 +879,22 @@ __global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
         if (j >= p.U) j -= p.U;
       }
       const float mag = sqrtf(re * re + im * im);
-      if (k == 1 || mag > best) { best = mag; kb = k; }
+      if (p.harmonics > 1) p.mag[(size_t)(k - 1) * p.nt + t] = mag;  // this thread's own column: no sync needed
+      else if (k == 1 || mag > best) { best = mag; kb = k; }
+    }
+    if (p.harmonics > 1) {
+      // harmonic summing (R26): s_h(k) = sum_{i<=h} m_{ik} / sqrt(h), h = 1, 2, 4, .., H, h*k <= K
+      bool first = true;
+      for (int k = 1; k <= K; ++k) {
+        float s = 0.f;
+        int have = 0;  // harmonics summed so far
+        for (int h = 1; h <= p.harmonics && h * k <= K; h *= 2) {
+          for (int i = have + 1; i <= h; ++i) s += p.mag[(size_t)(i * k - 1) * p.nt + t];  // m_k, m_2k, ... in order
+          have = h;
+          const float v = s * rsqrtf((float)h);
+          if (first || v > best) { best = v; kb = k; first = false; }
+        }
+      }
     }
     p.eta[t] = best;
     p.kstar[t] = kb;

@@ -43,6 +43,11 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
     return FITRIG_ERR_INVALID_ARG;
   }
   out->strip_rows = p->strip_rows;
+  out->harmonics = p->harmonics == 0 ? 1 : p->harmonics;
+  if (out->harmonics < 1 || out->harmonics > 32 || (out->harmonics & (out->harmonics - 1)) != 0) {
+    *why = "harmonics must be 1, 2, 4, 8, 16 or 32 (0 selects 1)";
+    return FITRIG_ERR_INVALID_ARG;
+  }
   if (p->row_offset < 0 || (p->row_offset % out->tile) != 0) {
     *why = "row_offset must be a non-negative multiple of tile";
     return FITRIG_ERR_INVALID_ARG;

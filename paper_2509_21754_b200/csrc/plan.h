@@ -26,6 +26,7 @@ struct NormParams {  // fitrig_params with defaults applied
   int device;
   int row_offset;
   int accumulate;  // >= 1
+  int harmonics;   // 1, 2, 4, .., 32
 };
 
 // Validates and applies defaults.  Returns FITRIG_OK or FITRIG_ERR_INVALID_ARG (+ message in *why).

@@ -360,6 +360,41 @@ def test_frequency_branch_reduced_config5(channel):
             assert tiles.get((t.y // 32, t.x // 32)) == 15
 
 
+@pytest.mark.parametrize("harmonics,U", [(2, 30), (4, 30), (8, 62), (32, 21)])
+def test_frequency_branch_harmonic_summing(harmonics, U):
+    """h = harmonic summing (R26) against oracle.spectrum_hsum; a periodic transient with a short duty
+    cycle puts power into several harmonics of its repetition rate."""
+    cfg = synth.scaled(synth.CONFIGS["imgfreq"], 512, 512, L=U + 2).replace(n_transients=2, transient_peak=9.0)
+    st, truth = synth.make_stack(cfg, device=DEV, channel=0)
+    taus = (3.0,)
+    g = gpu_run(st, taus=taus, branch=fitrig.BRANCH_FREQUENCY, harmonics=harmonics)
+    ref = oracle_run(st, tile=32, tau=3.0, branch=1, harmonics=harmonics)
+    np.testing.assert_allclose(g["eta"], ref.eta, rtol=3e-4, atol=1e-12)
+    diff = np.argwhere(g["kstar"] != ref.kstar)
+    assert len(diff) <= 0.01 * ref.kstar.size
+    eta_ref, ks_ref, mag = oracle.spectrum_hsum(ref.res.q, harmonics, want_mag=True)
+    K = U // 2
+    for (ty, tx) in diff:  # R23: another fundamental only where its harmonic sum is within rounding of the best
+        k = int(g["kstar"][ty, tx])
+        best_k = max(mag[k - 1:h * k:k, ty, tx].sum() / math.sqrt(h)
+                     for h in (1, 2, 4, 8, 16, 32) if h <= harmonics and h * k <= K)
+        assert best_k >= (1 - 3e-4) * ref.eta[ty, tx]
+    assert abs(g["mu"][0] - ref.mu[0]) <= 1e-4 * abs(ref.mu[0]) and abs(g["sigma"][0] - ref.sigma[0]) <= 3e-4 * ref.sigma[0]
+    Tx = ref.res.Tx
+    c, n = g["cands"][3.0]
+    lst = [(int(r["x"]), int(r["y"]), int(r["snapshot"]), float(r["score"]),
+            (int(r["y"]) // 32) * Tx + int(r["x"]) // 32, 0) for r in c]
+    util.compare_candidates(lst, ref.z[None], ref.mu, ref.sigma, 3.0, Tx, ref.res.Ty * Tx, rtol=5e-4)
+    assert n > 0
+
+
+def test_harmonics_argument_is_validated():
+    for bad in (3, 64, -1):
+        with pytest.raises(fitrig.FitrigError) as e:
+            fitrig.Context(64, 64, 8, branch=fitrig.BRANCH_FREQUENCY, harmonics=bad)
+        assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+
+
 def test_frequency_branch_odd_length_series():
     st = synth.gaussian_noise_stack(9, 96, 128, seed=11, device=DEV)  # U = 7
     g = gpu_run(st, taus=(1.0,), branch=fitrig.BRANCH_FREQUENCY)
