@@ -46,22 +46,26 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="fitrig", choices=["fitrig", "reference"])
-    ap.add_argument("--workload", default="meerkat", choices=["tiny", "meerkat", "ska_aa2", "stream50k", "imgfreq"])
+    ap.add_argument("--workload", default="meerkat", choices=["tiny", "meerkat", "ska_aa2", "stream50k", "imgfreq", "psr_like"])
     ap.add_argument("--tau", type=float, default=None)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--channels", type=int, default=0, help="imgfreq only: use the first N of the 16 channels")
     ap.add_argument("--tile", type=int, default=32, help="N_T (the paper's default and BASELINE.json's is 32)")
+    ap.add_argument("--harmonics", type=int, default=1, help="frequency branch: harmonic summing over 1,2,4..H harmonics")
     return ap.parse_args()
 
 
 TILE = 32  # N_T of this run (--tile)
+HARMONICS = 1  # --harmonics
 
 
 def workload_desc(cfg, tau, branch, n_ch=1):
     return (f"{cfg.name}: {f'{n_ch} channels x ' if n_ch > 1 else ''}{cfg.L} snapshots x {cfg.H}x{cfg.W} fp32 "
-            f"(BASELINE.json configs[{cfg.cfg_index - 1}]), "
+            + (f"(BASELINE.json configs[{cfg.cfg_index - 1}]), " if cfg.cfg_index <= 5 else
+               "(shape of the paper's real-data run, PAPER.md:371-395; not a BASELINE.json config), ")
+            +
             f"N_T={TILE}, tau={tau:g}, branch={'image-frequency' if branch else 'image'}")
 
 
@@ -138,7 +142,7 @@ def oracle_sample_rate(snaps, rows, tau, branch, repeats=1):
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        oracle.run(sub, tile=TILE, tau=tau, branch=branch)
+        oracle.run(sub, tile=TILE, tau=tau, branch=branch, harmonics=HARMONICS)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return best
@@ -248,7 +252,7 @@ def run_fitrig(args, cfg, tau, branch):
     stack = stacks[0]
     L, H, W = stack.shape
     pix = L * H * W * n_ch
-    ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE)
+    ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS)
     U, Ty, Tx = ctx.map_dims()
     d_tl = torch.empty((U, Ty, Tx), dtype=torch.float32, device=dev)
     cap = 1 << 16
@@ -385,7 +389,7 @@ def run_fitrig(args, cfg, tau, branch):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_desc(cfg, tau, branch, n_ch), "tile": TILE, "tau": tau,
+            "config": {"workload": workload_desc(cfg, tau, branch, n_ch), "tile": TILE, "tau": tau, "harmonics": HARMONICS,
                        "candidates_per_step": int(n_found),
                        "l2": f"input {4 * pix / 1e6:.0f} MB per step vs 126 MB L2: "
                              + ("larger than L2, no flush" if 4 * pix > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
@@ -401,13 +405,13 @@ def run_fitrig(args, cfg, tau, branch):
 
 
 def main():
-    global TILE
+    global TILE, HARMONICS
     args = parse_args()
-    TILE = args.tile
+    TILE, HARMONICS = args.tile, args.harmonics
     import synth
     cfg = synth.CONFIGS[args.workload]
     tau = args.tau if args.tau is not None else cfg.tau
-    branch = 1 if args.workload == "imgfreq" else 0
+    branch = 1 if args.workload in ("imgfreq", "psr_like") else 0
     if args.impl == "reference":
         run_reference(args, cfg, tau, branch)
     else:

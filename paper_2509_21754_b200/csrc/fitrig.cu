@@ -85,7 +85,7 @@ struct fitrig_ctx {
   // frequency branch
   float* eta;
   int* kstar;
-  float* mag;  // [U/2][nt], harmonic summing only
+  float* mag;  // [U/2][nt] magnitude spectrum
   float2* tw;
   StatPartial* sparts;
   unsigned* scounter;
@@ -254,7 +254,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   if (np.branch == FITRIG_BRANCH_FREQUENCY) {
     CTX_TRY(cudaMalloc(&c->eta, sizeof(float) * c->nt));
     CTX_TRY(cudaMalloc(&c->kstar, sizeof(int) * c->nt));
-    if (np.harmonics > 1 && c->U / 2 >= 1) CTX_TRY(cudaMalloc(&c->mag, sizeof(float) * (size_t)(c->U / 2) * c->nt));
+    CTX_TRY(cudaMalloc(&c->mag, sizeof(float) * (size_t)std::max(1, c->U / 2) * c->nt));
     CTX_TRY(cudaMalloc(&c->tw, sizeof(float2) * c->U));
     std::vector<float2> tw(c->U);
     for (int j = 0; j < c->U; ++j) {  // exp(-2 pi i j / U), Eq. 10's Fourier kernel (R17)
@@ -548,9 +548,15 @@ static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_
   if (freq && !c->eta_valid) {
     SpectrumParams sp;
     sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = c->nt; sp.U = c->U;
-    sp.mag = c->mag; sp.harmonics = c->mag ? c->prm.harmonics : 1;
+    sp.mag = c->mag; sp.harmonics = c->prm.harmonics;
     sp.nblk = c->spec_nblk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
-    spectrum_kernel<<<c->spec_nblk, 128, sizeof(float2) * c->U, st>>>(sp);
+    if (c->U / 2 >= 1) {
+      const dim3 grid((unsigned)((c->nt + 127) / 128), (unsigned)((c->U / 2 + kDftBins - 1) / kDftBins));
+      dft_mag_kernel<<<grid, 128, sizeof(float2) * c->U, st>>>(sp);
+      CUDA_TRY(cudaGetLastError());
+      c->launches++;
+    }
+    spectrum_kernel<<<c->spec_nblk, 128, 0, st>>>(sp);
     CUDA_TRY(cudaGetLastError());
     c->launches++;
     c->eta_valid = true;

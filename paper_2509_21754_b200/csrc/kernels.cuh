@@ -842,7 +842,7 @@ struct SpectrumParams {
   const float2* tw;     // [U] twiddles (cos, -sin)(2 pi j / U)
   float* eta;           // [nt]
   int* kstar;           // [nt]
-  float* mag;           // [U/2][nt] magnitude spectrum (harmonic summing only), or NULL
+  float* mag;           // [U/2][nt] magnitude spectrum
   int harmonics;        // H >= 1: h = harmonic sum over 1, 2, 4, .., H harmonics (R26); 1: maximum magnitude
   long long nt;
   int U;
@@ -853,36 +853,57 @@ struct SpectrumParams {
   double* sigma;        // [1]
 };
 
-__global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
-  __shared__ double sh[32];
+// Magnitude spectrum m_k = |F_k|, k = 1..K, of every tile's DC-free series (Eq. 10): one thread per (tile, block of
+// kDftBins bins), tiles fastest so that the loads of q coalesce and the twiddle index is warp uniform (shared-memory
+// broadcast).  Direct DFT: the series is short (U = 30 in config 5, 1498 in the paper's real-data run) and of arbitrary
+// length (R17).
+constexpr int kDftBins = 8;
+
+__global__ void __launch_bounds__(128) dft_mag_kernel(const SpectrumParams p) {
   extern __shared__ float2 tws[];  // U twiddles
   for (int i = threadIdx.x; i < p.U; i += blockDim.x) tws[i] = p.tw[i];
   __syncthreads();
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= p.nt) return;
+  const int K = p.U / 2, k0 = blockIdx.y * kDftBins + 1;
+  float mean = 0.f;
+  for (int u = 0; u < p.U; ++u) mean += p.q[(size_t)u * p.nt + t];
+  mean /= (float)p.U;  // DC removed
+  float re[kDftBins], im[kDftBins];
+  int j[kDftBins];  // (k * u) mod U
+#pragma unroll
+  for (int b = 0; b < kDftBins; ++b) { re[b] = 0.f; im[b] = 0.f; j[b] = 0; }
+  for (int u = 0; u < p.U; ++u) {
+    const float a = p.q[(size_t)u * p.nt + t] - mean;
+#pragma unroll
+    for (int b = 0; b < kDftBins; ++b) {
+      const float2 w = tws[j[b]];
+      re[b] = fmaf(a, w.x, re[b]);
+      im[b] = fmaf(a, w.y, im[b]);
+      j[b] += k0 + b;
+      if (j[b] >= p.U) j[b] -= p.U;
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < kDftBins; ++b)
+    if (k0 + b <= K) p.mag[(size_t)(k0 + b - 1) * p.nt + t] = sqrtf(re[b] * re[b] + im[b] * im[b]);
+}
+
+// eta = h(m) per tile (maximum magnitude, or harmonic summing), k*, and the statistics of eta (Eq. 11).
+__global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
+  __shared__ double sh[32];
   const long long per = (p.nt + p.nblk - 1) / p.nblk;
   const long long begin = min(p.nt, (long long)blockIdx.x * per), end = min(p.nt, begin + per);
+  const int K = p.U / 2;
   for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
-    float mean = 0.f;
-    for (int u = 0; u < p.U; ++u) mean += p.q[(size_t)u * p.nt + t];
-    mean /= (float)p.U;  // DC removed
     float best = 0.f;
-    int kb = (p.U / 2 >= 1) ? 1 : 0;
-    const int K = p.U / 2;
-    for (int k = 1; k <= K; ++k) {
-      float re = 0.f, im = 0.f;
-      int j = 0;  // (k * u) mod U
-      for (int u = 0; u < p.U; ++u) {
-        const float a = p.q[(size_t)u * p.nt + t] - mean;
-        const float2 w = tws[j];
-        re = fmaf(a, w.x, re);
-        im = fmaf(a, w.y, im);
-        j += k;
-        if (j >= p.U) j -= p.U;
+    int kb = (K >= 1) ? 1 : 0;
+    if (p.harmonics <= 1) {  // h = maximum spectral magnitude, first bin on ties
+      for (int k = 1; k <= K; ++k) {
+        const float mag = p.mag[(size_t)(k - 1) * p.nt + t];
+        if (k == 1 || mag > best) { best = mag; kb = k; }
       }
-      const float mag = sqrtf(re * re + im * im);
-      if (p.harmonics > 1) p.mag[(size_t)(k - 1) * p.nt + t] = mag;  // this thread's own column: no sync needed
-      else if (k == 1 || mag > best) { best = mag; kb = k; }
-    }
-    if (p.harmonics > 1) {
+    } else {
       // harmonic summing (R26): s_h(k) = sum_{i<=h} m_{ik} / sqrt(h), h = 1, 2, 4, .., H, h*k <= K
       bool first = true;
       for (int k = 1; k <= K; ++k) {

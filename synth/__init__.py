@@ -62,6 +62,7 @@ class StackConfig:
     tau: float = 5.0
     n_channels: int = 1
     border: int = 16
+    period: int = 8  # periodic transients: on when s % period == 3 % period
 
     def replace(self, **kw) -> "StackConfig":
         return dataclasses.replace(self, **kw)
@@ -91,6 +92,11 @@ CONFIGS: Dict[str, StackConfig] = {
     "imgfreq": StackConfig("imgfreq", 5, L=32, H=4096, W=4096, n_sources=1000, flux_lo=5.0, flux_hi=500.0,
                            fwhm=2.0, n_transients=5, transient_mode="periodic", transient_peak=5.0,
                            tau=6.0, n_channels=16),
+    # NOT a BASELINE.json config: the shape of the paper's real-data run (1500 snapshots of 2 s,
+    # 4096 x 4096, a 76 s pulsar = one pulse every 38 snapshots), used for a context line in DESIGN.md
+    "psr_like": StackConfig("psr_like", 6, L=1500, H=4096, W=4096, n_sources=1000, flux_lo=5.0, flux_hi=500.0,
+                            fwhm=2.0, n_transients=1, transient_mode="periodic", transient_peak=4.0,
+                            tau=6.0, period=38),
 }
 
 
@@ -186,7 +192,7 @@ def draw_truth(cfg: StackConfig, channel: int = 0) -> Truth:
     elif cfg.transient_mode == "periodic":
         tx = _randint(gen, m, b, max(b + 1, cfg.W - b))
         ty = _randint(gen, m, b, max(b + 1, cfg.H - b))
-        act = tuple(s for s in range(cfg.L) if s % 8 == 3)
+        act = tuple(s for s in range(cfg.L) if s % cfg.period == 3 % cfg.period)
         for j in range(m):
             tr.append(Transient(int(tx[j]), int(ty[j]), cfg.transient_peak, act))
     elif cfg.transient_mode == "near_bright":
