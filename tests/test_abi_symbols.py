@@ -79,3 +79,35 @@ def test_no_cpu_fallback_without_a_device():
     with pytest.raises(fitrig.FitrigError) as e:
         fitrig.Context(64, 64, 4)
     assert e.value.code == binding.ERR_CUDA  # fails loudly; nothing routes to the oracle
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """include/fitrig.h must compile as C99 (no C++, no torch types) and the host-only entry points must be
+    callable from a C program linked against the in-tree library."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = tmp_path / "abi.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include <string.h>
+#include "fitrig.h"
+int main(void) {
+  fitrig_params p;
+  fitrig_plan plan;
+  memset(&p, 0, sizeof p);
+  if (sizeof(fitrig_candidate) != 16 || sizeof(fitrig_params) != 64) return 2;
+  if (fitrig_plan_query(50000, 50000, 4, &p, 148, &plan) != FITRIG_OK) return 3;
+  if (plan.Ty != 1563 || plan.Tx != 1563 || plan.units != 2) return 4;
+  p.tile = -1;
+  if (fitrig_plan_query(64, 64, 8, &p, 0, &plan) != FITRIG_ERR_INVALID_ARG) return 5;
+  printf("%s\n", fitrig_version());
+  return 0;
+}
+''')
+    exe = tmp_path / "abi"
+    lib_dir = os.path.dirname(fitrig.lib_path())
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(root, "include"), str(src),
+                    "-o", str(exe), "-L", lib_dir, "-lfitrig", "-Wl,-rpath," + lib_dir], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    assert out.startswith("fitrig-b200")
