@@ -37,7 +37,7 @@ UNIT = "Mpix/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE fused-kernel launch on the default workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture has been taken for this build)
-NCU_TRAFFIC_BYTES = {"meerkat": 1090486256}  # profiles/r01_c_fused_sharedbox.md: 1 083 254 000 read + 7 232 256 written
+NCU_TRAFFIC_BYTES = {"meerkat": 1091050016}  # profiles/r01_e_final.md: 1 083 252 000 read + 7 798 016 written
 
 
 def parse_args():
