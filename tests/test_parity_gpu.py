@@ -212,6 +212,54 @@ def test_fused_and_generic_kernels_agree(tiny, monkeypatch, tile):
 
 
 # ------------------------------------------------------------------------------------------
+# seeded random sweep over shapes, tile sizes, modes and entry points (every kernel variant, ragged edges)
+# ------------------------------------------------------------------------------------------
+def _random_cases(n, seed=20250921):
+    rng = np.random.default_rng(seed)
+    cases = []
+    for i in range(n):
+        tile = int(rng.choice([32, 32, 16, 8, 64, 96, 5, 4, 12]))
+        H = int(rng.integers(max(3, tile // 2), 200))
+        W = int(rng.integers(3, 60)) * 4 if rng.random() < 0.8 else int(rng.integers(9, 230))
+        g = int(rng.choice([1, 1, 1, 2, 3]))
+        L = int(rng.integers(3, 8)) * g + int(rng.integers(0, g))
+        cases.append((i, H, W, L, tile, g, int(rng.integers(0, 3)), bool(rng.random() < 0.35), int(rng.integers(0, 2))))
+    return cases
+
+
+@pytest.mark.parametrize("i,H,W,L,tile,g,ref_mode,use_stream,branch", _random_cases(28))
+def test_random_shapes_and_modes(i, H, W, L, tile, g, ref_mode, use_stream, branch):
+    st = synth.gaussian_noise_stack(L, H, W, seed=1000 + i, device=DEV)
+    st[:, H // 2, W // 2] += 25.0 * (torch.arange(L, device=DEV) % 3 == 1)  # something to detect
+    if ref_mode == 2:
+        st = st + 3.0  # FLOOR: keep the reference mostly above C so that r is not saturated everywhere
+    st[0, 0, 0] = 0.0  # an exact zero (reference pixel of no unit) and one that is a reference pixel
+    if L // g >= 3:
+        st[g:2 * g, min(1, H - 1), min(2, W - 1)] = 0.0
+    n_tiles = (-(-H // tile)) * (-(-W // tile))
+    tau = 2.0 if n_tiles > 8 else 0.3
+    kw = dict(tile=tile, accumulate=g, ref_mode=ref_mode, branch=branch)
+    if use_stream:
+        q = tile if tile % 32 == 0 else (32 if 32 % tile == 0 else tile)
+        kw["strip_rows"] = q * int(1 + i % 2)
+    gp = gpu_run(st, taus=(tau,), use_stream=use_stream, **kw)
+    ref = oracle_run(st, tile=tile, tau=tau, ref_mode=ref_mode, branch=branch, accumulate_g=g)
+    imgs = np.stack(oracle.accumulate(st.cpu().numpy(), g))
+    extra = util.accumulation_slack(st.cpu().numpy(), g) if g > 1 else (np.zeros_like(imgs[:-2]) if tile < 8 else None)
+    if ref_mode == 1:  # LITERAL: r is signed and unbounded below, sums cancel: compare what stays well conditioned
+        sd, md, sr, ax, ay = gp["raw"]
+        np.testing.assert_allclose(sd, ref.res.sumD, rtol=1e-4, atol=1e-6)
+        np.testing.assert_allclose(md, ref.res.maxD, rtol=1e-5, atol=1e-7)
+        scale = np.abs(sr).max() + 1.0
+        assert np.all(np.abs(sr - ref.res.sumR) <= 1e-4 * scale + 1e-3 * np.abs(ref.res.sumR))
+        return
+    check_against_oracle(None, gp, ref, (tau,) if branch == 0 else (), tile, branch=branch, ref_mode=ref_mode,
+                         small_tiles=(tile < 8), stack_np=imgs, extra_slack=extra)
+    if branch == 1 and ref.res.U >= 2:
+        np.testing.assert_allclose(gp["eta"], ref.eta, rtol=5e-4, atol=1e-9 * float(np.abs(ref.eta).max() + 1e-30))
+
+
+# ------------------------------------------------------------------------------------------
 # degenerate and edge cases
 # ------------------------------------------------------------------------------------------
 def test_identical_snapshots_no_transient_value_and_no_candidates():
