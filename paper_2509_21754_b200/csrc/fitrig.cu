@@ -163,7 +163,13 @@ static cudaError_t set_fused_attr() {
   if ((e = set_fused_attr_one<REF, false, 16>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, true, 16>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, false, 8>()) != cudaSuccess) return e;
-  return set_fused_attr_one<REF, true, 8>();
+  if ((e = set_fused_attr_one<REF, true, 8>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, false, 4>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, true, 4>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, false, 2>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, true, 2>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr_one<REF, false, 1>()) != cudaSuccess) return e;
+  return set_fused_attr_one<REF, true, 1>();
 }
 
 template <int REF, int T>
@@ -178,6 +184,9 @@ static void launch_fused(bool acc, int tile, dim3 grid, dim3 block, size_t smem,
                          const FusedParams& fp) {
   if (tile == 16) launch_fused_t<REF, 16>(acc, grid, block, smem, st, tm, fp);
   else if (tile == 8) launch_fused_t<REF, 8>(acc, grid, block, smem, st, tm, fp);
+  else if (tile == 4) launch_fused_t<REF, 4>(acc, grid, block, smem, st, tm, fp);
+  else if (tile == 2) launch_fused_t<REF, 2>(acc, grid, block, smem, st, tm, fp);
+  else if (tile == 1) launch_fused_t<REF, 1>(acc, grid, block, smem, st, tm, fp);
   else launch_fused_t<REF, 32>(acc, grid, block, smem, st, tm, fp);
 }
 

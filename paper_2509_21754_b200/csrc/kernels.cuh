@@ -288,7 +288,10 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 template <int REF_MODE, bool ACC, int T>
 __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
-  using Geo = LaneGeom<T>;
+  // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
+  // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
+  constexpr bool kSmall = T < 8;
+  using Geo = LaneGeom<(kSmall ? 32 : T)>;
   constexpr int LPT = Geo::LPT, NGRP = 32 / LPT;  // lanes per tile, tiles (lane groups) per warp
   const int acc = ACC ? p.acc : 1;  // ACC = false compiles the accumulation loops away
   extern __shared__ __align__(1024) unsigned char smem[];
@@ -358,13 +361,13 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
     mbar_wait(full_addr + slot * 8, phase);
-    load_tile<T>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+    load_tile<(kSmall ? 32 : T)>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
     __syncwarp();  // every lane has its copy
     if (lane == 0) mbar_arrive(empty_addr + slot * 8);
     if (++slot == p.nstage) { slot = 0; phase ^= 1; }
     for (int i = 1; i < acc; ++i) {  // accumulation: the image is the sum of acc raw snapshots, added in order
       mbar_wait(full_addr + slot * 8, phase);
-      add_tile<T>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+      add_tile<(kSmall ? 32 : T)>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty_addr + slot * 8);
       if (++slot == p.nstage) { slot = 0; phase ^= 1; }
@@ -472,6 +475,73 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     rp += raw_step;
   };
 
+  // ---- tiles of 4, 2 or 1 pixels: N = x^(s+2), X = x^(s+1) (reference image), dp = signed x^(s+1) - x^(s).  Every
+  // 16-byte quad of a lane (row rb + 4j, columns 4cg .. 4cg+3) is one tile row (T = 4), two tiles' rows (T = 2) or
+  // four tiles (T = 1); lanes that hold the other rows of the same tiles differ in rb only (xor 8, 16), so a tile is
+  // reduced by at most two shuffle levels and its first max-Delta pixel (R20) is exact without a re-read.
+  int ty0 = 0, tx0 = 0;  // first tile of the warp's block, in tiles
+  auto small_step = [&](const float (&N)[32], const float (&X)[32], float (&dq)[32]) {
+    const int rb = lane >> 3, cg = lane & 7;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      float dl[4], rr[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int k = 4 * j + e;
+        const float d = N[k] - X[k];                          // signed D^(s+1), Eq. 3
+        dl[e] = fabsf(fabsf(d) - fabsf(dq[k]));               // |D^(s) - D^(s+1)|
+        dq[k] = d;
+        rr[e] = clamped_ratio<REF_MODE>(dl[e], X[k], p.C);    // Eq. 4-5, per pixel (R8 exact)
+      }
+      const int row = rb + 4 * j;  // row inside the block
+      if (T == 4) {
+        float S = ((dl[0] + dl[1]) + dl[2]) + dl[3], R = ((rr[0] + rr[1]) + rr[2]) + rr[3];
+        float Mx = fmaxf(fmaxf(dl[0], dl[1]), fmaxf(dl[2], dl[3]));
+        int pos = rb * 4 + ((dl[0] == Mx) ? 0 : (dl[1] == Mx) ? 1 : (dl[2] == Mx) ? 2 : 3);  // row-major in the tile
+#pragma unroll
+        for (int off = 8; off <= 16; off <<= 1) {
+          S += __shfl_xor_sync(0xffffffffu, S, off);
+          R += __shfl_xor_sync(0xffffffffu, R, off);
+          const float om = __shfl_xor_sync(0xffffffffu, Mx, off);
+          const int op = __shfl_xor_sync(0xffffffffu, pos, off);
+          if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
+        }
+        const int ty_r = j, tx_r = cg;
+        if (rb == 0 && ty0 + ty_r < p.Ty && tx0 + tx_r < p.Tx) {
+          RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
+          rp[(long long)ty_r * p.Tx + tx_r] = o;
+        }
+      } else if (T == 2) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          float S = dl[2 * h] + dl[2 * h + 1], R = rr[2 * h] + rr[2 * h + 1];
+          float Mx = fmaxf(dl[2 * h], dl[2 * h + 1]);
+          int pos = (rb & 1) * 2 + ((dl[2 * h] == Mx) ? 0 : 1);
+          S += __shfl_xor_sync(0xffffffffu, S, 8);
+          R += __shfl_xor_sync(0xffffffffu, R, 8);
+          const float om = __shfl_xor_sync(0xffffffffu, Mx, 8);
+          const int op = __shfl_xor_sync(0xffffffffu, pos, 8);
+          if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
+          const int ty_r = row >> 1, tx_r = 2 * cg + h;
+          if ((rb & 1) == 0 && ty0 + ty_r < p.Ty && tx0 + tx_r < p.Tx) {
+            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
+            rp[(long long)ty_r * p.Tx + tx_r] = o;
+          }
+        }
+      } else {  // T == 1: per-pixel detection
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int tx_r = 4 * cg + e;
+          if (ty0 + row < p.Ty && tx0 + tx_r < p.Tx) {
+            RawTile o; o.sumD = dl[e]; o.maxD = dl[e]; o.sumR = rr[e]; o.pos = 0;
+            rp[(long long)row * p.Tx + tx_r] = o;
+          }
+        }
+      }
+    }
+    rp += raw_step;
+  };
+
   for (int g = g_begin; g < g_end;) {
     const Segment c = decode_segment(p, g, g_end);
     g += c.nsteps - 2;
@@ -495,17 +565,32 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
 #pragma unroll
     for (int k = 0; k < 32; ++k) dp[k] = B[k] - A[k];
     int step = 2;
-    while (true) {
-      float S, R, Mx;
-      int jmax;
-      acquire(A, zA);
-      tile_step<REF_MODE>(A, B, dp, p.C, __any_sync(0xffffffffu, zB == 0.f), S, R, Mx, jmax);
-      finish(S, R, Mx, jmax);
-      if (++step >= c.nsteps) break;
-      acquire(B, zB);
-      tile_step<REF_MODE>(B, A, dp, p.C, __any_sync(0xffffffffu, zA == 0.f), S, R, Mx, jmax);
-      finish(S, R, Mx, jmax);
-      if (++step >= c.nsteps) break;
+    if constexpr (kSmall) {
+      constexpr int NS = kFastTile / T;  // tiles per block edge
+      ty0 = p.ty_base + c.ty_local * NS;
+      tx0 = tx * NS;
+      rp = p.raw + ((long long)c.u0 * p.Ty + ty0) * p.Tx + tx0;  // record of the block's first tile
+      while (true) {
+        acquire(A, zA);
+        small_step(A, B, dp);
+        if (++step >= c.nsteps) break;
+        acquire(B, zB);
+        small_step(B, A, dp);
+        if (++step >= c.nsteps) break;
+      }
+    } else {
+      while (true) {
+        float S, R, Mx;
+        int jmax;
+        acquire(A, zA);
+        tile_step<REF_MODE>(A, B, dp, p.C, __any_sync(0xffffffffu, zB == 0.f), S, R, Mx, jmax);
+        finish(S, R, Mx, jmax);
+        if (++step >= c.nsteps) break;
+        acquire(B, zB);
+        tile_step<REF_MODE>(B, A, dp, p.C, __any_sync(0xffffffffu, zA == 0.f), S, R, Mx, jmax);
+        finish(S, R, Mx, jmax);
+        if (++step >= c.nsteps) break;
+      }
     }
   }
   if (leader && pend) resolve_pending();

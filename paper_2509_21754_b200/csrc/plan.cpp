@@ -61,7 +61,9 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8 adjacent blocks is
 // 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes of 32 KB in flight per
 // SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
-bool fused_tile(int tile) { return tile == 16 || tile == 8 || (tile >= kFastTile && tile % kFastTile == 0); }
+bool fused_tile(int tile) {
+  return tile == 16 || tile == 8 || tile == 4 || tile == 2 || tile == 1 || (tile >= kFastTile && tile % kFastTile == 0);
+}
 
 void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
@@ -87,8 +89,8 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* pla
   const long long G = pairs(ntw);
   int grid = (int)std::max<long long>(1, std::min<long long>(num_sms, (G + kMinUnitsPerCta - 1) / kMinUnitsPerCta));
   if (fg > 0) grid = fg;
-  const int per_edge = tile < kFastTile ? kFastTile / tile : 1;
-  const int groups = per_edge * per_edge;  // tiles per warp, each with its own arg-max scratch
+  const int per_edge = (tile < kFastTile && tile >= 8) ? kFastTile / tile : 1;
+  const int groups = per_edge * per_edge;  // tiles per warp that keep an arg-max scratch (tiles below 8 pixels need none)
   const int scratch = ntw * groups * kScratchVec * 16;
   const int fit = (kMaxSmemPerCta - 2048 - scratch) / (ntw * kTileBytes);
   int stages = std::min(6, fit);

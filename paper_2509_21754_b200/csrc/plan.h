@@ -35,7 +35,7 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
 // `rows`: image rows covered by the launch (the whole image, or one strip).
 void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan);
-bool fused_tile(int tile);  // N_T the fused kernel serves: 8, 16 (sub-tiles of a block), 32, and 32 * m (merged blocks)
+bool fused_tile(int tile);  // N_T the fused kernel serves: 1, 2, 4, 8, 16 (tiles inside a block), 32, and 32 * m (merged blocks)
 
 // Debug/tuning overrides: FITRIG_BOX_TILES, FITRIG_STAGES, FITRIG_GRID, FITRIG_EVICT_FIRST, FITRIG_FORCE_GENERIC (integers).
 int env_int(const char* name, int dflt);
