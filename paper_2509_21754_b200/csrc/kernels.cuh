@@ -1037,10 +1037,23 @@ struct CompactParams {
   long long seg;        // entries per block (multiple of blockDim.x)
 };
 
-__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float* z_out) {
+// z of entry i (Eq. 8 on q, R21; sigma == 0 -> z = 0, R4) and the strict threshold (R6).  1 / sigma of the current
+// row is kept by the thread (its entries stay in one row for long stretches): one fp64 multiply per entry instead
+// of a double-precision division, which dominated per-pixel maps.
+struct RowCache {
+  int row = -1;
+  double mu = 0.0, inv_sigma = 0.0;
+};
+
+__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float* z_out, RowCache& rc) {
   const int row = (int)(i / p.nt);
-  const double sd = p.sigma[row];
-  const double z = (sd > 0.0) ? ((double)p.v[i] - p.mu[row]) / sd : 0.0;  // Eq. 8 on q (R21); R4
+  if (row != rc.row) {
+    const double sd = p.sigma[row];
+    rc.row = row;
+    rc.mu = p.mu[row];
+    rc.inv_sigma = (sd > 0.0) ? 1.0 / sd : 0.0;
+  }
+  const double z = ((double)p.v[i] - rc.mu) * rc.inv_sigma;
   *z_out = (float)z;
   return (float)z > p.tau;  // strict, R6
 }
@@ -1052,11 +1065,13 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   const long long N = (long long)p.rows * p.nt;
   const long long begin = min(N, (long long)blockIdx.x * p.seg), end = min(N, begin + p.seg);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+
+  RowCache rcache;
   // ---- pass 1: count ----
   unsigned cnt = 0;
   for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) {
     float z;
-    cnt += compact_flag(p, i, &z) ? 1u : 0u;
+    cnt += compact_flag(p, i, &z, rcache) ? 1u : 0u;
   }
   cnt = __reduce_add_sync(0xffffffffu, cnt);
   if (lane == 0) warp_cnt[warp] = cnt;
@@ -1084,7 +1099,7 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   for (long long c0 = begin; c0 < end; c0 += blockDim.x) {
     const long long i = c0 + threadIdx.x;
     float z = 0.f;
-    const bool f = (i < end) && compact_flag(p, i, &z);
+    const bool f = (i < end) && compact_flag(p, i, &z, rcache);
     const unsigned bal = __ballot_sync(0xffffffffu, f);
     if (lane == 0) warp_cnt[warp] = __popc(bal);
     __syncthreads();
