@@ -34,11 +34,24 @@ def nvcc() -> str:
     return "nvcc"
 
 
+STAMP = LIB + ".srchash"  # hash of the sources the library was built from (file times do not survive a copy)
+
+
+def source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for d in DEPS:
+        with open(d, "rb") as f:
+            h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS).encode())
+    return h.hexdigest()
+
+
 def stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(d) > t for d in DEPS)
+    with open(STAMP) as f:
+        return f.read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -47,6 +60,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
         subprocess.run(cmd, check=True)
         os.replace(tmp, LIB)
+        with open(STAMP, "w") as f:
+            f.write(source_hash() + "\n")
     return LIB
 
 
