@@ -827,7 +827,8 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
   const double inv_m2 = 1.0 / ((double)M * (double)M);
   const size_t base = (size_t)u * nt;
   for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
-    const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
+    const unsigned tu = (unsigned)t;  // tiles per unit < 2^31
+    const int ty = (int)(tu / (unsigned)p.Tx), tx = (int)(tu - (unsigned)ty * (unsigned)p.Tx);
     const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
     const double n_t = (double)h * (double)w;  // R5: partial tiles use their own pixel count
     const RawTile r = p.raw[base + t];
@@ -1042,15 +1043,21 @@ struct CompactParams {
 // of a double-precision division, which dominated per-pixel maps.
 struct RowCache {
   int row = -1;
+  long long row_end = 0;  // first entry index of the next row
   double mu = 0.0, inv_sigma = 0.0;
 };
 
 __device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float* z_out, RowCache& rc) {
-  const int row = (int)(i / p.nt);
-  if (row != rc.row) {
-    const double sd = p.sigma[row];
-    rc.row = row;
-    rc.mu = p.mu[row];
+  if (rc.row < 0 || i >= rc.row_end || i < rc.row_end - p.nt) {  // entries mostly move forward: rarely a division
+    if (rc.row < 0 || i >= rc.row_end + p.nt || i < rc.row_end - p.nt) {
+      rc.row = (int)(i / p.nt);
+      rc.row_end = (long long)(rc.row + 1) * p.nt;
+    } else {
+      rc.row += 1;
+      rc.row_end += p.nt;
+    }
+    const double sd = p.sigma[rc.row];
+    rc.mu = p.mu[rc.row];
     rc.inv_sigma = (sd > 0.0) ? 1.0 / sd : 0.0;
   }
   const double z = ((double)p.v[i] - rc.mu) * rc.inv_sigma;
@@ -1112,9 +1119,9 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
     if (f) {
       const unsigned long long dst = running + before + __popc(bal & ((1u << lane) - 1u));
       if ((long long)dst < p.cap) {
-        const int row = (int)(i / p.nt);
-        const long long t = i - (long long)row * p.nt;
-        const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
+        const int row = rcache.row;  // compact_flag has just placed entry i in its row
+        const unsigned t = (unsigned)(i - (rcache.row_end - p.nt));  // tile index inside the unit (< 2^31)
+        const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
         fitrig_candidate cd;
         if (p.branch == FITRIG_BRANCH_IMAGE) {
           const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
