@@ -50,6 +50,12 @@ def lib() -> ctypes.CDLL:
         L.fitrig_oracle_tlisi.argtypes = [c_f32pp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_double, ctypes.c_int, ctypes.c_double,
                                           dp, dp, dp, ip64, dp, dp]
+        L.fitrig_oracle_tlisi_windows.restype = ctypes.c_int
+        L.fitrig_oracle_tlisi_windows.argtypes = [c_f32pp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                  ctypes.c_int, ctypes.c_double, ctypes.c_int, ctypes.c_double,
+                                                  dp, dp, dp, ip64, dp, dp]
+        L.fitrig_oracle_n_windows.restype = ctypes.c_int
+        L.fitrig_oracle_n_windows.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int]
         L.fitrig_oracle_tlisi_f64.restype = ctypes.c_int
         L.fitrig_oracle_tlisi_f64.argtypes = L.fitrig_oracle_tlisi.argtypes
         L.fitrig_oracle_zscore.restype = None
@@ -138,6 +144,30 @@ def accumulate(stack, g: int) -> List[np.ndarray]:
             a += snaps[g * j + i].astype(np.float64)
         out.append(a)
     return out
+
+
+def tlisi_windows(stack, tile: int, stride: int, C: float = 1e-6, ref_mode: int = REF_ABS,
+                  M: Optional[float] = None) -> TlisiResult:
+    """Eq. 2-6 on overlapping windows of `tile` pixels every `stride` pixels (reading R27, an extension)."""
+    snaps = as_snapshots(stack)
+    L = len(snaps)
+    H, W = snaps[0].shape
+    arr, keep = _snap_ptrs(snaps, H, W)
+    if M is None:
+        M = float(lib().fitrig_oracle_global_max(arr, L, H, W, float(C)))
+    if L < 3 or stride < 1 or tile % stride:
+        raise ValueError("need L >= 3 and a stride that divides the tile")
+    U = L - 2
+    Ty, Tx = lib().fitrig_oracle_n_windows(H, tile, stride), lib().fitrig_oracle_n_windows(W, tile, stride)
+    shp = (U, Ty, Tx)
+    out = [np.zeros(shp, dtype=np.float64) for _ in range(5)]
+    arg = np.zeros(shp, dtype=np.int64)
+    rc = lib().fitrig_oracle_tlisi_windows(arr, L, H, W, int(tile), int(stride), float(C), int(ref_mode), float(M),
+                                           _ptr(out[0]), _ptr(out[1]), _ptr(out[2]), _ptr(arg), _ptr(out[3]),
+                                           _ptr(out[4]))
+    if rc != 0:
+        raise ValueError("fitrig_oracle_tlisi_windows: bad arguments")
+    return TlisiResult(M, U, Ty, Tx, out[0], out[1], out[2], arg, out[3], out[4])
 
 
 def tlisi(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
@@ -280,12 +310,18 @@ class DetectResult:
 
 
 def run(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS, M: Optional[float] = None,
-        tau: float = 5.0, branch: int = 0, accumulate_g: int = 1, harmonics: int = 1) -> DetectResult:
+        tau: float = 5.0, branch: int = 0, accumulate_g: int = 1, harmonics: int = 1,
+        stride: int = 0) -> DetectResult:
     """Whole path on one stack: O1..O7 (branch 0) or O1..O5 + O8 (branch 1); accumulate_g > 1 first combines
     groups of g snapshots."""
     snaps = as_snapshots(stack)
     H, W = snaps[0].shape
-    res = tlisi(snaps, tile, C, ref_mode, M, accumulate_g)
+    if stride and stride != tile:
+        if branch != 0 or accumulate_g != 1:
+            raise ValueError("overlapping windows: image branch, no accumulation")
+        res = tlisi_windows(snaps, tile, stride, C, ref_mode, M)
+    else:
+        res = tlisi(snaps, tile, C, ref_mode, M, accumulate_g)
     if branch == 0:
         mu, sd, z = zscore(res.q)
         c = select(z, res.argmax, W, tau)

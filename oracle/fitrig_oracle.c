@@ -92,19 +92,28 @@ static double px(const void* const* img, int is_f64, int k, int64_t p) {
   return is_f64 ? ((const double*)img[k])[p] : (double)((const float*)img[k])[p];
 }
 
-static int tlisi_core(const void* const* snaps, int is_f64, int L, int H, int W, int tile, double C, int ref_mode,
-                      double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
+/* Number of windows of `tile` pixels placed every `stride` pixels along an axis of n pixels (stride divides tile).
+ * stride == tile: the paper's non-overlapping tiles, ceil(n / tile) with a partial last tile (R5).  stride < tile
+ * (overlapping windows, reading R27): the image is cut into cells of `stride` pixels, C = ceil(n / stride) of them,
+ * and a window is tile / stride consecutive cells: C - tile/stride + 1 windows, at least one. */
+static int n_windows(int n, int tile, int stride) {
+  const int cells = (n + stride - 1) / stride, m = tile / stride;
+  return (cells - m + 1 > 1) ? cells - m + 1 : 1;
+}
+
+static int tlisi_core(const void* const* snaps, int is_f64, int L, int H, int W, int tile, int stride, double C,
+                      int ref_mode, double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
                       double* tlisi) {
-  if (L < 3 || H < 1 || W < 1 || tile < 1 || !snaps) return -1;
+  if (L < 3 || H < 1 || W < 1 || tile < 1 || stride < 1 || tile % stride != 0 || !snaps) return -1;
   const int U = L - 2;
-  const int Ty = (H + tile - 1) / tile, Tx = (W + tile - 1) / tile;
+  const int Ty = n_windows(H, tile, stride), Tx = n_windows(W, tile, stride);
 #pragma omp parallel for collapse(2) schedule(dynamic, 1)
   for (int u = 0; u < U; ++u) {
     for (int ty = 0; ty < Ty; ++ty) {
       /* images u, u+1, u+2 are x^(s), x^(s+1) (the reference image) and x^(s+2) */
       for (int tx = 0; tx < Tx; ++tx) {
-        const int r0 = ty * tile, r1 = (r0 + tile < H) ? r0 + tile : H;
-        const int c0 = tx * tile, c1 = (c0 + tile < W) ? c0 + tile : W;
+        const int r0 = ty * stride, r1 = (r0 + tile < H) ? r0 + tile : H;
+        const int c0 = tx * stride, c1 = (c0 + tile < W) ? c0 + tile : W;
         double s_delta = 0.0, m_delta = 0.0, s_r = 0.0;
         int64_t arg = (int64_t)r0 * W + c0;
         int first = 1;
@@ -147,7 +156,7 @@ static int tlisi_core(const void* const* snaps, int is_f64, int L, int H, int W,
 int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile, double C, int ref_mode,
                         double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
                         double* tlisi) {
-  return tlisi_core((const void* const*)snaps, 0, L, H, W, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
+  return tlisi_core((const void* const*)snaps, 0, L, H, W, tile, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
 }
 
 /* The same O2..O5 on fp64 images: used for ACCUMULATED snapshots (section 3.3.2, Fig. 16:
@@ -155,8 +164,21 @@ int fitrig_oracle_tlisi(const float* const* snaps, int L, int H, int W, int tile
 int fitrig_oracle_tlisi_f64(const double* const* imgs, int L, int H, int W, int tile, double C, int ref_mode,
                             double M, double* sumD, double* maxD, double* sumR, int64_t* argmax, double* q,
                             double* tlisi) {
-  return tlisi_core((const void* const*)imgs, 1, L, H, W, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
+  return tlisi_core((const void* const*)imgs, 1, L, H, W, tile, tile, C, ref_mode, M, sumD, maxD, sumR, argmax, q, tlisi);
 }
+
+/* Overlapping windows (an EXTENSION: the paper's tiles never overlap).  Reading
+ * R27: the same Eq. 2-6 on windows of tile x tile pixels placed every `stride` pixels (stride divides tile) in both
+ * directions; window (ty, tx) covers rows [ty*stride, min(H, ty*stride + tile)), columns likewise; outputs are
+ * [U][Ty][Tx] with Ty, Tx = n_windows().  stride == tile is fitrig_oracle_tlisi.  fp32 snapshots only. */
+int fitrig_oracle_tlisi_windows(const float* const* snaps, int L, int H, int W, int tile, int stride, double C,
+                                int ref_mode, double M, double* sumD, double* maxD, double* sumR, int64_t* argmax,
+                                double* q, double* tlisi) {
+  return tlisi_core((const void* const*)snaps, 0, L, H, W, tile, stride, C, ref_mode, M, sumD, maxD, sumR, argmax, q,
+                    tlisi);
+}
+
+int fitrig_oracle_n_windows(int n, int tile, int stride) { return n_windows(n, tile, stride); }
 
 /* O6.  z-score of the tile matrix of each unit, Eq. 8:
  *   z_t = ((1 - tLISI_t) - (1 - mu)) / sigma = (q_t - mean(q)) / std(q)

@@ -467,3 +467,38 @@ def test_harmonic_sum_brute_force_against_numpy_rfft():
                     best, kb = s, k
                 h *= 2
         assert abs(eta[idx] - best) <= 1e-10 * best and ks[idx] == kb
+
+
+# ------------------------------------------------------------------------------------------
+# overlapping windows (an extension; R27)
+# ------------------------------------------------------------------------------------------
+def test_windows_with_full_stride_are_the_tiles_and_aligned_windows_are_tile_values():
+    st = _noise_stack(6, 80, 112)
+    a, b = oracle.tlisi(st, tile=16), oracle.tlisi_windows(st, 16, 16)
+    assert np.array_equal(a.q, b.q) and np.array_equal(a.argmax, b.argmax)
+    w = oracle.tlisi_windows(st, 16, 4, M=a.M)
+    assert w.q.shape == (4, 80 // 4 - 3, 112 // 4 - 3)
+    # the windows that start on a tile boundary ARE the tiles
+    assert np.array_equal(w.q[:, ::4, ::4], a.q) and np.array_equal(w.argmax[:, ::4, ::4], a.argmax)
+
+
+@pytest.mark.parametrize("H,W,tile,stride", [(37, 50, 8, 4), (33, 20, 16, 8), (10, 70, 16, 4), (64, 64, 32, 16)])
+def test_windows_brute_force(H, W, tile, stride):
+    st = _noise_stack(5, H, W)
+    r = oracle.tlisi_windows(st, tile, stride)
+    x = st.astype(np.float64)
+    M = max(x.max(), 1e-6)
+    cy, cx = -(-H // stride), -(-W // stride)
+    Ty, Tx = max(1, cy - tile // stride + 1), max(1, cx - tile // stride + 1)
+    assert r.q.shape == (3, Ty, Tx)
+    for u in range(3):
+        delta = np.abs(np.abs(x[u + 1] - x[u]) - np.abs(x[u + 2] - x[u + 1]))
+        ref = np.abs(x[u + 1])
+        rr = np.minimum(delta / np.where(ref == 0, 1e-6, ref), 1.0)
+        for ty in range(Ty):
+            for tx in range(Tx):
+                d = delta[ty * stride:ty * stride + tile, tx * stride:tx * stride + tile]
+                q = d.mean() * d.max() * rr[ty * stride:ty * stride + tile, tx * stride:tx * stride + tile].mean() / M ** 2
+                assert abs(r.q[u, ty, tx] - q) <= 1e-13 * q
+                iy, ix = np.unravel_index(np.argmax(d), d.shape)  # first maximum in row-major order
+                assert r.argmax[u, ty, tx] == (ty * stride + iy) * W + tx * stride + ix
