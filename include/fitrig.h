@@ -69,7 +69,11 @@ typedef struct {
   int32_t harmonics;  /* frequency branch: H = 1, 2, 4, .., 32; 0 -> 1.  The spectral refinement h of Eq. 10:          */
                       /* H = 1 maximum magnitude; H > 1 harmonic summing (R26):      */
                       /* eta = max over k and h in {1,2,4..H}, h*k <= U/2, of (|F_k| + |F_2k| + .. + |F_hk|)/sqrt(h) */
-  int32_t reserved[6];
+  int32_t stride;     /* 0 -> tile.  Window stride in pixels, a divisor of tile.  stride == tile: the paper's         */
+                      /* non-overlapping tiles.  stride < tile: OVERLAPPING windows of tile pixels     */
+                      /* every stride pixels (an extension, R27); Ty = max(1, ceil(H/stride) - tile/stride + 1);     */
+                      /* image branch only, no accumulation, no row shards; candidate (x, y) stays the peak pixel    */
+  int32_t reserved[5];
 } fitrig_params;
 
 /* One candidate, 16 bytes.

@@ -26,7 +26,7 @@ class FitrigError(RuntimeError):
 class _Params(ctypes.Structure):
     _fields_ = [("tile", ctypes.c_int32), ("C", ctypes.c_float), ("ref_mode", ctypes.c_int32),
                 ("M_override", ctypes.c_float), ("branch", ctypes.c_int32), ("strip_rows", ctypes.c_int32),
-                ("device", ctypes.c_int32), ("row_offset", ctypes.c_int32), ("accumulate", ctypes.c_int32), ("harmonics", ctypes.c_int32), ("reserved", ctypes.c_int32 * 6)]
+                ("device", ctypes.c_int32), ("row_offset", ctypes.c_int32), ("accumulate", ctypes.c_int32), ("harmonics", ctypes.c_int32), ("stride", ctypes.c_int32), ("reserved", ctypes.c_int32 * 5)]
 
 
 class _Candidate(ctypes.Structure):
@@ -145,13 +145,14 @@ def _check(rc: int, allow: Tuple[int, ...] = ()) -> int:
 
 
 def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_IMAGE, strip_rows=0, device=0,
-                 row_offset=0, accumulate=0, harmonics=0):
+                 row_offset=0, accumulate=0, harmonics=0, stride=0):
     p = _Params()
     p.tile, p.C, p.ref_mode, p.M_override = int(tile), float(C), int(ref_mode), float(M_override)
     p.branch, p.strip_rows, p.device = int(branch), int(strip_rows), int(device)
     p.row_offset = int(row_offset)
     p.accumulate = int(accumulate)
     p.harmonics = int(harmonics)
+    p.stride = int(stride)
     return p
 
 

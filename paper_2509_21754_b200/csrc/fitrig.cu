@@ -71,9 +71,12 @@ struct fitrig_ctx {
   EncodeTiledFn encode;
   // map
   RawTile* raw;
-  RawTile* raw_blocks;  // N_T = 32 * m > 32: one record per 32x32 block, merged into `raw` before the finalise
-  int Ty32, Tx32;
-  bool blocks_pending;  // the last tLISI launches wrote raw_blocks (fused path), not raw (generic path)
+  RawTile* raw_blocks;  // windows made of several cells (N_T = 32 * m, overlapping windows): one record per cell,
+                        // merged into `raw` before the finalise
+  CellGeom geo;         // cell edge, cells per window edge, cells between windows
+  int Cy, Cx;           // cell grid
+  int Ty32, Tx32;       // 32-pixel block grid of the fused kernel
+  bool blocks_pending;  // the last tLISI launches wrote raw_blocks
   float *q, *tlisi, *M_dev;
   unsigned* gmax_key;  // two order-preserving keys of the running global maximum, used by alternate calls:
   int key_idx;         // the finalise kernel of one call zeroes the key of the next, so no memset sits in the stream
@@ -246,8 +249,9 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
 
   CTX_TRY(cudaMalloc(&c->raw, sizeof(RawTile) * c->nmap));
   c->Ty32 = (H + kFastTile - 1) / kFastTile; c->Tx32 = (W + kFastTile - 1) / kFastTile;
-  if (np.tile > kFastTile && np.tile % kFastTile == 0)
-    CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)c->U * c->Ty32 * c->Tx32));
+  c->geo = cell_geom(np.tile, np.stride);
+  c->Cy = (H + c->geo.cell - 1) / c->geo.cell; c->Cx = (W + c->geo.cell - 1) / c->geo.cell;
+  if (c->geo.m > 1) CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)c->U * c->Cy * c->Cx));
   CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->tlisi, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float)));
@@ -336,16 +340,20 @@ struct RowsOpt {
   unsigned* key = nullptr;  // global-maximum key to fold into (default: the key of the current call)
 };
 
-static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int ty_base,
+static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int r0,
                              bool with_max, cudaStream_t st, const RowsOpt& opt = RowsOpt()) {
-  const int tile = c->prm.tile;
+  const int tile = c->geo.cell;        // what the kernels reduce: cells (the tile itself in the plain case)
+  const int ty_base = r0 / tile;       // first cell row of this launch
+  const bool cells = c->geo.m > 1;     // records go to raw_blocks and are merged into windows before the finalise
+  RawTile* const out_raw = cells ? c->raw_blocks : c->raw;
+  const int out_Ty = cells ? c->Cy : c->Ty, out_Tx = cells ? c->Cx : c->Tx;
   unsigned* key = opt.key ? opt.key : c->gmax_key + c->key_idx;
   const int nslots = opt.zmod ? opt.zmod : c->L;
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
   if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
-  if (pl.path == 0 && ((long long)ty_base * tile) % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
+  if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
   if (pl.path == 0 && rows != c->H) plan_launch(tile, c->W, rows, c->U, c->num_sms, &pl);
 
   int rc = prof_begin(c, st);
@@ -361,12 +369,11 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
     FusedParams fp;
-    const bool big = tile > kFastTile;  // blocks of a 32 * m tile: the kernel sees a grid of 32-pixel tiles
-    fp.raw = big ? c->raw_blocks : c->raw; fp.gmax_key = key;
+    fp.raw = out_raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
-    fp.Tx = big ? c->Tx32 : c->Tx; fp.Ty = big ? c->Ty32 : c->Ty; fp.Tx32 = c->Tx32;
-    fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = big ? ty_base * (tile / kFastTile) : ty_base;
+    fp.Tx = out_Tx; fp.Ty = out_Ty; fp.Tx32 = c->Tx32;
+    fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = ty_base;
     fp.U = c->U;
     fp.ntw = pl.box_tiles; fp.ngx = (fp.Tx32 + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
     const long long G = (long long)fp.rows_tiles * fp.ngx * c->U;
@@ -382,7 +389,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;
-    if (big) c->blocks_pending = true;
+    if (cells) c->blocks_pending = true;
   } else {
     if (with_max) {
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
@@ -397,14 +404,15 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     }
     GenericParams gp;
     gp.base = base; gp.snap_stride = snap_stride; gp.rows = rows; gp.W = c->W; gp.tile = tile;
-    gp.raw = c->raw; gp.Tx = c->Tx; gp.Ty = c->Ty; gp.ty_base = ty_base; gp.rows_tiles = rows_tiles; gp.U = c->U;
+    gp.raw = out_raw; gp.Tx = out_Tx; gp.Ty = out_Ty; gp.ty_base = ty_base; gp.rows_tiles = rows_tiles; gp.U = c->U;
+    if (cells) c->blocks_pending = true;
     int G = 1;
     const long long n_t = (long long)tile * tile;
     while (G < 32 && G < n_t) G <<= 1;
     gp.G = G;
     gp.z0 = opt.z0; gp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; gp.acc = c->prm.accumulate;
     gp.C = c->prm.C;
-    const long long groups = (long long)rows_tiles * c->Tx * c->U;
+    const long long groups = (long long)rows_tiles * out_Tx * c->U;
     const long long threads = groups * G;
     const long long blocks = (threads + 255) / 256;
     if (blocks > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "generic path: too many tiles for one launch");
@@ -420,12 +428,12 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
 }
 
 static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, unsigned* key = nullptr) {
-  if (c->raw_blocks && c->blocks_pending) {  // N_T = 32 * m: block records -> tile records
+  if (c->raw_blocks && c->blocks_pending) {  // cell records -> window records
     MergeParams mp;
-    mp.blocks = c->raw_blocks; mp.raw = c->raw; mp.U = c->U; mp.Ty = c->Ty; mp.Tx = c->Tx;
-    mp.Ty32 = c->Ty32; mp.Tx32 = c->Tx32; mp.m = c->prm.tile / kFastTile; mp.tile = c->prm.tile;
+    mp.cells = c->raw_blocks; mp.raw = c->raw; mp.U = c->U; mp.Ty = c->Ty; mp.Tx = c->Tx;
+    mp.Cy = c->Cy; mp.Cx = c->Cx; mp.m = c->geo.m; mp.step = c->geo.step; mp.cell = c->geo.cell; mp.tile = c->prm.tile;
     const long long n = c->nmap;
-    merge_blocks_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4 * c->num_sms), 256, 0, st>>>(mp);
+    merge_cells_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4 * c->num_sms), 256, 0, st>>>(mp);
     CUDA_TRY(cudaGetLastError());
     c->launches++;
     c->blocks_pending = false;
@@ -434,7 +442,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
   fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
   fp.gmax_key = key ? key : c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1);
   fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
-  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
+  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.stride = c->prm.stride; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
   fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
   fp.shard_all = nullptr; fp.shard_world = 0;
   if (c->profile) {
@@ -525,7 +533,7 @@ extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, flo
     }
     CUDA_TRY(cudaEventRecord(c->ev_copied[b], c->copy_stream));
     CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copied[b], 0));
-    int rc = launch_tlisi_rows(c, c->strip_buf[b], snap_stride, rows, r0 / c->prm.tile, true, st);
+    int rc = launch_tlisi_rows(c, c->strip_buf[b], snap_stride, rows, r0, true, st);
     if (rc) return rc;
     CUDA_TRY(cudaEventRecord(c->ev_free[b], st));
     c->ev_free_pending[b] = true;
@@ -586,7 +594,7 @@ static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_
   cp.raw = c->raw; cp.kstar = c->kstar;
   cp.mu = freq ? c->smu : c->mu; cp.sigma = freq ? c->ssigma : c->sigma;
   cp.tau = tau; cp.rows = (int)rows; cp.nt = c->nt;
-  cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.branch = c->prm.branch;
+  cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.stride = c->prm.stride; cp.branch = c->prm.branch;
   cp.row_offset = c->prm.row_offset;
   cp.unit_offset = unit_offset;
   cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
@@ -707,7 +715,7 @@ extern "C" int fitrig_shard_export(fitrig_ctx* c, double* d_out, void* cuda_stre
   CUDA_TRY(cudaSetDevice(c->prm.device));
   ShardExportParams ep;
   ep.raw = c->raw; ep.gmax_key = c->gmax_key + c->key_idx; ep.out = d_out;
-  ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
+  ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.stride = c->prm.stride; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
   ep.nblk = c->fin_nblk; ep.parts = c->parts; ep.counters = c->counters;
   shard_export_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(ep);
   CUDA_TRY(cudaGetLastError());
@@ -727,7 +735,7 @@ extern "C" int fitrig_shard_import(fitrig_ctx* c, const double* d_all, int32_t w
   fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi;
   fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev;
   fp.M_override = c->prm.M_override; fp.C = c->prm.C;
-  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
+  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.stride = c->prm.stride; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
   fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
   fp.shard_all = d_all; fp.shard_world = world;
   finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
@@ -790,15 +798,15 @@ extern "C" int fitrig_get_raw(const fitrig_ctx* c, float* sumD, float* maxD, flo
   CUDA_TRY(cudaDeviceSynchronize());
   std::vector<RawTile> r(c->nmap);
   CUDA_TRY(cudaMemcpy(r.data(), c->raw, sizeof(RawTile) * c->nmap, cudaMemcpyDeviceToHost));
-  const int tile = c->prm.tile;
+  const int tile = c->prm.tile, stride = c->prm.stride;
   for (long long i = 0; i < c->nmap; ++i) {
     const long long t = i % c->nt;
     const int ty = (int)(t / c->Tx), tx = (int)(t % c->Tx);
     if (sumD) sumD[i] = r[i].sumD;
     if (maxD) maxD[i] = r[i].maxD;
     if (sumR) sumR[i] = r[i].sumR;
-    if (ax) ax[i] = tx * tile + r[i].pos % tile;
-    if (ay) ay[i] = ty * tile + r[i].pos / tile;
+    if (ax) ax[i] = tx * stride + r[i].pos % tile;
+    if (ay) ay[i] = ty * stride + r[i].pos / tile;
   }
   return FITRIG_OK;
 }

@@ -599,18 +599,20 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
 }
 // ---------------------------------------------------------------------------------------------
-// Tiles of N_T = 32 * m pixels: the fused kernel (T = 32) leaves one record per 32x32 block; a tile is the
-// union of m x m blocks (fewer at the image edge).  Sum Delta and sum r add up, max Delta is the max, and the
-// first max-Delta pixel in row-major order OF THE TILE (R20) is the candidate with the smallest
-// row * N_T + col among the blocks that attain the max.
+// Windows made of cells.  The tLISI kernels reduce square CELLS (the tile itself in the plain case); a window
+// is m x m cells, placed every `step` cells:
+//   tiles of N_T = 32 * m pixels        cells of 32, step = m   (non-overlapping)
+//   overlapping windows (R27, f-4)      cells of `stride` pixels (or 32), step = stride / cell < m
+// Sum Delta and sum r add up, max Delta is the max, and the first max-Delta pixel in row-major order OF THE
+// WINDOW (R20) is the candidate with the smallest row * N_T + col among the cells that attain the max.
 // ---------------------------------------------------------------------------------------------
 struct MergeParams {
-  const RawTile* blocks;  // [U][Ty32][Tx32]
-  RawTile* raw;           // [U][Ty][Tx]
-  int U, Ty, Tx, Ty32, Tx32, m, tile;
+  const RawTile* cells;  // [U][Cy][Cx]
+  RawTile* raw;          // [U][Ty][Tx]
+  int U, Ty, Tx, Cy, Cx, m, step, cell, tile;
 };
 
-__global__ void __launch_bounds__(256) merge_blocks_kernel(const MergeParams p) {
+__global__ void __launch_bounds__(256) merge_cells_kernel(const MergeParams p) {
   const long long n = (long long)p.U * p.Ty * p.Tx;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const int u = (int)(i / ((long long)p.Ty * p.Tx));
@@ -620,15 +622,15 @@ __global__ void __launch_bounds__(256) merge_blocks_kernel(const MergeParams p) 
     o.sumD = 0.f; o.maxD = 0.f; o.sumR = 0.f; o.pos = 0x7fffffff;
     bool first = true;
     for (int by = 0; by < p.m; ++by) {
-      const int y32 = ty * p.m + by;
-      if (y32 >= p.Ty32) break;
+      const int cy = ty * p.step + by;
+      if (cy >= p.Cy) break;
       for (int bx = 0; bx < p.m; ++bx) {
-        const int x32 = tx * p.m + bx;
-        if (x32 >= p.Tx32) break;
-        const RawTile b = p.blocks[((size_t)u * p.Ty32 + y32) * p.Tx32 + x32];
-        o.sumD += b.sumD;  // fixed (block row, block column) order: deterministic
+        const int cx = tx * p.step + bx;
+        if (cx >= p.Cx) break;
+        const RawTile b = p.cells[((size_t)u * p.Cy + cy) * p.Cx + cx];
+        o.sumD += b.sumD;  // fixed (cell row, cell column) order: deterministic
         o.sumR += b.sumR;
-        const int pos = (by * kFastTile + b.pos / kFastTile) * p.tile + bx * kFastTile + b.pos % kFastTile;
+        const int pos = (by * p.cell + b.pos / p.cell) * p.tile + bx * p.cell + b.pos % p.cell;
         if (first || b.maxD > o.maxD || (b.maxD == o.maxD && pos < o.pos)) { o.maxD = b.maxD; o.pos = pos; first = false; }
       }
     }
@@ -792,7 +794,7 @@ struct FinalizeParams {
   float* M_out;        // device scalar: the M that was used
   float M_override;
   float C;
-  int H, W, tile, Ty, Tx, U;
+  int H, W, tile, stride, Ty, Tx, U;  // windows of `tile` pixels every `stride` pixels (stride == tile: tiles)
   int nblk;            // blocks per unit
   StatPartial* parts;  // [U][nblk]
   unsigned* counters;  // [U]
@@ -829,7 +831,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
   for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
     const unsigned tu = (unsigned)t;  // tiles per unit < 2^31
     const int ty = (int)(tu / (unsigned)p.Tx), tx = (int)(tu - (unsigned)ty * (unsigned)p.Tx);
-    const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
+    const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
     const double n_t = (double)h * (double)w;  // R5: partial tiles use their own pixel count
     const RawTile r = p.raw[base + t];
     // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2
@@ -868,7 +870,7 @@ struct ShardExportParams {
   const RawTile* raw;
   const unsigned* gmax_key;
   double* out;          // [2 + 2U]
-  int H, W, tile, Ty, Tx, U;
+  int H, W, tile, stride, Ty, Tx, U;
   int nblk;             // blocks per unit
   StatPartial* parts;   // [U][nblk]
   unsigned* counters;   // [U]
@@ -884,7 +886,7 @@ __global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportPara
   double s = 0.0, s2 = 0.0;
   for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
     const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
-    const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
+    const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
     const double n_t = (double)h * (double)w;
     const RawTile r = p.raw[base + t];
     const double pv = ((double)r.sumD / n_t) * (double)r.maxD * ((double)r.sumR / n_t);  // Eq. 6 without 1/M^2
@@ -1025,7 +1027,7 @@ struct CompactParams {
   float tau;
   int rows;             // U or 1
   long long nt;         // tiles per row
-  int Tx, Ty, H, W, tile, branch;
+  int Tx, Ty, H, W, tile, stride, branch;
   int row_offset;       // image row of this context's first row (row shards), added to y
   int unit_offset;      // real-time mode: index of the unit the one-row map belongs to, added to `snapshot`
   fitrig_candidate* out;
@@ -1125,13 +1127,13 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
         fitrig_candidate cd;
         if (p.branch == FITRIG_BRANCH_IMAGE) {
           const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
-          cd.x = tx * p.tile + pos % p.tile;
-          cd.y = p.row_offset + ty * p.tile + pos / p.tile;
+          cd.x = tx * p.stride + pos % p.tile;
+          cd.y = p.row_offset + ty * p.stride + pos / p.tile;
           cd.snapshot = row + p.unit_offset;
         } else {
-          const int h = min(p.tile, p.H - ty * p.tile), w = min(p.tile, p.W - tx * p.tile);
-          cd.x = tx * p.tile + w / 2;  // tile centre (R18)
-          cd.y = p.row_offset + ty * p.tile + h / 2;
+          const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
+          cd.x = tx * p.stride + w / 2;  // tile centre (R18)
+          cd.y = p.row_offset + ty * p.stride + h / 2;
           cd.snapshot = p.kstar[t];
         }
         cd.score = z;

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <numeric>
 
 namespace fitrig {
 
@@ -43,6 +44,15 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
     return FITRIG_ERR_INVALID_ARG;
   }
   out->strip_rows = p->strip_rows;
+  out->stride = p->stride == 0 ? out->tile : p->stride;
+  if (out->stride < 1 || out->tile % out->stride != 0) {
+    *why = "stride must divide tile (0 selects tile: non-overlapping tiles)";
+    return FITRIG_ERR_INVALID_ARG;
+  }
+  if (out->stride != out->tile && (p->branch != 0 || out->accumulate != 1 || p->row_offset != 0)) {
+    *why = "overlapping windows (stride < tile): image branch, no accumulation, no row shards";
+    return FITRIG_ERR_INVALID_ARG;
+  }
   out->harmonics = p->harmonics == 0 ? 1 : p->harmonics;
   if (out->harmonics < 1 || out->harmonics > 32 || (out->harmonics & (out->harmonics - 1)) != 0) {
     *why = "harmonics must be 1, 2, 4, 8, 16 or 32 (0 selects 1)";
@@ -61,6 +71,25 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8 adjacent blocks is
 // 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes of 32 KB in flight per
 // SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
+CellGeom cell_geom(int tile, int stride) {
+  CellGeom g;
+  if (stride == tile) {  // non-overlapping: tiles of 32 * m pixels are m x m blocks of 32, everything else is its own cell
+    if (tile > kFastTile && tile % kFastTile == 0) { g.cell = kFastTile; g.m = tile / kFastTile; g.step = g.m; }
+    else { g.cell = tile; g.m = 1; g.step = 1; }
+  } else if (stride % kFastTile == 0) {
+    g.cell = kFastTile; g.m = tile / kFastTile; g.step = stride / kFastTile;
+  } else {
+    g.cell = stride; g.m = tile / stride; g.step = 1;
+  }
+  return g;
+}
+
+int n_windows(int n, int tile, int stride) {
+  if (stride == tile) return (n + tile - 1) / tile;  // R5: a partial last tile
+  const int cells = (n + stride - 1) / stride, m = tile / stride;
+  return std::max(1, cells - m + 1);  // R27
+}
+
 bool fused_tile(int tile) {
   return tile == 16 || tile == 8 || tile == 4 || tile == 2 || tile == 1 || (tile >= kFastTile && tile % kFastTile == 0);
 }
@@ -118,23 +147,25 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   memset(out, 0, sizeof(*out));
   const int tile = np.tile;
   out->units = L / np.accumulate - 2;
-  out->Ty = (H + tile - 1) / tile;
-  out->Tx = (W + tile - 1) / tile;
+  out->Ty = n_windows(H, tile, np.stride);
+  out->Tx = n_windows(W, tile, np.stride);
+  const int cell = cell_geom(tile, np.stride).cell;
   // strip schedule for fitrig_stream: ~256 MiB of snapshot rows per strip (all L snapshots), a multiple of tile
   long long rows = np.strip_rows;
   if (rows == 0) {
     const long long target = 256ll << 20;
     rows = target / ((long long)L * W * 4);
-    const long long q = (kFastTile % tile == 0) ? kFastTile : tile;  // whole 32-row blocks for the fused path
+    // whole tiles, and whole 32-row blocks when the cells ride the fused path
+    const long long q = (kFastTile % cell == 0) ? std::lcm((long long)tile, (long long)kFastTile) : tile;
     rows = std::max<long long>(q, rows / q * q);
   }
-  const long long Hpad = (long long)out->Ty * tile;
+  const long long Hpad = ((long long)H + tile - 1) / tile * tile;
   rows = std::min(rows, Hpad);
   out->strip_rows = (int32_t)rows;
   out->n_strips = (int32_t)((H + rows - 1) / rows);
   out->n_strip_buffers = out->n_strips >= 3 ? 3 : out->n_strips;
   out->strip_buffer_bytes = (int64_t)L * rows * W * 4;
-  plan_launch(tile, W, H, out->units, num_sms, out);
+  plan_launch(cell, W, H, out->units, num_sms, out);
   const int64_t n = (int64_t)out->units * out->Ty * out->Tx;
   out->workspace_bytes = n * (16 + 4 + 4) + (int64_t)out->Ty * out->Tx * 8 + (1 << 20);
   return FITRIG_OK;

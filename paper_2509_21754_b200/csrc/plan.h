@@ -27,7 +27,18 @@ struct NormParams {  // fitrig_params with defaults applied
   int row_offset;
   int accumulate;  // >= 1
   int harmonics;   // 1, 2, 4, .., 32
+  int stride;      // window stride in pixels; == tile: the paper's non-overlapping tiles
 };
+
+// What the tLISI kernels reduce (square cells) and how windows are made of cells (see kernels.cuh, merge_cells_kernel):
+// cell == tile and m == 1 in the plain case.
+struct CellGeom {
+  int cell;  // cell edge in pixels
+  int m;     // a window is m x m cells
+  int step;  // cells between consecutive windows
+};
+CellGeom cell_geom(int tile, int stride);
+int n_windows(int n, int tile, int stride);  // windows along an axis of n pixels
 
 // Validates and applies defaults.  Returns FITRIG_OK or FITRIG_ERR_INVALID_ARG (+ message in *why).
 int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, NormParams* out, const char** why);

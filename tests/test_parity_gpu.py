@@ -492,6 +492,64 @@ def test_accumulate_one_is_bit_identical_and_frequency_branch_accumulates(long_t
 
 
 # ------------------------------------------------------------------------------------------
+# overlapping windows (an extension; R27)
+# ------------------------------------------------------------------------------------------
+def _check_windows(st, g, ref, tile, stride, tau):
+    sd, md, sr, ax, ay = g["raw"]
+    res = ref.res
+    assert g["dims"] == (res.U, res.Ty, res.Tx)
+    np.testing.assert_allclose(sd, res.sumD, rtol=2e-5, atol=1e-30)
+    np.testing.assert_allclose(md, res.maxD, rtol=1e-6, atol=1e-30)
+    np.testing.assert_allclose(sr, res.sumR, rtol=2e-5, atol=2e-5)
+    W = st.shape[2]
+    exact = (ay.astype(np.int64) * W + ax) == res.argmax
+    assert exact.mean() > 0.99
+    stack_np = st.cpu().numpy()
+    for (u, ty, tx) in np.argwhere(~exact)[:2000]:
+        x, y = int(ax[u, ty, tx]), int(ay[u, ty, tx])
+        assert oracle_delta_at(stack_np, u, x, y) >= (1 - 1e-5) * res.maxD[u, ty, tx]
+        assert ty * stride <= y < ty * stride + tile and tx * stride <= x < tx * stride + tile
+    assert g["M"] == np.float32(res.M)
+    util.assert_map_close(g["q"], res.q, g["tlisi"], res.tlisi)
+    np.testing.assert_allclose(g["mu"], ref.mu, rtol=1e-5)
+    np.testing.assert_allclose(g["sigma"], ref.sigma, rtol=2e-4, atol=1e-30)
+    c, n = g["cands"][tau]
+    Tx = res.Tx
+    lst = []
+    for r in c:  # the window of a candidate is not recoverable from its peak pixel: find it through the oracle's z order
+        lst.append((int(r["x"]), int(r["y"]), int(r["snapshot"]), float(r["score"])))
+    sel = [(int(u), int(t)) for u, t in zip(ref.cands.snapshot, ref.cands.tile)]
+    band = 1e-4 * (np.abs(ref.mu) / ref.sigma)[:, None, None] + 1e-4 * np.abs(ref.z)
+    sure = {(u, t) for (u, t) in sel if ref.z[u].flat[t] > tau + band[u].flat[t]}
+    assert len(lst) >= len(sure) and abs(len(lst) - len(sel)) <= int((np.abs(ref.z - tau) <= band).sum())
+    if len(lst) == len(sel):
+        for (x, y, u, score), (ru, rt) in zip(lst, sel):
+            assert u == ru and abs(score - ref.z[ru].flat[rt]) <= band[ru].flat[rt] + 1e-6 * abs(score)
+            ty, tx = divmod(rt, Tx)
+            assert ty * stride <= y < ty * stride + tile and tx * stride <= x < tx * stride + tile
+
+
+@pytest.mark.parametrize("H,W,tile,stride,use_stream", [(256, 256, 32, 16, False), (250, 252, 32, 8, False), (256, 256, 64, 32, False),
+                                                        (200, 120, 16, 4, False), (96, 64, 32, 32, False), (250, 252, 32, 16, True),
+                                                        (130, 100, 64, 16, False), (120, 100, 24, 12, False), (90, 250, 32, 8, False)])
+def test_overlapping_windows_match_oracle(tiny, H, W, tile, stride, use_stream):
+    st = tiny[0][:, :H, :W].contiguous()
+    tau = 3.0
+    kw = dict(strip_rows=64) if use_stream else {}
+    g = gpu_run(st, taus=(tau,), tile=tile, stride=stride, use_stream=use_stream, capacity=1 << 18, **kw)
+    ref = oracle_run(st, tile=tile, tau=tau, stride=stride)
+    _check_windows(st, g, ref, tile, stride, tau)
+
+
+def test_windows_arguments_are_validated():
+    for kw in (dict(tile=32, stride=12), dict(tile=32, stride=16, branch=fitrig.BRANCH_FREQUENCY),
+               dict(tile=32, stride=16, accumulate=2), dict(tile=32, stride=16, row_offset=32), dict(tile=32, stride=-4)):
+        with pytest.raises(fitrig.FitrigError) as e:
+            fitrig.Context(128, 128, 8, **kw)
+        assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------
 # real-time mode: fitrig_push (PAPER.md:189 running maximum; Fig. 14 timeline), against oracle.run_realtime
 # ------------------------------------------------------------------------------------------
 def _push_all(ctx, snaps, tau, want_maps=True):
