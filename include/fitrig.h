@@ -90,7 +90,8 @@ typedef struct {
 /* How the library will run a problem; pure host arithmetic (no CUDA call), see fitrig_plan_query. */
 typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
-  int32_t path;              /* 0: fused TMA time-marching kernel (N_T = 32, 16 or 8; W % 4 == 0)*/
+  int32_t path;              /* 0: fused TMA time-marching kernel: cells (= tiles, or the stride of overlapping */
+                             /*    windows) of 1, 2, 4, 8, 16, 32 or 32*m pixels; W % 4 == 0                     */
                              /* 1: generic kernel (any N_T, any W)                               */
   int32_t units_per_cta;     /* fused path: (box column, unit) pairs per CTA, ceil(boxes * U / grid) */
   int32_t box_tiles;         /* fused path: adjacent 32x32 pixel blocks fetched as one TMA box (1..8) */

@@ -133,7 +133,7 @@ struct FusedParams {
   const float* base;     // snapshot 0 of this launch's rows (the memory the TMA descriptor covers)
   long long snap_stride; // elements between consecutive snapshots
   int W;                 // image width (row pitch in elements)
-  int Tx, Ty;            // whole-map tile grid (tiles of N_T = 32, 16 or 8 pixels)
+  int Tx, Ty;            // grid of the cells this launch reduces, over the whole map (cells of 1 .. 32 pixels)
   int Tx32;              // 32-pixel block columns = ceil(W / 32): a consumer warp owns one 32x32 block
   int rows_tiles;        // rows of 32x32 blocks covered by this launch (whole image, or one strip)
   int ty_base;           // first tile row (in tiles of N_T) of this launch inside the whole map

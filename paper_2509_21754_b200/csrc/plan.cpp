@@ -67,7 +67,7 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 }
 
 // Fused path: one persistent CTA per SM; a consumer warp owns a 32x32 pixel block = (32 / N_T)^2 tiles for
-// N_T = 32, 16 or 8, and the CTAs share the G = boxes * U (box column, unit) pairs evenly (see
+// cells of 32, 16 or 8 pixels (a lane holds several tiles for 4, 2, 1), and the CTAs share the G = boxes * U (box column, unit) pairs evenly (see
 // kernels.cuh), so only the box width, ring depth and grid are chosen here.  A box of 8 adjacent blocks is
 // 32 rows of 1 KB: long enough bursts for HBM to run at its streaming rate.  6 boxes of 32 KB in flight per
 // SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
