@@ -4,7 +4,10 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
 bench.py's cpu_baseline / --impl reference legs may import this package.  It does not
 import, link or read anything of the CUDA path (paper_2509_21754_b200).
 
-All arithmetic lives in the C file; this module only marshals numpy arrays.
+The per-pixel, per-tile and spectral arithmetic lives in the C file; this module marshals numpy arrays and holds
+the three steps that are plain numpy one-liners: the fp64 sums of snapshot accumulation (`accumulate`), the
+maximum of the accumulated images (`_tlisi_f64`), and the running maximum of the real-time forms
+(`run_realtime`, `run_realtime_frequency`).
 """
 from __future__ import annotations
 
@@ -21,6 +24,7 @@ _SRC = os.path.join(_HERE, "fitrig_oracle.c")
 _LIB = os.path.join(_HERE, "libfitrig_oracle.so")
 
 REF_ABS, REF_LITERAL, REF_FLOOR = 0, 1, 2
+INTERP_BILINEAR, INTERP_BICUBIC, INTERP_SPLINE, INTERP_MAKIMA = 0, 1, 2, 3
 
 
 def build(force: bool = False) -> str:
@@ -71,6 +75,11 @@ def lib() -> ctypes.CDLL:
         L.fitrig_oracle_select_spectrum.argtypes = [dp, ip32, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                                     ctypes.c_int, ctypes.c_double, ip32, ip32, ip32, ip64, dp,
                                                     ctypes.c_int64]
+        L.fitrig_oracle_interp_eval.restype = ctypes.c_int
+        L.fitrig_oracle_interp_eval.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, ctypes.c_int64, dp]
+        L.fitrig_oracle_localise.restype = ctypes.c_int
+        L.fitrig_oracle_localise.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                             ip64, ctypes.c_int64, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -356,4 +365,69 @@ def run_realtime(stack, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS
         c = select(z, res.argmax, W, tau)
         c.snapshot[:] = n
         out.append(DetectResult(res, mu, sd, z, c))
+    return out
+
+
+def interp_eval(eta: np.ndarray, method: int, u, v) -> np.ndarray:
+    """The interpolated eta surface of reading R28 at index coordinates (u, v) (tile centres at integers)."""
+    eta = np.ascontiguousarray(eta, dtype=np.float64)
+    Ty, Tx = eta.shape
+    u, v = np.broadcast_arrays(np.asarray(u, dtype=np.float64), np.asarray(v, dtype=np.float64))
+    u, v = np.ascontiguousarray(u).reshape(-1), np.ascontiguousarray(v).reshape(-1)
+    assert u.shape == v.shape
+    out = np.zeros(u.shape, dtype=np.float64)
+    rc = lib().fitrig_oracle_interp_eval(_ptr(eta), Ty, Tx, int(method), _ptr(u), _ptr(v), len(u), _ptr(out))
+    if rc != 0:
+        raise ValueError("fitrig_oracle_interp_eval: bad arguments")
+    return out
+
+
+@dataclass
+class Positions:
+    x: np.ndarray  # pixels, pixel centres at integers
+    y: np.ndarray
+    value: np.ndarray  # the interpolated surface at (x, y)
+
+
+def localise(eta: np.ndarray, tile: int, cand_tiles, method: int = INTERP_SPLINE, oversample: int = 1) -> Positions:
+    """O9 (reading R28): the maximum of the interpolated eta surface within one tile of the
+    centre of each selected tile (cand_tiles = ty * Tx + tx)."""
+    eta = np.ascontiguousarray(eta, dtype=np.float64)
+    Ty, Tx = eta.shape
+    t = np.ascontiguousarray(cand_tiles, dtype=np.int64).reshape(-1)
+    x, y, val = np.zeros(len(t)), np.zeros(len(t)), np.zeros(len(t))
+    rc = lib().fitrig_oracle_localise(_ptr(eta), Ty, Tx, int(tile), int(method), int(oversample), _ptr(t), len(t),
+                                      _ptr(x), _ptr(y), _ptr(val))
+    if rc != 0:
+        raise ValueError("fitrig_oracle_localise: bad arguments")
+    return Positions(x, y, val)
+
+
+def run_realtime_frequency(stack, window: int, tile: int = 32, C: float = 1e-6, ref_mode: int = REF_ABS,
+                           tau: float = 5.0, harmonics: int = 1) -> List[Optional[DetectResult]]:
+    """Real-time form of the image-frequency branch: one entry per unit n = 0..L-3, None while fewer than
+    `window` - 2 units exist.
+
+    PAPER.md:453 (section 3.2): "In image-frequency domain FITrig, a set of time-sequential snapshots needs to be
+    loaded onto the device.  Rather than loading all snapshots at once ..." with the timeline of Fig. 14
+    (PAPER.md:457-467), and the tLISI cube of PAPER.md:341.  Reading R29 (DESIGN.md): snapshots arrive one at a time;
+    once unit n is computed, Eq. 10-12 run over the cube of the LAST U_w = window - 2 units, n - U_w + 1 .. n, i.e.
+    over snapshots x_{n-U_w+1} .. x_{n+2}; every tile matrix of that cube is normalised by the running maximum
+    M_n = max(largest pixel of x_0 .. x_{n+2}, C) (R24).  eta scales with 1/M^2, z (Eq. 11) does not, so the
+    candidates are those of the batch branch on the same `window` snapshots.
+    """
+    snaps = as_snapshots(stack)
+    L = len(snaps)
+    if L < 3 or window < 3:
+        raise ValueError("need L >= 3 snapshots and a window of at least 3 snapshots (PAPER.md:155)")
+    Uw = window - 2
+    out: List[Optional[DetectResult]] = []
+    running = max(float(np.max(snaps[0])), float(np.max(snaps[1])))
+    for n in range(L - 2):
+        running = max(running, float(np.max(snaps[n + 2])))  # x_{n+2} has just arrived
+        if n < Uw - 1:
+            out.append(None)
+            continue
+        out.append(run(snaps[n - Uw + 1:n + 3], tile=tile, C=C, ref_mode=ref_mode, M=max(running, C), tau=tau,
+                       branch=1, harmonics=harmonics))
     return out

@@ -11,7 +11,7 @@
  * concession to run time is an OpenMP "parallel for" over independent (unit, tile-row)
  * pairs, which the paper itself states are independent.
  *
- * Citations are /root/reference/PAPER.md line numbers (+ equation).  Readings R1..R23
+ * Citations are /root/reference/PAPER.md line numbers (+ equation).  Readings R1..R28
  * of silent / ambiguous passages are SURVEY.md section 8(c), restated in DESIGN.md.
  *
  * Notation (0-based): snapshots x_0..x_{L-1}, each H x W row-major fp32.
@@ -334,4 +334,246 @@ int64_t fitrig_oracle_select_spectrum(const double* z, const int32_t* kstar, int
       }
     }
   return k;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O9.  Sub-tile localisation by interpolating the spectrum matrix eta (section 2.4.2: "interpolation
+ * methods are activated for precise pulsar localisation in the selected regions ... bilinear, spline, bicubic, or
+ * Makima cubic interpolation"; section 3.1: "We apply spline interpolation to the spectrum matrix ...
+ * the peak position, corresponding to the pulsar position").  The paper names the four schemes and gives no formula;
+ * reading R28:
+ *
+ *   - eta_t is a sample of a surface at the CENTRE of tile t.  Index coordinates: tile column tx sits at u = tx, tile
+ *     row ty at v = ty; pixel x (pixel centres at integers) is u = (x + 0.5) / N_T - 0.5, i.e. the centre of tile tx
+ *     is x_c = (tx + 0.5) N_T - 0.5.  (A partial edge tile is placed at its nominal full-tile centre.)
+ *   - the surface is the tensor-product interpolant of the Ty x Tx samples on that uniform grid: first along x
+ *     (within every tile row), then along y, with one of the four named 1-D schemes -- the four methods of the
+ *     usual gridded-interpolation routine ('linear', 'cubic', 'spline', 'makima'):
+ *       0 BILINEAR  piecewise linear
+ *       1 BICUBIC   cubic convolution, Keys (1981) kernel a = -1/2, with Keys' boundary samples
+ *                   f_{-1} = 3 f_0 - 3 f_1 + f_2 and f_n = 3 f_{n-1} - 3 f_{n-2} + f_{n-3}
+ *       2 SPLINE    cubic spline with not-a-knot end conditions (3 samples: the parabola through them)
+ *       3 MAKIMA    modified Akima piecewise cubic Hermite: node slopes from the weights
+ *                   w1 = |d_{i+1} - d_i| + |d_{i+1} + d_i| / 2, w2 = |d_{i-1} - d_{i-2}| + |d_{i-1} + d_{i-2}| / 2,
+ *                   slope = (w1 d_{i-1} + w2 d_i) / (w1 + w2), 0 when w1 + w2 = 0; d extended by
+ *                   d_{-1} = 2 d_0 - d_1, d_{-2} = 2 d_{-1} - d_0 and likewise at the far end
+ *     (2 samples along an axis: every scheme is the straight line; 1 sample: the constant).
+ *   - for a selected tile (ty, tx) the surface is evaluated on the lattice
+ *         x = x_c + i / r,  y = y_c + j / r,   i, j = -N_T r .. +N_T r   (r = oversample >= 1)
+ *     that is u = tx + i / (r N_T), v = ty + j / (r N_T): one tile either side of the tile's centre, which the
+ *     centres of the neighbouring tiles bound exactly; lattice points outside the hull of the tile centres
+ *     (u < 0, u > Tx - 1, v < 0, v > Ty - 1) are left out (no extrapolation);
+ *   - the position is the lattice point with the largest value, the first in (j, i) row-major order on ties.
+ *
+ * Everything is evaluated literally: the spline solves its full linear system (n equations, the two not-a-knot rows
+ * written out) by Gaussian elimination, row by row and then for every lattice column (built once per column: it does
+ * not depend on v).
+ * --------------------------------------------------------------------------------------------- */
+#define ORACLE_INTERP_BILINEAR 0
+#define ORACLE_INTERP_BICUBIC 1
+#define ORACLE_INTERP_SPLINE 2
+#define ORACLE_INTERP_MAKIMA 3
+
+/* Gaussian elimination with partial pivoting: A is n x n row-major, b is overwritten with the solution. */
+static void solve_dense(int n, double* A, double* b) {
+  for (int c = 0; c < n; ++c) {
+    int piv = c;
+    for (int r = c + 1; r < n; ++r)
+      if (fabs(A[(size_t)r * n + c]) > fabs(A[(size_t)piv * n + c])) piv = r;
+    if (piv != c) {
+      for (int k = 0; k < n; ++k) {
+        const double t = A[(size_t)c * n + k];
+        A[(size_t)c * n + k] = A[(size_t)piv * n + k];
+        A[(size_t)piv * n + k] = t;
+      }
+      const double t = b[c];
+      b[c] = b[piv];
+      b[piv] = t;
+    }
+    for (int r = c + 1; r < n; ++r) {
+      const double f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+      if (f == 0.0) continue;
+      for (int k = c; k < n; ++k) A[(size_t)r * n + k] -= f * A[(size_t)c * n + k];
+      b[r] -= f * b[c];
+    }
+  }
+  for (int r = n - 1; r >= 0; --r) {
+    double s = b[r];
+    for (int k = r + 1; k < n; ++k) s -= A[(size_t)r * n + k] * b[k];
+    b[r] = s / A[(size_t)r * n + r];
+  }
+}
+
+/* Second derivatives m_0..m_{n-1} of the not-a-knot cubic spline through (i, f_i), i = 0..n-1 (unit spacing), n >= 3:
+ *   interior knots  m_{i-1} + 4 m_i + m_{i+1} = 6 (f_{i-1} - 2 f_i + f_{i+1}),  i = 1..n-2
+ *   not-a-knot      m_0 - 2 m_1 + m_2 = 0  and  m_{n-3} - 2 m_{n-2} + m_{n-1} = 0   (continuous third derivative at
+ *                   the second and the second-to-last knot)
+ * n == 3: both end conditions are the same equation; the spline is the parabola, m_i = f_0 - 2 f_1 + f_2. */
+static void spline_second_derivs(const double* f, int n, double* m) {
+  if (n < 3) {
+    for (int i = 0; i < n; ++i) m[i] = 0.0;
+    return;
+  }
+  if (n == 3) {
+    m[0] = m[1] = m[2] = f[0] - 2.0 * f[1] + f[2];
+    return;
+  }
+  double* A = (double*)calloc((size_t)n * n, sizeof(double));
+  A[0] = 1.0; A[1] = -2.0; A[2] = 1.0;
+  m[0] = 0.0;
+  for (int i = 1; i <= n - 2; ++i) {
+    A[(size_t)i * n + i - 1] = 1.0;
+    A[(size_t)i * n + i] = 4.0;
+    A[(size_t)i * n + i + 1] = 1.0;
+    m[i] = 6.0 * (f[i - 1] - 2.0 * f[i] + f[i + 1]);
+  }
+  A[(size_t)(n - 1) * n + n - 3] = 1.0; A[(size_t)(n - 1) * n + n - 2] = -2.0; A[(size_t)(n - 1) * n + n - 1] = 1.0;
+  m[n - 1] = 0.0;
+  solve_dense(n, A, m);
+  free(A);
+}
+
+/* Keys' cubic convolution kernel, a = -1/2. */
+static double keys_kernel(double s) {
+  s = fabs(s);
+  if (s <= 1.0) return (1.5 * s - 2.5) * s * s + 1.0;
+  if (s < 2.0) return ((-0.5 * s + 2.5) * s - 4.0) * s + 2.0;
+  return 0.0;
+}
+
+/* Sample f_i with Keys' boundary extension (two samples: the straight line through them). */
+static double keys_sample(const double* f, int n, int i) {
+  if (i >= 0 && i < n) return f[i];
+  if (n == 2) return (i < 0) ? 2.0 * f[0] - f[1] : 2.0 * f[1] - f[0];
+  return (i < 0) ? 3.0 * f[0] - 3.0 * f[1] + f[2] : 3.0 * f[n - 1] - 3.0 * f[n - 2] + f[n - 3];
+}
+
+/* Difference d_i = f_{i+1} - f_i, i = 0..n-2, extended linearly by two entries at either end (makima). */
+static double makima_diff(const double* f, int n, int i) {
+  if (i >= 0 && i <= n - 2) return f[i + 1] - f[i];
+  if (n == 2) return f[1] - f[0];
+  if (i < 0) {
+    const double d0 = f[1] - f[0], d1 = f[2] - f[1];
+    const double dm1 = 2.0 * d0 - d1;
+    return (i == -1) ? dm1 : 2.0 * dm1 - d0;
+  }
+  const double e0 = f[n - 1] - f[n - 2], e1 = f[n - 2] - f[n - 3];
+  const double ep1 = 2.0 * e0 - e1;
+  return (i == n - 1) ? ep1 : 2.0 * ep1 - e0;
+}
+
+static double makima_slope(const double* f, int n, int i) {
+  const double dm2 = makima_diff(f, n, i - 2), dm1 = makima_diff(f, n, i - 1);
+  const double d0 = makima_diff(f, n, i), d1 = makima_diff(f, n, i + 1);
+  const double w1 = fabs(d1 - d0) + fabs(d1 + d0) / 2.0;
+  const double w2 = fabs(dm1 - dm2) + fabs(dm1 + dm2) / 2.0;
+  return (w1 + w2 > 0.0) ? (w1 * dm1 + w2 * d0) / (w1 + w2) : 0.0;
+}
+
+/* Value at index coordinate u in [0, n-1] of the 1-D interpolant through (i, f_i).  m: the spline's second
+ * derivatives (method SPLINE only). */
+static double interp1_eval(const double* f, const double* m, int n, int method, double u) {
+  if (n == 1) return f[0];
+  int i = (int)floor(u);
+  if (i < 0) i = 0;
+  if (i > n - 2) i = n - 2;
+  const double t = u - (double)i;
+  if (method == ORACLE_INTERP_BILINEAR || n == 2) return (1.0 - t) * f[i] + t * f[i + 1];
+  if (method == ORACLE_INTERP_BICUBIC) {
+    double s = 0.0;
+    for (int k = -1; k <= 2; ++k) s += keys_sample(f, n, i + k) * keys_kernel(t - (double)k);
+    return s;
+  }
+  if (method == ORACLE_INTERP_SPLINE) {
+    const double a = 1.0 - t;
+    return a * f[i] + t * f[i + 1] + ((a * a * a - a) * m[i] + (t * t * t - t) * m[i + 1]) / 6.0;
+  }
+  /* makima: cubic Hermite with the modified Akima slopes */
+  const double s0 = makima_slope(f, n, i), s1 = makima_slope(f, n, i + 1);
+  const double t2 = t * t, t3 = t2 * t;
+  return (2.0 * t3 - 3.0 * t2 + 1.0) * f[i] + (t3 - 2.0 * t2 + t) * s0 + (-2.0 * t3 + 3.0 * t2) * f[i + 1] +
+         (t3 - t2) * s1;
+}
+
+/* Tensor-product surface at (u, v): along x in every row, then along y.  rowm: [Ty][Tx] second derivatives of the
+ * row splines (SPLINE) or NULL.  col, colm: scratch of Ty doubles each. */
+static double surface_eval(const double* eta, const double* rowm, int Ty, int Tx, int method, double u, double v,
+                           double* col, double* colm) {
+  for (int ty = 0; ty < Ty; ++ty)
+    col[ty] = interp1_eval(eta + (size_t)ty * Tx, rowm ? rowm + (size_t)ty * Tx : NULL, Tx, method, u);
+  if (method == ORACLE_INTERP_SPLINE) spline_second_derivs(col, Ty, colm);
+  return interp1_eval(col, colm, Ty, method, v);
+}
+
+/* The surface at npts index coordinates (u_k, v_k), 0 <= u <= Tx-1, 0 <= v <= Ty-1 (for the pins).  Returns 0 or -1. */
+int fitrig_oracle_interp_eval(const double* eta, int Ty, int Tx, int method, const double* u, const double* v,
+                              int64_t npts, double* out) {
+  if (!eta || Ty < 1 || Tx < 1 || method < 0 || method > 3) return -1;
+  double* rowm = NULL;
+  if (method == ORACLE_INTERP_SPLINE) {
+    rowm = (double*)malloc(sizeof(double) * (size_t)Ty * Tx);
+    for (int ty = 0; ty < Ty; ++ty) spline_second_derivs(eta + (size_t)ty * Tx, Tx, rowm + (size_t)ty * Tx);
+  }
+  double* col = (double*)malloc(sizeof(double) * (size_t)Ty * 2);
+  for (int64_t k = 0; k < npts; ++k) out[k] = surface_eval(eta, rowm, Ty, Tx, method, u[k], v[k], col, col + Ty);
+  free(col);
+  free(rowm);
+  return 0;
+}
+
+/* Position of the surface's maximum around each selected tile (R28).  cand_tile[k] = ty * Tx + tx.  Outputs per
+ * candidate: x, y in pixels (pixel centres at integers) and the surface value there.  Returns 0 or -1. */
+int fitrig_oracle_localise(const double* eta, int Ty, int Tx, int tile, int method, int oversample,
+                           const int64_t* cand_tile, int64_t ncand, double* out_x, double* out_y, double* out_val) {
+  if (!eta || Ty < 1 || Tx < 1 || tile < 1 || oversample < 1 || method < 0 || method > 3) return -1;
+  double* rowm = NULL;
+  if (method == ORACLE_INTERP_SPLINE) {
+    rowm = (double*)malloc(sizeof(double) * (size_t)Ty * Tx);
+    for (int ty = 0; ty < Ty; ++ty) spline_second_derivs(eta + (size_t)ty * Tx, Tx, rowm + (size_t)ty * Tx);
+  }
+  const int half = tile * oversample;  /* lattice offsets -half .. +half, spacing 1 / oversample pixels */
+  const int side = 2 * half + 1;
+  double* col = (double*)malloc(sizeof(double) * (size_t)Ty * 2);
+  double* val = (double*)malloc(sizeof(double) * (size_t)side * side);  /* surface on the lattice, [j][i] */
+  for (int64_t k = 0; k < ncand; ++k) {
+    const int ty = (int)(cand_tile[k] / Tx), tx = (int)(cand_tile[k] % Tx);
+    const double xc = ((double)tx + 0.5) * (double)tile - 0.5, yc = ((double)ty + 0.5) * (double)tile - 0.5;
+    /* the column of row-interpolant values at u does not depend on v: built once per lattice column */
+    for (int i = -half; i <= half; ++i) {
+      const double u = (double)tx + (double)i / (double)half;
+      if (u < 0.0 || u > (double)(Tx - 1)) continue;
+      for (int r = 0; r < Ty; ++r)
+        col[r] = interp1_eval(eta + (size_t)r * Tx, rowm ? rowm + (size_t)r * Tx : NULL, Tx, method, u);
+      if (method == ORACLE_INTERP_SPLINE) spline_second_derivs(col, Ty, col + Ty);
+      for (int j = -half; j <= half; ++j) {
+        const double v = (double)ty + (double)j / (double)half;
+        if (v < 0.0 || v > (double)(Ty - 1)) continue;
+        val[(size_t)(j + half) * side + (i + half)] = interp1_eval(col, col + Ty, Ty, method, v);
+      }
+    }
+    double best = 0.0, bx = xc, by = yc;
+    int first = 1;
+    for (int j = -half; j <= half; ++j) {
+      const double v = (double)ty + (double)j / (double)half;
+      if (v < 0.0 || v > (double)(Ty - 1)) continue;
+      for (int i = -half; i <= half; ++i) {
+        const double u = (double)tx + (double)i / (double)half;
+        if (u < 0.0 || u > (double)(Tx - 1)) continue;
+        const double w = val[(size_t)(j + half) * side + (i + half)];
+        if (first || w > best) {
+          best = w;
+          bx = xc + (double)i / (double)oversample;
+          by = yc + (double)j / (double)oversample;
+          first = 0;
+        }
+      }
+    }
+    out_x[k] = bx;
+    out_y[k] = by;
+    if (out_val) out_val[k] = best;
+  }
+  free(val);
+  free(col);
+  free(rowm);
+  return 0;
 }
