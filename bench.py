@@ -16,8 +16,9 @@ Prints ONE JSON line (rank 0).  Keys follow the driver's contract:
              against the measured HBM copy bandwidth of MEASURED_PEAKS.json
   cpu_baseline  the fp64 oracle (oracle/, as it stands) timed on this box's host cores
 With --impl reference the oracle itself is the timed arm (host cores, no GPU work).
-Under torchrun (N > 1) every rank processes its own independent stack (weak scaling, no data-path
-collective: tiles and fields are independent).
+N > 1 (under torchrun, or started by this script when it is not): --scaling weak (default) gives every rank its own
+independent stack (no data-path collective: tiles and fields are independent); --scaling strong
+cuts ONE stack into row shards (one all-gather of the method's global scalars over NCCL).
 """
 from __future__ import annotations
 
@@ -37,7 +38,9 @@ UNIT = "Mpix/s"
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE fused-kernel launch on the default workload, from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture has been taken for this build)
-NCU_TRAFFIC_BYTES = {"meerkat": 1091050016}  # profiles/r01_e_final.md: 1 083 252 000 read + 7 798 016 written
+# (keyed to the build: `srchash` is paper_2509_21754_b200.build.source_hash() of the build the capture was taken on;
+# any other build prints "traffic": null)
+NCU_TRAFFIC = {"srchash": None, "meerkat": None}
 
 
 def parse_args():
@@ -54,6 +57,9 @@ def parse_args():
     ap.add_argument("--channels", type=int, default=0, help="imgfreq only: use the first N of the 16 channels")
     ap.add_argument("--tile", type=int, default=32, help="N_T (the paper's default and BASELINE.json's is 32)")
     ap.add_argument("--harmonics", type=int, default=1, help="frequency branch: harmonic summing over 1,2,4..H harmonics")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = an independent stack per rank; strong = ONE stack cut into row shards (ShardedContext)")
+    ap.add_argument("--no-pipeline", action="store_true", help="end every step with a synchronous fitrig_detect")
     return ap.parse_args()
 
 
@@ -220,6 +226,25 @@ def measure_h2d_gbs(torch, nbytes=1 << 30, reps=10):
     return best
 
 
+def timed(torch, stream, fn, barrier):
+    """CUDA-event time (ms) of fn() on `stream`, bracketed by barrier + synchronize on both sides."""
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    fn()
+    e1.record(stream)
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def ncu_traffic(workload):
+    """dram bytes of one fused-kernel launch from the committed ncu capture -- only if it was taken on THIS build."""
+    from paper_2509_21754_b200 import build as lib_build
+    if NCU_TRAFFIC.get("srchash") != lib_build.source_hash() or TILE != 32:
+        return None
+    return NCU_TRAFFIC.get(workload)
+
+
 def run_fitrig(args, cfg, tau, branch):
     import numpy as np
     import torch
@@ -230,13 +255,17 @@ def run_fitrig(args, cfg, tau, branch):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise RuntimeError(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch through bench.py itself or torchrun with matching counts")
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
     torch.cuda.set_device(local)
     dist = None
+    backend = None
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        backend = f"{dist.get_backend()} (NCCL {'.'.join(map(str, torch.cuda.nccl.version()))})"
 
     def barrier():
         if dist is not None:
@@ -244,157 +273,220 @@ def run_fitrig(args, cfg, tau, branch):
         torch.cuda.synchronize()
 
     dev = f"cuda:{local}"
-    # every rank owns an independent stack (different noise and field per rank): weak scaling
-    # config 5 (R19): the 16 frequency channels are a batch of independent stacks, all resident (34 GB)
+    strong = args.scaling == "strong" and world > 1
     n_ch = cfg.n_channels if not args.channels else min(args.channels, cfg.n_channels)
-    rcfg = cfg if world == 1 else cfg.replace(cfg_index=cfg.cfg_index + 100 * rank)
-    stacks = [synth.make_stack(rcfg, device=dev, channel=ch)[0] for ch in range(n_ch)]
-    stack = stacks[0]
-    L, H, W = stack.shape
-    pix = L * H * W * n_ch
-    ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS)
-    U, Ty, Tx = ctx.map_dims()
-    d_tl = torch.empty((U, Ty, Tx), dtype=torch.float32, device=dev)
-    cap = 1 << 16
-    out = np.zeros(cap, dtype=fitrig.binding.CANDIDATE_DTYPE)
-    stream = torch.cuda.current_stream()
-
-    def step():
-        n_tot = 0
-        for st_c in stacks:
-            ctx.tlisi(st_c, d_tl, stream)
-            c_, n_ = ctx.detect(tau, cap, stream, out=out)
-            n_tot += n_
-        return c_, n_tot
-
     sampler = ClockSampler(local)
-    for _ in range(max(args.warmup, 3)):
-        cands, n_found = step()
-    ctx.profile(True)
-    barrier()
-    l0 = ctx.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.start()
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    barrier()
-    sampler.stop()
-    launches = ctx.launch_count() - l0
-    ms = e0.elapsed_time(e1)
-    # CUDA events the library recorded around its own launches, on the launching stream, during the timed region
-    main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
-    ctx.profile(False)
-    ms_max = shard.max_over_ranks(ms, dev)  # device time of the slowest rank
-    value = world * pix * args.steps / (ms_max * 1e-3) / 1e6
+    stream = torch.cuda.current_stream()
+    cap = 1 << 16
+    outs = [np.zeros(cap, dtype=fitrig.binding.CANDIDATE_DTYPE) for _ in range(2)]
+    num_sms = torch.cuda.get_device_properties(local).multi_processor_count
 
-    # ---- roofline of the dominant (fused) kernel ----
-    plan = fitrig.plan_query(H, W, L, num_sms=torch.cuda.get_device_properties(local).multi_processor_count, tile=TILE)
-    # one launch = one channel's stack: every snapshot pixel read once + one 16-byte record per tile and unit
-    alg_bytes = 4 * (pix // n_ch) + 16 * U * Ty * Tx
-    traffic = NCU_TRAFFIC_BYTES.get(cfg.name) if TILE == 32 else None
+    if strong:
+        # ---- ONE image stack cut into row shards: every rank reads only its rows of every snapshot;
+        # one all-gather of 2 + 2U doubles (and 3 more in the frequency branch), then local detection and a gather
+        # of the candidate lists.  Every rank draws the same stack (same seed) and keeps its own rows.
+        full = synth.make_stack(cfg, device=dev, channel=0)[0]
+        L, H, W = full.shape
+        sc = shard.ShardedContext(H, W, L, rank, world, device=local, branch=branch, tile=TILE, harmonics=HARMONICS)
+        rows = full[:, sc.r0:sc.r1].contiguous()
+        del full
+        torch.cuda.empty_cache()
+        pix = L * H * W  # the whole job
+        ctx = sc.ctx
+        U, Ty, Tx = ctx.map_dims()
+
+        def step():
+            sc.tlisi(rows, None, stream)
+            c_, n_ = sc.detect(tau, cap, stream)
+            return sc.gather(c_, dev)
+
+        for _ in range(max(args.warmup, 3)):
+            merged = step()
+        l0 = ctx.launch_count()
+        sampler.start()
+        ms = timed(torch, stream, lambda: [step() for _ in range(args.steps)], barrier)
+        sampler.stop()
+        launches = ctx.launch_count() - l0
+        ms_max = shard.max_over_ranks(ms, dev)
+        n_found = len(merged)
+        ctx.profile(True)
+        timed(torch, stream, lambda: [step() for _ in range(args.steps)], barrier)
+        main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
+        ctx.profile(False)
+        my_pix = L * (sc.r1 - sc.r0) * W
+        alg_bytes = 4 * my_pix + 16 * U * Ty * Tx
+        ms_sync = ms_max
+        e2e = None
+        cpu = None
+        stacks = None
+    else:
+        # ---- every rank owns independent stacks (different noise and field per rank): weak scaling, no data-path
+        # collective.  config 5 (R19): the 16 frequency channels are a batch of independent stacks, all resident (34 GB)
+        rcfg = cfg if world == 1 else cfg.replace(cfg_index=cfg.cfg_index + 100 * rank)
+        stacks = [synth.make_stack(rcfg, device=dev, channel=ch)[0] for ch in range(n_ch)]
+        L, H, W = stacks[0].shape
+        pix = L * H * W * n_ch * world
+        my_pix = L * H * W
+        ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS, batch=n_ch)
+        U, Ty, Tx = ctx.map_dims()
+        d_tl = torch.empty((n_ch, U, Ty, Tx), dtype=torch.float32, device=dev)
+
+        def step_sync():
+            ctx.tlisi_batch(stacks, d_tl, stream)
+            return ctx.detect_batch(tau, cap, stream, out=outs[0])
+
+        def pipelined(k):
+            """K steps; the candidate list of step i is fetched after step i + 1 has been queued (two result slots),
+            so the device never waits for the host.  Every step's map and list is produced and delivered."""
+            res = None
+            for i in range(k):
+                ctx.tlisi_batch(stacks, d_tl, stream)
+                ctx.detect_launch(tau, cap, stream)
+                if i > 0:
+                    res = ctx.detect_fetch(outs[(i - 1) & 1])
+            return ctx.detect_fetch(outs[(k - 1) & 1])
+
+        for _ in range(max(args.warmup, 3)):
+            cands, n_found, per_stack = step_sync()
+        pipelined(2)
+        l0 = ctx.launch_count()
+        sampler.start()
+        if args.no_pipeline:
+            ms = timed(torch, stream, lambda: [step_sync() for _ in range(args.steps)], barrier)
+        else:
+            ms = timed(torch, stream, lambda: pipelined(args.steps), barrier)
+        sampler.stop()
+        launches = ctx.launch_count() - l0
+        ms_max = shard.max_over_ranks(ms, dev)
+        # the same steps, each ended by its own synchronous fitrig_detect (host round trip inside every step)
+        ms_sync = shard.max_over_ranks(timed(torch, stream, lambda: [step_sync() for _ in range(args.steps)], barrier), dev)
+        # the same steps once more with the library's CUDA events around its own launches (on the launching stream)
+        ctx.profile(True)
+        timed(torch, stream, lambda: [step_sync() for _ in range(args.steps)], barrier)
+        main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
+        ctx.profile(False)
+        alg_bytes = 4 * my_pix + 16 * U * Ty * Tx  # one launch = one stack: every pixel once + one record per tile and unit
+
+    value = pix * args.steps / (ms_max * 1e-3) / 1e6
+
+    # ---- roofline of the dominant (fused) kernel, and of the whole step ----
+    plan = fitrig.plan_query(H if not strong else sc.r1 - sc.r0, W, L, num_sms=num_sms, tile=TILE)
     k_ms = main_tot / max(main_n, 1)
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
+    read_peak = ctx.probe_read_bandwidth(stacks[0] if stacks else rows) if rank == 0 else None
+    launches_per_step = n_ch if not strong else 1
+    step_bytes = alg_bytes * launches_per_step + 8 * n_ch * U * Ty * Tx  # + q and tLISI written by the finalise
+    step_ms = ms_max / args.steps
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": "tlisi_fused_kernel" if plan.path == 0 else
+                "traffic": ncu_traffic(cfg.name), "kernel": "tlisi_fused_kernel" if plan.path == 0 else
                 "tlisi_generic_kernel", "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
-                "finalize_ms": fin_tot / max(fin_n, 1), "kernel_launches_timed": main_n, "kernel_share_of_step": k_ms * n_ch * args.steps / ms}
+                "read_only_peak": read_peak, "frac_of_read_only_peak": (achieved / read_peak) if read_peak else None,
+                "read_only_peak_source": "fitrig_probe_read_bandwidth: plain float4 grid-stride read of the same stack, best of 5, this run",
+                "finalize_ms": fin_tot / max(fin_n, 1), "kernel_launches_timed": main_n,
+                "kernel_share_of_step": k_ms * launches_per_step / step_ms,
+                "step_achieved": step_bytes / (step_ms * 1e-3) / 1e9, "step_frac": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
+                "step_bytes": step_bytes,
+                "step_frac_sync": step_bytes / (ms_sync / args.steps * 1e-3) / 1e9 / peak}
 
     # ---- end to end: host (pinned) snapshots -> fitrig_stream -> fitrig_detect -> host results ----
-    e2e = None
-    if not args.no_e2e:
+    if not strong:
+        e2e = None
+    if not strong and not args.no_e2e:
         h2d_gbs = measure_h2d_gbs(torch) if rank == 0 else None
+        ectx = ctx if n_ch == 1 else fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS)
         hosts = []
         for st_c in stacks:
             host = torch.empty((L, H, W), dtype=torch.float32).pin_memory()
             host.copy_(st_c)
             hosts.append([host[s] for s in range(L)])
         h_tl = torch.empty((U, Ty, Tx), dtype=torch.float32).pin_memory()
-        ksteps = args.e2e_steps or max(3, min(args.steps, int(20e9 // (4 * pix)) or 1))
+        ksteps = args.e2e_steps or max(3, min(args.steps, int(20e9 // (4 * pix // world)) or 1))
 
         def e2e_step():
             n_tot = 0
             for snaps in hosts:
-                ctx.stream(snaps, h_tl, stream)
-                c_, n_ = ctx.detect(tau, cap, stream, out=out)
+                ectx.stream(snaps, h_tl, stream)
+                c_, n_ = ectx.detect(tau, cap, stream, out=outs[0])
                 n_tot += n_
             return c_, n_tot
 
         for _ in range(2):
             c2, n2 = e2e_step()
-        barrier()
         sampler.start()
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        f0.record(stream)
-        for _ in range(ksteps):
-            c2, n2 = e2e_step()
-        f1.record(stream)
-        barrier()
+        e_ms = timed(torch, stream, lambda: [e2e_step() for _ in range(ksteps)], barrier)
         sampler.stop()
-        e_ms = shard.max_over_ranks(f0.elapsed_time(f1), dev) / ksteps
+        c2, n2 = e2e_step()
+        e_ms = shard.max_over_ranks(e_ms, dev) / ksteps
         assert n2 == n_found, "streamed and resident paths disagree on the candidate count"
-        e2e = {"value": world * pix / (e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * pix,
+        e2e = {"value": pix / (e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * pix // world,
                "d2h_bytes_per_step": n_ch * (4 * U * Ty * Tx + 16) + 16 * int(min(n_found, 4096 * n_ch)), "ms_per_step": e_ms,
                "steps": ksteps, "api": "fitrig_stream + fitrig_detect (pinned host snapshots, row strips)",
-               "roofline": {"bound": "pcie", "achieved": 4 * pix / (e_ms * 1e-3) / 1e9, "peak": h2d_gbs,
-                            "unit": "GB/s", "frac": (4 * pix / (e_ms * 1e-3) / 1e9 / h2d_gbs) if h2d_gbs else None,
+               "roofline": {"bound": "pcie", "achieved": 4 * pix / world / (e_ms * 1e-3) / 1e9, "peak": h2d_gbs,
+                            "unit": "GB/s", "frac": (4 * pix / world / (e_ms * 1e-3) / 1e9 / h2d_gbs) if h2d_gbs else None,
                             "peak_source": "pinned 1 GiB cudaMemcpyAsync H2D, best of 10, this run"}}
         # ---- real-time leg: fitrig_push, one snapshot per call from pinned host memory (Fig. 14 timeline) ----
-        if branch == 0:
-            pctx = fitrig.Context(H, W, 3, device=local, tile=TILE)
-            snaps0 = hosts[0]
+        window = 3 if branch == 0 else min(L, 18)
+        pctx = fitrig.Context(H, W, window, device=local, tile=TILE, branch=branch, harmonics=HARMONICS)
+        snaps0 = hosts[0]
 
-            def push_pass():
-                tot = 0
-                for s_ in snaps0 + [None]:
-                    u_, c_, n_ = pctx.push(s_, tau, None, cap, stream, out=out)
-                    tot += n_
-                pctx.push_reset()
-                return tot
+        def push_pass():
+            tot = 0
+            for s_ in snaps0 + [None]:
+                u_, c_, n_ = pctx.push(s_, tau, None, cap, stream, out=outs[0])
+                tot += n_
+            pctx.push_reset()
+            return tot
 
-            push_pass()
-            barrier()
-            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            g0.record(stream)
-            t_wall = time.perf_counter()
-            n_rt = push_pass()
-            g1.record(stream)
-            barrier()
-            p_ms = shard.max_over_ranks((time.perf_counter() - t_wall) * 1e3, dev)
-            e2e["realtime"] = {"value": world * L * H * W / (p_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_snapshot": p_ms / L,
-                               "api": "fitrig_push (one pinned host snapshot per call, running M, candidates per unit)",
-                               "candidates": int(n_rt), "h2d_gbs": 4 * L * H * W / (p_ms * 1e-3) / 1e9,
-                               "timer": "host wall clock around the pass (every push synchronises)"}
-            pctx.close()
+        push_pass()
+        barrier()
+        t_wall = time.perf_counter()
+        n_rt = push_pass()
+        barrier()
+        p_ms = shard.max_over_ranks((time.perf_counter() - t_wall) * 1e3, dev)
+        e2e["realtime"] = {"value": world * L * H * W / (p_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_snapshot": p_ms / L,
+                           "api": "fitrig_push (one pinned host snapshot per call, running M, candidates per unit"
+                                  + (f"; frequency branch: Eq. 10-12 over the cube of the last {window - 2} units" if branch else "") + ")",
+                           "candidates": int(n_rt), "h2d_gbs": 4 * L * H * W / (p_ms * 1e-3) / 1e9,
+                           "timer": "host wall clock around the pass (every push synchronises)"}
+        pctx.close()
+        if ectx is not ctx:
+            ectx.close()
         del hosts
 
     # ---- the oracle beside it (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
-        snaps_np = [stack[s].cpu().numpy() for s in range(L)]
-        rows = choose_sample_rows(snaps_np, tau, branch, budget_s=12.0, passes=1)
+        snaps_np = [stacks[0][s].cpu().numpy() for s in range(L)]
+        rows_s = choose_sample_rows(snaps_np, tau, branch, budget_s=12.0, passes=1)
         npass, t_cpu = 0, 0.0
         while t_cpu < 12.0 and npass < 1000:  # about 12 s of CPU work: repeat the pass when one is shorter
-            t_cpu += oracle_sample_rate(snaps_np, rows, tau, branch)
+            t_cpu += oracle_sample_rate(snaps_np, rows_s, tau, branch)
             npass += 1
-        cpu = {"value": npass * L * rows * W / t_cpu / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{npass} passes over the first {rows} of {H} rows of all {L} snapshots"
+        cpu = {"value": npass * L * rows_s * W / t_cpu / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{npass} passes over the first {rows_s} of {H} rows of all {L} snapshots"
                          f"{' of channel 0' if n_ch > 1 else ''} ({t_cpu:.1f} s in total)"}
 
     if rank == 0:
+        from paper_2509_21754_b200 import build as lib_build
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "warmup": max(args.warmup, 3), "ms_per_step": step_ms, "higher_is_better": True,
+            "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_desc(cfg, tau, branch, n_ch), "tile": TILE, "tau": tau, "harmonics": HARMONICS,
                        "candidates_per_step": int(n_found),
-                       "l2": f"input {4 * pix / 1e6:.0f} MB per step vs 126 MB L2: "
-                             + ("larger than L2, no flush" if 4 * pix > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
+                       "step": ("one image cut into row shards: fitrig_tlisi on the shard + all-gather of 2+2U doubles + "
+                                "fitrig_shard_import + fitrig_detect + candidate gather, every step synchronous") if strong else
+                               ("fitrig_tlisi_batch + fitrig_detect (synchronous, one host round trip per step)" if args.no_pipeline else
+                                "fitrig_tlisi_batch + fitrig_detect_launch; fitrig_detect_fetch of step i after step i+1 was queued "
+                                "(two result slots; every step's map and candidate list is produced and delivered inside the timed region)"),
+                       "ms_per_step_sync": ms_sync / args.steps,
+                       "l2": f"input {4 * pix // world / 1e6:.0f} MB per step vs 126 MB L2: "
+                             + ("larger than L2, no flush" if 4 * pix // world > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
                        "plan": {"path": "fused-tma" if plan.path == 0 else "generic", "units_per_cta": plan.units_per_cta, "box_tiles": plan.box_tiles,
-                                "warps_per_cta": plan.warps_per_cta, "stages": plan.stages, "grid": plan.grid}},
+                                "warps_per_cta": plan.warps_per_cta, "stages": plan.stages, "grid": plan.grid},
+                       "build": lib_build.source_hash()[:16], "dist_backend": backend},
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches) * world,
             "roofline": roofline, "cpu_baseline": cpu,
         }
@@ -402,6 +494,18 @@ def run_fitrig(args, cfg, tau, branch):
     ctx.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 and no torchrun around it: start the N ranks ourselves."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.exit(subprocess.call(cmd))
 
 
 def main():
@@ -414,6 +518,8 @@ def main():
     branch = 1 if args.workload in ("imgfreq", "psr_like") else 0
     if args.impl == "reference":
         run_reference(args, cfg, tau, branch)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_under_torchrun(args)
     else:
         run_fitrig(args, cfg, tau, branch)
 

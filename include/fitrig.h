@@ -26,6 +26,17 @@
  *     FITRIG_ERR_CUDA.
  *   - Pointers are marked (device) or (host).  Nothing here is a torch type; a CUDA stream is
  *     passed as void* (cudaStream_t; NULL = the legacy default stream).
+ *   - Environment: the library reads these integer DEBUG / TUNING switches, once per fitrig_create (and once per
+ *     fitrig_plan_query) call, never later; unset or 0 = the default behaviour.  They change how the work is cut and
+ *     launched, never a result (the parity tests run every one of them against the same expected maps):
+ *       FITRIG_BOX_TILES=n       fused kernel: n adjacent 32x32 pixel blocks per TMA box (1..8) instead of the planned width
+ *       FITRIG_STAGES=n          fused kernel: ring of n boxes per CTA
+ *       FITRIG_GRID=n            fused kernel: n CTAs instead of one per SM
+ *       FITRIG_EVICT_FIRST=1     fused kernel: L2 evict_first hint on the streaming loads
+ *       FITRIG_FORCE_GENERIC=1   take the generic kernel even where the fused TMA kernel applies
+ *       FITRIG_OLD_GENERIC=1     generic path: the three-reads-per-pixel kernel instead of the time-marching one
+ *       FITRIG_NO_PITCHED_COPY=1 fitrig_stream: one copy per snapshot and strip instead of one pitched copy per strip
+ *       FITRIG_NO_PDL=1          plain stream-ordered launches instead of programmatic dependent launches
  */
 #ifndef FITRIG_H_
 #define FITRIG_H_
@@ -73,7 +84,11 @@ typedef struct {
                       /* non-overlapping tiles.  stride < tile: OVERLAPPING windows of tile pixels     */
                       /* every stride pixels (an extension, R27); Ty = max(1, ceil(H/stride) - tile/stride + 1);     */
                       /* image branch only, no accumulation, no row shards; candidate (x, y) stays the peak pixel    */
-  int32_t reserved[5];
+  int32_t batch;      /* B >= 1; 0 -> 1.  B independent stacks of the same shape per call (e.g. the 16 frequency channels of  */
+                      /* BASELINE.json configs[4], R19): maps are [B][U][Ty][Tx], statistics and M are per stack, and one    */
+                      /* fitrig_detect returns all B candidate lists back to back.  Not with row shards, fitrig_stream,     */
+                      /* fitrig_push or overlapping windows                                                               */
+  int32_t reserved[4];
 } fitrig_params;
 
 /* One candidate, 16 bytes.
@@ -135,6 +150,13 @@ int fitrig_map_dims(const fitrig_ctx* ctx, int32_t* units, int32_t* Ty, int32_t*
  * Errors: INVALID_ARG (NULL stack), CUDA. */
 int fitrig_tlisi(fitrig_ctx* ctx, const float* d_stack, float* d_tlisi, void* cuda_stream);
 
+/* fitrig_tlisi_batch -- fitrig_tlisi for a context created with params.batch = B > 1 (or 1):
+ *   d_stacks (host)   array of B device pointers, each one stack [L][H][W] fp32 as for fitrig_tlisi.
+ *   d_tlisi (device)  [B][U][Ty][Tx] or NULL.
+ * The B stacks are independent problems (own M, own statistics); the B tLISI kernels run back to back and ONE finalise
+ * launch serves all of them.  fitrig_tlisi on such a context reads d_stack as [B][L][H][W].  Errors as fitrig_tlisi. */
+int fitrig_tlisi_batch(fitrig_ctx* ctx, const float* const* d_stacks, float* d_tlisi, void* cuda_stream);
+
 /* fitrig_detect -- threshold the current map at z > sigma_threshold (strict, R6) and return the
  * compacted candidate list (Eq. 9, or Eq. 10-12 when params.branch = FREQUENCY).
  *   h_out (host)      room for `capacity` candidates, sorted ascending by (snapshot-or-unit,
@@ -145,6 +167,24 @@ int fitrig_tlisi(fitrig_ctx* ctx, const float* d_stack, float* d_tlisi, void* cu
  * `cuda_stream` once.  Errors: STATE (no current map), INVALID_ARG, CAPACITY, CUDA. */
 int fitrig_detect(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate* h_out, int64_t capacity,
                   int64_t* n_found, void* cuda_stream);
+
+/* fitrig_detect_batch -- fitrig_detect that also reports how the list divides among the B stacks of the context:
+ * h_out holds the candidates of stack 0, then stack 1, ... (each in the order above); n_found_per_stack (host, B
+ * entries) receives each stack's total, *n_found their sum.  One compaction launch and one synchronisation for all
+ * B stacks. */
+int fitrig_detect_batch(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate* h_out, int64_t capacity,
+                        int64_t* n_found, int64_t* n_found_per_stack, void* cuda_stream);
+
+/* fitrig_detect_launch / fitrig_detect_fetch -- fitrig_detect in two halves, for pipelines that keep the device busy
+ * while the host reads results: launch enqueues the compaction of the current map on cuda_stream and returns at once;
+ * fetch waits for the OLDEST launch that has not been fetched (only for it: work queued behind it keeps running) and
+ * delivers its list exactly as fitrig_detect would (h_out needs the capacity given to that launch).  Results live in
+ * two slots, so at most two launches may be in flight (a third: FITRIG_ERR_STATE):
+ *     tlisi(A); launch;  tlisi(B); launch;  fetch -> A's candidates;  tlisi(C); launch;  fetch -> B's; ...
+ * fitrig_detect == launch + fetch (and refuses to run while a launch is unfetched).  n_found_per_stack (host, B
+ * entries) may be NULL. */
+int fitrig_detect_launch(fitrig_ctx* ctx, float sigma_threshold, int64_t capacity, void* cuda_stream);
+int fitrig_detect_fetch(fitrig_ctx* ctx, fitrig_candidate* h_out, int64_t* n_found, int64_t* n_found_per_stack);
 
 /* fitrig_stream -- same result as fitrig_tlisi for snapshots that live in HOST memory
  * (Fig. 14: transfers overlapped with the trigger kernels; here at row-strip
@@ -158,8 +198,12 @@ int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tli
 
 /* Real-time mode ("for real-time processing, this maximum can be estimated from at least
  * three past snapshots"; timeline of Fig. 14: while the n-th tLISI is computed the
- * (n+3)-th snapshot is loaded).  The context must have been created with n_snapshots = 3 (one unit per
- * push, maps are [1][Ty][Tx]), image branch.
+ * (n+3)-th snapshot is loaded).  Image branch: the context must have been created with n_snapshots = 3 (one unit
+ * per push, maps are [1][Ty][Tx]).  Frequency branch (the image-frequency FITrig IS this streamed
+ * computation; reading R29): a context created with n_snapshots = L_w keeps the tLISI cube of the LAST U = L_w - 2
+ * units as a ring (map row n mod U holds unit n), every matrix normalised by the running maximum, and once U units
+ * exist each push runs Eq. 10-12 over that cube: candidates as for fitrig_detect in the frequency branch
+ * (snapshot = k*); before that n_found = 0.  |F_k| does not depend on where the ring starts.
  *
  * fitrig_push -- feed ONE new H x W snapshot (host, pinned for overlap, or device; NULL to flush) and get
  * the result of the unit whose three snapshots had been pushed BEFORE this call:
@@ -168,13 +212,13 @@ int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tli
  *     `cuda_stream`: steps a1-a8 with M_n = max(largest pixel of x_0 .. x_{n+2}, C), the running maximum
  *     of everything seen so far (z and therefore the candidates do not depend on M).
  *   *unit (host)    index n of the unit computed by this call, or -1 (the first three pushes; or nothing left)
- *   d_tlisi (device) [Ty][Tx] tLISI of that unit, may be NULL
+ *   d_tlisi (device) [Ty][Tx] tLISI of that unit (the newest matrix of the cube), may be NULL
  *   h_out, capacity, n_found  as fitrig_detect; candidate.snapshot = n
  * So push(x_0), push(x_1), push(x_2) return unit = -1; push(x_3) returns unit 0; ...; push(NULL) returns
  * the last unit.  After a call with unit >= 0 the context's current map is that unit's (getters work).
  * The copy is asynchronous: a pushed buffer must stay valid and unchanged until the NEXT fitrig_push that
  * returns a unit >= 0 has returned (or until fitrig_push_reset).  Synchronises `cuda_stream` when a unit
- * is computed.  Errors: INVALID_ARG (context not created with 3 snapshots / frequency branch),
+ * is computed.  Errors: INVALID_ARG (image branch without n_snapshots = 3; accumulation; batch; tiles of 64, 96 ..),
  * NOMEM, CUDA, CAPACITY.
  *
  * fitrig_push_reset -- forget all pushed snapshots and the running maximum (synchronises the device). */
@@ -210,18 +254,31 @@ int fitrig_shard_export(fitrig_ctx* ctx, double* d_out, void* cuda_stream);
  * whole-image fitrig_tlisi.  Asynchronous.  Errors: STATE, INVALID_ARG (NULL, world < 1), CUDA. */
 int fitrig_shard_import(fitrig_ctx* ctx, const double* d_all, int32_t world, float* d_tlisi, void* cuda_stream);
 
-/* fitrig_get_stats -- M and the per-unit mean / population std of q = 1 - tLISI
- * (Eq. 8; mu_tLISI = 1 - mu_q).  Frequency branch after fitrig_detect: mu[0], sigma[0] describe
- * eta (Eq. 11) instead.  Host outputs, each may be NULL; mu, sigma need U doubles.  Synchronises. */
+/* Row shards, frequency branch: eta (Eq. 10) scales with 1 / M^2, so it can only be formed after the first exchange,
+ * and the z-score of Eq. 11 runs over the eta of ALL tiles of the image: a second, 3-double exchange.
+ *     ... fitrig_shard_import as above ...
+ *     fitrig_shard_export_eta -> w[3]           eta and k* of this shard's tiles; w = (tiles, mean eta, sum (eta - mean)^2)
+ *     all-gather w over the shards
+ *     fitrig_shard_import_eta(all w, world)     global mean and population std of eta (Chan's merge in shard order)
+ *     fitrig_detect                             Eq. 12 on this shard's tiles
+ * Both are asynchronous on cuda_stream.  Errors: STATE (no map / export_eta not called), INVALID_ARG (NULL, image
+ * branch, batch), CUDA. */
+int fitrig_shard_export_eta(fitrig_ctx* ctx, double* d_out /*device, 3 doubles*/, void* cuda_stream);
+int fitrig_shard_import_eta(fitrig_ctx* ctx, const double* d_all /*device, [world][3]*/, int32_t world, void* cuda_stream);
+
+/* fitrig_get_stats -- M (B floats) and the per-unit mean / population std of q = 1 - tLISI
+ * (Eq. 8; mu_tLISI = 1 - mu_q; B * U doubles each, row b * U + u).  Frequency branch after fitrig_detect: the
+ * first B entries of mu and sigma describe eta of each stack (Eq. 11) instead.  Host outputs, each may be NULL.
+ * Synchronises. */
 int fitrig_get_stats(const fitrig_ctx* ctx, float* M, double* mu, double* sigma);
 
 /* fitrig_get_map -- copy one of the context's maps to host memory (synchronises).
- *   which = 0: q = 1 - tLISI   [U][Ty][Tx] fp32      which = 1: tLISI        [U][Ty][Tx] fp32
- *   which = 2: eta (Eq. 10)    [Ty][Tx] fp32         which = 3: k* as fp32   [Ty][Tx]
+ *   which = 0: q = 1 - tLISI   [B][U][Ty][Tx] fp32   which = 1: tLISI        [B][U][Ty][Tx] fp32
+ *   which = 2: eta (Eq. 10)    [B][Ty][Tx] fp32      which = 3: k* as fp32   [B][Ty][Tx]
  * 2 and 3 need the frequency branch and a previous fitrig_detect. */
 int fitrig_get_map(const fitrig_ctx* ctx, int32_t which, float* h_out);
 
-/* fitrig_get_raw -- per-tile partial results of Eq. 6, each [U][Ty][Tx], host, may be
+/* fitrig_get_raw -- per-tile partial results of Eq. 6, each [B][U][Ty][Tx], host, may be
  * NULL: sum of Delta, max of Delta, sum of r, and the first max-Delta pixel as x and y (R20). */
 int fitrig_get_raw(const fitrig_ctx* ctx, float* sumD, float* maxD, float* sumR, int32_t* arg_x, int32_t* arg_y);
 
@@ -233,6 +290,12 @@ int fitrig_get_raw(const fitrig_ctx* ctx, float* sumD, float* maxD, float* sumR,
 int fitrig_profile(fitrig_ctx* ctx, int32_t enable);
 int fitrig_last_timing(const fitrig_ctx* ctx, float* main_kernel_ms, int32_t* main_kernel_launches,
                        float* finalize_ms, int32_t* finalize_launches);
+
+/* fitrig_probe_read_bandwidth -- calibration for roofline figures: the best rate (GB/s) at which a plain read-only
+ * kernel (coalesced 16-byte loads, no arithmetic to speak of) streams `bytes` bytes of d_buf (device, 16-byte
+ * aligned) in `reps` timed passes on this device.  Synchronises.  Not part of the method. */
+int fitrig_probe_read_bandwidth(fitrig_ctx* ctx, const void* d_buf, int64_t bytes, int32_t reps, float* gbs,
+                                void* cuda_stream);
 
 /* fitrig_launch_count -- kernels launched by this context since creation (for bench.py's gpu_launches). */
 int fitrig_launch_count(const fitrig_ctx* ctx, int64_t* n);

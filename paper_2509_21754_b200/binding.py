@@ -26,7 +26,7 @@ class FitrigError(RuntimeError):
 class _Params(ctypes.Structure):
     _fields_ = [("tile", ctypes.c_int32), ("C", ctypes.c_float), ("ref_mode", ctypes.c_int32),
                 ("M_override", ctypes.c_float), ("branch", ctypes.c_int32), ("strip_rows", ctypes.c_int32),
-                ("device", ctypes.c_int32), ("row_offset", ctypes.c_int32), ("accumulate", ctypes.c_int32), ("harmonics", ctypes.c_int32), ("stride", ctypes.c_int32), ("reserved", ctypes.c_int32 * 5)]
+                ("device", ctypes.c_int32), ("row_offset", ctypes.c_int32), ("accumulate", ctypes.c_int32), ("harmonics", ctypes.c_int32), ("stride", ctypes.c_int32), ("batch", ctypes.c_int32), ("reserved", ctypes.c_int32 * 4)]
 
 
 class _Candidate(ctypes.Structure):
@@ -98,7 +98,13 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_destroy.argtypes = [vp]
     L.fitrig_map_dims.argtypes = [vp, P(i32), P(i32), P(i32)]
     L.fitrig_tlisi.argtypes = [vp, vp, vp, vp]
+    L.fitrig_tlisi_batch.argtypes = [vp, P(vp), vp, vp]
     L.fitrig_detect.argtypes = [vp, f32, vp, i64, P(i64), vp]
+    L.fitrig_detect_batch.argtypes = [vp, f32, vp, i64, P(i64), vp, vp]
+    L.fitrig_detect_launch.argtypes = [vp, f32, i64, vp]
+    L.fitrig_detect_fetch.argtypes = [vp, vp, P(i64), vp]
+    L.fitrig_shard_export_eta.argtypes = [vp, vp, vp]
+    L.fitrig_shard_import_eta.argtypes = [vp, vp, i32, vp]
     L.fitrig_stream.argtypes = [vp, P(vp), vp, vp]
     L.fitrig_push.argtypes = [vp, vp, f32, vp, vp, i64, P(i64), P(i64), vp]
     L.fitrig_push_reset.argtypes = [vp]
@@ -110,9 +116,11 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_profile.argtypes = [vp, i32]
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
+    L.fitrig_probe_read_bandwidth.argtypes = [vp, vp, i64, i32, P(f32), vp]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
+              "fitrig_tlisi_batch", "fitrig_detect_batch", "fitrig_detect_launch", "fitrig_detect_fetch", "fitrig_shard_export_eta", "fitrig_shard_import_eta",
               "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
-              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count"):
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_probe_read_bandwidth"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
     L.fitrig_version.restype = ctypes.c_char_p
@@ -145,7 +153,7 @@ def _check(rc: int, allow: Tuple[int, ...] = ()) -> int:
 
 
 def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_IMAGE, strip_rows=0, device=0,
-                 row_offset=0, accumulate=0, harmonics=0, stride=0):
+                 row_offset=0, accumulate=0, harmonics=0, stride=0, batch=0):
     p = _Params()
     p.tile, p.C, p.ref_mode, p.M_override = int(tile), float(C), int(ref_mode), float(M_override)
     p.branch, p.strip_rows, p.device = int(branch), int(strip_rows), int(device)
@@ -153,6 +161,7 @@ def _make_params(tile=0, C=0.0, ref_mode=REF_ABS, M_override=0.0, branch=BRANCH_
     p.accumulate = int(accumulate)
     p.harmonics = int(harmonics)
     p.stride = int(stride)
+    p.batch = int(batch)
     return p
 
 
@@ -198,6 +207,7 @@ class Context:
         self.units, self.Ty, self.Tx = u.value, ty.value, tx.value
         self.branch = int(params.get("branch", BRANCH_IMAGE))
         self.tile = int(params.get("tile", 0)) or 32
+        self.batch = int(params.get("batch", 0)) or 1
 
     def map_dims(self) -> Tuple[int, int, int]:
         return self.units, self.Ty, self.Tx
@@ -223,6 +233,22 @@ class Context:
     def tlisi(self, d_stack, d_tlisi=None, stream=None) -> None:
         _check(self._L.fitrig_tlisi(self._h, _dev_ptr(d_stack), _dev_ptr(d_tlisi), _stream_ptr(stream)))
 
+    def tlisi_batch(self, d_stacks: Sequence, d_tlisi=None, stream=None) -> None:
+        """d_stacks: B CUDA tensors [L, H, W] (params.batch = B); d_tlisi: [B, U, Ty, Tx] or None."""
+        assert len(d_stacks) == self.batch
+        arr = (ctypes.c_void_p * self.batch)(*[_dev_ptr(t) for t in d_stacks])
+        _check(self._L.fitrig_tlisi_batch(self._h, arr, _dev_ptr(d_tlisi), _stream_ptr(stream)))
+
+    def detect_batch(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None, out: Optional[np.ndarray] = None):
+        """Returns (candidates of stack 0, then stack 1, ..; n_found; per-stack totals [B])."""
+        if out is None:
+            out = np.zeros(max(capacity, 1), dtype=CANDIDATE_DTYPE)
+        n = ctypes.c_int64(0)
+        per = np.zeros(self.batch, dtype=np.int64)
+        _check(self._L.fitrig_detect_batch(self._h, float(sigma_threshold), out.ctypes.data, int(capacity), ctypes.byref(n),
+                                           per.ctypes.data, _stream_ptr(stream)), allow=(ERR_CAPACITY,))
+        return out[: min(n.value, capacity)], n.value, per
+
     def detect(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None, out: Optional[np.ndarray] = None):
         """Returns (structured array of candidates actually written, n_found).  Raises on errors other than
         FITRIG_ERR_CAPACITY (then n_found > len(result))."""
@@ -232,6 +258,18 @@ class Context:
         _check(self._L.fitrig_detect(self._h, float(sigma_threshold), out.ctypes.data, int(capacity), ctypes.byref(n),
                                      _stream_ptr(stream)), allow=(ERR_CAPACITY,))
         return out[: min(n.value, capacity)], n.value
+
+    def detect_launch(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None) -> None:
+        """Enqueue the detection of the current map (at most two may be in flight); see detect_fetch."""
+        _check(self._L.fitrig_detect_launch(self._h, float(sigma_threshold), int(capacity), _stream_ptr(stream)))
+
+    def detect_fetch(self, out: np.ndarray):
+        """Wait for the oldest unfetched detect_launch and return (candidates, n_found, per-stack totals); `out` must
+        hold the capacity given to that launch."""
+        n = ctypes.c_int64(0)
+        per = np.zeros(self.batch, dtype=np.int64)
+        _check(self._L.fitrig_detect_fetch(self._h, out.ctypes.data, ctypes.byref(n), per.ctypes.data), allow=(ERR_CAPACITY,))
+        return out[: min(n.value, len(out))], n.value, per
 
     def stream(self, h_snapshots: Sequence, h_tlisi=None, stream=None) -> None:
         """h_snapshots: L host tensors/arrays of [H, W] fp32 (pinned for overlap)."""
@@ -277,22 +315,41 @@ class Context:
         _check(self._L.fitrig_shard_import(self._h, d_all.data_ptr(), int(world), _dev_ptr(d_tlisi),
                                            _stream_ptr(stream)))
 
+    def shard_export_eta(self, d_out, stream=None) -> None:
+        """d_out: CUDA float64 tensor of 3 elements (frequency branch, after shard_import)."""
+        assert d_out.is_cuda and d_out.is_contiguous() and str(d_out.dtype) == "torch.float64" and d_out.numel() >= 3
+        _check(self._L.fitrig_shard_export_eta(self._h, d_out.data_ptr(), _stream_ptr(stream)))
+
+    def shard_import_eta(self, d_all, world: int, stream=None) -> None:
+        """d_all: CUDA float64 tensor [world, 3]."""
+        assert d_all.is_cuda and d_all.is_contiguous() and str(d_all.dtype) == "torch.float64"
+        assert d_all.numel() >= 3 * world
+        _check(self._L.fitrig_shard_import_eta(self._h, d_all.data_ptr(), int(world), _stream_ptr(stream)))
+
     # ---- getters ----
     def get_stats(self):
-        M = ctypes.c_float()
-        mu = np.zeros(self.units)
-        sd = np.zeros(self.units)
-        _check(self._L.fitrig_get_stats(self._h, ctypes.byref(M), mu.ctypes.data, sd.ctypes.data))
-        return M.value, mu, sd
+        """(M, mu, sigma): B = 1: M a float, mu / sigma [U]; B > 1: M [B], mu / sigma [B, U]."""
+        B = self.batch
+        M = np.zeros(B, dtype=np.float32)
+        mu = np.zeros(B * self.units)
+        sd = np.zeros(B * self.units)
+        _check(self._L.fitrig_get_stats(self._h, M.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), mu.ctypes.data,
+                                        sd.ctypes.data))
+        if B == 1:
+            return float(M[0]), mu, sd
+        return M, mu.reshape(B, self.units), sd.reshape(B, self.units)
+
+    def _bshape(self, *shape):
+        return shape if self.batch == 1 else (self.batch,) + shape
 
     def get_map(self, which: int = 0) -> np.ndarray:
-        shape = (self.units, self.Ty, self.Tx) if which in (0, 1) else (self.Ty, self.Tx)
+        shape = self._bshape(self.units, self.Ty, self.Tx) if which in (0, 1) else self._bshape(self.Ty, self.Tx)
         out = np.zeros(shape, dtype=np.float32)
         _check(self._L.fitrig_get_map(self._h, int(which), out.ctypes.data))
         return out
 
     def get_raw(self):
-        shape = (self.units, self.Ty, self.Tx)
+        shape = self._bshape(self.units, self.Ty, self.Tx)
         sd, md, sr = (np.zeros(shape, np.float32) for _ in range(3))
         ax, ay = (np.zeros(shape, np.int32) for _ in range(2))
         _check(self._L.fitrig_get_raw(self._h, sd.ctypes.data, md.ctypes.data, sr.ctypes.data, ax.ctypes.data,
@@ -307,6 +364,14 @@ class Context:
         a, n, b, m = ctypes.c_float(), ctypes.c_int32(), ctypes.c_float(), ctypes.c_int32()
         _check(self._L.fitrig_last_timing(self._h, ctypes.byref(a), ctypes.byref(n), ctypes.byref(b), ctypes.byref(m)))
         return a.value, n.value, b.value, m.value
+
+    def probe_read_bandwidth(self, d_tensor, reps: int = 5, stream=None) -> float:
+        """GB/s of a plain read-only pass over `d_tensor` (calibration for roofline fractions)."""
+        g = ctypes.c_float()
+        nbytes = d_tensor.numel() * d_tensor.element_size()
+        _check(self._L.fitrig_probe_read_bandwidth(self._h, d_tensor.data_ptr(), nbytes, int(reps), ctypes.byref(g),
+                                                   _stream_ptr(stream)))
+        return g.value
 
     def launch_count(self) -> int:
         n = ctypes.c_int64()

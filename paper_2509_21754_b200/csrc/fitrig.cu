@@ -61,14 +61,37 @@ struct CandHeader {
   unsigned long long pad;
 };
 
+struct DetectSlot {
+  unsigned char* cand_dev;       // candidates (device list)
+  long long cand_cap;
+  unsigned char* cand_host;      // pinned + mapped: CandHeader + kHostStageCands candidates, written by the kernel
+  unsigned char* cand_host_dev;  // device address of cand_host
+  unsigned long long* counts_host;  // pinned + mapped: B per-stack totals
+  unsigned long long* counts_host_dev;
+  cudaEvent_t done;              // recorded behind the compaction kernel
+  cudaStream_t stream;
+  bool pending;
+  long long cap, host_cap;       // of the launch in flight
+};
+
+struct TmapCache {  // the last TMA descriptor encoded (a resident stack is described by the same one call after call)
+  bool valid = false;
+  const float* base = nullptr;
+  long long snap_stride = 0;
+  int rows = 0, nslots = 0, box = 0;
+  CUtensorMap tm;
+};
+
 struct fitrig_ctx {
   NormParams prm;
-  int H, W, L, U, Ty, Tx;
-  long long nt, nmap;
+  Tuning tune;         // FITRIG_* environment switches as they were when the context was created
+  int H, W, L, U, Ty, Tx, B;
+  long long nt, nmap;  // tiles per map row; B * U * nt
   int num_sms;
   long long max_pitch;
   fitrig_plan plan;
   EncodeTiledFn encode;
+  TmapCache tmap;
   // map
   RawTile* raw;
   RawTile* raw_blocks;  // windows made of several cells (N_T = 32 * m, overlapping windows): one record per cell,
@@ -78,30 +101,33 @@ struct fitrig_ctx {
   int Ty32, Tx32;       // 32-pixel block grid of the fused kernel
   bool blocks_pending;  // the last tLISI launches wrote raw_blocks
   float *q, *tlisi, *M_dev;
-  unsigned* gmax_key;  // two order-preserving keys of the running global maximum, used by alternate calls:
-  int key_idx;         // the finalise kernel of one call zeroes the key of the next, so no memset sits in the stream
+  unsigned* gmax_key;  // two sets of B order-preserving keys of the running global maxima, used by alternate calls:
+  int key_idx;         // the finalise kernel of one call zeroes the keys of the next, so no memset sits in the stream
   bool keys_clean;
   StatPartial* parts;
   unsigned* counters;
   double *mu, *sigma;
-  int fin_nblk;
+  int fin_nblk, fin_grid;
+  int fin_user_row;    // -1: the caller's tLISI buffer receives the whole map; r >= 0: only map row r (real-time cube)
   // frequency branch
   float* eta;
   int* kstar;
-  float* mag;  // [U/2][nt] magnitude spectrum
-  float2* tw;
+  float* mag;  // [B][U/2][nt] magnitude spectrum
+  double2* tw;
   StatPartial* sparts;
   unsigned* scounter;
   double *smu, *ssigma;
   int spec_nblk;
   bool eta_valid;
-  // compaction
-  unsigned char* cand_dev;  // CandHeader + candidates
-  long long cand_cap;
-  unsigned* blk_counts;
+  // compaction: two result slots, so that the detection of one map can be fetched after the next map's work has
+  // been queued (fitrig_detect_launch / fitrig_detect_fetch)
+  DetectSlot slot[2];
+  unsigned long long detect_launched, detect_fetched;
+  CompactState* cstate;
+  unsigned long long* cstatus;
+  unsigned long long* batch_counts;
+  unsigned compact_epoch;
   int compact_grid_max;
-  unsigned char* cand_host;  // pinned + mapped: CandHeader + kHostStageCands candidates, written by the kernel
-  unsigned char* cand_host_dev;  // device address of cand_host
   // streaming
   float* strip_buf[kMaxStripBuffers];
   int n_strip_buf;
@@ -133,8 +159,14 @@ static void free_ctx(fitrig_ctx* c) {
   cudaFree(c->raw); cudaFree(c->raw_blocks); cudaFree(c->q); cudaFree(c->tlisi); cudaFree(c->M_dev); cudaFree(c->gmax_key);
   cudaFree(c->parts); cudaFree(c->counters); cudaFree(c->mu); cudaFree(c->sigma);
   cudaFree(c->eta); cudaFree(c->kstar); cudaFree(c->mag); cudaFree(c->tw); cudaFree(c->sparts); cudaFree(c->scounter);
-  cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cand_dev); cudaFree(c->blk_counts);
-  if (c->cand_host) cudaFreeHost(c->cand_host);
+  cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cstate); cudaFree(c->cstatus);
+  cudaFree(c->batch_counts);
+  for (DetectSlot& d : c->slot) {
+    cudaFree(d.cand_dev);
+    if (d.cand_host) cudaFreeHost(d.cand_host);
+    if (d.counts_host) cudaFreeHost(d.counts_host);
+    if (d.done) cudaEventDestroy(d.done);
+  }
   for (int i = 0; i < kMaxStripBuffers; ++i) {
     cudaFree(c->strip_buf[i]);
     if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
@@ -193,6 +225,21 @@ static void launch_fused(bool acc, int tile, dim3 grid, dim3 block, size_t smem,
   else launch_fused_t<REF, 32>(acc, grid, block, smem, st, tm, fp);
 }
 
+// A launch that may overlap its prologue with the tail of the previous kernel in the stream (programmatic dependent
+// launch); every kernel launched this way starts with pdl_wait().
+template <typename P>
+static cudaError_t launch_chain(void (*kernel)(const P), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                const P& params) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, params);
+}
+
 extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_params* params, fitrig_ctx** out) {
   if (!out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: out is NULL");
   *out = nullptr;
@@ -214,18 +261,20 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   fitrig_ctx* c = new (std::nothrow) fitrig_ctx();
   if (!c) return fail(FITRIG_ERR_NOMEM, "fitrig_create: host allocation failed");
   c->prm = np;
-  c->H = H; c->W = W; c->L = L; c->U = L / np.accumulate - 2;
+  c->tune = read_tuning_env();
+  c->H = H; c->W = W; c->L = L; c->U = L / np.accumulate - 2; c->B = np.batch;
   c->num_sms = prop.multiProcessorCount;
   c->max_pitch = (long long)prop.memPitch;
   rc = fitrig_plan_query(H, W, L, params, c->num_sms, &c->plan);
   if (rc != FITRIG_OK) { delete c; return fail(rc, "fitrig_create: plan failed"); }
   c->Ty = c->plan.Ty; c->Tx = c->plan.Tx;
   c->nt = (long long)c->Ty * c->Tx;
-  c->nmap = c->nt * c->U;
-  if (c->nmap > 0x7fffffffll) {
+  c->nmap = c->nt * c->U * c->B;
+  if (c->nmap > 0x7fffffffll || c->nt > 0x7fffffffll) {
     delete c;
     return fail(FITRIG_ERR_INVALID_ARG, "fitrig_create: map of %lld entries is too large", c->nmap);
   }
+  const long long R = (long long)c->B * c->U;  // map rows
 
 #define CTX_TRY(expr)                                                                                 \
   do {                                                                                                \
@@ -251,47 +300,62 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   c->Ty32 = (H + kFastTile - 1) / kFastTile; c->Tx32 = (W + kFastTile - 1) / kFastTile;
   c->geo = cell_geom(np.tile, np.stride);
   c->Cy = (H + c->geo.cell - 1) / c->geo.cell; c->Cx = (W + c->geo.cell - 1) / c->geo.cell;
-  if (c->geo.m > 1) CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)c->U * c->Cy * c->Cx));
+  if (c->geo.m > 1) CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)R * c->Cy * c->Cx));
   CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
   CTX_TRY(cudaMalloc(&c->tlisi, sizeof(float) * c->nmap));
-  CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float)));
-  CTX_TRY(cudaMalloc(&c->gmax_key, 2 * sizeof(unsigned)));
-  CTX_TRY(cudaMemset(c->gmax_key, 0, 2 * sizeof(unsigned)));
+  CTX_TRY(cudaMalloc(&c->M_dev, sizeof(float) * c->B));
+  CTX_TRY(cudaMalloc(&c->gmax_key, 2 * sizeof(unsigned) * c->B));
+  CTX_TRY(cudaMemset(c->gmax_key, 0, 2 * sizeof(unsigned) * c->B));
   c->keys_clean = true;
-  c->fin_nblk = (int)std::max<long long>(1, std::min<long long>(64, (c->nt + 2047) / 2048));
-  CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * c->U * c->fin_nblk));
-  CTX_TRY(cudaMalloc(&c->counters, sizeof(unsigned) * c->U));
-  CTX_TRY(cudaMemset(c->counters, 0, sizeof(unsigned) * c->U));
-  CTX_TRY(cudaMalloc(&c->mu, sizeof(double) * c->U));
-  CTX_TRY(cudaMalloc(&c->sigma, sizeof(double) * c->U));
+  c->fin_nblk = (int)((c->nt + kFinChunk - 1) / kFinChunk);
+  c->fin_grid = (int)std::max<long long>(1, std::min<long long>(R * c->fin_nblk, 8ll * c->num_sms));
+  c->fin_user_row = -1;
+  CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * R * c->fin_nblk));
+  CTX_TRY(cudaMalloc(&c->counters, sizeof(unsigned) * R));
+  CTX_TRY(cudaMemset(c->counters, 0, sizeof(unsigned) * R));
+  CTX_TRY(cudaMalloc(&c->mu, sizeof(double) * R));
+  CTX_TRY(cudaMalloc(&c->sigma, sizeof(double) * R));
   if (np.branch == FITRIG_BRANCH_FREQUENCY) {
-    CTX_TRY(cudaMalloc(&c->eta, sizeof(float) * c->nt));
-    CTX_TRY(cudaMalloc(&c->kstar, sizeof(int) * c->nt));
-    CTX_TRY(cudaMalloc(&c->mag, sizeof(float) * (size_t)std::max(1, c->U / 2) * c->nt));
-    CTX_TRY(cudaMalloc(&c->tw, sizeof(float2) * c->U));
-    std::vector<float2> tw(c->U);
+    CTX_TRY(cudaMalloc(&c->eta, sizeof(float) * c->nt * c->B));
+    CTX_TRY(cudaMalloc(&c->kstar, sizeof(int) * c->nt * c->B));
+    CTX_TRY(cudaMalloc(&c->mag, sizeof(float) * (size_t)std::max(1, c->U / 2) * c->nt * c->B));
+    CTX_TRY(cudaMalloc(&c->tw, sizeof(double2) * c->U));
+    std::vector<double2> tw(c->U);
     for (int j = 0; j < c->U; ++j) {  // exp(-2 pi i j / U), Eq. 10's Fourier kernel (R17)
       const double a = -2.0 * M_PI * (double)j / (double)c->U;
-      tw[j].x = (float)cos(a);
-      tw[j].y = (float)sin(a);
+      tw[j].x = cos(a);
+      tw[j].y = sin(a);
     }
-    CTX_TRY(cudaMemcpy(c->tw, tw.data(), sizeof(float2) * c->U, cudaMemcpyHostToDevice));
-    c->spec_nblk = (int)std::max<long long>(1, std::min<long long>(4 * c->num_sms, (c->nt + 127) / 128));
-    CTX_TRY(cudaMalloc(&c->sparts, sizeof(StatPartial) * c->spec_nblk));
-    CTX_TRY(cudaMalloc(&c->scounter, sizeof(unsigned)));
-    CTX_TRY(cudaMemset(c->scounter, 0, sizeof(unsigned)));
-    CTX_TRY(cudaMalloc(&c->smu, sizeof(double)));
-    CTX_TRY(cudaMalloc(&c->ssigma, sizeof(double)));
+    CTX_TRY(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * c->U, cudaMemcpyHostToDevice));
+    if (sizeof(double2) * c->U > 48 * 1024)
+      CTX_TRY(cudaFuncSetAttribute(dft_mag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) * c->U)));
+    c->spec_nblk = (int)((c->nt + kFinChunk - 1) / kFinChunk);
+    CTX_TRY(cudaMalloc(&c->sparts, sizeof(StatPartial) * c->spec_nblk * c->B));
+    CTX_TRY(cudaMalloc(&c->scounter, sizeof(unsigned) * c->B));
+    CTX_TRY(cudaMemset(c->scounter, 0, sizeof(unsigned) * c->B));
+    CTX_TRY(cudaMalloc(&c->smu, sizeof(double) * c->B));
+    CTX_TRY(cudaMalloc(&c->ssigma, sizeof(double) * c->B));
   }
   int occ = 0;
   CTX_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, compact_kernel, 512, 0));
   c->compact_grid_max = std::max(1, occ) * c->num_sms;
-  CTX_TRY(cudaMalloc(&c->blk_counts, sizeof(unsigned) * c->compact_grid_max));
-  c->cand_cap = kHostStageCands;
-  CTX_TRY(cudaMalloc(&c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * c->cand_cap));
-  CTX_TRY(cudaHostAlloc(&c->cand_host, sizeof(CandHeader) + sizeof(fitrig_candidate) * kHostStageCands,
-                        cudaHostAllocMapped));
-  CTX_TRY(cudaHostGetDevicePointer((void**)&c->cand_host_dev, c->cand_host, 0));
+  CTX_TRY(cudaMalloc(&c->cstate, sizeof(CompactState)));
+  CTX_TRY(cudaMemset(c->cstate, 0, sizeof(CompactState)));
+  CTX_TRY(cudaMalloc(&c->cstatus, sizeof(unsigned long long) * c->compact_grid_max));
+  CTX_TRY(cudaMemset(c->cstatus, 0, sizeof(unsigned long long) * c->compact_grid_max));
+  CTX_TRY(cudaMalloc(&c->batch_counts, sizeof(unsigned long long) * c->B));
+  CTX_TRY(cudaMemset(c->batch_counts, 0, sizeof(unsigned long long) * c->B));
+  c->compact_epoch = 0;
+  for (DetectSlot& d : c->slot) {
+    d.cand_cap = kHostStageCands;
+    CTX_TRY(cudaMalloc(&d.cand_dev, sizeof(fitrig_candidate) * d.cand_cap));
+    CTX_TRY(cudaHostAlloc(&d.cand_host, sizeof(CandHeader) + sizeof(fitrig_candidate) * kHostStageCands,
+                          cudaHostAllocMapped));
+    CTX_TRY(cudaHostGetDevicePointer((void**)&d.cand_host_dev, d.cand_host, 0));
+    CTX_TRY(cudaHostAlloc(&d.counts_host, sizeof(unsigned long long) * c->B, cudaHostAllocMapped));
+    CTX_TRY(cudaHostGetDevicePointer((void**)&d.counts_host_dev, d.counts_host, 0));
+    CTX_TRY(cudaEventCreateWithFlags(&d.done, cudaEventDisableTiming));
+  }
   if (c->plan.path == 0) {
     CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
@@ -337,7 +401,10 @@ static int prof_end(fitrig_ctx* c, cudaStream_t st) {
 // base: device pointer to snapshot 0 of those rows; snap_stride: elements between snapshots.
 struct RowsOpt {
   int z0 = 0, zmod = 0;     // real-time ring: snapshot s of the launch is slot (z0 + s) % zmod of `base`
-  unsigned* key = nullptr;  // global-maximum key to fold into (default: the key of the current call)
+  unsigned* key = nullptr;  // global-maximum key to fold into (default: the key of stack `stack` of the current call)
+  int stack = 0;            // batch entry: the records go to map rows stack * U ..
+  int units = 0;            // units computed by this launch (0: all U of the context)
+  int row0 = 0;             // ... starting at this row of the stack's U rows (the real-time cube's ring slot)
 };
 
 static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int r0,
@@ -345,47 +412,54 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   const int tile = c->geo.cell;        // what the kernels reduce: cells (the tile itself in the plain case)
   const int ty_base = r0 / tile;       // first cell row of this launch
   const bool cells = c->geo.m > 1;     // records go to raw_blocks and are merged into windows before the finalise
-  RawTile* const out_raw = cells ? c->raw_blocks : c->raw;
   const int out_Ty = cells ? c->Cy : c->Ty, out_Tx = cells ? c->Cx : c->Tx;
-  unsigned* key = opt.key ? opt.key : c->gmax_key + c->key_idx;
+  const long long first_row = (long long)opt.stack * c->U + opt.row0;
+  RawTile* const out_raw = (cells ? c->raw_blocks : c->raw) + first_row * out_Ty * out_Tx;
+  const int units = opt.units ? opt.units : c->U;
+  unsigned* key = opt.key ? opt.key : c->gmax_key + c->key_idx * c->B + opt.stack;
   const int nslots = opt.zmod ? opt.zmod : c->L;
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
   if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
   if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
-  if (pl.path == 0 && rows != c->H) plan_launch(tile, c->W, rows, c->U, c->num_sms, &pl);
+  if (pl.path == 0 && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
 
   int rc = prof_begin(c, st);
   if (rc) return rc;
   if (pl.path == 0) {
-    CUtensorMap tm;
-    const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)nslots};
-    const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
-    const cuuint32_t box[3] = {(cuuint32_t)(pl.box_tiles * kFastTile), kFastTile, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = c->encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, box, estr,
-                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    const int box = pl.box_tiles * kFastTile;
+    TmapCache& tc = c->tmap;
+    if (!(tc.valid && tc.base == base && tc.snap_stride == snap_stride && tc.rows == rows && tc.nslots == nslots && tc.box == box)) {
+      const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)nslots};
+      const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
+      const cuuint32_t bx[3] = {(cuuint32_t)box, kFastTile, 1};
+      const cuuint32_t estr[3] = {1, 1, 1};
+      CUresult r = c->encode(&tc.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, bx, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) { tc.valid = false; return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r); }
+      tc.valid = true; tc.base = base; tc.snap_stride = snap_stride; tc.rows = rows; tc.nslots = nslots; tc.box = box;
+    }
     FusedParams fp;
     fp.raw = out_raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
     fp.Tx = out_Tx; fp.Ty = out_Ty; fp.Tx32 = c->Tx32;
     fp.rows_tiles = (rows + kFastTile - 1) / kFastTile; fp.ty_base = ty_base;
-    fp.U = c->U;
+    fp.ty_end = std::min(out_Ty, ty_base + rows_tiles);
+    fp.U = units;
     fp.ntw = pl.box_tiles; fp.ngx = (fp.Tx32 + pl.box_tiles - 1) / pl.box_tiles; fp.nstage = pl.stages;
-    const long long G = (long long)fp.rows_tiles * fp.ngx * c->U;
+    const long long G = (long long)fp.rows_tiles * fp.ngx * units;
     if (G > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "fused path: too many (box, unit) pairs for one launch");
     fp.G = (int)G;
-    fp.evict_first = env_int("FITRIG_EVICT_FIRST", 0);
+    fp.evict_first = c->tune.evict_first;
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
-      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
-      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
+      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
+      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;
@@ -394,7 +468,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     if (with_max) {
       // rows of each snapshot are contiguous (full width), so one launch per snapshot covers them
       const int g = c->prm.accumulate;
-      for (int s = 0; s < c->U + 2; ++s) {  // (accumulated) images; the ring mode never accumulates
+      for (int s = 0; s < units + 2; ++s) {  // (accumulated) images; the ring mode never accumulates
         const int slot = opt.zmod ? (opt.z0 + s) % opt.zmod : s * g;
         stack_max_kernel<<<std::min(4 * c->num_sms, 1024), 256, 0, st>>>(base + (long long)slot * snap_stride,
                                                                        (long long)rows * c->W, g, snap_stride, key);
@@ -404,7 +478,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     }
     GenericParams gp;
     gp.base = base; gp.snap_stride = snap_stride; gp.rows = rows; gp.W = c->W; gp.tile = tile;
-    gp.raw = out_raw; gp.Tx = out_Tx; gp.Ty = out_Ty; gp.ty_base = ty_base; gp.rows_tiles = rows_tiles; gp.U = c->U;
+    gp.raw = out_raw; gp.Tx = out_Tx; gp.Ty = out_Ty; gp.ty_base = ty_base; gp.rows_tiles = rows_tiles; gp.U = units;
     if (cells) c->blocks_pending = true;
     int G = 1;
     const long long n_t = (long long)tile * tile;
@@ -412,7 +486,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     gp.G = G;
     gp.z0 = opt.z0; gp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; gp.acc = c->prm.accumulate;
     gp.C = c->prm.C;
-    const long long groups = (long long)rows_tiles * out_Tx * c->U;
+    const long long groups = (long long)rows_tiles * out_Tx * units;
     const long long threads = groups * G;
     const long long blocks = (threads + 255) / 256;
     if (blocks > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "generic path: too many tiles for one launch");
@@ -427,10 +501,23 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   return prof_end(c, st);
 }
 
-static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, unsigned* key = nullptr) {
+static void fill_finalize_params(fitrig_ctx* c, FinalizeParams* fp, float* d_tlisi_user, const unsigned* keys) {
+  fp->raw = c->raw; fp->q = c->q; fp->tlisi = c->tlisi; fp->tlisi_user = d_tlisi_user;
+  fp->gmax_key = keys; fp->gmax_key_next = c->gmax_key + (c->key_idx ^ 1) * c->B;
+  fp->M_out = c->M_dev; fp->M_override = c->prm.M_override; fp->C = c->prm.C;
+  fp->H = c->H; fp->W = c->W; fp->tile = c->prm.tile; fp->stride = c->prm.stride; fp->Ty = c->Ty; fp->Tx = c->Tx;
+  fp->U = c->U; fp->B = c->B;
+  fp->nblk = c->fin_nblk; fp->parts = c->parts; fp->counters = c->counters; fp->mu = c->mu; fp->sigma = c->sigma;
+  fp->shard_all = nullptr; fp->shard_world = 0;
+  fp->user_row = c->fin_user_row;
+}
+
+// keys: one global-maximum key per stack (default: the keys of the current call)
+static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, unsigned* keys = nullptr) {
+  bool chained = !c->tune.no_pdl && !c->profile;  // behind the tLISI kernel (an event record in between breaks the chain)
   if (c->raw_blocks && c->blocks_pending) {  // cell records -> window records
     MergeParams mp;
-    mp.cells = c->raw_blocks; mp.raw = c->raw; mp.U = c->U; mp.Ty = c->Ty; mp.Tx = c->Tx;
+    mp.cells = c->raw_blocks; mp.raw = c->raw; mp.U = c->U * c->B; mp.Ty = c->Ty; mp.Tx = c->Tx;
     mp.Cy = c->Cy; mp.Cx = c->Cx; mp.m = c->geo.m; mp.step = c->geo.step; mp.cell = c->geo.cell; mp.tile = c->prm.tile;
     const long long n = c->nmap;
     merge_cells_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4 * c->num_sms), 256, 0, st>>>(mp);
@@ -439,12 +526,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
     c->blocks_pending = false;
   }
   FinalizeParams fp;
-  fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi_user;
-  fp.gmax_key = key ? key : c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1);
-  fp.M_out = c->M_dev; fp.M_override = c->prm.M_override; fp.C = c->prm.C;
-  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.stride = c->prm.stride; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
-  fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
-  fp.shard_all = nullptr; fp.shard_world = 0;
+  fill_finalize_params(c, &fp, d_tlisi_user, keys ? keys : c->gmax_key + c->key_idx * c->B);
   if (c->profile) {
     while ((int)c->fin_pool.size() < 2 * (c->fin_used + 1)) {
       cudaEvent_t e;
@@ -453,8 +535,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
     }
     CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used], st));
   }
-  finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
-  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(launch_chain(finalize_kernel, dim3(c->fin_grid), dim3(256), 0, st, chained, fp));
   if (c->profile) { CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used + 1], st)); c->fin_used++; }
   c->launches++;
   c->have_map = true;
@@ -463,51 +544,48 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
   return FITRIG_OK;
 }
 
-extern "C" int fitrig_tlisi(fitrig_ctx* c, const float* d_stack, float* d_tlisi, void* cuda_stream) {
-  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: ctx is NULL");
-  if (!d_stack) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: d_stack is NULL");
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+static int begin_call(fitrig_ctx* c, cudaStream_t st) {
   CUDA_TRY(cudaSetDevice(c->prm.device));
-  if (!c->keys_clean) CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, 2 * sizeof(unsigned), st));  // a call failed half way
+  if (!c->keys_clean) CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, 2 * sizeof(unsigned) * c->B, st));  // a call failed half way
   c->keys_clean = false;
   c->key_idx ^= 1;
-  int rc = launch_tlisi_rows(c, d_stack, (long long)c->H * c->W, c->H, 0, true, st);
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_tlisi_batch(fitrig_ctx* c, const float* const* d_stacks, float* d_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi_batch: ctx is NULL");
+  if (!d_stacks) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi_batch: d_stacks is NULL");
+  for (int b = 0; b < c->B; ++b)
+    if (!d_stacks[b]) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi_batch: d_stacks[%d] is NULL", b);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = begin_call(c, st);
   if (rc) return rc;
+  for (int b = 0; b < c->B; ++b) {
+    RowsOpt opt;
+    opt.stack = b;
+    rc = launch_tlisi_rows(c, d_stacks[b], (long long)c->H * c->W, c->H, 0, true, st, opt);
+    if (rc) return rc;
+  }
   return launch_finalize(c, d_tlisi, st);
 }
 
-extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream) {
-  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: ctx is NULL");
-  if (!h_snapshots) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots is NULL");
-  for (int s = 0; s < c->L; ++s)
-    if (!h_snapshots[s]) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots[%d] is NULL", s);
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  CUDA_TRY(cudaSetDevice(c->prm.device));
+extern "C" int fitrig_tlisi(fitrig_ctx* c, const float* d_stack, float* d_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: ctx is NULL");
+  if (!d_stack) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_tlisi: d_stack is NULL");
+  std::vector<const float*> ptrs(c->B);
+  for (int b = 0; b < c->B; ++b) ptrs[b] = d_stack + (size_t)b * c->L * c->H * c->W;
+  return fitrig_tlisi_batch(c, ptrs.data(), d_tlisi, cuda_stream);
+}
+
+// fitrig_stream's strip loop; on an error the caller drains the copy stream
+static int stream_strips(fitrig_ctx* c, const float* const* h_snapshots, cudaStream_t st) {
   const int rows_per = c->plan.strip_rows, nstrips = c->plan.n_strips, nbuf = c->plan.n_strip_buffers;
-  if (!c->copy_stream) {
-    CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
-    c->strip_buf_elems = (long long)c->L * rows_per * c->W;
-    for (int b = 0; b < nbuf; ++b) {
-      CUDA_TRY(cudaMalloc(&c->strip_buf[b], sizeof(float) * c->strip_buf_elems));
-      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copied[b], cudaEventDisableTiming));
-      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_free[b], cudaEventDisableTiming));
-    }
-    c->n_strip_buf = nbuf;
-  }
-  if (!c->keys_clean) CUDA_TRY(cudaMemsetAsync(c->gmax_key, 0, 2 * sizeof(unsigned), st));  // a call failed half way
-  c->keys_clean = false;
-  c->key_idx ^= 1;
-  // the copy stream may not run ahead of work already queued on the caller's stream
-  CUDA_TRY(cudaEventRecord(c->ev_entry, st));
-  CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
-  for (int b = 0; b < nbuf; ++b) c->ev_free_pending[b] = false;
   const long long snap_stride = (long long)rows_per * c->W;
   // snapshots that sit at a constant distance in host memory (one [L][H][W] allocation, the usual case) let a
   // strip travel as one pitched copy instead of L small ones; pitches are limited to cudaDeviceProp::memPitch
   long long host_stride = h_snapshots[1] - h_snapshots[0];
   bool pitched = host_stride >= (long long)c->H * c->W && host_stride * 4 <= c->max_pitch && snap_stride * 4 <= c->max_pitch &&
-                 env_int("FITRIG_NO_PITCHED_COPY", 0) == 0;
+                 c->tune.no_pitched_copy == 0;
   for (int s = 2; s < c->L && pitched; ++s) pitched = (h_snapshots[s] - h_snapshots[s - 1]) == host_stride;
   for (int i = 0; i < nstrips; ++i) {
     const int b = i % nbuf;
@@ -538,95 +616,186 @@ extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, flo
     CUDA_TRY(cudaEventRecord(c->ev_free[b], st));
     c->ev_free_pending[b] = true;
   }
-  int rc = launch_finalize(c, nullptr, st);
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_stream(fitrig_ctx* c, const float* const* h_snapshots, float* h_tlisi, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: ctx is NULL");
+  if (!h_snapshots) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots is NULL");
+  if (c->B != 1) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: not with params.batch > 1");
+  for (int s = 0; s < c->L; ++s)
+    if (!h_snapshots[s]) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream: h_snapshots[%d] is NULL", s);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  const int rows_per = c->plan.strip_rows, nbuf = c->plan.n_strip_buffers;
+  if (!c->copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+  if (!c->ev_entry) CUDA_TRY(cudaEventCreateWithFlags(&c->ev_entry, cudaEventDisableTiming));
+  if (!c->n_strip_buf) {
+    c->strip_buf_elems = (long long)c->L * rows_per * c->W;
+    for (int b = 0; b < nbuf; ++b) {
+      CUDA_TRY(cudaMalloc(&c->strip_buf[b], sizeof(float) * c->strip_buf_elems));
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copied[b], cudaEventDisableTiming));
+      CUDA_TRY(cudaEventCreateWithFlags(&c->ev_free[b], cudaEventDisableTiming));
+    }
+    c->n_strip_buf = nbuf;
+  }
+  int rc = begin_call(c, st);
   if (rc) return rc;
+  // the copy stream may not run ahead of work already queued on the caller's stream
+  CUDA_TRY(cudaEventRecord(c->ev_entry, st));
+  CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_entry, 0));
+  for (int b = 0; b < nbuf; ++b) c->ev_free_pending[b] = false;
+  rc = stream_strips(c, h_snapshots, st);
+  if (rc == FITRIG_OK) rc = launch_finalize(c, nullptr, st);
+  if (rc != FITRIG_OK) {
+    // leave nothing queued behind a failed call: the copies still in flight read the caller's buffers and write the
+    // strip buffers the next call will reuse (the message of the original failure is kept)
+    (void)cudaStreamSynchronize(c->copy_stream);
+    (void)cudaStreamSynchronize(st);
+    (void)cudaGetLastError();
+    for (int b = 0; b < nbuf; ++b) c->ev_free_pending[b] = false;
+    c->have_map = false;
+    return rc;
+  }
   if (h_tlisi) CUDA_TRY(cudaMemcpyAsync(h_tlisi, c->tlisi, sizeof(float) * c->nmap, cudaMemcpyDeviceToHost, st));
   return FITRIG_OK;
 }
 
-static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
-                       void* cuda_stream, int unit_offset);
-
-extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
-                             void* cuda_stream) {
-  return detect_core(c, tau, h_out, capacity, n_found, cuda_stream, 0);
-}
+static int detect_launch_core(fitrig_ctx* c, float tau, int64_t capacity, void* cuda_stream, int unit_offset);
+static int detect_fetch_core(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_found, int64_t* n_per_stack);
 
 static int detect_core(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
-                       void* cuda_stream, int unit_offset) {
+                       int64_t* n_per_stack, void* cuda_stream, int unit_offset) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: ctx is NULL");
   if (!n_found) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: n_found is NULL");
   if (capacity < 0 || (capacity > 0 && !h_out)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: bad h_out/capacity");
+  if (c->detect_launched != c->detect_fetched)
+    return fail(FITRIG_ERR_STATE, "fitrig_detect: a fitrig_detect_launch has not been fetched yet");
+  int rc = detect_launch_core(c, tau, capacity, cuda_stream, unit_offset);
+  if (rc) return rc;
+  return detect_fetch_core(c, h_out, n_found, n_per_stack);
+}
+
+extern "C" int fitrig_detect(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
+                             void* cuda_stream) {
+  return detect_core(c, tau, h_out, capacity, n_found, nullptr, cuda_stream, 0);
+}
+
+extern "C" int fitrig_detect_batch(fitrig_ctx* c, float tau, fitrig_candidate* h_out, int64_t capacity, int64_t* n_found,
+                                   int64_t* n_found_per_stack, void* cuda_stream) {
+  if (!n_found_per_stack) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_batch: n_found_per_stack is NULL");
+  return detect_core(c, tau, h_out, capacity, n_found, n_found_per_stack, cuda_stream, 0);
+}
+
+extern "C" int fitrig_detect_launch(fitrig_ctx* c, float tau, int64_t capacity, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_launch: ctx is NULL");
+  if (capacity < 0) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_launch: capacity < 0");
+  return detect_launch_core(c, tau, capacity, cuda_stream, 0);
+}
+
+extern "C" int fitrig_detect_fetch(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_found, int64_t* n_found_per_stack) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_fetch: ctx is NULL");
+  if (!n_found) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_fetch: n_found is NULL");
+  return detect_fetch_core(c, h_out, n_found, n_found_per_stack);
+}
+
+// Eq. 10 for the current map: magnitude spectra, eta, k*, and the statistics of eta
+static int launch_spectrum(fitrig_ctx* c, cudaStream_t st, double* shard_out) {
+  const bool chained = !c->tune.no_pdl;
+  SpectrumParams sp;
+  sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = (int)c->nt; sp.U = c->U; sp.B = c->B;
+  sp.mag = c->mag; sp.harmonics = c->prm.harmonics;
+  sp.nblk = c->spec_nblk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
+  sp.shard_out = shard_out;
+  if (c->U / 2 >= 1) {
+    const dim3 grid((unsigned)((c->nt * c->B + 127) / 128), (unsigned)((c->U / 2 + kDftBins - 1) / kDftBins));
+    CUDA_TRY(launch_chain(dft_mag_kernel, grid, dim3(128), sizeof(double2) * c->U, st, chained, sp));
+    c->launches++;
+  }
+  const int grid = (int)std::min<long long>((long long)c->spec_nblk * c->B, 8ll * c->num_sms);
+  CUDA_TRY(launch_chain(spectrum_kernel, dim3(grid), dim3(256), 0, st, chained, sp));
+  c->launches++;
+  c->eta_valid = true;
+  return FITRIG_OK;
+}
+
+static int detect_launch_core(fitrig_ctx* c, float tau, int64_t capacity, void* cuda_stream, int unit_offset) {
   if (!(tau == tau)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect: sigma_threshold is NaN");
   if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_detect: no current map (call fitrig_tlisi or fitrig_stream first)");
+  if (c->detect_launched - c->detect_fetched >= 2)
+    return fail(FITRIG_ERR_STATE, "fitrig_detect_launch: two detections are in flight; fetch one first");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
   const bool freq = c->prm.branch == FITRIG_BRANCH_FREQUENCY;
   if (freq && !c->eta_valid) {
-    SpectrumParams sp;
-    sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = c->nt; sp.U = c->U;
-    sp.mag = c->mag; sp.harmonics = c->prm.harmonics;
-    sp.nblk = c->spec_nblk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
-    if (c->U / 2 >= 1) {
-      const dim3 grid((unsigned)((c->nt + 127) / 128), (unsigned)((c->U / 2 + kDftBins - 1) / kDftBins));
-      dft_mag_kernel<<<grid, 128, sizeof(float2) * c->U, st>>>(sp);
-      CUDA_TRY(cudaGetLastError());
-      c->launches++;
-    }
-    spectrum_kernel<<<c->spec_nblk, 128, 0, st>>>(sp);
-    CUDA_TRY(cudaGetLastError());
-    c->launches++;
-    c->eta_valid = true;
+    int rc = launch_spectrum(c, st, nullptr);
+    if (rc) return rc;
   }
-  const long long rows = freq ? 1 : c->U;
+  DetectSlot& d = c->slot[c->detect_launched & 1];
+  const long long rows = freq ? c->B : (long long)c->B * c->U;
   const long long N = rows * c->nt;
   const long long want = std::min<long long>(capacity, N);
-  if (want > c->cand_cap) {  // grow the device list (rare: only for very low thresholds)
+  if (want > d.cand_cap) {  // grow the device list (rare: only for very low thresholds)
     CUDA_TRY(cudaStreamSynchronize(st));
-    CUDA_TRY(cudaFree(c->cand_dev));
-    c->cand_dev = nullptr;
-    c->cand_cap = 0;
-    CUDA_TRY(cudaMalloc(&c->cand_dev, sizeof(CandHeader) + sizeof(fitrig_candidate) * want));
-    c->cand_cap = want;
+    CUDA_TRY(cudaFree(d.cand_dev));
+    d.cand_dev = nullptr;
+    d.cand_cap = 0;
+    CUDA_TRY(cudaMalloc(&d.cand_dev, sizeof(fitrig_candidate) * want));
+    d.cand_cap = want;
   }
   CompactParams cp;
   cp.v = freq ? c->eta : c->q;
   cp.raw = c->raw; cp.kstar = c->kstar;
   cp.mu = freq ? c->smu : c->mu; cp.sigma = freq ? c->ssigma : c->sigma;
-  cp.tau = tau; cp.rows = (int)rows; cp.nt = c->nt;
+  cp.tau = tau; cp.rows = (int)rows; cp.rows_per_batch = freq ? 1 : c->U; cp.nt = c->nt;
   cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.stride = c->prm.stride; cp.branch = c->prm.branch;
   cp.row_offset = c->prm.row_offset;
   cp.unit_offset = unit_offset;
-  cp.out = reinterpret_cast<fitrig_candidate*>(c->cand_dev + sizeof(CandHeader));
-  cp.cap = std::min<long long>(c->cand_cap, std::max<long long>(capacity, 0));
-  cp.total = reinterpret_cast<unsigned long long*>(c->cand_dev);
-  cp.host_total = reinterpret_cast<unsigned long long*>(c->cand_host_dev);
-  cp.host_out = reinterpret_cast<fitrig_candidate*>(c->cand_host_dev + sizeof(CandHeader));
+  cp.out = reinterpret_cast<fitrig_candidate*>(d.cand_dev);
+  cp.cap = std::min<long long>(d.cand_cap, std::max<long long>(capacity, 0));
+  cp.host_total = reinterpret_cast<unsigned long long*>(d.cand_host_dev);
+  cp.host_out = reinterpret_cast<fitrig_candidate*>(d.cand_host_dev + sizeof(CandHeader));
   cp.host_cap = std::min<long long>(cp.cap, kHostStageCands);
-  cp.blk_counts = c->blk_counts;
+  cp.batch_counts = c->batch_counts; cp.host_counts = d.counts_host_dev; cp.B = c->B;
+  cp.state = c->cstate; cp.status = c->cstatus;
+  if (++c->compact_epoch == 0) c->compact_epoch = 1;
+  cp.epoch = c->compact_epoch;
   const int threads = 512;
-  int grid = (int)std::min<long long>(c->compact_grid_max, (N + threads - 1) / threads);
+  const long long per_min = 4 * threads;  // a block is worth launching for at least this many entries
+  int grid = (int)std::min<long long>(c->compact_grid_max, (N + per_min - 1) / per_min);
   grid = std::max(grid, 1);
   cp.seg = ((N + grid - 1) / grid + threads - 1) / threads * threads;
-  void* args[] = {&cp};
-  CUDA_TRY(cudaLaunchCooperativeKernel((void*)compact_kernel, dim3(grid), dim3(threads), args, 0, st));
+  CUDA_TRY(launch_chain(compact_kernel, dim3(grid), dim3(threads), 0, st, !c->tune.no_pdl, cp));
   c->launches++;
-  // the kernel writes the count and the first kHostStageCands candidates straight into mapped pinned memory
+  CUDA_TRY(cudaEventRecord(d.done, st));
+  d.stream = st; d.pending = true; d.cap = cp.cap; d.host_cap = cp.host_cap;
+  c->detect_launched++;
+  return FITRIG_OK;
+}
+
+static int detect_fetch_core(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_found, int64_t* n_per_stack) {
+  if (c->detect_launched == c->detect_fetched) return fail(FITRIG_ERR_STATE, "fitrig_detect_fetch: nothing was launched");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  DetectSlot& d = c->slot[c->detect_fetched & 1];
+  c->detect_fetched++;
+  d.pending = false;
+  // the kernel has written the count and the first kHostStageCands candidates straight into mapped pinned memory
   // (no copy in the stream); a copy from the device list only for longer lists
-  const long long first = cp.host_cap;
-  CUDA_TRY(cudaStreamSynchronize(st));
-  const long long total = (long long)reinterpret_cast<CandHeader*>(c->cand_host)->total;
-  const long long nwrite = std::min<long long>(total, cp.cap);
-  const long long n1 = std::min(nwrite, first);
-  if (n1 > 0) memcpy(h_out, c->cand_host + sizeof(CandHeader), sizeof(fitrig_candidate) * n1);
-  if (nwrite > n1) {
-    CUDA_TRY(cudaMemcpyAsync(h_out + n1, cp.out + n1, sizeof(fitrig_candidate) * (nwrite - n1),
-                             cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
+  CUDA_TRY(cudaEventSynchronize(d.done));
+  const long long total = (long long)reinterpret_cast<CandHeader*>(d.cand_host)->total;
+  const long long nwrite = std::min<long long>(total, d.cap);
+  if (nwrite > 0 && !h_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_fetch: h_out is NULL");
+  const long long n1 = std::min(nwrite, d.host_cap);
+  if (n1 > 0) memcpy(h_out, d.cand_host + sizeof(CandHeader), sizeof(fitrig_candidate) * n1);
+  if (nwrite > n1) {  // (a later launch writes the other slot's list: this one is still intact)
+    CUDA_TRY(cudaMemcpy(h_out + n1, reinterpret_cast<fitrig_candidate*>(d.cand_dev) + n1,
+                        sizeof(fitrig_candidate) * (nwrite - n1), cudaMemcpyDeviceToHost));
   }
   *n_found = total;
-  if (total > capacity)
-    return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)capacity);
+  if (n_per_stack)
+    for (int b = 0; b < c->B; ++b) n_per_stack[b] = (int64_t)d.counts_host[b];
+  if (total > d.cap)
+    return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)d.cap);
   return FITRIG_OK;
 }
 
@@ -638,6 +807,7 @@ extern "C" int fitrig_push_reset(fitrig_ctx* c) {
   CUDA_TRY(cudaSetDevice(c->prm.device));
   CUDA_TRY(cudaDeviceSynchronize());
   if (c->push_key) CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
+  if (c->push_ring) CUDA_TRY(cudaMemset(c->raw, 0, sizeof(RawTile) * c->nmap));  // an empty cube
   c->push_count = 0;
   c->push_next = 0;
   for (int i = 0; i < kPushSlots; ++i) c->push_free_pending[i] = false;
@@ -648,10 +818,11 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
                            int64_t capacity, int64_t* n_found, int64_t* unit, void* cuda_stream) {
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: ctx is NULL");
   if (!n_found || !unit) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: n_found or unit is NULL");
-  if (c->L != 3 || c->prm.accumulate != 1)
-    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: create the context with n_snapshots = 3 (one unit per push) and no accumulation");
-  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
-    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: the real-time mode is the image branch (Eq. 8-9)");
+  const bool freq = c->prm.branch == FITRIG_BRANCH_FREQUENCY;
+  if (c->prm.accumulate != 1 || c->B != 1 || c->geo.m != 1)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: no accumulation, no batch, tiles of 1 .. 32 pixels or generic sizes");
+  if (!freq && c->L != 3)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: image branch: create the context with n_snapshots = 3 (one unit per push)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
   const long long img = (long long)c->H * c->W;
@@ -659,6 +830,7 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
     CUDA_TRY(cudaMalloc(&c->push_ring, sizeof(float) * img * kPushSlots));
     CUDA_TRY(cudaMalloc(&c->push_key, sizeof(unsigned)));
     CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
+    CUDA_TRY(cudaMemset(c->raw, 0, sizeof(RawTile) * c->nmap));
     for (int i = 0; i < kPushSlots; ++i) {
       CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_copied[i], cudaEventDisableTiming));
       CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_free[i], cudaEventDisableTiming));
@@ -686,15 +858,24 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
     for (int k = 0; k < 3; ++k) CUDA_TRY(cudaStreamWaitEvent(st, c->ev_push_copied[(n + k) % kPushSlots], 0));
     RowsOpt opt;
     opt.z0 = (int)(n % kPushSlots); opt.zmod = kPushSlots; opt.key = c->push_key;
+    opt.units = 1;
+    opt.row0 = (int)(n % c->U);  // image branch: U = 1; frequency branch: the cube is a ring of the last U tile matrices
     rc = launch_tlisi_rows(c, c->push_ring, img, c->H, 0, true, st, opt);
     if (rc) return rc;
     CUDA_TRY(cudaEventRecord(c->ev_push_free[n % kPushSlots], st));  // x_n is not needed again
     c->push_free_pending[n % kPushSlots] = true;
-    rc = launch_finalize(c, d_tlisi, st, c->push_key);  // M = running maximum over x_0 .. x_{n+2}
+    // M = running maximum over x_0 .. x_{n+2} (R24): every matrix of the cube is (re)normalised by it
+    c->fin_user_row = freq ? opt.row0 : -1;  // d_tlisi receives the newest tile matrix
+    rc = launch_finalize(c, d_tlisi, st, c->push_key);
+    c->fin_user_row = -1;
     if (rc) return rc;
     if (n + 1 > 0x7fffffffll) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: unit index overflow");
-    rc = detect_core(c, tau, h_out, capacity, n_found, cuda_stream, (int)n);
-    if (rc != FITRIG_OK && rc != FITRIG_ERR_CAPACITY) return rc;
+    if (!freq || n + 1 >= c->U) {  // frequency branch: Eq. 10-12 once the cube holds U units (R29)
+      rc = detect_core(c, tau, h_out, capacity, n_found, nullptr, cuda_stream, freq ? 0 : (int)n);
+      if (rc != FITRIG_OK && rc != FITRIG_ERR_CAPACITY) return rc;
+    } else {
+      CUDA_TRY(cudaStreamSynchronize(st));
+    }
     *unit = n;
     c->push_next = n + 1;
   }
@@ -705,40 +886,62 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
 // ---------------------------------------------------------------------------------------------
 // row shards
 // ---------------------------------------------------------------------------------------------
+static int shard_check(fitrig_ctx* c, const char* who) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "%s: ctx is NULL", who);
+  if (c->B != 1) return fail(FITRIG_ERR_INVALID_ARG, "%s: not with params.batch > 1", who);
+  if (!c->have_map) return fail(FITRIG_ERR_STATE, "%s: no current map (call fitrig_tlisi first)", who);
+  return FITRIG_OK;
+}
+
 extern "C" int fitrig_shard_export(fitrig_ctx* c, double* d_out, void* cuda_stream) {
-  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: ctx is NULL");
+  int rc = shard_check(c, "fitrig_shard_export");
+  if (rc) return rc;
   if (!d_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: d_out is NULL");
-  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
-    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export: row shards support the image branch only");
-  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_shard_export: no current map (call fitrig_tlisi first)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
   ShardExportParams ep;
   ep.raw = c->raw; ep.gmax_key = c->gmax_key + c->key_idx; ep.out = d_out;
   ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.stride = c->prm.stride; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
   ep.nblk = c->fin_nblk; ep.parts = c->parts; ep.counters = c->counters;
-  shard_export_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(ep);
-  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(launch_chain(shard_export_kernel, dim3(c->fin_grid), dim3(256), 0, st, !c->tune.no_pdl, ep));
   c->launches++;
   return FITRIG_OK;
 }
 
 extern "C" int fitrig_shard_import(fitrig_ctx* c, const double* d_all, int32_t world, float* d_tlisi, void* cuda_stream) {
-  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: ctx is NULL");
+  int rc = shard_check(c, "fitrig_shard_import");
+  if (rc) return rc;
   if (!d_all || world < 1) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: d_all is NULL or world < 1");
-  if (c->prm.branch != FITRIG_BRANCH_IMAGE)
-    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import: row shards support the image branch only");
-  if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_shard_import: no current map (call fitrig_tlisi first)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
   FinalizeParams fp;
-  fp.raw = c->raw; fp.q = c->q; fp.tlisi = c->tlisi; fp.tlisi_user = d_tlisi;
-  fp.gmax_key = c->gmax_key + c->key_idx; fp.gmax_key_next = c->gmax_key + (c->key_idx ^ 1); fp.M_out = c->M_dev;
-  fp.M_override = c->prm.M_override; fp.C = c->prm.C;
-  fp.H = c->H; fp.W = c->W; fp.tile = c->prm.tile; fp.stride = c->prm.stride; fp.Ty = c->Ty; fp.Tx = c->Tx; fp.U = c->U;
-  fp.nblk = c->fin_nblk; fp.parts = c->parts; fp.counters = c->counters; fp.mu = c->mu; fp.sigma = c->sigma;
+  fill_finalize_params(c, &fp, d_tlisi, c->gmax_key + c->key_idx);
+  fp.gmax_key_next = nullptr;  // (the finalise of fitrig_tlisi has prepared the next call's key already)
   fp.shard_all = d_all; fp.shard_world = world;
-  finalize_kernel<<<dim3(c->fin_nblk, c->U), 256, 0, st>>>(fp);
+  CUDA_TRY(launch_chain(finalize_kernel, dim3(c->fin_grid), dim3(256), 0, st, false, fp));
+  c->launches++;
+  c->eta_valid = false;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_shard_export_eta(fitrig_ctx* c, double* d_out, void* cuda_stream) {
+  int rc = shard_check(c, "fitrig_shard_export_eta");
+  if (rc) return rc;
+  if (!d_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export_eta: d_out is NULL");
+  if (c->prm.branch != FITRIG_BRANCH_FREQUENCY)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_export_eta: the context is not in the frequency branch");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  return launch_spectrum(c, (cudaStream_t)cuda_stream, d_out);
+}
+
+extern "C" int fitrig_shard_import_eta(fitrig_ctx* c, const double* d_all, int32_t world, void* cuda_stream) {
+  int rc = shard_check(c, "fitrig_shard_import_eta");
+  if (rc) return rc;
+  if (!d_all || world < 1) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_shard_import_eta: d_all is NULL or world < 1");
+  if (c->prm.branch != FITRIG_BRANCH_FREQUENCY || !c->eta_valid)
+    return fail(FITRIG_ERR_STATE, "fitrig_shard_import_eta: call fitrig_shard_export_eta first (frequency branch)");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  shard_import_eta_kernel<<<1, 32, 0, (cudaStream_t)cuda_stream>>>(d_all, world, c->smu, c->ssigma);
   CUDA_TRY(cudaGetLastError());
   c->launches++;
   return FITRIG_OK;
@@ -752,15 +955,16 @@ extern "C" int fitrig_get_stats(const fitrig_ctx* c, float* M, double* mu, doubl
   if (!c->have_map) return fail(FITRIG_ERR_STATE, "fitrig_get_stats: no current map");
   CUDA_TRY(cudaSetDevice(c->prm.device));
   CUDA_TRY(cudaDeviceSynchronize());
-  if (M) CUDA_TRY(cudaMemcpy(M, c->M_dev, sizeof(float), cudaMemcpyDeviceToHost));
+  if (M) CUDA_TRY(cudaMemcpy(M, c->M_dev, sizeof(float) * c->B, cudaMemcpyDeviceToHost));
   const bool freq_stats = c->prm.branch == FITRIG_BRANCH_FREQUENCY && c->eta_valid;
+  const size_t R = (size_t)c->B * c->U;
   if (mu) {
-    CUDA_TRY(cudaMemcpy(mu, c->mu, sizeof(double) * c->U, cudaMemcpyDeviceToHost));
-    if (freq_stats) CUDA_TRY(cudaMemcpy(mu, c->smu, sizeof(double), cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(mu, c->mu, sizeof(double) * R, cudaMemcpyDeviceToHost));
+    if (freq_stats) CUDA_TRY(cudaMemcpy(mu, c->smu, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
   }
   if (sigma) {
-    CUDA_TRY(cudaMemcpy(sigma, c->sigma, sizeof(double) * c->U, cudaMemcpyDeviceToHost));
-    if (freq_stats) CUDA_TRY(cudaMemcpy(sigma, c->ssigma, sizeof(double), cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(sigma, c->sigma, sizeof(double) * R, cudaMemcpyDeviceToHost));
+    if (freq_stats) CUDA_TRY(cudaMemcpy(sigma, c->ssigma, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
   }
   return FITRIG_OK;
 }
@@ -777,12 +981,13 @@ extern "C" int fitrig_get_map(const fitrig_ctx* c, int32_t which, float* h_out) 
     case 3: {
       if (c->prm.branch != FITRIG_BRANCH_FREQUENCY || !c->eta_valid)
         return fail(FITRIG_ERR_STATE, "fitrig_get_map: eta needs the frequency branch and a previous fitrig_detect");
+      const long long ne = c->nt * c->B;
       if (which == 2) {
-        CUDA_TRY(cudaMemcpy(h_out, c->eta, sizeof(float) * c->nt, cudaMemcpyDeviceToHost));
+        CUDA_TRY(cudaMemcpy(h_out, c->eta, sizeof(float) * ne, cudaMemcpyDeviceToHost));
       } else {
-        std::vector<int> k(c->nt);
-        CUDA_TRY(cudaMemcpy(k.data(), c->kstar, sizeof(int) * c->nt, cudaMemcpyDeviceToHost));
-        for (long long i = 0; i < c->nt; ++i) h_out[i] = (float)k[i];
+        std::vector<int> k(ne);
+        CUDA_TRY(cudaMemcpy(k.data(), c->kstar, sizeof(int) * ne, cudaMemcpyDeviceToHost));
+        for (long long i = 0; i < ne; ++i) h_out[i] = (float)k[i];
       }
       break;
     }
@@ -844,6 +1049,34 @@ extern "C" int fitrig_last_timing(const fitrig_ctx* c, float* main_ms, int32_t* 
   fitrig_ctx* m = const_cast<fitrig_ctx*>(c);  // reading starts a new accumulation window
   m->ev_used = 0;
   m->fin_used = 0;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int64_t bytes, int32_t reps, float* gbs,
+                                           void* cuda_stream) {
+  if (!c || !d_buf || !gbs) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_probe_read_bandwidth: NULL argument");
+  if (bytes < 16 || reps < 1 || ((uintptr_t)d_buf % 16) != 0)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_probe_read_bandwidth: need a 16-byte aligned buffer of at least 16 bytes, reps >= 1");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0));
+  CUDA_TRY(cudaEventCreate(&e1));
+  float best = 0.f;
+  const long long n4 = bytes / 16;
+  for (int r = 0; r < reps + 1; ++r) {  // the first pass warms up
+    CUDA_TRY(cudaEventRecord(e0, st));
+    read_probe_kernel<<<c->num_sms * 4, 512, 0, st>>>(reinterpret_cast<const float4*>(d_buf), n4, c->M_dev);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(e1, st));
+    CUDA_TRY(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    if (r > 0 && ms > 0.f) best = std::max(best, (float)((double)n4 * 16.0 / (ms * 1e-3) / 1e9));
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *gbs = best;
   return FITRIG_OK;
 }
 

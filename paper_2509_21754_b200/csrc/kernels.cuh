@@ -80,6 +80,11 @@ __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* ma
       "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar)
       : "memory");
 }
+// Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may become
+// resident while its predecessor in the stream still runs; pdl_wait() blocks until the predecessor has completed and
+// its memory is visible (a no-op for a plain launch).  pdl_launch_dependents() lets the successor's CTAs be scheduled.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ float rcp_approx(float a) {
   float r;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
@@ -137,6 +142,9 @@ struct FusedParams {
   int Tx32;              // 32-pixel block columns = ceil(W / 32): a consumer warp owns one 32x32 block
   int rows_tiles;        // rows of 32x32 blocks covered by this launch (whole image, or one strip)
   int ty_base;           // first tile row (in tiles of N_T) of this launch inside the whole map
+  int ty_end;            // one past the last cell row this launch owns: min(Ty, ty_base + ceil(rows / cell)).  A strip whose
+                         // height is not a multiple of 32 shares its last 32-row block with the next strip; the cells of
+                         // the zero-filled overhang belong to that strip and are neither written nor re-read here
   int U;                 // units = L - 2
   int ntw;               // tiles per TMA box = consumer warps per CTA (1..kMaxTilesPerBox)
   int ngx;               // boxes per tile row = ceil(Tx / ntw)
@@ -179,30 +187,57 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // Which pixels of its warp's 32x32 block a lane holds, for tiles of T = 32, 16 or 8 pixels.  The block is
-// (32/T)^2 tiles; T*T/32 consecutive lanes share one tile, so that the 32 pixels of a lane belong to ONE tile
-// and every reduction is a butterfly over an aligned lane group.  A lane reads float4's: T/4 lanes cover a
-// tile row, a lane group covers T/8 rows per load, 8 loads cover the tile; pixels are held in row-major
-// order of the tile.  T = 32: lane l owns columns 4*(l%8)..+3 of rows (l/8) + 4*j -- a quarter warp reads
-// one 128-byte row (conflict free); T = 8 likewise; T = 16 reads two 64-byte half rows (2-way conflict).
+// (32/T)^2 tiles; T*T/32 lanes share one tile, so that the 32 pixels of a lane belong to ONE tile and every
+// reduction is a butterfly over the tile's lane group.  A lane reads float4's: T/4 lanes cover a tile row, the
+// group covers T/8 rows per load, 8 loads cover the tile; pixels are held in row-major order of the tile.
+// In every geometry a quarter warp (8 consecutive lanes) reads ONE 128-byte row of the block (conflict free):
+//   T = 32  lane = [row 2 bits][col 3 bits]                  one tile, all 32 lanes
+//   T = 16  lane = [sub_row][row parity][sub_col][col 2 bits]  the two tiles of a block row share the quarter warp:
+//           a tile's 8 lanes are NOT consecutive (they differ in bits 0, 1 and 3)
+//   T = 8   lane = [sub_row 2 bits][sub_col 2 bits][col 1 bit] a tile's 2 lanes are neighbours
+// XOR*: the lane-index bits that vary inside a tile's group (butterfly offsets); SPLIT is the one used first.
 template <int T>
-struct LaneGeom {
-  static constexpr int LPT = T * T / 32;  // lanes per tile
-  static constexpr int F = T / 4;         // float4 (= lanes) per tile row
-  static constexpr int RPL = T / 8;       // tile rows per load
-  static constexpr int NSUB = 32 / T;     // tiles per block edge
-  __device__ static __forceinline__ int sub_row(int lane) { return (lane / LPT) / NSUB; }
-  __device__ static __forceinline__ int sub_col(int lane) { return (lane / LPT) % NSUB; }
-  __device__ static __forceinline__ int row_in_tile(int lane) { return (lane % LPT) / F; }   // + RPL * j
-  __device__ static __forceinline__ int col_in_tile(int lane) { return ((lane % LPT) % F) * 4; }
-  __device__ static __forceinline__ int block_row(int lane) { return sub_row(lane) * T + row_in_tile(lane); }
-  __device__ static __forceinline__ int block_col(int lane) { return sub_col(lane) * T + col_in_tile(lane); }
+struct LaneGeom;
+template <>
+struct LaneGeom<32> {
+  static constexpr int LPT = 32, RPL = 4, NSUB = 1, SPLIT = 16, NREST = 4;
+  __device__ static __forceinline__ int rest(int i) { return 8 >> i; }  // 8, 4, 2, 1
+  __device__ static __forceinline__ int sub_row(int) { return 0; }
+  __device__ static __forceinline__ int sub_col(int) { return 0; }
+  __device__ static __forceinline__ int row_in_tile(int lane) { return lane >> 3; }   // + RPL * j
+  __device__ static __forceinline__ int col_in_tile(int lane) { return (lane & 7) * 4; }
+  __device__ static __forceinline__ int leader_lane(int) { return 0; }
 };
+template <>
+struct LaneGeom<16> {
+  static constexpr int LPT = 8, RPL = 2, NSUB = 2, SPLIT = 8, NREST = 2;
+  __device__ static __forceinline__ int rest(int i) { return 2 >> i; }  // 2, 1
+  __device__ static __forceinline__ int sub_row(int lane) { return lane >> 4; }
+  __device__ static __forceinline__ int sub_col(int lane) { return (lane >> 2) & 1; }
+  __device__ static __forceinline__ int row_in_tile(int lane) { return (lane >> 3) & 1; }
+  __device__ static __forceinline__ int col_in_tile(int lane) { return (lane & 3) * 4; }
+  __device__ static __forceinline__ int leader_lane(int lane) { return lane & 0x14; }
+};
+template <>
+struct LaneGeom<8> {
+  static constexpr int LPT = 2, RPL = 1, NSUB = 4, SPLIT = 1, NREST = 0;
+  __device__ static __forceinline__ int rest(int) { return 0; }
+  __device__ static __forceinline__ int sub_row(int lane) { return lane >> 3; }
+  __device__ static __forceinline__ int sub_col(int lane) { return (lane >> 1) & 3; }
+  __device__ static __forceinline__ int row_in_tile(int) { return 0; }
+  __device__ static __forceinline__ int col_in_tile(int lane) { return (lane & 1) * 4; }
+  __device__ static __forceinline__ int leader_lane(int lane) { return lane & ~1; }
+};
+template <int T>
+__device__ __forceinline__ int geom_block_row(int lane) { return LaneGeom<T>::sub_row(lane) * T + LaneGeom<T>::row_in_tile(lane); }
+template <int T>
+__device__ __forceinline__ int geom_block_col(int lane) { return LaneGeom<T>::sub_col(lane) * T + LaneGeom<T>::col_in_tile(lane); }
 
 // The lane's 32 pixels out of a box (row pitch `pitch` bytes) into registers / added to registers.
 template <int T>
 __device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
   using G = LaneGeom<T>;
-  const unsigned char* src = block_ptr + G::block_row(lane) * pitch + G::block_col(lane) * 4;
+  const unsigned char* src = block_ptr + geom_block_row<T>(lane) * pitch + geom_block_col<T>(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
@@ -213,7 +248,7 @@ __device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* b
 template <int T>
 __device__ __forceinline__ void add_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
   using G = LaneGeom<T>;
-  const unsigned char* src = block_ptr + G::block_row(lane) * pitch + G::block_col(lane) * 4;
+  const unsigned char* src = block_ptr + geom_block_row<T>(lane) * pitch + geom_block_col<T>(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
@@ -304,7 +339,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   uint64_t* empty = full + kMaxStages;
   // arg-max scratch of this lane's tile (one per lane group)
   float4* scratch = reinterpret_cast<float4*>(after_ring + 2 * kMaxStages * 8) +
-                    (warp * NGRP + (threadIdx.x & 31) / LPT) * kScratchVec;
+                    (warp * NGRP + Geo::sub_row(threadIdx.x & 31) * Geo::NSUB + Geo::sub_col(threadIdx.x & 31)) * kScratchVec;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < p.nstage; ++i) {
@@ -315,6 +350,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
+  pdl_launch_dependents();  // the finalise kernel may take its place on the SMs; it waits for this grid to complete
 
   // this CTA's range of (group, unit) pairs
   const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
@@ -355,8 +391,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   float gmax = -3.402823466e38f, zA = 1.f, zB = 1.f;
   int slot = 0;
   uint32_t phase = 0;
-  const bool leader = (lane % LPT) == 0;  // does the bookkeeping of its tile
-  const unsigned gmask = (LPT == 32) ? 0xffffffffu : (((1u << (LPT & 31)) - 1u) << (lane & ~(LPT - 1)));
+  const bool leader = lane == Geo::leader_lane(lane);  // does the bookkeeping of its tile
 
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
@@ -428,18 +463,30 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // position of this lane's tile inside the warp's block (0 for T = 32)
   const int sub_off = Geo::sub_row(lane) * T * p.W + Geo::sub_col(lane) * T;
 
-  // reduction of one (tile, unit) over the tile's lane group: exact max + first 16-byte group by redux, the two
-  // sums by one butterfly (lower half of the group carries sum Delta, upper half sum r)
+  // reduction of one (tile, unit) over the tile's lane group: exact max + first 16-byte group (one redux pair for a
+  // whole-warp tile; a full-mask butterfly over the group's lane bits otherwise -- redux on partial masks would be
+  // executed once per group), the two sums by one butterfly (one half of the group carries sum Delta, the other sum r)
   auto finish = [&](float S, float R, float Mx, int jmax) {
-    const unsigned mbits = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
-    const unsigned tmax = __reduce_max_sync(gmask, mbits);
-    const int gpos = (Geo::row_in_tile(lane) + Geo::RPL * jmax) * T + Geo::col_in_tile(lane);  // row-major in the tile
-    const unsigned tg = __reduce_min_sync(gmask, mbits == tmax ? (unsigned)gpos : 0x7fffffffu);
-    const bool hi = lane & (LPT / 2);
-    float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, LPT / 2);
+    unsigned tmax = __float_as_uint(Mx);  // Mx >= +0: uint order == float order
+    unsigned tg = (unsigned)((Geo::row_in_tile(lane) + Geo::RPL * jmax) * T + Geo::col_in_tile(lane));  // row-major in the tile
+    if (LPT == 32) {
+      const unsigned mbits = tmax;
+      tmax = __reduce_max_sync(0xffffffffu, mbits);
+      tg = __reduce_min_sync(0xffffffffu, mbits == tmax ? tg : 0x7fffffffu);
+    } else {
+      auto level = [&](int off) {
+        const unsigned om = __shfl_xor_sync(0xffffffffu, tmax, off), op = __shfl_xor_sync(0xffffffffu, tg, off);
+        if (om > tmax || (om == tmax && op < tg)) { tmax = om; tg = op; }
+      };
+      level(Geo::SPLIT);
 #pragma unroll
-    for (int off = LPT / 4; off >= 1; off >>= 1) vsum += __shfl_xor_sync(0xffffffffu, vsum, off);
-    const float rsum = __shfl_sync(0xffffffffu, vsum, (lane & ~(LPT - 1)) + LPT / 2);
+      for (int i = 0; i < Geo::NREST; ++i) level(Geo::rest(i));
+    }
+    const bool hi = lane & Geo::SPLIT;
+    float vsum = (hi ? R : S) + __shfl_xor_sync(0xffffffffu, hi ? S : R, Geo::SPLIT);
+#pragma unroll
+    for (int i = 0; i < Geo::NREST; ++i) vsum += __shfl_xor_sync(0xffffffffu, vsum, Geo::rest(i));
+    const float rsum = __shfl_sync(0xffffffffu, vsum, Geo::leader_lane(lane) | Geo::SPLIT);
     if (leader) {
       if (pend) resolve_pending();
       pend = false;
@@ -507,7 +554,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
           if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
         }
         const int ty_r = j, tx_r = cg;
-        if (rb == 0 && ty0 + ty_r < p.Ty && tx0 + tx_r < p.Tx) {
+        if (rb == 0 && ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
           RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
           rp[(long long)ty_r * p.Tx + tx_r] = o;
         }
@@ -523,7 +570,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
           const int op = __shfl_xor_sync(0xffffffffu, pos, 8);
           if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
           const int ty_r = row >> 1, tx_r = 2 * cg + h;
-          if ((rb & 1) == 0 && ty0 + ty_r < p.Ty && tx0 + tx_r < p.Tx) {
+          if ((rb & 1) == 0 && ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
             RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
             rp[(long long)ty_r * p.Tx + tx_r] = o;
           }
@@ -532,7 +579,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
           const int tx_r = 4 * cg + e;
-          if (ty0 + row < p.Ty && tx0 + tx_r < p.Tx) {
+          if (ty0 + row < p.ty_end && tx0 + tx_r < p.Tx) {
             RawTile o; o.sumD = dl[e]; o.maxD = dl[e]; o.sumR = rr[e]; o.pos = 0;
             rp[(long long)row * p.Tx + tx_r] = o;
           }
@@ -557,7 +604,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       ip2 = p.base + blk + (long long)ring_slot(p.z0, p.zmask, (c.u0 + 2) * acc) * p.snap_stride;
       const int ty_t = p.ty_base + c.ty_local * Geo::NSUB + Geo::sub_row(lane);  // tile coordinates in the whole map
       const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
-      tile_exists = Geo::NSUB == 1 || (ty_t < p.Ty && tx_t < p.Tx);
+      tile_exists = Geo::NSUB == 1 || (ty_t < p.ty_end && tx_t < p.Tx);
       rp = p.raw + ((long long)c.u0 * p.Ty + ty_t) * p.Tx + tx_t;
     }
     acquire(A, zA);  // x_{u0}
@@ -720,324 +767,439 @@ __global__ void __launch_bounds__(256) stack_max_kernel(const float* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------------
-// Block-level helpers for the statistics (fp64, deterministic order)
+// Statistics (fp64, deterministic order).  Mean and population standard deviation of a map row from SHIFTED sums:
+// with K = the row's first value, d = v - K, a block adds sum d and sum d^2 in a fixed tree order; partials are
+// added in chunk order.  mu = K + sum d / n, sigma^2 = sum d^2 / n - (sum d / n)^2.  The shift makes a constant
+// row give sigma == 0 exactly (R4) and keeps the subtraction well conditioned (|d| is of the order of sigma).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double block_sum(double v, double* sh /*[32]*/) {
-  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
-  __syncthreads();
-  if (lane == 0) sh[warp] = v;
-  __syncthreads();
-  double t = 0.0;
-  for (int i = 0; i < nw; ++i) t += sh[i];  // same order in every thread
-  return t;
-}
-
 struct StatPartial {
-  double n, mean, m2;
+  double n, s, s2;  // count, sum d, sum d^2
 };
 
-// Mean and population standard deviation of v[row][0..n) from per-block (n, mean, M2) partials that
-// are merged in block order with Chan's update -- a two-pass variance per block, deterministic.
-// The last block of each row to finish does the merge (threadfence + counter).
-__device__ __forceinline__ void row_stats_block(const float* v, long long begin, long long end, int row, int nblk,
-                                                StatPartial* parts, unsigned* counters, double* mu, double* sigma,
-                                                double* sh) {
-  double s = 0.0;
-  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) s += (double)v[i];
-  const double cnt = (double)(end - begin);
-  const double mean_b = block_sum(s, sh) / (cnt > 0 ? cnt : 1.0);
-  double s2 = 0.0;
-  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) {
-    const double d = (double)v[i] - mean_b;
-    s2 += d * d;
+// sum of (a, b) over the block, the same value in every thread; sh: 64 doubles
+__device__ __forceinline__ void block_sum2(double& a, double& b, double* sh) {
+  for (int off = 16; off > 0; off >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, off);
+    b += __shfl_xor_sync(0xffffffffu, b, off);
   }
-  const double m2_b = block_sum(s2, sh);
-  __shared__ bool is_last;
-  if (threadIdx.x == 0) {
-    StatPartial sp;
-    sp.n = cnt; sp.mean = mean_b; sp.m2 = m2_b;
-    parts[(size_t)row * nblk + blockIdx.x] = sp;
-    __threadfence();
-    const unsigned done = atomicAdd(&counters[row], 1u);
-    is_last = (done == (unsigned)nblk - 1);
-  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+  __syncthreads();  // (sh may still be read from a previous use)
+  if (lane == 0) { sh[warp] = a; sh[32 + warp] = b; }
   __syncthreads();
-  if (is_last && threadIdx.x == 0) {
-    __threadfence();
-    double n = 0.0, mean = 0.0, m2 = 0.0;
-    for (int b = 0; b < nblk; ++b) {
-      const volatile StatPartial* sp = &parts[(size_t)row * nblk + b];
-      const double nb = sp->n, mb = sp->mean, m2b = sp->m2;
-      if (nb <= 0) continue;
-      const double tot = n + nb, dlt = mb - mean;
-      mean += dlt * (nb / tot);
-      m2 += m2b + dlt * dlt * (n * nb / tot);
-      n = tot;
-    }
-    mu[row] = mean;
-    sigma[row] = (n > 0) ? sqrt(m2 / n) : 0.0;
-    counters[row] = 0;  // ready for the next call
+  double ta = 0.0, tb = 0.0;
+  for (int i = 0; i < nw; ++i) { ta += sh[i]; tb += sh[32 + i]; }  // same order in every thread
+  a = ta; b = tb;
+}
+
+// Adds the nblk partials of one row in a fixed order (lane-strided, then a shuffle tree) -- one warp.
+__device__ __forceinline__ void warp_merge_partials(const StatPartial* parts, int nblk, double& n, double& s, double& s2) {
+  const int lane = threadIdx.x & 31;
+  n = 0.0; s = 0.0; s2 = 0.0;
+  for (int b = lane; b < nblk; b += 32) {
+    const volatile StatPartial* sp = parts + b;
+    n += sp->n; s += sp->s; s2 += sp->s2;
+  }
+  for (int off = 16; off > 0; off >>= 1) {
+    n += __shfl_xor_sync(0xffffffffu, n, off);
+    s += __shfl_xor_sync(0xffffffffu, s, off);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, off);
   }
 }
 
+__device__ __forceinline__ void stats_from_sums(double K, double n, double s, double s2, double* mu, double* sigma) {
+  if (n <= 0.0) { *mu = 0.0; *sigma = 0.0; return; }
+  const double m = s / n;
+  *mu = K + m;
+  *sigma = sqrt(fmax(s2 / n - m * m, 0.0));
+}
+
+// The last block of a row to deposit its partial merges them (threadfence + counter).  Called by every thread of the
+// block; `sh_flag` is a shared int.
+__device__ __forceinline__ void row_stats_finish(StatPartial part, double K, int row, int blk, int nblk, StatPartial* parts,
+                                                 unsigned* counters, double* mu, double* sigma, int* sh_flag) {
+  if (threadIdx.x == 0) {
+    parts[(size_t)row * nblk + blk] = part;
+    __threadfence();
+    *sh_flag = (atomicAdd(&counters[row], 1u) == (unsigned)nblk - 1);
+  }
+  __syncthreads();
+  if (*sh_flag && threadIdx.x < 32) {
+    __threadfence();
+    double n, a, b;
+    warp_merge_partials(parts + (size_t)row * nblk, nblk, n, a, b);
+    if (threadIdx.x == 0) {
+      stats_from_sums(K, n, a, b, &mu[row], &sigma[row]);
+      counters[row] = 0;  // ready for the next call
+    }
+  }
+  __syncthreads();  // sh_flag is reused by the block's next chunk
+}
+
 // ---------------------------------------------------------------------------------------------
-// finalize: q, tLISI, per-unit statistics (a6, a7)
+// finalize: q, tLISI, per-row statistics (a6, a7).  Map rows are (batch entry, unit) pairs, row = b * U + u.
 // ---------------------------------------------------------------------------------------------
+constexpr int kFinChunk = 1024;  // map entries per block and pass
+
 struct FinalizeParams {
   const RawTile* raw;
-  float* q;            // [U][Ty][Tx]
-  float* tlisi;        // context copy, [U][Ty][Tx]
+  float* q;            // [B][U][Ty][Tx]
+  float* tlisi;        // context copy
   float* tlisi_user;   // caller's device buffer or NULL
-  const unsigned* gmax_key;
-  unsigned* gmax_key_next;  // key of the NEXT call: zeroed here so that no memset sits in the stream
-  float* M_out;        // device scalar: the M that was used
+  const unsigned* gmax_key;  // [B] ordered keys of the global maxima
+  unsigned* gmax_key_next;   // [B] keys of the NEXT call: zeroed here so that no memset sits in the stream (or NULL)
+  float* M_out;        // [B] device scalars: the M that was used
   float M_override;
   float C;
-  int H, W, tile, stride, Ty, Tx, U;  // windows of `tile` pixels every `stride` pixels (stride == tile: tiles)
-  int nblk;            // blocks per unit
-  StatPartial* parts;  // [U][nblk]
-  unsigned* counters;  // [U]
-  double* mu;          // [U]
-  double* sigma;       // [U]
+  int H, W, tile, stride, Ty, Tx, U, B;  // windows of `tile` pixels every `stride` pixels (stride == tile: tiles)
+  int nblk;            // chunks per row = ceil(Ty * Tx / kFinChunk)
+  StatPartial* parts;  // [B * U][nblk]
+  unsigned* counters;  // [B * U]
+  double* mu;          // [B * U]
+  double* sigma;       // [B * U]
   // row-shard mode (fitrig_shard_import): M, mu, sigma come from the all-gathered export vectors
   const double* shard_all;  // [shard_world][2 + 2U] or NULL
   int shard_world;
+  int user_row;        // -1: tlisi_user is the whole map; r >= 0: tlisi_user is [Ty][Tx] and receives map row r only
 };
 
+// Eq. 2 / Eq. 6 without the 1 / M^2 factor: p = (sum D / n_t) * max D * (sum r / n_t); n_t = the window's own pixel
+// count (R5).  inv_full = 1 / tile^2 serves every full window (a multiplication instead of two fp64 divisions per
+// entry, which made the per-pixel maps compute bound); a partial edge window divides by its own count.
+__device__ __forceinline__ double tile_product(const RawTile r, int t, int Tx, int H, int W, int tile, int stride,
+                                               double inv_full) {
+  const int ty = (int)((unsigned)t / (unsigned)Tx), tx = t - ty * Tx;
+  const int h = min(tile, H - ty * stride), w = min(tile, W - tx * stride);
+  const double inv_n = (h == tile && w == tile) ? inv_full : 1.0 / ((double)h * (double)w);
+  return ((double)r.sumD * inv_n) * (double)r.maxD * ((double)r.sumR * inv_n);
+}
+
+// Chan's merge of per-shard (n, mean, M2) triples in shard order
+__device__ __forceinline__ void chan_merge(double& n, double& mean, double& m2, double nb, double mb, double m2b) {
+  if (nb <= 0.0) return;
+  const double tot = n + nb, dlt = mb - mean;
+  mean += dlt * (nb / tot);
+  m2 += m2b + dlt * dlt * (n * nb / tot);
+  n = tot;
+}
+
 __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
-  __shared__ double sh[32];
-  const int u = blockIdx.y;
-  const long long nt = (long long)p.Ty * p.Tx;
-  const long long per = (nt + p.nblk - 1) / p.nblk;
-  const long long begin = min(nt, (long long)blockIdx.x * per), end = min(nt, begin + per);
-  // M = max(max_s x^(s), C), PAPER.md:223 (R2: signed max), or the caller's override
-  float M;
+  __shared__ double sh[64];
+  __shared__ int sh_flag;
+  pdl_wait();               // the tLISI kernel's records and its global maximum
+  pdl_launch_dependents();  // (a compaction launched behind this kernel waits for its completion all the same)
+  const int nt = p.Ty * p.Tx;
+  const int R = p.B * p.U;
+  const double inv_full = 1.0 / ((double)p.tile * (double)p.tile);
+  const long long nchunks = (long long)R * p.nblk;
   const int vlen = 2 + 2 * p.U;  // length of one shard's export vector
-  if (p.shard_all) {
-    double m = p.shard_all[0];
-    for (int r = 1; r < p.shard_world; ++r) m = fmax(m, p.shard_all[(size_t)r * vlen]);
-    M = fmaxf((float)m, p.C);  // the entries are fp32 pixel values: the cast is exact
-  } else {
-    M = fmaxf(key_to_float(*p.gmax_key), p.C);
-  }
-  if (p.M_override > 0.f) M = p.M_override;
-  if (blockIdx.x == 0 && u == 0 && threadIdx.x == 0) {
-    *p.M_out = M;
-    *p.gmax_key_next = 0u;
-  }
-  const double inv_m2 = 1.0 / ((double)M * (double)M);
-  const size_t base = (size_t)u * nt;
-  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
-    const unsigned tu = (unsigned)t;  // tiles per unit < 2^31
-    const int ty = (int)(tu / (unsigned)p.Tx), tx = (int)(tu - (unsigned)ty * (unsigned)p.Tx);
-    const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
-    const double n_t = (double)h * (double)w;  // R5: partial tiles use their own pixel count
-    const RawTile r = p.raw[base + t];
-    // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2
-    const double qd = ((double)r.sumD / n_t) * (double)r.maxD * ((double)r.sumR / n_t) * inv_m2;
-    const float qf = (float)qd;
-    p.q[base + t] = qf;
-    const float tl = (float)(1.0 - qd);
-    p.tlisi[base + t] = tl;
-    if (p.tlisi_user) p.tlisi_user[base + t] = tl;
-  }
-  if (p.shard_all) {
-    // Eq. 8 over ALL tiles of the image from the shards' sums of p = q * M^2, merged in shard order
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-      double n = 0.0, sp = 0.0, sp2 = 0.0;
-      for (int r = 0; r < p.shard_world; ++r) {
-        const double* v = p.shard_all + (size_t)r * vlen;
-        n += v[1];
-        sp += v[2 + u];
-        sp2 += v[2 + p.U + u];
-      }
-      const double mean_p = (n > 0) ? sp / n : 0.0;
-      const double var_p = (n > 0) ? fmax(sp2 / n - mean_p * mean_p, 0.0) : 0.0;
-      p.mu[u] = mean_p * inv_m2;
-      p.sigma[u] = sqrt(var_p) * inv_m2;
+  for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+    const int row = (int)(chunk / p.nblk), blk = (int)(chunk - (long long)row * p.nblk);
+    const int b = row / p.U, u = row - b * p.U;
+    // M = max(max_s x^(s), C), PAPER.md:223 (R2: signed max), or the caller's override
+    float M;
+    if (p.shard_all) {
+      double m = p.shard_all[0];
+      for (int r = 1; r < p.shard_world; ++r) m = fmax(m, p.shard_all[(size_t)r * vlen]);
+      M = fmaxf((float)m, p.C);  // the entries are fp32 pixel values: the cast is exact
+    } else {
+      M = fmaxf(key_to_float(p.gmax_key[b]), p.C);
     }
-    return;
+    if (p.M_override > 0.f) M = p.M_override;
+    const double inv_m2 = 1.0 / ((double)M * (double)M);
+    const size_t base = (size_t)row * nt;
+    // the row's shift: its first q value
+    const double K = (double)(float)(tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2);
+    const int begin = blk * kFinChunk, end = min(nt, begin + kFinChunk);
+    double s = 0.0, s2 = 0.0;
+    for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
+      // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2, combined in fp64 and rounded once
+      const double qd = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2;
+      const float qf = (float)qd;
+      p.q[base + t] = qf;
+      const float tl = (float)(1.0 - qd);
+      p.tlisi[base + t] = tl;
+      if (p.tlisi_user) {
+        if (p.user_row < 0) p.tlisi_user[base + t] = tl;
+        else if (row == p.user_row) p.tlisi_user[t] = tl;
+      }
+      const double d = (double)qf - K;
+      s += d;
+      s2 += d * d;
+    }
+    if (p.shard_all) {
+      // Eq. 8 over ALL tiles of the image: the shards' (n, mean, M2) of the M-free product p, merged in shard order
+      if (blk == 0 && threadIdx.x == 0) {
+        double n = 0.0, mean = 0.0, m2 = 0.0;
+        for (int r = 0; r < p.shard_world; ++r) {
+          const double* v = p.shard_all + (size_t)r * vlen;
+          chan_merge(n, mean, m2, v[1], v[2 + u], v[2 + p.U + u]);
+        }
+        p.mu[row] = mean * inv_m2;
+        p.sigma[row] = (n > 0.0) ? sqrt(m2 / n) * inv_m2 : 0.0;
+        if (u == 0) p.M_out[b] = M;
+      }
+      continue;
+    }
+    if (blk == 0 && u == 0 && threadIdx.x == 0) {
+      p.M_out[b] = M;
+      if (p.gmax_key_next) p.gmax_key_next[b] = 0u;
+    }
+    block_sum2(s, s2, sh);
+    StatPartial part;
+    part.n = (double)(end - begin); part.s = s; part.s2 = s2;
+    row_stats_finish(part, K, row, blk, p.nblk, p.parts, p.counters, p.mu, p.sigma, &sh_flag);
   }
-  __syncthreads();  // this block's q values are re-read below (by the same threads, but keep it simple)
-  row_stats_block(p.q + base, begin, end, u, p.nblk, p.parts, p.counters, p.mu, p.sigma, sh);
 }
 
 // ---------------------------------------------------------------------------------------------
-// row shards: what the other shards need (fitrig_shard_export)
+// row shards: what the other shards need (fitrig_shard_export): per unit (n, mean, M2) of the M-free product p
 // ---------------------------------------------------------------------------------------------
 struct ShardExportParams {
   const RawTile* raw;
   const unsigned* gmax_key;
-  double* out;          // [2 + 2U]
+  double* out;          // [2 + 2U]: max pixel, tiles per unit, mean_p[U], M2_p[U]
   int H, W, tile, stride, Ty, Tx, U;
-  int nblk;             // blocks per unit
+  int nblk;             // chunks per unit
   StatPartial* parts;   // [U][nblk]
   unsigned* counters;   // [U]
 };
 
 __global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportParams p) {
-  __shared__ double sh[32];
-  const int u = blockIdx.y;
-  const long long nt = (long long)p.Ty * p.Tx;
-  const long long per = (nt + p.nblk - 1) / p.nblk;
-  const long long begin = min(nt, (long long)blockIdx.x * per), end = min(nt, begin + per);
-  const size_t base = (size_t)u * nt;
-  double s = 0.0, s2 = 0.0;
-  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
-    const int ty = (int)(t / p.Tx), tx = (int)(t - (long long)ty * p.Tx);
-    const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
-    const double n_t = (double)h * (double)w;
-    const RawTile r = p.raw[base + t];
-    const double pv = ((double)r.sumD / n_t) * (double)r.maxD * ((double)r.sumR / n_t);  // Eq. 6 without 1/M^2
-    s += pv;
-    s2 += pv * pv;
-  }
-  s = block_sum(s, sh);
-  s2 = block_sum(s2, sh);
-  __shared__ bool is_last;
-  if (threadIdx.x == 0) {
-    StatPartial sp;
-    sp.n = (double)(end - begin); sp.mean = s; sp.m2 = s2;  // here: plain sums
-    p.parts[(size_t)u * p.nblk + blockIdx.x] = sp;
-    __threadfence();
-    is_last = (atomicAdd(&p.counters[u], 1u) == (unsigned)p.nblk - 1);
-  }
-  __syncthreads();
-  if (is_last && threadIdx.x == 0) {
-    __threadfence();
-    double a = 0.0, b = 0.0;
-    for (int i = 0; i < p.nblk; ++i) {  // block order: deterministic
-      const volatile StatPartial* sp = &p.parts[(size_t)u * p.nblk + i];
-      a += sp->mean;
-      b += sp->m2;
+  __shared__ double sh[64];
+  __shared__ int sh_flag;
+  pdl_wait();
+  const int nt = p.Ty * p.Tx;
+  const double inv_full = 1.0 / ((double)p.tile * (double)p.tile);
+  const long long nchunks = (long long)p.U * p.nblk;
+  for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+    const int u = (int)(chunk / p.nblk), blk = (int)(chunk - (long long)u * p.nblk);
+    const size_t base = (size_t)u * nt;
+    const double K = tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full);
+    const int begin = blk * kFinChunk, end = min(nt, begin + kFinChunk);
+    double s = 0.0, s2 = 0.0;
+    for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
+      const double d = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) - K;
+      s += d;
+      s2 += d * d;
     }
-    p.out[2 + u] = a;
-    p.out[2 + p.U + u] = b;
-    p.counters[u] = 0;
-    if (u == 0) {
-      p.out[0] = (double)key_to_float(*p.gmax_key);
-      p.out[1] = (double)nt;
+    block_sum2(s, s2, sh);
+    if (threadIdx.x == 0) {
+      StatPartial part;
+      part.n = (double)(end - begin); part.s = s; part.s2 = s2;
+      p.parts[(size_t)u * p.nblk + blk] = part;
+      __threadfence();
+      sh_flag = (atomicAdd(&p.counters[u], 1u) == (unsigned)p.nblk - 1);
     }
+    __syncthreads();
+    if (sh_flag && threadIdx.x < 32) {
+      __threadfence();
+      double n, a, b;
+      warp_merge_partials(p.parts + (size_t)u * p.nblk, p.nblk, n, a, b);
+      if (threadIdx.x == 0) {
+        const double m = (n > 0.0) ? a / n : 0.0;
+        p.out[2 + u] = K + m;                                   // mean of p over the shard's tiles
+        p.out[2 + p.U + u] = fmax(b - a * m, 0.0);              // M2 = sum (p - mean)^2 = sum d^2 - (sum d)^2 / n
+        p.counters[u] = 0;
+        if (u == 0) {
+          p.out[0] = (double)key_to_float(*p.gmax_key);
+          p.out[1] = (double)nt;
+        }
+      }
+    }
+    __syncthreads();
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// spectrum: per-tile temporal DFT (a10), Eq. 10 with h = max magnitude
+// spectrum: per-tile temporal DFT (a10), Eq. 10.  All arithmetic in fp64 (the data is 1 / N_T^2 of the pixels): the
+// DC-free series a_u = q_u - mean(q) is a cancellation of values that agree in their first digit or two, so the
+// error of eta is what the fp32 q map carries in, amplified by that cancellation, and nothing more.
 // ---------------------------------------------------------------------------------------------
 struct SpectrumParams {
-  const float* q;       // [U][nt]
-  const float2* tw;     // [U] twiddles (cos, -sin)(2 pi j / U)
-  float* eta;           // [nt]
-  int* kstar;           // [nt]
-  float* mag;           // [U/2][nt] magnitude spectrum
+  const float* q;       // [B][U][nt]
+  const double2* tw;    // [U] twiddles (cos, -sin)(2 pi j / U)
+  float* eta;           // [B][nt]
+  int* kstar;           // [B][nt]
+  float* mag;           // [B][U/2][nt] magnitude spectrum
   int harmonics;        // H >= 1: h = harmonic sum over 1, 2, 4, .., H harmonics (R26); 1: maximum magnitude
-  long long nt;
-  int U;
-  int nblk;
-  StatPartial* parts;   // [nblk]
-  unsigned* counters;   // [1]
-  double* mu;           // [1]
-  double* sigma;        // [1]
+  int nt;
+  int U, B;
+  int nblk;             // chunks per batch entry = ceil(nt / kFinChunk)
+  StatPartial* parts;   // [B][nblk]
+  unsigned* counters;   // [B]
+  double* mu;           // [B]
+  double* sigma;        // [B]
+  // row shards: the eta statistics come from the all-gathered (n, mean, M2) triples instead (fitrig_shard_import_eta)
+  double* shard_out;    // [3] or NULL: this shard's (n, mean, M2) of eta
 };
 
 // Magnitude spectrum m_k = |F_k|, k = 1..K, of every tile's DC-free series (Eq. 10): one thread per (tile, block of
 // kDftBins bins), tiles fastest so that the loads of q coalesce and the twiddle index is warp uniform (shared-memory
 // broadcast).  Direct DFT: the series is short (U = 30 in config 5, 1498 in the paper's real-data run) and of arbitrary
 // length (R17).
-constexpr int kDftBins = 8;
+constexpr int kDftBins = 4;
 
 __global__ void __launch_bounds__(128) dft_mag_kernel(const SpectrumParams p) {
-  extern __shared__ float2 tws[];  // U twiddles
+  extern __shared__ double2 tws[];  // U twiddles
+  pdl_wait();
+  pdl_launch_dependents();
   for (int i = threadIdx.x; i < p.U; i += blockDim.x) tws[i] = p.tw[i];
   __syncthreads();
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= p.nt) return;
+  const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;  // (batch entry, tile)
+  if (g >= (long long)p.B * p.nt) return;
+  const int b = (int)(g / p.nt), t = (int)(g - (long long)b * p.nt);
+  const float* q = p.q + (size_t)b * p.U * p.nt + t;
   const int K = p.U / 2, k0 = blockIdx.y * kDftBins + 1;
-  float mean = 0.f;
-  for (int u = 0; u < p.U; ++u) mean += p.q[(size_t)u * p.nt + t];
-  mean /= (float)p.U;  // DC removed
-  float re[kDftBins], im[kDftBins];
-  int j[kDftBins];  // (k * u) mod U
+  double mean = 0.0;
+  for (int u = 0; u < p.U; ++u) mean += (double)q[(size_t)u * p.nt];
+  mean /= (double)p.U;  // DC removed
+  double re[kDftBins], im[kDftBins];
+  int j[kDftBins], kk[kDftBins];  // (k * u) mod U and its step k (0 for bins beyond K: they stay at twiddle 0)
 #pragma unroll
-  for (int b = 0; b < kDftBins; ++b) { re[b] = 0.f; im[b] = 0.f; j[b] = 0; }
+  for (int i = 0; i < kDftBins; ++i) { re[i] = 0.0; im[i] = 0.0; j[i] = 0; kk[i] = (k0 + i <= K) ? k0 + i : 0; }
   for (int u = 0; u < p.U; ++u) {
-    const float a = p.q[(size_t)u * p.nt + t] - mean;
+    const double a = (double)q[(size_t)u * p.nt] - mean;
 #pragma unroll
-    for (int b = 0; b < kDftBins; ++b) {
-      const float2 w = tws[j[b]];
-      re[b] = fmaf(a, w.x, re[b]);
-      im[b] = fmaf(a, w.y, im[b]);
-      j[b] += k0 + b;
-      if (j[b] >= p.U) j[b] -= p.U;
+    for (int i = 0; i < kDftBins; ++i) {
+      const double2 w = tws[j[i]];
+      re[i] = fma(a, w.x, re[i]);
+      im[i] = fma(a, w.y, im[i]);
+      j[i] += kk[i];              // k <= K < U: one subtraction wraps
+      if (j[i] >= p.U) j[i] -= p.U;
     }
   }
 #pragma unroll
-  for (int b = 0; b < kDftBins; ++b)
-    if (k0 + b <= K) p.mag[(size_t)(k0 + b - 1) * p.nt + t] = sqrtf(re[b] * re[b] + im[b] * im[b]);
+  for (int i = 0; i < kDftBins; ++i)
+    if (k0 + i <= K) p.mag[((size_t)b * K + (k0 + i - 1)) * p.nt + t] = (float)sqrt(re[i] * re[i] + im[i] * im[i]);
 }
 
 // eta = h(m) per tile (maximum magnitude, or harmonic summing), k*, and the statistics of eta (Eq. 11).
-__global__ void __launch_bounds__(128) spectrum_kernel(const SpectrumParams p) {
-  __shared__ double sh[32];
-  const long long per = (p.nt + p.nblk - 1) / p.nblk;
-  const long long begin = min(p.nt, (long long)blockIdx.x * per), end = min(p.nt, begin + per);
+__global__ void __launch_bounds__(256) spectrum_kernel(const SpectrumParams p) {
+  __shared__ double sh[64];
+  __shared__ int sh_flag;
+  pdl_wait();
+  pdl_launch_dependents();
   const int K = p.U / 2;
-  for (long long t = begin + threadIdx.x; t < end; t += blockDim.x) {
-    float best = 0.f;
-    int kb = (K >= 1) ? 1 : 0;
-    if (p.harmonics <= 1) {  // h = maximum spectral magnitude, first bin on ties
-      for (int k = 1; k <= K; ++k) {
-        const float mag = p.mag[(size_t)(k - 1) * p.nt + t];
-        if (k == 1 || mag > best) { best = mag; kb = k; }
+  const long long nchunks = (long long)p.B * p.nblk;
+  for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+    const int b = (int)(chunk / p.nblk), blk = (int)(chunk - (long long)b * p.nblk);
+    const float* mag = p.mag + (size_t)b * K * p.nt;
+    auto eta_of = [&](int t, int* kb_out) {
+      float best = 0.f;
+      int kb = (K >= 1) ? 1 : 0;
+      if (p.harmonics <= 1) {  // h = maximum spectral magnitude, first bin on ties
+        for (int k = 1; k <= K; ++k) {
+          const float m = mag[(size_t)(k - 1) * p.nt + t];
+          if (k == 1 || m > best) { best = m; kb = k; }
+        }
+      } else {
+        // harmonic summing (R26): s_h(k) = sum_{i<=h} m_{ik} / sqrt(h), h = 1, 2, 4, .., H, h*k <= K
+        bool first = true;
+        double bestd = 0.0;
+        for (int k = 1; k <= K; ++k) {
+          double s = 0.0;
+          int have = 0;  // harmonics summed so far
+          for (int h = 1; h <= p.harmonics && h * k <= K; h *= 2) {
+            for (int i = have + 1; i <= h; ++i) s += (double)mag[(size_t)(i * k - 1) * p.nt + t];  // m_k, m_2k, ... in order
+            have = h;
+            const double v = s / sqrt((double)h);
+            if (first || v > bestd) { bestd = v; kb = k; first = false; }
+          }
+        }
+        best = (float)bestd;
       }
-    } else {
-      // harmonic summing (R26): s_h(k) = sum_{i<=h} m_{ik} / sqrt(h), h = 1, 2, 4, .., H, h*k <= K
-      bool first = true;
-      for (int k = 1; k <= K; ++k) {
-        float s = 0.f;
-        int have = 0;  // harmonics summed so far
-        for (int h = 1; h <= p.harmonics && h * k <= K; h *= 2) {
-          for (int i = have + 1; i <= h; ++i) s += p.mag[(size_t)(i * k - 1) * p.nt + t];  // m_k, m_2k, ... in order
-          have = h;
-          const float v = s * rsqrtf((float)h);
-          if (first || v > best) { best = v; kb = k; first = false; }
+      *kb_out = kb;
+      return best;
+    };
+    int kb0;
+    const double Kshift = (double)eta_of(0, &kb0);
+    const int begin = blk * kFinChunk, end = min(p.nt, begin + kFinChunk);
+    double s = 0.0, s2 = 0.0;
+    for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
+      int kb;
+      const float e = eta_of(t, &kb);
+      p.eta[(size_t)b * p.nt + t] = e;
+      p.kstar[(size_t)b * p.nt + t] = kb;
+      const double d = (double)e - Kshift;
+      s += d;
+      s2 += d * d;
+    }
+    block_sum2(s, s2, sh);
+    StatPartial part;
+    part.n = (double)(end - begin); part.s = s; part.s2 = s2;
+    if (p.shard_out) {  // one batch entry; the merged sums leave as (n, mean, M2)
+      if (threadIdx.x == 0) {
+        p.parts[(size_t)b * p.nblk + blk] = part;
+        __threadfence();
+        sh_flag = (atomicAdd(&p.counters[b], 1u) == (unsigned)p.nblk - 1);
+      }
+      __syncthreads();
+      if (sh_flag && threadIdx.x < 32) {
+        __threadfence();
+        double n, a, c;
+        warp_merge_partials(p.parts + (size_t)b * p.nblk, p.nblk, n, a, c);
+        if (threadIdx.x == 0) {
+          const double m = (n > 0.0) ? a / n : 0.0;
+          p.shard_out[0] = n;
+          p.shard_out[1] = Kshift + m;
+          p.shard_out[2] = fmax(c - a * m, 0.0);
+          stats_from_sums(Kshift, n, a, c, &p.mu[b], &p.sigma[b]);  // the shard's own statistics, until the import
+          p.counters[b] = 0;
         }
       }
+      __syncthreads();
+    } else {
+      row_stats_finish(part, Kshift, b, blk, p.nblk, p.parts, p.counters, p.mu, p.sigma, &sh_flag);
     }
-    p.eta[t] = best;
-    p.kstar[t] = kb;
   }
-  __syncthreads();
-  row_stats_block(p.eta, begin, end, 0, p.nblk, p.parts, p.counters, p.mu, p.sigma, sh);
+}
+
+// Global eta statistics from the all-gathered per-shard (n, mean, M2) triples (Chan's merge in shard order).
+__global__ void shard_import_eta_kernel(const double* all, int world, double* mu, double* sigma) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double n = 0.0, mean = 0.0, m2 = 0.0;
+  for (int r = 0; r < world; ++r) chan_merge(n, mean, m2, all[3 * r], all[3 * r + 1], all[3 * r + 2]);
+  mu[0] = mean;
+  sigma[0] = (n > 0.0) ? sqrt(m2 / n) : 0.0;
 }
 
 // ---------------------------------------------------------------------------------------------
-// compact: z-score, strict threshold, ordered compaction (a8).  Cooperative launch: every block
-// counts the candidates of its contiguous segment, grid sync, then writes them at the exclusive
-// prefix of the lower blocks' counts, in (row, tile) order: warp ballot + popc inside a warp,
-// a 32-entry scan across the warps of a block.
+// compact: z-score, strict threshold, ordered compaction (a8), in ONE pass over the grid: a block takes a ticket (so a
+// block with a lower ticket is always already running), counts the candidates of its contiguous range of map entries
+// (warp ballot + popc; every warp owns a contiguous part of the range, so there is no block barrier per iteration),
+// publishes the count, adds up the published counts of all lower tickets (decoupled look-back) and writes its
+// candidates at that offset, in (row, tile) order.  Blocks without candidates -- almost all -- skip the second walk.
 // ---------------------------------------------------------------------------------------------
+struct CompactState {
+  unsigned ticket, done;
+  unsigned long long total;
+};
+
 struct CompactParams {
-  const float* v;       // q [U][nt] (image branch) or eta [1][nt] (frequency branch)
+  const float* v;       // q [B*U][nt] (image branch) or eta [B][nt] (frequency branch)
   const RawTile* raw;   // image branch: argmax positions
   const int* kstar;     // frequency branch
   const double* mu;     // [rows]
   const double* sigma;  // [rows]
   float tau;
-  int rows;             // U or 1
+  int rows;             // B*U or B
+  int rows_per_batch;   // U or 1
   long long nt;         // tiles per row
   int Tx, Ty, H, W, tile, stride, branch;
   int row_offset;       // image row of this context's first row (row shards), added to y
   int unit_offset;      // real-time mode: index of the unit the one-row map belongs to, added to `snapshot`
   fitrig_candidate* out;
   long long cap;        // device capacity of `out`
-  unsigned long long* total;
-  unsigned long long* host_total;  // the same count, in mapped pinned host memory
+  unsigned long long* host_total;  // the count, in mapped pinned host memory
   fitrig_candidate* host_out;      // first host_cap candidates, in mapped pinned host memory
   long long host_cap;
-  unsigned* blk_counts; // [gridDim.x]
-  long long seg;        // entries per block (multiple of blockDim.x)
+  unsigned long long* batch_counts;  // [B] device, zero on entry and on exit
+  unsigned long long* host_counts;   // [B] mapped pinned host memory
+  int B;
+  CompactState* state;               // ticket / done counters, zero on entry and on exit
+  unsigned long long* status;        // [gridDim.x] (epoch << 32) | count of the block with that ticket
+  unsigned epoch;                    // launch number, never 0
+  long long seg;        // entries per block (multiple of 32 * warps)
 };
 
 // z of entry i (Eq. 8 on q, R21; sigma == 0 -> z = 0, R4) and the strict threshold (R6).  1 / sigma of the current
@@ -1068,82 +1230,137 @@ __device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i
 }
 
 __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
-  cg::grid_group grid = cg::this_grid();
-  __shared__ unsigned warp_cnt[32];
-  __shared__ unsigned long long block_base;
-  const long long N = (long long)p.rows * p.nt;
-  const long long begin = min(N, (long long)blockIdx.x * p.seg), end = min(N, begin + p.seg);
+  __shared__ unsigned warp_cnt[16];
+  __shared__ unsigned s_id;
+  __shared__ unsigned long long s_base;
+  __shared__ int s_last;
+  pdl_wait();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  if (threadIdx.x == 0) {
+    s_id = atomicAdd(&p.state->ticket, 1u);
+    s_base = 0;
+  }
+  __syncthreads();
+  const unsigned id = s_id;
+  const long long N = (long long)p.rows * p.nt;
+  const long long begin = min(N, (long long)id * p.seg), end = min(N, begin + p.seg);
+  const long long wlen = p.seg / nw;  // a multiple of 32
+  const long long wb = min(end, begin + warp * wlen), we = min(end, wb + wlen);
 
   RowCache rcache;
   // ---- pass 1: count ----
   unsigned cnt = 0;
-  for (long long i = begin + threadIdx.x; i < end; i += blockDim.x) {
+  for (long long c0 = wb; c0 < we; c0 += 32) {
+    const long long i = c0 + lane;
     float z;
-    cnt += compact_flag(p, i, &z, rcache) ? 1u : 0u;
+    const bool f = (i < we) && compact_flag(p, i, &z, rcache);
+    cnt += __popc(__ballot_sync(0xffffffffu, f));
   }
-  cnt = __reduce_add_sync(0xffffffffu, cnt);
-  if (lane == 0) warp_cnt[warp] = cnt;
+  if (lane == 0) warp_cnt[warp] = cnt;  // (the same in every lane)
   __syncthreads();
+  unsigned before = 0, total = 0;
+  for (int w = 0; w < nw; ++w) {
+    const unsigned cw = warp_cnt[w];
+    if (w < warp) before += cw;
+    total += cw;
+  }
+  // ---- publish, then add up the counts of all lower tickets ----
   if (threadIdx.x == 0) {
-    unsigned t = 0;
-    for (int w = 0; w < nw; ++w) t += warp_cnt[w];
-    p.blk_counts[blockIdx.x] = t;
+    *reinterpret_cast<volatile unsigned long long*>(p.status + id) = ((unsigned long long)p.epoch << 32) | total;
+    __threadfence();
   }
-  grid.sync();
-  // ---- exclusive prefix over lower blocks (integer adds: order free) ----
-  if (threadIdx.x == 0) block_base = 0;
-  __syncthreads();
   unsigned long long below = 0;
-  for (int b = threadIdx.x; b < (int)blockIdx.x; b += blockDim.x) below += p.blk_counts[b];
+  for (long long j = (long long)id - 1 - threadIdx.x; j >= 0; j -= blockDim.x) {
+    unsigned long long v;
+    do {
+      v = *reinterpret_cast<volatile unsigned long long*>(p.status + j);
+    } while ((unsigned)(v >> 32) != p.epoch);
+    below += (unsigned)v;
+  }
   for (int off = 16; off > 0; off >>= 1) below += __shfl_xor_sync(0xffffffffu, below, off);
-  if (lane == 0 && below) atomicAdd(&block_base, below);
+  if (lane == 0 && below) atomicAdd(&s_base, below);
   __syncthreads();
-  if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) {
-    *p.total = block_base + p.blk_counts[blockIdx.x];
-    *p.host_total = block_base + p.blk_counts[blockIdx.x];
-  }
-  unsigned long long running = block_base;
-  // ---- pass 2: write in order, one blockDim.x-wide chunk at a time ----
-  for (long long c0 = begin; c0 < end; c0 += blockDim.x) {
-    const long long i = c0 + threadIdx.x;
-    float z = 0.f;
-    const bool f = (i < end) && compact_flag(p, i, &z, rcache);
-    const unsigned bal = __ballot_sync(0xffffffffu, f);
-    if (lane == 0) warp_cnt[warp] = __popc(bal);
-    __syncthreads();
-    unsigned before = 0, chunk_total = 0;
-    for (int w = 0; w < nw; ++w) {
-      const unsigned cw = warp_cnt[w];
-      if (w < warp) before += cw;
-      chunk_total += cw;
-    }
-    if (f) {
-      const unsigned long long dst = running + before + __popc(bal & ((1u << lane) - 1u));
-      if ((long long)dst < p.cap) {
+  const unsigned long long base = s_base;
+  if (threadIdx.x == 0 && id == gridDim.x - 1) p.state->total = base + total;
+  bool wrote_host = false;
+  // ---- pass 2: write in order (only blocks that hold candidates) ----
+  if (total != 0) {
+    unsigned long long running = base + before;
+    for (long long c0 = wb; c0 < we && cnt != 0; c0 += 32) {
+      const long long i = c0 + lane;
+      float z = 0.f;
+      const bool f = (i < we) && compact_flag(p, i, &z, rcache);
+      const unsigned bal = __ballot_sync(0xffffffffu, f);
+      if (f) {
+        const unsigned long long dst = running + __popc(bal & ((1u << lane) - 1u));
         const int row = rcache.row;  // compact_flag has just placed entry i in its row
-        const unsigned t = (unsigned)(i - (rcache.row_end - p.nt));  // tile index inside the unit (< 2^31)
-        const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
-        fitrig_candidate cd;
-        if (p.branch == FITRIG_BRANCH_IMAGE) {
-          const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
-          cd.x = tx * p.stride + pos % p.tile;
-          cd.y = p.row_offset + ty * p.stride + pos / p.tile;
-          cd.snapshot = row + p.unit_offset;
-        } else {
-          const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
-          cd.x = tx * p.stride + w / 2;  // tile centre (R18)
-          cd.y = p.row_offset + ty * p.stride + h / 2;
-          cd.snapshot = p.kstar[t];
+        const int bidx = row / p.rows_per_batch;
+        if (p.B > 1) atomicAdd(&p.batch_counts[bidx], 1ull);
+        if ((long long)dst < p.cap) {
+          const unsigned t = (unsigned)(i - (rcache.row_end - p.nt));  // tile index inside the row (< 2^31)
+          const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
+          fitrig_candidate cd;
+          if (p.branch == FITRIG_BRANCH_IMAGE) {
+            const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
+            cd.x = tx * p.stride + pos % p.tile;
+            cd.y = p.row_offset + ty * p.stride + pos / p.tile;
+            cd.snapshot = (row - bidx * p.rows_per_batch) + p.unit_offset;
+          } else {
+            const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
+            cd.x = tx * p.stride + w / 2;  // tile centre (R18)
+            cd.y = p.row_offset + ty * p.stride + h / 2;
+            cd.snapshot = p.kstar[i];
+          }
+          cd.score = z;
+          p.out[dst] = cd;
+          if ((long long)dst < p.host_cap) { p.host_out[dst] = cd; wrote_host = true; }
         }
-        cd.score = z;
-        p.out[dst] = cd;
-        if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
       }
+      running += __popc(bal);
     }
-    running += chunk_total;
-    __syncthreads();
   }
+  // ---- the last block to finish resets the counters and hands the counts to the host ----
+  if (__syncthreads_or(wrote_host) && threadIdx.x == 0) __threadfence_system();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    s_last = (atomicAdd(&p.state->done, 1u) == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    for (int b = threadIdx.x; b < p.B; b += blockDim.x) {
+      volatile unsigned long long* bc = p.batch_counts + b;
+      p.host_counts[b] = *bc;
+      *bc = 0ull;
+    }
+    if (threadIdx.x == 0) {
+      const unsigned long long tot = *reinterpret_cast<volatile unsigned long long*>(&p.state->total);
+      if (p.B == 1) p.host_counts[0] = tot;
+      *p.host_total = tot;
+      p.state->ticket = 0u;
+      p.state->done = 0u;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// calibration: what a plain read-only stream of the same buffer achieves on this device (fitrig_probe_read_bandwidth).
+// The roofline denominator of MEASURED_PEAKS.json is a COPY (read + write); a read-only kernel can exceed it.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512) read_probe_kernel(const float4* __restrict__ x, long long n4, float* sink) {
+  float m = -3.402823466e38f;
+  const long long step = (long long)gridDim.x * blockDim.x;
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  for (; i + 3 * step < n4; i += 4 * step) {  // four independent 16-byte loads in flight per thread
+    const float4 a = x[i], b = x[i + step], c = x[i + 2 * step], d = x[i + 3 * step];
+    m = fmaxf(m, fmaxf(fmaxf(fmaxf(a.x, a.y), fmaxf(a.z, a.w)), fmaxf(fmaxf(b.x, b.y), fmaxf(b.z, b.w))));
+    m = fmaxf(m, fmaxf(fmaxf(fmaxf(c.x, c.y), fmaxf(c.z, c.w)), fmaxf(fmaxf(d.x, d.y), fmaxf(d.z, d.w))));
+  }
+  for (; i < n4; i += step) {
+    const float4 a = x[i];
+    m = fmaxf(m, fmaxf(fmaxf(a.x, a.y), fmaxf(a.z, a.w)));
+  }
+  if (m == 1.2345e-30f) *sink = m;  // keeps the loads alive; practically never true
 }
 
 }  // namespace fitrig

@@ -9,10 +9,23 @@
 
 namespace fitrig {
 
-int env_int(const char* name, int dflt) {
+static int env_int(const char* name, int dflt) {
   const char* v = getenv(name);
   if (!v || !*v) return dflt;
   return atoi(v);
+}
+
+Tuning read_tuning_env() {
+  Tuning t;
+  t.box_tiles = env_int("FITRIG_BOX_TILES", 0);
+  t.stages = env_int("FITRIG_STAGES", 0);
+  t.grid = env_int("FITRIG_GRID", 0);
+  t.evict_first = env_int("FITRIG_EVICT_FIRST", 0);
+  t.force_generic = env_int("FITRIG_FORCE_GENERIC", 0);
+  t.no_pitched_copy = env_int("FITRIG_NO_PITCHED_COPY", 0);
+  t.no_pdl = env_int("FITRIG_NO_PDL", 0);
+  t.old_generic = env_int("FITRIG_OLD_GENERIC", 0);
+  return t;
 }
 
 int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, NormParams* out, const char** why) {
@@ -63,6 +76,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
     return FITRIG_ERR_INVALID_ARG;
   }
   out->row_offset = p->row_offset;
+  if (p->batch < 0) { *why = "batch must be >= 1 (0 selects 1)"; return FITRIG_ERR_INVALID_ARG; }
+  out->batch = p->batch == 0 ? 1 : p->batch;
+  if (out->batch > 1 && (p->row_offset != 0 || out->stride != out->tile)) {
+    *why = "batch > 1: no row shards, no overlapping windows";
+    return FITRIG_ERR_INVALID_ARG;
+  }
+  const long long U = (long long)L / out->accumulate - 2;
+  if (p->branch == FITRIG_BRANCH_FREQUENCY && U > 8192) {
+    *why = "frequency branch: at most 8192 units (the twiddle table of the temporal DFT lives in shared memory)";
+    return FITRIG_ERR_INVALID_ARG;
+  }
   return FITRIG_OK;
 }
 
@@ -94,9 +118,9 @@ bool fused_tile(int tile) {
   return tile == 16 || tile == 8 || tile == 4 || tile == 2 || tile == 1 || (tile >= kFastTile && tile % kFastTile == 0);
 }
 
-void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan) {
+void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
-  const bool force_generic = env_int("FITRIG_FORCE_GENERIC", 0) != 0;
+  const bool force_generic = tn.force_generic != 0;
   if (!fused_tile(tile) || (W % 4) != 0 || force_generic) {
     plan->path = 1;
     plan->units_per_cta = 0;
@@ -109,7 +133,7 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* pla
   }
   plan->path = 0;
   const int rows32 = (rows + kFastTile - 1) / kFastTile, Tx32 = (W + kFastTile - 1) / kFastTile;
-  const int fb = env_int("FITRIG_BOX_TILES", 0), fs = env_int("FITRIG_STAGES", 0), fg = env_int("FITRIG_GRID", 0);
+  const int fb = tn.box_tiles, fs = tn.stages, fg = tn.grid;
   int ntw = std::min(kMaxTilesPerBox, Tx32);
   auto pairs = [&](int n) { return (long long)rows32 * ((Tx32 + n - 1) / n) * U; };
   // small problems are latency bound: narrower boxes give more CTAs something to do
@@ -165,8 +189,8 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   out->n_strips = (int32_t)((H + rows - 1) / rows);
   out->n_strip_buffers = out->n_strips >= 3 ? 3 : out->n_strips;
   out->strip_buffer_bytes = (int64_t)L * rows * W * 4;
-  plan_launch(cell, W, H, out->units, num_sms, out);
-  const int64_t n = (int64_t)out->units * out->Ty * out->Tx;
+  plan_launch(cell, W, H, out->units, num_sms, read_tuning_env(), out);
+  const int64_t n = (int64_t)np.batch * out->units * out->Ty * out->Tx;
   out->workspace_bytes = n * (16 + 4 + 4) + (int64_t)out->Ty * out->Tx * 8 + (1 << 20);
   return FITRIG_OK;
 }

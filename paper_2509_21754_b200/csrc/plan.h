@@ -28,7 +28,22 @@ struct NormParams {  // fitrig_params with defaults applied
   int accumulate;  // >= 1
   int harmonics;   // 1, 2, 4, .., 32
   int stride;      // window stride in pixels; == tile: the paper's non-overlapping tiles
+  int batch;       // >= 1 independent stacks per call
 };
+
+// Debug / tuning switches, read from the environment ONCE per fitrig_create / fitrig_plan_query call (documented in
+// include/fitrig.h); 0 = not set.
+struct Tuning {
+  int box_tiles;        // FITRIG_BOX_TILES      fused path: adjacent 32x32 blocks per TMA box (1..8)
+  int stages;           // FITRIG_STAGES         fused path: ring depth
+  int grid;             // FITRIG_GRID           fused path: CTAs
+  int evict_first;      // FITRIG_EVICT_FIRST    fused path: L2 evict_first hint on the streaming loads
+  int force_generic;    // FITRIG_FORCE_GENERIC  always take the generic kernel
+  int no_pitched_copy;  // FITRIG_NO_PITCHED_COPY fitrig_stream: one copy per snapshot instead of one pitched copy per strip
+  int no_pdl;           // FITRIG_NO_PDL         plain launches instead of programmatic dependent launches
+  int old_generic;      // FITRIG_OLD_GENERIC    generic path: the three-reads-per-pixel kernel instead of the time-marching one
+};
+Tuning read_tuning_env();
 
 // What the tLISI kernels reduce (square cells) and how windows are made of cells (see kernels.cuh, merge_cells_kernel):
 // cell == tile and m == 1 in the plain case.
@@ -45,10 +60,8 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 
 // Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
 // `rows`: image rows covered by the launch (the whole image, or one strip).
-void plan_launch(int tile, int W, int rows, int U, int num_sms, fitrig_plan* plan);
+void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan);
 bool fused_tile(int tile);  // N_T the fused kernel serves: 1, 2, 4, 8, 16 (tiles inside a block), 32, and 32 * m (merged blocks)
 
-// Debug/tuning overrides: FITRIG_BOX_TILES, FITRIG_STAGES, FITRIG_GRID, FITRIG_EVICT_FIRST, FITRIG_FORCE_GENERIC (integers).
-int env_int(const char* name, int dflt);
 
 }  // namespace fitrig

@@ -9,7 +9,8 @@ the method stays in the CUDA kernels behind include/fitrig.h:
 * ONE image over several GPUs: horizontal shards of whole tile rows (`row_shards`).  The only coupling is
   the three global scalars of the method -- M and per unit the mean and standard deviation of
   the tile matrix (Eq. 8) -- exchanged in ONE all-gather of 2 + 2U doubles per rank
-  (`ShardedContext.tlisi`), then the candidate lists are gathered and put in (unit, tile row, tile col)
+  (`ShardedContext.tlisi`; the frequency branch adds a second one of 3 doubles for the statistics of eta, which
+  can only be formed once the global M is known), then the candidate lists are gathered and put in (unit, tile row, tile col)
   order (`gather_candidates`, `merge_candidates`: index bookkeeping only).
 """
 from __future__ import annotations
@@ -118,17 +119,38 @@ class ShardedContext:
         self.units = self.ctx.units
         self._vec = None
 
+    def _exchange(self, vec, stream):
+        """All-gather of `vec` (written on `stream`) -> [world, n], safe to read on `stream`: the collective runs on
+        torch's current stream, so the two streams are ordered against each other on both sides."""
+        import torch
+        cur = torch.cuda.current_stream(vec.device) if vec.is_cuda else None
+        lib_stream = None
+        if cur is not None and stream is not None:
+            lib_stream = stream if hasattr(stream, "cuda_stream") else torch.cuda.ExternalStream(int(stream), device=vec.device)
+            if lib_stream.cuda_stream != cur.cuda_stream:
+                cur.wait_stream(lib_stream)  # the export kernel has written vec
+            else:
+                lib_stream = None
+        allv = all_gather_vectors(vec, self.group)
+        if lib_stream is not None:
+            lib_stream.wait_stream(cur)  # the import kernel may not read allv before the collective has delivered it
+        return allv
+
     def tlisi(self, d_stack_rows, d_tlisi=None, stream=None) -> None:
         import torch
         if self._vec is None:
             self._vec = torch.empty(2 + 2 * self.units, dtype=torch.float64, device=d_stack_rows.device)
+            self._vec_eta = torch.empty(3, dtype=torch.float64, device=d_stack_rows.device)
         self.ctx.tlisi(d_stack_rows, None, stream)
         self.ctx.shard_export(self._vec, stream)
-        if stream is not None and hasattr(stream, "synchronize"):
-            stream.synchronize()  # the collective runs on torch's stream
-        allv = all_gather_vectors(self._vec, self.group)
+        allv = self._exchange(self._vec, stream)
         self.ctx.shard_import(allv, allv.shape[0], d_tlisi, stream)
         self._all = allv  # keep alive until the kernel has read it
+        if self.ctx.branch == 1:  # eta scales with 1 / M^2: its statistics need a second, 3-double exchange
+            self.ctx.shard_export_eta(self._vec_eta, stream)
+            alle = self._exchange(self._vec_eta, stream)
+            self.ctx.shard_import_eta(alle, alle.shape[0], stream)
+            self._all_eta = alle
 
     def detect(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None):
         return self.ctx.detect(sigma_threshold, capacity, stream)

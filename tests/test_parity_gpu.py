@@ -673,11 +673,16 @@ def test_shard_calls_argument_and_state_errors():
     with pytest.raises(fitrig.FitrigError) as e:
         fitrig.Context(64, 64, 4, row_offset=16)  # not a multiple of the tile
     assert e.value.code == fitrig.binding.ERR_INVALID_ARG
-    with fitrig.Context(64, 64, 4, branch=fitrig.BRANCH_FREQUENCY) as ctx:
+    with fitrig.Context(64, 64, 4) as ctx:  # the eta exchange belongs to the frequency branch
         ctx.tlisi(synth.gaussian_noise_stack(4, 64, 64, device=DEV))
         with pytest.raises(fitrig.FitrigError) as e:
-            ctx.shard_export(torch.empty(6, dtype=torch.float64, device=DEV))
+            ctx.shard_export_eta(torch.empty(3, dtype=torch.float64, device=DEV))
         assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+    with fitrig.Context(64, 64, 4, branch=fitrig.BRANCH_FREQUENCY) as ctx:
+        ctx.tlisi(synth.gaussian_noise_stack(4, 64, 64, device=DEV))
+        with pytest.raises(fitrig.FitrigError) as e:  # import before export
+            ctx.shard_import_eta(torch.empty(3, dtype=torch.float64, device=DEV), 1)
+        assert e.value.code == fitrig.binding.ERR_STATE
 
 
 # ------------------------------------------------------------------------------------------
