@@ -57,6 +57,7 @@ def parse_args():
     ap.add_argument("--channels", type=int, default=0, help="imgfreq only: use the first N of the 16 channels")
     ap.add_argument("--tile", type=int, default=32, help="N_T (the paper's default and BASELINE.json's is 32)")
     ap.add_argument("--harmonics", type=int, default=1, help="frequency branch: harmonic summing over 1,2,4..H harmonics")
+    ap.add_argument("--width", type=int, default=0, help="override the image width W (e.g. 2050: W % 4 != 0 takes the generic path)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = an independent stack per rank; strong = ONE stack cut into row shards (ShardedContext)")
     ap.add_argument("--no-pipeline", action="store_true", help="end every step with a synchronous fitrig_detect")
@@ -514,6 +515,8 @@ def main():
     TILE, HARMONICS = args.tile, args.harmonics
     import synth
     cfg = synth.CONFIGS[args.workload]
+    if args.width:
+        cfg = cfg.replace(W=args.width, name=f"{cfg.name}_w{args.width}")
     tau = args.tau if args.tau is not None else cfg.tau
     branch = 1 if args.workload in ("imgfreq", "psr_like") else 0
     if args.impl == "reference":

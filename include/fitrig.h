@@ -300,6 +300,10 @@ int fitrig_probe_read_bandwidth(fitrig_ctx* ctx, const void* d_buf, int64_t byte
 /* fitrig_launch_count -- kernels launched by this context since creation (for bench.py's gpu_launches). */
 int fitrig_launch_count(const fitrig_ctx* ctx, int64_t* n);
 
+/* fitrig_copy_count -- host-to-device copy calls issued by this context's fitrig_stream / fitrig_push since creation
+ * (one per strip when the snapshots travel as pitched copies, L per strip otherwise; one per pushed snapshot). */
+int fitrig_copy_count(const fitrig_ctx* ctx, int64_t* n);
+
 /* fitrig_last_error -- thread-local message of the last failing call on this thread; never NULL. */
 const char* fitrig_last_error(void);
 

@@ -116,11 +116,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_profile.argtypes = [vp, i32]
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
+    L.fitrig_copy_count.argtypes = [vp, P(i64)]
     L.fitrig_probe_read_bandwidth.argtypes = [vp, vp, i64, i32, P(f32), vp]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
               "fitrig_tlisi_batch", "fitrig_detect_batch", "fitrig_detect_launch", "fitrig_detect_fetch", "fitrig_shard_export_eta", "fitrig_shard_import_eta",
               "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
-              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_probe_read_bandwidth"):
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_probe_read_bandwidth"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
     L.fitrig_version.restype = ctypes.c_char_p
@@ -372,6 +373,11 @@ class Context:
         _check(self._L.fitrig_probe_read_bandwidth(self._h, d_tensor.data_ptr(), nbytes, int(reps), ctypes.byref(g),
                                                    _stream_ptr(stream)))
         return g.value
+
+    def copy_count(self) -> int:
+        n = ctypes.c_int64()
+        _check(self._L.fitrig_copy_count(self._h, ctypes.byref(n)))
+        return n.value
 
     def launch_count(self) -> int:
         n = ctypes.c_int64()

@@ -78,7 +78,7 @@ struct TmapCache {  // the last TMA descriptor encoded (a resident stack is desc
   bool valid = false;
   const float* base = nullptr;
   long long snap_stride = 0;
-  int rows = 0, nslots = 0, box = 0;
+  int rows = 0, nslots = 0, box = 0, boxh = 0;
   CUtensorMap tm;
 };
 
@@ -123,9 +123,9 @@ struct fitrig_ctx {
   // been queued (fitrig_detect_launch / fitrig_detect_fetch)
   DetectSlot slot[2];
   unsigned long long detect_launched, detect_fetched;
-  CompactState* cstate;
   unsigned long long* cstatus;
-  unsigned long long* batch_counts;
+  unsigned* cticket;
+  unsigned ticket_base;  // tickets drawn by all compaction launches so far (mod 2^32)
   unsigned compact_epoch;
   int compact_grid_max;
   // streaming
@@ -150,6 +150,7 @@ struct fitrig_ctx {
   int fin_used;
   bool have_map;
   long long launches;
+  long long copies;  // host-to-device copy calls issued by fitrig_stream / fitrig_push
 };
 
 static void free_ctx(fitrig_ctx* c) {
@@ -159,8 +160,7 @@ static void free_ctx(fitrig_ctx* c) {
   cudaFree(c->raw); cudaFree(c->raw_blocks); cudaFree(c->q); cudaFree(c->tlisi); cudaFree(c->M_dev); cudaFree(c->gmax_key);
   cudaFree(c->parts); cudaFree(c->counters); cudaFree(c->mu); cudaFree(c->sigma);
   cudaFree(c->eta); cudaFree(c->kstar); cudaFree(c->mag); cudaFree(c->tw); cudaFree(c->sparts); cudaFree(c->scounter);
-  cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cstate); cudaFree(c->cstatus);
-  cudaFree(c->batch_counts);
+  cudaFree(c->smu); cudaFree(c->ssigma); cudaFree(c->cstatus); cudaFree(c->cticket);
   for (DetectSlot& d : c->slot) {
     cudaFree(d.cand_dev);
     if (d.cand_host) cudaFreeHost(d.cand_host);
@@ -339,12 +339,11 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   int occ = 0;
   CTX_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, compact_kernel, 512, 0));
   c->compact_grid_max = std::max(1, occ) * c->num_sms;
-  CTX_TRY(cudaMalloc(&c->cstate, sizeof(CompactState)));
-  CTX_TRY(cudaMemset(c->cstate, 0, sizeof(CompactState)));
+  CTX_TRY(cudaMalloc(&c->cticket, sizeof(unsigned)));
+  CTX_TRY(cudaMemset(c->cticket, 0, sizeof(unsigned)));
+  c->ticket_base = 0;
   CTX_TRY(cudaMalloc(&c->cstatus, sizeof(unsigned long long) * c->compact_grid_max));
   CTX_TRY(cudaMemset(c->cstatus, 0, sizeof(unsigned long long) * c->compact_grid_max));
-  CTX_TRY(cudaMalloc(&c->batch_counts, sizeof(unsigned long long) * c->B));
-  CTX_TRY(cudaMemset(c->batch_counts, 0, sizeof(unsigned long long) * c->B));
   c->compact_epoch = 0;
   for (DetectSlot& d : c->slot) {
     d.cand_cap = kHostStageCands;
@@ -359,6 +358,9 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   if (c->plan.path == 0) {
     CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
+  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
+  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
+  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
 #undef CTX_TRY
   *out = c;
   return FITRIG_OK;
@@ -397,6 +399,27 @@ static int prof_end(fitrig_ctx* c, cudaStream_t st) {
   return FITRIG_OK;
 }
 
+// The TMA descriptor of `nslots` images of rows x W (rows `snap_stride` elements apart per image) with boxes of
+// box x boxh pixels; the last one encoded is kept (a resident stack is described by the same one call after call).
+static int get_tmap(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int nslots, int box, int boxh,
+                    const CUtensorMap** out) {
+  TmapCache& tc = c->tmap;
+  if (!(tc.valid && tc.base == base && tc.snap_stride == snap_stride && tc.rows == rows && tc.nslots == nslots &&
+        tc.box == box && tc.boxh == boxh)) {
+    const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)nslots};
+    const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
+    const cuuint32_t bx[3] = {(cuuint32_t)box, (cuuint32_t)boxh, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = c->encode(&tc.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, bx, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { tc.valid = false; return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r); }
+    tc.valid = true; tc.base = base; tc.snap_stride = snap_stride; tc.rows = rows; tc.nslots = nslots; tc.box = box; tc.boxh = boxh;
+  }
+  *out = &tc.tm;
+  return FITRIG_OK;
+}
+
 // tLISI partial sums of `rows` image rows (all L snapshots) that start at tile row ty_base.
 // base: device pointer to snapshot 0 of those rows; snap_stride: elements between snapshots.
 struct RowsOpt {
@@ -428,19 +451,10 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   int rc = prof_begin(c, st);
   if (rc) return rc;
   if (pl.path == 0) {
-    const int box = pl.box_tiles * kFastTile;
-    TmapCache& tc = c->tmap;
-    if (!(tc.valid && tc.base == base && tc.snap_stride == snap_stride && tc.rows == rows && tc.nslots == nslots && tc.box == box)) {
-      const cuuint64_t gdim[3] = {(cuuint64_t)c->W, (cuuint64_t)rows, (cuuint64_t)nslots};
-      const cuuint64_t gstr[2] = {(cuuint64_t)c->W * 4, (cuuint64_t)snap_stride * 4};
-      const cuuint32_t bx[3] = {(cuuint32_t)box, kFastTile, 1};
-      const cuuint32_t estr[3] = {1, 1, 1};
-      CUresult r = c->encode(&tc.tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)base, gdim, gstr, bx, estr,
-                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) { tc.valid = false; return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r); }
-      tc.valid = true; tc.base = base; tc.snap_stride = snap_stride; tc.rows = rows; tc.nslots = nslots; tc.box = box;
-    }
+    const CUtensorMap* tmp = nullptr;
+    rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
+    if (rc) return rc;
+    const CUtensorMap& tm = *tmp;
     FusedParams fp;
     fp.raw = out_raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; fp.acc = c->prm.accumulate;
@@ -457,9 +471,35 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.C = c->prm.C;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
-      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
-      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tc.tm, fp); break;
+      case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+      case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+      default: launch_fused<FITRIG_REF_FLOOR>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
+    }
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+    if (cells) c->blocks_pending = true;
+  } else if (MarchPlan mp = (c->prm.accumulate == 1 && !c->tune.old_generic)
+                                ? plan_march(tile, c->W, rows, units, c->num_sms, c->tune) : MarchPlan(); mp.ok) {
+    // any cell size / width / alignment, every snapshot byte read once (time-marching through a shared-memory ring)
+    const bool tma = aligned && (c->W % 4 == 0) && mp.x_aligned;
+    const CUtensorMap* tmp = &c->tmap.tm;  // (unused by the cp.async variant)
+    if (tma) {
+      rc = get_tmap(c, base, snap_stride, rows, nslots, mp.bwp, mp.bh, &tmp);
+      if (rc) return rc;
+    }
+    MarchParams q;
+    q.raw = out_raw; q.gmax_key = key; q.base = base; q.snap_stride = snap_stride; q.W = c->W; q.rows = rows;
+    q.Tx = out_Tx; q.Ty = out_Ty; q.ty_base = ty_base; q.ty_end = std::min(out_Ty, ty_base + rows_tiles);
+    q.U = units; q.c = tile; q.ntx = mp.ntx; q.nty = mp.nty; q.bwp = mp.bwp; q.bh = mp.bh; q.ngx = mp.ngx;
+    q.nstage = mp.nstage; q.G = (int)((long long)mp.ngx * mp.ngy * units);
+    q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
+    // cp.async variant: 8-byte copies where every row and box origin allows it, else 4-byte
+    q.vec = (!tma && (uintptr_t)base % 8 == 0 && snap_stride % 2 == 0 && c->W % 2 == 0 && (mp.ntx * tile) % 2 == 0) ? 2 : 1;
+    const dim3 grid(mp.grid), block(32 * (kMarchWarps + (tma ? 1 : kMarchProducers)));
+    switch (c->prm.ref_mode) {
+      case FITRIG_REF_ABS: tlisi_march_kernel<FITRIG_REF_ABS><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
+      case FITRIG_REF_LITERAL: tlisi_march_kernel<FITRIG_REF_LITERAL><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
+      default: tlisi_march_kernel<FITRIG_REF_FLOOR><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;
@@ -601,12 +641,14 @@ static int stream_strips(fitrig_ctx* c, const float* const* h_snapshots, cudaStr
         pitched = false;
       } else {
         CUDA_TRY(e2);
+        c->copies++;
       }
     }
     if (!pitched) {
       for (int s = 0; s < c->L; ++s) {  // snapshot s, rows r0..r0+rows: contiguous on both sides
         CUDA_TRY(cudaMemcpyAsync(c->strip_buf[b] + (long long)s * snap_stride, h_snapshots[s] + (long long)r0 * c->W,
                                  sizeof(float) * (long long)rows * c->W, cudaMemcpyHostToDevice, c->copy_stream));
+        c->copies++;
       }
     }
     CUDA_TRY(cudaEventRecord(c->ev_copied[b], c->copy_stream));
@@ -756,8 +798,8 @@ static int detect_launch_core(fitrig_ctx* c, float tau, int64_t capacity, void* 
   cp.host_total = reinterpret_cast<unsigned long long*>(d.cand_host_dev);
   cp.host_out = reinterpret_cast<fitrig_candidate*>(d.cand_host_dev + sizeof(CandHeader));
   cp.host_cap = std::min<long long>(cp.cap, kHostStageCands);
-  cp.batch_counts = c->batch_counts; cp.host_counts = d.counts_host_dev; cp.B = c->B;
-  cp.state = c->cstate; cp.status = c->cstatus;
+  cp.host_offsets = d.counts_host_dev; cp.B = c->B;
+  cp.status = c->cstatus; cp.ticket = c->cticket; cp.ticket_base = c->ticket_base;
   if (++c->compact_epoch == 0) c->compact_epoch = 1;
   cp.epoch = c->compact_epoch;
   const int threads = 512;
@@ -766,6 +808,7 @@ static int detect_launch_core(fitrig_ctx* c, float tau, int64_t capacity, void* 
   grid = std::max(grid, 1);
   cp.seg = ((N + grid - 1) / grid + threads - 1) / threads * threads;
   CUDA_TRY(launch_chain(compact_kernel, dim3(grid), dim3(threads), 0, st, !c->tune.no_pdl, cp));
+  c->ticket_base += (unsigned)grid;
   c->launches++;
   CUDA_TRY(cudaEventRecord(d.done, st));
   d.stream = st; d.pending = true; d.cap = cp.cap; d.host_cap = cp.host_cap;
@@ -792,8 +835,12 @@ static int detect_fetch_core(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_
                         sizeof(fitrig_candidate) * (nwrite - n1), cudaMemcpyDeviceToHost));
   }
   *n_found = total;
-  if (n_per_stack)
-    for (int b = 0; b < c->B; ++b) n_per_stack[b] = (int64_t)d.counts_host[b];
+  if (n_per_stack)  // the kernel reports how many candidates precede each stack; the counts are the differences
+    for (int b = 0; b < c->B; ++b) {
+      const long long lo = b == 0 ? 0 : (long long)d.counts_host[b];
+      const long long hi = b + 1 < c->B ? (long long)d.counts_host[b + 1] : total;
+      n_per_stack[b] = hi - lo;
+    }
   if (total > d.cap)
     return fail(FITRIG_ERR_CAPACITY, "fitrig_detect: %lld candidates, capacity %lld", total, (long long)d.cap);
   return FITRIG_OK;
@@ -807,7 +854,10 @@ extern "C" int fitrig_push_reset(fitrig_ctx* c) {
   CUDA_TRY(cudaSetDevice(c->prm.device));
   CUDA_TRY(cudaDeviceSynchronize());
   if (c->push_key) CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
-  if (c->push_ring) CUDA_TRY(cudaMemset(c->raw, 0, sizeof(RawTile) * c->nmap));  // an empty cube
+  if (c->push_ring) {  // an empty cube
+    CUDA_TRY(cudaMemset(c->raw, 0, sizeof(RawTile) * c->nmap));
+    if (c->raw_blocks) CUDA_TRY(cudaMemset(c->raw_blocks, 0, sizeof(RawTile) * (size_t)c->B * c->U * c->Cy * c->Cx));
+  }
   c->push_count = 0;
   c->push_next = 0;
   for (int i = 0; i < kPushSlots; ++i) c->push_free_pending[i] = false;
@@ -819,8 +869,8 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
   if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: ctx is NULL");
   if (!n_found || !unit) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: n_found or unit is NULL");
   const bool freq = c->prm.branch == FITRIG_BRANCH_FREQUENCY;
-  if (c->prm.accumulate != 1 || c->B != 1 || c->geo.m != 1)
-    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: no accumulation, no batch, tiles of 1 .. 32 pixels or generic sizes");
+  if (c->prm.accumulate != 1 || c->B != 1 || c->prm.stride != c->prm.tile)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: no accumulation, no batch, no overlapping windows");
   if (!freq && c->L != 3)
     return fail(FITRIG_ERR_INVALID_ARG, "fitrig_push: image branch: create the context with n_snapshots = 3 (one unit per push)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -831,6 +881,7 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
     CUDA_TRY(cudaMalloc(&c->push_key, sizeof(unsigned)));
     CUDA_TRY(cudaMemset(c->push_key, 0, sizeof(unsigned)));
     CUDA_TRY(cudaMemset(c->raw, 0, sizeof(RawTile) * c->nmap));
+    if (c->raw_blocks) CUDA_TRY(cudaMemset(c->raw_blocks, 0, sizeof(RawTile) * (size_t)c->B * c->U * c->Cy * c->Cx));
     for (int i = 0; i < kPushSlots; ++i) {
       CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_copied[i], cudaEventDisableTiming));
       CUDA_TRY(cudaEventCreateWithFlags(&c->ev_push_free[i], cudaEventDisableTiming));
@@ -848,6 +899,7 @@ extern "C" int fitrig_push(fitrig_ctx* c, const float* snapshot, float tau, floa
     if (c->push_free_pending[slot]) CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_push_free[slot], 0));
     CUDA_TRY(cudaMemcpyAsync(c->push_ring + (long long)slot * img, snapshot, sizeof(float) * img, cudaMemcpyDefault,
                              c->copy_stream));
+    c->copies++;
     CUDA_TRY(cudaEventRecord(c->ev_push_copied[slot], c->copy_stream));
   }
   // (2) ... while the unit whose three snapshots were pushed BEFORE this call is computed (Fig. 14: copy of
@@ -1083,5 +1135,11 @@ extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int
 extern "C" int fitrig_launch_count(const fitrig_ctx* c, int64_t* n) {
   if (!c || !n) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_launch_count: NULL argument");
   *n = c->launches;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_copy_count(const fitrig_ctx* c, int64_t* n) {
+  if (!c || !n) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_copy_count: NULL argument");
+  *n = c->copies;
   return FITRIG_OK;
 }

@@ -751,6 +751,241 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Time-marching kernel for ANY cell size and ANY width / alignment (the generic path).  Same structure as the fused
+// kernel -- persistent CTAs, a producer warp that fills a ring of boxes guarded by full / empty mbarriers, every
+// snapshot byte read from HBM once, the global maximum folded in -- but nothing is held in registers across time
+// steps: the ring keeps the three snapshots of the current unit in shared memory and the consumers read each pixel
+// three times from there (shared-memory bandwidth is plentiful), so threads can be mapped to pixels per tile
+// geometry at run time:
+//   c <= 32  a warp takes floor(32 / c) adjacent tiles at once: lane = column, a loop over the c rows, then a segmented
+//            shuffle reduction over each tile's c lanes (consecutive lanes read consecutive words: conflict free)
+//   c  > 32  a warp takes one tile, lanes stride over its pixels in row-major order, then a whole-warp butterfly
+// A box is nty x ntx whole cells.  Aligned images (16-byte base and strides, W % 4 == 0) are fetched by TMA (box
+// coordinates are element-granular, so cell columns need no alignment); anything else by 4-byte cp.async copies
+// of the producer warp (zero fill outside the image, completion on the same mbarrier).
+// ---------------------------------------------------------------------------------------------
+constexpr int kMarchWarps = 16;      // consumer warps (their only state across iterations is a handful of registers)
+constexpr int kMarchProducers = 4;   // producer warps of the cp.async variant (the TMA variant needs one lane)
+
+struct MarchParams {
+  RawTile* raw;          // [U][Ty][Tx]
+  unsigned* gmax_key;
+  const float* base;
+  long long snap_stride;
+  int W, rows;           // image width; rows covered by this launch
+  int Tx, Ty, ty_base, ty_end;
+  int U;
+  int c;                 // cell edge in pixels
+  int ntx, nty;          // cells per box
+  int bwp, bh;           // box width (floats, a multiple of 4) and height
+  int ngx;               // boxes per row of boxes
+  int nstage, G;
+  int z0, zmask;
+  int tma;               // 1: TMA boxes, 0: cp.async copies
+  int vec;               // cp.async variant: floats per copy (1 or 2)
+  float C;
+};
+
+__device__ __forceinline__ void cp_async4_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+template <int REF_MODE>
+__global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
+    tlisi_march_kernel(const __grid_constant__ CUtensorMap tmap, const MarchParams p) {
+  extern __shared__ __align__(1024) unsigned char smem[];
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+  const int box_floats = p.bh * p.bwp, box_bytes = box_floats * 4;
+  const int slot_bytes = (box_bytes + 127) & ~127;  // TMA destinations are 128-byte aligned
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)p.nstage * slot_bytes);
+  uint64_t* empty = full + kMaxStages;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < p.nstage; ++i) {
+      mbar_init(smem_u32(&full[i]), p.tma ? 1 : 32 * kMarchProducers);
+      mbar_init(smem_u32(&empty[i]), kMarchWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_launch_dependents();
+  const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
+  const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
+  const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty), ring_addr = smem_u32(smem);
+  // the segment walk of the fused kernel, with boxes of cells: group = box, box-major / time-minor
+  auto decode = [&](int g, int& gx, int& gy, int& u0, int& nsteps) {
+    const int group = g / p.U;
+    u0 = g - group * p.U;
+    gy = group / p.ngx;
+    gx = group - gy * p.ngx;
+    nsteps = min(p.U - u0, g_end - g) + 2;
+  };
+
+  if (warp >= kMarchWarps) {
+    // ---- producers: one lane (TMA), or kMarchProducers warps that share the rows of a box (cp.async) ----
+    const int pw = warp - kMarchWarps;
+    unsigned pos = 0;  // snapshots fetched so far: ring position
+    for (int g = g_begin; g < g_end;) {
+      int gx, gy, u0, nsteps;
+      decode(g, gx, gy, u0, nsteps);
+      g += nsteps - 2;
+      const int x0 = gx * p.ntx * p.c, y0 = gy * p.nty * p.c;
+      for (int s = 0; s < nsteps; ++s, ++pos) {
+        const int slot = pos % p.nstage;
+        const uint32_t phase = (pos / p.nstage) & 1;
+        const int z = ring_slot(p.z0, p.zmask, u0 + s);
+        if (p.tma) {
+          if (pw == 0 && lane == 0) {
+            mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
+            mbar_arrive_expect_tx(full_addr + slot * 8, box_bytes);
+            tma_load_box(ring_addr + slot * slot_bytes, &tmap, full_addr + slot * 8, x0, y0, z);
+          }
+        } else {
+          mbar_wait(empty_addr + slot * 8, phase ^ 1);
+          const float* src = p.base + (long long)z * p.snap_stride;
+          const uint32_t dst = ring_addr + slot * slot_bytes;
+          for (int r = pw; r < p.bh; r += kMarchProducers) {  // rows of the box, dealt out to the producer warps
+            const int y = y0 + r;
+            const float* row = src + (long long)y * p.W + x0;
+            const uint32_t drow = dst + r * p.bwp * 4;
+            if (p.vec == 2) {
+              for (int col = 2 * lane; col < p.bwp; col += 64) {
+                const int left = (y < p.rows) ? min(2, p.W - (x0 + col)) : 0;  // floats inside the image
+                cp_async8_zfill(drow + col * 4, left > 0 ? row + col : src, left > 0 ? 4 * left : 0);
+              }
+            } else {
+              for (int col = lane; col < p.bwp; col += 32) {
+                const bool in = (y < p.rows) && (x0 + col < p.W);
+                cp_async4_zfill(drow + col * 4, in ? row + col : src, in ? 4 : 0);
+              }
+            }
+          }
+          cp_async_mbar_arrive_noinc(full_addr + slot * 8);  // arrives once this lane's copies have landed
+        }
+      }
+    }
+    if (!p.tma) cp_async_wait_all();
+    return;
+  }
+
+  // ---- consumers ----
+  const int c = p.c;
+  const bool small = c <= 32;
+  const int gt = small ? 32 / c : 1;                       // tiles per warp item
+  const int ngroups = small ? (p.ntx + gt - 1) / gt : p.ntx;
+  const int nitems = p.nty * ngroups;
+  const int jt = small ? lane / c : 0, cc0 = small ? lane - jt * c : 0;  // this lane's tile in the group, column in it
+  float gmax = -3.402823466e38f;
+  unsigned pos = 0;
+  const long long raw_step = (long long)p.Ty * p.Tx;
+  for (int g = g_begin; g < g_end;) {
+    int gx, gy, u0, nsteps;
+    decode(g, gx, gy, u0, nsteps);
+    g += nsteps - 2;
+    const int nunits = nsteps - 2;
+    // the first two snapshots of the segment
+    mbar_wait(full_addr + (pos % p.nstage) * 8, (pos / p.nstage) & 1);
+    mbar_wait(full_addr + ((pos + 1) % p.nstage) * 8, ((pos + 1) / p.nstage) & 1);
+    for (int i = 0; i < nunits; ++i) {
+      const unsigned pc = pos + i + 2;
+      mbar_wait(full_addr + (pc % p.nstage) * 8, (pc / p.nstage) & 1);
+      const float* A = reinterpret_cast<const float*>(smem + (size_t)((pos + i) % p.nstage) * slot_bytes);
+      const float* B = reinterpret_cast<const float*>(smem + (size_t)((pos + i + 1) % p.nstage) * slot_bytes);
+      const float* Cc = reinterpret_cast<const float*>(smem + (size_t)(pc % p.nstage) * slot_bytes);
+      RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
+      for (int item = warp; item < nitems; item += kMarchWarps) {
+        const int r = item / ngroups, gi = item - r * ngroups;
+        const int ty = p.ty_base + gy * p.nty + r;
+        float S = 0.f, R = 0.f, Mx = 0.f;
+        int mpos = 0;
+        if (small) {
+          const int tcol = gi * gt + jt;                    // tile column inside the box
+          const bool lane_ok = jt < gt && tcol < p.ntx;
+          const float* a = A + (size_t)(r * c) * p.bwp + (lane_ok ? tcol * c + cc0 : 0);
+          const float* b = B + (a - A);
+          const float* cv = Cc + (a - A);
+          bool first = true;
+#pragma unroll 4
+          for (int rr = 0; rr < c; ++rr) {
+            const float xa = a[rr * p.bwp], xb = b[rr * p.bwp], xc = cv[rr * p.bwp];
+            const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
+            S += delta;
+            R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
+            if (first || delta > Mx) { Mx = delta; mpos = rr * c + cc0; first = false; }
+            gmax = fmaxf(gmax, xc);
+            if (i == 0) gmax = fmaxf(gmax, fmaxf(xa, xb));
+          }
+          // segmented reduction over the c lanes of each tile (fixed tree order: deterministic)
+          for (int off = 1; off < c; off <<= 1) {
+            const float oS = __shfl_down_sync(0xffffffffu, S, off), oR = __shfl_down_sync(0xffffffffu, R, off);
+            const float om = __shfl_down_sync(0xffffffffu, Mx, off);
+            const int op = __shfl_down_sync(0xffffffffu, mpos, off);
+            if (cc0 + off < c) {
+              S += oS; R += oR;
+              if (om > Mx || (om == Mx && op < mpos)) { Mx = om; mpos = op; }
+            }
+          }
+          const int tx = gx * p.ntx + tcol;
+          if (lane_ok && cc0 == 0 && ty < p.ty_end && tx < p.Tx) {
+            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
+            rawu[(long long)ty * p.Tx + tx] = o;
+          }
+        } else {
+          const int tcol = gi;
+          const size_t org = (size_t)(r * c) * p.bwp + tcol * c;
+          int rr = 0, cc = lane;  // c > 32: no wrap needed at the start
+          bool first = true;
+          const int n = c * c;
+#pragma unroll 4
+          for (int k = lane; k < n; k += 32) {
+            const size_t o = org + (size_t)rr * p.bwp + cc;
+            const float xa = A[o], xb = B[o], xc = Cc[o];
+            const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));
+            S += delta;
+            R += clamped_ratio<REF_MODE>(delta, xb, p.C);
+            if (first || delta > Mx) { Mx = delta; mpos = k; first = false; }  // k = rr * c + cc, ascending per lane
+            gmax = fmaxf(gmax, xc);
+            if (i == 0) gmax = fmaxf(gmax, fmaxf(xa, xb));
+            cc += 32;
+            if (cc >= c) { cc -= c; ++rr; }
+          }
+          if (first) mpos = 0x7fffffff;  // (a lane without pixels: c * c < 32 cannot happen for c > 32)
+#pragma unroll
+          for (int off = 16; off > 0; off >>= 1) {
+            S += __shfl_xor_sync(0xffffffffu, S, off);
+            R += __shfl_xor_sync(0xffffffffu, R, off);
+            const float om = __shfl_xor_sync(0xffffffffu, Mx, off);
+            const int op = __shfl_xor_sync(0xffffffffu, mpos, off);
+            if (om > Mx || (om == Mx && op < mpos)) { Mx = om; mpos = op; }
+          }
+          const int tx = gx * p.ntx + tcol;
+          if (lane == 0 && ty < p.ty_end && tx < p.Tx) {
+            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
+            rawu[(long long)ty * p.Tx + tx] = o;
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty_addr + ((pos + i) % p.nstage) * 8);  // snapshot u0 + i is not needed again
+    }
+    __syncwarp();
+    if (lane == 0) {
+      mbar_arrive(empty_addr + ((pos + nunits) % p.nstage) * 8);
+      mbar_arrive(empty_addr + ((pos + nunits + 1) % p.nstage) * 8);
+    }
+    pos += nsteps;
+  }
+  const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
+  if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
+}
+
 // Global maximum over the n pixels of one image (generic path; the fused path folds this into its single
 // pass): the image is the sum of `acc` raw snapshots `stride` elements apart, added in order.
 __global__ void __launch_bounds__(256) stack_max_kernel(const float* __restrict__ x, long long n, int acc, long long stride,
@@ -1164,17 +1399,13 @@ __global__ void shard_import_eta_kernel(const double* all, int world, double* mu
 }
 
 // ---------------------------------------------------------------------------------------------
-// compact: z-score, strict threshold, ordered compaction (a8), in ONE pass over the grid: a block takes a ticket (so a
-// block with a lower ticket is always already running), counts the candidates of its contiguous range of map entries
-// (warp ballot + popc; every warp owns a contiguous part of the range, so there is no block barrier per iteration),
-// publishes the count, adds up the published counts of all lower tickets (decoupled look-back) and writes its
-// candidates at that offset, in (row, tile) order.  Blocks without candidates -- almost all -- skip the second walk.
+// compact: z-score, strict threshold, ordered compaction (a8), in ONE pass over the grid: a block counts the candidates
+// of its contiguous range of map entries (warp ballot + popc; every warp owns a contiguous part of the range, so there
+// is no block barrier per iteration), publishes the count, adds up the published counts of all lower blocks
+// (decoupled look-back; blocks take their place in the order from a ticket, so every lower block is running) and writes
+// its candidates at that offset, in (row, tile) order.  Blocks without candidates -- almost all -- skip the second
+// walk.  The chain is four dependent memory round trips: ticket, entries, publish, look-back.
 // ---------------------------------------------------------------------------------------------
-struct CompactState {
-  unsigned ticket, done;
-  unsigned long long total;
-};
-
 struct CompactParams {
   const float* v;       // q [B*U][nt] (image branch) or eta [B][nt] (frequency branch)
   const RawTile* raw;   // image branch: argmax positions
@@ -1193,11 +1424,11 @@ struct CompactParams {
   unsigned long long* host_total;  // the count, in mapped pinned host memory
   fitrig_candidate* host_out;      // first host_cap candidates, in mapped pinned host memory
   long long host_cap;
-  unsigned long long* batch_counts;  // [B] device, zero on entry and on exit
-  unsigned long long* host_counts;   // [B] mapped pinned host memory
+  unsigned long long* host_offsets;  // [B] mapped pinned host memory: candidates that precede stack b (b >= 1; [0] unused)
   int B;
-  CompactState* state;               // ticket / done counters, zero on entry and on exit
   unsigned long long* status;        // [gridDim.x] (epoch << 32) | count of the block with that ticket
+  unsigned* ticket;                  // never reset: every launch draws gridDim.x tickets, the host keeps the running base
+  unsigned ticket_base;
   unsigned epoch;                    // launch number, never 0
   long long seg;        // entries per block (multiple of 32 * warps)
 };
@@ -1231,14 +1462,15 @@ __device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i
 
 __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   __shared__ unsigned warp_cnt[16];
-  __shared__ unsigned s_id;
   __shared__ unsigned long long s_base;
-  __shared__ int s_last;
+  __shared__ unsigned s_id;
   pdl_wait();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  // a block's place in the order is the ticket it draws, so a block with a lower place is always already running
+  // (block indices carry no such guarantee when other kernels share the device)
   if (threadIdx.x == 0) {
-    s_id = atomicAdd(&p.state->ticket, 1u);
     s_base = 0;
+    s_id = atomicAdd(p.ticket, 1u) - p.ticket_base;
   }
   __syncthreads();
   const unsigned id = s_id;
@@ -1264,11 +1496,9 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
     if (w < warp) before += cw;
     total += cw;
   }
-  // ---- publish, then add up the counts of all lower tickets ----
-  if (threadIdx.x == 0) {
+  // ---- publish, then add up the counts of all lower blocks ----
+  if (threadIdx.x == 0)
     *reinterpret_cast<volatile unsigned long long*>(p.status + id) = ((unsigned long long)p.epoch << 32) | total;
-    __threadfence();
-  }
   unsigned long long below = 0;
   for (long long j = (long long)id - 1 - threadIdx.x; j >= 0; j -= blockDim.x) {
     unsigned long long v;
@@ -1281,22 +1511,43 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   if (lane == 0 && below) atomicAdd(&s_base, below);
   __syncthreads();
   const unsigned long long base = s_base;
-  if (threadIdx.x == 0 && id == gridDim.x - 1) p.state->total = base + total;
-  bool wrote_host = false;
-  // ---- pass 2: write in order (only blocks that hold candidates) ----
-  if (total != 0) {
+  if (threadIdx.x == 0 && id == gridDim.x - 1) *p.host_total = base + total;
+  // ---- stacks of a batch: how many candidates precede the first entry of stack b (the host takes differences) ----
+  if (p.B > 1 && warp == 0) {
+    const long long per = (long long)p.rows_per_batch * p.nt;  // entries per stack
+    for (long long b = (begin + per - 1) / per; b < p.B && b * per < end; ++b) {
+      if (b == 0) continue;
+      const long long edge = b * per;  // begin <= edge < end
+      unsigned long long c = base;
+      for (int w = 0; w < nw; ++w) {   // whole warps below the edge, then a recount inside the one that holds it
+        const long long swb = min(end, begin + w * wlen), swe = min(end, swb + wlen);
+        if (swe <= edge) { c += warp_cnt[w]; continue; }
+        if (swb >= edge) break;
+        RowCache rc2;
+        for (long long c0 = swb; c0 < edge; c0 += 32) {
+          const long long i = c0 + lane;
+          float z;
+          const bool f = (i < edge) && compact_flag(p, i, &z, rc2);
+          c += __popc(__ballot_sync(0xffffffffu, f));
+        }
+        break;
+      }
+      if (lane == 0) p.host_offsets[b] = c;
+    }
+  }
+  // ---- pass 2: write in order (only warps that hold candidates) ----
+  if (cnt != 0) {
     unsigned long long running = base + before;
-    for (long long c0 = wb; c0 < we && cnt != 0; c0 += 32) {
+    for (long long c0 = wb; c0 < we; c0 += 32) {
       const long long i = c0 + lane;
       float z = 0.f;
       const bool f = (i < we) && compact_flag(p, i, &z, rcache);
       const unsigned bal = __ballot_sync(0xffffffffu, f);
       if (f) {
         const unsigned long long dst = running + __popc(bal & ((1u << lane) - 1u));
-        const int row = rcache.row;  // compact_flag has just placed entry i in its row
-        const int bidx = row / p.rows_per_batch;
-        if (p.B > 1) atomicAdd(&p.batch_counts[bidx], 1ull);
         if ((long long)dst < p.cap) {
+          const int row = rcache.row;  // compact_flag has just placed entry i in its row
+          const int bidx = row / p.rows_per_batch;
           const unsigned t = (unsigned)(i - (rcache.row_end - p.nt));  // tile index inside the row (< 2^31)
           const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
           fitrig_candidate cd;
@@ -1313,32 +1564,10 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
           }
           cd.score = z;
           p.out[dst] = cd;
-          if ((long long)dst < p.host_cap) { p.host_out[dst] = cd; wrote_host = true; }
+          if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
         }
       }
       running += __popc(bal);
-    }
-  }
-  // ---- the last block to finish resets the counters and hands the counts to the host ----
-  if (__syncthreads_or(wrote_host) && threadIdx.x == 0) __threadfence_system();
-  if (threadIdx.x == 0) {
-    __threadfence();
-    s_last = (atomicAdd(&p.state->done, 1u) == gridDim.x - 1);
-  }
-  __syncthreads();
-  if (s_last) {
-    __threadfence();
-    for (int b = threadIdx.x; b < p.B; b += blockDim.x) {
-      volatile unsigned long long* bc = p.batch_counts + b;
-      p.host_counts[b] = *bc;
-      *bc = 0ull;
-    }
-    if (threadIdx.x == 0) {
-      const unsigned long long tot = *reinterpret_cast<volatile unsigned long long*>(&p.state->total);
-      if (p.B == 1) p.host_counts[0] = tot;
-      *p.host_total = tot;
-      p.state->ticket = 0u;
-      p.state->done = 0u;
     }
   }
 }

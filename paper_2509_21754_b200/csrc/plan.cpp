@@ -97,9 +97,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // SM are about 3x the HBM latency-bandwidth product (~65 KB per SM).
 CellGeom cell_geom(int tile, int stride) {
   CellGeom g;
-  if (stride == tile) {  // non-overlapping: tiles of 32 * m pixels are m x m blocks of 32, everything else is its own cell
-    if (tile > kFastTile && tile % kFastTile == 0) { g.cell = kFastTile; g.m = tile / kFastTile; g.step = g.m; }
-    else { g.cell = tile; g.m = 1; g.step = 1; }
+  if (stride == tile) {
+    // non-overlapping: tiles of 32 * m pixels are m x m blocks of 32; a tile with a divisor of 16, 8 or 4 pixels (12, 24,
+    // 48, 100 ...) is m x m cells of that size, which the fused kernel reduces at (nearly) the rate of a plain read;
+    // everything else (5, 7, 9, 10 ...) is its own cell and takes the generic time-marching kernel
+    g.cell = tile; g.m = 1; g.step = 1;
+    if (!fused_tile(tile)) {
+      for (int d = 16; d >= 4; d >>= 1)
+        if (tile % d == 0) { g.cell = d; g.m = tile / d; g.step = g.m; break; }
+    } else if (tile > kFastTile) {
+      g.cell = kFastTile; g.m = tile / kFastTile; g.step = g.m;
+    }
   } else if (stride % kFastTile == 0) {
     g.cell = kFastTile; g.m = tile / kFastTile; g.step = stride / kFastTile;
   } else {
@@ -155,6 +163,44 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn
   plan->grid = grid;
   plan->units_per_cta = (int32_t)((G + grid - 1) / grid);
   plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + scratch;  // ring, mbarriers, scratch
+}
+
+MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn) {
+  MarchPlan m;
+  memset(&m, 0, sizeof(m));
+  if (num_sms <= 0) num_sms = 148;
+  if (c < 1 || c > kMarchMaxCell || U < 1) return m;
+  const int cells_x = (W + c - 1) / c, cells_y = (rows + c - 1) / c;
+  auto width = [&](int ntx) { return (ntx * c + 3) / 4 * 4; };
+  int ntx = std::max(1, std::min(cells_x, 256 / c));
+  while (ntx > 1 && (width(ntx) > 256 || (long long)width(ntx) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
+  // boxes of about 32 KB (the fused kernel's box): long rows for HBM, several boxes in flight per SM
+  int nty = std::max(1, std::min(cells_y, (32 * 1024) / (width(ntx) * 4 * c)));
+  nty = std::max(1, std::min(nty, 256 / c));
+  auto pairs = [&](int nx, int ny) { return (long long)((cells_x + nx - 1) / nx) * ((cells_y + ny - 1) / ny) * U; };
+  // small problems are latency bound: smaller boxes give more CTAs something to do
+  while ((pairs(ntx, nty) + kMinUnitsPerCta - 1) / kMinUnitsPerCta < num_sms && (nty > 1 || ntx > 1)) {
+    if (nty > 1) nty = (nty + 1) / 2;
+    else ntx = (ntx + 1) / 2;
+  }
+  // box columns start at multiples of ntx * c pixels: keep them on 16-byte boundaries where the cell size allows
+  // (TMA faults on other box origins; where it cannot be had the kernel copies with cp.async instead, see x_aligned)
+  const int qx = 4 / std::gcd(c, 4);
+  if (ntx < cells_x && ntx >= qx) ntx = ntx / qx * qx;
+  m.x_aligned = (ntx >= cells_x) || ((ntx * c) % 4 == 0);
+  m.ntx = ntx; m.nty = nty; m.bwp = width(ntx); m.bh = nty * c;
+  m.ngx = (cells_x + ntx - 1) / ntx; m.ngy = (cells_y + nty - 1) / nty;
+  const int slot = (m.bh * m.bwp * 4 + 127) / 128 * 128;
+  int stages = std::min(kMaxStages, (kMaxSmemPerCta - 2048) / slot);
+  if (tn.stages > 0) stages = std::min(stages, std::max(4, tn.stages));
+  if (stages < 4) return m;  // three snapshots in use + one in flight
+  m.nstage = stages;
+  const long long G = pairs(ntx, nty);
+  m.grid = (int)std::max<long long>(1, std::min<long long>(num_sms, (G + kMinUnitsPerCta - 1) / kMinUnitsPerCta));
+  if (tn.grid > 0) m.grid = tn.grid;
+  m.smem_bytes = stages * slot + 2 * kMaxStages * 8;
+  m.ok = G <= 0x7fffffffll;
+  return m;
 }
 
 }  // namespace fitrig

@@ -61,6 +61,17 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
 // `rows`: image rows covered by the launch (the whole image, or one strip).
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan);
+// Generic time-marching kernel (kernels.cuh, tlisi_march_kernel): boxes of nty x ntx whole cells of c pixels.
+constexpr int kMarchMaxCell = 112;     // the ring needs >= 4 boxes of c x c floats in shared memory
+struct MarchPlan {
+  bool ok;        // false: the cell is too large for the ring (the caller takes the three-reads-per-pixel kernel)
+  int ntx, nty;   // cells per box
+  int bwp, bh;    // box width (floats, multiple of 4, <= 256) and height (<= 256)
+  int ngx, ngy;   // boxes per row of boxes, rows of boxes
+  int nstage, grid, smem_bytes;
+  bool x_aligned; // every box starts on a 16-byte boundary of its row (a condition for fetching it by TMA)
+};
+MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn);
 bool fused_tile(int tile);  // N_T the fused kernel serves: 1, 2, 4, 8, 16 (tiles inside a block), 32, and 32 * m (merged blocks)
 
 

@@ -34,7 +34,9 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert (p.Ty, p.Tx, p.path) == (32, 32, 0) and p.strip_rows % 32 == 0  # N_T = 8, 16 ride the fused kernel
     assert fitrig.plan_query(250, 252, 8, tile=16).path == 0
     assert fitrig.plan_query(250, 252, 8, tile=64).path == 0 and fitrig.plan_query(250, 252, 8, tile=96).path == 0  # 32 * m
-    assert fitrig.plan_query(250, 252, 8, tile=5).path == 1 and fitrig.plan_query(250, 252, 8, tile=48).path == 1
+    assert fitrig.plan_query(250, 252, 8, tile=5).path == 1 and fitrig.plan_query(250, 252, 8, tile=7).path == 1
+    # tiles with a divisor of 16, 8 or 4 pixels are m x m cells of that size on the fused kernel
+    assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (12, 24, 48, 100))
     assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (1, 2, 4))  # tiles inside a lane's quads
     p = fitrig.plan_query(256, 250, 8)
     assert p.path == 1  # W % 4 != 0: rows are not 16-byte aligned, no TMA

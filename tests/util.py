@@ -130,12 +130,33 @@ def accumulation_slack(raw: np.ndarray, g: int):
     return e[:-2] + 2.0 * e[1:-1] + e[2:]
 
 
+def min_tile_pixels(H: int, W: int, tile: int) -> int:
+    """Pixel count of the smallest tile of the grid (the partial corner tile, R5)."""
+    h = H % tile or min(tile, H)
+    w = W % tile or min(tile, W)
+    return min(h, tile) * min(w, tile)
+
+
+# THE rule for the derived fp32 slack (DESIGN.md section 3): a purely relative 1e-4 bound on q is attainable only when
+# a tile's sums are dominated by terms that do not cancel; a tile of a few pixels can consist of pixels whose Delta is
+# itself the cancellation of fp32-rounded differences.  Tiles of fewer than this many pixels (N_T <= 3, or the partial
+# edge tiles of any N_T) get the first-order input-rounding bound of fp32_slack added to the 1e-4 budget; every other
+# case, and every full-size config, is held to the bare 1e-4.
+SLACK_BELOW_PIXELS = 16
+
+
+def needs_slack(H: int, W: int, tile: int) -> bool:
+    return min_tile_pixels(H, W, tile) < SLACK_BELOW_PIXELS
+
+
 def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0, extra=None):
     """First-order bound on what fp32 evaluation of Eq. 3-5 can differ from exact arithmetic, per tile.
 
     fl(b-a) = (b-a)(1+d), |d| <= 2^-24, three times: |Delta_fp32 - Delta| <= 2^-24 (D1 + D2 + Delta); a factor 2
     is added for the neglected second-order terms.  For r = min(Delta / x_hat, 1): the same error divided by
-    |x_hat| (capped at 1) plus 2^-21 r for the approximate reciprocal and the multiply.
+    |x_hat| (capped at 1 where r is: for a negative LITERAL reference r is unbounded below and so is its error) plus
+    2^-21 |r| for the approximate reciprocal and the multiply, plus -- it matters only for LITERAL's signed terms --
+    the rounding of the fp32 summation itself, 32 * 2^-24 * sum |r| (a tree of depth <= 32 for tiles up to 32 x 32).
     Returns (eS, eM, eR), each [U, Ty, Tx]: slack of sum Delta, max Delta, sum r.
     """
     L = stack.shape[0]
@@ -154,8 +175,12 @@ def fp32_slack(stack: np.ndarray, tile: int, C: float = 1e-6, ref_mode: int = 0,
             xh = np.abs(np.where(b == 0, C, b))
         else:
             xh = np.maximum(b, C)
-        r = np.minimum(dl / xh, 1.0)
-        er = np.minimum(e / xh, 1.0) + 2.0 ** -21 * np.abs(r)
+        if ref_mode == 1:
+            r = np.minimum(dl / np.where(b == 0, C, b), 1.0)  # signed, unbounded below
+            er = np.where(b < 0, e / xh, np.minimum(e / xh, 1.0)) + (2.0 ** -21 + 2.0 ** -19) * np.abs(r)
+        else:
+            r = np.minimum(dl / xh, 1.0)
+            er = np.minimum(e / xh, 1.0) + 2.0 ** -21 * np.abs(r)
         eS.append(_tile_reduce(e, tile, np.sum))
         eM.append(_tile_reduce(e, tile, np.max))
         eR.append(_tile_reduce(er, tile, np.sum))
@@ -184,16 +209,45 @@ def assert_map_close(q_gpu, q_ref, tl_gpu=None, tl_ref=None, rtol=Q_RTOL, slack=
         assert np.all(np.abs(tl_gpu - tl_ref) <= rtol * np.abs(tl_ref) + 1e-30)
 
 
-def compare_candidates(gpu, ref_z, ref_mu, ref_sigma, tau, Tx, n_tiles, rtol=Q_RTOL, branch=0):
-    """Candidate-set equality up to the borderline band of R22.
+# ----- frequency branch (Eq. 10-12): what the fp32 map can move eta by -----
+# q is an fp32 evaluation: two tree sums of <= 1024 non-negative terms (16 sequential additions per lane, one pair, five
+# shuffle levels: <= 22 roundings each), the three subtractions of Eq. 3 (<= 2^-24 (D1 + D2 + Delta) per pixel, about
+# 4 * 2^-24 of sum Delta on noise), one approximate reciprocal and one multiply per pixel (2 * 2^-24), the fp64 combine
+# rounded once: at most about 52 * 2^-24 = 3.1e-6 relative; EPS_Q_FP32 rounds that up.  Observed: <= 5e-7.
+EPS_Q_FP32 = 4e-6
+
+
+def eta_bound(q_ref: np.ndarray, harmonics: int = 1, eps_q: float = EPS_Q_FP32) -> np.ndarray:
+    """|eta_gpu - eta_ref| <= this, per tile.  The DFT is linear and |e^{i..}| = 1, so a perturbation dq of the series
+    moves every |F_k| by at most sum_u |dq_u - mean(dq)| <= 2 sum_u |dq_u| <= 2 eps_q sum_u |q_u|; the maximum over k
+    inherits the bound; a harmonic sum of h magnitudes divided by sqrt(h) inherits sqrt(h) times it.  The DC removal
+    is a cancellation (q_u agree in their leading digits), which is why this is far above eps_q * eta.  The device's
+    own arithmetic is fp64 and adds only the two fp32 roundings of |F_k| and eta (2 * 2^-24 eta, folded into 2e-7)."""
+    q = np.abs(np.asarray(q_ref, dtype=np.float64))
+    return 2.0 * eps_q * q.sum(axis=0) * np.sqrt(float(harmonics))
+
+
+def eta_z_band(eta_ref, z_ref, sigma_eta, bound):
+    """What `bound` on eta can move z = (eta - mean) / std by: the tile's own error and the mean's over sigma, plus
+    |z| times the relative error of sigma (<= max bound / sigma)."""
+    bmax = float(np.max(bound))
+    return (bound + bmax) / sigma_eta + np.abs(z_ref) * bmax / sigma_eta + 2e-7 * np.abs(eta_ref) / sigma_eta
+
+
+def compare_candidates(gpu, ref_z, ref_mu, ref_sigma, tau, Tx, n_tiles, rtol=Q_RTOL, branch=0, band=None):
+    """Candidate-set equality up to the borderline band of R22 (or an explicit `band` [U, n_tiles], for quantities
+    whose error bound is derived otherwise: eta, LITERAL sums).
 
     gpu: list of (x, y, snapshot, score, tile_index, unit_index); ref_z: [U, n_tiles] oracle z.
     Returns the number of borderline tiles that were tolerated.
     """
     ref_z = np.asarray(ref_z, dtype=np.float64).reshape(ref_z.shape[0], -1)
     U = ref_z.shape[0]
-    band = np.zeros_like(ref_z)
+    explicit = band is not None
+    band = np.zeros_like(ref_z) if band is None else np.asarray(band, dtype=np.float64).reshape(ref_z.shape)
     for u in range(U):
+        if explicit:
+            break
         cv = abs(ref_mu[u]) / ref_sigma[u] if ref_sigma[u] > 0 else 0.0
         band[u] = rtol * (cv + np.abs(ref_z[u]))
     must = ref_z > tau + band
