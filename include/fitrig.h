@@ -102,6 +102,17 @@ typedef struct {
   float score;
 } fitrig_candidate;
 
+/* Sub-tile position of a candidate of the frequency branch (fitrig_localise), 24 bytes. */
+typedef struct {
+  double x, y;  /* pixels; pixel centres at integers, so the centre of tile tx is (tx + 0.5) * N_T - 0.5 */
+  double value; /* the interpolated eta surface at (x, y) */
+} fitrig_position;
+
+#define FITRIG_INTERP_BILINEAR 0 /* piecewise linear                                                        */
+#define FITRIG_INTERP_BICUBIC 1  /* cubic convolution, Keys (1981) a = -1/2, Keys' boundary samples            */
+#define FITRIG_INTERP_SPLINE 2   /* cubic spline, not-a-knot end conditions (the scheme of PAPER.md:385)        */
+#define FITRIG_INTERP_MAKIMA 3   /* modified Akima piecewise cubic Hermite                                     */
+
 /* How the library will run a problem; pure host arithmetic (no CUDA call), see fitrig_plan_query. */
 typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
@@ -186,6 +197,25 @@ int fitrig_detect_batch(fitrig_ctx* ctx, float sigma_threshold, fitrig_candidate
 int fitrig_detect_launch(fitrig_ctx* ctx, float sigma_threshold, int64_t capacity, void* cuda_stream);
 int fitrig_detect_fetch(fitrig_ctx* ctx, fitrig_candidate* h_out, int64_t* n_found, int64_t* n_found_per_stack);
 
+/* fitrig_localise -- sub-tile localisation by interpolating the spectrum matrix eta (section 2.4.2:
+ * "interpolation methods are activated for precise pulsar localisation in the selected regions ... bilinear, spline,
+ * bicubic, or Makima cubic interpolation"; spline interpolation of the spectrum matrix, the peak
+ * position is the pulsar position).  The paper names the schemes and prints no rule; reading R28:
+ *   - eta_t is a sample of a surface at the centre of tile t; the surface is the tensor product (along x within every
+ *     tile row, then along y) of the chosen 1-D scheme on the uniform grid of tile centres (a partial edge tile sits
+ *     at its nominal full-tile centre);
+ *   - for every candidate the surface is evaluated at x = x_c + i / r, y = y_c + j / r, i, j = -N_T r .. +N_T r
+ *     (r = oversample >= 1; (x_c, y_c) the centre of the candidate's tile), without the points outside the hull of
+ *     the tile centres, and the position is the largest value, the first in (j, i) row-major order on ties.
+ *   h_cands (host)  n candidates as fitrig_detect returned them for the frequency branch ((x, y) inside the tile)
+ *   h_eta (host)    NULL: the context's current eta (needs a previous fitrig_detect); otherwise a caller-supplied
+ *                   [Ty][Tx] fp32 matrix to interpolate instead (e.g. an eta averaged over several windows)
+ *   h_out (host)    n positions
+ * Frequency-branch contexts without batch.  Synchronises.  Errors: INVALID_ARG (NULL, method, oversample outside
+ * 1..8, a candidate outside the image, image branch, batch), STATE (no eta yet), NOMEM, CUDA. */
+int fitrig_localise(fitrig_ctx* ctx, const fitrig_candidate* h_cands, int64_t n, int32_t method, int32_t oversample,
+                    const float* h_eta, fitrig_position* h_out, void* cuda_stream);
+
 /* fitrig_stream -- same result as fitrig_tlisi for snapshots that live in HOST memory
  * (Fig. 14: transfers overlapped with the trigger kernels; here at row-strip
  * granularity so images need not be resident).
@@ -267,9 +297,9 @@ int fitrig_shard_export_eta(fitrig_ctx* ctx, double* d_out /*device, 3 doubles*/
 int fitrig_shard_import_eta(fitrig_ctx* ctx, const double* d_all /*device, [world][3]*/, int32_t world, void* cuda_stream);
 
 /* fitrig_get_stats -- M (B floats) and the per-unit mean / population std of q = 1 - tLISI
- * (Eq. 8; mu_tLISI = 1 - mu_q; B * U doubles each, row b * U + u).  Frequency branch after fitrig_detect: the
- * first B entries of mu and sigma describe eta of each stack (Eq. 11) instead.  Host outputs, each may be NULL.
- * Synchronises. */
+ * (Eq. 8; mu_tLISI = 1 - mu_q; B * U doubles each, row b * U + u).  Frequency branch after fitrig_detect: entry
+ * b * U of mu and sigma (unit 0 of stack b) describes eta of that stack (Eq. 11) instead.  Host outputs, each may
+ * be NULL.  Synchronises. */
 int fitrig_get_stats(const fitrig_ctx* ctx, float* M, double* mu, double* sigma);
 
 /* fitrig_get_map -- copy one of the context's maps to host memory (synchronises).

@@ -4,6 +4,6 @@ Thin ctypes binding over the C ABI of include/fitrig.h (argument marshalling onl
 path runs in the CUDA kernels of csrc/).  PyTorch is used by callers for device memory and streams.
 """
 from .binding import (  # noqa: F401
-    BRANCH_FREQUENCY, BRANCH_IMAGE, REF_ABS, REF_FLOOR, REF_LITERAL, Candidate, Context, FitrigError, Plan,
+    BRANCH_FREQUENCY, BRANCH_IMAGE, INTERP_BICUBIC, INTERP_BILINEAR, INTERP_MAKIMA, INTERP_SPLINE, REF_ABS, REF_FLOOR, REF_LITERAL, Candidate, Context, FitrigError, Plan,
     exported_symbols, last_error, lib_path, load_library, plan_query, version,
 )

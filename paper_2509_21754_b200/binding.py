@@ -41,6 +41,8 @@ class _Plan(ctypes.Structure):
                [("strip_buffer_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64)]
 
 
+POSITION_DTYPE = np.dtype([("x", np.float64), ("y", np.float64), ("value", np.float64)])
+INTERP_BILINEAR, INTERP_BICUBIC, INTERP_SPLINE, INTERP_MAKIMA = 0, 1, 2, 3
 CANDIDATE_DTYPE = np.dtype([("x", np.int32), ("y", np.int32), ("snapshot", np.int32), ("score", np.float32)])
 
 
@@ -115,13 +117,14 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_get_raw.argtypes = [vp, vp, vp, vp, vp, vp]
     L.fitrig_profile.argtypes = [vp, i32]
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
+    L.fitrig_localise.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
     L.fitrig_copy_count.argtypes = [vp, P(i64)]
     L.fitrig_probe_read_bandwidth.argtypes = [vp, vp, i64, i32, P(f32), vp]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
               "fitrig_tlisi_batch", "fitrig_detect_batch", "fitrig_detect_launch", "fitrig_detect_fetch", "fitrig_shard_export_eta", "fitrig_shard_import_eta",
               "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
-              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_probe_read_bandwidth"):
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_localise", "fitrig_probe_read_bandwidth"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
     L.fitrig_version.restype = ctypes.c_char_p
@@ -282,6 +285,20 @@ class Context:
         if h_tlisi is not None:
             out = h_tlisi.data_ptr() if hasattr(h_tlisi, "data_ptr") else h_tlisi.ctypes.data
         _check(self._L.fitrig_stream(self._h, arr, out, _stream_ptr(stream)))
+
+    def localise(self, cands: np.ndarray, method: int = INTERP_SPLINE, oversample: int = 1, eta: Optional[np.ndarray] = None,
+                 stream=None) -> np.ndarray:
+        """fitrig_localise: sub-tile positions (structured array x, y, value) of frequency-branch candidates; `eta`
+        (fp32 [Ty, Tx]) replaces the context's own spectrum matrix when given."""
+        cands = np.ascontiguousarray(cands, dtype=CANDIDATE_DTYPE)
+        out = np.zeros(len(cands), dtype=POSITION_DTYPE)
+        e = None
+        if eta is not None:
+            e = np.ascontiguousarray(eta, dtype=np.float32)
+            assert e.shape == (self.Ty, self.Tx)
+        _check(self._L.fitrig_localise(self._h, cands.ctypes.data, len(cands), int(method), int(oversample),
+                                       e.ctypes.data if e is not None else None, out.ctypes.data, _stream_ptr(stream)))
+        return out
 
     # ---- real-time mode ----
     def push(self, snapshot, sigma_threshold: float, d_tlisi=None, capacity: int = 1 << 16, stream=None,

@@ -559,8 +559,8 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
     MergeParams mp;
     mp.cells = c->raw_blocks; mp.raw = c->raw; mp.U = c->U * c->B; mp.Ty = c->Ty; mp.Tx = c->Tx;
     mp.Cy = c->Cy; mp.Cx = c->Cx; mp.m = c->geo.m; mp.step = c->geo.step; mp.cell = c->geo.cell; mp.tile = c->prm.tile;
-    const long long n = c->nmap;
-    merge_cells_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4 * c->num_sms), 256, 0, st>>>(mp);
+    const long long n = c->nmap * (mp.m * mp.m >= 32 ? 32 : 1);  // threads wanted (a warp per window of many cells)
+    merge_cells_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 16 * c->num_sms), 256, 0, st>>>(mp);
     CUDA_TRY(cudaGetLastError());
     c->launches++;
     c->blocks_pending = false;
@@ -847,6 +847,78 @@ static int detect_fetch_core(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_
 }
 
 // ---------------------------------------------------------------------------------------------
+// sub-tile localisation (R28)
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+struct DevBuf {  // a device allocation that frees itself on every return path
+  T* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  cudaError_t alloc(size_t n) { return cudaMalloc(&p, sizeof(T) * std::max<size_t>(n, 1)); }
+};
+
+extern "C" int fitrig_localise(fitrig_ctx* c, const fitrig_candidate* h_cands, int64_t n, int32_t method, int32_t oversample,
+                               const float* h_eta, fitrig_position* h_out, void* cuda_stream) {
+  if (!c) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: ctx is NULL");
+  if (n < 0 || (n > 0 && (!h_cands || !h_out))) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: NULL argument");
+  if (method < 0 || method > 3) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: unknown method %d", method);
+  if (oversample < 1 || oversample > 8) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: oversample must be 1 .. 8");
+  if (c->prm.branch != FITRIG_BRANCH_FREQUENCY || c->B != 1)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: needs a frequency-branch context without batch");
+  if (!h_eta && !c->eta_valid) return fail(FITRIG_ERR_STATE, "fitrig_localise: no eta yet (call fitrig_detect first)");
+  if (n == 0) return FITRIG_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  const int tile = c->prm.tile;
+  std::vector<int2> tiles(n);
+  for (int64_t k = 0; k < n; ++k) {
+    const int x = h_cands[k].x, y = h_cands[k].y - c->prm.row_offset;
+    if (x < 0 || x >= c->W || y < 0 || y >= c->H) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_localise: candidate %lld is outside the image", (long long)k);
+    tiles[k] = make_int2(x / tile, y / tile);
+  }
+  // eta as doubles
+  std::vector<float> ef(c->nt);
+  if (h_eta) memcpy(ef.data(), h_eta, sizeof(float) * c->nt);
+  else {
+    CUDA_TRY(cudaStreamSynchronize(st));
+    CUDA_TRY(cudaMemcpy(ef.data(), c->eta, sizeof(float) * c->nt, cudaMemcpyDeviceToHost));
+  }
+  std::vector<double> ed(ef.begin(), ef.end());
+  const int side = 2 * tile * oversample + 1;
+  const size_t per_cand = (size_t)3 * side * c->Ty;  // doubles of scratch per candidate
+  const int64_t chunk = std::max<int64_t>(1, std::min<int64_t>(n, (int64_t)((256ull << 20) / (per_cand * 8))));
+  DevBuf<double> d_eta, d_rowm, d_scr;
+  DevBuf<int2> d_tiles;
+  DevBuf<fitrig_position> d_out;
+  CUDA_TRY(d_eta.alloc(c->nt));
+  CUDA_TRY(d_rowm.alloc(c->nt));
+  CUDA_TRY(d_scr.alloc(std::max<size_t>((size_t)c->nt, per_cand * chunk)));
+  CUDA_TRY(d_tiles.alloc(chunk));
+  CUDA_TRY(d_out.alloc(chunk));
+  CUDA_TRY(cudaMemcpyAsync(d_eta.p, ed.data(), sizeof(double) * c->nt, cudaMemcpyHostToDevice, st));
+  LocaliseParams lp;
+  lp.eta = d_eta.p; lp.rowm = d_rowm.p; lp.scratch = d_scr.p; lp.tiles = d_tiles.p; lp.out = d_out.p;
+  lp.Ty = c->Ty; lp.Tx = c->Tx; lp.tile = tile; lp.method = method; lp.oversample = oversample; lp.n = 0;
+  if (method == FITRIG_INTERP_SPLINE) {
+    spline_rows_kernel<<<(c->Ty + 63) / 64, 64, 0, st>>>(lp);
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+  }
+  for (int64_t k0 = 0; k0 < n; k0 += chunk) {
+    const int m = (int)std::min<int64_t>(chunk, n - k0);
+    lp.n = m;
+    CUDA_TRY(cudaMemcpyAsync(d_tiles.p, tiles.data() + k0, sizeof(int2) * m, cudaMemcpyHostToDevice, st));
+    localise_kernel<<<m, 128, 0, st>>>(lp);
+    CUDA_TRY(cudaGetLastError());
+    c->launches++;
+    CUDA_TRY(cudaMemcpyAsync(h_out + k0, d_out.p, sizeof(fitrig_position) * m, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+  }
+  if (c->prm.row_offset)
+    for (int64_t k = 0; k < n; ++k) h_out[k].y += (double)c->prm.row_offset;
+  return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // real-time mode (timeline of Fig. 14)
 // ---------------------------------------------------------------------------------------------
 extern "C" int fitrig_push_reset(fitrig_ctx* c) {
@@ -1010,13 +1082,16 @@ extern "C" int fitrig_get_stats(const fitrig_ctx* c, float* M, double* mu, doubl
   if (M) CUDA_TRY(cudaMemcpy(M, c->M_dev, sizeof(float) * c->B, cudaMemcpyDeviceToHost));
   const bool freq_stats = c->prm.branch == FITRIG_BRANCH_FREQUENCY && c->eta_valid;
   const size_t R = (size_t)c->B * c->U;
-  if (mu) {
-    CUDA_TRY(cudaMemcpy(mu, c->mu, sizeof(double) * R, cudaMemcpyDeviceToHost));
-    if (freq_stats) CUDA_TRY(cudaMemcpy(mu, c->smu, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
-  }
-  if (sigma) {
-    CUDA_TRY(cudaMemcpy(sigma, c->sigma, sizeof(double) * R, cudaMemcpyDeviceToHost));
-    if (freq_stats) CUDA_TRY(cudaMemcpy(sigma, c->ssigma, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
+  if (mu) CUDA_TRY(cudaMemcpy(mu, c->mu, sizeof(double) * R, cudaMemcpyDeviceToHost));
+  if (sigma) CUDA_TRY(cudaMemcpy(sigma, c->sigma, sizeof(double) * R, cudaMemcpyDeviceToHost));
+  if (freq_stats) {  // eta's statistics take the place of unit 0's in every stack
+    std::vector<double> m(c->B), sd(c->B);
+    CUDA_TRY(cudaMemcpy(m.data(), c->smu, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(sd.data(), c->ssigma, sizeof(double) * c->B, cudaMemcpyDeviceToHost));
+    for (int b = 0; b < c->B; ++b) {
+      if (mu) mu[(size_t)b * c->U] = m[b];
+      if (sigma) sigma[(size_t)b * c->U] = sd[b];
+    }
   }
   return FITRIG_OK;
 }

@@ -660,28 +660,41 @@ struct MergeParams {
 };
 
 __global__ void __launch_bounds__(256) merge_cells_kernel(const MergeParams p) {
+  pdl_wait();
   const long long n = (long long)p.U * p.Ty * p.Tx;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+  // a window of many cells (m * m >= 32) is merged by a whole warp, lanes striding over its cells; a window of a few
+  // cells by one thread.  Either way the order of the additions is fixed by the geometry alone: deterministic.
+  const bool by_warp = p.m * p.m >= 32;
+  const int lane = threadIdx.x & 31;
+  const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x, nthreads = (long long)gridDim.x * blockDim.x;
+  for (long long i = by_warp ? tid / 32 : tid; i < n; i += by_warp ? nthreads / 32 : nthreads) {
     const int u = (int)(i / ((long long)p.Ty * p.Tx));
     const int t = (int)(i - (long long)u * p.Ty * p.Tx);
     const int ty = t / p.Tx, tx = t - ty * p.Tx;
     RawTile o;
-    o.sumD = 0.f; o.maxD = 0.f; o.sumR = 0.f; o.pos = 0x7fffffff;
-    bool first = true;
-    for (int by = 0; by < p.m; ++by) {
-      const int cy = ty * p.step + by;
-      if (cy >= p.Cy) break;
-      for (int bx = 0; bx < p.m; ++bx) {
-        const int cx = tx * p.step + bx;
-        if (cx >= p.Cx) break;
-        const RawTile b = p.cells[((size_t)u * p.Cy + cy) * p.Cx + cx];
-        o.sumD += b.sumD;  // fixed (cell row, cell column) order: deterministic
-        o.sumR += b.sumR;
-        const int pos = (by * p.cell + b.pos / p.cell) * p.tile + bx * p.cell + b.pos % p.cell;
-        if (first || b.maxD > o.maxD || (b.maxD == o.maxD && pos < o.pos)) { o.maxD = b.maxD; o.pos = pos; first = false; }
+    o.sumD = 0.f; o.maxD = -1.f; o.sumR = 0.f; o.pos = 0x7fffffff;
+    const int ncell = p.m * p.m;
+    for (int k = by_warp ? lane : 0; k < ncell; k += by_warp ? 32 : 1) {
+      const int by = k / p.m, bx = k - by * p.m;
+      const int cy = ty * p.step + by, cx = tx * p.step + bx;
+      if (cy >= p.Cy || cx >= p.Cx) continue;
+      const RawTile b = p.cells[((size_t)u * p.Cy + cy) * p.Cx + cx];
+      o.sumD += b.sumD;
+      o.sumR += b.sumR;
+      const int pos = (by * p.cell + b.pos / p.cell) * p.tile + bx * p.cell + b.pos % p.cell;
+      if (b.maxD > o.maxD || (b.maxD == o.maxD && pos < o.pos)) { o.maxD = b.maxD; o.pos = pos; }
+    }
+    if (by_warp) {
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        o.sumD += __shfl_xor_sync(0xffffffffu, o.sumD, off);
+        o.sumR += __shfl_xor_sync(0xffffffffu, o.sumR, off);
+        const float om = __shfl_xor_sync(0xffffffffu, o.maxD, off);
+        const int op = __shfl_xor_sync(0xffffffffu, o.pos, off);
+        if (om > o.maxD || (om == o.maxD && op < o.pos)) { o.maxD = om; o.pos = op; }
       }
     }
-    p.raw[i] = o;
+    if (!by_warp || lane == 0) p.raw[i] = o;
   }
 }
 
@@ -765,8 +778,9 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
 // coordinates are element-granular, so cell columns need no alignment); anything else by 4-byte cp.async copies
 // of the producer warp (zero fill outside the image, completion on the same mbarrier).
 // ---------------------------------------------------------------------------------------------
-constexpr int kMarchWarps = 16;      // consumer warps (their only state across iterations is a handful of registers)
-constexpr int kMarchProducers = 4;   // producer warps of the cp.async variant (the TMA variant needs one lane)
+constexpr int kMarchWarps = 24;      // consumer warps: the inner loop is a chain of dependent shared-memory loads and
+                                     // fp32 operations, so it is latency bound and wants many warps (state: a few registers)
+constexpr int kMarchProducers = 8;   // producer warps of the cp.async variant (the TMA variant needs one lane)
 
 struct MarchParams {
   RawTile* raw;          // [U][Ty][Tx]
@@ -903,7 +917,7 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
       for (int item = warp; item < nitems; item += kMarchWarps) {
         const int r = item / ngroups, gi = item - r * ngroups;
         const int ty = p.ty_base + gy * p.nty + r;
-        float S = 0.f, R = 0.f, Mx = 0.f;
+        float S = 0.f, R = 0.f, Mx;
         int mpos = 0;
         if (small) {
           const int tcol = gi * gt + jt;                    // tile column inside the box
@@ -911,17 +925,24 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
           const float* a = A + (size_t)(r * c) * p.bwp + (lane_ok ? tcol * c + cc0 : 0);
           const float* b = B + (a - A);
           const float* cv = Cc + (a - A);
-          bool first = true;
+          // Mx starts below every Delta (>= 0), so the first pixel always takes it: no "first" flag in the loop.  The
+          // global maximum takes x_s and x_{s+2} of every unit -- every snapshot of a segment but the second of a
+          // one-unit segment, which is added after the loop.
+          Mx = -1.f;
+          int mrow = 0;
+          float gb = gmax;
 #pragma unroll 4
           for (int rr = 0; rr < c; ++rr) {
             const float xa = a[rr * p.bwp], xb = b[rr * p.bwp], xc = cv[rr * p.bwp];
             const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
             S += delta;
             R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
-            if (first || delta > Mx) { Mx = delta; mpos = rr * c + cc0; first = false; }
-            gmax = fmaxf(gmax, xc);
-            if (i == 0) gmax = fmaxf(gmax, fmaxf(xa, xb));
+            if (delta > Mx) { Mx = delta; mrow = rr; }
+            gmax = fmaxf(gmax, fmaxf(xa, xc));
+            gb = fmaxf(gb, xb);
           }
+          if (nunits == 1) gmax = fmaxf(gmax, gb);
+          mpos = mrow * c + cc0;
           // segmented reduction over the c lanes of each tile (fixed tree order: deterministic)
           for (int off = 1; off < c; off <<= 1) {
             const float oS = __shfl_down_sync(0xffffffffu, S, off), oR = __shfl_down_sync(0xffffffffu, R, off);
@@ -941,7 +962,8 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
           const int tcol = gi;
           const size_t org = (size_t)(r * c) * p.bwp + tcol * c;
           int rr = 0, cc = lane;  // c > 32: no wrap needed at the start
-          bool first = true;
+          Mx = -1.f;
+          float gb = gmax;
           const int n = c * c;
 #pragma unroll 4
           for (int k = lane; k < n; k += 32) {
@@ -950,13 +972,13 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
             const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));
             S += delta;
             R += clamped_ratio<REF_MODE>(delta, xb, p.C);
-            if (first || delta > Mx) { Mx = delta; mpos = k; first = false; }  // k = rr * c + cc, ascending per lane
-            gmax = fmaxf(gmax, xc);
-            if (i == 0) gmax = fmaxf(gmax, fmaxf(xa, xb));
+            if (delta > Mx) { Mx = delta; mpos = k; }  // k = rr * c + cc, ascending per lane
+            gmax = fmaxf(gmax, fmaxf(xa, xc));
+            gb = fmaxf(gb, xb);
             cc += 32;
             if (cc >= c) { cc -= c; ++rr; }
           }
-          if (first) mpos = 0x7fffffff;  // (a lane without pixels: c * c < 32 cannot happen for c > 32)
+          if (nunits == 1) gmax = fmaxf(gmax, gb);
 #pragma unroll
           for (int off = 16; off > 0; off >>= 1) {
             S += __shfl_xor_sync(0xffffffffu, S, off);
@@ -1569,6 +1591,163 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
       }
       running += __popc(bal);
     }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sub-tile localisation by interpolating eta (reading R28 in DESIGN.md): the spectrum matrix is a
+// sample of a surface at the tile centres (index coordinates: tile column tx at u = tx); the surface is the tensor
+// product -- along x in every tile row, then along y -- of one of the four named 1-D schemes; for a selected tile it
+// is evaluated on a lattice of 1 / oversample pixels within one tile of the tile's centre (clipped to the hull of the
+// centres) and the position is the first maximum in row-major order.  fp64 throughout (a few thousand operations per
+// candidate).  spline_rows_kernel: one thread per tile row solves that row's not-a-knot spline.  localise_kernel: one
+// CTA per candidate, one thread per lattice column: the column of row-interpolant values at its u (all Ty rows: the
+// spline is global), that column's own spline, the best lattice row; then the first maximum over the columns.
+// ---------------------------------------------------------------------------------------------
+// Second derivatives of the not-a-knot cubic spline through (i, f_i), unit spacing.  With equal spacing the end
+// condition m_0 - 2 m_1 + m_2 = 0 turns the first interior equation into m_1 = d_1 (d_i = f_{i-1} - 2 f_i + f_{i+1}),
+// likewise m_{n-2} = d_{n-2}; the rest is the (1, 4, 1) system for m_2 .. m_{n-3} (Thomas), then m_0 = 2 m_1 - m_2 and
+// m_{n-1} = 2 m_{n-2} - m_{n-3}.  f and m may have any stride; cp: n doubles of scratch.
+__device__ inline void spline_nak(const double* f, int fs, int n, double* m, int ms, double* cp, int cs) {
+  if (n < 3) {
+    for (int i = 0; i < n; ++i) m[i * ms] = 0.0;
+    return;
+  }
+  auto d = [&](int i) { return f[(i - 1) * fs] - 2.0 * f[i * fs] + f[(i + 1) * fs]; };
+  if (n == 3) {
+    m[0] = m[ms] = m[2 * ms] = d(1);
+    return;
+  }
+  m[ms] = d(1);
+  m[(n - 2) * ms] = d(n - 2);
+  if (n > 4) {
+    // unknowns k = 2 .. n-3; forward sweep stores the modified right-hand side in m, the modified diagonal in cp
+    double cprev = 0.0, dprev = 0.0;
+    for (int k = 2; k <= n - 3; ++k) {
+      double rhs = 6.0 * d(k);
+      if (k == 2) rhs -= m[ms];
+      if (k == n - 3) rhs -= m[(n - 2) * ms];
+      const double den = 4.0 - ((k == 2) ? 0.0 : cprev);
+      cprev = 1.0 / den;
+      dprev = (rhs - ((k == 2) ? 0.0 : dprev)) / den;
+      cp[k * cs] = cprev;
+      m[k * ms] = dprev;
+    }
+    for (int k = n - 4; k >= 2; --k) m[k * ms] -= cp[k * cs] * m[(k + 1) * ms];
+  }
+  m[0] = 2.0 * m[ms] - m[2 * ms];
+  m[(n - 1) * ms] = 2.0 * m[(n - 2) * ms] - m[(n - 3) * ms];
+}
+
+struct Interp1 {
+  // value at u in [0, n-1] of the 1-D interpolant through (i, f[i * fs]); m: spline second derivatives (stride ms)
+  __device__ static double keys_w(double s) {  // Keys (1981), a = -1/2
+    s = fabs(s);
+    if (s <= 1.0) return (1.5 * s - 2.5) * s * s + 1.0;
+    if (s < 2.0) return ((-0.5 * s + 2.5) * s - 4.0) * s + 2.0;
+    return 0.0;
+  }
+  __device__ static double sample(const double* f, int fs, int n, int i) {  // Keys' boundary samples
+    if (i >= 0 && i < n) return f[i * fs];
+    if (n == 2) return (i < 0) ? 2.0 * f[0] - f[fs] : 2.0 * f[fs] - f[0];
+    return (i < 0) ? 3.0 * f[0] - 3.0 * f[fs] + f[2 * fs]
+                   : 3.0 * f[(n - 1) * fs] - 3.0 * f[(n - 2) * fs] + f[(n - 3) * fs];
+  }
+  __device__ static double diff(const double* f, int fs, int n, int i) {  // f_{i+1} - f_i, extended linearly twice
+    if (i >= 0 && i <= n - 2) return f[(i + 1) * fs] - f[i * fs];
+    if (i < 0) {
+      const double d0 = f[fs] - f[0], d1 = f[2 * fs] - f[fs];
+      const double a = 2.0 * d0 - d1;
+      return (i == -1) ? a : 2.0 * a - d0;
+    }
+    const double e0 = f[(n - 1) * fs] - f[(n - 2) * fs], e1 = f[(n - 2) * fs] - f[(n - 3) * fs];
+    const double a = 2.0 * e0 - e1;
+    return (i == n - 1) ? a : 2.0 * a - e0;
+  }
+  __device__ static double makima_slope(const double* f, int fs, int n, int i) {
+    const double a = diff(f, fs, n, i - 2), b = diff(f, fs, n, i - 1), c = diff(f, fs, n, i), e = diff(f, fs, n, i + 1);
+    const double w1 = fabs(e - c) + fabs(e + c) / 2.0, w2 = fabs(b - a) + fabs(b + a) / 2.0;
+    return (w1 + w2 > 0.0) ? (w1 * b + w2 * c) / (w1 + w2) : 0.0;
+  }
+  __device__ static double eval(const double* f, int fs, const double* m, int ms, int n, int method, double u) {
+    if (n == 1) return f[0];
+    int i = (int)floor(u);
+    i = max(0, min(i, n - 2));
+    const double t = u - (double)i;
+    if (method == FITRIG_INTERP_BILINEAR || n == 2) return (1.0 - t) * f[i * fs] + t * f[(i + 1) * fs];
+    if (method == FITRIG_INTERP_BICUBIC) {
+      double s = 0.0;
+      for (int k = -1; k <= 2; ++k) s += sample(f, fs, n, i + k) * keys_w(t - (double)k);
+      return s;
+    }
+    if (method == FITRIG_INTERP_SPLINE) {
+      const double a = 1.0 - t;
+      return a * f[i * fs] + t * f[(i + 1) * fs] + ((a * a * a - a) * m[i * ms] + (t * t * t - t) * m[(i + 1) * ms]) / 6.0;
+    }
+    const double s0 = makima_slope(f, fs, n, i), s1 = makima_slope(f, fs, n, i + 1);
+    const double t2 = t * t, t3 = t2 * t;
+    return (2.0 * t3 - 3.0 * t2 + 1.0) * f[i * fs] + (t3 - 2.0 * t2 + t) * s0 + (-2.0 * t3 + 3.0 * t2) * f[(i + 1) * fs] +
+           (t3 - t2) * s1;
+  }
+};
+
+struct LocaliseParams {
+  const double* eta;    // [Ty][Tx]
+  double* rowm;         // [Ty][Tx] second derivatives of the row splines (spline only)
+  double* scratch;      // [Ty][Tx] (spline_rows_kernel) / per candidate [3][side][Ty] (localise_kernel)
+  const int2* tiles;    // [n] (tx, ty) of the selected tiles
+  fitrig_position* out; // [n]
+  int n, Ty, Tx, tile, method, oversample;
+};
+
+__global__ void spline_rows_kernel(const LocaliseParams p) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= p.Ty) return;
+  spline_nak(p.eta + (size_t)r * p.Tx, 1, p.Tx, p.rowm + (size_t)r * p.Tx, 1, p.scratch + (size_t)r * p.Tx, 1);
+}
+
+__global__ void __launch_bounds__(128) localise_kernel(const LocaliseParams p) {
+  __shared__ double s_val[128];
+  __shared__ int s_j[128], s_i[128];
+  const int k = blockIdx.x;
+  const int tx = p.tiles[k].x, ty = p.tiles[k].y;
+  const int half = p.tile * p.oversample, side = 2 * half + 1;
+  // per candidate scratch: col, colm, cp, each [side][Ty] with the lattice column fastest (coalesced across threads)
+  double* col = p.scratch + (size_t)k * 3 * side * p.Ty;
+  double* colm = col + (size_t)side * p.Ty;
+  double* cp = colm + (size_t)side * p.Ty;
+  double best = 0.0;
+  int bj = 0x7fffffff, bi = 0x7fffffff;
+  for (int ii = threadIdx.x; ii < side; ii += blockDim.x) {  // lattice columns, ascending per thread
+    const int i = ii - half;
+    const double u = (double)tx + (double)i / (double)half;
+    if (u < 0.0 || u > (double)(p.Tx - 1)) continue;
+    for (int r = 0; r < p.Ty; ++r)
+      col[(size_t)r * side + ii] = Interp1::eval(p.eta + (size_t)r * p.Tx, 1, p.rowm + (size_t)r * p.Tx, 1, p.Tx, p.method, u);
+    if (p.method == FITRIG_INTERP_SPLINE) spline_nak(col + ii, side, p.Ty, colm + ii, side, cp + ii, side);
+    for (int j = -half; j <= half; ++j) {
+      const double v = (double)ty + (double)j / (double)half;
+      if (v < 0.0 || v > (double)(p.Ty - 1)) continue;
+      const double val = Interp1::eval(col + ii, side, colm + ii, side, p.Ty, p.method, v);
+      // first maximum in (j, i) order: this thread walks i ascending, j ascending
+      if (bj == 0x7fffffff || val > best || (val == best && (j < bj || (j == bj && i < bi)))) { best = val; bj = j; bi = i; }
+    }
+  }
+  s_val[threadIdx.x] = best; s_j[threadIdx.x] = bj; s_i[threadIdx.x] = bi;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int t = 1; t < (int)blockDim.x; ++t) {
+      if (s_j[t] == 0x7fffffff) continue;
+      if (bj == 0x7fffffff || s_val[t] > best || (s_val[t] == best && (s_j[t] < bj || (s_j[t] == bj && s_i[t] < bi)))) {
+        best = s_val[t]; bj = s_j[t]; bi = s_i[t];
+      }
+    }
+    const double xc = ((double)tx + 0.5) * (double)p.tile - 0.5, yc = ((double)ty + 0.5) * (double)p.tile - 0.5;
+    fitrig_position o;
+    o.x = xc + (double)bi / (double)p.oversample;
+    o.y = yc + (double)bj / (double)p.oversample;
+    o.value = best;
+    p.out[k] = o;
   }
 }
 
