@@ -327,6 +327,13 @@ int fitrig_last_timing(const fitrig_ctx* ctx, float* main_kernel_ms, int32_t* ma
 int fitrig_probe_read_bandwidth(fitrig_ctx* ctx, const void* d_buf, int64_t bytes, int32_t reps, float* gbs,
                                 void* cuda_stream);
 
+/* fitrig_stream_timeline -- the copy / compute timeline of the last fitrig_stream that ran with fitrig_profile(1)
+ * (Fig. 13-14: the transfer of the next input overlapped with the trigger kernel of the current one;
+ * here per row strip).  ms (host) receives, for each of the first `capacity` strips, four times in milliseconds
+ * relative to the start of the first copy: copy start, copy end (on the library's copy stream), kernel start, kernel
+ * end (on the caller's stream); *n_strips the number of strips of that call.  Synchronises.  Errors: STATE. */
+int fitrig_stream_timeline(const fitrig_ctx* ctx, float* ms, int32_t capacity, int32_t* n_strips);
+
 /* fitrig_launch_count -- kernels launched by this context since creation (for bench.py's gpu_launches). */
 int fitrig_launch_count(const fitrig_ctx* ctx, int64_t* n);
 

@@ -118,13 +118,14 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_profile.argtypes = [vp, i32]
     L.fitrig_last_timing.argtypes = [vp, P(f32), P(i32), P(f32), P(i32)]
     L.fitrig_localise.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp]
+    L.fitrig_stream_timeline.argtypes = [vp, vp, i32, P(i32)]
     L.fitrig_launch_count.argtypes = [vp, P(i64)]
     L.fitrig_copy_count.argtypes = [vp, P(i64)]
     L.fitrig_probe_read_bandwidth.argtypes = [vp, vp, i64, i32, P(f32), vp]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
               "fitrig_tlisi_batch", "fitrig_detect_batch", "fitrig_detect_launch", "fitrig_detect_fetch", "fitrig_shard_export_eta", "fitrig_shard_import_eta",
               "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
-              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_localise", "fitrig_probe_read_bandwidth"):
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_localise", "fitrig_stream_timeline", "fitrig_probe_read_bandwidth"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
     L.fitrig_version.restype = ctypes.c_char_p
@@ -390,6 +391,14 @@ class Context:
         _check(self._L.fitrig_probe_read_bandwidth(self._h, d_tensor.data_ptr(), nbytes, int(reps), ctypes.byref(g),
                                                    _stream_ptr(stream)))
         return g.value
+
+    def stream_timeline(self, max_strips: int = 4096) -> np.ndarray:
+        """[n_strips, 4] ms since the first copy started: copy start, copy end, kernel start, kernel end of every strip
+        of the last stream() that ran under profile(True)."""
+        out = np.zeros((max_strips, 4), dtype=np.float32)
+        n = ctypes.c_int32()
+        _check(self._L.fitrig_stream_timeline(self._h, out.ctypes.data, max_strips, ctypes.byref(n)))
+        return out[: min(n.value, max_strips)]
 
     def copy_count(self) -> int:
         n = ctypes.c_int64()

@@ -107,7 +107,7 @@ struct fitrig_ctx {
   StatPartial* parts;
   unsigned* counters;
   double *mu, *sigma;
-  int fin_nblk, fin_grid;
+  int fin_nblk, fin_grid, fin_chunk;
   int fin_user_row;    // -1: the caller's tLISI buffer receives the whole map; r >= 0: only map row r (real-time cube)
   // frequency branch
   float* eta;
@@ -148,6 +148,8 @@ struct fitrig_ctx {
   int ev_used;
   std::vector<cudaEvent_t> fin_pool;  // pairs around each finalise launch since the last read
   int fin_used;
+  std::vector<cudaEvent_t> tl_pool;   // fitrig_stream under profiling: per strip copy start / stop, kernel start / stop
+  int tl_strips;                      // strips of the last profiled fitrig_stream
   bool have_map;
   long long launches;
   long long copies;  // host-to-device copy calls issued by fitrig_stream / fitrig_push
@@ -181,6 +183,7 @@ static void free_ctx(fitrig_ctx* c) {
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   for (cudaEvent_t e : c->fin_pool) cudaEventDestroy(e);
+  for (cudaEvent_t e : c->tl_pool) cudaEventDestroy(e);
   (void)cudaGetLastError();
   delete c;
 }
@@ -307,7 +310,8 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   CTX_TRY(cudaMalloc(&c->gmax_key, 2 * sizeof(unsigned) * c->B));
   CTX_TRY(cudaMemset(c->gmax_key, 0, 2 * sizeof(unsigned) * c->B));
   c->keys_clean = true;
-  c->fin_nblk = (int)((c->nt + kFinChunk - 1) / kFinChunk);
+  c->fin_chunk = c->nt > kFinLargeMap ? kFinChunkLarge : kFinChunk;
+  c->fin_nblk = (int)((c->nt + c->fin_chunk - 1) / c->fin_chunk);
   c->fin_grid = (int)std::max<long long>(1, std::min<long long>(R * c->fin_nblk, 8ll * c->num_sms));
   c->fin_user_row = -1;
   CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * R * c->fin_nblk));
@@ -329,7 +333,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
     CTX_TRY(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * c->U, cudaMemcpyHostToDevice));
     if (sizeof(double2) * c->U > 48 * 1024)
       CTX_TRY(cudaFuncSetAttribute(dft_mag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) * c->U)));
-    c->spec_nblk = (int)((c->nt + kFinChunk - 1) / kFinChunk);
+    c->spec_nblk = c->fin_nblk;
     CTX_TRY(cudaMalloc(&c->sparts, sizeof(StatPartial) * c->spec_nblk * c->B));
     CTX_TRY(cudaMalloc(&c->scounter, sizeof(unsigned) * c->B));
     CTX_TRY(cudaMemset(c->scounter, 0, sizeof(unsigned) * c->B));
@@ -547,7 +551,7 @@ static void fill_finalize_params(fitrig_ctx* c, FinalizeParams* fp, float* d_tli
   fp->M_out = c->M_dev; fp->M_override = c->prm.M_override; fp->C = c->prm.C;
   fp->H = c->H; fp->W = c->W; fp->tile = c->prm.tile; fp->stride = c->prm.stride; fp->Ty = c->Ty; fp->Tx = c->Tx;
   fp->U = c->U; fp->B = c->B;
-  fp->nblk = c->fin_nblk; fp->parts = c->parts; fp->counters = c->counters; fp->mu = c->mu; fp->sigma = c->sigma;
+  fp->nblk = c->fin_nblk; fp->chunk = c->fin_chunk; fp->parts = c->parts; fp->counters = c->counters; fp->mu = c->mu; fp->sigma = c->sigma;
   fp->shard_all = nullptr; fp->shard_world = 0;
   fp->user_row = c->fin_user_row;
 }
@@ -627,11 +631,20 @@ static int stream_strips(fitrig_ctx* c, const float* const* h_snapshots, cudaStr
   bool pitched = host_stride >= (long long)c->H * c->W && host_stride * 4 <= c->max_pitch && snap_stride * 4 <= c->max_pitch &&
                  c->tune.no_pitched_copy == 0;
   for (int s = 2; s < c->L && pitched; ++s) pitched = (h_snapshots[s] - h_snapshots[s - 1]) == host_stride;
+  c->tl_strips = 0;
+  if (c->profile) {  // the copy / kernel timeline of this call (fitrig_stream_timeline)
+    while ((int)c->tl_pool.size() < 4 * nstrips) {
+      cudaEvent_t e;
+      CUDA_TRY(cudaEventCreate(&e));
+      c->tl_pool.push_back(e);
+    }
+  }
   for (int i = 0; i < nstrips; ++i) {
     const int b = i % nbuf;
     const int r0 = i * rows_per;
     const int rows = std::min(rows_per, c->H - r0);
     if (c->ev_free_pending[b]) CUDA_TRY(cudaStreamWaitEvent(c->copy_stream, c->ev_free[b], 0));
+    if (c->profile) CUDA_TRY(cudaEventRecord(c->tl_pool[4 * i], c->copy_stream));
     if (pitched) {  // equally spaced snapshots: the whole strip (L row blocks) is ONE pitched copy
       cudaError_t e2 = cudaMemcpy2DAsync(c->strip_buf[b], sizeof(float) * snap_stride, h_snapshots[0] + (long long)r0 * c->W,
                                          sizeof(float) * host_stride, sizeof(float) * (long long)rows * c->W, c->L,
@@ -651,13 +664,17 @@ static int stream_strips(fitrig_ctx* c, const float* const* h_snapshots, cudaStr
         c->copies++;
       }
     }
+    if (c->profile) CUDA_TRY(cudaEventRecord(c->tl_pool[4 * i + 1], c->copy_stream));
     CUDA_TRY(cudaEventRecord(c->ev_copied[b], c->copy_stream));
     CUDA_TRY(cudaStreamWaitEvent(st, c->ev_copied[b], 0));
+    if (c->profile) CUDA_TRY(cudaEventRecord(c->tl_pool[4 * i + 2], st));
     int rc = launch_tlisi_rows(c, c->strip_buf[b], snap_stride, rows, r0, true, st);
     if (rc) return rc;
+    if (c->profile) CUDA_TRY(cudaEventRecord(c->tl_pool[4 * i + 3], st));
     CUDA_TRY(cudaEventRecord(c->ev_free[b], st));
     c->ev_free_pending[b] = true;
   }
+  if (c->profile) c->tl_strips = nstrips;
   return FITRIG_OK;
 }
 
@@ -747,7 +764,7 @@ static int launch_spectrum(fitrig_ctx* c, cudaStream_t st, double* shard_out) {
   SpectrumParams sp;
   sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = (int)c->nt; sp.U = c->U; sp.B = c->B;
   sp.mag = c->mag; sp.harmonics = c->prm.harmonics;
-  sp.nblk = c->spec_nblk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
+  sp.nblk = c->spec_nblk; sp.chunk = c->fin_chunk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
   sp.shard_out = shard_out;
   if (c->U / 2 >= 1) {
     const dim3 grid((unsigned)((c->nt * c->B + 127) / 128), (unsigned)((c->U / 2 + kDftBins - 1) / kDftBins));
@@ -1026,7 +1043,7 @@ extern "C" int fitrig_shard_export(fitrig_ctx* c, double* d_out, void* cuda_stre
   ShardExportParams ep;
   ep.raw = c->raw; ep.gmax_key = c->gmax_key + c->key_idx; ep.out = d_out;
   ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.stride = c->prm.stride; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
-  ep.nblk = c->fin_nblk; ep.parts = c->parts; ep.counters = c->counters;
+  ep.nblk = c->fin_nblk; ep.chunk = c->fin_chunk; ep.parts = c->parts; ep.counters = c->counters;
   CUDA_TRY(launch_chain(shard_export_kernel, dim3(c->fin_grid), dim3(256), 0, st, !c->tune.no_pdl, ep));
   c->launches++;
   return FITRIG_OK;
@@ -1204,6 +1221,19 @@ extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   *gbs = best;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_stream_timeline(const fitrig_ctx* c, float* ms, int32_t capacity, int32_t* n_strips) {
+  if (!c || !n_strips) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream_timeline: NULL argument");
+  if (capacity < 0 || (capacity > 0 && !ms)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream_timeline: bad ms/capacity");
+  *n_strips = c->tl_strips;
+  if (c->tl_strips == 0) return fail(FITRIG_ERR_STATE, "fitrig_stream_timeline: no fitrig_stream ran under fitrig_profile(1)");
+  CUDA_TRY(cudaSetDevice(c->prm.device));
+  CUDA_TRY(cudaDeviceSynchronize());
+  for (int i = 0; i < std::min(capacity, c->tl_strips); ++i)
+    for (int k = 0; k < 4; ++k)
+      CUDA_TRY(cudaEventElapsedTime(&ms[4 * i + k], c->tl_pool[0], c->tl_pool[4 * i + k]));
   return FITRIG_OK;
 }
 

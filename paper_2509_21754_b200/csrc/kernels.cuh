@@ -1095,7 +1095,9 @@ __device__ __forceinline__ void row_stats_finish(StatPartial part, double K, int
 // ---------------------------------------------------------------------------------------------
 // finalize: q, tLISI, per-row statistics (a6, a7).  Map rows are (batch entry, unit) pairs, row = b * U + u.
 // ---------------------------------------------------------------------------------------------
-constexpr int kFinChunk = 1024;  // map entries per block and pass
+constexpr int kFinChunk = 1024;       // map entries per block and pass ...
+constexpr int kFinChunkLarge = 8192;  // ... and for maps of more than kFinLargeMap entries per row (per-pixel maps): the
+constexpr int kFinLargeMap = 1 << 20; // per-chunk reduction and hand-over is amortised over eight times the entries
 
 struct FinalizeParams {
   const RawTile* raw;
@@ -1108,7 +1110,8 @@ struct FinalizeParams {
   float M_override;
   float C;
   int H, W, tile, stride, Ty, Tx, U, B;  // windows of `tile` pixels every `stride` pixels (stride == tile: tiles)
-  int nblk;            // chunks per row = ceil(Ty * Tx / kFinChunk)
+  int nblk;            // chunks per row = ceil(Ty * Tx / chunk)
+  int chunk;           // map entries per chunk (kFinChunk or kFinChunkLarge)
   StatPartial* parts;  // [B * U][nblk]
   unsigned* counters;  // [B * U]
   double* mu;          // [B * U]
@@ -1166,8 +1169,9 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
     const size_t base = (size_t)row * nt;
     // the row's shift: its first q value
     const double K = (double)(float)(tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2);
-    const int begin = blk * kFinChunk, end = min(nt, begin + kFinChunk);
+    const int begin = blk * p.chunk, end = min(nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
+#pragma unroll 4
     for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
       // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2, combined in fp64 and rounded once
       const double qd = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2;
@@ -1216,7 +1220,7 @@ struct ShardExportParams {
   const unsigned* gmax_key;
   double* out;          // [2 + 2U]: max pixel, tiles per unit, mean_p[U], M2_p[U]
   int H, W, tile, stride, Ty, Tx, U;
-  int nblk;             // chunks per unit
+  int nblk, chunk;      // chunks per unit, entries per chunk
   StatPartial* parts;   // [U][nblk]
   unsigned* counters;   // [U]
 };
@@ -1232,7 +1236,7 @@ __global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportPara
     const int u = (int)(chunk / p.nblk), blk = (int)(chunk - (long long)u * p.nblk);
     const size_t base = (size_t)u * nt;
     const double K = tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full);
-    const int begin = blk * kFinChunk, end = min(nt, begin + kFinChunk);
+    const int begin = blk * p.chunk, end = min(nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
     for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
       const double d = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) - K;
@@ -1281,7 +1285,7 @@ struct SpectrumParams {
   int harmonics;        // H >= 1: h = harmonic sum over 1, 2, 4, .., H harmonics (R26); 1: maximum magnitude
   int nt;
   int U, B;
-  int nblk;             // chunks per batch entry = ceil(nt / kFinChunk)
+  int nblk, chunk;      // chunks per batch entry = ceil(nt / chunk), entries per chunk
   StatPartial* parts;   // [B][nblk]
   unsigned* counters;   // [B]
   double* mu;           // [B]
@@ -1370,7 +1374,7 @@ __global__ void __launch_bounds__(256) spectrum_kernel(const SpectrumParams p) {
     };
     int kb0;
     const double Kshift = (double)eta_of(0, &kb0);
-    const int begin = blk * kFinChunk, end = min(p.nt, begin + kFinChunk);
+    const int begin = blk * p.chunk, end = min(p.nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
     for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
       int kb;

@@ -158,30 +158,31 @@ def test_all_entry_points_chained_on_one_context():
 def test_detect_launch_fetch_pipeline_and_state_errors():
     a = synth.make_stack(synth.scaled(synth.CONFIGS["tiny"], 256, 256), device=DEV)[0]
     b = a.flip(0).contiguous()
-    ra, rb = gpu_run(a, taus=(3.0,), tile=8), gpu_run(b, taus=(3.0,), tile=8)
-    outs = [np.zeros(1 << 16, dtype=fitrig.binding.CANDIDATE_DTYPE) for _ in range(2)]
-    with fitrig.Context(256, 256, 8, tile=8) as ctx:
+    tau, cap = 1.0, 1 << 17  # tiles of 2 pixels at 1 sigma: thousands of candidates
+    ra, rb = gpu_run(a, taus=(tau,), tile=2, capacity=cap), gpu_run(b, taus=(tau,), tile=2, capacity=cap)
+    outs = [np.zeros(cap, dtype=fitrig.binding.CANDIDATE_DTYPE) for _ in range(2)]
+    with fitrig.Context(256, 256, 8, tile=2) as ctx:
         with pytest.raises(fitrig.FitrigError) as e:
             ctx.detect_fetch(outs[0])
         assert e.value.code == fitrig.binding.ERR_STATE
         ctx.tlisi(a)
-        ctx.detect_launch(3.0)
+        ctx.detect_launch(tau, cap)
         ctx.tlisi(b)  # queued behind the first detection: the device never idles
-        ctx.detect_launch(3.0)
+        ctx.detect_launch(tau, cap)
         with pytest.raises(fitrig.FitrigError) as e:
-            ctx.detect_launch(3.0)  # two in flight
+            ctx.detect_launch(tau, cap)  # two in flight
         assert e.value.code == fitrig.binding.ERR_STATE
         with pytest.raises(fitrig.FitrigError) as e:
-            ctx.detect(3.0)
+            ctx.detect(tau)
         assert e.value.code == fitrig.binding.ERR_STATE
         ca, na, _ = ctx.detect_fetch(outs[0])
         cb, nb, _ = ctx.detect_fetch(outs[1])
-        assert na == len(ca) and np.array_equal(ca, ra["cands"][3.0][0]) and np.array_equal(cb, rb["cands"][3.0][0])
+        assert na == len(ca) and np.array_equal(ca, ra["cands"][tau][0]) and np.array_equal(cb, rb["cands"][tau][0])
         assert na > 4096  # longer than the pinned staging chunk: the rest comes from that slot's device list
-        c3, n3 = ctx.detect(3.0)
+        c3, n3 = ctx.detect(tau, cap)
         assert np.array_equal(c3, cb)
         small = np.zeros(10, dtype=fitrig.binding.CANDIDATE_DTYPE)
-        ctx.detect_launch(3.0, capacity=10)
+        ctx.detect_launch(tau, capacity=10)
         cs, ns, _ = ctx.detect_fetch(small)  # FITRIG_ERR_CAPACITY is reported through n_found
         assert ns == nb and np.array_equal(cs, cb[:10])
 
