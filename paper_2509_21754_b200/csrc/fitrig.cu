@@ -447,17 +447,19 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   const int nslots = opt.zmod ? opt.zmod : c->L;
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
-  const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0);
-  if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
+  const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0) && (c->W % 4 == 0);  // what TMA needs
+  const bool aligned8 = ((uintptr_t)base % 8 == 0) && (snap_stride % 2 == 0) && (c->W % 2 == 0);
   if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
   if (pl.path == 0 && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
 
   int rc = prof_begin(c, st);
   if (rc) return rc;
   if (pl.path == 0) {
-    const CUtensorMap* tmp = nullptr;
-    rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
-    if (rc) return rc;
+    const CUtensorMap* tmp = &c->tmap.tm;  // (unused by the cp.async variant)
+    if (aligned) {
+      rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
+      if (rc) return rc;
+    }
     const CUtensorMap& tm = *tmp;
     FusedParams fp;
     fp.raw = out_raw; fp.gmax_key = key;
@@ -473,7 +475,8 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.G = (int)G;
     fp.evict_first = c->tune.evict_first;
     fp.C = c->prm.C;
-    const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
+    fp.tma = aligned ? 1 : 0; fp.vec = aligned8 ? 2 : 1; fp.rows = rows;
+    const dim3 grid(pl.grid), block(32 * (pl.box_tiles + (aligned ? 1 : kFusedProducers)));
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
       case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
@@ -485,7 +488,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   } else if (MarchPlan mp = (c->prm.accumulate == 1 && !c->tune.old_generic)
                                 ? plan_march(tile, c->W, rows, units, c->num_sms, c->tune) : MarchPlan(); mp.ok) {
     // any cell size / width / alignment, every snapshot byte read once (time-marching through a shared-memory ring)
-    const bool tma = aligned && (c->W % 4 == 0) && mp.x_aligned;
+    const bool tma = aligned && mp.x_aligned;
     const CUtensorMap* tmp = &c->tmap.tm;  // (unused by the cp.async variant)
     if (tma) {
       rc = get_tmap(c, base, snap_stride, rows, nslots, mp.bwp, mp.bh, &tmp);
@@ -498,7 +501,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     q.nstage = mp.nstage; q.G = (int)((long long)mp.ngx * mp.ngy * units);
     q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
     // cp.async variant: 8-byte copies where every row and box origin allows it, else 4-byte
-    q.vec = (!tma && (uintptr_t)base % 8 == 0 && snap_stride % 2 == 0 && c->W % 2 == 0 && (mp.ntx * tile) % 2 == 0) ? 2 : 1;
+    q.vec = (!tma && aligned8 && (mp.ntx * tile) % 2 == 0) ? 2 : 1;
     const dim3 grid(mp.grid), block(32 * (kMarchWarps + (tma ? 1 : kMarchProducers)));
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: tlisi_march_kernel<FITRIG_REF_ABS><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;

@@ -154,8 +154,14 @@ struct FusedParams {
   int z0, zmask;         // snapshot s of the launch lives in slot (z0 + s) & zmask: real-time ring of 4 slots: zmask = 3;
                          // a plain stack: z0 = 0, zmask = 0x7fffffff (no modulo, no branch in the lane-0 paths)
   int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
+  int tma;               // 1: boxes fetched by TMA (16-byte aligned base and strides, W % 4 == 0); 0: by the cp.async copies
+                         // of kFusedProducers producer warps (any width / alignment), zero fill outside the image
+  int vec;               // cp.async variant: floats per copy, 2 (8-byte aligned rows and base) or 1
+  int rows;              // image rows covered by this launch (cp.async variant: zero fill below)
   float C;
 };
+
+constexpr int kFusedProducers = 3;  // producer warps of the cp.async variant (the TMA variant needs one lane)
 
 __device__ __forceinline__ int ring_slot(int z0, int zmask, int s) { return (z0 + s) & zmask; }
 
@@ -182,6 +188,31 @@ __device__ __forceinline__ Segment decode_segment(const FusedParams& p, int g, i
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 16 bytes global -> shared in pieces of `vec` floats (4: one 16-byte copy; 2, 1: for rows that are not 16-byte aligned)
+__device__ __forceinline__ void cp_async16_pieces(uint32_t dst, const float* src, int vec) {
+  if (vec == 4) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+  } else if (vec == 2) {
+    cp_async8_zfill(dst, src, 8);
+    cp_async8_zfill(dst + 8, src + 2, 8);
+  } else {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) cp_async4_zfill(dst + 4 * e, src + e, 4);
+  }
+}
+__device__ __forceinline__ float4 load4_pieces(const float* src, int vec) {
+  if (vec == 4) return *reinterpret_cast<const float4*>(src);
+  return make_float4(src[0], src[1], src[2], src[3]);
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -321,7 +352,7 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 // step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
 // by lane 0, off the critical path.
 template <int REF_MODE, bool ACC, int T>
-__global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
+__global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
   // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
   // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
@@ -343,7 +374,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < p.nstage; ++i) {
-      mbar_init(smem_u32(&full[i]), 1);
+      mbar_init(smem_u32(&full[i]), p.tma ? 1 : 32 * kFusedProducers);
       mbar_init(smem_u32(&empty[i]), p.ntw);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -357,30 +388,53 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
   const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty);
 
-  if (warp == p.ntw) {
-    // ---- producer ----
-    if (lane == 0) {
-      const uint64_t policy = l2_evict_first_policy();
-      const uint32_t ring_addr = smem_u32(smem);
-      int slot = 0;
-      uint32_t phase = 0;
-      for (int g = g_begin; g < g_end;) {
-        const Segment c = decode_segment(p, g, g_end);
-        g += c.nsteps - 2;
-        for (int s = 0; s < c.nsteps * acc; ++s) {  // raw snapshots (u0 + step) * acc + i, in order
-          mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
-          const uint32_t bar = full_addr + slot * 8;
+  if (warp >= p.ntw) {
+    // ---- producers: one lane issues TMA boxes; or, for images that TMA cannot describe (rows or base not 16-byte
+    // aligned), kFusedProducers warps copy the rows of a box with cp.async (completion on the same mbarrier) ----
+    const int pw = warp - p.ntw;
+    const uint64_t policy = l2_evict_first_policy();
+    const uint32_t ring_addr = smem_u32(smem);
+    int slot = 0;
+    uint32_t phase = 0;
+    if (p.tma && (pw != 0 || lane != 0)) return;
+    for (int g = g_begin; g < g_end;) {
+      const Segment c = decode_segment(p, g, g_end);
+      g += c.nsteps - 2;
+      for (int s = 0; s < c.nsteps * acc; ++s) {  // raw snapshots (u0 + step) * acc + i, in order
+        mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
+        const uint32_t bar = full_addr + slot * 8;
+        const int z = ring_slot(p.z0, p.zmask, c.u0 * acc + s);
+        if (p.tma) {
           mbar_arrive_expect_tx(bar, box_bytes);
           if (p.evict_first)
-            tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                              ring_slot(p.z0, p.zmask, c.u0 * acc + s), policy);
+            tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile, z, policy);
           else
-            tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
-                         ring_slot(p.z0, p.zmask, c.u0 * acc + s));
-          if (++slot == p.nstage) { slot = 0; phase ^= 1; }
+            tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile, z);
+        } else {
+          const int x0 = c.gx * p.ntw * kFastTile, y0 = c.ty_local * kFastTile;
+          const float* src = p.base + (long long)z * p.snap_stride;
+          for (int r = pw; r < kFastTile; r += kFusedProducers) {  // rows of the box, dealt out to the producer warps
+            const int y = y0 + r;
+            const float* row = src + (long long)y * p.W + x0;
+            const uint32_t drow = ring_addr + slot * box_bytes + r * pitch;
+            if (p.vec == 2) {
+              for (int col = 2 * lane; col < p.ntw * kFastTile; col += 64) {
+                const int left = (y < p.rows) ? min(2, p.W - (x0 + col)) : 0;  // floats inside the image
+                cp_async8_zfill(drow + col * 4, left > 0 ? row + col : src, left > 0 ? 4 * left : 0);
+              }
+            } else {
+              for (int col = lane; col < p.ntw * kFastTile; col += 32) {
+                const bool in = (y < p.rows) && (x0 + col < p.W);
+                cp_async4_zfill(drow + col * 4, in ? row + col : src, in ? 4 : 0);
+              }
+            }
+          }
+          cp_async_mbar_arrive_noinc(bar);  // arrives once this lane's copies have landed
         }
+        if (++slot == p.nstage) { slot = 0; phase ^= 1; }
       }
     }
+    if (!p.tma) cp_async_wait_all();
     return;
   }
 
@@ -392,6 +446,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   int slot = 0;
   uint32_t phase = 0;
   const bool leader = lane == Geo::leader_lane(lane);  // does the bookkeeping of its tile
+  const int rvec = p.tma ? 4 : p.vec;                  // floats per piece of the arg-max re-read (global alignment)
 
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
@@ -497,17 +552,17 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
         const int off = sub_off + (int)(tg / T) * p.W + (int)(tg % T);
         if (acc <= kMaxAccAsync) {
           for (int i = 0; i < acc; ++i) {
-            cp_async16(scratch_addr + i * 16, ip0 + off + i * p.snap_stride);
-            cp_async16(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride);
-            cp_async16(scratch_addr + (2 * acc + i) * 16, ip2 + off + i * p.snap_stride);
+            cp_async16_pieces(scratch_addr + i * 16, ip0 + off + i * p.snap_stride, rvec);
+            cp_async16_pieces(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride, rvec);
+            cp_async16_pieces(scratch_addr + (2 * acc + i) * 16, ip2 + off + i * p.snap_stride, rvec);
           }
         } else {  // long accumulations: plain (blocking) loads, L2 hits; the three sums are parked as if acc were 1
           const float* ip[3] = {ip0, ip1, ip2};
 #pragma unroll
           for (int k = 0; k < 3; ++k) {
-            float4 v = *reinterpret_cast<const float4*>(ip[k] + off);
+            float4 v = load4_pieces(ip[k] + off, rvec);
             for (int i = 1; i < acc; ++i) {
-              const float4 t = *reinterpret_cast<const float4*>(ip[k] + off + i * p.snap_stride);
+              const float4 t = load4_pieces(ip[k] + off + i * p.snap_stride, rvec);
               v.x += t.x; v.y += t.y; v.z += t.z; v.w += t.w;
             }
             scratch[k] = v;
@@ -801,15 +856,6 @@ struct MarchParams {
   float C;
 };
 
-__device__ __forceinline__ void cp_async4_zfill(uint32_t dst, const void* src, int src_bytes) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void* src, int src_bytes) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
-  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
-}
 
 template <int REF_MODE>
 __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
@@ -897,32 +943,39 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
   const int nitems = p.nty * ngroups;
   const int jt = small ? lane / c : 0, cc0 = small ? lane - jt * c : 0;  // this lane's tile in the group, column in it
   float gmax = -3.402823466e38f;
-  unsigned pos = 0;
   const long long raw_step = (long long)p.Ty * p.Tx;
+  // ring positions of the unit's three snapshots, carried along (no modulo in the loops)
+  int sa = 0, sb = (1 % p.nstage), sc = (2 % p.nstage);
+  uint32_t pha = 0, phb = (1 / p.nstage) & 1, phc = (2 / p.nstage) & 1;  // parity of the lap each position is in
+  auto advance = [&](int& slot, uint32_t& ph) { if (++slot == p.nstage) { slot = 0; ph ^= 1; } };
+  // this warp's items (row r, group gi) never change: decomposed once, then walked with a fixed stride
+  const int r_first = warp / ngroups, gi_first = warp - r_first * ngroups;
+  const int dr = kMarchWarps / ngroups, dgi = kMarchWarps - dr * ngroups;
   for (int g = g_begin; g < g_end;) {
     int gx, gy, u0, nsteps;
     decode(g, gx, gy, u0, nsteps);
     g += nsteps - 2;
     const int nunits = nsteps - 2;
     // the first two snapshots of the segment
-    mbar_wait(full_addr + (pos % p.nstage) * 8, (pos / p.nstage) & 1);
-    mbar_wait(full_addr + ((pos + 1) % p.nstage) * 8, ((pos + 1) / p.nstage) & 1);
+    mbar_wait(full_addr + sa * 8, pha);
+    mbar_wait(full_addr + sb * 8, phb);
     for (int i = 0; i < nunits; ++i) {
-      const unsigned pc = pos + i + 2;
-      mbar_wait(full_addr + (pc % p.nstage) * 8, (pc / p.nstage) & 1);
-      const float* A = reinterpret_cast<const float*>(smem + (size_t)((pos + i) % p.nstage) * slot_bytes);
-      const float* B = reinterpret_cast<const float*>(smem + (size_t)((pos + i + 1) % p.nstage) * slot_bytes);
-      const float* Cc = reinterpret_cast<const float*>(smem + (size_t)(pc % p.nstage) * slot_bytes);
+      mbar_wait(full_addr + sc * 8, phc);
+      const float* A = reinterpret_cast<const float*>(smem + (size_t)sa * slot_bytes);
+      const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes);
+      const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes);
       RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
+      int r = r_first, gi = gi_first;
       for (int item = warp; item < nitems; item += kMarchWarps) {
-        const int r = item / ngroups, gi = item - r * ngroups;
         const int ty = p.ty_base + gy * p.nty + r;
         float S = 0.f, R = 0.f, Mx;
         int mpos = 0;
         if (small) {
           const int tcol = gi * gt + jt;                    // tile column inside the box
           const bool lane_ok = jt < gt && tcol < p.ntx;
-          const float* a = A + (size_t)(r * c) * p.bwp + (lane_ok ? tcol * c + cc0 : 0);
+          // lanes without a tile read next to the others (distinct banks), their values go nowhere
+          const int col = lane_ok ? tcol * c + cc0 : max(0, min(gi * gt * c + lane, p.bwp - 32 + lane));
+          const float* a = A + (size_t)(r * c) * p.bwp + col;
           const float* b = B + (a - A);
           const float* cv = Cc + (a - A);
           // Mx starts below every Delta (>= 0), so the first pixel always takes it: no "first" flag in the loop.  The
@@ -993,16 +1046,21 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
             rawu[(long long)ty * p.Tx + tx] = o;
           }
         }
+        r += dr; gi += dgi;
+        if (gi >= ngroups) { gi -= ngroups; ++r; }
       }
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty_addr + ((pos + i) % p.nstage) * 8);  // snapshot u0 + i is not needed again
+      if (lane == 0) mbar_arrive(empty_addr + sa * 8);  // snapshot u0 + i is not needed again
+      advance(sa, pha); advance(sb, phb); advance(sc, phc);
     }
     __syncwarp();
-    if (lane == 0) {
-      mbar_arrive(empty_addr + ((pos + nunits) % p.nstage) * 8);
-      mbar_arrive(empty_addr + ((pos + nunits + 1) % p.nstage) * 8);
+    if (lane == 0) {  // the last two snapshots of the segment
+      mbar_arrive(empty_addr + sa * 8);
+      mbar_arrive(empty_addr + sb * 8);
     }
-    pos += nsteps;
+    advance(sa, pha); advance(sa, pha);
+    advance(sb, phb); advance(sb, phb);
+    advance(sc, phc); advance(sc, phc);
   }
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);

@@ -103,8 +103,13 @@ CellGeom cell_geom(int tile, int stride) {
     // everything else (5, 7, 9, 10 ...) is its own cell and takes the generic time-marching kernel
     g.cell = tile; g.m = 1; g.step = 1;
     if (!fused_tile(tile)) {
-      for (int d = 16; d >= 4; d >>= 1)
-        if (tile % d == 0) { g.cell = d; g.m = tile / d; g.step = g.m; break; }
+      bool found = false;
+      for (int d = 16; d >= 4 && !found; d >>= 1)
+        if (tile % d == 0) { g.cell = d; g.m = tile / d; g.step = g.m; found = true; }
+      // no such divisor and more than 32 pixels (50, 66, 98 ...): the generic kernel is at its best on cells of at most
+      // 32 pixels (a warp takes whole cell rows), so the largest divisor in 5 .. 32 becomes the cell
+      for (int d = 32; d >= 5 && !found && tile > kFastTile; --d)
+        if (tile % d == 0) { g.cell = d; g.m = tile / d; g.step = g.m; found = true; }
     } else if (tile > kFastTile) {
       g.cell = kFastTile; g.m = tile / kFastTile; g.step = g.m;
     }
@@ -129,7 +134,8 @@ bool fused_tile(int tile) {
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
   const bool force_generic = tn.force_generic != 0;
-  if (!fused_tile(tile) || (W % 4) != 0 || force_generic) {
+  (void)W;  // (any width: rows that TMA cannot describe are copied by cp.async producers, kernels.cuh)
+  if (!fused_tile(tile) || force_generic) {
     plan->path = 1;
     plan->units_per_cta = 0;
     plan->box_tiles = 0;
@@ -175,13 +181,26 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   int ntx = std::max(1, std::min(cells_x, 256 / c));
   while (ntx > 1 && (width(ntx) > 256 || (long long)width(ntx) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
   // boxes of about 32 KB (the fused kernel's box): long rows for HBM, several boxes in flight per SM
-  int nty = std::max(1, std::min(cells_y, (32 * 1024) / (width(ntx) * 4 * c)));
-  nty = std::max(1, std::min(nty, 256 / c));
+  const int kWarps = 24;  // consumer warps of the kernel (kMarchWarps)
+  auto rows_fit = [&](int bytes) { return std::max(1, std::min(std::min(cells_y, 256 / c), bytes / (width(ntx) * 4 * c))); };
+  int nty = rows_fit(32 * 1024);
   auto pairs = [&](int nx, int ny) { return (long long)((cells_x + nx - 1) / nx) * ((cells_y + ny - 1) / ny) * U; };
   // small problems are latency bound: smaller boxes give more CTAs something to do
+  bool shrunk = false;
   while ((pairs(ntx, nty) + kMinUnitsPerCta - 1) / kMinUnitsPerCta < num_sms && (nty > 1 || ntx > 1)) {
     if (nty > 1) nty = (nty + 1) / 2;
     else ntx = (ntx + 1) / 2;
+    shrunk = true;
+  }
+  if (!shrunk) {
+    // the consumer warps share a box's items (a row of floor(32 / c) adjacent cells, or one cell when c > 32): prefer
+    // the box height, up to 40 KB, that leaves the fewest warps idle in the last round
+    const int per_row = (c <= 32) ? (ntx + 32 / c - 1) / (32 / c) : ntx;
+    auto eff = [&](int ny) { const int it = ny * per_row; return (double)it / (double)((it + kWarps - 1) / kWarps * kWarps); };
+    int best = nty;
+    for (int ny = std::max(1, nty / 2); ny <= rows_fit(40 * 1024); ++ny)
+      if (eff(ny) > eff(best) + 1e-9 || (eff(ny) > eff(best) - 1e-9 && ny > best && ny <= nty)) best = ny;
+    nty = best;
   }
   // box columns start at multiples of ntx * c pixels: keep them on 16-byte boundaries where the cell size allows
   // (TMA faults on other box origins; where it cannot be had the kernel copies with cp.async instead, see x_aligned)
