@@ -118,8 +118,9 @@ typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
   int32_t path;              /* 0: fused time-marching kernel (registers): cells of 1, 2, 4, 8, 16 or 32 pixels -- the  */
                              /*    tile itself, a divisor of it (12 = 3 x 4, 48 = 3 x 16, 64 = 2 x 32 ...) or the stride */
-                             /*    of overlapping windows; boxes by TMA, or by cp.async when rows / base are unaligned   */
-                             /* 1: generic time-marching kernel (shared-memory ring): any other cell size (5, 7, 10 ..)  */
+                             /*    of overlapping windows; W % 4 == 0 (TMA needs 16-byte aligned rows)                   */
+                             /* 1: generic time-marching kernel (shared-memory ring): any other cell size (5, 7, 10 ..), */
+                             /*    any width, any alignment                                                              */
   int32_t units_per_cta;     /* fused path: (box column, unit) pairs per CTA, ceil(boxes * U / grid) */
   int32_t box_tiles;         /* fused path: adjacent 32x32 pixel blocks fetched as one TMA box (1..8) */
   int32_t warps_per_cta;     /* fused path: box_tiles consumer warps + 1 producer warp           */

@@ -449,17 +449,16 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0) && (c->W % 4 == 0);  // what TMA needs
   const bool aligned8 = ((uintptr_t)base % 8 == 0) && (snap_stride % 2 == 0) && (c->W % 2 == 0);
+  if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
   if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
   if (pl.path == 0 && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
 
   int rc = prof_begin(c, st);
   if (rc) return rc;
   if (pl.path == 0) {
-    const CUtensorMap* tmp = &c->tmap.tm;  // (unused by the cp.async variant)
-    if (aligned) {
-      rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
-      if (rc) return rc;
-    }
+    const CUtensorMap* tmp = nullptr;
+    rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
+    if (rc) return rc;
     const CUtensorMap& tm = *tmp;
     FusedParams fp;
     fp.raw = out_raw; fp.gmax_key = key;
@@ -475,8 +474,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.G = (int)G;
     fp.evict_first = c->tune.evict_first;
     fp.C = c->prm.C;
-    fp.tma = aligned ? 1 : 0; fp.vec = aligned8 ? 2 : 1; fp.rows = rows;
-    const dim3 grid(pl.grid), block(32 * (pl.box_tiles + (aligned ? 1 : kFusedProducers)));
+    const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
       case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;

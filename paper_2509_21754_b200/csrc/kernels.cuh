@@ -154,14 +154,8 @@ struct FusedParams {
   int z0, zmask;         // snapshot s of the launch lives in slot (z0 + s) & zmask: real-time ring of 4 slots: zmask = 3;
                          // a plain stack: z0 = 0, zmask = 0x7fffffff (no modulo, no branch in the lane-0 paths)
   int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
-  int tma;               // 1: boxes fetched by TMA (16-byte aligned base and strides, W % 4 == 0); 0: by the cp.async copies
-                         // of kFusedProducers producer warps (any width / alignment), zero fill outside the image
-  int vec;               // cp.async variant: floats per copy, 2 (8-byte aligned rows and base) or 1
-  int rows;              // image rows covered by this launch (cp.async variant: zero fill below)
   float C;
 };
-
-constexpr int kFusedProducers = 3;  // producer warps of the cp.async variant (the TMA variant needs one lane)
 
 __device__ __forceinline__ int ring_slot(int z0, int zmask, int s) { return (z0 + s) & zmask; }
 
@@ -197,22 +191,6 @@ __device__ __forceinline__ void cp_async8_zfill(uint32_t dst, const void* src, i
 }
 __device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
-}
-// 16 bytes global -> shared in pieces of `vec` floats (4: one 16-byte copy; 2, 1: for rows that are not 16-byte aligned)
-__device__ __forceinline__ void cp_async16_pieces(uint32_t dst, const float* src, int vec) {
-  if (vec == 4) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-  } else if (vec == 2) {
-    cp_async8_zfill(dst, src, 8);
-    cp_async8_zfill(dst + 8, src + 2, 8);
-  } else {
-#pragma unroll
-    for (int e = 0; e < 4; ++e) cp_async4_zfill(dst + 4 * e, src + e, 4);
-  }
-}
-__device__ __forceinline__ float4 load4_pieces(const float* src, int vec) {
-  if (vec == 4) return *reinterpret_cast<const float4*>(src);
-  return make_float4(src[0], src[1], src[2], src[3]);
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -352,7 +330,7 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 // step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
 // by lane 0, off the critical path.
 template <int REF_MODE, bool ACC, int T>
-__global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
+__global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
   // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
   // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
@@ -374,7 +352,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < p.nstage; ++i) {
-      mbar_init(smem_u32(&full[i]), p.tma ? 1 : 32 * kFusedProducers);
+      mbar_init(smem_u32(&full[i]), 1);
       mbar_init(smem_u32(&empty[i]), p.ntw);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -388,53 +366,30 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
   const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
   const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty);
 
-  if (warp >= p.ntw) {
-    // ---- producers: one lane issues TMA boxes; or, for images that TMA cannot describe (rows or base not 16-byte
-    // aligned), kFusedProducers warps copy the rows of a box with cp.async (completion on the same mbarrier) ----
-    const int pw = warp - p.ntw;
-    const uint64_t policy = l2_evict_first_policy();
-    const uint32_t ring_addr = smem_u32(smem);
-    int slot = 0;
-    uint32_t phase = 0;
-    if (p.tma && (pw != 0 || lane != 0)) return;
-    for (int g = g_begin; g < g_end;) {
-      const Segment c = decode_segment(p, g, g_end);
-      g += c.nsteps - 2;
-      for (int s = 0; s < c.nsteps * acc; ++s) {  // raw snapshots (u0 + step) * acc + i, in order
-        mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
-        const uint32_t bar = full_addr + slot * 8;
-        const int z = ring_slot(p.z0, p.zmask, c.u0 * acc + s);
-        if (p.tma) {
+  if (warp == p.ntw) {
+    // ---- producer ----
+    if (lane == 0) {
+      const uint64_t policy = l2_evict_first_policy();
+      const uint32_t ring_addr = smem_u32(smem);
+      int slot = 0;
+      uint32_t phase = 0;
+      for (int g = g_begin; g < g_end;) {
+        const Segment c = decode_segment(p, g, g_end);
+        g += c.nsteps - 2;
+        for (int s = 0; s < c.nsteps * acc; ++s) {  // raw snapshots (u0 + step) * acc + i, in order
+          mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
+          const uint32_t bar = full_addr + slot * 8;
           mbar_arrive_expect_tx(bar, box_bytes);
           if (p.evict_first)
-            tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile, z, policy);
+            tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
+                              ring_slot(p.z0, p.zmask, c.u0 * acc + s), policy);
           else
-            tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile, z);
-        } else {
-          const int x0 = c.gx * p.ntw * kFastTile, y0 = c.ty_local * kFastTile;
-          const float* src = p.base + (long long)z * p.snap_stride;
-          for (int r = pw; r < kFastTile; r += kFusedProducers) {  // rows of the box, dealt out to the producer warps
-            const int y = y0 + r;
-            const float* row = src + (long long)y * p.W + x0;
-            const uint32_t drow = ring_addr + slot * box_bytes + r * pitch;
-            if (p.vec == 2) {
-              for (int col = 2 * lane; col < p.ntw * kFastTile; col += 64) {
-                const int left = (y < p.rows) ? min(2, p.W - (x0 + col)) : 0;  // floats inside the image
-                cp_async8_zfill(drow + col * 4, left > 0 ? row + col : src, left > 0 ? 4 * left : 0);
-              }
-            } else {
-              for (int col = lane; col < p.ntw * kFastTile; col += 32) {
-                const bool in = (y < p.rows) && (x0 + col < p.W);
-                cp_async4_zfill(drow + col * 4, in ? row + col : src, in ? 4 : 0);
-              }
-            }
-          }
-          cp_async_mbar_arrive_noinc(bar);  // arrives once this lane's copies have landed
+            tma_load_box(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
+                         ring_slot(p.z0, p.zmask, c.u0 * acc + s));
+          if (++slot == p.nstage) { slot = 0; phase ^= 1; }
         }
-        if (++slot == p.nstage) { slot = 0; phase ^= 1; }
       }
     }
-    if (!p.tma) cp_async_wait_all();
     return;
   }
 
@@ -446,7 +401,6 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
   int slot = 0;
   uint32_t phase = 0;
   const bool leader = lane == Geo::leader_lane(lane);  // does the bookkeeping of its tile
-  const int rvec = p.tma ? 4 : p.vec;                  // floats per piece of the arg-max re-read (global alignment)
 
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
@@ -552,17 +506,17 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + kFusedProducers), 1)
         const int off = sub_off + (int)(tg / T) * p.W + (int)(tg % T);
         if (acc <= kMaxAccAsync) {
           for (int i = 0; i < acc; ++i) {
-            cp_async16_pieces(scratch_addr + i * 16, ip0 + off + i * p.snap_stride, rvec);
-            cp_async16_pieces(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride, rvec);
-            cp_async16_pieces(scratch_addr + (2 * acc + i) * 16, ip2 + off + i * p.snap_stride, rvec);
+            cp_async16(scratch_addr + i * 16, ip0 + off + i * p.snap_stride);
+            cp_async16(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride);
+            cp_async16(scratch_addr + (2 * acc + i) * 16, ip2 + off + i * p.snap_stride);
           }
         } else {  // long accumulations: plain (blocking) loads, L2 hits; the three sums are parked as if acc were 1
           const float* ip[3] = {ip0, ip1, ip2};
 #pragma unroll
           for (int k = 0; k < 3; ++k) {
-            float4 v = load4_pieces(ip[k] + off, rvec);
+            float4 v = *reinterpret_cast<const float4*>(ip[k] + off);
             for (int i = 1; i < acc; ++i) {
-              const float4 t = load4_pieces(ip[k] + off + i * p.snap_stride, rvec);
+              const float4 t = *reinterpret_cast<const float4*>(ip[k] + off + i * p.snap_stride);
               v.x += t.x; v.y += t.y; v.z += t.z; v.w += t.w;
             }
             scratch[k] = v;
@@ -948,9 +902,11 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
   int sa = 0, sb = (1 % p.nstage), sc = (2 % p.nstage);
   uint32_t pha = 0, phb = (1 / p.nstage) & 1, phc = (2 / p.nstage) & 1;  // parity of the lap each position is in
   auto advance = [&](int& slot, uint32_t& ph) { if (++slot == p.nstage) { slot = 0; ph ^= 1; } };
-  // this warp's items (row r, group gi) never change: decomposed once, then walked with a fixed stride
-  const int r_first = warp / ngroups, gi_first = warp - r_first * ngroups;
-  const int dr = kMarchWarps / ngroups, dgi = kMarchWarps - dr * ngroups;
+  // Items are dealt to the warps round-robin over ALL units the CTA walks (item `next` of the running sequence unit 0's
+  // items, unit 1's items, ...), not per unit: a box of few items (8 cells of 32 pixels) would leave most warps idle,
+  // this way they work on the following units (the ring holds their snapshots already).
+  long long next = warp, ubase = 0;
+  const unsigned magic = (unsigned)((0x100000000ull + ngroups - 1) / ngroups);  // item / ngroups for item < 2^16
   for (int g = g_begin; g < g_end;) {
     int gx, gy, u0, nsteps;
     decode(g, gx, gy, u0, nsteps);
@@ -965,8 +921,9 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
       const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes);
       const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes);
       RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
-      int r = r_first, gi = gi_first;
-      for (int item = warp; item < nitems; item += kMarchWarps) {
+      for (; next < ubase + nitems; next += kMarchWarps) {
+        const int item = (int)(next - ubase);
+        const int r = (ngroups == 1) ? item : (int)__umulhi((unsigned)item, magic), gi = item - r * ngroups;
         const int ty = p.ty_base + gy * p.nty + r;
         float S = 0.f, R = 0.f, Mx;
         int mpos = 0;
@@ -1046,9 +1003,8 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
             rawu[(long long)ty * p.Tx + tx] = o;
           }
         }
-        r += dr; gi += dgi;
-        if (gi >= ngroups) { gi -= ngroups; ++r; }
       }
+      ubase += nitems;
       __syncwarp();
       if (lane == 0) mbar_arrive(empty_addr + sa * 8);  // snapshot u0 + i is not needed again
       advance(sa, pha); advance(sb, phb); advance(sc, phc);

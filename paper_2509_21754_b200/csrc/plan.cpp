@@ -134,8 +134,7 @@ bool fused_tile(int tile) {
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan) {
   if (num_sms <= 0) num_sms = 148;
   const bool force_generic = tn.force_generic != 0;
-  (void)W;  // (any width: rows that TMA cannot describe are copied by cp.async producers, kernels.cuh)
-  if (!fused_tile(tile) || force_generic) {
+  if (!fused_tile(tile) || (W % 4) != 0 || force_generic) {
     plan->path = 1;
     plan->units_per_cta = 0;
     plan->box_tiles = 0;

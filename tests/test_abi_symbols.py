@@ -29,7 +29,7 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert (p.units, p.Ty, p.Tx) == (2, 1563, 1563)  # ceil(50000/32), R5
     assert p.path == 0 and p.strip_rows % 32 == 0 and p.n_strips * p.strip_rows >= 50000
     p = fitrig.plan_query(250, 250, 8, tile=8)
-    assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 0)  # (W % 4 != 0: the fused kernel with cp.async producers)
+    assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 1)  # W % 4 != 0 -> generic (time-marching, cp.async) kernel
     p = fitrig.plan_query(250, 252, 8, tile=8)
     assert (p.Ty, p.Tx, p.path) == (32, 32, 0) and p.strip_rows % 32 == 0  # N_T = 8, 16 ride the fused kernel
     assert fitrig.plan_query(250, 252, 8, tile=16).path == 0
@@ -39,7 +39,7 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (12, 24, 48, 100))
     assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (1, 2, 4))  # tiles inside a lane's quads
     p = fitrig.plan_query(256, 250, 8)
-    assert p.path == 0  # W % 4 != 0: rows are not 16-byte aligned, no TMA -- the same kernel, fed by cp.async copies
+    assert p.path == 1  # W % 4 != 0: rows are not 16-byte aligned, no TMA
     p = fitrig.plan_query(256, 252, 8)
     assert p.path == 0 and p.Tx == 8
 
