@@ -500,7 +500,8 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
     // cp.async variant: 8-byte copies where every row and box origin allows it, else 4-byte
     q.vec = (!tma && aligned8 && (mp.ntx * tile) % 2 == 0) ? 2 : 1;
-    const dim3 grid(mp.grid), block(32 * (kMarchWarps + (tma ? 1 : kMarchProducers)));
+    q.ncons = tma ? kMarchWarps : kMarchWarpsCp; q.nprod = tma ? 1 : kMarchProducers;
+    const dim3 grid(mp.grid), block(32 * (q.ncons + q.nprod));
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: tlisi_march_kernel<FITRIG_REF_ABS><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
       case FITRIG_REF_LITERAL: tlisi_march_kernel<FITRIG_REF_LITERAL><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;

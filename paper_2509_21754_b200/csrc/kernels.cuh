@@ -787,9 +787,11 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
 // coordinates are element-granular, so cell columns need no alignment); anything else by 4-byte cp.async copies
 // of the producer warp (zero fill outside the image, completion on the same mbarrier).
 // ---------------------------------------------------------------------------------------------
-constexpr int kMarchWarps = 24;      // consumer warps: the inner loop is a chain of dependent shared-memory loads and
+constexpr int kMarchWarps = 24;      // consumer warps (TMA variant): the inner loop is a chain of dependent shared-memory loads and
                                      // fp32 operations, so it is latency bound and wants many warps (state: a few registers)
-constexpr int kMarchProducers = 8;   // producer warps of the cp.async variant (the TMA variant needs one lane)
+constexpr int kMarchTinyCell = 10;   // cells up to this size: one lane per cell (see the kernel)
+constexpr int kMarchProducers = 16;  // producer warps of the cp.async variant (the TMA variant needs one lane): small
+constexpr int kMarchWarpsCp = 16;    // asynchronous copies move few bytes per instruction, so half the CTA issues them
 
 struct MarchParams {
   RawTile* raw;          // [U][Ty][Tx]
@@ -806,13 +808,14 @@ struct MarchParams {
   int nstage, G;
   int z0, zmask;
   int tma;               // 1: TMA boxes, 0: cp.async copies
+  int ncons, nprod;      // consumer and producer warps of this launch
   int vec;               // cp.async variant: floats per copy (1 or 2)
   float C;
 };
 
 
 template <int REF_MODE>
-__global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
+__global__ void __launch_bounds__(1024, 1)
     tlisi_march_kernel(const __grid_constant__ CUtensorMap tmap, const MarchParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
@@ -822,8 +825,8 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
   uint64_t* empty = full + kMaxStages;
   if (threadIdx.x == 0) {
     for (int i = 0; i < p.nstage; ++i) {
-      mbar_init(smem_u32(&full[i]), p.tma ? 1 : 32 * kMarchProducers);
-      mbar_init(smem_u32(&empty[i]), kMarchWarps);
+      mbar_init(smem_u32(&full[i]), p.tma ? 1 : 32 * p.nprod);
+      mbar_init(smem_u32(&empty[i]), p.ncons);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -842,9 +845,9 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
     nsteps = min(p.U - u0, g_end - g) + 2;
   };
 
-  if (warp >= kMarchWarps) {
-    // ---- producers: one lane (TMA), or kMarchProducers warps that share the rows of a box (cp.async) ----
-    const int pw = warp - kMarchWarps;
+  if (warp >= p.ncons) {
+    // ---- producers: one lane (TMA), or p.nprod warps that share the rows of a box (cp.async) ----
+    const int pw = warp - p.ncons;
     unsigned pos = 0;  // snapshots fetched so far: ring position
     for (int g = g_begin; g < g_end;) {
       int gx, gy, u0, nsteps;
@@ -865,7 +868,7 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
           mbar_wait(empty_addr + slot * 8, phase ^ 1);
           const float* src = p.base + (long long)z * p.snap_stride;
           const uint32_t dst = ring_addr + slot * slot_bytes;
-          for (int r = pw; r < p.bh; r += kMarchProducers) {  // rows of the box, dealt out to the producer warps
+          for (int r = pw; r < p.bh; r += p.nprod) {  // rows of the box, dealt out to the producer warps
             const int y = y0 + r;
             const float* row = src + (long long)y * p.W + x0;
             const uint32_t drow = dst + r * p.bwp * 4;
@@ -891,11 +894,12 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
 
   // ---- consumers ----
   const int c = p.c;
+  const bool tiny = c <= kMarchTinyCell;                   // a lane takes a whole tile
   const bool small = c <= 32;
-  const int gt = small ? 32 / c : 1;                       // tiles per warp item
+  const int gt = tiny ? 32 : (small ? 32 / c : 1);         // tiles per warp item
   const int ngroups = small ? (p.ntx + gt - 1) / gt : p.ntx;
   const int nitems = p.nty * ngroups;
-  const int jt = small ? lane / c : 0, cc0 = small ? lane - jt * c : 0;  // this lane's tile in the group, column in it
+  const int jt = small ? lane / c : 0, cc0 = small ? lane - jt * c : 0;  // (lanes = columns) this lane's tile in the group, column in it
   float gmax = -3.402823466e38f;
   const long long raw_step = (long long)p.Ty * p.Tx;
   // ring positions of the unit's three snapshots, carried along (no modulo in the loops)
@@ -921,13 +925,42 @@ __global__ void __launch_bounds__(32 * (kMarchWarps + kMarchProducers), 1)
       const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes);
       const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes);
       RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
-      for (; next < ubase + nitems; next += kMarchWarps) {
+      for (; next < ubase + nitems; next += p.ncons) {
         const int item = (int)(next - ubase);
         const int r = (ngroups == 1) ? item : (int)__umulhi((unsigned)item, magic), gi = item - r * ngroups;
         const int ty = p.ty_base + gy * p.nty + r;
         float S = 0.f, R = 0.f, Mx;
         int mpos = 0;
-        if (small) {
+        if (tiny) {
+          // cells of a few pixels: a lane walks ONE whole cell (no reduction across lanes, no idle lanes inside a group of
+          // 32 cells); neighbouring lanes are c words apart: conflict free for odd c, two-way for c = 6, 10
+          const int tcol = gi * 32 + lane;
+          const bool lane_ok = tcol < p.ntx;
+          const size_t org = (size_t)(r * c) * p.bwp + (lane_ok ? tcol * c : 0);
+          Mx = -1.f;
+          float gb = gmax;
+          int k = 0;
+          for (int rr = 0; rr < c; ++rr) {
+            const float* a = A + org + (size_t)rr * p.bwp;
+            const float* b = B + (a - A);
+            const float* cv = Cc + (a - A);
+            for (int cc = 0; cc < c; ++cc, ++k) {
+              const float xa = a[cc], xb = b[cc], xc = cv[cc];
+              const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
+              S += delta;
+              R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
+              if (delta > Mx) { Mx = delta; mpos = k; }                      // k = rr * c + cc, ascending
+              gmax = fmaxf(gmax, fmaxf(xa, xc));
+              gb = fmaxf(gb, xb);
+            }
+          }
+          if (nunits == 1) gmax = fmaxf(gmax, gb);
+          const int tx = gx * p.ntx + tcol;
+          if (lane_ok && ty < p.ty_end && tx < p.Tx) {
+            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
+            rawu[(long long)ty * p.Tx + tx] = o;
+          }
+        } else if (small) {
           const int tcol = gi * gt + jt;                    // tile column inside the box
           const bool lane_ok = jt < gt && tcol < p.ntx;
           // lanes without a tile read next to the others (distinct banks), their values go nowhere

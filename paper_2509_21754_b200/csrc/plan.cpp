@@ -178,6 +178,7 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   const int cells_x = (W + c - 1) / c, cells_y = (rows + c - 1) / c;
   auto width = [&](int ntx) { return (ntx * c + 3) / 4 * 4; };
   int ntx = std::max(1, std::min(cells_x, 256 / c));
+  if (c <= 10 && ntx > 32) ntx = 32;  // cells of a few pixels: a warp takes 32 adjacent cells, one per lane (kMarchTinyCell)
   while (ntx > 1 && (width(ntx) > 256 || (long long)width(ntx) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
   // boxes of about 32 KB (the fused kernel's box): long rows for HBM, several boxes in flight per SM
   const int kWarps = 24;  // consumer warps of the kernel (kMarchWarps)
@@ -194,7 +195,7 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   if (!shrunk) {
     // the consumer warps share a box's items (a row of floor(32 / c) adjacent cells, or one cell when c > 32): prefer
     // the box height, up to 40 KB, that leaves the fewest warps idle in the last round
-    const int per_row = (c <= 32) ? (ntx + 32 / c - 1) / (32 / c) : ntx;
+    const int per_row = (c <= 10) ? (ntx + 31) / 32 : (c <= 32) ? (ntx + 32 / c - 1) / (32 / c) : ntx;
     auto eff = [&](int ny) { const int it = ny * per_row; return (double)it / (double)((it + kWarps - 1) / kWarps * kWarps); };
     int best = nty;
     for (int ny = std::max(1, nty / 2); ny <= rows_fit(40 * 1024); ++ny)
