@@ -362,9 +362,12 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   if (c->plan.path == 0) {
     CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
-  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
-  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
-  CTX_TRY(cudaFuncSetAttribute(tlisi_march_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
 #undef CTX_TRY
   *out = c;
   return FITRIG_OK;
@@ -448,11 +451,18 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0) && (c->W % 4 == 0);  // what TMA needs
-  const bool aligned8 = ((uintptr_t)base % 8 == 0) && (snap_stride % 2 == 0) && (c->W % 2 == 0);
   if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
   if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
   if (pl.path == 0 && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
 
+  // generic path: the time-marching kernel (TMA boxes where the image allows, else cp.async copies into shifted rows)
+  MarchPlan mp = MarchPlan();
+  bool tma = false;
+  if (pl.path != 0 && c->prm.accumulate == 1 && !c->tune.old_generic) {
+    mp = plan_march(tile, c->W, rows, units, c->num_sms, c->tune, false);
+    tma = mp.ok && aligned && mp.x_aligned;
+    if (mp.ok && !tma) mp = plan_march(tile, c->W, rows, units, c->num_sms, c->tune, true);
+  }
   int rc = prof_begin(c, st);
   if (rc) return rc;
   if (pl.path == 0) {
@@ -483,10 +493,8 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     CUDA_TRY(cudaGetLastError());
     c->launches++;
     if (cells) c->blocks_pending = true;
-  } else if (MarchPlan mp = (c->prm.accumulate == 1 && !c->tune.old_generic)
-                                ? plan_march(tile, c->W, rows, units, c->num_sms, c->tune) : MarchPlan(); mp.ok) {
+  } else if (mp.ok) {
     // any cell size / width / alignment, every snapshot byte read once (time-marching through a shared-memory ring)
-    const bool tma = aligned && mp.x_aligned;
     const CUtensorMap* tmp = &c->tmap.tm;  // (unused by the cp.async variant)
     if (tma) {
       rc = get_tmap(c, base, snap_stride, rows, nslots, mp.bwp, mp.bh, &tmp);
@@ -495,17 +503,16 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     MarchParams q;
     q.raw = out_raw; q.gmax_key = key; q.base = base; q.snap_stride = snap_stride; q.W = c->W; q.rows = rows;
     q.Tx = out_Tx; q.Ty = out_Ty; q.ty_base = ty_base; q.ty_end = std::min(out_Ty, ty_base + rows_tiles);
-    q.U = units; q.c = tile; q.ntx = mp.ntx; q.nty = mp.nty; q.bwp = mp.bwp; q.bh = mp.bh; q.ngx = mp.ngx;
+    q.U = units; q.c = tile; q.ntx = mp.ntx; q.nty = mp.nty; q.bwp = mp.bwp; q.bh = mp.bh; q.pitch = mp.pitch; q.ngx = mp.ngx;
     q.nstage = mp.nstage; q.G = (int)((long long)mp.ngx * mp.ngy * units);
     q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
-    // cp.async variant: 8-byte copies where every row and box origin allows it, else 4-byte
-    q.vec = (!tma && aligned8 && (mp.ntx * tile) % 2 == 0) ? 2 : 1;
     q.ncons = tma ? kMarchWarps : kMarchWarpsCp; q.nprod = tma ? 1 : kMarchProducers;
     const dim3 grid(mp.grid), block(32 * (q.ncons + q.nprod));
+    auto launch = [&](auto kernel) { kernel<<<grid, block, mp.smem_bytes, st>>>(*tmp, q); };
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: tlisi_march_kernel<FITRIG_REF_ABS><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
-      case FITRIG_REF_LITERAL: tlisi_march_kernel<FITRIG_REF_LITERAL><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
-      default: tlisi_march_kernel<FITRIG_REF_FLOOR><<<grid, block, mp.smem_bytes, st>>>(*tmp, q); break;
+      case FITRIG_REF_ABS: tma ? launch(tlisi_march_kernel<FITRIG_REF_ABS, false>) : launch(tlisi_march_kernel<FITRIG_REF_ABS, true>); break;
+      case FITRIG_REF_LITERAL: tma ? launch(tlisi_march_kernel<FITRIG_REF_LITERAL, false>) : launch(tlisi_march_kernel<FITRIG_REF_LITERAL, true>); break;
+      default: tma ? launch(tlisi_march_kernel<FITRIG_REF_FLOOR, false>) : launch(tlisi_march_kernel<FITRIG_REF_FLOOR, true>); break;
     }
     CUDA_TRY(cudaGetLastError());
     c->launches++;

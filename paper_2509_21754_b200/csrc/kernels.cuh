@@ -804,22 +804,26 @@ struct MarchParams {
   int c;                 // cell edge in pixels
   int ntx, nty;          // cells per box
   int bwp, bh;           // box width (floats, a multiple of 4) and height
+  int pitch;             // floats between box rows in shared memory: bwp (TMA) or bwp + 8 (cp.async: shifted rows)
   int ngx;               // boxes per row of boxes
   int nstage, G;
   int z0, zmask;
   int tma;               // 1: TMA boxes, 0: cp.async copies
   int ncons, nprod;      // consumer and producer warps of this launch
-  int vec;               // cp.async variant: floats per copy (1 or 2)
   float C;
 };
 
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
 
-template <int REF_MODE>
+template <int REF_MODE, bool SHIFT>
 __global__ void __launch_bounds__(1024, 1)
     tlisi_march_kernel(const __grid_constant__ CUtensorMap tmap, const MarchParams p) {
   extern __shared__ __align__(1024) unsigned char smem[];
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-  const int box_floats = p.bh * p.bwp, box_bytes = box_floats * 4;
+  const int pitch = p.pitch;  // floats between rows of a box in shared memory
+  const int box_floats = p.bh * pitch, box_bytes = box_floats * 4;
   const int slot_bytes = (box_bytes + 127) & ~127;  // TMA destinations are 128-byte aligned
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)p.nstage * slot_bytes);
   uint64_t* empty = full + kMaxStages;
@@ -868,20 +872,21 @@ __global__ void __launch_bounds__(1024, 1)
           mbar_wait(empty_addr + slot * 8, phase ^ 1);
           const float* src = p.base + (long long)z * p.snap_stride;
           const uint32_t dst = ring_addr + slot * slot_bytes;
+          // A row of the box starts anywhere in its 16-byte line.  Shared memory takes it SHIFTED by that same offset
+          // (row r's pixel col sits at float r * pitch + a_r + col, a_r = its global float address mod 4), so that global
+          // and shared addresses are 16-byte aligned together: up to 3 single floats, then 16-byte copies (zero fill
+          // outside the image by the source size).  The consumers add a_r back (march_shift below).
+          const float* aligned_in = reinterpret_cast<const float*>(((uintptr_t)p.base + 15) & ~(uintptr_t)15);
           for (int r = pw; r < p.bh; r += p.nprod) {  // rows of the box, dealt out to the producer warps
             const int y = y0 + r;
             const float* row = src + (long long)y * p.W + x0;
-            const uint32_t drow = dst + r * p.bwp * 4;
-            if (p.vec == 2) {
-              for (int col = 2 * lane; col < p.bwp; col += 64) {
-                const int left = (y < p.rows) ? min(2, p.W - (x0 + col)) : 0;  // floats inside the image
-                cp_async8_zfill(drow + col * 4, left > 0 ? row + col : src, left > 0 ? 4 * left : 0);
-              }
-            } else {
-              for (int col = lane; col < p.bwp; col += 32) {
-                const bool in = (y < p.rows) && (x0 + col < p.W);
-                cp_async4_zfill(drow + col * 4, in ? row + col : src, in ? 4 : 0);
-              }
+            const int a_r = (int)(((uintptr_t)row >> 2) & 3), head = (4 - a_r) & 3;
+            const int valid = (y < p.rows) ? max(0, min(p.bwp, p.W - x0)) : 0;  // floats of this row inside the image
+            const uint32_t drow = dst + (r * pitch + a_r) * 4;
+            if (lane < head) cp_async4_zfill(drow + 4 * lane, lane < valid ? row + lane : src, lane < valid ? 4 : 0);
+            for (int col = head + 4 * lane; col < p.bwp; col += 128) {
+              const int bytes = max(0, min(16, 4 * (valid - col)));
+              cp_async16_zfill(drow + 4 * col, bytes > 0 ? row + col : aligned_in, bytes);
             }
           }
           cp_async_mbar_arrive_noinc(full_addr + slot * 8);  // arrives once this lane's copies have landed
@@ -924,6 +929,15 @@ __global__ void __launch_bounds__(1024, 1)
       const float* A = reinterpret_cast<const float*>(smem + (size_t)sa * slot_bytes);
       const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes);
       const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes);
+      // cp.async variant: row y of a box is shifted by the low bits of its global address (see the producer)
+      int a0A = 0, a0B = 0, a0C = 0;
+      if (SHIFT) {
+        const long long org0 = (long long)(gy * p.nty * p.c) * p.W + gx * p.ntx * p.c;
+        a0A = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i) * p.snap_stride + org0) >> 2) & 3);
+        a0B = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i + 1) * p.snap_stride + org0) >> 2) & 3);
+        a0C = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i + 2) * p.snap_stride + org0) >> 2) & 3);
+      }
+      const int Wm = p.W & 3;
       RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
       for (; next < ubase + nitems; next += p.ncons) {
         const int item = (int)(next - ubase);
@@ -936,14 +950,15 @@ __global__ void __launch_bounds__(1024, 1)
           // 32 cells); neighbouring lanes are c words apart: conflict free for odd c, two-way for c = 6, 10
           const int tcol = gi * 32 + lane;
           const bool lane_ok = tcol < p.ntx;
-          const size_t org = (size_t)(r * c) * p.bwp + (lane_ok ? tcol * c : 0);
+          const size_t org = (size_t)(r * c) * pitch + (lane_ok ? tcol * c : 0);
           Mx = -1.f;
           float gb = gmax;
           int k = 0;
-          for (int rr = 0; rr < c; ++rr) {
-            const float* a = A + org + (size_t)rr * p.bwp;
-            const float* b = B + (a - A);
-            const float* cv = Cc + (a - A);
+          int t = SHIFT ? (r * c) * Wm : 0;
+          for (int rr = 0; rr < c; ++rr, t += Wm) {
+            const float* a = A + org + (size_t)rr * pitch + (SHIFT ? ((a0A + t) & 3) : 0);
+            const float* b = B + org + (size_t)rr * pitch + (SHIFT ? ((a0B + t) & 3) : 0);
+            const float* cv = Cc + org + (size_t)rr * pitch + (SHIFT ? ((a0C + t) & 3) : 0);
             for (int cc = 0; cc < c; ++cc, ++k) {
               const float xa = a[cc], xb = b[cc], xc = cv[cc];
               const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
@@ -965,9 +980,10 @@ __global__ void __launch_bounds__(1024, 1)
           const bool lane_ok = jt < gt && tcol < p.ntx;
           // lanes without a tile read next to the others (distinct banks), their values go nowhere
           const int col = lane_ok ? tcol * c + cc0 : max(0, min(gi * gt * c + lane, p.bwp - 32 + lane));
-          const float* a = A + (size_t)(r * c) * p.bwp + col;
+          const float* a = A + (size_t)(r * c) * pitch + col;
           const float* b = B + (a - A);
           const float* cv = Cc + (a - A);
+          int t = SHIFT ? (r * c) * Wm : 0;
           // Mx starts below every Delta (>= 0), so the first pixel always takes it: no "first" flag in the loop.  The
           // global maximum takes x_s and x_{s+2} of every unit -- every snapshot of a segment but the second of a
           // one-unit segment, which is added after the loop.
@@ -975,8 +991,9 @@ __global__ void __launch_bounds__(1024, 1)
           int mrow = 0;
           float gb = gmax;
 #pragma unroll 4
-          for (int rr = 0; rr < c; ++rr) {
-            const float xa = a[rr * p.bwp], xb = b[rr * p.bwp], xc = cv[rr * p.bwp];
+          for (int rr = 0; rr < c; ++rr, t += Wm) {
+            const float xa = a[rr * pitch + (SHIFT ? ((a0A + t) & 3) : 0)], xb = b[rr * pitch + (SHIFT ? ((a0B + t) & 3) : 0)],
+                        xc = cv[rr * pitch + (SHIFT ? ((a0C + t) & 3) : 0)];
             const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
             S += delta;
             R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
@@ -1003,15 +1020,17 @@ __global__ void __launch_bounds__(1024, 1)
           }
         } else {
           const int tcol = gi;
-          const size_t org = (size_t)(r * c) * p.bwp + tcol * c;
+          const size_t org = (size_t)(r * c) * pitch + tcol * c;
           int rr = 0, cc = lane;  // c > 32: no wrap needed at the start
           Mx = -1.f;
           float gb = gmax;
           const int n = c * c;
+          int t = SHIFT ? (r * c) * Wm : 0;
 #pragma unroll 4
           for (int k = lane; k < n; k += 32) {
-            const size_t o = org + (size_t)rr * p.bwp + cc;
-            const float xa = A[o], xb = B[o], xc = Cc[o];
+            const size_t o = org + (size_t)rr * pitch + cc;
+            const float xa = A[o + (SHIFT ? ((a0A + t) & 3) : 0)], xb = B[o + (SHIFT ? ((a0B + t) & 3) : 0)],
+                        xc = Cc[o + (SHIFT ? ((a0C + t) & 3) : 0)];
             const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));
             S += delta;
             R += clamped_ratio<REF_MODE>(delta, xb, p.C);
@@ -1019,7 +1038,7 @@ __global__ void __launch_bounds__(1024, 1)
             gmax = fmaxf(gmax, fmaxf(xa, xc));
             gb = fmaxf(gb, xb);
             cc += 32;
-            if (cc >= c) { cc -= c; ++rr; }
+            if (cc >= c) { cc -= c; ++rr; t += Wm; }
           }
           if (nunits == 1) gmax = fmaxf(gmax, gb);
 #pragma unroll

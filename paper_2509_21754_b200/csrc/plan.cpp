@@ -170,19 +170,20 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn
   plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + scratch;  // ring, mbarriers, scratch
 }
 
-MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn) {
+MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn, bool shifted_rows) {
   MarchPlan m;
   memset(&m, 0, sizeof(m));
   if (num_sms <= 0) num_sms = 148;
   if (c < 1 || c > kMarchMaxCell || U < 1) return m;
   const int cells_x = (W + c - 1) / c, cells_y = (rows + c - 1) / c;
   auto width = [&](int ntx) { return (ntx * c + 3) / 4 * 4; };
+  const int pad = shifted_rows ? 8 : 0;  // (cp.async variant: a row is shifted by up to 3 floats and its last 16-byte copy may overhang)
   int ntx = std::max(1, std::min(cells_x, 256 / c));
   if (c <= 10 && ntx > 32) ntx = 32;  // cells of a few pixels: a warp takes 32 adjacent cells, one per lane (kMarchTinyCell)
-  while (ntx > 1 && (width(ntx) > 256 || (long long)width(ntx) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
+  while (ntx > 1 && (width(ntx) > 256 || (long long)(width(ntx) + pad) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
   // boxes of about 32 KB (the fused kernel's box): long rows for HBM, several boxes in flight per SM
   const int kWarps = 24;  // consumer warps of the kernel (kMarchWarps)
-  auto rows_fit = [&](int bytes) { return std::max(1, std::min(std::min(cells_y, 256 / c), bytes / (width(ntx) * 4 * c))); };
+  auto rows_fit = [&](int bytes) { return std::max(1, std::min(std::min(cells_y, 256 / c), bytes / ((width(ntx) + pad) * 4 * c))); };
   int nty = rows_fit(32 * 1024);
   auto pairs = [&](int nx, int ny) { return (long long)((cells_x + nx - 1) / nx) * ((cells_y + ny - 1) / ny) * U; };
   // small problems are latency bound: smaller boxes give more CTAs something to do
@@ -207,9 +208,9 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   const int qx = 4 / std::gcd(c, 4);
   if (ntx < cells_x && ntx >= qx) ntx = ntx / qx * qx;
   m.x_aligned = (ntx >= cells_x) || ((ntx * c) % 4 == 0);
-  m.ntx = ntx; m.nty = nty; m.bwp = width(ntx); m.bh = nty * c;
+  m.ntx = ntx; m.nty = nty; m.bwp = width(ntx); m.bh = nty * c; m.pitch = m.bwp + pad;
   m.ngx = (cells_x + ntx - 1) / ntx; m.ngy = (cells_y + nty - 1) / nty;
-  const int slot = (m.bh * m.bwp * 4 + 127) / 128 * 128;
+  const int slot = (m.bh * m.pitch * 4 + 127) / 128 * 128;
   int stages = std::min(kMaxStages, (kMaxSmemPerCta - 2048) / slot);
   if (tn.stages > 0) stages = std::min(stages, std::max(4, tn.stages));
   if (stages < 4) return m;  // three snapshots in use + one in flight

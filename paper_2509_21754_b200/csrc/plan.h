@@ -67,11 +67,12 @@ struct MarchPlan {
   bool ok;        // false: the cell is too large for the ring (the caller takes the three-reads-per-pixel kernel)
   int ntx, nty;   // cells per box
   int bwp, bh;    // box width (floats, multiple of 4, <= 256) and height (<= 256)
+  int pitch;      // floats between box rows in shared memory: bwp, or bwp + 8 for the shifted rows of the cp.async variant
   int ngx, ngy;   // boxes per row of boxes, rows of boxes
   int nstage, grid, smem_bytes;
   bool x_aligned; // every box starts on a 16-byte boundary of its row (a condition for fetching it by TMA)
 };
-MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn);
+MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn, bool shifted_rows);
 bool fused_tile(int tile);  // N_T the fused kernel serves: 1, 2, 4, 8, 16 (tiles inside a block), 32, and 32 * m (merged blocks)
 
 
