@@ -210,11 +210,25 @@ static cudaError_t set_fused_attr() {
   return set_fused_attr_one<REF, true, 1>();
 }
 
+// A tLISI launch; with fp.dep != 0 as a programmatic dependent launch (the kernel places its own griddepcontrol.wait).
+template <typename P>
+static void launch_tlisi_kernel(void (*kernel)(const CUtensorMap, const P), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                const CUtensorMap& tm, const P& prm) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = prm.dep ? 1 : 0;
+  (void)cudaLaunchKernelEx(&cfg, kernel, tm, prm);  // (the caller reads cudaGetLastError)
+}
+
 template <int REF, int T>
 static void launch_fused_t(bool acc, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const CUtensorMap& tm,
                            const FusedParams& fp) {
-  if (acc) tlisi_fused_kernel<REF, true, T><<<grid, block, smem, st>>>(tm, fp);
-  else tlisi_fused_kernel<REF, false, T><<<grid, block, smem, st>>>(tm, fp);
+  if (acc) launch_tlisi_kernel(tlisi_fused_kernel<REF, true, T>, grid, block, smem, st, tm, fp);
+  else launch_tlisi_kernel(tlisi_fused_kernel<REF, false, T>, grid, block, smem, st, tm, fp);
 }
 
 template <int REF>
@@ -310,9 +324,12 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   CTX_TRY(cudaMalloc(&c->gmax_key, 2 * sizeof(unsigned) * c->B));
   CTX_TRY(cudaMemset(c->gmax_key, 0, 2 * sizeof(unsigned) * c->B));
   c->keys_clean = true;
-  c->fin_chunk = c->nt > kFinLargeMap ? kFinChunkLarge : kFinChunk;
+  // map entries per block and pass: every chunk costs a block-wide reduction and a hand-over (fence + atomic), so big
+  // maps (small tiles) get chunks large enough that each block of the grid sees only a few of them
+  const long long fin_blocks = 8ll * c->num_sms;
+  c->fin_chunk = (int)std::min<long long>(kFinChunkMax, std::max<long long>(kFinChunk, (c->nmap / (2 * fin_blocks) + 255) / 256 * 256));
   c->fin_nblk = (int)((c->nt + c->fin_chunk - 1) / c->fin_chunk);
-  c->fin_grid = (int)std::max<long long>(1, std::min<long long>(R * c->fin_nblk, 8ll * c->num_sms));
+  c->fin_grid = (int)std::max<long long>(1, std::min<long long>(R * c->fin_nblk, fin_blocks));
   c->fin_user_row = -1;
   CTX_TRY(cudaMalloc(&c->parts, sizeof(StatPartial) * R * c->fin_nblk));
   CTX_TRY(cudaMalloc(&c->counters, sizeof(unsigned) * R));
@@ -362,12 +379,11 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   if (c->plan.path == 0) {
     CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
   }
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)));
+#define MARCH_ATTR(R, S) \
+  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<R, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)))
+  MARCH_ATTR(0, false); MARCH_ATTR(1, false); MARCH_ATTR(2, false);
+  MARCH_ATTR(0, true); MARCH_ATTR(1, true); MARCH_ATTR(2, true);
+#undef MARCH_ATTR
 #undef CTX_TRY
   *out = c;
   return FITRIG_OK;
@@ -435,6 +451,7 @@ struct RowsOpt {
   int stack = 0;            // batch entry: the records go to map rows stack * U ..
   int units = 0;            // units computed by this launch (0: all U of the context)
   int row0 = 0;             // ... starting at this row of the stack's U rows (the real-time cube's ring slot)
+  int dep = 0;              // programmatic dependent launch of the tLISI kernel (FusedParams::dep)
 };
 
 static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_stride, int rows, int r0,
@@ -484,6 +501,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.G = (int)G;
     fp.evict_first = c->tune.evict_first;
     fp.C = c->prm.C;
+    fp.dep = (c->tune.no_pdl || c->profile) ? 0 : opt.dep;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
@@ -506,14 +524,17 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     q.U = units; q.c = tile; q.ntx = mp.ntx; q.nty = mp.nty; q.bwp = mp.bwp; q.bh = mp.bh; q.pitch = mp.pitch; q.ngx = mp.ngx;
     q.nstage = mp.nstage; q.G = (int)((long long)mp.ngx * mp.ngy * units);
     q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
-    q.ncons = tma ? kMarchWarps : kMarchWarpsCp; q.nprod = tma ? 1 : kMarchProducers;
+    q.ncons = mp.ncons; q.nprod = mp.nprod;
+    q.dep = (c->tune.no_pdl || c->profile) ? 0 : opt.dep;
     const dim3 grid(mp.grid), block(32 * (q.ncons + q.nprod));
-    auto launch = [&](auto kernel) { kernel<<<grid, block, mp.smem_bytes, st>>>(*tmp, q); };
+    auto launch = [&](auto kernel) { launch_tlisi_kernel(kernel, grid, block, (size_t)mp.smem_bytes, st, *tmp, q); };
+#define MARCH_LAUNCH(R) (tma ? launch(tlisi_march_kernel<R, false>) : launch(tlisi_march_kernel<R, true>))
     switch (c->prm.ref_mode) {
-      case FITRIG_REF_ABS: tma ? launch(tlisi_march_kernel<FITRIG_REF_ABS, false>) : launch(tlisi_march_kernel<FITRIG_REF_ABS, true>); break;
-      case FITRIG_REF_LITERAL: tma ? launch(tlisi_march_kernel<FITRIG_REF_LITERAL, false>) : launch(tlisi_march_kernel<FITRIG_REF_LITERAL, true>); break;
-      default: tma ? launch(tlisi_march_kernel<FITRIG_REF_FLOOR, false>) : launch(tlisi_march_kernel<FITRIG_REF_FLOOR, true>); break;
+      case FITRIG_REF_ABS: MARCH_LAUNCH(FITRIG_REF_ABS); break;
+      case FITRIG_REF_LITERAL: MARCH_LAUNCH(FITRIG_REF_LITERAL); break;
+      default: MARCH_LAUNCH(FITRIG_REF_FLOOR); break;
     }
+#undef MARCH_LAUNCH
     CUDA_TRY(cudaGetLastError());
     c->launches++;
     if (cells) c->blocks_pending = true;
@@ -616,6 +637,7 @@ extern "C" int fitrig_tlisi_batch(fitrig_ctx* c, const float* const* d_stacks, f
   for (int b = 0; b < c->B; ++b) {
     RowsOpt opt;
     opt.stack = b;
+    opt.dep = b == 0 ? 1 : 2;  // the stacks are independent: their kernels overlap tail and ramp-up
     rc = launch_tlisi_rows(c, d_stacks[b], (long long)c->H * c->W, c->H, 0, true, st, opt);
     if (rc) return rc;
   }

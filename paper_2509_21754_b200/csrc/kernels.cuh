@@ -154,6 +154,11 @@ struct FusedParams {
   int z0, zmask;         // snapshot s of the launch lives in slot (z0 + s) & zmask: real-time ring of 4 slots: zmask = 3;
                          // a plain stack: z0 = 0, zmask = 0x7fffffff (no modulo, no branch in the lane-0 paths)
   int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
+  int dep;               // programmatic dependent launch (see pdl_wait): 1 = this grid must not touch memory before the grid
+                         // ahead of it in the stream has completed (wait at the start, after the prologue); 2 = the grid
+                         // ahead is an independent tLISI launch of the same call (another stack of a batch): run beside
+                         // its tail, but do not COMPLETE before it has (wait at the end), so that the finalise kernel,
+                         // which waits for the last of the chain, finds all of them done; 0 = a plain launch
   float C;
 };
 
@@ -359,7 +364,8 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-  pdl_launch_dependents();  // the finalise kernel may take its place on the SMs; it waits for this grid to complete
+  pdl_launch_dependents();  // the next kernel of the chain may take its place on the SMs as they fall free
+  if (p.dep == 1) pdl_wait();
 
   // this CTA's range of (group, unit) pairs
   const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
@@ -653,6 +659,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // ---- global maximum (a5): zero-filled out-of-bounds pixels are harmless because M >= C > 0 ----
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
+  if (p.dep == 2) pdl_wait();
 }
 // ---------------------------------------------------------------------------------------------
 // Windows made of cells.  The tLISI kernels reduce square CELLS (the tile itself in the plain case); a window
@@ -787,12 +794,6 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
 // coordinates are element-granular, so cell columns need no alignment); anything else by 4-byte cp.async copies
 // of the producer warp (zero fill outside the image, completion on the same mbarrier).
 // ---------------------------------------------------------------------------------------------
-constexpr int kMarchWarps = 24;      // consumer warps (TMA variant): the inner loop is a chain of dependent shared-memory loads and
-                                     // fp32 operations, so it is latency bound and wants many warps (state: a few registers)
-constexpr int kMarchTinyCell = 10;   // cells up to this size: one lane per cell (see the kernel)
-constexpr int kMarchProducers = 16;  // producer warps of the cp.async variant (the TMA variant needs one lane): small
-constexpr int kMarchWarpsCp = 16;    // asynchronous copies move few bytes per instruction, so half the CTA issues them
-
 struct MarchParams {
   RawTile* raw;          // [U][Ty][Tx]
   unsigned* gmax_key;
@@ -804,22 +805,88 @@ struct MarchParams {
   int c;                 // cell edge in pixels
   int ntx, nty;          // cells per box
   int bwp, bh;           // box width (floats, a multiple of 4) and height
-  int pitch;             // floats between box rows in shared memory: bwp (TMA) or bwp + 8 (cp.async: shifted rows)
+  int pitch;             // floats between box rows in shared memory: bwp (TMA), or >= bwp + 8 with pitch = W (mod 4) (cp.async)
   int ngx;               // boxes per row of boxes
   int nstage, G;
   int z0, zmask;
   int tma;               // 1: TMA boxes, 0: cp.async copies
   int ncons, nprod;      // consumer and producer warps of this launch
+  int dep;               // programmatic dependent launch: as FusedParams::dep
   float C;
 };
 
 __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
+// mbar_wait for the many consumer warps of the generic kernel: a warp that finds the barrier closed sleeps between polls
+// (a polling warp takes issue slots from the warps that work; 12 % of all instructions of the cp.async variant were polls)
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
+  while (true) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (done) return;
+    __nanosleep(64);
+  }
+}
+
+// One pixel of a unit: xa, xb, xc = x_s, x_{s+1} (the reference image), x_{s+2}; k = its row-major index in the cell.
+// FAST (REF_ABS only): r = sat(Delta * rcp(|x|)) without Eq. 5's "x == 0 -> C" case -- a zero reference pixel then
+// yields 1 (Delta > 0) or 0 (sat(NaN), Delta == 0) instead of min(Delta / C, 1); zmin records the smallest |x| seen so
+// that the caller can add the difference afterwards (march_zero_fix), which is almost never needed.
+template <int REF_MODE, bool FAST>
+__device__ __forceinline__ void march_pixel(float xa, float xb, float xc, int k, float C, float& S, float& R, float& Mx, int& mpos,
+                                            float& zmin) {
+  const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
+  S += delta;
+  if (FAST) {
+    R += __saturatef(delta * rcp_approx(fabsf(xb)));
+    zmin = fminf(zmin, fabsf(xb));
+  } else {
+    R += clamped_ratio<REF_MODE>(delta, xb, C);                  // Eq. 4-5
+  }
+  if (delta > Mx) { Mx = delta; mpos = k; }                      // strict: the first maximum in ascending k
+}
+__device__ __forceinline__ float march_zero_fix(float xa, float xb, float xc, float invC) {
+  if (xb != 0.f) return 0.f;
+  const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));
+  return __saturatef(delta * invC) - (delta > 0.f ? 1.f : 0.f);
+}
+
+// One whole cell of CS x CS pixels (CS = 0: c_rt x c_rt, loops not unrolled) walked by one lane in row-major order.
+template <int REF_MODE, bool FAST, bool FIRST, int CS>
+__device__ __forceinline__ void march_tiny_cell(const float* a, const float* b, const float* cv, int pitch, int c_rt, float C,
+                                                float& S, float& R, float& Mx, int& mpos, float& zmin, float& gmax) {
+  const int c = CS ? CS : c_rt;
+  auto row = [&](int rr) {
+#pragma unroll
+    for (int cc = 0; cc < c; ++cc) {
+      const float xa = a[rr * pitch + cc], xb = b[rr * pitch + cc], xc = cv[rr * pitch + cc];
+      march_pixel<REF_MODE, FAST>(xa, xb, xc, rr * c + cc, C, S, R, Mx, mpos, zmin);
+      gmax = FIRST ? fmaxf(fmaxf(gmax, xc), fmaxf(xa, xb)) : fmaxf(gmax, xc);
+    }
+  };
+  if (CS > 0 && CS <= 7) {  // whole cell unrolled
+#pragma unroll
+    for (int rr = 0; rr < c; ++rr) row(rr);
+  } else {                  // rows unrolled (CS > 0), a loop over the rows
+#pragma unroll 1
+    for (int rr = 0; rr < c; ++rr) row(rr);
+  }
+}
+
+struct TagTrue { static constexpr bool value = true; };
+struct TagFalse { static constexpr bool value = false; };
 
 template <int REF_MODE, bool SHIFT>
-__global__ void __launch_bounds__(1024, 1)
+__global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
     tlisi_march_kernel(const __grid_constant__ CUtensorMap tmap, const MarchParams p) {
+  constexpr bool FAST = REF_MODE == FITRIG_REF_ABS;
   extern __shared__ __align__(1024) unsigned char smem[];
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   const int pitch = p.pitch;  // floats between rows of a box in shared memory
@@ -837,6 +904,7 @@ __global__ void __launch_bounds__(1024, 1)
   }
   __syncthreads();
   pdl_launch_dependents();
+  if (p.dep == 1) pdl_wait();
   const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
   const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
   const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty), ring_addr = smem_u32(smem);
@@ -847,6 +915,12 @@ __global__ void __launch_bounds__(1024, 1)
     gy = group / p.ngx;
     gx = group - gy * p.ngx;
     nsteps = min(p.U - u0, g_end - g) + 2;
+  };
+  // cp.async variant: where the first pixel of a box sits in its 16-byte line of global memory (0..3 floats).  Shared
+  // memory takes the box SHIFTED by that much, and its row pitch is congruent to W modulo 4, so that the global and the
+  // shared address of every pixel agree modulo 16 bytes: rows travel as 16-byte copies whatever W and the base are.
+  auto box_shift = [&](int z, long long org0) {
+    return (int)(((uintptr_t)(p.base + (long long)z * p.snap_stride + org0) >> 2) & 3);
   };
 
   if (warp >= p.ncons) {
@@ -869,24 +943,31 @@ __global__ void __launch_bounds__(1024, 1)
             tma_load_box(ring_addr + slot * slot_bytes, &tmap, full_addr + slot * 8, x0, y0, z);
           }
         } else {
-          mbar_wait(empty_addr + slot * 8, phase ^ 1);
+          // one producer warp polls the barrier, the others sleep at a named barrier until it has passed (polling warps
+          // take issue slots from the consumers)
+          if (pw == 0) mbar_wait(empty_addr + slot * 8, phase ^ 1);
+          asm volatile("bar.sync 1, %0;" ::"r"(32 * p.nprod) : "memory");
           const float* src = p.base + (long long)z * p.snap_stride;
-          const uint32_t dst = ring_addr + slot * slot_bytes;
-          // A row of the box starts anywhere in its 16-byte line.  Shared memory takes it SHIFTED by that same offset
-          // (row r's pixel col sits at float r * pitch + a_r + col, a_r = its global float address mod 4), so that global
-          // and shared addresses are 16-byte aligned together: up to 3 single floats, then 16-byte copies (zero fill
-          // outside the image by the source size).  The consumers add a_r back (march_shift below).
+          const int a0 = box_shift(z, (long long)y0 * p.W + x0);
+          const uint32_t dst = ring_addr + slot * slot_bytes + a0 * 4;
           const float* aligned_in = reinterpret_cast<const float*>(((uintptr_t)p.base + 15) & ~(uintptr_t)15);
           for (int r = pw; r < p.bh; r += p.nprod) {  // rows of the box, dealt out to the producer warps
             const int y = y0 + r;
             const float* row = src + (long long)y * p.W + x0;
-            const int a_r = (int)(((uintptr_t)row >> 2) & 3), head = (4 - a_r) & 3;
+            // up to 3 single floats bring the row to a 16-byte boundary (of global AND shared memory), then 16-byte
+            // copies; zero fill outside the image by the source size
+            const int head = (4 - (int)(((uintptr_t)row >> 2) & 3)) & 3;
             const int valid = (y < p.rows) ? max(0, min(p.bwp, p.W - x0)) : 0;  // floats of this row inside the image
-            const uint32_t drow = dst + (r * pitch + a_r) * 4;
-            if (lane < head) cp_async4_zfill(drow + 4 * lane, lane < valid ? row + lane : src, lane < valid ? 4 : 0);
-            for (int col = head + 4 * lane; col < p.bwp; col += 128) {
-              const int bytes = max(0, min(16, 4 * (valid - col)));
-              cp_async16_zfill(drow + 4 * col, bytes > 0 ? row + col : aligned_in, bytes);
+            const uint32_t drow = dst + r * pitch * 4;
+            if (y < p.rows && x0 + p.bwp + 4 <= p.W) {  // the row and its last (overhanging) 16-byte copy lie inside the image row
+              if (lane < head) cp_async4_zfill(drow + 4 * lane, row + lane, 4);
+              for (int col = head + 4 * lane; col < p.bwp; col += 128) cp_async16(drow + 4 * col, row + col);
+            } else {
+              if (lane < head) cp_async4_zfill(drow + 4 * lane, lane < valid ? row + lane : src, lane < valid ? 4 : 0);
+              for (int col = head + 4 * lane; col < p.bwp; col += 128) {
+                const int bytes = max(0, min(16, 4 * (valid - col)));
+                cp_async16_zfill(drow + 4 * col, bytes > 0 ? row + col : aligned_in, bytes);
+              }
             }
           }
           cp_async_mbar_arrive_noinc(full_addr + slot * 8);  // arrives once this lane's copies have landed
@@ -905,6 +986,7 @@ __global__ void __launch_bounds__(1024, 1)
   const int ngroups = small ? (p.ntx + gt - 1) / gt : p.ntx;
   const int nitems = p.nty * ngroups;
   const int jt = small ? lane / c : 0, cc0 = small ? lane - jt * c : 0;  // (lanes = columns) this lane's tile in the group, column in it
+  const float invC = rcp_approx(p.C);
   float gmax = -3.402823466e38f;
   const long long raw_step = (long long)p.Ty * p.Tx;
   // ring positions of the unit's three snapshots, carried along (no modulo in the loops)
@@ -921,55 +1003,53 @@ __global__ void __launch_bounds__(1024, 1)
     decode(g, gx, gy, u0, nsteps);
     g += nsteps - 2;
     const int nunits = nsteps - 2;
+    const long long org0 = (long long)(gy * p.nty * p.c) * p.W + gx * p.ntx * p.c;
     // the first two snapshots of the segment
-    mbar_wait(full_addr + sa * 8, pha);
-    mbar_wait(full_addr + sb * 8, phb);
+    mbar_wait_sleep(full_addr + sa * 8, pha);
+    mbar_wait_sleep(full_addr + sb * 8, phb);
     for (int i = 0; i < nunits; ++i) {
-      mbar_wait(full_addr + sc * 8, phc);
-      const float* A = reinterpret_cast<const float*>(smem + (size_t)sa * slot_bytes);
-      const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes);
-      const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes);
-      // cp.async variant: row y of a box is shifted by the low bits of its global address (see the producer)
-      int a0A = 0, a0B = 0, a0C = 0;
-      if (SHIFT) {
-        const long long org0 = (long long)(gy * p.nty * p.c) * p.W + gx * p.ntx * p.c;
-        a0A = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i) * p.snap_stride + org0) >> 2) & 3);
-        a0B = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i + 1) * p.snap_stride + org0) >> 2) & 3);
-        a0C = (int)(((uintptr_t)(p.base + (long long)ring_slot(p.z0, p.zmask, u0 + i + 2) * p.snap_stride + org0) >> 2) & 3);
-      }
-      const int Wm = p.W & 3;
+      mbar_wait_sleep(full_addr + sc * 8, phc);
+      // the three snapshots of the unit (cp.async variant: each box shifted by the low bits of its global address)
+      const float* A = reinterpret_cast<const float*>(smem + (size_t)sa * slot_bytes) +
+                       (SHIFT ? box_shift(ring_slot(p.z0, p.zmask, u0 + i), org0) : 0);
+      const float* B = reinterpret_cast<const float*>(smem + (size_t)sb * slot_bytes) +
+                       (SHIFT ? box_shift(ring_slot(p.z0, p.zmask, u0 + i + 1), org0) : 0);
+      const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes) +
+                        (SHIFT ? box_shift(ring_slot(p.z0, p.zmask, u0 + i + 2), org0) : 0);
       RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
+      // The global maximum takes x_{s+2} of every unit and x_s, x_{s+1} of the first unit of a segment: every snapshot of
+      // the segment once.  The item loop is compiled twice so that the steady state pays one FMNMX per pixel.
+      auto unit_items = [&](auto first_tag) {
+      constexpr bool FIRST = decltype(first_tag)::value;
       for (; next < ubase + nitems; next += p.ncons) {
         const int item = (int)(next - ubase);
         const int r = (ngroups == 1) ? item : (int)__umulhi((unsigned)item, magic), gi = item - r * ngroups;
         const int ty = p.ty_base + gy * p.nty + r;
-        float S = 0.f, R = 0.f, Mx;
+        // Mx starts below every Delta (>= 0), so the first pixel always takes it: no "first" flag in the loops
+        float S = 0.f, R = 0.f, Mx = -1.f, zmin = 1.f;
         int mpos = 0;
         if (tiny) {
           // cells of a few pixels: a lane walks ONE whole cell (no reduction across lanes, no idle lanes inside a group of
           // 32 cells); neighbouring lanes are c words apart: conflict free for odd c, two-way for c = 6, 10
           const int tcol = gi * 32 + lane;
           const bool lane_ok = tcol < p.ntx;
-          const size_t org = (size_t)(r * c) * pitch + (lane_ok ? tcol * c : 0);
-          Mx = -1.f;
-          float gb = gmax;
-          int k = 0;
-          int t = SHIFT ? (r * c) * Wm : 0;
-          for (int rr = 0; rr < c; ++rr, t += Wm) {
-            const float* a = A + org + (size_t)rr * pitch + (SHIFT ? ((a0A + t) & 3) : 0);
-            const float* b = B + org + (size_t)rr * pitch + (SHIFT ? ((a0B + t) & 3) : 0);
-            const float* cv = Cc + org + (size_t)rr * pitch + (SHIFT ? ((a0C + t) & 3) : 0);
-            for (int cc = 0; cc < c; ++cc, ++k) {
-              const float xa = a[cc], xb = b[cc], xc = cv[cc];
-              const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
-              S += delta;
-              R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
-              if (delta > Mx) { Mx = delta; mpos = k; }                      // k = rr * c + cc, ascending
-              gmax = fmaxf(gmax, fmaxf(xa, xc));
-              gb = fmaxf(gb, xb);
-            }
+          const int org = (r * c) * pitch + (lane_ok ? tcol * c : 0);
+          const float* a = A + org;
+          const float* b = B + org;
+          const float* cv = Cc + org;
+          switch (c) {  // the sizes that reach this path (1, 2, 4, 8 ride the fused kernel) are unrolled at compile time
+            case 3: march_tiny_cell<REF_MODE, FAST, FIRST, 3>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            case 5: march_tiny_cell<REF_MODE, FAST, FIRST, 5>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            case 6: march_tiny_cell<REF_MODE, FAST, FIRST, 6>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            case 7: march_tiny_cell<REF_MODE, FAST, FIRST, 7>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            case 9: march_tiny_cell<REF_MODE, FAST, FIRST, 9>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            case 10: march_tiny_cell<REF_MODE, FAST, FIRST, 10>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
+            default: march_tiny_cell<REF_MODE, FAST, FIRST, 0>(a, b, cv, pitch, c, p.C, S, R, Mx, mpos, zmin, gmax); break;
           }
-          if (nunits == 1) gmax = fmaxf(gmax, gb);
+          if (FAST && zmin == 0.f) {  // Eq. 5's x == 0 -> C for this cell's zero reference pixels
+            for (int rr = 0; rr < c; ++rr, a += pitch, b += pitch, cv += pitch)
+              for (int cc = 0; cc < c; ++cc) R += march_zero_fix(a[cc], b[cc], cv[cc], invC);
+          }
           const int tx = gx * p.ntx + tcol;
           if (lane_ok && ty < p.ty_end && tx < p.Tx) {
             RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
@@ -980,29 +1060,21 @@ __global__ void __launch_bounds__(1024, 1)
           const bool lane_ok = jt < gt && tcol < p.ntx;
           // lanes without a tile read next to the others (distinct banks), their values go nowhere
           const int col = lane_ok ? tcol * c + cc0 : max(0, min(gi * gt * c + lane, p.bwp - 32 + lane));
-          const float* a = A + (size_t)(r * c) * pitch + col;
-          const float* b = B + (a - A);
-          const float* cv = Cc + (a - A);
-          int t = SHIFT ? (r * c) * Wm : 0;
-          // Mx starts below every Delta (>= 0), so the first pixel always takes it: no "first" flag in the loop.  The
-          // global maximum takes x_s and x_{s+2} of every unit -- every snapshot of a segment but the second of a
-          // one-unit segment, which is added after the loop.
-          Mx = -1.f;
-          int mrow = 0;
-          float gb = gmax;
+          const int org = (r * c) * pitch + col;
+          const float* a = A + org;
+          const float* b = B + org;
+          const float* cv = Cc + org;
 #pragma unroll 4
-          for (int rr = 0; rr < c; ++rr, t += Wm) {
-            const float xa = a[rr * pitch + (SHIFT ? ((a0A + t) & 3) : 0)], xb = b[rr * pitch + (SHIFT ? ((a0B + t) & 3) : 0)],
-                        xc = cv[rr * pitch + (SHIFT ? ((a0C + t) & 3) : 0)];
-            const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));  // Eq. 3
-            S += delta;
-            R += clamped_ratio<REF_MODE>(delta, xb, p.C);                  // Eq. 4-5
-            if (delta > Mx) { Mx = delta; mrow = rr; }
-            gmax = fmaxf(gmax, fmaxf(xa, xc));
-            gb = fmaxf(gb, xb);
+          for (int rr = 0; rr < c; ++rr, a += pitch, b += pitch, cv += pitch) {
+            const float xa = *a, xb = *b, xc = *cv;
+            march_pixel<REF_MODE, FAST>(xa, xb, xc, rr, p.C, S, R, Mx, mpos, zmin);  // (mpos = the row, for now)
+            gmax = FIRST ? fmaxf(fmaxf(gmax, xc), fmaxf(xa, xb)) : fmaxf(gmax, xc);
           }
-          if (nunits == 1) gmax = fmaxf(gmax, gb);
-          mpos = mrow * c + cc0;
+          if (FAST && zmin == 0.f) {
+            a = A + org; b = B + org; cv = Cc + org;
+            for (int rr = 0; rr < c; ++rr, a += pitch, b += pitch, cv += pitch) R += march_zero_fix(*a, *b, *cv, invC);
+          }
+          mpos = mpos * c + cc0;
           // segmented reduction over the c lanes of each tile (fixed tree order: deterministic)
           for (int off = 1; off < c; off <<= 1) {
             const float oS = __shfl_down_sync(0xffffffffu, S, off), oR = __shfl_down_sync(0xffffffffu, R, off);
@@ -1020,27 +1092,27 @@ __global__ void __launch_bounds__(1024, 1)
           }
         } else {
           const int tcol = gi;
-          const size_t org = (size_t)(r * c) * pitch + tcol * c;
-          int rr = 0, cc = lane;  // c > 32: no wrap needed at the start
-          Mx = -1.f;
-          float gb = gmax;
+          const int org = (r * c) * pitch + tcol * c;
           const int n = c * c;
-          int t = SHIFT ? (r * c) * Wm : 0;
+          {
+            int o = org + lane, cc = lane;  // c > 32: no wrap needed at the start
 #pragma unroll 4
-          for (int k = lane; k < n; k += 32) {
-            const size_t o = org + (size_t)rr * pitch + cc;
-            const float xa = A[o + (SHIFT ? ((a0A + t) & 3) : 0)], xb = B[o + (SHIFT ? ((a0B + t) & 3) : 0)],
-                        xc = Cc[o + (SHIFT ? ((a0C + t) & 3) : 0)];
-            const float delta = fabsf(fabsf(xb - xa) - fabsf(xc - xb));
-            S += delta;
-            R += clamped_ratio<REF_MODE>(delta, xb, p.C);
-            if (delta > Mx) { Mx = delta; mpos = k; }  // k = rr * c + cc, ascending per lane
-            gmax = fmaxf(gmax, fmaxf(xa, xc));
-            gb = fmaxf(gb, xb);
-            cc += 32;
-            if (cc >= c) { cc -= c; ++rr; t += Wm; }
+            for (int k = lane; k < n; k += 32) {
+              const float xa = A[o], xb = B[o], xc = Cc[o];
+              march_pixel<REF_MODE, FAST>(xa, xb, xc, k, p.C, S, R, Mx, mpos, zmin);  // k = row * c + col, ascending per lane
+              gmax = FIRST ? fmaxf(fmaxf(gmax, xc), fmaxf(xa, xb)) : fmaxf(gmax, xc);
+              cc += 32; o += 32;
+              if (cc >= c) { cc -= c; o += pitch - c; }
+            }
           }
-          if (nunits == 1) gmax = fmaxf(gmax, gb);
+          if (FAST && zmin == 0.f) {
+            int o = org + lane, cc = lane;
+            for (int k = lane; k < n; k += 32) {
+              R += march_zero_fix(A[o], B[o], Cc[o], invC);
+              cc += 32; o += 32;
+              if (cc >= c) { cc -= c; o += pitch - c; }
+            }
+          }
 #pragma unroll
           for (int off = 16; off > 0; off >>= 1) {
             S += __shfl_xor_sync(0xffffffffu, S, off);
@@ -1056,6 +1128,8 @@ __global__ void __launch_bounds__(1024, 1)
           }
         }
       }
+      };
+      if (i == 0) unit_items(TagTrue()); else unit_items(TagFalse());
       ubase += nitems;
       __syncwarp();
       if (lane == 0) mbar_arrive(empty_addr + sa * 8);  // snapshot u0 + i is not needed again
@@ -1072,6 +1146,7 @@ __global__ void __launch_bounds__(1024, 1)
   }
   const unsigned key = __reduce_max_sync(0xffffffffu, float_to_key(gmax));
   if (lane == 0 && g_begin < g_end) atomicMax(p.gmax_key, key);
+  if (p.dep == 2) pdl_wait();
 }
 
 // Global maximum over the n pixels of one image (generic path; the fused path folds this into its single
@@ -1161,9 +1236,8 @@ __device__ __forceinline__ void row_stats_finish(StatPartial part, double K, int
 // ---------------------------------------------------------------------------------------------
 // finalize: q, tLISI, per-row statistics (a6, a7).  Map rows are (batch entry, unit) pairs, row = b * U + u.
 // ---------------------------------------------------------------------------------------------
-constexpr int kFinChunk = 1024;       // map entries per block and pass ...
-constexpr int kFinChunkLarge = 8192;  // ... and for maps of more than kFinLargeMap entries per row (per-pixel maps): the
-constexpr int kFinLargeMap = 1 << 20; // per-chunk reduction and hand-over is amortised over eight times the entries
+constexpr int kFinChunk = 1024;       // map entries per block and pass: at least this many ...
+constexpr int kFinChunkMax = 16384;   // ... and at most this many (chosen per context from the map size, fitrig_create)
 
 struct FinalizeParams {
   const RawTile* raw;
@@ -1177,7 +1251,7 @@ struct FinalizeParams {
   float C;
   int H, W, tile, stride, Ty, Tx, U, B;  // windows of `tile` pixels every `stride` pixels (stride == tile: tiles)
   int nblk;            // chunks per row = ceil(Ty * Tx / chunk)
-  int chunk;           // map entries per chunk (kFinChunk or kFinChunkLarge)
+  int chunk;           // map entries per chunk (kFinChunk .. kFinChunkMax, fitrig_create)
   StatPartial* parts;  // [B * U][nblk]
   unsigned* counters;  // [B * U]
   double* mu;          // [B * U]
@@ -1528,13 +1602,15 @@ struct CompactParams {
 // z of entry i (Eq. 8 on q, R21; sigma == 0 -> z = 0, R4) and the strict threshold (R6).  1 / sigma of the current
 // row is kept by the thread (its entries stay in one row for long stretches): one fp64 multiply per entry instead
 // of a double-precision division, which dominated per-pixel maps.
+constexpr int kCompactLoads = 4;  // map entries a lane loads before it tests them (pass 1)
+
 struct RowCache {
   int row = -1;
   long long row_end = 0;  // first entry index of the next row
   double mu = 0.0, inv_sigma = 0.0;
 };
 
-__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float* z_out, RowCache& rc) {
+__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float v, float* z_out, RowCache& rc) {
   if (rc.row < 0 || i >= rc.row_end || i < rc.row_end - p.nt) {  // entries mostly move forward: rarely a division
     if (rc.row < 0 || i >= rc.row_end + p.nt || i < rc.row_end - p.nt) {
       rc.row = (int)(i / p.nt);
@@ -1547,7 +1623,7 @@ __device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i
     rc.mu = p.mu[rc.row];
     rc.inv_sigma = (sd > 0.0) ? 1.0 / sd : 0.0;
   }
-  const double z = ((double)p.v[i] - rc.mu) * rc.inv_sigma;
+  const double z = ((double)v - rc.mu) * rc.inv_sigma;
   *z_out = (float)z;
   return (float)z > p.tau;  // strict, R6
 }
@@ -1574,11 +1650,20 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   RowCache rcache;
   // ---- pass 1: count ----
   unsigned cnt = 0;
-  for (long long c0 = wb; c0 < we; c0 += 32) {
-    const long long i = c0 + lane;
-    float z;
-    const bool f = (i < we) && compact_flag(p, i, &z, rcache);
-    cnt += __popc(__ballot_sync(0xffffffffu, f));
+  for (long long c0 = wb; c0 < we; c0 += 32 * kCompactLoads) {
+    float v[kCompactLoads];  // independent loads first: one outstanding line per warp cannot feed a map of 10^8 entries
+#pragma unroll
+    for (int k = 0; k < kCompactLoads; ++k) {
+      const long long i = c0 + 32 * k + lane;
+      v[k] = (i < we) ? p.v[i] : 0.f;
+    }
+#pragma unroll
+    for (int k = 0; k < kCompactLoads; ++k) {
+      const long long i = c0 + 32 * k + lane;
+      float z;
+      const bool f = (i < we) && compact_flag(p, i, v[k], &z, rcache);
+      cnt += __popc(__ballot_sync(0xffffffffu, f));
+    }
   }
   if (lane == 0) warp_cnt[warp] = cnt;  // (the same in every lane)
   __syncthreads();
@@ -1619,7 +1704,7 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
         for (long long c0 = swb; c0 < edge; c0 += 32) {
           const long long i = c0 + lane;
           float z;
-          const bool f = (i < edge) && compact_flag(p, i, &z, rc2);
+          const bool f = (i < edge) && compact_flag(p, i, (i < edge) ? p.v[i] : 0.f, &z, rc2);
           c += __popc(__ballot_sync(0xffffffffu, f));
         }
         break;
@@ -1633,7 +1718,7 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
     for (long long c0 = wb; c0 < we; c0 += 32) {
       const long long i = c0 + lane;
       float z = 0.f;
-      const bool f = (i < we) && compact_flag(p, i, &z, rcache);
+      const bool f = (i < we) && compact_flag(p, i, (i < we) ? p.v[i] : 0.f, &z, rcache);
       const unsigned bal = __ballot_sync(0xffffffffu, f);
       if (f) {
         const unsigned long long dst = running + __popc(bal & ((1u << lane) - 1u));

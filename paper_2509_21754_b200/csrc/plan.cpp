@@ -25,6 +25,9 @@ Tuning read_tuning_env() {
   t.no_pitched_copy = env_int("FITRIG_NO_PITCHED_COPY", 0);
   t.no_pdl = env_int("FITRIG_NO_PDL", 0);
   t.old_generic = env_int("FITRIG_OLD_GENERIC", 0);
+  t.march_cons = env_int("FITRIG_MARCH_CONS", 0);
+  t.march_prod = env_int("FITRIG_MARCH_PROD", 0);
+  t.march_box_kb = env_int("FITRIG_MARCH_BOX_KB", 0);
   return t;
 }
 
@@ -177,14 +180,22 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   if (c < 1 || c > kMarchMaxCell || U < 1) return m;
   const int cells_x = (W + c - 1) / c, cells_y = (rows + c - 1) / c;
   auto width = [&](int ntx) { return (ntx * c + 3) / 4 * 4; };
-  const int pad = shifted_rows ? 8 : 0;  // (cp.async variant: a row is shifted by up to 3 floats and its last 16-byte copy may overhang)
+  // cp.async variant: a box is shifted by up to 3 floats, the last 16-byte copy of a row may overhang by 3 more, and the
+  // pitch must be congruent to W modulo 4 (global and shared addresses then agree modulo 16 bytes in every row)
+  auto pad_of = [&](int bw) { return shifted_rows ? 8 + (((W - bw - 8) % 4) + 4) % 4 : 0; };
+  const int pad = shifted_rows ? 11 : 0;  // (the largest pad_of: sizes the boxes)
   int ntx = std::max(1, std::min(cells_x, 256 / c));
-  if (c <= 10 && ntx > 32) ntx = 32;  // cells of a few pixels: a warp takes 32 adjacent cells, one per lane (kMarchTinyCell)
+  if (c <= kMarchTinyCell && ntx > 32) ntx = 32;  // cells of a few pixels: a warp takes 32 adjacent cells, one per lane
   while (ntx > 1 && (width(ntx) > 256 || (long long)(width(ntx) + pad) * c * 4 > 48 * 1024)) --ntx;  // >= 4 boxes in the ring
   // boxes of about 32 KB (the fused kernel's box): long rows for HBM, several boxes in flight per SM
-  const int kWarps = 24;  // consumer warps of the kernel (kMarchWarps)
+  int nprod = shifted_rows ? kMarchProducers : 1;
+  if (shifted_rows && tn.march_prod > 0) nprod = std::min(tn.march_prod, kMarchMaxWarps - 1);
+  int kWarps = shifted_rows ? kMarchWarpsCp : kMarchWarps;  // consumer warps of the kernel
+  if (tn.march_cons > 0) kWarps = tn.march_cons;
+  kWarps = std::max(1, std::min(kWarps, kMarchMaxWarps - nprod));
+  const int box_target = (tn.march_box_kb > 0 ? tn.march_box_kb : 32) * 1024;
   auto rows_fit = [&](int bytes) { return std::max(1, std::min(std::min(cells_y, 256 / c), bytes / ((width(ntx) + pad) * 4 * c))); };
-  int nty = rows_fit(32 * 1024);
+  int nty = rows_fit(box_target);
   auto pairs = [&](int nx, int ny) { return (long long)((cells_x + nx - 1) / nx) * ((cells_y + ny - 1) / ny) * U; };
   // small problems are latency bound: smaller boxes give more CTAs something to do
   bool shrunk = false;
@@ -196,10 +207,10 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   if (!shrunk) {
     // the consumer warps share a box's items (a row of floor(32 / c) adjacent cells, or one cell when c > 32): prefer
     // the box height, up to 40 KB, that leaves the fewest warps idle in the last round
-    const int per_row = (c <= 10) ? (ntx + 31) / 32 : (c <= 32) ? (ntx + 32 / c - 1) / (32 / c) : ntx;
+    const int per_row = (c <= kMarchTinyCell) ? (ntx + 31) / 32 : (c <= 32) ? (ntx + 32 / c - 1) / (32 / c) : ntx;
     auto eff = [&](int ny) { const int it = ny * per_row; return (double)it / (double)((it + kWarps - 1) / kWarps * kWarps); };
     int best = nty;
-    for (int ny = std::max(1, nty / 2); ny <= rows_fit(40 * 1024); ++ny)
+    for (int ny = std::max(1, nty / 2); ny <= rows_fit(box_target + box_target / 4); ++ny)
       if (eff(ny) > eff(best) + 1e-9 || (eff(ny) > eff(best) - 1e-9 && ny > best && ny <= nty)) best = ny;
     nty = best;
   }
@@ -208,7 +219,8 @@ MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& t
   const int qx = 4 / std::gcd(c, 4);
   if (ntx < cells_x && ntx >= qx) ntx = ntx / qx * qx;
   m.x_aligned = (ntx >= cells_x) || ((ntx * c) % 4 == 0);
-  m.ntx = ntx; m.nty = nty; m.bwp = width(ntx); m.bh = nty * c; m.pitch = m.bwp + pad;
+  m.ncons = kWarps; m.nprod = nprod;
+  m.ntx = ntx; m.nty = nty; m.bwp = width(ntx); m.bh = nty * c; m.pitch = m.bwp + pad_of(m.bwp);
   m.ngx = (cells_x + ntx - 1) / ntx; m.ngy = (cells_y + nty - 1) / nty;
   const int slot = (m.bh * m.pitch * 4 + 127) / 128 * 128;
   int stages = std::min(kMaxStages, (kMaxSmemPerCta - 2048) / slot);

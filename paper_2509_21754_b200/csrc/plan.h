@@ -42,6 +42,9 @@ struct Tuning {
   int no_pitched_copy;  // FITRIG_NO_PITCHED_COPY fitrig_stream: one copy per snapshot instead of one pitched copy per strip
   int no_pdl;           // FITRIG_NO_PDL         plain launches instead of programmatic dependent launches
   int old_generic;      // FITRIG_OLD_GENERIC    generic path: the three-reads-per-pixel kernel instead of the time-marching one
+  int march_cons;       // FITRIG_MARCH_CONS     generic time-marching kernel: consumer warps per CTA
+  int march_prod;       // FITRIG_MARCH_PROD     generic time-marching kernel, cp.async variant: producer warps per CTA
+  int march_box_kb;     // FITRIG_MARCH_BOX_KB   generic time-marching kernel: target size of a box in KB
 };
 Tuning read_tuning_env();
 
@@ -63,6 +66,12 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan);
 // Generic time-marching kernel (kernels.cuh, tlisi_march_kernel): boxes of nty x ntx whole cells of c pixels.
 constexpr int kMarchMaxCell = 112;     // the ring needs >= 4 boxes of c x c floats in shared memory
+constexpr int kMarchMaxWarps = 24;     // warps per CTA (768 threads: up to 85 registers each)
+constexpr int kMarchWarps = 23;        // consumer warps of the TMA variant (+ 1 producer warp, one lane of which issues the boxes): the
+                                       // inner loop is a chain of dependent shared-memory loads and fp32 operations, so it wants many warps
+constexpr int kMarchWarpsCp = 16;      // consumer warps of the cp.async variant ...
+constexpr int kMarchProducers = 8;     // ... and its producer warps (16-byte copies: 512 bytes per warp instruction)
+constexpr int kMarchTinyCell = 10;     // cells up to this size: one lane per cell (see the kernel)
 struct MarchPlan {
   bool ok;        // false: the cell is too large for the ring (the caller takes the three-reads-per-pixel kernel)
   int ntx, nty;   // cells per box
@@ -70,6 +79,7 @@ struct MarchPlan {
   int pitch;      // floats between box rows in shared memory: bwp, or bwp + 8 for the shifted rows of the cp.async variant
   int ngx, ngy;   // boxes per row of boxes, rows of boxes
   int nstage, grid, smem_bytes;
+  int ncons, nprod; // consumer and producer warps per CTA
   bool x_aligned; // every box starts on a 16-byte boundary of its row (a condition for fetching it by TMA)
 };
 MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn, bool shifted_rows);
