@@ -247,25 +247,38 @@ __device__ __forceinline__ int geom_block_row(int lane) { return LaneGeom<T>::su
 template <int T>
 __device__ __forceinline__ int geom_block_col(int lane) { return LaneGeom<T>::sub_col(lane) * T + LaneGeom<T>::col_in_tile(lane); }
 
+// Which row of its warp's 32x32 block the j-th float4 (j = 0..7) of a lane comes from; its columns are 4 (lane & 7) ..
+// for LT = 32, 4, 2 and geom_block_col<LT> otherwise.  LT = 32, 16, 8: LaneGeom above.  Tiles of 4 and 2 pixels: a lane
+// holds WHOLE tiles (no reduction across lanes): lane = [rq 2 bits][cg 3 bits],
+//   LT = 4  rows 16 (j / 4) + 4 rq + j % 4: the two 4x4 tiles (tile row rq and rq + 4, tile column cg)
+//   LT = 2  rows  8 (j / 2) + 2 rq + j % 2: the eight 2x2 tiles (tile rows rq + 4 (j / 2), tile columns 2 cg, 2 cg + 1)
+// In every geometry a quarter warp reads one 128-byte row per load (conflict free).
+template <int LT>
+__device__ __forceinline__ int lane_row(int lane, int j) {
+  if (LT == 4) return 16 * (j >> 2) + 4 * (lane >> 3) + (j & 3);
+  if (LT == 2) return 8 * (j >> 1) + 2 * (lane >> 3) + (j & 1);
+  return geom_block_row<(LT == 4 || LT == 2) ? 32 : LT>(lane) + LaneGeom<(LT == 4 || LT == 2) ? 32 : LT>::RPL * j;
+}
+template <int LT>
+__device__ __forceinline__ int lane_col(int lane) { return geom_block_col<(LT == 4 || LT == 2) ? 32 : LT>(lane); }
+
 // The lane's 32 pixels out of a box (row pitch `pitch` bytes) into registers / added to registers.
-template <int T>
+template <int LT>
 __device__ __forceinline__ void load_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
-  using G = LaneGeom<T>;
-  const unsigned char* src = block_ptr + geom_block_row<T>(lane) * pitch + geom_block_col<T>(lane) * 4;
+  const unsigned char* src = block_ptr + lane_col<LT>(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
+    const float4 t = *reinterpret_cast<const float4*>(src + lane_row<LT>(lane, j) * pitch);
     N[4 * j] = t.x; N[4 * j + 1] = t.y; N[4 * j + 2] = t.z; N[4 * j + 3] = t.w;
   }
 }
 
-template <int T>
+template <int LT>
 __device__ __forceinline__ void add_tile(float (&N)[32], const unsigned char* block_ptr, int pitch, int lane) {
-  using G = LaneGeom<T>;
-  const unsigned char* src = block_ptr + geom_block_row<T>(lane) * pitch + geom_block_col<T>(lane) * 4;
+  const unsigned char* src = block_ptr + lane_col<LT>(lane) * 4;
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    const float4 t = *reinterpret_cast<const float4*>(src + G::RPL * j * pitch);
+    const float4 t = *reinterpret_cast<const float4*>(src + lane_row<LT>(lane, j) * pitch);
     N[4 * j] += t.x; N[4 * j + 1] += t.y; N[4 * j + 2] += t.z; N[4 * j + 3] += t.w;
   }
 }
@@ -340,6 +353,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
   // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
   constexpr bool kSmall = T < 8;
+  constexpr int kLoadGeom = (T == 1) ? 32 : T;  // which pixels a lane holds (lane_row / lane_col)
   using Geo = LaneGeom<(kSmall ? 32 : T)>;
   constexpr int LPT = Geo::LPT, NGRP = 32 / LPT;  // lanes per tile, tiles (lane groups) per warp
   const int acc = ACC ? p.acc : 1;  // ACC = false compiles the accumulation loops away
@@ -411,13 +425,13 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
   auto acquire = [&](float (&N)[32], float& zmin) {
     mbar_wait(full_addr + slot * 8, phase);
-    load_tile<(kSmall ? 32 : T)>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+    load_tile<kLoadGeom>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
     __syncwarp();  // every lane has its copy
     if (lane == 0) mbar_arrive(empty_addr + slot * 8);
     if (++slot == p.nstage) { slot = 0; phase ^= 1; }
     for (int i = 1; i < acc; ++i) {  // accumulation: the image is the sum of acc raw snapshots, added in order
       mbar_wait(full_addr + slot * 8, phase);
-      add_tile<(kSmall ? 32 : T)>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+      add_tile<kLoadGeom>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty_addr + slot * 8);
       if (++slot == p.nstage) { slot = 0; phase ^= 1; }
@@ -537,65 +551,71 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     rp += raw_step;
   };
 
-  // ---- tiles of 4, 2 or 1 pixels: N = x^(s+2), X = x^(s+1) (reference image), dp = signed x^(s+1) - x^(s).  Every
-  // 16-byte quad of a lane (row rb + 4j, columns 4cg .. 4cg+3) is one tile row (T = 4), two tiles' rows (T = 2) or
-  // four tiles (T = 1); lanes that hold the other rows of the same tiles differ in rb only (xor 8, 16), so a tile is
-  // reduced by at most two shuffle levels and its first max-Delta pixel (R20) is exact without a re-read.
+  // ---- tiles of 4, 2 or 1 pixels: N = x^(s+2), X = x^(s+1) (reference image), dp = signed x^(s+1) - x^(s).  A lane holds
+  // whole tiles (lane_row above; T = 1: every pixel is a tile), so there is no reduction across lanes, the first max-Delta
+  // pixel (R20) is exact without a re-read, and a lane writes its tiles' records itself (the 8 lanes of a quarter warp
+  // write consecutive records: 128 to 512 contiguous bytes).
   int ty0 = 0, tx0 = 0;  // first tile of the warp's block, in tiles
   auto small_step = [&](const float (&N)[32], const float (&X)[32], float (&dq)[32]) {
-    const int rb = lane >> 3, cg = lane & 7;
+    const int rq = lane >> 3, cg = lane & 7;
+    auto pixel = [&](int k, float& delta, float& r) {
+      const float d = N[k] - X[k];                          // signed D^(s+1), Eq. 3
+      delta = fabsf(fabsf(d) - fabsf(dq[k]));               // |D^(s) - D^(s+1)|
+      dq[k] = d;
+      r = clamped_ratio<REF_MODE>(delta, X[k], p.C);        // Eq. 4-5, per pixel (R8 exact)
+    };
+    if (T == 4) {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      float dl[4], rr[4];
+      for (int h = 0; h < 2; ++h) {  // pixels 16 h .. 16 h + 15 are tile (rq + 4 h, cg) in row-major order
+        float S = 0.f, R = 0.f, Mx = -1.f;
+        int pos = 0;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const int k = 4 * j + e;
-        const float d = N[k] - X[k];                          // signed D^(s+1), Eq. 3
-        dl[e] = fabsf(fabsf(d) - fabsf(dq[k]));               // |D^(s) - D^(s+1)|
-        dq[k] = d;
-        rr[e] = clamped_ratio<REF_MODE>(dl[e], X[k], p.C);    // Eq. 4-5, per pixel (R8 exact)
-      }
-      const int row = rb + 4 * j;  // row inside the block
-      if (T == 4) {
-        float S = ((dl[0] + dl[1]) + dl[2]) + dl[3], R = ((rr[0] + rr[1]) + rr[2]) + rr[3];
-        float Mx = fmaxf(fmaxf(dl[0], dl[1]), fmaxf(dl[2], dl[3]));
-        int pos = rb * 4 + ((dl[0] == Mx) ? 0 : (dl[1] == Mx) ? 1 : (dl[2] == Mx) ? 2 : 3);  // row-major in the tile
-#pragma unroll
-        for (int off = 8; off <= 16; off <<= 1) {
-          S += __shfl_xor_sync(0xffffffffu, S, off);
-          R += __shfl_xor_sync(0xffffffffu, R, off);
-          const float om = __shfl_xor_sync(0xffffffffu, Mx, off);
-          const int op = __shfl_xor_sync(0xffffffffu, pos, off);
-          if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
+        for (int k = 0; k < 16; ++k) {
+          float delta, r;
+          pixel(16 * h + k, delta, r);
+          S += delta;
+          R += r;
+          if (delta > Mx) { Mx = delta; pos = k; }  // strict: the first maximum
         }
-        const int ty_r = j, tx_r = cg;
-        if (rb == 0 && ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
+        const int ty_r = rq + 4 * h, tx_r = cg;
+        if (ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
           RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
           rp[(long long)ty_r * p.Tx + tx_r] = o;
         }
-      } else if (T == 2) {
+      }
+    } else if (T == 2) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          float S = dl[2 * h] + dl[2 * h + 1], R = rr[2 * h] + rr[2 * h + 1];
-          float Mx = fmaxf(dl[2 * h], dl[2 * h + 1]);
-          int pos = (rb & 1) * 2 + ((dl[2 * h] == Mx) ? 0 : 1);
-          S += __shfl_xor_sync(0xffffffffu, S, 8);
-          R += __shfl_xor_sync(0xffffffffu, R, 8);
-          const float om = __shfl_xor_sync(0xffffffffu, Mx, 8);
-          const int op = __shfl_xor_sync(0xffffffffu, pos, 8);
-          if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
-          const int ty_r = row >> 1, tx_r = 2 * cg + h;
-          if ((rb & 1) == 0 && ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
+      for (int jp = 0; jp < 4; ++jp) {  // row pair jp: float4 2 jp (upper row) and 2 jp + 1 (lower row)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {   // the left / right tile of the quad
+          const int k0 = 8 * jp + 2 * h, k1 = k0 + 4;
+          float d0, d1, d2, d3, r0, r1, r2, r3;
+          pixel(k0, d0, r0); pixel(k0 + 1, d1, r1); pixel(k1, d2, r2); pixel(k1 + 1, d3, r3);
+          const float S = ((d0 + d1) + d2) + d3;
+          const float R = ((r0 + r1) + r2) + r3;
+          float Mx = d0;
+          int pos = 0;
+          if (d1 > Mx) { Mx = d1; pos = 1; }
+          if (d2 > Mx) { Mx = d2; pos = 2; }
+          if (d3 > Mx) { Mx = d3; pos = 3; }
+          const int ty_r = rq + 4 * jp, tx_r = 2 * cg + h;
+          if (ty0 + ty_r < p.ty_end && tx0 + tx_r < p.Tx) {
             RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
             rp[(long long)ty_r * p.Tx + tx_r] = o;
           }
         }
-      } else {  // T == 1: per-pixel detection
+      }
+    } else {  // T == 1: per-pixel detection; float4 j holds row rq + 4 j, columns 4 cg ..
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int row = rq + 4 * j;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
           const int tx_r = 4 * cg + e;
+          float delta, r;
+          pixel(4 * j + e, delta, r);
           if (ty0 + row < p.ty_end && tx0 + tx_r < p.Tx) {
-            RawTile o; o.sumD = dl[e]; o.maxD = dl[e]; o.sumR = rr[e]; o.pos = 0;
+            RawTile o; o.sumD = delta; o.maxD = delta; o.sumR = r; o.pos = 0;
             rp[(long long)row * p.Tx + tx_r] = o;
           }
         }
@@ -1237,6 +1257,7 @@ __device__ __forceinline__ void row_stats_finish(StatPartial part, double K, int
 // finalize: q, tLISI, per-row statistics (a6, a7).  Map rows are (batch entry, unit) pairs, row = b * U + u.
 // ---------------------------------------------------------------------------------------------
 constexpr int kFinChunk = 1024;       // map entries per block and pass: at least this many ...
+constexpr int kFinLoads = 4;          // records a thread has in flight
 constexpr int kFinChunkMax = 16384;   // ... and at most this many (chosen per context from the map size, fitrig_create)
 
 struct FinalizeParams {
@@ -1267,6 +1288,7 @@ struct FinalizeParams {
 // entry, which made the per-pixel maps compute bound); a partial edge window divides by its own count.
 __device__ __forceinline__ double tile_product(const RawTile r, int t, int Tx, int H, int W, int tile, int stride,
                                                double inv_full) {
+  if (H < 0) return ((double)r.sumD * inv_full) * (double)r.maxD * ((double)r.sumR * inv_full);  // (the caller says: no partial window)
   const int ty = (int)((unsigned)t / (unsigned)Tx), tx = t - ty * Tx;
   const int h = min(tile, H - ty * stride), w = min(tile, W - tx * stride);
   const double inv_n = (h == tile && w == tile) ? inv_full : 1.0 / ((double)h * (double)w);
@@ -1290,6 +1312,9 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
   const int nt = p.Ty * p.Tx;
   const int R = p.B * p.U;
   const double inv_full = 1.0 / ((double)p.tile * (double)p.tile);
+  // no partial window at the bottom / right edge: every entry divides by tile^2 (no index arithmetic per entry)
+  const bool all_full = (p.Ty - 1) * p.stride + p.tile <= p.H && (p.Tx - 1) * p.stride + p.tile <= p.W;
+  const int Hq = all_full ? -1 : p.H;
   const long long nchunks = (long long)R * p.nblk;
   const int vlen = 2 + 2 * p.U;  // length of one shard's export vector
   for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
@@ -1308,24 +1333,37 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
     const double inv_m2 = 1.0 / ((double)M * (double)M);
     const size_t base = (size_t)row * nt;
     // the row's shift: its first q value
-    const double K = (double)(float)(tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2);
+    const double K = (double)(float)(tile_product(p.raw[base], 0, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2);
     const int begin = blk * p.chunk, end = min(nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
-#pragma unroll 4
-    for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
-      // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2, combined in fp64 and rounded once
-      const double qd = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) * inv_m2;
-      const float qf = (float)qd;
-      p.q[base + t] = qf;
-      const float tl = (float)(1.0 - qd);
-      p.tlisi[base + t] = tl;
-      if (p.tlisi_user) {
-        if (p.user_row < 0) p.tlisi_user[base + t] = tl;
-        else if (row == p.user_row) p.tlisi_user[t] = tl;
+    // kFinLoads records per thread are fetched before the first is used (the stores below may alias the loads as far as
+    // the compiler knows, so it would not hoist them itself): a big map is a stream, and one record in flight per thread
+    // leaves it latency bound
+    for (int t0 = begin + threadIdx.x; t0 < end; t0 += kFinLoads * blockDim.x) {
+      RawTile rec[kFinLoads];
+#pragma unroll
+      for (int k = 0; k < kFinLoads; ++k) {
+        const int t = t0 + k * blockDim.x;
+        if (t < end) rec[k] = p.raw[base + t];
       }
-      const double d = (double)qf - K;
-      s += d;
-      s2 += d * d;
+#pragma unroll
+      for (int k = 0; k < kFinLoads; ++k) {
+        const int t = t0 + k * blockDim.x;
+        if (t >= end) break;
+        // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2, combined in fp64 and rounded once
+        const double qd = tile_product(rec[k], t, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2;
+        const float qf = (float)qd;
+        p.q[base + t] = qf;
+        const float tl = (float)(1.0 - qd);
+        p.tlisi[base + t] = tl;
+        if (p.tlisi_user) {
+          if (p.user_row < 0) p.tlisi_user[base + t] = tl;
+          else if (row == p.user_row) p.tlisi_user[t] = tl;
+        }
+        const double d = (double)qf - K;
+        s += d;
+        s2 += d * d;
+      }
     }
     if (p.shard_all) {
       // Eq. 8 over ALL tiles of the image: the shards' (n, mean, M2) of the M-free product p, merged in shard order
@@ -1599,37 +1637,108 @@ struct CompactParams {
   long long seg;        // entries per block (multiple of 32 * warps)
 };
 
-// z of entry i (Eq. 8 on q, R21; sigma == 0 -> z = 0, R4) and the strict threshold (R6).  1 / sigma of the current
-// row is kept by the thread (its entries stay in one row for long stretches): one fp64 multiply per entry instead
-// of a double-precision division, which dominated per-pixel maps.
-constexpr int kCompactLoads = 4;  // map entries a lane loads before it tests them (pass 1)
+constexpr int kCompactLoads = 8;  // map entries a lane has in flight
 
-struct RowCache {
-  int row = -1;
-  long long row_end = 0;  // first entry index of the next row
-  double mu = 0.0, inv_sigma = 0.0;
+// Walks the map entries [b, e) in order -- one warp, all lanes -- and counts (WRITE: also writes, from position
+// `running` on) the entries with z > tau.  z of an entry (Eq. 8 on q, R21; sigma == 0 -> z = 0, R4) is formed in fp64,
+// rounded to fp32 and compared strictly (R6).  The walk goes row by row: per row, mu, 1 / sigma and a CONSERVATIVE
+// fp32 bound thr are set up once (every entry with z > tau has v > thr: thr lies 4e-7 (|mu| + |tau sigma|) below
+// mu + tau sigma, far more than the rounding of the fp64 test), so that an entry costs one load and one fp32
+// comparison, and only the (rare) survivors of a 32-entry group take the exact test.
+// A candidate record from its map entry (row, tile t of the row) and score.
+__device__ __forceinline__ fitrig_candidate make_candidate(const CompactParams& p, int row, unsigned t, float z) {
+  const long long row_begin = (long long)row * p.nt;
+  const int bidx = row / p.rows_per_batch;
+  const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
+  fitrig_candidate cd;
+  if (p.branch == FITRIG_BRANCH_IMAGE) {
+    const int pos = p.raw[row_begin + t].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
+    cd.x = tx * p.stride + pos % p.tile;
+    cd.y = p.row_offset + ty * p.stride + pos / p.tile;
+    cd.snapshot = (row - bidx * p.rows_per_batch) + p.unit_offset;
+  } else {
+    const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
+    cd.x = tx * p.stride + w / 2;  // tile centre (R18)
+    cd.y = p.row_offset + ty * p.stride + h / 2;
+    cd.snapshot = p.kstar[row_begin + t];
+  }
+  cd.score = z;
+  return cd;
+}
+
+constexpr int kCompactStage = 64;  // candidates a warp keeps from its counting pass (more: it walks its range again)
+struct StagedCand {
+  int row;
+  unsigned t;
+  float z;
 };
 
-__device__ __forceinline__ bool compact_flag(const CompactParams& p, long long i, float v, float* z_out, RowCache& rc) {
-  if (rc.row < 0 || i >= rc.row_end || i < rc.row_end - p.nt) {  // entries mostly move forward: rarely a division
-    if (rc.row < 0 || i >= rc.row_end + p.nt || i < rc.row_end - p.nt) {
-      rc.row = (int)(i / p.nt);
-      rc.row_end = (long long)(rc.row + 1) * p.nt;
+// MODE 0: count; 1: count and keep the first kCompactStage candidates in `stage`; 2: write from position `running` on
+template <int MODE>
+__device__ __forceinline__ unsigned compact_walk(const CompactParams& p, long long b, long long e, int lane,
+                                                 unsigned long long running, StagedCand* stage) {
+  constexpr bool WRITE = MODE == 2;
+  unsigned cnt = 0;
+  while (b < e) {
+    const int row = (int)(b / p.nt);
+    const long long row_begin = (long long)row * p.nt;
+    const int n = (int)(min(e, row_begin + p.nt) - b);  // entries of this row in the range
+    const double sd = p.sigma[row], mu = p.mu[row];
+    const double inv_sigma = (sd > 0.0) ? 1.0 / sd : 0.0;
+    float thr;
+    if (sd > 0.0) {
+      const double ts = (double)p.tau * sd;
+      thr = __double2float_rd(mu + ts - 4e-7 * (fabs(mu) + fabs(ts)));
     } else {
-      rc.row += 1;
-      rc.row_end += p.nt;
+      thr = (0.f > p.tau) ? -3.402823466e38f : 3.402823466e38f;  // z == 0 everywhere: all entries, or none
     }
-    const double sd = p.sigma[rc.row];
-    rc.mu = p.mu[rc.row];
-    rc.inv_sigma = (sd > 0.0) ? 1.0 / sd : 0.0;
+    const float* v = p.v + b;
+    const int t0 = (int)(b - row_begin);  // tile index of v[0] inside the row
+    for (int c0 = 0; c0 < n; c0 += 32 * kCompactLoads) {
+      float vv[kCompactLoads];
+#pragma unroll
+      for (int k = 0; k < kCompactLoads; ++k) {
+        const int o = c0 + 32 * k + lane;
+        vv[k] = (o < n) ? v[o] : 0.f;
+      }
+#pragma unroll
+      for (int k = 0; k < kCompactLoads; ++k) {
+        const int o = c0 + 32 * k + lane;
+        const bool pre = (o < n) && (vv[k] > thr || sd <= 0.0 && 0.f > p.tau);
+        if (__ballot_sync(0xffffffffu, pre) == 0u) continue;
+        float z = 0.f;
+        bool f = false;
+        if (pre) {
+          z = (float)(((double)vv[k] - mu) * inv_sigma);
+          f = z > p.tau;  // strict, R6
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, f);
+        if (MODE != 0 && f) {
+          const unsigned k_in = cnt + __popc(bal & ((1u << lane) - 1u));  // place among this walk's candidates
+          const unsigned t = (unsigned)(t0 + o);                          // tile index inside the row (< 2^31)
+          if (WRITE) {
+            const unsigned long long dst = running + k_in;
+            if ((long long)dst < p.cap) {
+              const fitrig_candidate cd = make_candidate(p, row, t, z);
+              p.out[dst] = cd;
+              if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
+            }
+          } else if (k_in < (unsigned)kCompactStage) {
+            StagedCand sc; sc.row = row; sc.t = t; sc.z = z;
+            stage[k_in] = sc;
+          }
+        }
+        cnt += __popc(bal);
+      }
+    }
+    b += n;
   }
-  const double z = ((double)v - rc.mu) * rc.inv_sigma;
-  *z_out = (float)z;
-  return (float)z > p.tau;  // strict, R6
+  return cnt;
 }
 
 __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   __shared__ unsigned warp_cnt[16];
+  __shared__ StagedCand s_stage[16][kCompactStage];
   __shared__ unsigned long long s_base;
   __shared__ unsigned s_id;
   pdl_wait();
@@ -1647,24 +1756,8 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
   const long long wlen = p.seg / nw;  // a multiple of 32
   const long long wb = min(end, begin + warp * wlen), we = min(end, wb + wlen);
 
-  RowCache rcache;
   // ---- pass 1: count ----
-  unsigned cnt = 0;
-  for (long long c0 = wb; c0 < we; c0 += 32 * kCompactLoads) {
-    float v[kCompactLoads];  // independent loads first: one outstanding line per warp cannot feed a map of 10^8 entries
-#pragma unroll
-    for (int k = 0; k < kCompactLoads; ++k) {
-      const long long i = c0 + 32 * k + lane;
-      v[k] = (i < we) ? p.v[i] : 0.f;
-    }
-#pragma unroll
-    for (int k = 0; k < kCompactLoads; ++k) {
-      const long long i = c0 + 32 * k + lane;
-      float z;
-      const bool f = (i < we) && compact_flag(p, i, v[k], &z, rcache);
-      cnt += __popc(__ballot_sync(0xffffffffu, f));
-    }
-  }
+  const unsigned cnt = compact_walk<1>(p, wb, we, lane, 0ull, s_stage[warp]);
   if (lane == 0) warp_cnt[warp] = cnt;  // (the same in every lane)
   __syncthreads();
   unsigned before = 0, total = 0;
@@ -1700,51 +1793,25 @@ __global__ void __launch_bounds__(512) compact_kernel(const CompactParams p) {
         const long long swb = min(end, begin + w * wlen), swe = min(end, swb + wlen);
         if (swe <= edge) { c += warp_cnt[w]; continue; }
         if (swb >= edge) break;
-        RowCache rc2;
-        for (long long c0 = swb; c0 < edge; c0 += 32) {
-          const long long i = c0 + lane;
-          float z;
-          const bool f = (i < edge) && compact_flag(p, i, (i < edge) ? p.v[i] : 0.f, &z, rc2);
-          c += __popc(__ballot_sync(0xffffffffu, f));
-        }
+        c += compact_walk<0>(p, swb, edge, lane, 0ull, nullptr);
         break;
       }
       if (lane == 0) p.host_offsets[b] = c;
     }
   }
-  // ---- pass 2: write in order (only warps that hold candidates) ----
-  if (cnt != 0) {
-    unsigned long long running = base + before;
-    for (long long c0 = wb; c0 < we; c0 += 32) {
-      const long long i = c0 + lane;
-      float z = 0.f;
-      const bool f = (i < we) && compact_flag(p, i, (i < we) ? p.v[i] : 0.f, &z, rcache);
-      const unsigned bal = __ballot_sync(0xffffffffu, f);
-      if (f) {
-        const unsigned long long dst = running + __popc(bal & ((1u << lane) - 1u));
-        if ((long long)dst < p.cap) {
-          const int row = rcache.row;  // compact_flag has just placed entry i in its row
-          const int bidx = row / p.rows_per_batch;
-          const unsigned t = (unsigned)(i - (rcache.row_end - p.nt));  // tile index inside the row (< 2^31)
-          const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
-          fitrig_candidate cd;
-          if (p.branch == FITRIG_BRANCH_IMAGE) {
-            const int pos = p.raw[i].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
-            cd.x = tx * p.stride + pos % p.tile;
-            cd.y = p.row_offset + ty * p.stride + pos / p.tile;
-            cd.snapshot = (row - bidx * p.rows_per_batch) + p.unit_offset;
-          } else {
-            const int h = min(p.tile, p.H - ty * p.stride), w = min(p.tile, p.W - tx * p.stride);
-            cd.x = tx * p.stride + w / 2;  // tile centre (R18)
-            cd.y = p.row_offset + ty * p.stride + h / 2;
-            cd.snapshot = p.kstar[i];
-          }
-          cd.score = z;
-          p.out[dst] = cd;
-          if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
-        }
+  // ---- write in order: the candidates kept from the counting pass, or -- a warp with more of them than it could keep --
+  // a second walk
+  if (cnt > (unsigned)kCompactStage) {
+    compact_walk<2>(p, wb, we, lane, base + before, nullptr);
+  } else {
+    for (unsigned k = lane; k < cnt; k += 32) {
+      const unsigned long long dst = base + before + k;
+      if ((long long)dst < p.cap) {
+        const StagedCand sc = s_stage[warp][k];
+        const fitrig_candidate cd = make_candidate(p, sc.row, sc.t, sc.z);
+        p.out[dst] = cd;
+        if ((long long)dst < p.host_cap) p.host_out[dst] = cd;
       }
-      running += __popc(bal);
     }
   }
 }
