@@ -37,6 +37,9 @@
  *       FITRIG_OLD_GENERIC=1     generic path: the three-reads-per-pixel kernel instead of the time-marching one
  *       FITRIG_NO_PITCHED_COPY=1 fitrig_stream: one copy per snapshot and strip instead of one pitched copy per strip
  *       FITRIG_NO_PDL=1          plain stream-ordered launches instead of programmatic dependent launches
+ *       FITRIG_MARCH_CONS=n      generic kernel: n consumer warps per CTA (default 23 with TMA boxes, 16 with cp.async rows)
+ *       FITRIG_MARCH_PROD=n      generic kernel, cp.async variant: n producer warps per CTA (default 8)
+ *       FITRIG_MARCH_BOX_KB=n    generic kernel: boxes of about n KB (default 32)
  */
 #ifndef FITRIG_H_
 #define FITRIG_H_
@@ -261,8 +264,8 @@ int fitrig_push_reset(fitrig_ctx* ctx);
 /* Row shards (tiles are independent).  One image is cut into
  * horizontal shards of whole tile rows, one context (normally one GPU) per shard, each created with the
  * shard's own H and params.row_offset.  Only the three global scalars of the method couple the shards:
- * M and, per unit, the mean and standard deviation of the tile matrix (Eq. 8).  Protocol,
- * image branch only:
+ * M and, per unit, the mean and standard deviation of the tile matrix (Eq. 8).  Protocol
+ * (the frequency branch adds the second exchange described below):
  *     fitrig_tlisi(shard)                       local map, provisional (M of the shard alone)
  *     fitrig_shard_export -> v[2 + 2U]          what the other shards need
  *     all-gather v over the shards              the ONE exchange step (NCCL; (2 + 2U) * 8 bytes per rank)
@@ -272,16 +275,19 @@ int fitrig_push_reset(fitrig_ctx* ctx);
  * fitrig_shard_export -- d_out (device) receives 2 + 2U doubles:
  *   [0]            largest pixel value of this shard's L snapshots (signed, not floored at C; R2)
  *   [1]            number of tiles per unit in this shard
- *   [2 .. 2+U)     per unit: sum over tiles of p = (sum Delta / n_t) * max Delta * (sum r / n_t), i.e. the
- *                  product of Eq. 2 / Eq. 6 WITHOUT the 1/M^2 factor (q = p / M^2)
- *   [2+U .. 2+2U)  per unit: sum over tiles of p^2
- * Asynchronous on cuda_stream.  Errors: STATE (no current map), INVALID_ARG (NULL; frequency branch), CUDA. */
+ *   [2 .. 2+U)     per unit: MEAN over this shard's tiles of p = (sum Delta / n_t) * max Delta * (sum r / n_t), i.e.
+ *                  the product of Eq. 2 / Eq. 6 WITHOUT the 1/M^2 factor (q = p / M^2)
+ *   [2+U .. 2+2U)  per unit: M2 = sum over this shard's tiles of (p - that mean)^2
+ * ((n, mean, M2) triples merge without cancellation -- Chan's formula -- so a constant map keeps sigma == 0 exactly, R4.)
+ * Asynchronous on cuda_stream.  Errors: STATE (no current map), INVALID_ARG (NULL, batch), CUDA. */
 int fitrig_shard_export(fitrig_ctx* ctx, double* d_out, void* cuda_stream);
 
 /* fitrig_shard_import -- d_all (device): `world` export vectors back to back, [world][2 + 2U], in shard
  * order (identical on every shard so that all shards derive bit-identical M, mu, sigma).  Sets
  * M = max(max over shards, C), mu_u and sigma_u of q = p / M^2 over ALL tiles of the image (population
- * std, R3), rewrites this shard's q and tLISI with that M, and writes tLISI to d_tlisi (device,
+ * std, R3: the shards' (n, mean, M2) merged in shard order, n += n_b, mean += d n_b / n, M2 += M2_b + d^2 n_a n_b / n
+ * with d = mean_b - mean_a; mu = mean / M^2, sigma = sqrt(M2 / n) / M^2), rewrites this shard's q and tLISI with
+ * that M, and writes tLISI to d_tlisi (device,
  * [U][Ty_shard][Tx], may be NULL).  The shard's map is then bit-identical to the same rows of a
  * whole-image fitrig_tlisi.  Asynchronous.  Errors: STATE, INVALID_ARG (NULL, world < 1), CUDA. */
 int fitrig_shard_import(fitrig_ctx* ctx, const double* d_all, int32_t world, float* d_tlisi, void* cuda_stream);

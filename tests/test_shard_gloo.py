@@ -2,8 +2,8 @@
 
 The CUDA kernels cannot run here, so every rank stands in for its GPU with the ORACLE restricted to its own
 row shard (tests may use the oracle); what is under test is the product's host side of the sharded path
-(paper_2509_21754_b200/shard.py): the row split, the ONE all-gather of 2 + 2U doubles, the candidate gather
-and the (unit, tile row, tile col) merge -- and that the exchange protocol of include/fitrig.h
+(paper_2509_21754_b200/shard.py): the row split, the ONE all-gather of 2 + 2U doubles (plus the 3-double one of the
+frequency branch), the candidate gather and the (unit, tile row, tile col) merge -- and that the exchange protocol of include/fitrig.h
 (fitrig_shard_export / fitrig_shard_import) reproduces the whole-image result.  The merge arithmetic of
 fitrig_shard_import is restated below in numpy from its header comment.
 """
@@ -31,24 +31,47 @@ def _free_port():
 
 
 def _export_vector(stack_rows, tile):
-    """What fitrig_shard_export returns for a shard, from the oracle: M = 1 makes q the M-free product p."""
+    """What fitrig_shard_export returns for a shard, from the oracle: M = 1 makes q the M-free product p.
+    v = [largest pixel, tiles per unit, mean_p[U], M2_p[U]] (M2 = sum of squared deviations from the shard's mean)."""
     r = oracle.tlisi(stack_rows, tile=tile, M=1.0)
     U = r.U
     mx = max(float(s.max()) for s in stack_rows)
+    p = r.q.reshape(U, -1)
     v = np.zeros(2 + 2 * U)
     v[0], v[1] = mx, r.Ty * r.Tx
-    v[2:2 + U] = r.q.reshape(U, -1).sum(axis=1)
-    v[2 + U:] = (r.q.reshape(U, -1) ** 2).sum(axis=1)
+    v[2:2 + U] = p.mean(axis=1)
+    v[2 + U:] = ((p - p.mean(axis=1, keepdims=True)) ** 2).sum(axis=1)
     return v, r
 
 
+def _chan(n, mean, m2, nb, mb, m2b):
+    """Chan's merge of two (count, mean, M2) triples, as include/fitrig.h states it for fitrig_shard_import."""
+    if nb <= 0:
+        return n, mean, m2
+    tot = n + nb
+    d = mb - mean
+    return tot, mean + d * (nb / tot), m2 + m2b + d * d * (n * nb / tot)
+
+
 def _import(allv, U, C=1e-6):
-    """fitrig_shard_import's merge, restated from include/fitrig.h."""
+    """fitrig_shard_import's merge, restated from include/fitrig.h: M = max over shards (floored at C), and per unit the
+    shards' (n, mean, M2) merged in shard order; mu = mean / M^2, sigma = sqrt(M2 / n) / M^2."""
     M = max(float(np.float32(allv[:, 0].max())), C)
-    n = allv[:, 1].sum()
-    mean_p = allv[:, 2:2 + U].sum(axis=0) / n
-    var_p = np.maximum(allv[:, 2 + U:].sum(axis=0) / n - mean_p ** 2, 0.0)
-    return M, mean_p / M ** 2, np.sqrt(var_p) / M ** 2
+    mu, sd = np.zeros(U), np.zeros(U)
+    for u in range(U):
+        n, mean, m2 = 0.0, 0.0, 0.0
+        for r in range(allv.shape[0]):
+            n, mean, m2 = _chan(n, mean, m2, allv[r, 1], allv[r, 2 + u], allv[r, 2 + U + u])
+        mu[u], sd[u] = mean / M ** 2, np.sqrt(m2 / n) / M ** 2
+    return M, mu, sd
+
+
+def _import_eta(allw):
+    """fitrig_shard_import_eta's merge: the shards' (tiles, mean eta, M2 of eta) in shard order."""
+    n, mean, m2 = 0.0, 0.0, 0.0
+    for r in range(allw.shape[0]):
+        n, mean, m2 = _chan(n, mean, m2, allw[r, 0], allw[r, 1], allw[r, 2])
+    return mean, np.sqrt(m2 / n)
 
 
 def _worker(rank, world, port, H, W, L, tile, tau, ret):
@@ -95,6 +118,54 @@ def test_row_sharded_image_over_gloo(world, H, W, tile):
     mgr = mp.Manager()
     ret = mgr.dict()
     mp.spawn(_worker, args=(world, _free_port(), H, W, 8, tile, 3.0, ret), nprocs=world, join=True)
+    assert len(ret) == world and len(set(ret.values())) == 1
+
+
+def _worker_frequency(rank, world, port, H, W, L, tile, tau, ret):
+    """Frequency branch under row shards: the SECOND exchange (3 doubles: tiles, mean eta, M2 of eta), which can only
+    follow the first because eta scales with 1 / M^2 (include/fitrig.h, fitrig_shard_export_eta / _import_eta)."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        oracle.set_threads(1)
+        cfg = synth.scaled(synth.CONFIGS["imgfreq"], H, W, L=L)
+        st, _ = synth.make_stack(cfg, device="cpu")
+        full = [st[s].numpy() for s in range(L)]
+        r0, r1 = shard.row_shards(H, tile, world)[rank]
+        rows = [np.ascontiguousarray(x[r0:r1]) for x in full]
+        v, res = _export_vector(rows, tile)
+        allv = shard.all_gather_vectors(torch.from_numpy(v)).numpy()          # first exchange: M (and mu, sigma of q)
+        M, _, _ = _import(allv, L - 2)
+        eta, ks = oracle.spectrum(res.q / M ** 2)                              # this shard's tiles, global M
+        w = np.array([eta.size, eta.mean(), ((eta - eta.mean()) ** 2).sum()])
+        allw = shard.all_gather_vectors(torch.from_numpy(w)).numpy()          # second exchange: statistics of eta
+        assert allw.shape == (world, 3) and np.array_equal(allw[rank], w)
+        mean_eta, sd_eta = _import_eta(allw)
+        z = (eta - mean_eta) / sd_eta
+        sel = oracle.select_spectrum(z, ks, r1 - r0, W, tile, tau)
+        local = np.zeros(len(sel.x), dtype=CANDIDATE_DTYPE)
+        local["x"], local["y"], local["snapshot"], local["score"] = sel.x, sel.y + r0, sel.snapshot, sel.score
+        # (one unit-free list: the frequency branch sorts by tile row, tile col; shards are in row order already)
+        merged = np.concatenate(shard.gather_candidates(local))
+        ref = oracle.run(full, tile=tile, tau=tau, branch=1)
+        assert abs(mean_eta - ref.mu[0]) <= 1e-10 * abs(ref.mu[0]) and abs(sd_eta - ref.sigma[0]) <= 1e-8 * ref.sigma[0]
+        ty0 = r0 // tile
+        np.testing.assert_allclose(eta, ref.eta[ty0:ty0 + res.Ty], rtol=1e-9, atol=1e-12 * float(ref.eta.max()))
+        assert len(merged) == ref.cands.n_found > 0
+        assert np.array_equal(merged["x"], ref.cands.x) and np.array_equal(merged["y"], ref.cands.y)
+        assert np.array_equal(merged["snapshot"], ref.cands.snapshot)
+        np.testing.assert_allclose(merged["score"], ref.cands.score, rtol=1e-5)
+        ret[rank] = len(merged)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,H,W,tile", [(2, 256, 256, 16), (3, 200, 96, 8)])
+def test_row_sharded_frequency_branch_over_gloo(world, H, W, tile):
+    mgr = mp.Manager()
+    ret = mgr.dict()
+    mp.spawn(_worker_frequency, args=(world, _free_port(), H, W, 12, tile, 2.0, ret), nprocs=world, join=True)
     assert len(ret) == world and len(set(ret.values())) == 1
 
 
