@@ -65,6 +65,7 @@ def parse_args():
 
 
 TILE = 32  # N_T of this run (--tile)
+REC_BYTES = 16  # bytes of the per-tile, per-unit record the tLISI kernel writes (8 for tiles of one pixel)
 HARMONICS = 1  # --harmonics
 
 
@@ -315,7 +316,7 @@ def run_fitrig(args, cfg, tau, branch):
         main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
         ctx.profile(False)
         my_pix = L * (sc.r1 - sc.r0) * W
-        alg_bytes = 4 * my_pix + 16 * U * Ty * Tx
+        alg_bytes = 4 * my_pix + REC_BYTES * U * Ty * Tx
         ms_sync = ms_max
         e2e = None
         cpu = None
@@ -366,7 +367,7 @@ def run_fitrig(args, cfg, tau, branch):
         timed(torch, stream, lambda: [step_sync() for _ in range(args.steps)], barrier)
         main_tot, main_n, fin_tot, fin_n = ctx.last_timing()
         ctx.profile(False)
-        alg_bytes = 4 * my_pix + 16 * U * Ty * Tx  # one launch = one stack: every pixel once + one record per tile and unit
+        alg_bytes = 4 * my_pix + REC_BYTES * U * Ty * Tx  # one launch = one stack: every pixel once + one record per tile and unit
 
     value = pix * args.steps / (ms_max * 1e-3) / 1e6
 
@@ -510,9 +511,10 @@ def relaunch_under_torchrun(args):
 
 
 def main():
-    global TILE, HARMONICS
+    global TILE, HARMONICS, REC_BYTES
     args = parse_args()
     TILE, HARMONICS = args.tile, args.harmonics
+    REC_BYTES = 8 if TILE == 1 else 16
     import synth
     cfg = synth.CONFIGS[args.workload]
     if args.width:

@@ -100,6 +100,8 @@ struct fitrig_ctx {
   int Cy, Cx;           // cell grid
   int Ty32, Tx32;       // 32-pixel block grid of the fused kernel
   bool blocks_pending;  // the last tLISI launches wrote raw_blocks
+  int cell_pix8;        // cells of one pixel: the tLISI kernels write 8-byte records (RawPix) ...
+  int map_pix8;         // ... which are the map records themselves when a tile is one pixel
   float *q, *tlisi, *M_dev;
   unsigned* gmax_key;  // two sets of B order-preserving keys of the running global maxima, used by alternate calls:
   int key_idx;         // the finalise kernel of one call zeroes the keys of the next, so no memset sits in the stream
@@ -316,6 +318,8 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
   CTX_TRY(cudaMalloc(&c->raw, sizeof(RawTile) * c->nmap));
   c->Ty32 = (H + kFastTile - 1) / kFastTile; c->Tx32 = (W + kFastTile - 1) / kFastTile;
   c->geo = cell_geom(np.tile, np.stride);
+  c->cell_pix8 = c->geo.cell == 1;
+  c->map_pix8 = c->cell_pix8 && c->geo.m == 1;
   c->Cy = (H + c->geo.cell - 1) / c->geo.cell; c->Cx = (W + c->geo.cell - 1) / c->geo.cell;
   if (c->geo.m > 1) CTX_TRY(cudaMalloc(&c->raw_blocks, sizeof(RawTile) * (size_t)R * c->Cy * c->Cx));
   CTX_TRY(cudaMalloc(&c->q, sizeof(float) * c->nmap));
@@ -526,6 +530,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     q.z0 = opt.z0; q.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; q.tma = tma ? 1 : 0; q.C = c->prm.C;
     q.ncons = mp.ncons; q.nprod = mp.nprod;
     q.dep = (c->tune.no_pdl || c->profile) ? 0 : opt.dep;
+    q.pix8 = c->cell_pix8;
     const dim3 grid(mp.grid), block(32 * (q.ncons + q.nprod));
     auto launch = [&](auto kernel) { launch_tlisi_kernel(kernel, grid, block, (size_t)mp.smem_bytes, st, *tmp, q); };
 #define MARCH_LAUNCH(R) (tma ? launch(tlisi_march_kernel<R, false>) : launch(tlisi_march_kernel<R, true>))
@@ -560,6 +565,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     gp.G = G;
     gp.z0 = opt.z0; gp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; gp.acc = c->prm.accumulate;
     gp.C = c->prm.C;
+    gp.pix8 = c->cell_pix8;
     const long long groups = (long long)rows_tiles * out_Tx * units;
     const long long threads = groups * G;
     const long long blocks = (threads + 255) / 256;
@@ -584,6 +590,7 @@ static void fill_finalize_params(fitrig_ctx* c, FinalizeParams* fp, float* d_tli
   fp->nblk = c->fin_nblk; fp->chunk = c->fin_chunk; fp->parts = c->parts; fp->counters = c->counters; fp->mu = c->mu; fp->sigma = c->sigma;
   fp->shard_all = nullptr; fp->shard_world = 0;
   fp->user_row = c->fin_user_row;
+  fp->pix8 = c->map_pix8;
 }
 
 // keys: one global-maximum key per stack (default: the keys of the current call)
@@ -593,6 +600,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
     MergeParams mp;
     mp.cells = c->raw_blocks; mp.raw = c->raw; mp.U = c->U * c->B; mp.Ty = c->Ty; mp.Tx = c->Tx;
     mp.Cy = c->Cy; mp.Cx = c->Cx; mp.m = c->geo.m; mp.step = c->geo.step; mp.cell = c->geo.cell; mp.tile = c->prm.tile;
+    mp.pix8 = c->cell_pix8;
     const long long n = c->nmap * (mp.m * mp.m >= 32 ? 32 : 1);  // threads wanted (a warp per window of many cells)
     merge_cells_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 16 * c->num_sms), 256, 0, st>>>(mp);
     CUDA_TRY(cudaGetLastError());
@@ -609,7 +617,7 @@ static int launch_finalize(fitrig_ctx* c, float* d_tlisi_user, cudaStream_t st, 
     }
     CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used], st));
   }
-  CUDA_TRY(launch_chain(finalize_kernel, dim3(c->fin_grid), dim3(256), 0, st, chained, fp));
+  CUDA_TRY(launch_chain(c->map_pix8 ? finalize_kernel<true> : finalize_kernel<false>, dim3(c->fin_grid), dim3(256), 0, st, chained, fp));
   if (c->profile) { CUDA_TRY(cudaEventRecord(c->fin_pool[2 * c->fin_used + 1], st)); c->fin_used++; }
   c->launches++;
   c->have_map = true;
@@ -841,6 +849,7 @@ static int detect_launch_core(fitrig_ctx* c, float tau, int64_t capacity, void* 
   cp.Tx = c->Tx; cp.Ty = c->Ty; cp.H = c->H; cp.W = c->W; cp.tile = c->prm.tile; cp.stride = c->prm.stride; cp.branch = c->prm.branch;
   cp.row_offset = c->prm.row_offset;
   cp.unit_offset = unit_offset;
+  cp.pix8 = c->map_pix8;
   cp.out = reinterpret_cast<fitrig_candidate*>(d.cand_dev);
   cp.cap = std::min<long long>(d.cand_cap, std::max<long long>(capacity, 0));
   cp.host_total = reinterpret_cast<unsigned long long*>(d.cand_host_dev);
@@ -1075,6 +1084,7 @@ extern "C" int fitrig_shard_export(fitrig_ctx* c, double* d_out, void* cuda_stre
   ep.raw = c->raw; ep.gmax_key = c->gmax_key + c->key_idx; ep.out = d_out;
   ep.H = c->H; ep.W = c->W; ep.tile = c->prm.tile; ep.stride = c->prm.stride; ep.Ty = c->Ty; ep.Tx = c->Tx; ep.U = c->U;
   ep.nblk = c->fin_nblk; ep.chunk = c->fin_chunk; ep.parts = c->parts; ep.counters = c->counters;
+  ep.pix8 = c->map_pix8;
   CUDA_TRY(launch_chain(shard_export_kernel, dim3(c->fin_grid), dim3(256), 0, st, !c->tune.no_pdl, ep));
   c->launches++;
   return FITRIG_OK;
@@ -1090,7 +1100,7 @@ extern "C" int fitrig_shard_import(fitrig_ctx* c, const double* d_all, int32_t w
   fill_finalize_params(c, &fp, d_tlisi, c->gmax_key + c->key_idx);
   fp.gmax_key_next = nullptr;  // (the finalise of fitrig_tlisi has prepared the next call's key already)
   fp.shard_all = d_all; fp.shard_world = world;
-  CUDA_TRY(launch_chain(finalize_kernel, dim3(c->fin_grid), dim3(256), 0, st, false, fp));
+  CUDA_TRY(launch_chain(c->map_pix8 ? finalize_kernel<true> : finalize_kernel<false>, dim3(c->fin_grid), dim3(256), 0, st, false, fp));
   c->launches++;
   c->eta_valid = false;
   return FITRIG_OK;
@@ -1177,7 +1187,13 @@ extern "C" int fitrig_get_raw(const fitrig_ctx* c, float* sumD, float* maxD, flo
   CUDA_TRY(cudaSetDevice(c->prm.device));
   CUDA_TRY(cudaDeviceSynchronize());
   std::vector<RawTile> r(c->nmap);
-  CUDA_TRY(cudaMemcpy(r.data(), c->raw, sizeof(RawTile) * c->nmap, cudaMemcpyDeviceToHost));
+  if (c->map_pix8) {  // tiles of one pixel: 8-byte records {Delta, r}
+    std::vector<RawPix> px(c->nmap);
+    CUDA_TRY(cudaMemcpy(px.data(), c->raw, sizeof(RawPix) * c->nmap, cudaMemcpyDeviceToHost));
+    for (long long i = 0; i < c->nmap; ++i) { r[i].sumD = px[i].delta; r[i].maxD = px[i].delta; r[i].sumR = px[i].r; r[i].pos = 0; }
+  } else {
+    CUDA_TRY(cudaMemcpy(r.data(), c->raw, sizeof(RawTile) * c->nmap, cudaMemcpyDeviceToHost));
+  }
   const int tile = c->prm.tile, stride = c->prm.stride;
   for (long long i = 0; i < c->nmap; ++i) {
     const long long t = i % c->nt;

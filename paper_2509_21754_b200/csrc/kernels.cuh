@@ -33,6 +33,30 @@ struct __align__(16) RawTile {
   int32_t pos;
 };
 
+// Cells of ONE pixel ("per-pixel detection"; overlapping windows at stride 1): sum Delta = max Delta =
+// Delta and the position is 0, so the record shrinks to {Delta, r}: 8 bytes instead of 16 (the per-pixel map of a
+// 64 x 2048 x 2048 stack is 260 M records: 2 GB less to write and 2 GB less to read back).  Such a context keeps its
+// cell records in this form in the same buffer (`pix8` in the kernel parameters).
+struct __align__(8) RawPix {
+  float delta;
+  float r;
+};
+__device__ __forceinline__ RawTile load_raw(const RawTile* raw, long long i, int pix8) {
+  if (!pix8) return raw[i];
+  const RawPix v = reinterpret_cast<const RawPix*>(raw)[i];
+  RawTile o; o.sumD = v.delta; o.maxD = v.delta; o.sumR = v.r; o.pos = 0;
+  return o;
+}
+__device__ __forceinline__ void store_raw(RawTile* raw, long long i, int pix8, float S, float Mx, float R, int pos) {
+  if (pix8) {
+    RawPix v; v.delta = Mx; v.r = R;
+    reinterpret_cast<RawPix*>(raw)[i] = v;
+  } else {
+    RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
+    raw[i] = o;
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // small device helpers
 // ---------------------------------------------------------------------------------------------
@@ -606,18 +630,19 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
         }
       }
     } else {  // T == 1: per-pixel detection; float4 j holds row rq + 4 j, columns 4 cg ..
+      // cells of one pixel are kept as 8-byte records {Delta, r} (RawPix; rp - p.raw is a record index); the four
+      // records of a quad are 32 contiguous, 16-byte aligned bytes (W % 4 == 0 on this path): two 16-byte stores
+      RawPix* const pix = reinterpret_cast<RawPix*>(p.raw) + (rp - p.raw) + 4 * cg;  // (rp is the record of tile (ty0, tx0))
+      const bool col_ok = tx0 + 4 * cg < p.Tx;
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int row = rq + 4 * j;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int tx_r = 4 * cg + e;
-          float delta, r;
-          pixel(4 * j + e, delta, r);
-          if (ty0 + row < p.ty_end && tx0 + tx_r < p.Tx) {
-            RawTile o; o.sumD = delta; o.maxD = delta; o.sumR = r; o.pos = 0;
-            rp[(long long)row * p.Tx + tx_r] = o;
-          }
+        float d0, d1, d2, d3, r0, r1, r2, r3;
+        pixel(4 * j, d0, r0); pixel(4 * j + 1, d1, r1); pixel(4 * j + 2, d2, r2); pixel(4 * j + 3, d3, r3);
+        if (col_ok && ty0 + row < p.ty_end) {
+          float4* dst = reinterpret_cast<float4*>(pix + (long long)row * p.Tx);
+          dst[0] = make_float4(d0, r0, d1, r1);
+          dst[1] = make_float4(d2, r2, d3, r3);
         }
       }
     }
@@ -693,6 +718,7 @@ struct MergeParams {
   const RawTile* cells;  // [U][Cy][Cx]
   RawTile* raw;          // [U][Ty][Tx]
   int U, Ty, Tx, Cy, Cx, m, step, cell, tile;
+  int pix8;              // the cells are 8-byte records (cells of one pixel)
 };
 
 __global__ void __launch_bounds__(256) merge_cells_kernel(const MergeParams p) {
@@ -714,7 +740,7 @@ __global__ void __launch_bounds__(256) merge_cells_kernel(const MergeParams p) {
       const int by = k / p.m, bx = k - by * p.m;
       const int cy = ty * p.step + by, cx = tx * p.step + bx;
       if (cy >= p.Cy || cx >= p.Cx) continue;
-      const RawTile b = p.cells[((size_t)u * p.Cy + cy) * p.Cx + cx];
+      const RawTile b = load_raw(p.cells, ((long long)u * p.Cy + cy) * p.Cx + cx, p.pix8);
       o.sumD += b.sumD;
       o.sumR += b.sumR;
       const int pos = (by * p.cell + b.pos / p.cell) * p.tile + bx * p.cell + b.pos % p.cell;
@@ -748,6 +774,7 @@ struct GenericParams {
   int G;                    // lanes per tile
   int z0, zmask;            // real-time mode ring (see FusedParams)
   int acc;                  // snapshot accumulation (see FusedParams)
+  int pix8;                 // cells of one pixel: 8-byte records (RawPix)
   float C;
 };
 
@@ -794,9 +821,7 @@ __global__ void __launch_bounds__(256) tlisi_generic_kernel(const GenericParams 
     if (om > Mx || (om == Mx && op < pos)) { Mx = om; pos = op; }
   }
   if (live && gl == 0) {
-    RawTile o;
-    o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = pos;
-    p.raw[((size_t)u * p.Ty + (p.ty_base + ty_local)) * p.Tx + tx] = o;
+    store_raw(p.raw, ((long long)u * p.Ty + (p.ty_base + ty_local)) * p.Tx + tx, p.pix8, S, Mx, R, pos);
   }
 }
 
@@ -832,6 +857,7 @@ struct MarchParams {
   int tma;               // 1: TMA boxes, 0: cp.async copies
   int ncons, nprod;      // consumer and producer warps of this launch
   int dep;               // programmatic dependent launch: as FusedParams::dep
+  int pix8;              // cells of one pixel: 8-byte records (RawPix)
   float C;
 };
 
@@ -1036,7 +1062,7 @@ __global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
                        (SHIFT ? box_shift(ring_slot(p.z0, p.zmask, u0 + i + 1), org0) : 0);
       const float* Cc = reinterpret_cast<const float*>(smem + (size_t)sc * slot_bytes) +
                         (SHIFT ? box_shift(ring_slot(p.z0, p.zmask, u0 + i + 2), org0) : 0);
-      RawTile* const rawu = p.raw + (long long)(u0 + i) * raw_step;
+      const long long rawu = (long long)(u0 + i) * raw_step;  // first record of the unit
       // The global maximum takes x_{s+2} of every unit and x_s, x_{s+1} of the first unit of a segment: every snapshot of
       // the segment once.  The item loop is compiled twice so that the steady state pays one FMNMX per pixel.
       auto unit_items = [&](auto first_tag) {
@@ -1072,8 +1098,7 @@ __global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
           }
           const int tx = gx * p.ntx + tcol;
           if (lane_ok && ty < p.ty_end && tx < p.Tx) {
-            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
-            rawu[(long long)ty * p.Tx + tx] = o;
+            store_raw(p.raw, rawu + (long long)ty * p.Tx + tx, p.pix8, S, Mx, R, mpos);
           }
         } else if (small) {
           const int tcol = gi * gt + jt;                    // tile column inside the box
@@ -1107,8 +1132,7 @@ __global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
           }
           const int tx = gx * p.ntx + tcol;
           if (lane_ok && cc0 == 0 && ty < p.ty_end && tx < p.Tx) {
-            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
-            rawu[(long long)ty * p.Tx + tx] = o;
+            store_raw(p.raw, rawu + (long long)ty * p.Tx + tx, p.pix8, S, Mx, R, mpos);
           }
         } else {
           const int tcol = gi;
@@ -1143,8 +1167,7 @@ __global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
           }
           const int tx = gx * p.ntx + tcol;
           if (lane == 0 && ty < p.ty_end && tx < p.Tx) {
-            RawTile o; o.sumD = S; o.maxD = Mx; o.sumR = R; o.pos = mpos;
-            rawu[(long long)ty * p.Tx + tx] = o;
+            store_raw(p.raw, rawu + (long long)ty * p.Tx + tx, p.pix8, S, Mx, R, mpos);
           }
         }
       }
@@ -1281,6 +1304,7 @@ struct FinalizeParams {
   const double* shard_all;  // [shard_world][2 + 2U] or NULL
   int shard_world;
   int user_row;        // -1: tlisi_user is the whole map; r >= 0: tlisi_user is [Ty][Tx] and receives map row r only
+  int pix8;            // the map records are 8-byte RawPix (tiles of one pixel)
 };
 
 // Eq. 2 / Eq. 6 without the 1 / M^2 factor: p = (sum D / n_t) * max D * (sum r / n_t); n_t = the window's own pixel
@@ -1295,6 +1319,19 @@ __device__ __forceinline__ double tile_product(const RawTile r, int t, int Tx, i
   return ((double)r.sumD * inv_n) * (double)r.maxD * ((double)r.sumR * inv_n);
 }
 
+template <bool PIX8> struct FinRec;  // the record type of the map the finalise reads
+template <> struct FinRec<false> {
+  typedef RawTile type;
+  __device__ static __forceinline__ RawTile widen(const RawTile& r) { return r; }
+};
+template <> struct FinRec<true> {
+  typedef RawPix type;
+  __device__ static __forceinline__ RawTile widen(const RawPix& v) {
+    RawTile o; o.sumD = v.delta; o.maxD = v.delta; o.sumR = v.r; o.pos = 0;
+    return o;
+  }
+};
+
 // Chan's merge of per-shard (n, mean, M2) triples in shard order
 __device__ __forceinline__ void chan_merge(double& n, double& mean, double& m2, double nb, double mb, double m2b) {
   if (nb <= 0.0) return;
@@ -1304,7 +1341,9 @@ __device__ __forceinline__ void chan_merge(double& n, double& mean, double& m2, 
   n = tot;
 }
 
-__global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
+template <bool PIX8>
+__global__ void __launch_bounds__(256, 4) finalize_kernel(const FinalizeParams p) {
+  constexpr int kLoads = PIX8 ? 2 * kFinLoads : kFinLoads;  // (8-byte records: twice as many for the same bytes in flight)
   __shared__ double sh[64];
   __shared__ int sh_flag;
   pdl_wait();               // the tLISI kernel's records and its global maximum
@@ -1333,25 +1372,25 @@ __global__ void __launch_bounds__(256) finalize_kernel(const FinalizeParams p) {
     const double inv_m2 = 1.0 / ((double)M * (double)M);
     const size_t base = (size_t)row * nt;
     // the row's shift: its first q value
-    const double K = (double)(float)(tile_product(p.raw[base], 0, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2);
+    const double K = (double)(float)(tile_product(load_raw(p.raw, base, p.pix8), 0, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2);
     const int begin = blk * p.chunk, end = min(nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
     // kFinLoads records per thread are fetched before the first is used (the stores below may alias the loads as far as
     // the compiler knows, so it would not hoist them itself): a big map is a stream, and one record in flight per thread
     // leaves it latency bound
-    for (int t0 = begin + threadIdx.x; t0 < end; t0 += kFinLoads * blockDim.x) {
-      RawTile rec[kFinLoads];
+    for (int t0 = begin + threadIdx.x; t0 < end; t0 += kLoads * blockDim.x) {
+      typename FinRec<PIX8>::type rec[kLoads];
 #pragma unroll
-      for (int k = 0; k < kFinLoads; ++k) {
+      for (int k = 0; k < kLoads; ++k) {
         const int t = t0 + k * blockDim.x;
-        if (t < end) rec[k] = p.raw[base + t];
+        if (t < end) rec[k] = reinterpret_cast<const typename FinRec<PIX8>::type*>(p.raw)[base + t];
       }
 #pragma unroll
-      for (int k = 0; k < kFinLoads; ++k) {
+      for (int k = 0; k < kLoads; ++k) {
         const int t = t0 + k * blockDim.x;
         if (t >= end) break;
         // Eq. 2 / Eq. 6: q = (sum D / n_t) * max D * (sum r / n_t) / M^2, combined in fp64 and rounded once
-        const double qd = tile_product(rec[k], t, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2;
+        const double qd = tile_product(FinRec<PIX8>::widen(rec[k]), t, p.Tx, Hq, p.W, p.tile, p.stride, inv_full) * inv_m2;
         const float qf = (float)qd;
         p.q[base + t] = qf;
         const float tl = (float)(1.0 - qd);
@@ -1401,6 +1440,7 @@ struct ShardExportParams {
   int nblk, chunk;      // chunks per unit, entries per chunk
   StatPartial* parts;   // [U][nblk]
   unsigned* counters;   // [U]
+  int pix8;             // the map records are 8-byte RawPix (tiles of one pixel)
 };
 
 __global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportParams p) {
@@ -1413,11 +1453,11 @@ __global__ void __launch_bounds__(256) shard_export_kernel(const ShardExportPara
   for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
     const int u = (int)(chunk / p.nblk), blk = (int)(chunk - (long long)u * p.nblk);
     const size_t base = (size_t)u * nt;
-    const double K = tile_product(p.raw[base], 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full);
+    const double K = tile_product(load_raw(p.raw, base, p.pix8), 0, p.Tx, p.H, p.W, p.tile, p.stride, inv_full);
     const int begin = blk * p.chunk, end = min(nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
     for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
-      const double d = tile_product(p.raw[base + t], t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) - K;
+      const double d = tile_product(load_raw(p.raw, base + t, p.pix8), t, p.Tx, p.H, p.W, p.tile, p.stride, inv_full) - K;
       s += d;
       s2 += d * d;
     }
@@ -1635,6 +1675,7 @@ struct CompactParams {
   unsigned ticket_base;
   unsigned epoch;                    // launch number, never 0
   long long seg;        // entries per block (multiple of 32 * warps)
+  int pix8;             // tiles of one pixel: no position to look up
 };
 
 constexpr int kCompactLoads = 8;  // map entries a lane has in flight
@@ -1652,7 +1693,7 @@ __device__ __forceinline__ fitrig_candidate make_candidate(const CompactParams& 
   const int ty = (int)(t / (unsigned)p.Tx), tx = (int)(t - (unsigned)ty * (unsigned)p.Tx);
   fitrig_candidate cd;
   if (p.branch == FITRIG_BRANCH_IMAGE) {
-    const int pos = p.raw[row_begin + t].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
+    const int pos = p.pix8 ? 0 : p.raw[row_begin + t].pos;  // tile-relative row * N_T + col of the first max-Delta pixel (R20)
     cd.x = tx * p.stride + pos % p.tile;
     cd.y = p.row_offset + ty * p.stride + pos / p.tile;
     cd.snapshot = (row - bidx * p.rows_per_batch) + p.unit_offset;
