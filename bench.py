@@ -61,11 +61,13 @@ def parse_args():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = an independent stack per rank; strong = ONE stack cut into row shards (ShardedContext)")
     ap.add_argument("--no-pipeline", action="store_true", help="end every step with a synchronous fitrig_detect")
+    ap.add_argument("--accumulate", type=int, default=1, help="snapshot accumulation g (PAPER.md:497): units = L / g - 2")
     return ap.parse_args()
 
 
 TILE = 32  # N_T of this run (--tile)
 REC_BYTES = 16  # bytes of the per-tile, per-unit record the tLISI kernel writes (8 for tiles of one pixel)
+ACCUMULATE = 1  # --accumulate
 HARMONICS = 1  # --harmonics
 
 
@@ -74,7 +76,8 @@ def workload_desc(cfg, tau, branch, n_ch=1):
             + (f"(BASELINE.json configs[{cfg.cfg_index - 1}]), " if cfg.cfg_index <= 5 else
                "(shape of the paper's real-data run, PAPER.md:371-395; not a BASELINE.json config), ")
             +
-            f"N_T={TILE}, tau={tau:g}, branch={'image-frequency' if branch else 'image'}")
+            f"N_T={TILE}, tau={tau:g}, branch={'image-frequency' if branch else 'image'}"
+            + (f", accumulate={ACCUMULATE}" if ACCUMULATE > 1 else ""))
 
 
 # ---------------------------------------------------------------------------------------------
@@ -150,7 +153,7 @@ def oracle_sample_rate(snaps, rows, tau, branch, repeats=1):
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        oracle.run(sub, tile=TILE, tau=tau, branch=branch, harmonics=HARMONICS)
+        oracle.run(sub, tile=TILE, tau=tau, branch=branch, harmonics=HARMONICS, accumulate_g=ACCUMULATE)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return best
@@ -329,7 +332,7 @@ def run_fitrig(args, cfg, tau, branch):
         L, H, W = stacks[0].shape
         pix = L * H * W * n_ch * world
         my_pix = L * H * W
-        ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS, batch=n_ch)
+        ctx = fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS, batch=n_ch, accumulate=ACCUMULATE)
         U, Ty, Tx = ctx.map_dims()
         d_tl = torch.empty((n_ch, U, Ty, Tx), dtype=torch.float32, device=dev)
 
@@ -396,7 +399,7 @@ def run_fitrig(args, cfg, tau, branch):
         e2e = None
     if not strong and not args.no_e2e:
         h2d_gbs = measure_h2d_gbs(torch) if rank == 0 else None
-        ectx = ctx if n_ch == 1 else fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS)
+        ectx = ctx if n_ch == 1 else fitrig.Context(H, W, L, device=local, branch=branch, tile=TILE, harmonics=HARMONICS, accumulate=ACCUMULATE)
         hosts = []
         for st_c in stacks:
             host = torch.empty((L, H, W), dtype=torch.float32).pin_memory()
@@ -428,30 +431,50 @@ def run_fitrig(args, cfg, tau, branch):
                             "unit": "GB/s", "frac": (4 * pix / world / (e_ms * 1e-3) / 1e9 / h2d_gbs) if h2d_gbs else None,
                             "peak_source": "pinned 1 GiB cudaMemcpyAsync H2D, best of 10, this run"}}
         # ---- real-time leg: fitrig_push, one snapshot per call from pinned host memory (Fig. 14 timeline) ----
-        window = 3 if branch == 0 else min(L, 18)
-        pctx = fitrig.Context(H, W, window, device=local, tile=TILE, branch=branch, harmonics=HARMONICS)
-        snaps0 = hosts[0]
+        # ---- the copy / kernel timeline of one more streamed pass (library CUDA events, fitrig_stream_timeline) ----
+        ectx.profile(True)
+        ectx.stream(hosts[0], h_tl, stream)
+        torch.cuda.synchronize()
+        tl = ectx.stream_timeline()
+        ectx.profile(False)
+        if len(tl):
+            copy_ms = float((tl[:, 1] - tl[:, 0]).sum())
+            kern_ms = float((tl[:, 3] - tl[:, 2]).sum())
+            # time a kernel spends while the copy stream is busy with a LATER strip's copy
+            hidden = 0.0
+            for i in range(len(tl)):
+                for j in range(i + 1, len(tl)):
+                    hidden += max(0.0, min(tl[i, 3], tl[j, 1]) - max(tl[i, 2], tl[j, 0]))
+            e2e["timeline"] = {"strips": int(len(tl)), "span_ms": float(tl[:, 3].max() - tl[:, 0].min()), "copy_ms_sum": copy_ms,
+                               "kernel_ms_sum": kern_ms, "kernel_ms_hidden_under_later_copies": hidden,
+                               "first_strips_ms": [[round(float(v), 4) for v in row] for row in tl[:4]],
+                               "columns": "copy start, copy end, kernel start, kernel end (ms from the first copy's start)",
+                               "source": "fitrig_stream_timeline: CUDA events of one streamed pass of stack 0 under fitrig_profile(1), outside the timed region"}
+        if ACCUMULATE == 1:  # (fitrig_push does not accumulate)
+            window = 3 if branch == 0 else min(L, 18)
+            pctx = fitrig.Context(H, W, window, device=local, tile=TILE, branch=branch, harmonics=HARMONICS)
+            snaps0 = hosts[0]
 
-        def push_pass():
-            tot = 0
-            for s_ in snaps0 + [None]:
-                u_, c_, n_ = pctx.push(s_, tau, None, cap, stream, out=outs[0])
-                tot += n_
-            pctx.push_reset()
-            return tot
+            def push_pass():
+                tot = 0
+                for s_ in snaps0 + [None]:
+                    u_, c_, n_ = pctx.push(s_, tau, None, cap, stream, out=outs[0])
+                    tot += n_
+                pctx.push_reset()
+                return tot
 
-        push_pass()
-        barrier()
-        t_wall = time.perf_counter()
-        n_rt = push_pass()
-        barrier()
-        p_ms = shard.max_over_ranks((time.perf_counter() - t_wall) * 1e3, dev)
-        e2e["realtime"] = {"value": world * L * H * W / (p_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_snapshot": p_ms / L,
-                           "api": "fitrig_push (one pinned host snapshot per call, running M, candidates per unit"
-                                  + (f"; frequency branch: Eq. 10-12 over the cube of the last {window - 2} units" if branch else "") + ")",
-                           "candidates": int(n_rt), "h2d_gbs": 4 * L * H * W / (p_ms * 1e-3) / 1e9,
-                           "timer": "host wall clock around the pass (every push synchronises)"}
-        pctx.close()
+            push_pass()
+            barrier()
+            t_wall = time.perf_counter()
+            n_rt = push_pass()
+            barrier()
+            p_ms = shard.max_over_ranks((time.perf_counter() - t_wall) * 1e3, dev)
+            e2e["realtime"] = {"value": world * L * H * W / (p_ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_snapshot": p_ms / L,
+                               "api": "fitrig_push (one pinned host snapshot per call, running M, candidates per unit"
+                                      + (f"; frequency branch: Eq. 10-12 over the cube of the last {window - 2} units" if branch else "") + ")",
+                               "candidates": int(n_rt), "h2d_gbs": 4 * L * H * W / (p_ms * 1e-3) / 1e9,
+                               "timer": "host wall clock around the pass (every push synchronises)"}
+            pctx.close()
         if ectx is not ctx:
             ectx.close()
         del hosts
@@ -511,9 +534,9 @@ def relaunch_under_torchrun(args):
 
 
 def main():
-    global TILE, HARMONICS, REC_BYTES
+    global TILE, HARMONICS, REC_BYTES, ACCUMULATE
     args = parse_args()
-    TILE, HARMONICS = args.tile, args.harmonics
+    TILE, HARMONICS, ACCUMULATE = args.tile, args.harmonics, args.accumulate
     REC_BYTES = 8 if TILE == 1 else 16
     import synth
     cfg = synth.CONFIGS[args.workload]
