@@ -444,7 +444,7 @@ def run_fitrig(args, cfg, tau, branch):
             hidden = 0.0
             for i in range(len(tl)):
                 for j in range(i + 1, len(tl)):
-                    hidden += max(0.0, min(tl[i, 3], tl[j, 1]) - max(tl[i, 2], tl[j, 0]))
+                    hidden += max(0.0, float(min(tl[i, 3], tl[j, 1]) - max(tl[i, 2], tl[j, 0])))
             e2e["timeline"] = {"strips": int(len(tl)), "span_ms": float(tl[:, 3].max() - tl[:, 0].min()), "copy_ms_sum": copy_ms,
                                "kernel_ms_sum": kern_ms, "kernel_ms_hidden_under_later_copies": hidden,
                                "first_strips_ms": [[round(float(v), 4) for v in row] for row in tl[:4]],

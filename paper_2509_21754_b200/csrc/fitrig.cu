@@ -354,7 +354,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
     CTX_TRY(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * c->U, cudaMemcpyHostToDevice));
     if (sizeof(double2) * c->U > 48 * 1024)
       CTX_TRY(cudaFuncSetAttribute(dft_mag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double2) * c->U)));
-    c->spec_nblk = c->fin_nblk;
+    c->spec_nblk = (int)((c->nt + kSpecChunk - 1) / kSpecChunk);
     CTX_TRY(cudaMalloc(&c->sparts, sizeof(StatPartial) * c->spec_nblk * c->B));
     CTX_TRY(cudaMalloc(&c->scounter, sizeof(unsigned) * c->B));
     CTX_TRY(cudaMemset(c->scounter, 0, sizeof(unsigned) * c->B));
@@ -803,7 +803,7 @@ static int launch_spectrum(fitrig_ctx* c, cudaStream_t st, double* shard_out) {
   SpectrumParams sp;
   sp.q = c->q; sp.tw = c->tw; sp.eta = c->eta; sp.kstar = c->kstar; sp.nt = (int)c->nt; sp.U = c->U; sp.B = c->B;
   sp.mag = c->mag; sp.harmonics = c->prm.harmonics;
-  sp.nblk = c->spec_nblk; sp.chunk = c->fin_chunk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
+  sp.nblk = c->spec_nblk; sp.chunk = kSpecChunk; sp.parts = c->sparts; sp.counters = c->scounter; sp.mu = c->smu; sp.sigma = c->ssigma;
   sp.shard_out = shard_out;
   if (c->U / 2 >= 1) {
     const dim3 grid((unsigned)((c->nt * c->B + 127) / 128), (unsigned)((c->U / 2 + kDftBins - 1) / kDftBins));
@@ -811,7 +811,7 @@ static int launch_spectrum(fitrig_ctx* c, cudaStream_t st, double* shard_out) {
     c->launches++;
   }
   const int grid = (int)std::min<long long>((long long)c->spec_nblk * c->B, 8ll * c->num_sms);
-  CUDA_TRY(launch_chain(spectrum_kernel, dim3(grid), dim3(256), 0, st, chained, sp));
+  CUDA_TRY(launch_chain(spectrum_kernel, dim3(grid), dim3(kSpecChunk), 0, st, chained, sp));
   c->launches++;
   c->eta_valid = true;
   return FITRIG_OK;

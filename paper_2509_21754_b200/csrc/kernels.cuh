@@ -1516,7 +1516,8 @@ struct SpectrumParams {
 // kDftBins bins), tiles fastest so that the loads of q coalesce and the twiddle index is warp uniform (shared-memory
 // broadcast).  Direct DFT: the series is short (U = 30 in config 5, 1498 in the paper's real-data run) and of arbitrary
 // length (R17).
-constexpr int kDftBins = 4;
+constexpr int kDftBins = 8;    // bins per thread: every load of q serves this many complex multiply-adds
+constexpr int kDftUnroll = 4;  // samples fetched before they are used (the loop is a stream of L2 loads otherwise)
 
 __global__ void __launch_bounds__(128) dft_mag_kernel(const SpectrumParams p) {
   extern __shared__ double2 tws[];  // U twiddles
@@ -1529,15 +1530,15 @@ __global__ void __launch_bounds__(128) dft_mag_kernel(const SpectrumParams p) {
   const int b = (int)(g / p.nt), t = (int)(g - (long long)b * p.nt);
   const float* q = p.q + (size_t)b * p.U * p.nt + t;
   const int K = p.U / 2, k0 = blockIdx.y * kDftBins + 1;
-  double mean = 0.0;
-  for (int u = 0; u < p.U; ++u) mean += (double)q[(size_t)u * p.nt];
-  mean /= (double)p.U;  // DC removed
+  // DC removed: a_u = q_u - c.  Any constant c leaves every bin k = 1 .. U-1 unchanged (sum_u e^{-2 pi i k u / U}
+  // = 0); the series' mean is the paper's c, its first sample serves the same purpose here -- the q_u agree in their
+  // leading digits, so the subtraction keeps the sums well conditioned -- without a pass of its own over the series.
+  const double c0 = (double)q[0];
   double re[kDftBins], im[kDftBins];
   int j[kDftBins], kk[kDftBins];  // (k * u) mod U and its step k (0 for bins beyond K: they stay at twiddle 0)
 #pragma unroll
   for (int i = 0; i < kDftBins; ++i) { re[i] = 0.0; im[i] = 0.0; j[i] = 0; kk[i] = (k0 + i <= K) ? k0 + i : 0; }
-  for (int u = 0; u < p.U; ++u) {
-    const double a = (double)q[(size_t)u * p.nt] - mean;
+  auto accumulate = [&](double a) {
 #pragma unroll
     for (int i = 0; i < kDftBins; ++i) {
       const double2 w = tws[j[i]];
@@ -1546,16 +1547,28 @@ __global__ void __launch_bounds__(128) dft_mag_kernel(const SpectrumParams p) {
       j[i] += kk[i];              // k <= K < U: one subtraction wraps
       if (j[i] >= p.U) j[i] -= p.U;
     }
+  };
+  int u = 0;
+  for (; u + kDftUnroll <= p.U; u += kDftUnroll) {
+    float v[kDftUnroll];
+#pragma unroll
+    for (int d = 0; d < kDftUnroll; ++d) v[d] = q[(size_t)(u + d) * p.nt];
+#pragma unroll
+    for (int d = 0; d < kDftUnroll; ++d) accumulate((double)v[d] - c0);
   }
+  for (; u < p.U; ++u) accumulate((double)q[(size_t)u * p.nt] - c0);
 #pragma unroll
   for (int i = 0; i < kDftBins; ++i)
     if (k0 + i <= K) p.mag[((size_t)b * K + (k0 + i - 1)) * p.nt + t] = (float)sqrt(re[i] * re[i] + im[i] * im[i]);
 }
 
 // eta = h(m) per tile (maximum magnitude, or harmonic summing), k*, and the statistics of eta (Eq. 11).
-__global__ void __launch_bounds__(256) spectrum_kernel(const SpectrumParams p) {
+constexpr int kSpecChunk = 256;  // tiles per chunk of the spectrum kernel = its block size
+
+__global__ void __launch_bounds__(kSpecChunk) spectrum_kernel(const SpectrumParams p) {
   __shared__ double sh[64];
   __shared__ int sh_flag;
+  __shared__ float sh_e;
   pdl_wait();
   pdl_launch_dependents();
   const int K = p.U / 2;
@@ -1578,10 +1591,11 @@ __global__ void __launch_bounds__(256) spectrum_kernel(const SpectrumParams p) {
         for (int k = 1; k <= K; ++k) {
           double s = 0.0;
           int have = 0;  // harmonics summed so far
-          for (int h = 1; h <= p.harmonics && h * k <= K; h *= 2) {
+          double inv_sqrt_h = 1.0;  // 1 / sqrt(h) for h = 1, 2, 4, ..: times 1 / sqrt(2) per level
+          for (int h = 1; h <= p.harmonics && h * k <= K; h *= 2, inv_sqrt_h *= 0.70710678118654752440) {
             for (int i = have + 1; i <= h; ++i) s += (double)mag[(size_t)(i * k - 1) * p.nt + t];  // m_k, m_2k, ... in order
             have = h;
-            const double v = s / sqrt((double)h);
+            const double v = s * inv_sqrt_h;
             if (first || v > bestd) { bestd = v; kb = k; first = false; }
           }
         }
@@ -1590,46 +1604,54 @@ __global__ void __launch_bounds__(256) spectrum_kernel(const SpectrumParams p) {
       *kb_out = kb;
       return best;
     };
-    int kb0;
-    const double Kshift = (double)eta_of(0, &kb0);
+    // A chunk is one tile per thread (the work per tile is a loop over the spectrum).  Its statistics are shifted sums
+    // around the chunk's OWN first eta (no tile's eta is computed twice), turned into (n, mean, M2); the last block of a
+    // stack merges the chunks' triples in chunk order (Chan: exact for a constant map, R4; deterministic).
     const int begin = blk * p.chunk, end = min(p.nt, begin + p.chunk);
     double s = 0.0, s2 = 0.0;
-    for (int t = begin + threadIdx.x; t < end; t += blockDim.x) {
-      int kb;
-      const float e = eta_of(t, &kb);
-      p.eta[(size_t)b * p.nt + t] = e;
-      p.kstar[(size_t)b * p.nt + t] = kb;
-      const double d = (double)e - Kshift;
-      s += d;
-      s2 += d * d;
+    float e_first = 0.f;
+    {
+      const int t = begin + threadIdx.x;  // p.chunk <= blockDim.x
+      float e = 0.f;
+      if (t < end) {
+        int kb;
+        e = eta_of(t, &kb);
+        p.eta[(size_t)b * p.nt + t] = e;
+        p.kstar[(size_t)b * p.nt + t] = kb;
+      }
+      __syncthreads();  // (sh_e may still be read from the previous chunk)
+      if (threadIdx.x == 0) sh_e = e;
+      __syncthreads();
+      e_first = sh_e;
+      if (t < end) {
+        const double d = (double)e - (double)e_first;
+        s = d;
+        s2 = d * d;
+      }
     }
     block_sum2(s, s2, sh);
-    StatPartial part;
-    part.n = (double)(end - begin); part.s = s; part.s2 = s2;
-    if (p.shard_out) {  // one batch entry; the merged sums leave as (n, mean, M2)
-      if (threadIdx.x == 0) {
-        p.parts[(size_t)b * p.nblk + blk] = part;
-        __threadfence();
-        sh_flag = (atomicAdd(&p.counters[b], 1u) == (unsigned)p.nblk - 1);
-      }
-      __syncthreads();
-      if (sh_flag && threadIdx.x < 32) {
-        __threadfence();
-        double n, a, c;
-        warp_merge_partials(p.parts + (size_t)b * p.nblk, p.nblk, n, a, c);
-        if (threadIdx.x == 0) {
-          const double m = (n > 0.0) ? a / n : 0.0;
-          p.shard_out[0] = n;
-          p.shard_out[1] = Kshift + m;
-          p.shard_out[2] = fmax(c - a * m, 0.0);
-          stats_from_sums(Kshift, n, a, c, &p.mu[b], &p.sigma[b]);  // the shard's own statistics, until the import
-          p.counters[b] = 0;
-        }
-      }
-      __syncthreads();
-    } else {
-      row_stats_finish(part, Kshift, b, blk, p.nblk, p.parts, p.counters, p.mu, p.sigma, &sh_flag);
+    if (threadIdx.x == 0) {
+      const double n = (double)(end - begin), m = s / n;
+      StatPartial part;
+      part.n = n; part.s = (double)e_first + m; part.s2 = fmax(s2 - s * m, 0.0);  // (n, mean, M2)
+      p.parts[(size_t)b * p.nblk + blk] = part;
+      __threadfence();
+      sh_flag = (atomicAdd(&p.counters[b], 1u) == (unsigned)p.nblk - 1);
     }
+    __syncthreads();
+    if (sh_flag && threadIdx.x == 0) {
+      __threadfence();
+      double n = 0.0, mean = 0.0, m2 = 0.0;
+      for (int c = 0; c < p.nblk; ++c) {
+        const volatile StatPartial* sp = p.parts + (size_t)b * p.nblk + c;
+        chan_merge(n, mean, m2, sp->n, sp->s, sp->s2);
+      }
+      if (p.shard_out) { p.shard_out[0] = n; p.shard_out[1] = mean; p.shard_out[2] = m2; }  // one batch entry
+      p.mu[b] = mean;                                   // (a shard: its own statistics, until the import)
+      p.sigma[b] = (n > 0.0) ? sqrt(m2 / n) : 0.0;
+      p.counters[b] = 0;
+    }
+    __syncthreads();
   }
 }
 

@@ -1,0 +1,165 @@
+"""GPU tier, second batch of round 2: the code paths added after the first batch -- 8-byte records of one-pixel
+tiles through every entry point, tiles of 4 / 2 pixels held whole by one lane, the staged / re-walked compaction,
+the degenerate sigma == 0 rows with a negative threshold, batches whose tLISI kernels are chained by programmatic
+dependent launches.  Same rules as test_parity_gpu.py: through the C ABI, against the CPU fp64 oracle on the same
+seeded buffers, tolerances of DESIGN.md section 3.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2509_21754_b200 as fitrig
+import synth
+from tests import util
+from tests.test_parity_gpu import check_against_oracle, gpu_run, oracle_delta_at, oracle_run
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _stack(H, W, L=8, seed_cfg="tiny"):
+    cfg = synth.scaled(synth.CONFIGS[seed_cfg], H, W, L=L)
+    return synth.make_stack(cfg, device=DEV)[0]
+
+
+# ------------------------------------------------------------------------------------------
+# tiles of ONE pixel keep {Delta, r} records of 8 bytes: every reader of the map records must agree
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("H,W,use_stream", [(96, 128, False), (70, 100, False), (96, 128, True), (65, 36, True)])
+def test_pixel_tiles_whole_path(H, W, use_stream):
+    st = _stack(H, W)
+    taus = (4.0, 6.0)
+    g = gpu_run(st, taus=taus, tile=1, capacity=1 << 18, use_stream=use_stream)
+    ref = oracle_run(st, tile=1, tau=5.0)
+    check_against_oracle(st, g, ref, taus, 1, small_tiles=True)
+    sd, md, sr, ax, ay = g["raw"]
+    assert np.array_equal(sd, md)  # one pixel: sum Delta == max Delta, and the position is the pixel itself
+    U, Ty, Tx = g["dims"]
+    assert np.array_equal(ax, np.broadcast_to(np.arange(Tx), (U, Ty, Tx))) and np.array_equal(ay, np.broadcast_to(np.arange(Ty)[:, None], (U, Ty, Tx)))
+
+
+def test_pixel_tiles_unaligned_base_take_the_generic_kernel_with_the_same_records():
+    H, W = 64, 96
+    big = _stack(H, W + 4)
+    flat = torch.empty(big.shape[0] * H * W + 1, dtype=torch.float32, device=DEV)
+    view = flat[1:].view(big.shape[0], H, W)  # base pointer 4 bytes off a 16-byte boundary
+    view.copy_(big[:, :, :W])
+    a = gpu_run(view, taus=(5.0,), tile=1, capacity=1 << 18)
+    b = gpu_run(view.clone(), taus=(5.0,), tile=1, capacity=1 << 18)  # aligned copy: the fused kernel
+    np.testing.assert_allclose(a["q"], b["q"], rtol=2e-6, atol=1e-30)
+    assert a["cands"][5.0][1] == b["cands"][5.0][1]
+    ref = oracle_run(view, tile=1, tau=5.0)
+    check_against_oracle(view, a, ref, (5.0,), 1, small_tiles=True)
+
+
+def test_pixel_tiles_push_and_row_shards():
+    H, W, L, tau = 64, 96, 7, 5.0
+    st = _stack(H, W, L)
+    ref = oracle.run_realtime(st.cpu().numpy(), tile=1, tau=tau)
+    with fitrig.Context(H, W, 3, tile=1) as ctx:
+        units = {}
+        for s in list(st) + [None]:
+            u, c, n = ctx.push(s, tau, None, 1 << 18)
+            if u >= 0:
+                units[u] = (c.copy(), n, ctx.get_map(0)[0])
+    assert sorted(units) == list(range(L - 2))
+    for n_, (c, cnt, q) in units.items():
+        eS, eM, eR = util.fp32_slack(st[n_:n_ + 3].cpu().numpy(), 1)
+        r = ref[n_]
+        slack = (eS * r.res.maxD * r.res.sumR + r.res.sumD * eM * r.res.sumR + r.res.sumD * r.res.maxD * eR)[0] / r.res.M ** 2
+        util.assert_map_close(q, r.res.q[0], slack=slack)
+    # two row shards of the same image against the whole-image context (bit-identical rows)
+    whole = gpu_run(st, taus=(tau,), tile=1, capacity=1 << 18)
+    from paper_2509_21754_b200 import shard
+    rows = shard.row_shards(H, 1, 2)
+    ctxs, vecs = [], []
+    try:
+        for (r0, r1) in rows:
+            ctx = fitrig.Context(r1 - r0, W, L, tile=1, row_offset=r0)
+            ctxs.append(ctx)
+            ctx.tlisi(st[:, r0:r1].contiguous())
+            v = torch.empty(2 + 2 * (L - 2), dtype=torch.float64, device=DEV)
+            ctx.shard_export(v)
+            vecs.append(v)
+        allv = torch.stack(vecs).contiguous()
+        for (r0, r1), ctx in zip(rows, ctxs):
+            ctx.shard_import(allv, 2)
+            assert np.array_equal(ctx.get_map(0), whole["q"][:, r0:r1])
+    finally:
+        for ctx in ctxs:
+            ctx.close()
+
+
+def test_windows_at_stride_one_are_built_from_pixel_records():
+    """tile 4, stride 1: cells of one pixel (8-byte records) merged into 4 x 4 windows (R27)."""
+    H, W = 40, 52
+    st = _stack(H, W)
+    g = gpu_run(st, taus=(4.0,), tile=4, stride=1, capacity=1 << 18)
+    ref = oracle.run(st.cpu().numpy(), tile=4, tau=4.0, stride=1)
+    util.assert_map_close(g["q"], ref.res.q, g["tlisi"], ref.res.tlisi)
+    assert g["cands"][4.0][1] == ref.cands.n_found or abs(g["cands"][4.0][1] - ref.cands.n_found) <= 2
+
+
+# ------------------------------------------------------------------------------------------
+# compaction: warps with more candidates than they can keep from the counting pass walk their range again;
+# sigma == 0 rows with a negative threshold select every tile (z == 0 > tau, R4 + R6)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tile,tau", [(4, -0.5), (2, -0.3), (8, -0.5), (32, -3.0)])
+def test_low_thresholds_many_candidates_per_warp(tile, tau):
+    H, W = 256, 256
+    st = _stack(H, W)
+    g = gpu_run(st, taus=(tau,), tile=tile, capacity=1 << 20)
+    ref = oracle_run(st, tile=tile, tau=tau)
+    U, Ty, Tx = g["dims"]
+    c, n = g["cands"][tau]
+    assert n == len(c) and n > 0
+    if tile <= 4:
+        assert n > 0.5 * U * Ty * Tx  # more than half of every warp's 128 entries: no warp can keep them all
+    lst = [(int(k["x"]), int(k["y"]), int(k["snapshot"]), float(k["score"]), (int(k["y"]) // tile) * Tx + int(k["x"]) // tile,
+            int(k["snapshot"])) for k in c]
+    util.compare_candidates(lst, ref.z, ref.mu, ref.sigma, tau, Tx, Ty * Tx)
+
+
+def test_negative_threshold_on_constant_rows_selects_every_tile():
+    L, H, W, tile = 5, 64, 96, 32
+    one = synth.gaussian_noise_stack(L, tile, tile, seed=11, device=DEV)
+    st = one.repeat(1, H // tile, W // tile).contiguous()  # identical tiles: q is constant over every unit, sigma == 0
+    with fitrig.Context(H, W, L, tile=tile) as ctx:
+        ctx.tlisi(st)
+        M, mu, sd = ctx.get_stats()
+        assert np.all(sd == 0.0)
+        c, n = ctx.detect(-1.0)
+        U, Ty, Tx = ctx.map_dims()
+        assert n == U * Ty * Tx and np.all(c["score"] == 0.0)
+        order = [(int(k["snapshot"]), int(k["y"]) // tile, int(k["x"]) // tile) for k in c]
+        assert order == sorted(order) and len(set(order)) == n
+        assert ctx.detect(0.0)[1] == 0  # strict: z == 0 is not > 0
+    ref = oracle.run(st.cpu().numpy(), tile=tile, tau=-1.0)
+    assert ref.cands.n_found == n
+
+
+# ------------------------------------------------------------------------------------------
+# tiles of 4 and 2 pixels (a lane holds whole tiles): every position of a maximum inside a tile, ties included
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("tile", [4, 2])
+def test_small_tiles_first_maximum_in_row_major_order(tile):
+    L, H, W = 3, 64, 64
+    st = torch.zeros((L, H, W), dtype=torch.float32, device=DEV)  # Delta = 0 everywhere ...
+    rng = np.random.default_rng(3)
+    want = {}
+    for ty in range(H // tile):
+        for tx in range(W // tile):
+            k = int(rng.integers(0, tile * tile))
+            y, x = ty * tile + k // tile, tx * tile + k % tile
+            st[2, y, x] = 3.0  # ... except here: D_0 = 0, D_1 = 3, Delta = 3
+            if rng.random() < 0.5 and k + 1 < tile * tile:  # a second, equal maximum later in row-major order
+                k2 = int(rng.integers(k + 1, tile * tile))
+                st[2, ty * tile + k2 // tile, tx * tile + k2 % tile] = 3.0
+            want[(ty, tx)] = (x, y)
+    with fitrig.Context(H, W, L, tile=tile) as ctx:
+        ctx.tlisi(st)
+        sd, md, sr, ax, ay = ctx.get_raw()
+    assert np.all(md == 3.0)
+    for (ty, tx), (x, y) in want.items():
+        assert (int(ax[0, ty, tx]), int(ay[0, ty, tx])) == (x, y)
