@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <numeric>
 #include <new>
 #include <vector>
 
@@ -198,6 +199,8 @@ static cudaError_t set_fused_attr_one() {
 template <int REF>
 static cudaError_t set_fused_attr() {
   cudaError_t e;
+  if ((e = cudaFuncSetAttribute(tlisi_fused_kernel<REF, false, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kMaxSmemPerCta)) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, false, 32>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, true, 32>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, false, 16>()) != cudaSuccess) return e;
@@ -380,9 +383,8 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
     CTX_TRY(cudaHostGetDevicePointer((void**)&d.counts_host_dev, d.counts_host, 0));
     CTX_TRY(cudaEventCreateWithFlags(&d.done, cudaEventDisableTiming));
   }
-  if (c->plan.path == 0) {
-    CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
-  }
+  // (also where the plan says generic: the unaligned variant and aligned strips of such a context ride the fused kernel)
+  CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
 #define MARCH_ATTR(R, S) \
   CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<R, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)))
   MARCH_ATTR(0, false); MARCH_ATTR(1, false); MARCH_ATTR(2, false);
@@ -472,9 +474,26 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   const int rows_tiles = (rows + tile - 1) / tile;
   fitrig_plan pl = c->plan;
   const bool aligned = ((uintptr_t)base % 16 == 0) && (snap_stride % 4 == 0) && (c->W % 4 == 0);  // what TMA needs
-  if (pl.path == 0 && !aligned) pl.path = 1;  // TMA needs 16-byte aligned base and strides
+  // Rows that do not start on 16-byte boundaries: cells of 32 pixels of ONE contiguous stack still ride the fused kernel,
+  // through a tensor map of "super rows" of k image rows (kernels.cuh, UNAL); everything else takes the generic kernel.
+  bool unal = false;
+  int unal_k = 1;
+  const int unal_a = (int)(((uintptr_t)base >> 2) & 3);
+  if (!aligned && tile == kFastTile && c->prm.accumulate == 1 && !c->tune.force_generic && !c->tune.no_unaligned_fused &&
+      (uintptr_t)base % 4 == 0 && snap_stride % c->W == 0 && snap_stride / c->W >= rows && r0 % kFastTile == 0) {
+    unal_k = 4 / std::gcd(c->W, 4);
+    // (dim0 = k W + a_off exceeds the row stride of k W by a_off: rows of the tensor map overlap, which the driver accepts
+    // and which reads the flat continuation -- checked on the B200)
+    unal = (nslots * (snap_stride / c->W)) % unal_k == 0 && (long long)unal_k * c->W + 4 <= 0x7fffffffll &&
+           nslots * (snap_stride / c->W) <= 0x7fffffffll;
+    if (unal) {
+      Tuning tn = c->tune;
+      plan_launch_fused(tile, c->W, rows, units, c->num_sms, tn, /*extra_row_bytes=*/16, &pl);
+    }
+  }
+  if (pl.path == 0 && !aligned && !unal) pl.path = 1;  // TMA needs 16-byte aligned base and strides
   if (pl.path == 0 && r0 % kFastTile != 0) pl.path = 1;  // strips must start on a 32-row block
-  if (pl.path == 0 && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
+  if (pl.path == 0 && !unal && (rows != c->H || units != c->U)) plan_launch(tile, c->W, rows, units, c->num_sms, c->tune, &pl);
 
   // generic path: the time-marching kernel (TMA boxes where the image allows, else cp.async copies into shifted rows)
   MarchPlan mp = MarchPlan();
@@ -488,10 +507,25 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   if (rc) return rc;
   if (pl.path == 0) {
     const CUtensorMap* tmp = nullptr;
-    rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
-    if (rc) return rc;
+    CUtensorMap tm_unal;
+    if (unal) {
+      // super rows of k image rows, from the 16-byte boundary at or below the base
+      const cuuint64_t gdim[2] = {(cuuint64_t)unal_k * c->W + unal_a, (cuuint64_t)(nslots * (snap_stride / c->W) / unal_k)};
+      const cuuint64_t gstr[1] = {(cuuint64_t)unal_k * c->W * 4};
+      const cuuint32_t bx[2] = {(cuuint32_t)(pl.box_tiles * kFastTile + 4), (cuuint32_t)(kFastTile / unal_k)};
+      const cuuint32_t estr[2] = {1, 1};
+      CUresult r = c->encode(&tm_unal, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)(base - unal_a), gdim, gstr, bx, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled (super rows) failed (CUresult %d)", (int)r);
+      tmp = &tm_unal;
+    } else {
+      rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
+      if (rc) return rc;
+    }
     const CUtensorMap& tm = *tmp;
     FusedParams fp;
+    fp.k_rows = unal_k; fp.a_off = unal_a; fp.rows = rows; fp.srows = (int)(snap_stride / c->W); fp.even_shifts = (c->W % 2 == 0) && (unal_a % 2 == 0);
     fp.raw = out_raw; fp.gmax_key = key;
     fp.z0 = opt.z0; fp.zmask = opt.zmod ? opt.zmod - 1 : 0x7fffffff; fp.acc = c->prm.accumulate;
     fp.base = base; fp.snap_stride = snap_stride; fp.W = c->W;
@@ -507,6 +541,13 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.C = c->prm.C;
     fp.dep = (c->tune.no_pdl || c->profile) ? 0 : opt.dep;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
+    if (unal) {
+      switch (c->prm.ref_mode) {
+        case FITRIG_REF_ABS: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_ABS, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
+        case FITRIG_REF_LITERAL: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_LITERAL, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
+        default: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_FLOOR, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
+      }
+    } else
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;
       case FITRIG_REF_LITERAL: launch_fused<FITRIG_REF_LITERAL>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;

@@ -104,6 +104,13 @@ __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* ma
       "l"(map), "r"(x), "r"(y), "r"(z), "r"(bar)
       : "memory");
 }
+__device__ __forceinline__ void tma_load_box2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int x, int y) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes"
+      " [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+      "l"(map), "r"(x), "r"(y), "r"(bar)
+      : "memory");
+}
 // Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may become
 // resident while its predecessor in the stream still runs; pdl_wait() blocks until the predecessor has completed and
 // its memory is visible (a no-op for a plain launch).  pdl_launch_dependents() lets the successor's CTAs be scheduled.
@@ -178,6 +185,10 @@ struct FusedParams {
   int z0, zmask;         // snapshot s of the launch lives in slot (z0 + s) & zmask: real-time ring of 4 slots: zmask = 3;
                          // a plain stack: z0 = 0, zmask = 0x7fffffff (no modulo, no branch in the lane-0 paths)
   int acc;               // snapshot accumulation: image j of the method = sum of raw snapshots g*j .. g*j+g-1
+  int k_rows, a_off, rows;  // the unaligned variant (UNAL): image rows per super row, floats between the 16-byte boundary
+                            // below the base pointer and the base, image rows per snapshot of this launch
+  int srows;                // UNAL: rows between consecutive snapshots (snap_stride / W; >= rows: the last strip is shorter)
+  int even_shifts;          // UNAL: every row starts on an 8-byte boundary (W and a_off even)
   int dep;               // programmatic dependent launch (see pdl_wait): 1 = this grid must not touch memory before the grid
                          // ahead of it in the stream has completed (wait at the start, after the prologue); 2 = the grid
                          // ahead is an independent tLISI launch of the same call (another stack of a batch): run beside
@@ -371,9 +382,20 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 // of Delta (R20) is tracked per 16-byte group in the loop; which of its 4 pixels it was is found one
 // step later from a 48-byte re-read (3 x cp.async of lines that were fetched moments ago: L2 hits)
 // by lane 0, off the critical path.
-template <int REF_MODE, bool ACC, int T>
+// UNAL (T = 32, no accumulation): images whose rows do not start on 16-byte boundaries (W % 4 != 0, or an unaligned
+// base pointer).  TMA can neither describe such rows (strides must be multiples of 16 bytes) nor start a box off a
+// 16-byte boundary, but the stack is ONE contiguous array, and k = 4 / gcd(W, 4) consecutive image rows are a multiple of 16
+// bytes: the tensor map describes "super rows" of k image rows (from the base rounded down to 16 bytes, a_off floats
+// earlier).  Image row g (counted through the whole stack) is class g % k of super row g / k and starts at element
+// (g % k) * W + a_off of it.  The 32 rows of a block are fetched as k boxes of 32 / k rows, one per class, each from the
+// 16-byte boundary at or before its rows' first pixel and 4 floats wider: the rows of a class land SHIFTED by
+// (class * W + a_off) % 4 floats.  A lane's rows (lane / 8 + 4 j) all belong to one class, so it reads its pixels with
+// one base pointer and, depending on the shift, 16-, 8- or 4-byte loads.  Pixels beyond the right / bottom edge are
+// not zero-filled by TMA here (the next row / snapshot follows in the super row): the consumer zeroes them.
+template <int REF_MODE, bool ACC, int T, bool UNAL = false>
 __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
+  static_assert(!UNAL || (T == 32 && !ACC), "the unaligned variant serves cells of 32 pixels without accumulation");
   // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
   // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
   constexpr bool kSmall = T < 8;
@@ -385,7 +407,8 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   // the shuffle tells the compiler the warp index is warp uniform, so cursors and addresses derived
   // from it live in uniform registers and the vector registers are left to the three tile arrays
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-  const int box_bytes = p.ntw * kTileBytes, pitch = p.ntw * 128;
+  const int pitch = p.ntw * 128 + (UNAL ? 16 : 0);  // bytes between rows of a box (UNAL: 4 floats wider, see above)
+  const int box_bytes = kFastTile * pitch;
   unsigned char* after_ring = smem + (size_t)p.nstage * box_bytes;
   uint64_t* full = reinterpret_cast<uint64_t*>(after_ring);
   uint64_t* empty = full + kMaxStages;
@@ -424,7 +447,15 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
           mbar_wait(empty_addr + slot * 8, phase ^ 1);  // passes at once on the first lap
           const uint32_t bar = full_addr + slot * 8;
           mbar_arrive_expect_tx(bar, box_bytes);
-          if (p.evict_first)
+          if constexpr (UNAL) {
+            const int k = p.k_rows, rpc = kFastTile / k;  // rows per class
+            const int g0 = ring_slot(p.z0, p.zmask, c.u0 + s) * p.srows + c.ty_local * kFastTile;  // first row of the block
+            for (int cls = 0; cls < k; ++cls) {
+              const int gf = g0 + ((cls - g0) & (k - 1));  // first row of the block in this class
+              const int x = cls * p.W + p.a_off + c.gx * p.ntw * kFastTile;
+              tma_load_box2d(ring_addr + slot * box_bytes + cls * rpc * pitch, &tmap, bar, x & ~3, gf / k);
+            }
+          } else if (p.evict_first)
             tma_load_box_hint(ring_addr + slot * box_bytes, &tmap, bar, c.gx * p.ntw * kFastTile, c.ty_local * kFastTile,
                               ring_slot(p.z0, p.zmask, c.u0 * acc + s), policy);
           else
@@ -447,9 +478,46 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   const bool leader = lane == Geo::leader_lane(lane);  // does the bookkeeping of its tile
 
   // next snapshot of the current segment: box slot -> registers, then hand the slot back
+  int zs = 0, seg_ty = 0;      // UNAL: snapshot of the segment the next acquire() takes, and the segment's block row
+  int wv = kFastTile, hv = kFastTile;  // UNAL: valid columns / rows of this warp's block
   auto acquire = [&](float (&N)[32], float& zmin) {
     mbar_wait(full_addr + slot * 8, phase);
+    if constexpr (UNAL) {
+      const int k = p.k_rows, rb = lane >> 3, cg = lane & 7;
+      const int g0 = ring_slot(p.z0, p.zmask, zs) * p.srows + seg_ty * kFastTile;
+      ++zs;
+      const int cls = (g0 + rb) & (k - 1);                       // the class of this lane's rows
+      const int gf = g0 + ((cls - g0) & (k - 1));                // first row of the block in that class
+      const int shift = (cls * p.W + p.a_off) & 3;
+      const unsigned char* src = smem + (size_t)slot * box_bytes + (cls * (kFastTile / k) + (g0 + rb - gf) / k) * pitch +
+                                 warp * 128 + cg * 16 + shift * 4;
+      const int rstride = (4 / k) * pitch;                       // rows rb + 4 j are 4 / k rows apart inside their class
+      // one instruction sequence for all lanes (their shifts differ: a branch per shift would run every variant in
+      // turn): 8-byte loads when every shift of this launch is even, 4-byte loads otherwise
+      if (p.even_shifts) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float2 t0 = *reinterpret_cast<const float2*>(src + j * rstride);
+          const float2 t1 = *reinterpret_cast<const float2*>(src + j * rstride + 8);
+          N[4 * j] = t0.x; N[4 * j + 1] = t0.y; N[4 * j + 2] = t1.x; N[4 * j + 3] = t1.y;
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const float* t = reinterpret_cast<const float*>(src + j * rstride);
+          N[4 * j] = t[0]; N[4 * j + 1] = t[1]; N[4 * j + 2] = t[2]; N[4 * j + 3] = t[3];
+        }
+      }
+      if (wv < kFastTile || hv < kFastTile) {  // (warp uniform) the block hangs over the image edge
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            if (rb + 4 * j >= hv || 4 * cg + e >= wv) N[4 * j + e] = 0.f;
+      }
+    } else {
     load_tile<kLoadGeom>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
+    }
     __syncwarp();  // every lane has its copy
     if (lane == 0) mbar_arrive(empty_addr + slot * 8);
     if (++slot == p.nstage) { slot = 0; phase ^= 1; }
@@ -548,7 +616,17 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
         *reinterpret_cast<RawTile**>(&scratch[kScratchRec + 1]) = rp;
         // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
         const int off = sub_off + (int)(tg / T) * p.W + (int)(tg % T);
-        if (acc <= kMaxAccAsync) {
+        if constexpr (UNAL) {  // the group is not on a 16-byte boundary and may hang over the right edge (zeroes, as loaded)
+          const int col0 = (int)(tg % T);
+          const float* ip[3] = {ip0, ip1, ip2};
+#pragma unroll
+          for (int k3 = 0; k3 < 3; ++k3)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const bool in = col0 + e < wv;
+              cp_async4_zfill(scratch_addr + k3 * 16 + e * 4, in ? ip[k3] + off + e : p.base, in ? 4 : 0);
+            }
+        } else if (acc <= kMaxAccAsync) {
           for (int i = 0; i < acc; ++i) {
             cp_async16(scratch_addr + i * 16, ip0 + off + i * p.snap_stride);
             cp_async16(scratch_addr + (acc + i) * 16, ip1 + off + i * p.snap_stride);
@@ -666,6 +744,11 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       const int tx_t = tx * Geo::NSUB + Geo::sub_col(lane);
       tile_exists = Geo::NSUB == 1 || (ty_t < p.ty_end && tx_t < p.Tx);
       rp = p.raw + ((long long)c.u0 * p.Ty + ty_t) * p.Tx + tx_t;
+    }
+    if constexpr (UNAL) {
+      zs = c.u0; seg_ty = c.ty_local;
+      wv = min(kFastTile, p.W - tx * kFastTile);
+      hv = min(kFastTile, p.rows - c.ty_local * kFastTile);
     }
     acquire(A, zA);  // x_{u0}
     acquire(B, zB);  // x_{u0+1}

@@ -28,6 +28,7 @@ Tuning read_tuning_env() {
   t.march_cons = env_int("FITRIG_MARCH_CONS", 0);
   t.march_prod = env_int("FITRIG_MARCH_PROD", 0);
   t.march_box_kb = env_int("FITRIG_MARCH_BOX_KB", 0);
+  t.no_unaligned_fused = env_int("FITRIG_NO_UNALIGNED_FUSED", 0);
   return t;
 }
 
@@ -135,7 +136,6 @@ bool fused_tile(int tile) {
 }
 
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan) {
-  if (num_sms <= 0) num_sms = 148;
   const bool force_generic = tn.force_generic != 0;
   if (!fused_tile(tile) || (W % 4) != 0 || force_generic) {
     plan->path = 1;
@@ -147,21 +147,28 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn
     plan->grid = 0;  // sized per launch
     return;
   }
+  plan_launch_fused(tile, W, rows, U, num_sms, tn, 0, plan);
+}
+
+void plan_launch_fused(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, int extra_row_bytes, fitrig_plan* plan) {
+  if (num_sms <= 0) num_sms = 148;
   plan->path = 0;
   const int rows32 = (rows + kFastTile - 1) / kFastTile, Tx32 = (W + kFastTile - 1) / kFastTile;
   const int fb = tn.box_tiles, fs = tn.stages, fg = tn.grid;
-  int ntw = std::min(kMaxTilesPerBox, Tx32);
+  // (a TMA box is at most 256 elements wide: the unaligned variant's boxes are 4 floats wider than their tiles)
+  int ntw = std::min(extra_row_bytes ? kMaxTilesPerBox - 1 : kMaxTilesPerBox, Tx32);
   auto pairs = [&](int n) { return (long long)rows32 * ((Tx32 + n - 1) / n) * U; };
   // small problems are latency bound: narrower boxes give more CTAs something to do
   while (ntw > 1 && (pairs(ntw) + kMinUnitsPerCta - 1) / kMinUnitsPerCta < num_sms) ntw = (ntw + 1) / 2;
-  if (fb > 0) ntw = std::max(1, std::min(fb, std::min(kMaxTilesPerBox, Tx32)));
+  if (fb > 0) ntw = std::max(1, std::min(fb, std::min(extra_row_bytes ? kMaxTilesPerBox - 1 : kMaxTilesPerBox, Tx32)));
   const long long G = pairs(ntw);
   int grid = (int)std::max<long long>(1, std::min<long long>(num_sms, (G + kMinUnitsPerCta - 1) / kMinUnitsPerCta));
   if (fg > 0) grid = fg;
   const int per_edge = (tile < kFastTile && tile >= 8) ? kFastTile / tile : 1;
   const int groups = per_edge * per_edge;  // tiles per warp that keep an arg-max scratch (tiles below 8 pixels need none)
   const int scratch = ntw * groups * kScratchVec * 16;
-  const int fit = (kMaxSmemPerCta - 2048 - scratch) / (ntw * kTileBytes);
+  const int box_bytes = ntw * kTileBytes + kFastTile * extra_row_bytes;
+  const int fit = (kMaxSmemPerCta - 2048 - scratch) / box_bytes;
   int stages = std::min(6, fit);
   if (fs > 0) stages = std::min(fs, fit);
   stages = std::max(2, std::min(stages, kMaxStages));
@@ -170,7 +177,7 @@ void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn
   plan->stages = stages;
   plan->grid = grid;
   plan->units_per_cta = (int32_t)((G + grid - 1) / grid);
-  plan->smem_bytes = stages * ntw * kTileBytes + 2 * kMaxStages * 8 + scratch;  // ring, mbarriers, scratch
+  plan->smem_bytes = stages * box_bytes + 2 * kMaxStages * 8 + scratch;  // ring, mbarriers, scratch
 }
 
 MarchPlan plan_march(int c, int W, int rows, int U, int num_sms, const Tuning& tn, bool shifted_rows) {

@@ -45,6 +45,7 @@ struct Tuning {
   int march_cons;       // FITRIG_MARCH_CONS     generic time-marching kernel: consumer warps per CTA
   int march_prod;       // FITRIG_MARCH_PROD     generic time-marching kernel, cp.async variant: producer warps per CTA
   int march_box_kb;     // FITRIG_MARCH_BOX_KB   generic time-marching kernel: target size of a box in KB
+  int no_unaligned_fused;  // FITRIG_NO_UNALIGNED_FUSED  unaligned rows: the generic kernel instead of the fused kernel's super-row variant
 };
 Tuning read_tuning_env();
 
@@ -64,6 +65,9 @@ int normalize_params(int32_t H, int32_t W, int32_t L, const fitrig_params* p, No
 // Chooses path, tiles per box (consumer warps per CTA), ring depth and grid for `tile_rows` x Tx tiles of U units.
 // `rows`: image rows covered by the launch (the whole image, or one strip).
 void plan_launch(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, fitrig_plan* plan);
+// The fused path's box width, ring depth and grid whatever W % 4 is (the caller has checked that the fused kernel can run);
+// extra_row_bytes: what a box row is wider than its tiles (16 for the unaligned variant, kernels.cuh UNAL).
+void plan_launch_fused(int tile, int W, int rows, int U, int num_sms, const Tuning& tn, int extra_row_bytes, fitrig_plan* plan);
 // Generic time-marching kernel (kernels.cuh, tlisi_march_kernel): boxes of nty x ntx whole cells of c pixels.
 constexpr int kMarchMaxCell = 112;     // the ring needs >= 4 boxes of c x c floats in shared memory
 constexpr int kMarchMaxWarps = 24;     // warps per CTA (768 threads: up to 85 registers each)

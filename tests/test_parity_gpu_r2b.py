@@ -163,3 +163,64 @@ def test_small_tiles_first_maximum_in_row_major_order(tile):
     assert np.all(md == 3.0)
     for (ty, tx), (x, y) in want.items():
         assert (int(ax[0, ty, tx]), int(ay[0, ty, tx])) == (x, y)
+
+
+# ------------------------------------------------------------------------------------------
+# rows that do not start on 16-byte boundaries (W % 4 != 0): cells of 32 pixels ride the fused kernel through a
+# tensor map of "super rows" (k = 2 or 4 image rows); shapes whose total row count is not a multiple of k, and
+# unaligned base pointers, stay on the generic kernel
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("H,W,L,tile,use_stream", [(100, 250, 8, 32, False), (96, 251, 8, 32, False), (130, 253, 8, 32, False),
+                                                   (64, 66, 6, 32, False), (70, 255, 8, 64, False), (160, 250, 8, 32, True),
+                                                   (33, 251, 5, 32, False), (257, 1027, 4, 32, False)])
+def test_rows_off_16_byte_boundaries(H, W, L, tile, use_stream):
+    st = _stack(H, W, L)
+    taus = (2.0, 3.0)
+    kw = dict(strip_rows=64) if use_stream else {}
+    g = gpu_run(st, taus=taus, tile=tile, use_stream=use_stream, **kw)
+    ref = oracle_run(st, tile=tile, tau=3.0)
+    check_against_oracle(st, g, ref, taus, tile, small_tiles=util.needs_slack(H, W, tile))
+
+
+def test_rows_off_16_byte_boundaries_fused_and_generic_kernels_agree(monkeypatch):
+    H, W, L = 200, 254, 8
+    st = _stack(H, W, L)
+    a = gpu_run(st, taus=(3.0,))
+    monkeypatch.setenv("FITRIG_NO_UNALIGNED_FUSED", "1")
+    b = gpu_run(st, taus=(3.0,))
+    monkeypatch.delenv("FITRIG_NO_UNALIGNED_FUSED")
+    np.testing.assert_allclose(a["q"], b["q"], rtol=2e-6, atol=1e-30)  # (other summation order)
+    assert a["M"] == b["M"]
+    assert a["cands"][3.0][1] == b["cands"][3.0][1]
+    assert np.array_equal(a["raw"][3], b["raw"][3]) and np.array_equal(a["raw"][4], b["raw"][4])  # arg-max pixels
+
+
+def test_rows_off_16_byte_boundaries_push():
+    H, W, L, tau = 96, 250, 7, 3.0
+    st = _stack(H, W, L)
+    ref = oracle.run_realtime(st.cpu().numpy(), tile=32, tau=tau)
+    with fitrig.Context(H, W, 3) as ctx:
+        for i, s in enumerate(list(st) + [None]):
+            u, c, n = ctx.push(s, tau)
+            if u >= 0:
+                util.assert_map_close(ctx.get_map(0)[0], ref[u].res.q[0])
+                assert n == ref[u].cands.n_found or abs(n - ref[u].cands.n_found) <= 1
+
+
+@pytest.mark.parametrize("W,off", [(252, 1), (252, 2), (250, 1), (250, 3), (251, 2)])
+def test_unaligned_base_pointers_with_any_width(W, off):
+    """The stack starts `off` floats past a 16-byte boundary: the super rows start at the boundary below it."""
+    H, L, tau = 100, 8, 3.0
+    st = _stack(H, W, L)
+    flat = torch.empty(L * H * W + off, dtype=torch.float32, device=DEV)
+    view = flat[off:].view(L, H, W)
+    view.copy_(st)
+    assert view.data_ptr() % 16 == 4 * off
+    g = gpu_run(view, taus=(tau,))
+    ref = oracle_run(view, tile=32, tau=tau)
+    check_against_oracle(view, g, ref, (tau,), 32)
+    a = gpu_run(st, taus=(tau,))  # the same pixels from an aligned allocation
+    if W % 4 == 0:
+        assert np.array_equal(a["q"], g["q"])  # aligned rows ride the plain fused kernel: the same arithmetic, the same order
+    else:
+        np.testing.assert_allclose(a["q"], g["q"], rtol=0, atol=0)  # both take the super-row variant
