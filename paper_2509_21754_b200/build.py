@@ -43,7 +43,7 @@ def source_hash() -> str:
     for d in DEPS:
         with open(d, "rb") as f:
             h.update(f.read())
-    h.update(" ".join(NVCC_FLAGS).encode())
+    h.update(" ".join(NVCC_FLAGS).replace(ROOT, ".").encode())  # (the checkout's path is not part of the build)
     return h.hexdigest()
 
 
