@@ -40,7 +40,7 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when 
 # `ncu --set full` capture summarised in profiles/ (None until a capture has been taken for this build)
 # (keyed to the build: `srchash` is paper_2509_21754_b200.build.source_hash() of the build the capture was taken on;
 # any other build prints "traffic": null)
-NCU_TRAFFIC = {"srchash": None, "meerkat": None}
+NCU_TRAFFIC = {"srchash": "7270d9334f8034623974967e331b457c347d4b8174910ccee5fa24489ca1842f", "meerkat": 1090505296}  # profiles/r02_b_final.md
 
 
 def parse_args():
@@ -383,9 +383,17 @@ def run_fitrig(args, cfg, tau, branch):
     launches_per_step = n_ch if not strong else 1
     step_bytes = alg_bytes * launches_per_step + 8 * n_ch * U * Ty * Tx  # + q and tLISI written by the finalise
     step_ms = ms_max / args.steps
+    # which tLISI kernel the library takes (the plan is host-only and assumes a 16-byte aligned base): rows off 16-byte
+    # boundaries ride the fused kernel's super-row variant when the cells are 32 pixels and the stack's row count is a
+    # multiple of k = 4 / gcd(W, 4), the generic time-marching kernel otherwise
+    import math
+    rows_here = H if not strong else sc.r1 - sc.r0
+    super_rows = (plan.path != 0 and W % 4 != 0 and TILE % 32 == 0 and ACCUMULATE == 1 and (L * rows_here) % (4 // math.gcd(W, 4)) == 0
+                  and not os.environ.get("FITRIG_FORCE_GENERIC") and not os.environ.get("FITRIG_NO_UNALIGNED_FUSED"))
+    path_name = "fused-tma" if plan.path == 0 else ("fused-tma (super rows)" if super_rows else "generic")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": ncu_traffic(cfg.name), "kernel": "tlisi_fused_kernel" if plan.path == 0 else
-                "tlisi_generic_kernel", "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
+                "traffic": ncu_traffic(cfg.name), "kernel": "tlisi_fused_kernel" if path_name != "generic" else
+                "tlisi_march_kernel", "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "read_only_peak": read_peak, "frac_of_read_only_peak": (achieved / read_peak) if read_peak else None,
                 "read_only_peak_source": "fitrig_probe_read_bandwidth: plain float4 grid-stride read of the same stack, best of 5, this run",
                 "finalize_ms": fin_tot / max(fin_n, 1), "kernel_launches_timed": main_n,
@@ -509,7 +517,7 @@ def run_fitrig(args, cfg, tau, branch):
                        "ms_per_step_sync": ms_sync / args.steps,
                        "l2": f"input {4 * pix // world / 1e6:.0f} MB per step vs 126 MB L2: "
                              + ("larger than L2, no flush" if 4 * pix // world > 2 * 126e6 else "fits L2 (launch-latency-bound config)"),
-                       "plan": {"path": "fused-tma" if plan.path == 0 else "generic", "units_per_cta": plan.units_per_cta, "box_tiles": plan.box_tiles,
+                       "plan": {"path": path_name, "units_per_cta": plan.units_per_cta, "box_tiles": plan.box_tiles,
                                 "warps_per_cta": plan.warps_per_cta, "stages": plan.stages, "grid": plan.grid},
                        "build": lib_build.source_hash()[:16], "dist_backend": backend},
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches) * world,
