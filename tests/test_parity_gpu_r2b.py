@@ -4,6 +4,8 @@ the degenerate sigma == 0 rows with a negative threshold, batches whose tLISI ke
 dependent launches.  Same rules as test_parity_gpu.py: through the C ABI, against the CPU fp64 oracle on the same
 seeded buffers, tolerances of DESIGN.md section 3.
 """
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -220,7 +222,8 @@ def test_unaligned_base_pointers_with_any_width(W, off):
     ref = oracle_run(view, tile=32, tau=tau)
     check_against_oracle(view, g, ref, (tau,), 32)
     a = gpu_run(st, taus=(tau,))  # the same pixels from an aligned allocation
-    if W % 4 == 0:
-        assert np.array_equal(a["q"], g["q"])  # aligned rows ride the plain fused kernel: the same arithmetic, the same order
+    if os.environ.get("FITRIG_NO_UNALIGNED_FUSED") or os.environ.get("FITRIG_FORCE_GENERIC"):
+        np.testing.assert_allclose(a["q"], g["q"], rtol=2e-6, atol=1e-30)  # (the generic kernel sums in another order)
     else:
-        np.testing.assert_allclose(a["q"], g["q"], rtol=0, atol=0)  # both take the super-row variant
+        # the plain fused kernel (aligned, W % 4 == 0) and its super-row variant do the same arithmetic in the same order
+        assert np.array_equal(a["q"], g["q"])
