@@ -384,11 +384,12 @@ def run_fitrig(args, cfg, tau, branch):
     step_bytes = alg_bytes * launches_per_step + 8 * n_ch * U * Ty * Tx  # + q and tLISI written by the finalise
     step_ms = ms_max / args.steps
     # which tLISI kernel the library takes (the plan is host-only and assumes a 16-byte aligned base): rows off 16-byte
-    # boundaries ride the fused kernel's super-row variant when the cells are 32 pixels and the stack's row count is a
-    # multiple of k = 4 / gcd(W, 4), the generic time-marching kernel otherwise
+    # boundaries ride the fused kernel's super-row variant when the cell size is one the fused kernel serves and the stack's
+    # row count is a multiple of k = 4 / gcd(W, 4), the generic time-marching kernel otherwise
     import math
     rows_here = H if not strong else sc.r1 - sc.r0
-    super_rows = (plan.path != 0 and W % 4 != 0 and TILE % 32 == 0 and ACCUMULATE == 1 and (L * rows_here) % (4 // math.gcd(W, 4)) == 0
+    fused_cells = fitrig.plan_query(rows_here, (W + 3) // 4 * 4, L, num_sms=num_sms, tile=TILE).path == 0  # but for the width
+    super_rows = (plan.path != 0 and W % 4 != 0 and fused_cells and ACCUMULATE == 1 and (L * rows_here) % (4 // math.gcd(W, 4)) == 0
                   and not os.environ.get("FITRIG_FORCE_GENERIC") and not os.environ.get("FITRIG_NO_UNALIGNED_FUSED"))
     path_name = "fused-tma" if plan.path == 0 else ("fused-tma (super rows)" if super_rows else "generic")
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

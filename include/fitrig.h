@@ -41,7 +41,7 @@
  *       FITRIG_MARCH_PROD=n      generic kernel, cp.async variant: n producer warps per CTA (default 8)
  *       FITRIG_MARCH_BOX_KB=n    generic kernel: boxes of about n KB (default 32)
  *       FITRIG_NO_UNALIGNED_FUSED=1  images whose rows do not start on 16-byte boundaries: the generic kernel even where
- *                                the fused kernel's super-row variant applies (cells of 32 pixels)
+ *                                the fused kernel's super-row variant applies (cells of 1, 2, 4, 8, 16, 32 pixels)
  */
 #ifndef FITRIG_H_
 #define FITRIG_H_

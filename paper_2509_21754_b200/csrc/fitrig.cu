@@ -199,8 +199,11 @@ static cudaError_t set_fused_attr_one() {
 template <int REF>
 static cudaError_t set_fused_attr() {
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(tlisi_fused_kernel<REF, false, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+#define UNAL_ATTR(T)                                                                                                      \
+  if ((e = cudaFuncSetAttribute(tlisi_fused_kernel<REF, false, T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                 kMaxSmemPerCta)) != cudaSuccess) return e;
+  UNAL_ATTR(32) UNAL_ATTR(16) UNAL_ATTR(8) UNAL_ATTR(4) UNAL_ATTR(2) UNAL_ATTR(1)
+#undef UNAL_ATTR
   if ((e = set_fused_attr_one<REF, false, 32>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, true, 32>()) != cudaSuccess) return e;
   if ((e = set_fused_attr_one<REF, false, 16>()) != cudaSuccess) return e;
@@ -479,7 +482,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   bool unal = false;
   int unal_k = 1;
   const int unal_a = (int)(((uintptr_t)base >> 2) & 3);
-  if (!aligned && tile == kFastTile && c->prm.accumulate == 1 && !c->tune.force_generic && !c->tune.no_unaligned_fused &&
+  if (!aligned && tile <= kFastTile && fused_tile(tile) && c->prm.accumulate == 1 && !c->tune.force_generic && !c->tune.no_unaligned_fused &&
       (uintptr_t)base % 4 == 0 && snap_stride % c->W == 0 && snap_stride / c->W >= rows && r0 % kFastTile == 0) {
     unal_k = 4 / std::gcd(c->W, 4);
     // (dim0 = k W + a_off exceeds the row stride of k W by a_off: rows of the tensor map overlap, which the driver accepts
@@ -542,11 +545,17 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     fp.dep = (c->tune.no_pdl || c->profile) ? 0 : opt.dep;
     const dim3 grid(pl.grid), block(32 * pl.warps_per_cta);
     if (unal) {
+#define UNAL_LAUNCH(R, T) launch_tlisi_kernel(tlisi_fused_kernel<R, false, T, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp)
+#define UNAL_TILES(R)                                                                                               \
+  (tile == 16 ? UNAL_LAUNCH(R, 16) : tile == 8 ? UNAL_LAUNCH(R, 8) : tile == 4 ? UNAL_LAUNCH(R, 4) : tile == 2 ? UNAL_LAUNCH(R, 2) \
+   : tile == 1 ? UNAL_LAUNCH(R, 1) : UNAL_LAUNCH(R, 32))
       switch (c->prm.ref_mode) {
-        case FITRIG_REF_ABS: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_ABS, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
-        case FITRIG_REF_LITERAL: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_LITERAL, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
-        default: launch_tlisi_kernel(tlisi_fused_kernel<FITRIG_REF_FLOOR, false, 32, true>, grid, block, (size_t)pl.smem_bytes, st, tm, fp); break;
+        case FITRIG_REF_ABS: UNAL_TILES(FITRIG_REF_ABS); break;
+        case FITRIG_REF_LITERAL: UNAL_TILES(FITRIG_REF_LITERAL); break;
+        default: UNAL_TILES(FITRIG_REF_FLOOR); break;
       }
+#undef UNAL_TILES
+#undef UNAL_LAUNCH
     } else
     switch (c->prm.ref_mode) {
       case FITRIG_REF_ABS: launch_fused<FITRIG_REF_ABS>(fp.acc > 1, tile, grid, block, pl.smem_bytes, st, tm, fp); break;

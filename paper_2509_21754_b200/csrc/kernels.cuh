@@ -395,7 +395,7 @@ __device__ __forceinline__ void tile_step(const float (&N)[32], const float (&X)
 template <int REF_MODE, bool ACC, int T, bool UNAL = false>
 __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     tlisi_fused_kernel(const __grid_constant__ CUtensorMap tmap, const FusedParams p) {
-  static_assert(!UNAL || (T == 32 && !ACC), "the unaligned variant serves cells of 32 pixels without accumulation");
+  static_assert(!UNAL || !ACC, "the unaligned variant does not accumulate");
   // T >= 8: tiles are lane groups of a warp's block (LaneGeom<T>).  T = 4, 2, 1: a lane holds pixels of several
   // tiles; the block is read with the T = 32 geometry and reduced per 16-byte quad (small_step below).
   constexpr bool kSmall = T < 8;
@@ -483,37 +483,62 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
   auto acquire = [&](float (&N)[32], float& zmin) {
     mbar_wait(full_addr + slot * 8, phase);
     if constexpr (UNAL) {
-      const int k = p.k_rows, rb = lane >> 3, cg = lane & 7;
+      const int k = p.k_rows, lk = k >> 1;  // k = 1, 2, 4: log2 k = k / 2
       const int g0 = ring_slot(p.z0, p.zmask, zs) * p.srows + seg_ty * kFastTile;
       ++zs;
-      const int cls = (g0 + rb) & (k - 1);                       // the class of this lane's rows
-      const int gf = g0 + ((cls - g0) & (k - 1));                // first row of the block in that class
-      const int shift = (cls * p.W + p.a_off) & 3;
-      const unsigned char* src = smem + (size_t)slot * box_bytes + (cls * (kFastTile / k) + (g0 + rb - gf) / k) * pitch +
-                                 warp * 128 + cg * 16 + shift * 4;
-      const int rstride = (4 / k) * pitch;                       // rows rb + 4 j are 4 / k rows apart inside their class
+      const int o0 = g0 & (k - 1);          // the block's first row inside its super row
+      const unsigned char* slot_col = smem + (size_t)slot * box_bytes + warp * 128 + lane_col<kLoadGeom>(lane) * 4;
+      // where row r of the block sits: class cls = (g0 + r) % k, the ((g0 + r) / k - g0 / k - (cls < o0))-th row of that
+      // class's box, shifted by (cls * W + a_off) % 4 floats
+      auto row_ptr = [&](int r) {
+        const int g = g0 + r, cls = g & (k - 1);
+        const int idx = (g >> lk) - (g0 >> lk) - (cls < o0 ? 1 : 0);
+        return slot_col + (cls * (kFastTile / k) + idx) * pitch + ((cls * p.W + p.a_off) & 3) * 4;
+      };
       // one instruction sequence for all lanes (their shifts differ: a branch per shift would run every variant in
       // turn): 8-byte loads when every shift of this launch is even, 4-byte loads otherwise
-      if (p.even_shifts) {
+      if constexpr (kLoadGeom == 32) {
+        // rows lane / 8 + 4 j all belong to one class (4 j is a multiple of k): one pointer, a fixed stride
+        const unsigned char* src = row_ptr(lane >> 3);
+        const int rstride = (4 / k) * pitch;
+        if (p.even_shifts) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const float2 t0 = *reinterpret_cast<const float2*>(src + j * rstride);
-          const float2 t1 = *reinterpret_cast<const float2*>(src + j * rstride + 8);
-          N[4 * j] = t0.x; N[4 * j + 1] = t0.y; N[4 * j + 2] = t1.x; N[4 * j + 3] = t1.y;
+          for (int j = 0; j < 8; ++j) {
+            const float2 t0 = *reinterpret_cast<const float2*>(src + j * rstride);
+            const float2 t1 = *reinterpret_cast<const float2*>(src + j * rstride + 8);
+            N[4 * j] = t0.x; N[4 * j + 1] = t0.y; N[4 * j + 2] = t1.x; N[4 * j + 3] = t1.y;
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const float* t = reinterpret_cast<const float*>(src + j * rstride);
+            N[4 * j] = t[0]; N[4 * j + 1] = t[1]; N[4 * j + 2] = t[2]; N[4 * j + 3] = t[3];
+          }
         }
       } else {
+        if (p.even_shifts) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const float* t = reinterpret_cast<const float*>(src + j * rstride);
-          N[4 * j] = t[0]; N[4 * j + 1] = t[1]; N[4 * j + 2] = t[2]; N[4 * j + 3] = t[3];
+          for (int j = 0; j < 8; ++j) {
+            const unsigned char* src = row_ptr(lane_row<kLoadGeom>(lane, j));
+            const float2 t0 = *reinterpret_cast<const float2*>(src);
+            const float2 t1 = *reinterpret_cast<const float2*>(src + 8);
+            N[4 * j] = t0.x; N[4 * j + 1] = t0.y; N[4 * j + 2] = t1.x; N[4 * j + 3] = t1.y;
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const float* t = reinterpret_cast<const float*>(row_ptr(lane_row<kLoadGeom>(lane, j)));
+            N[4 * j] = t[0]; N[4 * j + 1] = t[1]; N[4 * j + 2] = t[2]; N[4 * j + 3] = t[3];
+          }
         }
       }
       if (wv < kFastTile || hv < kFastTile) {  // (warp uniform) the block hangs over the image edge
+        const int c0 = lane_col<kLoadGeom>(lane);
 #pragma unroll
         for (int j = 0; j < 8; ++j)
 #pragma unroll
           for (int e = 0; e < 4; ++e)
-            if (rb + 4 * j >= hv || 4 * cg + e >= wv) N[4 * j + e] = 0.f;
+            if (lane_row<kLoadGeom>(lane, j) >= hv || c0 + e >= wv) N[4 * j + e] = 0.f;
       }
     } else {
     load_tile<kLoadGeom>(N, my_col + (size_t)slot * box_bytes, pitch, lane);
@@ -617,7 +642,7 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
         // the winning group's 4 pixels in the three images: in bounds (a zero-filled pixel has Delta 0)
         const int off = sub_off + (int)(tg / T) * p.W + (int)(tg % T);
         if constexpr (UNAL) {  // the group is not on a 16-byte boundary and may hang over the right edge (zeroes, as loaded)
-          const int col0 = (int)(tg % T);
+          const int col0 = Geo::sub_col(lane) * T + (int)(tg % T);  // column inside the warp's 32 x 32 block
           const float* ip[3] = {ip0, ip1, ip2};
 #pragma unroll
           for (int k3 = 0; k3 < 3; ++k3)
@@ -711,16 +736,24 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
       // cells of one pixel are kept as 8-byte records {Delta, r} (RawPix; rp - p.raw is a record index); the four
       // records of a quad are 32 contiguous, 16-byte aligned bytes (W % 4 == 0 on this path): two 16-byte stores
       RawPix* const pix = reinterpret_cast<RawPix*>(p.raw) + (rp - p.raw) + 4 * cg;  // (rp is the record of tile (ty0, tx0))
-      const bool col_ok = tx0 + 4 * cg < p.Tx;
+      const int ncol = p.Tx - (tx0 + 4 * cg);  // records of this quad inside the map row (>= 4: all of them)
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         const int row = rq + 4 * j;
         float d0, d1, d2, d3, r0, r1, r2, r3;
         pixel(4 * j, d0, r0); pixel(4 * j + 1, d1, r1); pixel(4 * j + 2, d2, r2); pixel(4 * j + 3, d3, r3);
-        if (col_ok && ty0 + row < p.ty_end) {
-          float4* dst = reinterpret_cast<float4*>(pix + (long long)row * p.Tx);
-          dst[0] = make_float4(d0, r0, d1, r1);
-          dst[1] = make_float4(d2, r2, d3, r3);
+        if (ncol > 0 && ty0 + row < p.ty_end) {
+          RawPix* dst = pix + (long long)row * p.Tx;
+          if (!UNAL || (ncol >= 4 && (p.Tx & 1) == 0)) {  // (map rows of even length: the quad's records are 16-byte aligned)
+            reinterpret_cast<float4*>(dst)[0] = make_float4(d0, r0, d1, r1);
+            reinterpret_cast<float4*>(dst)[1] = make_float4(d2, r2, d3, r3);
+          } else {
+            RawPix v;
+            v.delta = d0; v.r = r0; dst[0] = v;
+            if (ncol > 1) { v.delta = d1; v.r = r1; dst[1] = v; }
+            if (ncol > 2) { v.delta = d2; v.r = r2; dst[2] = v; }
+            if (ncol > 3) { v.delta = d3; v.r = r3; dst[3] = v; }
+          }
         }
       }
     }

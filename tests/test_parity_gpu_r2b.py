@@ -174,12 +174,16 @@ def test_small_tiles_first_maximum_in_row_major_order(tile):
 # ------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("H,W,L,tile,use_stream", [(100, 250, 8, 32, False), (96, 251, 8, 32, False), (130, 253, 8, 32, False),
                                                    (64, 66, 6, 32, False), (70, 255, 8, 64, False), (160, 250, 8, 32, True),
-                                                   (33, 251, 5, 32, False), (257, 1027, 4, 32, False)])
+                                                   (33, 251, 5, 32, False), (257, 1027, 4, 32, False),
+                                                   (100, 250, 8, 16, False), (96, 251, 8, 16, False), (130, 253, 8, 8, False),
+                                                   (100, 250, 8, 8, True), (70, 254, 6, 4, False), (66, 251, 8, 4, False),
+                                                   (64, 250, 6, 2, False), (40, 253, 8, 2, False), (48, 250, 6, 1, False),
+                                                   (40, 251, 8, 1, False), (70, 255, 8, 48, False), (64, 250, 6, 12, False)])
 def test_rows_off_16_byte_boundaries(H, W, L, tile, use_stream):
     st = _stack(H, W, L)
     taus = (2.0, 3.0)
     kw = dict(strip_rows=64) if use_stream else {}
-    g = gpu_run(st, taus=taus, tile=tile, use_stream=use_stream, **kw)
+    g = gpu_run(st, taus=taus, tile=tile, use_stream=use_stream, capacity=1 << 18, **kw)
     ref = oracle_run(st, tile=tile, tau=3.0)
     check_against_oracle(st, g, ref, taus, tile, small_tiles=util.needs_slack(H, W, tile))
 
