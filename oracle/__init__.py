@@ -5,9 +5,10 @@ bench.py's cpu_baseline / --impl reference legs may import this package.  It doe
 import, link or read anything of the CUDA path (paper_2509_21754_b200).
 
 The per-pixel, per-tile and spectral arithmetic lives in the C file; this module marshals numpy arrays and holds
-the three steps that are plain numpy one-liners: the fp64 sums of snapshot accumulation (`accumulate`), the
-maximum of the accumulated images (`_tlisi_f64`), and the running maximum of the real-time forms
-(`run_realtime`, `run_realtime_frequency`).
+the steps that are plain numpy one-liners: the fp64 sums of snapshot accumulation (`accumulate`), the
+maximum of the accumulated images (`_tlisi_f64`), the running maximum of the real-time forms
+(`run_realtime`, `run_realtime_frequency`), and the accumulation rule (`accumulation_contrast`, `choose_accumulate`:
+means of absolute values).
 """
 from __future__ import annotations
 
@@ -153,6 +154,39 @@ def accumulate(stack, g: int) -> List[np.ndarray]:
             a += snaps[g * j + i].astype(np.float64)
         out.append(a)
     return out
+
+
+def accumulation_contrast(stack, g: int) -> float:
+    """How different adjacent g-accumulated snapshots are (reading R30): the mean over adjacent pairs and
+    pixels of the paper's own difference image |A_{j+1} - A_j| (Eq. 3, on accumulated snapshots), relative
+    to the mean over accumulated snapshots and pixels of the intensity level |A_j| (the quantity Eq. 4 normalises by,
+    PAPER.md:171, 201).  0 for identical (or all-zero) snapshots.  Needs at least two accumulated snapshots."""
+    A = accumulate(stack, g)
+    if len(A) < 2:
+        raise ValueError("accumulation_contrast: need at least two accumulated snapshots")
+    num = float(np.mean([np.mean(np.abs(A[j + 1] - A[j])) for j in range(len(A) - 1)]))
+    den = float(np.mean([np.mean(np.abs(a)) for a in A]))
+    return num / den if den > 0.0 else 0.0
+
+
+def choose_accumulate(stack, eps: float, g_max: int = 32):
+    """PAPER.md:497 (section 3.3.2): "Snapshots can be combined progressively until there is enough difference between
+    adjacent accumulated snapshots."  The paper gives neither the measure nor the threshold; reading R30:
+    combine progressively as in Fig. 16 -- g = 1, 2, 4, ... while g <= g_max and at least 3 accumulated snapshots remain
+     -- and stop at the FIRST g whose accumulation_contrast reaches eps; if none does, take the largest
+    admissible g.  Returns (g, [(g_level, contrast), ...] for the levels that were looked at)."""
+    snaps = as_snapshots(stack)
+    if len(snaps) < 3 or g_max < 1:
+        raise ValueError("choose_accumulate: need L >= 3 and g_max >= 1")
+    levels, g, last = [], 1, 1
+    while g <= g_max and len(snaps) // g >= 3:
+        d = accumulation_contrast(snaps, g)
+        levels.append((g, d))
+        last = g
+        if d >= eps:
+            break
+        g *= 2
+    return last, levels
 
 
 def tlisi_windows(stack, tile: int, stride: int, C: float = 1e-6, ref_mode: int = REF_ABS,
