@@ -306,6 +306,23 @@ int fitrig_shard_import(fitrig_ctx* ctx, const double* d_all, int32_t world, flo
 int fitrig_shard_export_eta(fitrig_ctx* ctx, double* d_out /*device, 3 doubles*/, void* cuda_stream);
 int fitrig_shard_import_eta(fitrig_ctx* ctx, const double* d_all /*device, [world][3]*/, int32_t world, void* cuda_stream);
 
+/* fitrig_choose_accumulate -- the stopping rule of snapshot accumulation (section 3.3.2: "Snapshots can be
+ * combined progressively until there is enough difference between adjacent accumulated snapshots").  The paper gives
+ * neither the measure nor the threshold; reading R30: the group sizes g = 1, 2, 4, .., 32 with g <= g_max and
+ * at least 3 accumulated snapshots left are tried in this order (Fig. 16's pairwise tree), and the first
+ * whose contrast
+ *     d(g) = mean over j, pixels of |A_{j+1} - A_j|  /  mean over j, pixels of |A_j|,   A_j = x_{gj} + .. + x_{gj+g-1}
+ * (the difference image of Eq. 3 on accumulated snapshots over the intensity level Eq. 4 normalises by) reaches eps
+ * (d >= eps) is returned; if none does, the largest admissible g.  The result goes into fitrig_params.accumulate.
+ *   d_stack (device)  [n_snapshots][H][W] fp32, contiguous; read once per level tried
+ *   g_out (host)      the group size
+ *   contrast (host)   d of the levels looked at, g = 1, 2, 4, .. up to the returned one (room for 6); may be NULL
+ *   n_levels (host)   how many that is; may be NULL
+ * Needs no context.  Synchronises cuda_stream.  Errors: INVALID_ARG (NULL, H, W < 1, n_snapshots < 3, g_max < 1, eps NaN,
+ * device), NOMEM, CUDA. */
+int fitrig_choose_accumulate(const float* d_stack, int32_t H, int32_t W, int32_t n_snapshots, float eps, int32_t g_max,
+                             int32_t device, int32_t* g_out, double* contrast, int32_t* n_levels, void* cuda_stream);
+
 /* fitrig_get_stats -- M (B floats) and the per-unit mean / population std of q = 1 - tLISI
  * (Eq. 8; mu_tLISI = 1 - mu_q; B * U doubles each, row b * U + u).  Frequency branch after fitrig_detect: entry
  * b * U of mu and sigma (unit 0 of stack b) describes eta of that stack (Eq. 11) instead.  Host outputs, each may

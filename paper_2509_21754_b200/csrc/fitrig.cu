@@ -1321,6 +1321,43 @@ extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int
   return FITRIG_OK;
 }
 
+extern "C" int fitrig_choose_accumulate(const float* d_stack, int32_t H, int32_t W, int32_t L, float eps, int32_t g_max, int32_t device,
+                                        int32_t* g_out, double* contrast, int32_t* n_levels, void* cuda_stream) {
+  if (!d_stack || !g_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate: NULL argument");
+  if (H < 1 || W < 1 || L < 3 || g_max < 1 || device < 0 || !(eps == eps))
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate: need H, W >= 1, n_snapshots >= 3 (PAPER.md:155), g_max >= 1, a threshold");
+  int ndev = 0;
+  CUDA_TRY(cudaGetDeviceCount(&ndev));
+  if (device >= ndev) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate: device %d of %d", device, ndev);
+  CUDA_TRY(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, device));
+  if (prop.major < 10) return fail(FITRIG_ERR_CUDA, "fitrig_choose_accumulate: this library is built for sm_100a (B200) only");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int levels = 0;
+  for (int g = 1; levels < kAccumLevels && g <= g_max && L / g >= 3; g *= 2) ++levels;  // admissible group sizes (R30)
+  const long long hw = (long long)H * W;
+  const int nblocks = (int)std::min<long long>((hw + 255) / 256, 8ll * prop.multiProcessorCount);
+  DevBuf<double2> parts;
+  DevBuf<AccumChoice> choice;
+  CUDA_TRY(parts.alloc((size_t)levels * nblocks));
+  CUDA_TRY(choice.alloc(1));
+  for (int lv = 0; lv < levels; ++lv) {
+    accum_contrast_kernel<<<nblocks, 256, 0, st>>>(d_stack, hw, L, 1 << lv, parts.p + (size_t)lv * nblocks);
+    CUDA_TRY(cudaGetLastError());
+  }
+  accum_choose_kernel<<<1, 256, 0, st>>>(parts.p, nblocks, levels, L, hw, eps, choice.p);
+  CUDA_TRY(cudaGetLastError());
+  AccumChoice h;
+  CUDA_TRY(cudaMemcpyAsync(&h, choice.p, sizeof(h), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  *g_out = h.g;
+  if (n_levels) *n_levels = h.n_levels;
+  if (contrast)
+    for (int i = 0; i < h.n_levels; ++i) contrast[i] = h.contrast[i];
+  return FITRIG_OK;
+}
+
 extern "C" int fitrig_stream_timeline(const fitrig_ctx* c, float* ms, int32_t capacity, int32_t* n_strips) {
   if (!c || !n_strips) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream_timeline: NULL argument");
   if (capacity < 0 || (capacity > 0 && !ms)) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_stream_timeline: bad ms/capacity");

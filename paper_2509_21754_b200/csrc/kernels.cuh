@@ -1696,6 +1696,7 @@ __global__ void __launch_bounds__(kSpecChunk) spectrum_kernel(const SpectrumPara
       float best = 0.f;
       int kb = (K >= 1) ? 1 : 0;
       if (p.harmonics <= 1) {  // h = maximum spectral magnitude, first bin on ties
+#pragma unroll 8
         for (int k = 1; k <= K; ++k) {
           const float m = mag[(size_t)(k - 1) * p.nt + t];
           if (k == 1 || m > best) { best = m; kb = k; }
@@ -2149,6 +2150,67 @@ __global__ void __launch_bounds__(128) localise_kernel(const LocaliseParams p) {
     o.y = yc + (double)bj / (double)p.oversample;
     o.value = best;
     p.out[k] = o;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Stopping rule of snapshot accumulation (reading R30): for a group size g, the contrast of adjacent
+// accumulated snapshots d(g) = mean |A_{j+1} - A_j| / mean |A_j|.  accum_contrast_kernel: a thread walks its pixels
+// (grid stride) through the J = L / g accumulated snapshots (A_j summed in fp32 in snapshot order, as the tLISI kernels
+// accumulate), keeps sum |A_{j+1} - A_j| and sum |A_j| in fp64; block partials in block order.  accum_choose_kernel:
+// one block adds the partials of every level in a fixed order, forms d, and takes the first level with d >= eps (else
+// the last level).  Every snapshot byte is read once per level.
+// ---------------------------------------------------------------------------------------------
+constexpr int kAccumLevels = 6;  // g = 1, 2, 4, 8, 16, 32
+
+struct AccumChoice {
+  int g;                        // the chosen group size
+  int n_levels;                 // levels looked at
+  double contrast[kAccumLevels];
+};
+
+__global__ void __launch_bounds__(256) accum_contrast_kernel(const float* __restrict__ x, long long hw, int L, int g, double2* partials) {
+  __shared__ double sh[64];
+  const int J = L / g;
+  double num = 0.0, den = 0.0;
+  const long long step = (long long)gridDim.x * blockDim.x;
+  for (long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x; p < hw; p += step) {
+    float prev = 0.f;
+    for (int j = 0; j < J; ++j) {
+      const float* s = x + (long long)j * g * hw + p;
+      float a = s[0];
+      for (int i = 1; i < g; ++i) a += s[(long long)i * hw];  // A_j: g raw snapshots added in order
+      if (j > 0) num += (double)fabsf(a - prev);                // Eq. 3 on accumulated snapshots
+      den += (double)fabsf(a);
+      prev = a;
+    }
+  }
+  block_sum2(num, den, sh);
+  if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(num, den);
+}
+
+__global__ void __launch_bounds__(256) accum_choose_kernel(const double2* partials, int nblocks, int n_levels, int L, long long hw,
+                                                           float eps, AccumChoice* out) {
+  __shared__ double sh[64];
+  int chosen = -1;
+  for (int lv = 0; lv < n_levels; ++lv) {
+    double num = 0.0, den = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+      const double2 v = partials[(size_t)lv * nblocks + b];
+      num += v.x;
+      den += v.y;
+    }
+    block_sum2(num, den, sh);
+    const int J = L / (1 << lv);
+    const double mn = num / ((double)(J - 1) * (double)hw), md = den / ((double)J * (double)hw);
+    const double d = (md > 0.0) ? mn / md : 0.0;
+    if (threadIdx.x == 0) out->contrast[lv] = d;
+    if (chosen < 0 && d >= (double)eps) chosen = lv;  // (the same value in every thread)
+  }
+  if (threadIdx.x == 0) {
+    // progressive combination stops at the first level that reaches eps: later levels are reported as not looked at
+    out->n_levels = (chosen < 0) ? n_levels : chosen + 1;
+    out->g = 1 << ((chosen < 0) ? n_levels - 1 : chosen);
   }
 }
 

@@ -231,3 +231,45 @@ def test_unaligned_base_pointers_with_any_width(W, off):
     else:
         # the plain fused kernel (aligned, W % 4 == 0) and its super-row variant do the same arithmetic in the same order
         assert np.array_equal(a["q"], g["q"])
+
+
+# ------------------------------------------------------------------------------------------
+# fitrig_choose_accumulate: the stopping rule of snapshot accumulation (reading R30)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,H,W", [(24, 96, 128), (17, 33, 50), (64, 40, 64)])
+def test_choose_accumulate_matches_oracle(L, H, W):
+    base = synth.gaussian_noise_stack(L, H, W, seed=21, device=DEV)
+    drift = torch.arange(L, dtype=torch.float32, device=DEV)[:, None, None] * 0.02
+    st = (5.0 + 0.05 * base + drift).contiguous()  # a slow drift under a little noise: contrast grows with g
+    snaps = st.cpu().numpy()
+    levels = []
+    g = 1
+    while g <= 32 and L // g >= 3:
+        levels.append((g, oracle.accumulation_contrast(snaps, g)))
+        g *= 2
+    # contrast of every admissible level (an unreachable eps looks at all of them)
+    g_dev, d_dev = fitrig.choose_accumulate(st, 1e30)
+    assert g_dev == levels[-1][0] and len(d_dev) == len(levels)
+    # fp32 accumulation of g <= 32 snapshots and fp32 differences against fp64: (g + 2) 2^-24 relative on every term
+    for (g_, d_ref), d in zip(levels, d_dev):
+        assert abs(d - d_ref) <= 4e-6 * d_ref, (g_, d, d_ref)
+    # thresholds between the levels: the first level that reaches eps; at the oracle's own value of a level: that level
+    # (unless the two contrasts differ in the last digits, which the band above allows)
+    for i in range(1, len(levels)):
+        lo, hi = levels[i - 1][1], levels[i][1]
+        if hi > lo * 1.001:
+            eps = 0.5 * (lo + hi)
+            assert fitrig.choose_accumulate(st, eps)[0] == oracle.choose_accumulate(snaps, eps)[0] == levels[i][0]
+    assert fitrig.choose_accumulate(st, 0.0)[0] == 1
+    assert fitrig.choose_accumulate(st, 1e30, g_max=2)[0] == min(2, levels[-1][0])
+
+
+def test_choose_accumulate_degenerate_inputs():
+    st = torch.full((12, 16, 16), 2.5, device=DEV)
+    g, d = fitrig.choose_accumulate(st, 1e-6)
+    assert g == 4 and d == [0.0, 0.0, 0.0]  # identical snapshots: no contrast at any level; 12 // 8 < 3
+    assert fitrig.choose_accumulate(torch.zeros((6, 8, 8), device=DEV), 0.5) == (2, [0.0, 0.0])
+    with pytest.raises(fitrig.FitrigError):
+        fitrig.choose_accumulate(st[:2].contiguous(), 0.1)
+    with pytest.raises(fitrig.FitrigError):
+        fitrig.choose_accumulate(st, float("nan"))
