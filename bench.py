@@ -375,7 +375,7 @@ def run_fitrig(args, cfg, tau, branch):
     value = pix * args.steps / (ms_max * 1e-3) / 1e6
 
     # ---- roofline of the dominant (fused) kernel, and of the whole step ----
-    plan = fitrig.plan_query(H if not strong else sc.r1 - sc.r0, W, L, num_sms=num_sms, tile=TILE)
+    plan = fitrig.plan_query(H if not strong else sc.r1 - sc.r0, W, L, num_sms=num_sms, tile=TILE, accumulate=ACCUMULATE)
     k_ms = main_tot / max(main_n, 1)
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
@@ -384,14 +384,8 @@ def run_fitrig(args, cfg, tau, branch):
     step_bytes = alg_bytes * launches_per_step + 8 * n_ch * U * Ty * Tx  # + q and tLISI written by the finalise
     step_ms = ms_max / args.steps
     # which tLISI kernel the library takes (the plan is host-only and assumes a 16-byte aligned base): rows off 16-byte
-    # boundaries ride the fused kernel's super-row variant when the cell size is one the fused kernel serves and the stack's
-    # row count is a multiple of k = 4 / gcd(W, 4), the generic time-marching kernel otherwise
-    import math
-    rows_here = H if not strong else sc.r1 - sc.r0
-    fused_cells = fitrig.plan_query(rows_here, (W + 3) // 4 * 4, L, num_sms=num_sms, tile=TILE).path == 0  # but for the width
-    super_rows = (plan.path != 0 and W % 4 != 0 and fused_cells and ACCUMULATE == 1 and (L * rows_here) % (4 // math.gcd(W, 4)) == 0
-                  and not os.environ.get("FITRIG_FORCE_GENERIC") and not os.environ.get("FITRIG_NO_UNALIGNED_FUSED"))
-    path_name = "fused-tma" if plan.path == 0 else ("fused-tma (super rows)" if super_rows else "generic")
+    # boundaries (W % 4 != 0) ride the fused kernel's super-row variant where the plan says fused
+    path_name = ("fused-tma (super rows)" if W % 4 else "fused-tma") if plan.path == 0 else "generic"  # (fitrig_plan_query decides)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": ncu_traffic(cfg.name), "kernel": "tlisi_fused_kernel" if path_name != "generic" else
                 "tlisi_march_kernel", "kernel_ms": k_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,

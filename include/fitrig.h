@@ -6,7 +6,7 @@
  *      unit, and
  *   2. the significance-thresholded, compacted candidate list
  *      (image domain: Eq. 8-9; image-frequency domain: Eq. 10-12,
- *      PAPER.md:343-359 with h = maximum spectral magnitude).
+ *      PAPER.md:343-359 with h = maximum spectral magnitude, or harmonic summing).
  *
  * Citations are /root/reference/PAPER.md line numbers.  "R<n>" are the readings of silent or
  * ambiguous passages listed in DESIGN.md.
@@ -123,9 +123,12 @@ typedef struct {
   int32_t units, Ty, Tx;     /* map dimensions                                                   */
   int32_t path;              /* 0: fused time-marching kernel (registers): cells of 1, 2, 4, 8, 16 or 32 pixels -- the  */
                              /*    tile itself, a divisor of it (12 = 3 x 4, 48 = 3 x 16, 64 = 2 x 32 ...) or the stride */
-                             /*    of overlapping windows; W % 4 == 0 (TMA needs 16-byte aligned rows)                   */
+                             /*    of overlapping windows.  Rows that do not start on 16-byte boundaries (W % 4 != 0, or */
+                             /*    -- known only at the call -- an unaligned stack pointer) ride it through a tensor map */
+                             /*    of "super rows" of k = 4 / gcd(W, 4) image rows when the stack's row count is a       */
+                             /*    multiple of k and nothing is accumulated; boxes are then at most 7 blocks wide        */
                              /* 1: generic time-marching kernel (shared-memory ring): any other cell size (5, 7, 10 ..), */
-                             /*    any width, any alignment                                                              */
+                             /*    and whatever the fused kernel cannot take; any width, any alignment                   */
   int32_t units_per_cta;     /* fused path: (box column, unit) pairs per CTA, ceil(boxes * U / grid) */
   int32_t box_tiles;         /* fused path: adjacent 32x32 pixel blocks fetched as one TMA box (1..8) */
   int32_t warps_per_cta;     /* fused path: box_tiles consumer warps + 1 producer warp           */

@@ -274,7 +274,11 @@ extern "C" int fitrig_plan_query(int32_t H, int32_t W, int32_t L, const fitrig_p
   out->n_strips = (int32_t)((H + rows - 1) / rows);
   out->n_strip_buffers = out->n_strips >= 3 ? 3 : out->n_strips;
   out->strip_buffer_bytes = (int64_t)L * rows * W * 4;
-  plan_launch(cell, W, H, out->units, num_sms, read_tuning_env(), out);
+  const Tuning tn = read_tuning_env();
+  plan_launch(cell, W, H, out->units, num_sms, tn, out);
+  if (out->path == 1 && W % 4 != 0 && cell <= kFastTile && fused_tile(cell) && np.accumulate == 1 && !tn.force_generic &&
+      !tn.no_unaligned_fused && ((long long)L * H) % (4 / std::gcd(W, 4)) == 0)
+    plan_launch_fused(cell, W, H, out->units, num_sms, tn, 16, out);  // the super-row variant (kernels.cuh, UNAL)
   const int64_t n = (int64_t)np.batch * out->units * out->Ty * out->Tx;
   out->workspace_bytes = n * (16 + 4 + 4) + (int64_t)out->Ty * out->Tx * 8 + (1 << 20);
   return FITRIG_OK;

@@ -29,7 +29,8 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert (p.units, p.Ty, p.Tx) == (2, 1563, 1563)  # ceil(50000/32), R5
     assert p.path == 0 and p.strip_rows % 32 == 0 and p.n_strips * p.strip_rows >= 50000
     p = fitrig.plan_query(250, 250, 8, tile=8)
-    assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 1)  # W % 4 != 0 -> generic (time-marching, cp.async) kernel
+    # W % 4 != 0: rows off 16-byte boundaries ride the fused kernel through super rows of k = 2 image rows (8 * 250 rows: even)
+    assert (p.units, p.Ty, p.Tx, p.path) == (6, 32, 32, 0) and p.box_tiles <= 7
     p = fitrig.plan_query(250, 252, 8, tile=8)
     assert (p.Ty, p.Tx, p.path) == (32, 32, 0) and p.strip_rows % 32 == 0  # N_T = 8, 16 ride the fused kernel
     assert fitrig.plan_query(250, 252, 8, tile=16).path == 0
@@ -39,7 +40,10 @@ def test_plan_query_tile_grid_and_partial_tiles():
     assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (12, 24, 48, 100))
     assert all(fitrig.plan_query(250, 252, 8, tile=t).path == 0 for t in (1, 2, 4))  # tiles inside a lane's quads
     p = fitrig.plan_query(256, 250, 8)
-    assert p.path == 1  # W % 4 != 0: rows are not 16-byte aligned, no TMA
+    assert p.path == 0 and p.box_tiles <= 7  # W % 4 != 0: super rows; a TMA box holds at most 256 elements, 4 of them are slack
+    assert fitrig.plan_query(33, 251, 5).path == 1   # 5 * 33 rows are not a multiple of k = 4: the generic kernel
+    assert fitrig.plan_query(33, 251, 8).path == 0
+    assert fitrig.plan_query(256, 250, 8, tile=5).path == 1 and fitrig.plan_query(256, 250, 8, accumulate=2).path == 1
     p = fitrig.plan_query(256, 252, 8)
     assert p.path == 0 and p.Tx == 8
 
