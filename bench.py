@@ -40,7 +40,7 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback when 
 # `ncu --set full` capture summarised in profiles/ (None until a capture has been taken for this build)
 # (keyed to the build: `srchash` is paper_2509_21754_b200.build.source_hash() of the build the capture was taken on;
 # any other build prints "traffic": null)
-NCU_TRAFFIC = {"srchash": "d5c535d960771c774e0e08359a25d90bda26b0acba00eafa80db4331e37eba1a", "meerkat": 1091126660}  # profiles/r02_b_final.md
+NCU_TRAFFIC = {"srchash": "60f840c43223bf303ba14f7edb4fdf7ab4609e98d524d0953a7d80ff6646bb74", "meerkat": 1091270964}  # profiles/r02_b_final.md
 
 
 def parse_args():
