@@ -326,6 +326,41 @@ int fitrig_shard_import_eta(fitrig_ctx* ctx, const double* d_all /*device, [worl
 int fitrig_choose_accumulate(const float* d_stack, int32_t H, int32_t W, int32_t n_snapshots, float eps, int32_t g_max,
                              int32_t device, int32_t* g_out, double* contrast, int32_t* n_levels, void* cuda_stream);
 
+/* fitrig_choose_accumulate_static -- fitrig_choose_accumulate for callers that must not allocate device memory.
+ *
+ * Who that is: fitrig_choose_accumulate does two cudaMalloc and two cudaFree on every call.  cudaFree waits until
+ * everything queued on the device has drained and cudaMalloc can block for milliseconds behind the driver's locks, so
+ * inside the real-time loop (fitrig_push, Fig. 14) they would break the overlap of the next snapshot's copy with the
+ * current unit's kernels; and a process whose device memory already belongs to someone else's pool (a framework's
+ * caching allocator that has taken the whole card, a fixed per-process memory budget) may simply be refused the
+ * allocation.  This entry point calls no cudaMalloc, cudaFree, cudaHostAlloc or any other allocating
+ * routine: its scratch (the per-block partial sums of every level and the decision record) is a fixed device array
+ * compiled into the library.
+ *
+ * Arguments, rule, outputs and results are those of fitrig_choose_accumulate (same kernels, same grid, same summation
+ * order: the contrasts are bit-identical).  What differs:
+ *   - Size limit.  The scratch holds FITRIG_STATIC_ACCUM_MAX_PARTIALS partial sums (128 KB); a call needs
+ *     levels * min(ceil(H * W / 256), 8 * SM count) of them, levels = the admissible group sizes g = 1, 2, 4, .. (at
+ *     most 6).  On one B200 (148 SMs) the largest request is 6 * 1184 = 7104, so every image size fits there; a request
+ *     beyond the limit (a device with more SMs and many levels) is refused with FITRIG_ERR_INVALID_ARG and a message
+ *     that gives both numbers -- nothing is launched, nothing is truncated.
+ *   - Cost of the array.  Every CUDA device on which the library is loaded holds its own copy of it from load until
+ *     the process exits, whether or not this function is ever called.
+ *   - First call on a device.  It looks up where that device keeps the array (cudaGetSymbolAddress, which may make
+ *     the runtime load the library's kernels onto the device) and the device's SM count, and caches both.  Make that
+ *     first call at set-up time, before any stream capture is begun on the device; later calls do no such work.
+ *   - One array for everybody.  All calls on a device, from any thread and on any stream, use the same scratch, and
+ *     it keeps whatever the last call left in it.  The call clears the decision record itself before it launches (the
+ *     partial sums are all rewritten before they are read), so calls issued one after the other need no care; two
+ *     calls whose GPU work OVERLAPS (two host threads, each with its own stream) race on the array and may both return
+ *     wrong results.  Serialise them, or give all but one fitrig_choose_accumulate.
+ * Synchronises cuda_stream, like fitrig_choose_accumulate.  Errors: INVALID_ARG (as fitrig_choose_accumulate; the size
+ * limit; device ordinal >= 64), CUDA. */
+#define FITRIG_STATIC_ACCUM_MAX_PARTIALS 8192
+int fitrig_choose_accumulate_static(const float* d_stack, int32_t H, int32_t W, int32_t n_snapshots, float eps,
+                                    int32_t g_max, int32_t device, int32_t* g_out, double* contrast, int32_t* n_levels,
+                                    void* cuda_stream);
+
 /* fitrig_get_stats -- M (B floats) and the per-unit mean / population std of q = 1 - tLISI
  * (Eq. 8; mu_tLISI = 1 - mu_q; B * U doubles each, row b * U + u).  Frequency branch after fitrig_detect: entry
  * b * U of mu and sigma (unit 0 of stack b) describes eta of that stack (Eq. 11) instead.  Host outputs, each may

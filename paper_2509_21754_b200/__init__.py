@@ -5,5 +5,5 @@ path runs in the CUDA kernels of csrc/).  PyTorch is used by callers for device 
 """
 from .binding import (  # noqa: F401
     BRANCH_FREQUENCY, BRANCH_IMAGE, INTERP_BICUBIC, INTERP_BILINEAR, INTERP_MAKIMA, INTERP_SPLINE, REF_ABS, REF_FLOOR, REF_LITERAL, Candidate, Context, FitrigError, Plan,
-    choose_accumulate, exported_symbols, last_error, lib_path, load_library, plan_query, version,
+    choose_accumulate, choose_accumulate_static, exported_symbols, last_error, lib_path, load_library, plan_query, version,
 )

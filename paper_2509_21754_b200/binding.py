@@ -123,10 +123,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     L.fitrig_copy_count.argtypes = [vp, P(i64)]
     L.fitrig_probe_read_bandwidth.argtypes = [vp, vp, i64, i32, P(f32), vp]
     L.fitrig_choose_accumulate.argtypes = [vp, i32, i32, i32, f32, i32, i32, P(i32), vp, P(i32), vp]
+    L.fitrig_choose_accumulate_static.argtypes = [vp, i32, i32, i32, f32, i32, i32, P(i32), vp, P(i32), vp]
     for n in ("fitrig_plan_query", "fitrig_create", "fitrig_destroy", "fitrig_map_dims", "fitrig_tlisi",
               "fitrig_tlisi_batch", "fitrig_detect_batch", "fitrig_detect_launch", "fitrig_detect_fetch", "fitrig_shard_export_eta", "fitrig_shard_import_eta",
               "fitrig_detect", "fitrig_stream", "fitrig_push", "fitrig_push_reset", "fitrig_shard_export", "fitrig_shard_import", "fitrig_get_stats", "fitrig_get_map", "fitrig_get_raw",
-              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_localise", "fitrig_stream_timeline", "fitrig_probe_read_bandwidth", "fitrig_choose_accumulate"):
+              "fitrig_profile", "fitrig_last_timing", "fitrig_launch_count", "fitrig_copy_count", "fitrig_localise", "fitrig_stream_timeline", "fitrig_probe_read_bandwidth", "fitrig_choose_accumulate",
+              "fitrig_choose_accumulate_static"):
         getattr(L, n).restype = ctypes.c_int
     L.fitrig_last_error.restype = ctypes.c_char_p
     L.fitrig_version.restype = ctypes.c_char_p
@@ -190,6 +192,27 @@ def choose_accumulate(d_stack, eps: float, g_max: int = 32, stream=None):
     d = (ctypes.c_double * 6)()
     _check(L.fitrig_choose_accumulate(_dev_ptr(d_stack), H, W, n, float(eps), int(g_max), d_stack.device.index or 0,
                                       ctypes.byref(g), ctypes.cast(d, ctypes.c_void_p), ctypes.byref(nl), _stream_ptr(stream)))
+    return g.value, [d[i] for i in range(nl.value)]
+
+
+STATIC_ACCUM_MAX_PARTIALS = 8192  # FITRIG_STATIC_ACCUM_MAX_PARTIALS of include/fitrig.h
+
+
+def choose_accumulate_static(d_stack, eps: float, g_max: int = 32, stream=None):
+    """fitrig_choose_accumulate_static: `choose_accumulate` for callers that must not allocate device memory -- a
+    real-time loop whose copy / compute overlap a cudaMalloc or cudaFree would stall, or a process whose device memory
+    is already held by another allocator.  Same arguments and the same (bit-identical) result; the scratch is a fixed
+    array inside the library (room for STATIC_ACCUM_MAX_PARTIALS partial sums: every image size on one B200), shared by
+    all calls on the device, so calls whose GPU work overlaps race.  The first call on a device does a one-time
+    set-up; make it before any stream capture on that device."""
+    L = load_library()
+    if not (d_stack.is_cuda and d_stack.is_contiguous() and d_stack.dim() == 3 and d_stack.dtype.is_floating_point and d_stack.element_size() == 4):
+        raise ValueError("choose_accumulate_static: need a contiguous [L, H, W] fp32 CUDA tensor")
+    n, H, W = d_stack.shape
+    g, nl = ctypes.c_int32(), ctypes.c_int32()
+    d = (ctypes.c_double * 6)()
+    _check(L.fitrig_choose_accumulate_static(_dev_ptr(d_stack), H, W, n, float(eps), int(g_max), d_stack.device.index or 0,
+                                             ctypes.byref(g), ctypes.cast(d, ctypes.c_void_p), ctypes.byref(nl), _stream_ptr(stream)))
     return g.value, [d[i] for i in range(nl.value)]
 
 

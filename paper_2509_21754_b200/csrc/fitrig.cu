@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <numeric>
 #include <new>
 #include <vector>
@@ -1351,6 +1352,97 @@ extern "C" int fitrig_choose_accumulate(const float* d_stack, int32_t H, int32_t
   AccumChoice h;
   CUDA_TRY(cudaMemcpyAsync(&h, choice.p, sizeof(h), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  *g_out = h.g;
+  if (n_levels) *n_levels = h.n_levels;
+  if (contrast)
+    for (int i = 0; i < h.n_levels; ++i) contrast[i] = h.contrast[i];
+  return FITRIG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// fitrig_choose_accumulate_static -- the same rule for callers that must not allocate (see fitrig.h).  The block
+// partials and the decision record live in ONE file-scope device array instead of two cudaMalloc'ed buffers; the same
+// two kernels run on it with the same grid, so the contrasts come out bit-identical to fitrig_choose_accumulate's.
+//
+// g_static_accum below is, in host code, only a handle for the runtime: its host-side address is NOT where the GPU
+// keeps the array.  The launches therefore get the device address that cudaGetSymbolAddress returns, looked up once
+// per device (with that device current) and cached.  Every CUDA device that loads this library carries its own copy of
+// the array (sizeof(StaticAccumScratch), about 128 KB) until the process exits.
+// ---------------------------------------------------------------------------------------------
+static_assert(FITRIG_STATIC_ACCUM_MAX_PARTIALS >= kAccumLevels * 8 * 148, "one B200 with all six levels must fit");
+
+struct StaticAccumScratch {
+  AccumChoice choice;  // decision record, cleared at the start of every call
+  unsigned char pad[256 - sizeof(AccumChoice)];
+  double2 partials[FITRIG_STATIC_ACCUM_MAX_PARTIALS];  // [level][block]; every entry a call reads, that call wrote first
+};
+static __device__ __align__(256) StaticAccumScratch g_static_accum;
+
+static const int kStaticAccumMaxDevices = 64;
+struct StaticAccumDevice {
+  StaticAccumScratch* scratch;  // DEVICE address of g_static_accum on this device; NULL until the set-up has run
+  int num_sms;
+};
+static StaticAccumDevice g_static_accum_dev[kStaticAccumMaxDevices];
+static std::mutex g_static_accum_mu;
+
+// Once per device, with `device` current: which GPU this is and where its copy of the array lives.
+static int static_accum_setup(int device, StaticAccumDevice* out) {
+  std::lock_guard<std::mutex> lock(g_static_accum_mu);
+  StaticAccumDevice& d = g_static_accum_dev[device];
+  if (!d.scratch) {
+    int major = 0, sms = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+    if (major < 10) return fail(FITRIG_ERR_CUDA, "fitrig_choose_accumulate_static: this library is built for sm_100a (B200) only");
+    void* addr = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&addr, g_static_accum));
+    if (!addr) return fail(FITRIG_ERR_CUDA, "fitrig_choose_accumulate_static: cudaGetSymbolAddress returned no address on device %d", device);
+    d.num_sms = sms;
+    d.scratch = static_cast<StaticAccumScratch*>(addr);
+  }
+  *out = d;
+  return FITRIG_OK;
+}
+
+extern "C" int fitrig_choose_accumulate_static(const float* d_stack, int32_t H, int32_t W, int32_t L, float eps, int32_t g_max,
+                                               int32_t device, int32_t* g_out, double* contrast, int32_t* n_levels,
+                                               void* cuda_stream) {
+  if (!d_stack || !g_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate_static: NULL argument");
+  if (H < 1 || W < 1 || L < 3 || g_max < 1 || device < 0 || !(eps == eps))
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate_static: need H, W >= 1, n_snapshots >= 3 (PAPER.md:155), g_max >= 1, a threshold");
+  int ndev = 0;
+  CUDA_TRY(cudaGetDeviceCount(&ndev));
+  if (device >= ndev || device >= kStaticAccumMaxDevices)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_choose_accumulate_static: device %d of %d (at most %d)", device, ndev, kStaticAccumMaxDevices);
+  CUDA_TRY(cudaSetDevice(device));
+  StaticAccumDevice dev;
+  if (int rc = static_accum_setup(device, &dev)) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int levels = 0;
+  for (int g = 1; levels < kAccumLevels && g <= g_max && L / g >= 3; g *= 2) ++levels;  // admissible group sizes (R30)
+  const long long hw = (long long)H * W;
+  const int nblocks = (int)std::min<long long>((hw + 255) / 256, 8ll * dev.num_sms);  // as fitrig_choose_accumulate
+  if ((long long)levels * nblocks > FITRIG_STATIC_ACCUM_MAX_PARTIALS)
+    return fail(FITRIG_ERR_INVALID_ARG,
+                "fitrig_choose_accumulate_static: %d levels x %d blocks = %lld partial sums, the static scratch holds %d "
+                "(lower g_max, or use fitrig_choose_accumulate, which allocates what it needs)",
+                levels, nblocks, (long long)levels * nblocks, FITRIG_STATIC_ACCUM_MAX_PARTIALS);
+  // The array still holds what the previous call left.  The partials need no clearing (each level's kernel writes all
+  // `nblocks` entries that the decision kernel then reads); the decision record is cleared so that nothing of an
+  // earlier call can be read back as this call's answer.
+  CUDA_TRY(cudaMemsetAsync(&dev.scratch->choice, 0, 256, st));
+  for (int lv = 0; lv < levels; ++lv) {
+    accum_contrast_kernel<<<nblocks, 256, 0, st>>>(d_stack, hw, L, 1 << lv, dev.scratch->partials + (size_t)lv * nblocks);
+    CUDA_TRY(cudaGetLastError());
+  }
+  accum_choose_kernel<<<1, 256, 0, st>>>(dev.scratch->partials, nblocks, levels, L, hw, eps, &dev.scratch->choice);
+  CUDA_TRY(cudaGetLastError());
+  AccumChoice h;
+  CUDA_TRY(cudaMemcpyAsync(&h, &dev.scratch->choice, sizeof(h), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (h.n_levels < 1 || h.n_levels > levels)
+    return fail(FITRIG_ERR_CUDA, "fitrig_choose_accumulate_static: no decision came back (did another call use the scratch at the same time?)");
   *g_out = h.g;
   if (n_levels) *n_levels = h.n_levels;
   if (contrast)
