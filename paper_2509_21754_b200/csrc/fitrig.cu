@@ -471,7 +471,10 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   const bool cells = c->geo.m > 1;     // records go to raw_blocks and are merged into windows before the finalise
   const int out_Ty = cells ? c->Cy : c->Ty, out_Tx = cells ? c->Cx : c->Tx;
   const long long first_row = (long long)opt.stack * c->U + opt.row0;
-  RawTile* const out_raw = (cells ? c->raw_blocks : c->raw) + first_row * out_Ty * out_Tx;
+  // (cells of one pixel are 8-byte RawPix records, which the kernels index from this base: the offset is in records of that size)
+  const size_t rec_bytes = c->cell_pix8 ? sizeof(RawPix) : sizeof(RawTile);
+  RawTile* const out_raw = reinterpret_cast<RawTile*>(reinterpret_cast<unsigned char*>(cells ? c->raw_blocks : c->raw) +
+                                                      (size_t)(first_row * out_Ty * out_Tx) * rec_bytes);
   const int units = opt.units ? opt.units : c->U;
   unsigned* key = opt.key ? opt.key : c->gmax_key + c->key_idx * c->B + opt.stack;
   const int nslots = opt.zmod ? opt.zmod : c->L;

@@ -425,8 +425,11 @@ __global__ void __launch_bounds__(32 * (kMaxTilesPerBox + 1), 1)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-  pdl_launch_dependents();  // the next kernel of the chain may take its place on the SMs as they fall free
+  // The first kernel of a call waits for everything ahead of it (the previous call's finalise still reads the records
+  // and resets the maximum keys) BEFORE it lets its successors in: a stack b >= 1 of a batch (dep == 2) does not wait at
+  // its start, so it may only become schedulable once this grid has seen the previous call complete.
   if (p.dep == 1) pdl_wait();
+  pdl_launch_dependents();  // the next kernel of the chain may take its place on the SMs as they fall free
 
   // this CTA's range of (group, unit) pairs
   const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
@@ -1065,8 +1068,8 @@ __global__ void __launch_bounds__(32 * kMarchMaxWarps, 1)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
+  if (p.dep == 1) pdl_wait();  // (before the trigger: see tlisi_fused_kernel)
   pdl_launch_dependents();
-  if (p.dep == 1) pdl_wait();
   const int g_begin = (int)((long long)blockIdx.x * p.G / gridDim.x);
   const int g_end = (int)((long long)(blockIdx.x + 1) * p.G / gridDim.x);
   const uint32_t full_addr = smem_u32(full), empty_addr = smem_u32(empty), ring_addr = smem_u32(smem);

@@ -217,7 +217,7 @@ def test_config5_sixteen_channel_batch_reduced_size():
             _check_frequency(g, ref, (tau,), 32)
 
 
-@pytest.mark.parametrize("tile,B", [(32, 3), (16, 2), (5, 2), (64, 2)])
+@pytest.mark.parametrize("tile,B", [(32, 3), (16, 2), (5, 2), (64, 2), (1, 3), (2, 2), (4, 2)])
 def test_image_branch_batch_equals_single_stacks(tile, B):
     stacks = [synth.gaussian_noise_stack(6, 200, 168, seed=40 + b, device=DEV) for b in range(B)]
     for b, s in enumerate(stacks):
@@ -242,6 +242,68 @@ def test_image_branch_batch_equals_single_stacks(tile, B):
     with pytest.raises(fitrig.FitrigError) as e:
         fitrig.Context(64, 64, 4, batch=2, row_offset=32)
     assert e.value.code == fitrig.binding.ERR_INVALID_ARG
+
+
+@pytest.mark.parametrize("tile,H,W", [(32, 64, 96), (8, 40, 64), (5, 40, 50)])
+def test_back_to_back_batch_calls_without_detect(tile, H, W):
+    """A caller that only consumes d_tlisi: call after call on a batch context, nothing in between.  The kernels of
+    stacks b >= 1 do not wait at their start, so they must not become schedulable before the previous call's finalise
+    (which still reads the records and resets the maximum keys) has completed.  Small images, so that the grids of
+    consecutive kernels fit on the device together."""
+    B, L = 3, 5
+    first = [synth.gaussian_noise_stack(L, H, W, seed=60 + b, device=DEV) for b in range(B)]
+    second = [(2.0 + b) * synth.gaussian_noise_stack(L, H, W, seed=70 + b, device=DEV) for b in range(B)]  # other maxima
+    for b in range(B):
+        second[b][1, 3 + b, 7] += 90.0 + 10.0 * b
+    exp = []
+    for stacks in (first, second):
+        runs = [gpu_run(s, taus=(3.0,), tile=tile) for s in stacks]
+        exp.append((torch.from_numpy(np.stack([r["tlisi"] for r in runs])).to(DEV), np.array([r["M"] for r in runs])))
+    assert not np.array_equal(exp[0][1], exp[1][1])
+    with fitrig.Context(H, W, L, tile=tile, batch=B) as ctx:
+        U, Ty, Tx = ctx.map_dims()
+        outs = [torch.empty((B, U, Ty, Tx), dtype=torch.float32, device=DEV) for _ in range(2)]
+        for it in range(25):
+            outs[0].fill_(-1.0)
+            outs[1].fill_(-1.0)
+            ctx.tlisi_batch(first, outs[0])
+            ctx.tlisi_batch(second, outs[1])
+            if it % 2:  # and a third call straight behind the second
+                ctx.tlisi_batch(first, outs[0])
+            torch.cuda.synchronize()
+            assert torch.equal(outs[0], exp[0][0]) and torch.equal(outs[1], exp[1][0]), it
+            M, _, _ = ctx.get_stats()
+            assert np.array_equal(M, exp[it % 2 == 0][1]), it
+
+
+@pytest.mark.parametrize("tile", [1, 2])
+def test_frequency_branch_batch_of_pixel_tiles_equals_single_stacks(tile):
+    # per-pixel detection (PAPER.md:431) keeps 8-byte records: stacks b >= 1 of a batch must land at their own rows
+    B, L, H, W, tau = 3, 10, 72, 88, 3.0
+    cfg = synth.scaled(synth.CONFIGS["imgfreq"], H, W, L=L).replace(n_transients=2, transient_peak=14.0, period=4)
+    stacks = [synth.make_stack(cfg, device=DEV, channel=ch)[0] for ch in range(B)]
+    with fitrig.Context(H, W, L, tile=tile, branch=fitrig.BRANCH_FREQUENCY, batch=B) as ctx:
+        ctx.tlisi_batch(stacks)
+        cands, n, per = ctx.detect_batch(tau)
+        q, eta, ks = ctx.get_map(0), ctx.get_map(2), ctx.get_map(3).astype(np.int32)
+        M, mu, sd = ctx.get_stats()
+    off = np.concatenate([[0], np.cumsum(per)])
+    for b in range(B):
+        one = gpu_run(stacks[b], taus=(tau,), tile=tile, branch=fitrig.BRANCH_FREQUENCY)
+        assert np.array_equal(q[b], one["q"]) and np.array_equal(eta[b], one["eta"]) and np.array_equal(ks[b], one["kstar"])
+        assert M[b] == one["M"] and mu[b, 0] == one["mu"][0] and sd[b, 0] == one["sigma"][0]
+        assert np.array_equal(cands[off[b]:off[b + 1]], one["cands"][tau][0])
+    # the last stack against the oracle: q within 1e-4 + the derived fp32 input-rounding bound of tiles of a few pixels
+    # (util.fp32_slack, as in check_against_oracle), eta within what that moves a DFT magnitude by (util.eta_bound's argument)
+    snaps = stacks[B - 1].cpu().numpy()
+    ref = oracle.run(snaps, tile=tile, tau=tau, branch=1)
+    res = ref.res
+    eS, eM, eR = util.fp32_slack(snaps, tile)
+    prod = res.sumD * res.maxD * res.sumR
+    slack = ((res.sumD + eS) * (res.maxD + eM) * (np.abs(res.sumR) + eR) - prod) * np.abs(res.q / np.where(prod == 0, 1.0, prod))
+    util.assert_map_close(q[B - 1], res.q, slack=slack)
+    bound = 2.0 * (util.Q_RTOL * np.abs(res.q) + slack).sum(axis=0)
+    assert np.all(np.abs(eta[B - 1] - ref.eta) <= bound + 2e-7 * np.abs(ref.eta))
 
 
 # ------------------------------------------------------------------------------------------
@@ -293,6 +355,46 @@ def test_push_frequency_branch_matches_oracle(H, W, tile, window, harmonics):
         for snap in host + [None]:
             u, c, n = ctx.push(snap, tau)
         assert np.array_equal(c, last[0]) and np.array_equal(ctx.get_map(2), last[1])
+
+
+@pytest.mark.parametrize("tile", [1, 2, 4])
+def test_push_frequency_branch_small_tiles_fill_their_own_ring_rows(tile):
+    """Tiles of one pixel keep 8-byte records: ring row n mod U of the cube must land where the finalise, the spectrum
+    and the getters read it.  The cube after the last push is the map of the last window of snapshots under the running
+    maximum, so it is compared bit for bit with a resident run on those snapshots with M_override = that maximum."""
+    H, W, window, L, tau = 40, 48, 6, 12, 2.0
+    cfg = synth.scaled(synth.CONFIGS["imgfreq"], H, W, L=L).replace(n_transients=2, transient_peak=14.0, period=4)
+    st, _ = synth.make_stack(cfg, device=DEV)
+    st[3, 7, 9] = 300.0  # the running maximum comes from a snapshot that has left the window
+    Uw = window - 2
+    host = [st[s].cpu().pin_memory() for s in range(L)]
+    with fitrig.Context(H, W, window, tile=tile, branch=fitrig.BRANCH_FREQUENCY) as ctx:
+        for snap in host + [None]:
+            u, c, n = ctx.push(snap, tau)
+        M, mu, sd = ctx.get_stats()
+        cube, eta, ks = ctx.get_map(0), ctx.get_map(2), ctx.get_map(3).astype(np.int32)
+        c = c.copy()
+    assert u == L - 3 and M == np.float32(300.0)
+    order = [(u - Uw + 1 + j) % Uw for j in range(Uw)]
+    one = gpu_run(st[L - window:].contiguous(), taus=(tau,), tile=tile, branch=fitrig.BRANCH_FREQUENCY, M_override=300.0)
+    assert np.array_equal(cube[order], one["q"])
+    # |F_k| does not depend on where the ring starts, up to the rounding of the fp64 sums (and one fp32 rounding of eta)
+    np.testing.assert_allclose(eta, one["eta"], rtol=1e-6, atol=0)
+    ref = oracle.run(st[L - window:].cpu().numpy(), tile=tile, tau=tau, branch=1, M=300.0)
+    slack = None
+    if util.needs_slack(H, W, tile):  # the derived fp32 input-rounding bound, as in check_against_oracle
+        res = ref.res
+        eS, eM, eR = util.fp32_slack(st[L - window:].cpu().numpy(), tile)
+        prod = res.sumD * res.maxD * res.sumR
+        slack = ((res.sumD + eS) * (res.maxD + eM) * (np.abs(res.sumR) + eR) - prod) * np.abs(res.q / np.where(prod == 0, 1.0, prod))
+    util.assert_map_close(cube[order], ref.res.q, slack=slack)
+    sure = np.abs(one["eta"] - (one["mu"][0] + tau * one["sigma"][0])) > 1e-5 * np.abs(one["eta"])  # away from the threshold
+    got = {(int(k["x"]), int(k["y"])) for k in c}
+    exp = {(int(k["x"]), int(k["y"])) for k in one["cands"][tau][0]}
+    Tx = one["dims"][2]
+    for (x, y) in got ^ exp:
+        assert not sure[y // tile, x // tile]
+    assert len(got & exp) > 0
 
 
 # ------------------------------------------------------------------------------------------
