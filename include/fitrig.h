@@ -42,6 +42,10 @@
  *       FITRIG_MARCH_BOX_KB=n    generic kernel: boxes of about n KB (default 32)
  *       FITRIG_NO_UNALIGNED_FUSED=1  images whose rows do not start on 16-byte boundaries: the generic kernel even where
  *                                the fused kernel's super-row variant applies (cells of 1, 2, 4, 8, 16, 32 pixels)
+ *       FITRIG_TEST_FAIL_UNALIGNED_ENCODE=1  behave as if the driver had refused the tensor map of the super-row variant
+ *                                (whose rows overlap: accepted by the driver this was built on, not promised by any
+ *                                document); the library then takes the generic kernel for that call, as it does when a
+ *                                driver really refuses
  */
 #ifndef FITRIG_H_
 #define FITRIG_H_
@@ -163,7 +167,10 @@ int fitrig_destroy(fitrig_ctx* ctx);
 int fitrig_map_dims(const fitrig_ctx* ctx, int32_t* units, int32_t* Ty, int32_t* Tx);
 
 /* fitrig_tlisi -- the tLISI map of a device-resident stack (Eq. 2-6; steps a1-a7 of DESIGN.md).
- *   d_stack (device)  [L][H][W] fp32, contiguous; owned by the caller, read once, never written.
+ *   d_stack (device)  [L][H][W] fp32, contiguous; owned by the caller, read once, never written.  4-byte alignment is
+ *                     enough; when d_stack is not 16-byte aligned the fused kernel's loads start at the 16-byte boundary
+ *                     below it, i.e. up to 12 bytes BEFORE d_stack are read (and ignored): they must be readable, which
+ *                     they are whenever d_stack points into a larger allocation (the only way to get such a pointer).
  *   d_tlisi (device)  [U][Ty][Tx] fp32 tLISI = 1 - q; may be NULL.  Owned by the caller.
  * The context keeps q = 1 - tLISI in fp32 (its complement carries the signal, R21), the per-tile
  * raw sums, the global M and per-unit mean / population std of q (Eq. 8, R3); this
@@ -258,8 +265,8 @@ int fitrig_stream(fitrig_ctx* ctx, const float* const* h_snapshots, float* h_tli
  * the last unit.  After a call with unit >= 0 the context's current map is that unit's (getters work).
  * The copy is asynchronous: a pushed buffer must stay valid and unchanged until the NEXT fitrig_push that
  * returns a unit >= 0 has returned (or until fitrig_push_reset).  Synchronises `cuda_stream` when a unit
- * is computed.  Errors: INVALID_ARG (image branch without n_snapshots = 3; accumulation; batch; tiles of 64, 96 ..),
- * NOMEM, CUDA, CAPACITY.
+ * is computed.  Errors: INVALID_ARG (image branch without n_snapshots = 3; accumulation; batch; overlapping windows),
+ * NOMEM, CUDA, CAPACITY.  (Every tile size works, tiles of 64, 96 .. pixels included: they are merged from 32-pixel cells.)
  *
  * fitrig_push_reset -- forget all pushed snapshots and the running maximum (synchronises the device). */
 int fitrig_push(fitrig_ctx* ctx, const float* snapshot, float sigma_threshold, float* d_tlisi,

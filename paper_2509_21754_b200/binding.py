@@ -250,6 +250,7 @@ class Context:
         self.branch = int(params.get("branch", BRANCH_IMAGE))
         self.tile = int(params.get("tile", 0)) or 32
         self.batch = int(params.get("batch", 0)) or 1
+        self._launch_caps: List[int] = []  # capacities of the detect_launch calls that have not been fetched yet
 
     def map_dims(self) -> Tuple[int, int, int]:
         return self.units, self.Ty, self.Tx
@@ -304,14 +305,21 @@ class Context:
     def detect_launch(self, sigma_threshold: float, capacity: int = 1 << 16, stream=None) -> None:
         """Enqueue the detection of the current map (at most two may be in flight); see detect_fetch."""
         _check(self._L.fitrig_detect_launch(self._h, float(sigma_threshold), int(capacity), _stream_ptr(stream)))
+        self._launch_caps.append(int(capacity))  # the library copies up to this many records into detect_fetch's array
 
     def detect_fetch(self, out: np.ndarray):
         """Wait for the oldest unfetched detect_launch and return (candidates, n_found, per-stack totals); `out` must
-        hold the capacity given to that launch."""
+        hold the capacity given to that launch (checked here: the library would write past a shorter array)."""
+        cap = self._launch_caps[0] if self._launch_caps else 0
+        if out.dtype != CANDIDATE_DTYPE or not out.flags["C_CONTIGUOUS"] or len(out) < cap:
+            raise ValueError(f"detect_fetch: need a contiguous candidate array of at least {cap} records (the capacity of the launch)")
         n = ctypes.c_int64(0)
         per = np.zeros(self.batch, dtype=np.int64)
-        _check(self._L.fitrig_detect_fetch(self._h, out.ctypes.data, ctypes.byref(n), per.ctypes.data), allow=(ERR_CAPACITY,))
-        return out[: min(n.value, len(out))], n.value, per
+        rc = self._L.fitrig_detect_fetch(self._h, out.ctypes.data, ctypes.byref(n), per.ctypes.data)
+        if self._launch_caps and rc in (OK, ERR_CAPACITY):
+            self._launch_caps.pop(0)
+        _check(rc, allow=(ERR_CAPACITY,))
+        return out[: min(n.value, cap)], n.value, per
 
     def stream(self, h_snapshots: Sequence, h_tlisi=None, stream=None) -> None:
         """h_snapshots: L host tensors/arrays of [H, W] fp32 (pinned for overlap)."""

@@ -485,6 +485,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   // through a tensor map of "super rows" of k image rows (kernels.cuh, UNAL); everything else takes the generic kernel.
   bool unal = false;
   int unal_k = 1;
+  CUtensorMap tm_unal;
   const int unal_a = (int)(((uintptr_t)base >> 2) & 3);
   if (!aligned && tile <= kFastTile && fused_tile(tile) && c->prm.accumulate == 1 && !c->tune.force_generic && !c->tune.no_unaligned_fused &&
       (uintptr_t)base % 4 == 0 && snap_stride % c->W == 0 && snap_stride / c->W >= rows && r0 % kFastTile == 0) {
@@ -496,6 +497,21 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
     if (unal) {
       Tuning tn = c->tune;
       plan_launch_fused(tile, c->W, rows, units, c->num_sms, tn, /*extra_row_bytes=*/16, &pl);
+      // super rows of k image rows, from the 16-byte boundary at or below the base.  Rows of this map overlap (dim0 exceeds
+      // the row stride), which the B200's driver accepts; a driver that refuses it sends the image to the generic kernel
+      const cuuint64_t gdim[2] = {(cuuint64_t)unal_k * c->W + unal_a, (cuuint64_t)(nslots * (snap_stride / c->W) / unal_k)};
+      const cuuint64_t gstr[1] = {(cuuint64_t)unal_k * c->W * 4};
+      const cuuint32_t bx[2] = {(cuuint32_t)(pl.box_tiles * kFastTile + 4), (cuuint32_t)(kFastTile / unal_k)};
+      const cuuint32_t estr[2] = {1, 1};
+      CUresult r = c->tune.fail_unaligned_encode
+                       ? CUDA_ERROR_INVALID_VALUE
+                       : c->encode(&tm_unal, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)(base - unal_a), gdim, gstr, bx, estr,
+                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) {
+        unal = false;
+        pl = c->plan;
+      }
     }
   }
   if (pl.path == 0 && !aligned && !unal) pl.path = 1;  // TMA needs 16-byte aligned base and strides
@@ -514,17 +530,7 @@ static int launch_tlisi_rows(fitrig_ctx* c, const float* base, long long snap_st
   if (rc) return rc;
   if (pl.path == 0) {
     const CUtensorMap* tmp = nullptr;
-    CUtensorMap tm_unal;
     if (unal) {
-      // super rows of k image rows, from the 16-byte boundary at or below the base
-      const cuuint64_t gdim[2] = {(cuuint64_t)unal_k * c->W + unal_a, (cuuint64_t)(nslots * (snap_stride / c->W) / unal_k)};
-      const cuuint64_t gstr[1] = {(cuuint64_t)unal_k * c->W * 4};
-      const cuuint32_t bx[2] = {(cuuint32_t)(pl.box_tiles * kFastTile + 4), (cuuint32_t)(kFastTile / unal_k)};
-      const cuuint32_t estr[2] = {1, 1};
-      CUresult r = c->encode(&tm_unal, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)(base - unal_a), gdim, gstr, bx, estr,
-                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-      if (r != CUDA_SUCCESS) return fail(FITRIG_ERR_CUDA, "cuTensorMapEncodeTiled (super rows) failed (CUresult %d)", (int)r);
       tmp = &tm_unal;
     } else {
       rc = get_tmap(c, base, snap_stride, rows, nslots, pl.box_tiles * kFastTile, kFastTile, &tmp);
@@ -931,14 +937,15 @@ static int detect_fetch_core(fitrig_ctx* c, fitrig_candidate* h_out, int64_t* n_
   if (c->detect_launched == c->detect_fetched) return fail(FITRIG_ERR_STATE, "fitrig_detect_fetch: nothing was launched");
   CUDA_TRY(cudaSetDevice(c->prm.device));
   DetectSlot& d = c->slot[c->detect_fetched & 1];
-  c->detect_fetched++;
-  d.pending = false;
   // the kernel has written the count and the first kHostStageCands candidates straight into mapped pinned memory
   // (no copy in the stream); a copy from the device list only for longer lists
   CUDA_TRY(cudaEventSynchronize(d.done));
   const long long total = (long long)reinterpret_cast<CandHeader*>(d.cand_host)->total;
   const long long nwrite = std::min<long long>(total, d.cap);
-  if (nwrite > 0 && !h_out) return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_fetch: h_out is NULL");
+  if (nwrite > 0 && !h_out)  // (the launch stays unfetched: a call with a proper buffer still gets its result)
+    return fail(FITRIG_ERR_INVALID_ARG, "fitrig_detect_fetch: h_out is NULL and there are %lld candidates to deliver", nwrite);
+  c->detect_fetched++;  // from here on the result counts as delivered and the slot is free for the next launch
+  d.pending = false;
   const long long n1 = std::min(nwrite, d.host_cap);
   if (n1 > 0) memcpy(h_out, d.cand_host + sizeof(CandHeader), sizeof(fitrig_candidate) * n1);
   if (nwrite > n1) {  // (a later launch writes the other slot's list: this one is still intact)

@@ -29,6 +29,7 @@ Tuning read_tuning_env() {
   t.march_prod = env_int("FITRIG_MARCH_PROD", 0);
   t.march_box_kb = env_int("FITRIG_MARCH_BOX_KB", 0);
   t.no_unaligned_fused = env_int("FITRIG_NO_UNALIGNED_FUSED", 0);
+  t.fail_unaligned_encode = env_int("FITRIG_TEST_FAIL_UNALIGNED_ENCODE", 0);
   return t;
 }
 

@@ -46,6 +46,7 @@ struct Tuning {
   int march_prod;       // FITRIG_MARCH_PROD     generic time-marching kernel, cp.async variant: producer warps per CTA
   int march_box_kb;     // FITRIG_MARCH_BOX_KB   generic time-marching kernel: target size of a box in KB
   int no_unaligned_fused;  // FITRIG_NO_UNALIGNED_FUSED  unaligned rows: the generic kernel instead of the fused kernel's super-row variant
+  int fail_unaligned_encode;  // FITRIG_TEST_FAIL_UNALIGNED_ENCODE  behave as if the driver refused the super-row tensor map (tests the fallback)
 };
 Tuning read_tuning_env();
 

@@ -587,7 +587,7 @@ def _push_all(ctx, snaps, tau, want_maps=True):
 
 @pytest.mark.parametrize("H,W,tile,on_device", [(256, 256, 32, False), (250, 252, 32, False), (256, 256, 32, True),
                                                 (120, 100, 8, False), (250, 252, 16, False), (120, 102, 8, False),
-                                                (120, 100, 4, False)])
+                                                (120, 100, 4, False), (256, 256, 64, False)])  # 64: merged from 32-pixel cells
 def test_push_realtime_matches_oracle(tiny, H, W, tile, on_device):
     st, _ = tiny
     st = st[:, :H, :W].contiguous()

@@ -2,6 +2,8 @@
 ("parity-test holes"), and the calls added in round 2.  Same rules as test_parity_gpu.py:
 through the C ABI, against the CPU fp64 oracle on the same seeded buffers, tolerances of DESIGN.md section 3.
 """
+import ctypes
+
 import numpy as np
 import pytest
 import torch
@@ -185,6 +187,16 @@ def test_detect_launch_fetch_pipeline_and_state_errors():
         ctx.detect_launch(tau, capacity=10)
         cs, ns, _ = ctx.detect_fetch(small)  # FITRIG_ERR_CAPACITY is reported through n_found
         assert ns == nb and np.array_equal(cs, cb[:10])
+        # an array shorter than the launch's capacity is refused before the library could write past its end, and a
+        # fetch without a buffer fails WITHOUT consuming the launch: the next fetch still delivers it
+        ctx.detect_launch(tau, cap)
+        with pytest.raises(ValueError):
+            ctx.detect_fetch(small)
+        n = ctypes.c_int64(0)
+        rc = ctx._L.fitrig_detect_fetch(ctx._h, None, ctypes.byref(n), None)
+        assert rc == fitrig.binding.ERR_INVALID_ARG and "h_out is NULL" in fitrig.last_error()
+        c4, n4, _ = ctx.detect_fetch(outs[0])
+        assert n4 == nb and np.array_equal(c4, cb)
 
 
 # ------------------------------------------------------------------------------------------

@@ -201,6 +201,24 @@ def test_rows_off_16_byte_boundaries_fused_and_generic_kernels_agree(monkeypatch
     assert np.array_equal(a["raw"][3], b["raw"][3]) and np.array_equal(a["raw"][4], b["raw"][4])  # arg-max pixels
 
 
+def test_driver_refusing_the_super_row_tensor_map_falls_back_to_the_generic_kernel(monkeypatch):
+    """The super-row tensor map has overlapping rows; if a driver refuses to encode it, the call must still succeed on
+    the generic kernel (same result as FITRIG_NO_UNALIGNED_FUSED), not return FITRIG_ERR_CUDA."""
+    H, W, L = 200, 254, 8
+    st = _stack(H, W, L)
+    monkeypatch.setenv("FITRIG_NO_UNALIGNED_FUSED", "1")
+    b = gpu_run(st, taus=(3.0,))
+    monkeypatch.delenv("FITRIG_NO_UNALIGNED_FUSED")
+    monkeypatch.setenv("FITRIG_TEST_FAIL_UNALIGNED_ENCODE", "1")
+    a = gpu_run(st, taus=(3.0,))
+    s = gpu_run(st, taus=(3.0,), use_stream=True, strip_rows=64)
+    monkeypatch.delenv("FITRIG_TEST_FAIL_UNALIGNED_ENCODE")
+    for g in (a, s):
+        assert np.array_equal(g["q"], b["q"]) and g["M"] == b["M"] and np.array_equal(g["cands"][3.0][0], b["cands"][3.0][0])
+    ref = oracle_run(st, tile=32, tau=3.0)
+    check_against_oracle(st, a, ref, (3.0,), 32)
+
+
 def test_rows_off_16_byte_boundaries_push():
     H, W, L, tau = 96, 250, 7, 3.0
     st = _stack(H, W, L)
