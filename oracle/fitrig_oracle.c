@@ -11,7 +11,7 @@
  * concession to run time is an OpenMP "parallel for" over independent (unit, tile-row)
  * pairs, which the paper itself states are independent.
  *
- * Citations are /root/reference/PAPER.md line numbers (+ equation).  Readings R1..R28
+ * Citations are /root/reference/PAPER.md line numbers (+ equation).  Readings R1..R30
  * of silent / ambiguous passages are SURVEY.md section 8(c), restated in DESIGN.md.
  *
  * Notation (0-based): snapshots x_0..x_{L-1}, each H x W row-major fp32.

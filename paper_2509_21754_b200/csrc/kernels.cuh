@@ -13,7 +13,6 @@
 //
 // Citations: PAPER.md line numbers; R<n> = readings in DESIGN.md.
 #pragma once
-#include <cooperative_groups.h>
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -22,7 +21,6 @@
 #include "plan.h"
 
 namespace fitrig {
-namespace cg = cooperative_groups;
 
 // Per-tile, per-unit partial results of Eq. 6: sum Delta, max Delta, sum r, and the
 // tile-relative position (row * N_T + col) of the first max-Delta pixel (R20).  16 bytes.
