@@ -27,3 +27,19 @@ def test_reference_arm_other_ranks_exit_quietly():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "tiny",
                         "--steps", "1", "--warmup", "1", "--gpus", "2"], capture_output=True, text=True, env=env, cwd=ROOT)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_default_workload_is_the_largest_single_gpu_config_and_a_failing_child_is_recorded():
+    """BASELINE.json's metric names no config: plain `python bench.py` measures configs[3] (50K x 50K) and embeds the
+    other configs; a child that cannot run (no GPU here) becomes an "error" record instead of ending the run."""
+    import argparse
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.DEFAULT_WORKLOAD == "stream50k" and set(bench.OTHER_CONFIGS) == {"meerkat", "ska_aa2", "imgfreq"}
+    import synth
+    assert (synth.CONFIGS["stream50k"].H, synth.CONFIGS["stream50k"].L, synth.CONFIGS["stream50k"].cfg_index) == (50000, 4, 4)
+    import torch
+    if not torch.cuda.is_available():
+        rec = bench.sub_record(argparse.Namespace(steps=1, warmup=1), "tiny")
+        assert set(rec) == {"error", "command"} and "--workload tiny" in rec["command"]
+    assert isinstance(bench.cpu_model(), str) and bench.cpu_model()
