@@ -50,7 +50,7 @@ CPU_SAMPLE_MAX_ROWS = 16384  # the oracle legs look at no more than this many im
 # `ncu --set full` capture summarised in profiles/ (None until a capture has been taken for this build)
 # (keyed to the build: `srchash` is paper_2509_21754_b200.build.source_hash() of the build the capture was taken on;
 # any other build prints "traffic": null)
-NCU_TRAFFIC = {"srchash": "60f840c43223bf303ba14f7edb4fdf7ab4609e98d524d0953a7d80ff6646bb74", "meerkat": 1091270964}  # profiles/r02_b_final.md
+NCU_TRAFFIC = {"srchash": "212816b41d21bdc36f28b11a590cf5e9c50cafc2580eec2b89eefbbb4186267c", "stream50k": 40110947848, "meerkat": 1090717752}  # profiles/r03_b_ncu.md
 
 
 def parse_args():

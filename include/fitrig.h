@@ -24,6 +24,11 @@
  *     then describes it.  No exceptions, no abort, nothing printed.
  *   - There is NO CPU fallback: without a CUDA device every compute call fails with
  *     FITRIG_ERR_CUDA.
+ *   - Threads: a context is NOT thread-safe -- it owns one set of workspaces, one current map and two result slots, so
+ *     calls on the same context must not overlap (serialise them, or give every thread its own context).  Different
+ *     contexts may be used from different threads at the same time, on the same or on different devices; the
+ *     library's only shared state is set-up work done once per device under a lock, and fitrig_last_error() is
+ *     thread-local.  fitrig_choose_accumulate_static is the exception noted at its declaration (one scratch per device).
  *   - Pointers are marked (device) or (host).  Nothing here is a torch type; a CUDA stream is
  *     passed as void* (cudaStream_t; NULL = the legacy default stream).
  *   - Environment: the library reads these integer DEBUG / TUNING switches, once per fitrig_create (and once per

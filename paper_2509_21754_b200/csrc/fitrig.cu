@@ -219,6 +219,29 @@ static cudaError_t set_fused_attr() {
   return set_fused_attr_one<REF, true, 1>();
 }
 
+// The dynamic shared-memory limit of every tLISI kernel variant (also where the plan says generic: the unaligned variant
+// and aligned strips of such a context ride the fused kernel).  A function attribute belongs to the device, not to a
+// context: set once per device and process (with that device current), not on every fitrig_create.
+static std::mutex g_attr_mu;
+static bool g_attr_done[64];
+
+static cudaError_t set_kernel_attributes_once(int device) {
+  std::lock_guard<std::mutex> lock(g_attr_mu);
+  if (device >= 0 && device < 64 && g_attr_done[device]) return cudaSuccess;
+  cudaError_t e;
+  if ((e = set_fused_attr<0>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr<1>()) != cudaSuccess) return e;
+  if ((e = set_fused_attr<2>()) != cudaSuccess) return e;
+#define MARCH_ATTR(R, S)                                                                                                    \
+  if ((e = cudaFuncSetAttribute(tlisi_march_kernel<R, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)) != \
+      cudaSuccess) return e;
+  MARCH_ATTR(0, false) MARCH_ATTR(1, false) MARCH_ATTR(2, false)
+  MARCH_ATTR(0, true) MARCH_ATTR(1, true) MARCH_ATTR(2, true)
+#undef MARCH_ATTR
+  if (device >= 0 && device < 64) g_attr_done[device] = true;
+  return cudaSuccess;
+}
+
 // A tLISI launch; with fp.dep != 0 as a programmatic dependent launch (the kernel places its own griddepcontrol.wait).
 template <typename P>
 static void launch_tlisi_kernel(void (*kernel)(const CUtensorMap, const P), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
@@ -387,13 +410,7 @@ extern "C" int fitrig_create(int32_t H, int32_t W, int32_t L, const fitrig_param
     CTX_TRY(cudaHostGetDevicePointer((void**)&d.counts_host_dev, d.counts_host, 0));
     CTX_TRY(cudaEventCreateWithFlags(&d.done, cudaEventDisableTiming));
   }
-  // (also where the plan says generic: the unaligned variant and aligned strips of such a context ride the fused kernel)
-  CTX_TRY((set_fused_attr<0>())); CTX_TRY((set_fused_attr<1>())); CTX_TRY((set_fused_attr<2>()));
-#define MARCH_ATTR(R, S) \
-  CTX_TRY((cudaFuncSetAttribute(tlisi_march_kernel<R, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmemPerCta)))
-  MARCH_ATTR(0, false); MARCH_ATTR(1, false); MARCH_ATTR(2, false);
-  MARCH_ATTR(0, true); MARCH_ATTR(1, true); MARCH_ATTR(2, true);
-#undef MARCH_ATTR
+  CTX_TRY(set_kernel_attributes_once(c->prm.device));
 #undef CTX_TRY
   *out = c;
   return FITRIG_OK;
@@ -1311,9 +1328,16 @@ extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int
     return fail(FITRIG_ERR_INVALID_ARG, "fitrig_probe_read_bandwidth: need a 16-byte aligned buffer of at least 16 bytes, reps >= 1");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   CUDA_TRY(cudaSetDevice(c->prm.device));
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
+  struct EventPair {  // destroyed on every return path
+    cudaEvent_t a = nullptr, b = nullptr;
+    ~EventPair() {
+      if (a) cudaEventDestroy(a);
+      if (b) cudaEventDestroy(b);
+    }
+  } ev;
+  CUDA_TRY(cudaEventCreate(&ev.a));
+  CUDA_TRY(cudaEventCreate(&ev.b));
+  const cudaEvent_t e0 = ev.a, e1 = ev.b;
   float best = 0.f;
   const long long n4 = bytes / 16;
   for (int r = 0; r < reps + 1; ++r) {  // the first pass warms up
@@ -1326,8 +1350,6 @@ extern "C" int fitrig_probe_read_bandwidth(fitrig_ctx* c, const void* d_buf, int
     CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
     if (r > 0 && ms > 0.f) best = std::max(best, (float)((double)n4 * 16.0 / (ms * 1e-3) / 1e9));
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   *gbs = best;
   return FITRIG_OK;
 }

@@ -76,6 +76,27 @@ def test_stream_separately_allocated_snapshots_fall_back_to_per_snapshot_copies(
 # ------------------------------------------------------------------------------------------
 # streams: a side stream, two contexts interleaved on two streams, all entry points chained on one context
 # ------------------------------------------------------------------------------------------
+def test_stream_from_pageable_host_memory_gives_the_pinned_result():
+    """fitrig.h: "pageable memory works, slowly" -- snapshots in ordinary (not page-locked) host memory, as one
+    allocation (pitched copies) and as separate numpy arrays, against the pinned run bit for bit; twice on one context."""
+    L, H, W, tile = 6, 300, 252, 32
+    st = synth.make_stack(synth.scaled(synth.CONFIGS["tiny"], H, W, L=L), device=DEV)[0]
+    pinned = gpu_run(st, taus=(3.0,), tile=tile, use_stream=True, strip_rows=64)
+    whole = st.cpu()  # pageable, one allocation
+    assert not whole.is_pinned()
+    separate = [np.array(st[s].cpu().numpy(), copy=True) for s in range(L)]  # pageable, one allocation per snapshot
+    with fitrig.Context(H, W, L, tile=tile, strip_rows=64) as ctx:
+        U, Ty, Tx = ctx.map_dims()
+        h_tl = np.empty((U, Ty, Tx), dtype=np.float32)  # a pageable output too
+        for hosts in ([whole[s] for s in range(L)], separate, [whole[s] for s in range(L)]):
+            h_tl.fill(-1.0)
+            ctx.stream(hosts, h_tl)
+            torch.cuda.synchronize()
+            c, n = ctx.detect(3.0)
+            assert np.array_equal(h_tl, pinned["tlisi_out"]) and np.array_equal(ctx.get_map(0), pinned["q"])
+            assert n == pinned["cands"][3.0][1] and np.array_equal(c, pinned["cands"][3.0][0])
+
+
 @pytest.mark.parametrize("H,W,tile", [(256, 256, 32), (250, 252, 16), (120, 100, 8), (96, 130, 5)])
 def test_side_stream_gives_the_default_stream_result(H, W, tile):
     st = synth.make_stack(synth.scaled(synth.CONFIGS["tiny"], H, W), device=DEV)[0]
