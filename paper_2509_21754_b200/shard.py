@@ -99,6 +99,22 @@ def merge_candidates(per_shard: Sequence[np.ndarray]) -> np.ndarray:
     return cat[np.argsort(cat["snapshot"], kind="stable")]
 
 
+def shard_host_rows(h_snapshots: Sequence, r0: int, r1: int) -> List:
+    """Rows [r0, r1) of every host snapshot ([H, W] torch tensors or numpy arrays), as views: what ONE rank streams of
+    an image that lives whole in (pinned) host memory.  Rows of a row-major image are contiguous, so each view is one
+    contiguous block that starts r0 * W elements into its snapshot -- index bookkeeping only, nothing is copied."""
+    out = []
+    for s in h_snapshots:
+        if s.ndim != 2 or not (0 <= r0 < r1 <= s.shape[0]):
+            raise ValueError(f"rows [{r0}, {r1}) of a snapshot of shape {tuple(s.shape)}")
+        v = s[r0:r1]
+        contiguous = v.is_contiguous() if hasattr(v, "is_contiguous") else v.flags["C_CONTIGUOUS"]
+        if not contiguous:
+            raise ValueError("host snapshots must be row-major and contiguous")
+        out.append(v)
+    return out
+
+
 class ShardedContext:
     """This rank's horizontal shard of ONE H x W image stack (image branch).
 
@@ -106,6 +122,11 @@ class ShardedContext:
         sc.tlisi(d_stack_rows)            # [L, r1 - r0, W] CUDA tensor: this rank's rows of every snapshot
         cands, n = sc.detect(tau)         # this shard's candidates, y in image rows
         everyone = sc.gather(cands)       # all candidates in (unit, tile row, tile col) order, on every rank
+
+    For an image that lives in host memory (BASELINE.json configs[3]; "sharding strips across G GPUs
+    multiplies host-to-device bandwidth"), `sc.stream(h_snapshots)` takes the WHOLE host snapshots and copies only this
+    rank's rows [r0, r1) of each through fitrig_stream: every rank moves H_shard * W * L * 4 bytes over its own PCIe
+    link, 1 / world of the image, and the exchange that follows is the same 2 + 2U doubles.
     """
 
     def __init__(self, H: int, W: int, n_snapshots: int, rank: int, world: int, group=None, **params):
@@ -117,6 +138,7 @@ class ShardedContext:
             raise ValueError(f"rank {rank} of {world} has no tile row of a {H}-row image (tile {tile})")
         self.ctx = Context(self.r1 - self.r0, W, n_snapshots, row_offset=self.r0, **params)
         self.units = self.ctx.units
+        self.device = int(params.get("device", 0))
         self._vec = None
 
     def _exchange(self, vec, stream):
@@ -137,11 +159,23 @@ class ShardedContext:
         return allv
 
     def tlisi(self, d_stack_rows, d_tlisi=None, stream=None) -> None:
+        self.ctx.tlisi(d_stack_rows, None, stream)
+        self._globalise(d_stack_rows.device, d_tlisi, stream)
+
+    def stream(self, h_snapshots: Sequence, d_tlisi=None, stream=None) -> None:
+        """h_snapshots: the L WHOLE host snapshots [H, W] (pinned for overlap), the same list on every rank; this rank
+        streams only its rows of each (`shard_host_rows`), then the shards exchange M and the statistics as in
+        `tlisi`.  d_tlisi (device, [U, Ty_shard, Tx]) receives this shard's tLISI under the global M."""
+        import torch
+        self.ctx.stream(shard_host_rows(h_snapshots, self.r0, self.r1), None, stream)
+        self._globalise(torch.device("cuda", self.device), d_tlisi, stream)
+
+    def _globalise(self, device, d_tlisi, stream) -> None:
+        """The exchange step: provisional shard map -> the map under the global M, mu, sigma (and eta's statistics)."""
         import torch
         if self._vec is None:
-            self._vec = torch.empty(2 + 2 * self.units, dtype=torch.float64, device=d_stack_rows.device)
-            self._vec_eta = torch.empty(3, dtype=torch.float64, device=d_stack_rows.device)
-        self.ctx.tlisi(d_stack_rows, None, stream)
+            self._vec = torch.empty(2 + 2 * self.units, dtype=torch.float64, device=device)
+            self._vec_eta = torch.empty(3, dtype=torch.float64, device=device)
         self.ctx.shard_export(self._vec, stream)
         allv = self._exchange(self._vec, stream)
         self.ctx.shard_import(allv, allv.shape[0], d_tlisi, stream)

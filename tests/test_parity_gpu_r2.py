@@ -477,6 +477,48 @@ def test_row_shards_frequency_branch_reproduce_the_whole_image(H, W, world):
     assert keep(merged) == keep(ref_c) and ref_n > 0
 
 
+@pytest.mark.parametrize("branch,H,W,tile,world", [(0, 250, 252, 32, 3), (1, 256, 256, 16, 2), (0, 96, 128, 1, 2)])
+def test_row_shards_streamed_from_whole_host_snapshots(branch, H, W, tile, world):
+    """ShardedContext.stream / shard_host_rows (SURVEY.md 8(e), config 4 over several GPUs): every shard copies only its
+    own rows of the whole pinned snapshots through fitrig_stream.  One GPU here, so the shards run one after another and
+    the all-gather is the stack of their export vectors; a world of one goes through ShardedContext.stream itself."""
+    from paper_2509_21754_b200 import shard
+    L, tau = (12, 2.0) if branch else (8, 3.0)
+    cfg = synth.scaled(synth.CONFIGS["imgfreq" if branch else "tiny"], H, W, L=L)
+    st = synth.make_stack(cfg, device=DEV)[0]
+    host = st.cpu().pin_memory()
+    snaps = [host[s] for s in range(L)]
+    whole = gpu_run(st, taus=(tau,), tile=tile, branch=branch, capacity=1 << 18)
+    with shard.ShardedContext(H, W, L, 0, 1, tile=tile, branch=branch) as sc:  # world = 1: no process group needed
+        U, Ty, Tx = sc.ctx.map_dims()
+        d_tl = torch.empty((U, Ty, Tx), dtype=torch.float32, device=DEV)
+        sc.stream(snaps, d_tl, torch.cuda.Stream(device=DEV))
+        torch.cuda.synchronize()
+        c1, n1 = sc.detect(tau, 1 << 18)
+        assert np.array_equal(sc.ctx.get_map(0), whole["q"]) and np.array_equal(d_tl.cpu().numpy(), whole["tlisi"])
+        assert n1 == whole["cands"][tau][1] or abs(n1 - whole["cands"][tau][1]) <= 2  # (z from sums of p: last bits)
+    rows = shard.row_shards(H, tile, world)
+    ctxs, vecs, qs = [], [], []
+    try:
+        for (r0, r1) in rows:
+            ctx = fitrig.Context(r1 - r0, W, L, row_offset=r0, tile=tile, branch=branch)
+            ctxs.append(ctx)
+            ctx.stream(shard.shard_host_rows(snaps, r0, r1))
+            v = torch.empty(2 + 2 * (L - 2), dtype=torch.float64, device=DEV)
+            ctx.shard_export(v)
+            vecs.append(v)
+        allv = torch.stack(vecs).contiguous()
+        for ctx in ctxs:
+            ctx.shard_import(allv, world)
+            qs.append(ctx.get_map(0))
+            assert ctx.get_stats()[0] == whole["M"]
+        assert sum(c.copy_count() for c in ctxs) > 0
+    finally:
+        for ctx in ctxs:
+            ctx.close()
+    assert np.array_equal(np.concatenate(qs, axis=1), whole["q"])
+
+
 def test_row_shards_of_a_constant_map_have_zero_sigma_and_no_candidates():
     """a one-pass variance of the shards' sums could turn sigma == 0 (R4) into a tiny positive number and
     spurious large z.  Every tile of this stack has the same raw sums, so q is constant over the image."""

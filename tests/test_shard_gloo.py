@@ -84,7 +84,13 @@ def _worker(rank, world, port, H, W, L, tile, tau, ret):
         st, _ = synth.make_stack(cfg, device="cpu")  # same seed on every rank: the same image
         full = [st[s].numpy() for s in range(L)]
         r0, r1 = shard.row_shards(H, tile, world)[rank]
-        rows = [np.ascontiguousarray(x[r0:r1]) for x in full]
+        # what ShardedContext.stream hands to fitrig_stream: this rank's rows of the WHOLE host snapshots, as views
+        # (one contiguous block per snapshot, r0 * W floats into it) -- no copy, and 1 / world of the bytes per rank
+        rows = shard.shard_host_rows(full, r0, r1)
+        assert all(v_.ctypes.data == x.ctypes.data + 4 * r0 * W and v_.flags["C_CONTIGUOUS"] and v_.shape == (r1 - r0, W)
+                   for v_, x in zip(rows, full))
+        nbytes = shard.all_gather_vectors(torch.tensor([sum(v_.nbytes for v_ in rows)], dtype=torch.int64)).reshape(-1)
+        assert int(nbytes.sum()) == 4 * L * H * W and int(nbytes[rank]) == 4 * L * (r1 - r0) * W
         v, res = _export_vector(rows, tile)
         allv = shard.all_gather_vectors(torch.from_numpy(v)).numpy()  # the ONE exchange
         assert allv.shape == (world, 2 + 2 * (L - 2)) and np.array_equal(allv[rank], v)
@@ -183,6 +189,28 @@ def test_split_range_and_row_shards():
     assert shard.row_shards(40, 32, 4) == [(0, 0), (0, 32), (32, 32), (32, 40)]  # more ranks than tile rows
     with pytest.raises(ValueError):
         shard.split_range(4, 2, 2)
+
+
+def test_shard_host_rows_are_views_that_tile_the_image():
+    H, W, L, tile = 200, 96, 3, 8
+    snaps = [np.arange(H * W, dtype=np.float32).reshape(H, W) + s for s in range(L)]
+    tsnaps = [torch.from_numpy(x) for x in snaps]
+    for world in (1, 2, 3, 7):
+        seen = np.zeros(H, dtype=np.int64)
+        for (r0, r1) in shard.row_shards(H, tile, world):
+            views = shard.shard_host_rows(snaps, r0, r1)
+            tviews = shard.shard_host_rows(tsnaps, r0, r1)
+            for x, v_, t_ in zip(snaps, views, tviews):
+                assert np.shares_memory(x, v_) and v_.ctypes.data == x.ctypes.data + 4 * r0 * W == t_.data_ptr()
+                assert np.array_equal(v_, x[r0:r1]) and r0 % tile == 0
+            seen[r0:r1] += 1
+        assert np.all(seen == 1)  # every image row is streamed by exactly one rank
+    with pytest.raises(ValueError):
+        shard.shard_host_rows(snaps, 10, 10)
+    with pytest.raises(ValueError):
+        shard.shard_host_rows(snaps, 0, H + 1)
+    with pytest.raises(ValueError):
+        shard.shard_host_rows([x.T for x in snaps], 0, 8)  # column-major: rows are not contiguous blocks
 
 
 def test_merge_candidates_orders_by_unit_then_shard():

@@ -48,6 +48,11 @@ def _worker(rank, world, port, H, W, L, tile, tau, branch, ret):
             q = sc.ctx.get_map(0)
             M, mu, sd = sc.ctx.get_stats()
             r0, r1 = sc.r0, sc.r1
+            # the same image from (pinned) host memory: every rank streams its own rows of the whole snapshots
+            host = full.cpu().pin_memory()
+            sc.stream([host[s] for s in range(L)], None, side)
+            cands_s, n_s = sc.detect(tau, 1 << 16, side)
+            assert n_s == n and np.array_equal(cands_s, cands) and np.array_equal(sc.ctx.get_map(0), q)
         with fitrig.Context(H, W, L, device=rank, tile=tile, branch=branch) as ctx:
             ctx.tlisi(full)
             ref_c, ref_n = ctx.detect(tau)
